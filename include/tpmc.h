@@ -1,0 +1,144 @@
+/*
+ * tpmc.h -- C ABI of libtpmc.so: the data-parallel hot path of the test-particle Monte Carlo
+ * (TPMC) free-molecular method of arXiv 1312.3691 (Parham & Barba, "Finding the Force"),
+ * hand-written CUDA for sm_100a (B200).
+ *
+ * Citations "P:<line>" are lines of the paper text; "O<n>/A<n>/G<n>" are the
+ * step definitions and readings listed in DESIGN.md (taken from SURVEY.md section 8(c)).
+ *
+ * Conventions (every entry point):
+ *   - returns TPMC_OK (0) or a negative TPMC_E* code; never aborts, never throws across the ABI;
+ *     tpmc_strerror() names a code, tpmc_last_cuda_error() gives the CUDA text after TPMC_ECUDA.
+ *   - "host"/"device" says where a pointer must live.  The library never frees caller buffers.
+ *   - work is enqueued on the caller's CUDA stream (cudaStream_t passed as void*, NULL = default
+ *     stream); device outputs are valid once the caller has synchronised that stream.
+ *   - one tpmc_run at a time per mesh handle (the handle caches per-run scratch).
+ *   - there is no CPU fallback: without a CUDA device every compute call returns TPMC_ECUDA.
+ */
+#ifndef TPMC_H
+#define TPMC_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TPMC_OK 0
+#define TPMC_EINVAL (-1) /* bad argument / degenerate mesh / bad parameter */
+#define TPMC_ENOMEM (-2) /* host or device allocation failed */
+#define TPMC_ECUDA (-3)  /* a CUDA call failed; see tpmc_last_cuda_error() */
+
+#define TPMC_MEM_HOST 0
+#define TPMC_MEM_DEVICE 1
+
+#define TPMC_MAX_SPECIES 8
+#define TPMC_FACET_TWO_SIDED 1u /* facet_flags bit0 */
+
+/* Opaque triangulated body + its on-device LBVH ("Satellite surfaces are represented by a
+ * triangulation, allowing the use of well-known ray-tracing methods").  Owns its device memory. */
+typedef struct tpmc_mesh tpmc_mesh;
+
+typedef struct {
+  double centre[3];        /* centre of the vertex AABB = centre of the control sphere (O1, A10) */
+  double bounding_radius;  /* R_b = max |vertex - centre| */
+  float aabb_lo[3], aabb_hi[3];
+  int64_t nt;              /* facets */
+  int64_t n_nodes;         /* LBVH internal nodes (max(nt-1,1)), 64 B each */
+  double build_ms;         /* device time of the LBVH build (Morton, sort, hierarchy, refit) */
+} tpmc_mesh_info_t;
+
+/* Gas, control volume and run selection (Table 1). */
+typedef struct {
+  double n;                /* number density, 1/m^3 */
+  double T_inf, T_W;       /* free-stream and wall temperature, K */
+  double V[3];             /* free-stream bulk velocity in the body frame, m/s (sweeps rotate V, not the mesh) */
+  double accommodation;    /* sigma in [0,1]: P(diffuse re-emission fully accommodated to T_W); else specular (A7) */
+  int32_t n_species;       /* 1..TPMC_MAX_SPECIES */
+  const double* m;         /* host [n_species] molecular mass, kg */
+  const double* x;         /* host [n_species] number fraction, sum 1 (species drawn per particle, A8) */
+  double cv_radius_factor; /* control-sphere radius / bounding radius (> 1; the configs use 1.5) */
+  uint64_t N;              /* particles of the whole stream; the particle weight is m Gamma / N */
+  uint64_t first, count;   /* run only particles [first, first+count) of that stream (slices, multi-GPU) */
+  uint64_t seed;           /* Philox4x32-10 key; counter = (particle index, block) (O3) */
+  uint32_t max_bounces;    /* cap on reflections per particle (>=1); cut-off particles are counted (A13) */
+  double x_ref[3];         /* torque reference point, body frame (A14) */
+} tpmc_params;
+
+typedef struct {
+  uint64_t hits;           /* surface interactions ("bounces") */
+  uint64_t segments;       /* closest-hit queries = count + hits */
+  uint64_t escaped;        /* particles that left without (further) hit */
+  uint64_t truncated;      /* particles stopped by max_bounces */
+  uint64_t culled;         /* particles whose first segment was answered by the mesh-AABB test in the seed kernel */
+  uint64_t tri_tests;      /* fp64 ray-triangle evaluations */
+  uint64_t node_visits;    /* 64-byte BVH nodes fetched */
+  uint64_t kernel_launches;/* kernels this run enqueued */
+  double ms;               /* device time of this run, CUDA events on the caller's stream */
+  double ms_seed;          /* summed device time of the seed-kernel launches (events around each launch) */
+  double ms_trace;         /* summed device time of the trace/reflect-kernel launches */
+  uint64_t timed_waves;    /* waves covered by ms_seed / ms_trace (all of them unless > 2048) */
+} tpmc_stats;
+
+/* Optional per-particle outputs for parity checks; each pointer is device [count] or NULL. */
+typedef struct {
+  uint64_t* hash;          /* FNV-1a 64 over the little-endian bytes of the hit facet ids, in order (O12) */
+  uint32_t* bounces;       /* number of surface interactions */
+  int32_t* first_facet;    /* first facet hit, or -1 */
+} tpmc_debug;
+
+/* Build a body: copies the triangulation to the device, computes centre / bounding radius (O1) and
+ * builds the LBVH there (63-bit Morton codes of centroids -> radix sort -> Karras hierarchy ->
+ * bottom-up AABB refit).  There is no host build path.
+ *   vertices   [nv][3] fp32, metres, body frame; indices [nt][3] int32, counter-clockwise seen from
+ *              outside for one-sided facets; facet_flags [nt] or NULL (bit0 = two-sided, A11);
+ *              all three live where mem_space says.  nt >= 1, nv >= 3, indices in range.
+ * Synchronises `stream` before returning.  *out is valid only on TPMC_OK. */
+int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t* indices, int64_t nt,
+                     const uint8_t* facet_flags, int mem_space, void* cuda_stream, tpmc_mesh** out);
+void tpmc_mesh_destroy(tpmc_mesh* mesh);
+int tpmc_mesh_info(const tpmc_mesh* mesh, tpmc_mesh_info_t* out /* host */);
+
+/* Copy the built hierarchy to the host for inspection: nodes [n_nodes][16] floats
+ * (lo0.xyz hi0.xyz lo1.xyz hi1.xyz, then child0, child1 as int32 bit patterns, 2 pad words;
+ * child >= 0: internal node, child < 0: leaf holding sorted triangle ~child),
+ * leaf_facet [nt] = facet id stored in each sorted triangle slot.  Either pointer may be NULL. */
+int tpmc_mesh_copy_bvh(const tpmc_mesh* mesh, float* h_nodes, int32_t* h_leaf_facet);
+
+/* The hot path: seed particles [first, first+count) on the spherical control
+ * volume from the drifting-Maxwellian number flux (eq. 10, 11, 14a-c, 15), trace each against the
+ * body (closest hit), apply the surface interaction, follow reflections until
+ * escape, and accumulate momentum transfer and torque.
+ *   d_force [3], d_torque [3]   device, overwritten: force (N) and torque about x_ref (N m) of this slice
+ *   d_facet_momentum [nt][3]    device or NULL, overwritten: momentum-transfer rate per facet (N)
+ *   h_stats                     host or NULL; if given the call synchronises the stream and fills it
+ *   debug                       host struct of device pointers, or NULL
+ * Slices are additive: summing the outputs of disjoint [first,count) slices of one N gives the full run. */
+int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* cuda_stream, double* d_force,
+             double* d_torque, double* d_facet_momentum, tpmc_stats* h_stats, const tpmc_debug* debug);
+
+/* Same run with HOST result buffers (h_facet_momentum may be NULL): device results are copied back
+ * inside the call and the stream is synchronised before returning. */
+int tpmc_run_host(const tpmc_mesh* mesh, const tpmc_params* params, void* cuda_stream, double* h_force,
+                  double* h_torque, double* h_facet_momentum, tpmc_stats* h_stats);
+
+/* Seeding step alone (O3-O8), for parity checks: fp64 position and velocity of particles
+ * [first, first+count) BEFORE the fp32 rounding of O9.  d_x, d_v device [count][3]; d_species device
+ * [count] or NULL.  Runs the same device code as tpmc_run's seed kernel. */
+int tpmc_seed(const tpmc_mesh* mesh, const tpmc_params* params, void* cuda_stream, double* d_x, double* d_v,
+              int32_t* d_species);
+
+/* Closest-hit step alone (O10), for parity checks: rays o + tau d with fp32 origin/direction,
+ * d_o, d_d device [n][3]; d_f_prev device [n] (facet to exclude, -1 for none) or NULL;
+ * outputs d_facet [n] (-1 = no hit) and d_tau [n] (fp64, +inf when no hit). */
+int tpmc_trace(const tpmc_mesh* mesh, const float* d_o, const float* d_d, const int32_t* d_f_prev, int64_t n,
+               void* cuda_stream, int32_t* d_facet, double* d_tau);
+
+const char* tpmc_strerror(int code);
+const char* tpmc_last_cuda_error(void);
+const char* tpmc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TPMC_H */

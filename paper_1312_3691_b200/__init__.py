@@ -1,0 +1,303 @@
+"""Thin Python binding of libtpmc.so (include/tpmc.h): argument marshalling only.
+
+Every step of the hot path (seed, LBVH build, trace, reflect, accumulate, reduce) runs in the
+hand-written CUDA kernels of csrc/; PyTorch is used here for device buffers and streams.
+There is no CPU fallback and this package never imports ``oracle``: if the library is missing
+or no CUDA device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtpmc.so")
+
+TPMC_OK, TPMC_EINVAL, TPMC_ENOMEM, TPMC_ECUDA = 0, -1, -2, -3
+TPMC_MEM_HOST, TPMC_MEM_DEVICE = 0, 1
+TPMC_MAX_SPECIES = 8
+
+EXPORTS = ["tpmc_mesh_create", "tpmc_mesh_destroy", "tpmc_mesh_info", "tpmc_mesh_copy_bvh", "tpmc_run",
+           "tpmc_run_host", "tpmc_seed", "tpmc_trace", "tpmc_strerror", "tpmc_last_cuda_error", "tpmc_version"]
+
+
+class TpmcError(RuntimeError):
+    pass
+
+
+class tpmc_mesh_info_t(C.Structure):
+    _fields_ = [("centre", C.c_double * 3), ("bounding_radius", C.c_double), ("aabb_lo", C.c_float * 3),
+                ("aabb_hi", C.c_float * 3), ("nt", C.c_int64), ("n_nodes", C.c_int64), ("build_ms", C.c_double)]
+
+
+class tpmc_params(C.Structure):
+    _fields_ = [("n", C.c_double), ("T_inf", C.c_double), ("T_W", C.c_double), ("V", C.c_double * 3),
+                ("accommodation", C.c_double), ("n_species", C.c_int32),
+                ("m", C.POINTER(C.c_double)), ("x", C.POINTER(C.c_double)),
+                ("cv_radius_factor", C.c_double), ("N", C.c_uint64), ("first", C.c_uint64),
+                ("count", C.c_uint64), ("seed", C.c_uint64), ("max_bounces", C.c_uint32),
+                ("x_ref", C.c_double * 3)]
+
+
+class tpmc_stats(C.Structure):
+    _fields_ = [("hits", C.c_uint64), ("segments", C.c_uint64), ("escaped", C.c_uint64), ("truncated", C.c_uint64),
+                ("culled", C.c_uint64), ("tri_tests", C.c_uint64), ("node_visits", C.c_uint64),
+                ("kernel_launches", C.c_uint64), ("ms", C.c_double), ("ms_seed", C.c_double), ("ms_trace", C.c_double),
+                ("timed_waves", C.c_uint64)]
+
+
+class tpmc_debug(C.Structure):
+    _fields_ = [("hash", C.c_void_p), ("bounces", C.c_void_p), ("first_facet", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib():
+    """Load libtpmc.so (built in-tree by build.py).  Raises if it is missing: no fallback."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise TpmcError(f"{LIB_PATH} not found: run `python -m paper_1312_3691_b200.build` "
+                            "(or __graft_entry__.build()); there is no CPU fallback")
+        L = C.CDLL(LIB_PATH)
+        vp = C.c_void_p
+        L.tpmc_mesh_create.restype = C.c_int
+        L.tpmc_mesh_create.argtypes = [vp, C.c_int64, vp, C.c_int64, vp, C.c_int, vp, C.POINTER(vp)]
+        L.tpmc_mesh_destroy.restype = None
+        L.tpmc_mesh_destroy.argtypes = [vp]
+        L.tpmc_mesh_info.restype = C.c_int
+        L.tpmc_mesh_info.argtypes = [vp, C.POINTER(tpmc_mesh_info_t)]
+        L.tpmc_mesh_copy_bvh.restype = C.c_int
+        L.tpmc_mesh_copy_bvh.argtypes = [vp, vp, vp]
+        L.tpmc_run.restype = C.c_int
+        L.tpmc_run.argtypes = [vp, C.POINTER(tpmc_params), vp, vp, vp, vp, C.POINTER(tpmc_stats), C.POINTER(tpmc_debug)]
+        L.tpmc_run_host.restype = C.c_int
+        L.tpmc_run_host.argtypes = [vp, C.POINTER(tpmc_params), vp, vp, vp, vp, C.POINTER(tpmc_stats)]
+        L.tpmc_seed.restype = C.c_int
+        L.tpmc_seed.argtypes = [vp, C.POINTER(tpmc_params), vp, vp, vp, vp]
+        L.tpmc_trace.restype = C.c_int
+        L.tpmc_trace.argtypes = [vp, vp, vp, vp, C.c_int64, vp, vp, vp]
+        for n in ("tpmc_strerror", "tpmc_last_cuda_error", "tpmc_version"):
+            getattr(L, n).restype = C.c_char_p
+        L.tpmc_strerror.argtypes = [C.c_int]
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, what: str):
+    if rc != TPMC_OK:
+        L = lib()
+        msg = L.tpmc_strerror(rc).decode()
+        if rc == TPMC_ECUDA:
+            msg += ": " + L.tpmc_last_cuda_error().decode()
+        raise TpmcError(f"{what} failed ({rc}): {msg}")
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise TpmcError("no CUDA device: the TPMC hot path has no CPU fallback")
+    return torch
+
+
+def _stream_ptr(stream) -> Optional[int]:
+    if stream is None:
+        return _torch().cuda.current_stream().cuda_stream or None
+    return getattr(stream, "cuda_stream", stream) or None
+
+
+def make_params(cfg, first=None, count=None, N=None):
+    """Marshal a parameter record (anything with the tpmc_params field names, e.g.
+    tpmc_inputs.RunConfig) into a C struct.  Returns (struct, keepalive)."""
+    p = tpmc_params()
+    p.n, p.T_inf, p.T_W = float(cfg.n), float(cfg.T_inf), float(cfg.T_W)
+    p.V = (C.c_double * 3)(*[float(a) for a in cfg.V])
+    p.accommodation = float(cfg.accommodation)
+    m = np.ascontiguousarray(cfg.m, dtype=np.float64)
+    x = np.ascontiguousarray(cfg.x, dtype=np.float64)
+    p.n_species = int(m.size)
+    p.m = m.ctypes.data_as(C.POINTER(C.c_double))
+    p.x = x.ctypes.data_as(C.POINTER(C.c_double))
+    p.cv_radius_factor = float(cfg.cv_radius_factor)
+    p.N = int(cfg.N if N is None else N)
+    p.first = int(0 if first is None else first)
+    p.count = int(p.N - p.first if count is None else count)
+    p.seed = int(cfg.seed)
+    p.max_bounces = int(cfg.max_bounces)
+    p.x_ref = (C.c_double * 3)(*[float(a) for a in cfg.x_ref])
+    return p, (m, x)
+
+
+@dataclass
+class RunResult:
+    force: "object"                 # torch [3] float64, device
+    torque: "object"                # torch [3] float64, device
+    facet_momentum: "object"        # torch [nt,3] float64 device, or None
+    stats: Optional[dict]
+    hash: "object" = None           # torch [count] int64 (bit pattern of the u64 hash), device
+    bounces: "object" = None        # torch [count] int32
+    first_facet: "object" = None    # torch [count] int32
+
+
+class Mesh:
+    """Owns a tpmc_mesh handle (triangulation + on-device LBVH)."""
+
+    def __init__(self, vertices, indices, flags=None, stream=None):
+        L = lib()
+        torch = _torch()
+        self._h = C.c_void_p()
+        if isinstance(vertices, np.ndarray) or not hasattr(vertices, "is_cuda"):
+            v = np.ascontiguousarray(vertices, dtype=np.float32)
+            i = np.ascontiguousarray(indices, dtype=np.int32)
+            f = None if flags is None else np.ascontiguousarray(flags, dtype=np.uint8)
+            nv, nt = v.shape[0], i.shape[0]
+            rc = L.tpmc_mesh_create(v.ctypes.data, nv, i.ctypes.data, nt, None if f is None else f.ctypes.data,
+                                    TPMC_MEM_HOST, _stream_ptr(stream), C.byref(self._h))
+        else:
+            v = vertices.to(dtype=torch.float32).contiguous()
+            i = indices.to(dtype=torch.int32).contiguous()
+            f = None if flags is None else flags.to(dtype=torch.uint8).contiguous()
+            if not (v.is_cuda and i.is_cuda and (f is None or f.is_cuda)):
+                raise TpmcError("device meshes need CUDA tensors")
+            nv, nt = v.shape[0], i.shape[0]
+            rc = L.tpmc_mesh_create(v.data_ptr(), nv, i.data_ptr(), nt, None if f is None else f.data_ptr(),
+                                    TPMC_MEM_DEVICE, _stream_ptr(stream), C.byref(self._h))
+        _check(rc, "tpmc_mesh_create")
+        self.nt = int(nt)
+        self.nv = int(nv)
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            lib().tpmc_mesh_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def info(self) -> dict:
+        out = tpmc_mesh_info_t()
+        _check(lib().tpmc_mesh_info(self._h, C.byref(out)), "tpmc_mesh_info")
+        return {"centre": np.array(list(out.centre)), "bounding_radius": out.bounding_radius,
+                "aabb_lo": np.array(list(out.aabb_lo)), "aabb_hi": np.array(list(out.aabb_hi)),
+                "nt": int(out.nt), "n_nodes": int(out.n_nodes), "build_ms": out.build_ms}
+
+    def copy_bvh(self):
+        n_nodes = self.info()["n_nodes"]
+        nodes = np.zeros((n_nodes, 16), dtype=np.float32)
+        leaf = np.zeros(self.nt, dtype=np.int32)
+        _check(lib().tpmc_mesh_copy_bvh(self._h, nodes.ctypes.data, leaf.ctypes.data), "tpmc_mesh_copy_bvh")
+        return nodes, leaf
+
+    # ------------------------------------------------------------------ the hot path
+    def run(self, cfg, first=None, count=None, N=None, facets=True, debug=False, stats=True, stream=None) -> RunResult:
+        torch = _torch()
+        p, keep = make_params(cfg, first, count, N)
+        dev = torch.device("cuda", torch.cuda.current_device())
+        force = torch.empty(3, dtype=torch.float64, device=dev)
+        torque = torch.empty(3, dtype=torch.float64, device=dev)
+        fm = torch.empty((self.nt, 3), dtype=torch.float64, device=dev) if facets else None
+        dbg, hs, nb, ff = None, None, None, None
+        if debug:
+            cnt = int(p.count)
+            hs = torch.empty(cnt, dtype=torch.int64, device=dev)
+            nb = torch.empty(cnt, dtype=torch.int32, device=dev)
+            ff = torch.empty(cnt, dtype=torch.int32, device=dev)
+            dbg = tpmc_debug(hs.data_ptr() or None, nb.data_ptr() or None, ff.data_ptr() or None)
+        st = tpmc_stats() if stats else None
+        rc = lib().tpmc_run(self._h, C.byref(p), _stream_ptr(stream), force.data_ptr(), torque.data_ptr(),
+                            None if fm is None else fm.data_ptr(), None if st is None else C.byref(st),
+                            None if dbg is None else C.byref(dbg))
+        _check(rc, "tpmc_run")
+        sd = None if st is None else {k: getattr(st, k) for k, _ in tpmc_stats._fields_}
+        return RunResult(force, torque, fm, sd, hs, nb, ff)
+
+    def run_host(self, cfg, first=None, count=None, N=None, facets=True, stats=True, stream=None,
+                 out_facets: Optional[np.ndarray] = None):
+        """tpmc_run_host: results land in HOST numpy buffers (D2H copies inside the call)."""
+        _torch()
+        p, keep = make_params(cfg, first, count, N)
+        force = np.empty(3, dtype=np.float64)
+        torque = np.empty(3, dtype=np.float64)
+        fm = None
+        if facets:
+            fm = out_facets if out_facets is not None else np.empty((self.nt, 3), dtype=np.float64)
+        st = tpmc_stats() if stats else None
+        rc = lib().tpmc_run_host(self._h, C.byref(p), _stream_ptr(stream), force.ctypes.data, torque.ctypes.data,
+                                 None if fm is None else fm.ctypes.data, None if st is None else C.byref(st))
+        _check(rc, "tpmc_run_host")
+        sd = None if st is None else {k: getattr(st, k) for k, _ in tpmc_stats._fields_}
+        return force, torque, fm, sd
+
+    def seed(self, cfg, first=None, count=None, N=None, stream=None):
+        """fp64 (x, v, species) of particles [first, first+count) before the fp32 rounding (tpmc_seed)."""
+        torch = _torch()
+        p, keep = make_params(cfg, first, count, N)
+        dev = torch.device("cuda", torch.cuda.current_device())
+        cnt = int(p.count)
+        x = torch.empty((cnt, 3), dtype=torch.float64, device=dev)
+        v = torch.empty((cnt, 3), dtype=torch.float64, device=dev)
+        s = torch.empty(cnt, dtype=torch.int32, device=dev)
+        _check(lib().tpmc_seed(self._h, C.byref(p), _stream_ptr(stream), x.data_ptr() or None, v.data_ptr() or None,
+                               s.data_ptr() or None), "tpmc_seed")
+        return x, v, s
+
+    def trace(self, o, d, f_prev=None, stream=None):
+        """Closest hit of rays o + tau d (tpmc_trace).  o, d: [n,3] float32 (numpy or CUDA tensors)."""
+        torch = _torch()
+        dev = torch.device("cuda", torch.cuda.current_device())
+        o = torch.as_tensor(np.ascontiguousarray(o, dtype=np.float32) if isinstance(o, np.ndarray) else o).to(dev, torch.float32).contiguous()
+        d = torch.as_tensor(np.ascontiguousarray(d, dtype=np.float32) if isinstance(d, np.ndarray) else d).to(dev, torch.float32).contiguous()
+        n = int(o.shape[0])
+        fp = None
+        if f_prev is not None:
+            fp = torch.as_tensor(f_prev).to(dev, torch.int32).contiguous()
+        facet = torch.empty(n, dtype=torch.int32, device=dev)
+        tau = torch.empty(n, dtype=torch.float64, device=dev)
+        _check(lib().tpmc_trace(self._h, o.data_ptr() or None, d.data_ptr() or None, None if fp is None else fp.data_ptr(),
+                                n, _stream_ptr(stream), facet.data_ptr() or None, tau.data_ptr() or None), "tpmc_trace")
+        return facet, tau
+
+
+# C-ABI names, as plain functions -------------------------------------------------------------------
+def tpmc_mesh_create(vertices, indices, flags=None, stream=None) -> Mesh:
+    return Mesh(vertices, indices, flags, stream)
+
+
+def tpmc_mesh_destroy(mesh: Mesh) -> None:
+    mesh.close()
+
+
+def tpmc_mesh_info(mesh: Mesh) -> dict:
+    return mesh.info()
+
+
+def tpmc_mesh_copy_bvh(mesh: Mesh):
+    return mesh.copy_bvh()
+
+
+def tpmc_run(mesh: Mesh, cfg, **kw) -> RunResult:
+    return mesh.run(cfg, **kw)
+
+
+def tpmc_run_host(mesh: Mesh, cfg, **kw):
+    return mesh.run_host(cfg, **kw)
+
+
+def tpmc_seed(mesh: Mesh, cfg, **kw):
+    return mesh.seed(cfg, **kw)
+
+
+def tpmc_trace(mesh: Mesh, o, d, f_prev=None, **kw):
+    return mesh.trace(o, d, f_prev, **kw)
+
+
+def tpmc_version() -> str:
+    return lib().tpmc_version().decode()

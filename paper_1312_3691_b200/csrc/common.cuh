@@ -1,0 +1,115 @@
+// common.cuh -- shared declarations of libtpmc (CUDA path only; nothing here is used by oracle/).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/tpmc.h"
+
+#define TPMC_SQRTPI 1.7724538509055160272981674833411
+#define TPMC_KB 1.380649e-23  // J/K
+
+extern thread_local char g_tpmc_cuda_error[512];
+
+#define TPMC_CUDA_TRY(expr)                                                                        \
+  do {                                                                                             \
+    cudaError_t _e = (expr);                                                                       \
+    if (_e != cudaSuccess) {                                                                       \
+      snprintf(g_tpmc_cuda_error, sizeof(g_tpmc_cuda_error), "%s:%d: %s: %s", __FILE__, __LINE__,  \
+               #expr, cudaGetErrorString(_e));                                                     \
+      cudaGetLastError();                                                                          \
+      return (_e == cudaErrorMemoryAllocation) ? TPMC_ENOMEM : TPMC_ECUDA;                         \
+    }                                                                                              \
+  } while (0)
+
+// ---------------------------------------------------------------------------------------------
+// Device-resident body.  nodes: 4 float4 per internal node (two child boxes + two child refs);
+// tris: 3 float4 per triangle in Morton order: (p0, facet id), (p1, flags), (p2, 0).
+struct tpmc_mesh {
+  int64_t nv, nt;
+  int64_t n_nodes;
+  float4* nodes;
+  float4* tris;
+  double centre[3];
+  double Rb;
+  float aabb_lo[3], aabb_hi[3];
+  double build_ms;
+  int device;
+  // per-run scratch, cached in the handle (one run at a time per handle)
+  size_t wave_cap;
+  float4* ray_o;
+  float4* ray_v;
+  unsigned int* queue_count;       // [4] device counters
+  double* facet_scratch;           // [nt][3] when the caller passes no per-facet buffer
+  double* partials;                // reduction partials
+  unsigned long long* stats;       // [8] device counters
+  double* totals;                  // [3] torque accumulators
+  cudaEvent_t ev0, ev1;
+  cudaEvent_t* wave_ev;            // [2*kMaxTimedWaves+1] per-kernel timing, created on first use
+  unsigned long long last_launches;
+  unsigned long long last_timed_waves;
+};
+
+constexpr int kMaxTimedWaves = 2048;
+
+// Per-run constants (a1: host, fp64), passed to kernels by value.
+struct SpeciesConst {
+  double c;      // c_mp = sqrt(2 k_B T_inf / m)
+  double S;      // speed ratio |V| / c_mp
+  double cW;     // sqrt(2 k_B T_W / m)
+  double w;      // particle weight m Gamma / N  [kg/s]     (eq. 10)
+  double g0;     // Gt(-S)                                  (position CDF constants, O5)
+  double gI;     // Gt(S) - Gt(-S)
+  double cumx;   // cumulative number fraction
+};
+
+struct RunConst {
+  SpeciesConst sp[TPMC_MAX_SPECIES];
+  int n_species;
+  double R[9];          // stream frame -> body frame, eq. (15)
+  double centre[3];
+  double r;             // control-sphere radius
+  double sigma;
+  double x_ref[3];
+  float aabb_lo[3], aabb_hi[3];
+  unsigned long long first, count;
+  unsigned int seed_lo, seed_hi;
+  unsigned int max_bounces;
+};
+
+#define TPMC_HD __host__ __device__ __forceinline__
+
+// ---------------------------------------------------------------------------------------------
+// Philox4x32-10 (Salmon et al. 2011), counter-based, keyed by particle index (O3).
+TPMC_HD uint32_t mulhi32(uint32_t a, uint32_t b) {
+#ifdef __CUDA_ARCH__
+  return __umulhi(a, b);
+#else
+  return (uint32_t)(((uint64_t)a * (uint64_t)b) >> 32);
+#endif
+}
+
+TPMC_HD uint4 philox4x32_10(uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t hi0 = mulhi32(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    const uint32_t hi1 = mulhi32(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    c0 = hi1 ^ c1 ^ k0;
+    c1 = lo1;
+    c2 = hi0 ^ c3 ^ k1;
+    c3 = lo0;
+    k0 += 0x9E3779B9u;
+    k1 += 0xBB67AE85u;
+  }
+  return make_uint4(c0, c1, c2, c3);
+}
+
+// word -> uniform in (0,1): (w + 1/2) 2^-32, exact in fp64 (A16)
+TPMC_HD double u01(uint32_t w) { return ((double)w + 0.5) * (1.0 / 4294967296.0); }
+
+TPMC_HD uint4 particle_block(const RunConst& rc, unsigned long long i, uint32_t block) {
+  return philox4x32_10(rc.seed_lo, rc.seed_hi, (uint32_t)i, (uint32_t)(i >> 32), block, 0u);
+}

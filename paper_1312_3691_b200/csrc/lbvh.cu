@@ -1,0 +1,361 @@
+// lbvh.cu -- tpmc_mesh_*: triangulation ingest and on-device LBVH build (step a0 of DESIGN.md).
+//
+// "Satellite surfaces are represented by a triangulation, allowing the use of well-known
+// ray-tracing methods"; the paper names no acceleration structure.  Here: 63-bit Morton
+// codes of facet centroids -> radix sort -> Karras (2012) binary radix tree -> bottom-up refit.
+// Everything runs on the device; there is no host build path.
+#include <cub/device/device_radix_sort.cuh>
+
+#include "common.cuh"
+
+thread_local char g_tpmc_cuda_error[512] = "";
+
+namespace {
+
+constexpr int kBlock = 256;
+
+// ---- vertex AABB (fp32 min/max are exact) and bounding radius about its centre (O1, A10) ----
+__global__ void k_vertex_aabb(const float* __restrict__ v, int64_t nv, float* __restrict__ out) {
+  __shared__ float s[6][1024];
+  float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+  for (int64_t i = threadIdx.x; i < nv; i += blockDim.x)
+    for (int a = 0; a < 3; ++a) {
+      const float p = v[3 * i + a];
+      lo[a] = fminf(lo[a], p);
+      hi[a] = fmaxf(hi[a], p);
+    }
+  for (int a = 0; a < 3; ++a) { s[a][threadIdx.x] = lo[a]; s[3 + a][threadIdx.x] = hi[a]; }
+  __syncthreads();
+  for (int st = blockDim.x / 2; st > 0; st >>= 1) {
+    if ((int)threadIdx.x < st)
+      for (int a = 0; a < 3; ++a) {
+        s[a][threadIdx.x] = fminf(s[a][threadIdx.x], s[a][threadIdx.x + st]);
+        s[3 + a][threadIdx.x] = fmaxf(s[3 + a][threadIdx.x], s[3 + a][threadIdx.x + st]);
+      }
+    __syncthreads();
+  }
+  if (threadIdx.x < 6) out[threadIdx.x] = s[threadIdx.x][0];
+}
+
+__global__ void k_vertex_r2(const float* __restrict__ v, int64_t nv, double cx, double cy, double cz,
+                            double* __restrict__ out) {
+  __shared__ double s[1024];
+  double r2 = 0.0;
+  for (int64_t i = threadIdx.x; i < nv; i += blockDim.x) {
+    const double dx = __dsub_rn((double)v[3 * i], cx), dy = __dsub_rn((double)v[3 * i + 1], cy),
+                 dz = __dsub_rn((double)v[3 * i + 2], cz);
+    // (dx*dx + dy*dy) + dz*dz without contraction: the bounding radius is a definition (O1)
+    const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+    r2 = fmax(r2, d2);
+  }
+  s[threadIdx.x] = r2;
+  __syncthreads();
+  for (int st = blockDim.x / 2; st > 0; st >>= 1) {
+    if ((int)threadIdx.x < st) s[threadIdx.x] = fmax(s[threadIdx.x], s[threadIdx.x + st]);
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) out[0] = s[0];
+}
+
+__global__ void k_check_indices(const int32_t* __restrict__ idx, int64_t n3, int64_t nv, int* __restrict__ bad) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i < n3 && (idx[i] < 0 || idx[i] >= nv)) atomicExch(bad, 1);
+}
+
+// ---- Morton codes ----
+__device__ __forceinline__ uint64_t spread21(uint64_t x) {  // 21 bits -> every third bit
+  x &= 0x1FFFFFull;
+  x = (x | (x << 32)) & 0x1F00000000FFFFull;
+  x = (x | (x << 16)) & 0x1F0000FF0000FFull;
+  x = (x | (x << 8)) & 0x100F00F00F00F00Full;
+  x = (x | (x << 4)) & 0x10C30C30C30C30C3ull;
+  x = (x | (x << 2)) & 0x1249249249249249ull;
+  return x;
+}
+
+__global__ void k_morton(const float* __restrict__ v, const int32_t* __restrict__ idx, int64_t nt, float3 lo,
+                         float3 inv_ext, uint64_t* __restrict__ keys, int32_t* __restrict__ ids) {
+  const int64_t f = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (f >= nt) return;
+  const int32_t i0 = idx[3 * f], i1 = idx[3 * f + 1], i2 = idx[3 * f + 2];
+  const float cx = (v[3 * i0] + v[3 * i1] + v[3 * i2]) * (1.0f / 3.0f);
+  const float cy = (v[3 * i0 + 1] + v[3 * i1 + 1] + v[3 * i2 + 1]) * (1.0f / 3.0f);
+  const float cz = (v[3 * i0 + 2] + v[3 * i1 + 2] + v[3 * i2 + 2]) * (1.0f / 3.0f);
+  const float s = 2097152.0f;  // 2^21
+  const uint64_t qx = (uint64_t)fminf(fmaxf((cx - lo.x) * inv_ext.x * s, 0.0f), s - 1.0f);
+  const uint64_t qy = (uint64_t)fminf(fmaxf((cy - lo.y) * inv_ext.y * s, 0.0f), s - 1.0f);
+  const uint64_t qz = (uint64_t)fminf(fmaxf((cz - lo.z) * inv_ext.z * s, 0.0f), s - 1.0f);
+  keys[f] = (spread21(qx) << 2) | (spread21(qy) << 1) | spread21(qz);
+  ids[f] = (int32_t)f;
+}
+
+// ---- sorted triangle records + leaf boxes ----
+__global__ void k_gather(const float* __restrict__ v, const int32_t* __restrict__ idx,
+                         const uint8_t* __restrict__ flags, const int32_t* __restrict__ sorted_ids, int64_t nt,
+                         float4* __restrict__ tris, float* __restrict__ box /* [(n_int + nt)][6] */, int64_t n_int) {
+  const int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (s >= nt) return;
+  const int32_t f = sorted_ids[s];
+  float p[3][3];
+  for (int k = 0; k < 3; ++k) {
+    const int32_t vi = idx[3 * (int64_t)f + k];
+    for (int a = 0; a < 3; ++a) p[k][a] = v[3 * (int64_t)vi + a];
+  }
+  const uint32_t fl = flags ? (uint32_t)flags[f] : 0u;
+  tris[3 * s + 0] = make_float4(p[0][0], p[0][1], p[0][2], __int_as_float(f));
+  tris[3 * s + 1] = make_float4(p[1][0], p[1][1], p[1][2], __uint_as_float(fl));
+  tris[3 * s + 2] = make_float4(p[2][0], p[2][1], p[2][2], 0.0f);
+  float* b = box + 6 * (n_int + s);
+  for (int a = 0; a < 3; ++a) {
+    b[a] = fminf(p[0][a], fminf(p[1][a], p[2][a]));      // exact: corners are fp32
+    b[3 + a] = fmaxf(p[0][a], fmaxf(p[1][a], p[2][a]));
+  }
+}
+
+// ---- Karras 2012: one thread per internal node ----
+__device__ __forceinline__ int delta(const uint64_t* __restrict__ k, int n, int i, int j) {
+  if (j < 0 || j >= n) return -1;
+  const uint64_t a = k[i], b = k[j];
+  if (a == b) return 64 + __clz(i ^ j);   // duplicate codes: fall back to the position
+  return __clzll((long long)(a ^ b));
+}
+
+__global__ void k_hierarchy(const uint64_t* __restrict__ keys, int n, int2* __restrict__ children,
+                            int* __restrict__ parent /* [n-1 internal | n leaves] */) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n - 1) return;
+  const int d = (delta(keys, n, i, i + 1) - delta(keys, n, i, i - 1)) >= 0 ? 1 : -1;
+  const int dmin = delta(keys, n, i, i - d);
+  int lmax = 2;
+  while (delta(keys, n, i, i + lmax * d) > dmin) lmax <<= 1;
+  int l = 0;
+  for (int t = lmax >> 1; t >= 1; t >>= 1)
+    if (delta(keys, n, i, i + (l + t) * d) > dmin) l += t;
+  const int j = i + l * d;
+  const int dnode = delta(keys, n, i, j);
+  int s = 0, t = l;
+  do {
+    t = (t + 1) >> 1;
+    if (delta(keys, n, i, i + (s + t) * d) > dnode) s += t;
+  } while (t > 1);
+  const int gamma = i + s * d + min(d, 0);
+  const int lo = min(i, j), hi = max(i, j);
+  const int left = (lo == gamma) ? ~gamma : gamma;              // ~x = leaf holding sorted triangle x
+  const int right = (hi == gamma + 1) ? ~(gamma + 1) : gamma + 1;
+  children[i] = make_int2(left, right);
+  parent[left >= 0 ? left : (n - 1) + ~left] = i;
+  parent[right >= 0 ? right : (n - 1) + ~right] = i;
+  if (i == 0) parent[0] = -1;
+}
+
+// ---- bottom-up refit: the second thread to arrive at a node owns it ----
+__global__ void k_refit(int n, const int2* __restrict__ children, const int* __restrict__ parent,
+                        float* __restrict__ box, int* __restrict__ arrive, float4* __restrict__ nodes) {
+  const int leaf = blockIdx.x * blockDim.x + threadIdx.x;
+  if (leaf >= n) return;
+  int cur = parent[(n - 1) + leaf];
+  while (cur >= 0) {
+    __threadfence();
+    if (atomicAdd(&arrive[cur], 1) == 0) return;
+    const int2 ch = children[cur];
+    const volatile float* b0 = box + 6 * (size_t)(ch.x >= 0 ? ch.x : (n - 1) + ~ch.x);
+    const volatile float* b1 = box + 6 * (size_t)(ch.y >= 0 ? ch.y : (n - 1) + ~ch.y);
+    float l0[3], h0[3], l1[3], h1[3];
+    for (int a = 0; a < 3; ++a) { l0[a] = b0[a]; h0[a] = b0[3 + a]; l1[a] = b1[a]; h1[a] = b1[3 + a]; }
+    float* b = box + 6 * (size_t)cur;
+    for (int a = 0; a < 3; ++a) { b[a] = fminf(l0[a], l1[a]); b[3 + a] = fmaxf(h0[a], h1[a]); }
+    nodes[4 * (size_t)cur + 0] = make_float4(l0[0], l0[1], l0[2], h0[0]);
+    nodes[4 * (size_t)cur + 1] = make_float4(h0[1], h0[2], l1[0], l1[1]);
+    nodes[4 * (size_t)cur + 2] = make_float4(l1[2], h1[0], h1[1], h1[2]);
+    nodes[4 * (size_t)cur + 3] = make_float4(__int_as_float(ch.x), __int_as_float(ch.y), 0.0f, 0.0f);
+    cur = parent[cur];
+  }
+}
+
+// single-triangle mesh: one node whose second child is an empty box
+__global__ void k_single(const float* __restrict__ box_leaf, float4* __restrict__ nodes) {
+  const float big = 3.0e38f;
+  nodes[0] = make_float4(box_leaf[0], box_leaf[1], box_leaf[2], box_leaf[3]);
+  nodes[1] = make_float4(box_leaf[4], box_leaf[5], big, big);
+  nodes[2] = make_float4(big, -big, -big, -big);
+  nodes[3] = make_float4(__int_as_float(~0), __int_as_float(~0), 0.0f, 0.0f);
+}
+
+struct DevBuf {  // frees on scope exit
+  void* p = nullptr;
+  ~DevBuf() { if (p) cudaFree(p); }
+  template <class T> T* as() { return (T*)p; }
+};
+
+}  // namespace
+
+extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t* indices, int64_t nt,
+                                const uint8_t* facet_flags, int mem_space, void* cuda_stream, tpmc_mesh** out) {
+  if (!out) return TPMC_EINVAL;
+  *out = nullptr;
+  if (!vertices || !indices || nv < 3 || nt < 1 || nt > 0x3FFFFFFF || nv > 0x7FFFFFFF) return TPMC_EINVAL;
+  if (mem_space != TPMC_MEM_HOST && mem_space != TPMC_MEM_DEVICE) return TPMC_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int dev = 0;
+  TPMC_CUDA_TRY(cudaGetDevice(&dev));
+
+  DevBuf dv, di, df;
+  const float* d_v = vertices;
+  const int32_t* d_i = indices;
+  const uint8_t* d_f = facet_flags;
+  if (mem_space == TPMC_MEM_HOST) {
+    TPMC_CUDA_TRY(cudaMalloc(&dv.p, sizeof(float) * 3 * nv));
+    TPMC_CUDA_TRY(cudaMalloc(&di.p, sizeof(int32_t) * 3 * nt));
+    TPMC_CUDA_TRY(cudaMemcpyAsync(dv.p, vertices, sizeof(float) * 3 * nv, cudaMemcpyHostToDevice, st));
+    TPMC_CUDA_TRY(cudaMemcpyAsync(di.p, indices, sizeof(int32_t) * 3 * nt, cudaMemcpyHostToDevice, st));
+    d_v = dv.as<float>();
+    d_i = di.as<int32_t>();
+    if (facet_flags) {
+      TPMC_CUDA_TRY(cudaMalloc(&df.p, nt));
+      TPMC_CUDA_TRY(cudaMemcpyAsync(df.p, facet_flags, nt, cudaMemcpyHostToDevice, st));
+      d_f = df.as<uint8_t>();
+    }
+  }
+
+  cudaEvent_t e0, e1;
+  TPMC_CUDA_TRY(cudaEventCreate(&e0));
+  TPMC_CUDA_TRY(cudaEventCreate(&e1));
+  TPMC_CUDA_TRY(cudaEventRecord(e0, st));
+
+  // validate indices, bounds (O1)
+  DevBuf small;
+  TPMC_CUDA_TRY(cudaMalloc(&small.p, 64));
+  TPMC_CUDA_TRY(cudaMemsetAsync(small.p, 0, 64, st));
+  int* d_bad = small.as<int>();
+  float* d_aabb = small.as<float>() + 2;
+  double* d_r2 = (double*)((char*)small.p + 32);
+  k_check_indices<<<(unsigned)((3 * nt + kBlock - 1) / kBlock), kBlock, 0, st>>>(d_i, 3 * nt, nv, d_bad);
+  k_vertex_aabb<<<1, 1024, 0, st>>>(d_v, nv, d_aabb);
+  struct { int bad; int pad; float aabb[6]; double r2; } h;
+  TPMC_CUDA_TRY(cudaMemcpyAsync(&h, small.p, 32, cudaMemcpyDeviceToHost, st));
+  TPMC_CUDA_TRY(cudaStreamSynchronize(st));
+  if (h.bad) { cudaEventDestroy(e0); cudaEventDestroy(e1); return TPMC_EINVAL; }
+  for (int a = 0; a < 6; ++a)
+    if (!isfinite(h.aabb[a])) { cudaEventDestroy(e0); cudaEventDestroy(e1); return TPMC_EINVAL; }
+  double centre[3];
+  for (int a = 0; a < 3; ++a) centre[a] = 0.5 * ((double)h.aabb[a] + (double)h.aabb[3 + a]);
+  k_vertex_r2<<<1, 1024, 0, st>>>(d_v, nv, centre[0], centre[1], centre[2], d_r2);
+  TPMC_CUDA_TRY(cudaMemcpyAsync(&h.r2, d_r2, 8, cudaMemcpyDeviceToHost, st));
+  TPMC_CUDA_TRY(cudaStreamSynchronize(st));
+  if (!(h.r2 > 0.0)) { cudaEventDestroy(e0); cudaEventDestroy(e1); return TPMC_EINVAL; }
+
+  tpmc_mesh* m = new (std::nothrow) tpmc_mesh();
+  if (!m) return TPMC_ENOMEM;
+  memset(m, 0, sizeof(*m));
+  m->nv = nv; m->nt = nt; m->device = dev;
+  m->n_nodes = nt > 1 ? nt - 1 : 1;
+  for (int a = 0; a < 3; ++a) { m->centre[a] = centre[a]; m->aabb_lo[a] = h.aabb[a]; m->aabb_hi[a] = h.aabb[3 + a]; }
+  m->Rb = sqrt(h.r2);
+  m->ev0 = e0; m->ev1 = e1;
+
+#define MESH_TRY(expr)                       \
+  do {                                       \
+    int _rc = [&]() -> int { TPMC_CUDA_TRY(expr); return TPMC_OK; }(); \
+    if (_rc != TPMC_OK) { tpmc_mesh_destroy(m); return _rc; }          \
+  } while (0)
+
+  MESH_TRY(cudaMalloc((void**)&m->nodes, sizeof(float4) * 4 * m->n_nodes));
+  MESH_TRY(cudaMalloc((void**)&m->tris, sizeof(float4) * 3 * nt));
+
+  DevBuf keys, keys2, ids, ids2, tmp, box, kids, par, arr;
+  const int64_t n_int = nt - 1;
+  MESH_TRY(cudaMalloc(&keys.p, sizeof(uint64_t) * nt));
+  MESH_TRY(cudaMalloc(&keys2.p, sizeof(uint64_t) * nt));
+  MESH_TRY(cudaMalloc(&ids.p, sizeof(int32_t) * nt));
+  MESH_TRY(cudaMalloc(&ids2.p, sizeof(int32_t) * nt));
+  MESH_TRY(cudaMalloc(&box.p, sizeof(float) * 6 * (size_t)(n_int + nt)));
+  const unsigned gt = (unsigned)((nt + kBlock - 1) / kBlock);
+  float3 lo = make_float3(h.aabb[0], h.aabb[1], h.aabb[2]);
+  float3 ie;
+  ie.x = h.aabb[3] > h.aabb[0] ? 1.0f / (h.aabb[3] - h.aabb[0]) : 0.0f;
+  ie.y = h.aabb[4] > h.aabb[1] ? 1.0f / (h.aabb[4] - h.aabb[1]) : 0.0f;
+  ie.z = h.aabb[5] > h.aabb[2] ? 1.0f / (h.aabb[5] - h.aabb[2]) : 0.0f;
+  k_morton<<<gt, kBlock, 0, st>>>(d_v, d_i, nt, lo, ie, keys.as<uint64_t>(), ids.as<int32_t>());
+  size_t tmp_bytes = 0;
+  MESH_TRY(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys.as<uint64_t>(), keys2.as<uint64_t>(),
+                                           ids.as<int32_t>(), ids2.as<int32_t>(), (int)nt, 0, 63, st));
+  MESH_TRY(cudaMalloc(&tmp.p, tmp_bytes ? tmp_bytes : 16));
+  MESH_TRY(cub::DeviceRadixSort::SortPairs(tmp.p, tmp_bytes, keys.as<uint64_t>(), keys2.as<uint64_t>(),
+                                           ids.as<int32_t>(), ids2.as<int32_t>(), (int)nt, 0, 63, st));
+  k_gather<<<gt, kBlock, 0, st>>>(d_v, d_i, d_f, ids2.as<int32_t>(), nt, m->tris, box.as<float>(), n_int);
+  if (nt == 1) {
+    k_single<<<1, 1, 0, st>>>(box.as<float>(), m->nodes);
+  } else {
+    MESH_TRY(cudaMalloc(&kids.p, sizeof(int2) * n_int));
+    MESH_TRY(cudaMalloc(&par.p, sizeof(int) * (size_t)(n_int + nt)));
+    MESH_TRY(cudaMalloc(&arr.p, sizeof(int) * n_int));
+    MESH_TRY(cudaMemsetAsync(arr.p, 0, sizeof(int) * n_int, st));
+    k_hierarchy<<<(unsigned)((n_int + kBlock - 1) / kBlock), kBlock, 0, st>>>(keys2.as<uint64_t>(), (int)nt,
+                                                                                kids.as<int2>(), par.as<int>());
+    k_refit<<<gt, kBlock, 0, st>>>((int)nt, kids.as<int2>(), par.as<int>(), box.as<float>(), arr.as<int>(), m->nodes);
+  }
+  MESH_TRY(cudaGetLastError());
+  MESH_TRY(cudaEventRecord(e1, st));
+  MESH_TRY(cudaStreamSynchronize(st));
+  float ms = 0.0f;
+  MESH_TRY(cudaEventElapsedTime(&ms, e0, e1));
+  m->build_ms = ms;
+#undef MESH_TRY
+  *out = m;
+  return TPMC_OK;
+}
+
+extern "C" void tpmc_mesh_destroy(tpmc_mesh* m) {
+  if (!m) return;
+  cudaFree(m->nodes); cudaFree(m->tris);
+  cudaFree(m->ray_o); cudaFree(m->ray_v); cudaFree(m->queue_count);
+  cudaFree(m->facet_scratch); cudaFree(m->partials); cudaFree(m->stats); cudaFree(m->totals);
+  if (m->wave_ev) {
+    for (int i = 0; i < 2 * kMaxTimedWaves + 1; ++i) cudaEventDestroy(m->wave_ev[i]);
+    delete[] m->wave_ev;
+  }
+  if (m->ev0) cudaEventDestroy(m->ev0);
+  if (m->ev1) cudaEventDestroy(m->ev1);
+  delete m;
+}
+
+extern "C" int tpmc_mesh_info(const tpmc_mesh* m, tpmc_mesh_info_t* out) {
+  if (!m || !out) return TPMC_EINVAL;
+  for (int a = 0; a < 3; ++a) { out->centre[a] = m->centre[a]; out->aabb_lo[a] = m->aabb_lo[a]; out->aabb_hi[a] = m->aabb_hi[a]; }
+  out->bounding_radius = m->Rb;
+  out->nt = m->nt;
+  out->n_nodes = m->n_nodes;
+  out->build_ms = m->build_ms;
+  return TPMC_OK;
+}
+
+namespace {
+__global__ void k_leaf_facets(const float4* __restrict__ tris, int64_t nt, int32_t* __restrict__ out) {
+  const int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (s < nt) out[s] = __float_as_int(tris[3 * s].w);
+}
+}  // namespace
+
+extern "C" int tpmc_mesh_copy_bvh(const tpmc_mesh* m, float* h_nodes, int32_t* h_leaf_facet) {
+  if (!m) return TPMC_EINVAL;
+  if (h_nodes) TPMC_CUDA_TRY(cudaMemcpy(h_nodes, m->nodes, sizeof(float4) * 4 * m->n_nodes, cudaMemcpyDeviceToHost));
+  if (h_leaf_facet) {
+    DevBuf t;
+    TPMC_CUDA_TRY(cudaMalloc(&t.p, sizeof(int32_t) * m->nt));
+    k_leaf_facets<<<(unsigned)((m->nt + kBlock - 1) / kBlock), kBlock>>>(m->tris, m->nt, t.as<int32_t>());
+    TPMC_CUDA_TRY(cudaMemcpy(h_leaf_facet, t.p, sizeof(int32_t) * m->nt, cudaMemcpyDeviceToHost));
+  }
+  return TPMC_OK;
+}
+
+extern "C" const char* tpmc_strerror(int code) {
+  switch (code) {
+    case TPMC_OK: return "ok";
+    case TPMC_EINVAL: return "invalid argument";
+    case TPMC_ENOMEM: return "out of memory";
+    case TPMC_ECUDA: return "CUDA error";
+    default: return "unknown error";
+  }
+}
+extern "C" const char* tpmc_last_cuda_error(void) { return g_tpmc_cuda_error; }
+extern "C" const char* tpmc_version(void) { return "tpmc-b200 0.1 (sm_100a)"; }

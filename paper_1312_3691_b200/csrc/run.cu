@@ -1,0 +1,482 @@
+// run.cu -- the hot path behind tpmc_run: seed -> trace -> reflect -> accumulate -> reduce
+// (steps a1-a7 of DESIGN.md).
+#include <algorithm>
+#include <cstdlib>
+#include <new>
+
+#include "common.cuh"
+#include "sampling.cuh"
+#include "trace.cuh"
+
+namespace {
+
+constexpr int kSeedBlock = 256;
+constexpr int kTraceBlock = 128;
+constexpr int kReduceBlock = 256;
+constexpr int kReduceParts = 296;   // 2 per SM
+
+enum { ST_HITS = 0, ST_TRUNC = 1, ST_CULLED = 2, ST_TRIS = 3, ST_NODES = 4, ST_COUNT = 8 };
+
+__device__ __forceinline__ unsigned lanemask_lt() {
+  unsigned m;
+  asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+  return m;
+}
+
+// ------------------------------------------------------------------------------------------------
+__global__ void k_init_debug(tpmc_debug dbg, unsigned long long count) {
+  const unsigned long long j = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x;
+  if (j >= count) return;
+  if (dbg.hash) dbg.hash[j] = 0xCBF29CE484222325ull;
+  if (dbg.bounces) dbg.bounces[j] = 0u;
+  if (dbg.first_facet) dbg.first_facet[j] = -1;
+}
+
+// a2: seed one wave of particles, round the state to fp32 (O9), drop the rays that cannot touch the
+// mesh AABB (their single segment is an escape) and append the rest to the ray queue.
+__global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned long long wave_first,
+                                                     unsigned int wave_n, float4* __restrict__ ray_o,
+                                                     float4* __restrict__ ray_v, unsigned int* __restrict__ qcount,
+                                                     unsigned long long* __restrict__ stats) {
+  const unsigned int j = blockIdx.x * blockDim.x + threadIdx.x;
+  const bool active = j < wave_n;
+  bool keep = false;
+  float o[3] = {0, 0, 0}, v[3] = {1, 1, 1};
+  int species = 0;
+  if (active) {
+    const SeedState s = seed_particle(rc, rc.first + wave_first + j);
+    species = s.species;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { o[k] = (float)s.x[k]; v[k] = (float)s.v[k]; }
+    const float id[3] = {1.0f / v[0], 1.0f / v[1], 1.0f / v[2]};
+    float tn;
+    keep = slab(rc.aabb_lo[0], rc.aabb_lo[1], rc.aabb_lo[2], rc.aabb_hi[0], rc.aabb_hi[1], rc.aabb_hi[2], o, id,
+                INFINITY, tn);
+  }
+  const unsigned m = __ballot_sync(0xFFFFFFFFu, keep);
+  const unsigned mc = __ballot_sync(0xFFFFFFFFu, active && !keep);
+  const int lane = threadIdx.x & 31;
+  unsigned base = 0;
+  if (lane == 0) {
+    if (m) base = atomicAdd(qcount, (unsigned)__popc(m));
+    if (mc) atomicAdd(&stats[ST_CULLED], (unsigned long long)__popc(mc));
+  }
+  base = __shfl_sync(0xFFFFFFFFu, base, 0);
+  if (keep) {
+    const unsigned slot = base + __popc(m & lanemask_lt());
+    ray_o[slot] = make_float4(o[0], o[1], o[2], __uint_as_float(j));
+    ray_v[slot] = make_float4(v[0], v[1], v[2], __int_as_float(species));
+  }
+}
+
+// a3-a6: every queued particle is followed to escape: closest hit -> surface interaction ->
+// per-facet momentum (fp64 atomics) -> next segment.
+__global__ void __launch_bounds__(kTraceBlock) k_trace(const RunConst rc, unsigned long long wave_first,
+                                                       const float4* __restrict__ nodes,
+                                                       const float4* __restrict__ tris,
+                                                       const float4* __restrict__ ray_o,
+                                                       const float4* __restrict__ ray_v,
+                                                       const unsigned int* __restrict__ qcount,
+                                                       double* __restrict__ P, double* __restrict__ torque,
+                                                       unsigned long long* __restrict__ stats, tpmc_debug dbg) {
+  __shared__ int sstack[TPMC_STACK_SMEM * kTraceBlock];
+  __shared__ double sred[3][kTraceBlock / 32];
+  __shared__ unsigned long long scnt[4][kTraceBlock / 32];
+  const unsigned int n = *qcount;
+  double tq[3] = {0.0, 0.0, 0.0};
+  unsigned long long hits = 0, trunc = 0;
+  TraceCounters cnt;
+  cnt.nodes = 0; cnt.tris = 0;
+  unsigned long long nodes_tot = 0, tris_tot = 0;
+  for (unsigned int r = blockIdx.x * blockDim.x + threadIdx.x; r < n; r += gridDim.x * blockDim.x) {
+    const float4 ro = ray_o[r], rv = ray_v[r];
+    float o[3] = {ro.x, ro.y, ro.z}, v[3] = {rv.x, rv.y, rv.z};
+    const unsigned long long j = wave_first + __float_as_uint(ro.w);
+    const unsigned long long i = rc.first + j;
+    const int species = __float_as_int(rv.w);
+    const double w = rc.sp[species].w, cW = rc.sp[species].cW;
+    int f_prev = -1, first = -1;
+    unsigned int k = 0;
+    unsigned long long h = 0xCBF29CE484222325ull;
+    for (;;) {
+      const Hit hit = closest_hit(nodes, tris, o, v, f_prev, sstack + threadIdx.x, kTraceBlock, cnt);
+      if (hit.facet < 0) break;
+      ++hits;
+      if (k == 0) first = hit.facet;
+      h = fnv1a_facet(h, hit.facet);
+      const float4 q0 = __ldg(tris + 3 * (size_t)hit.slot), q1 = __ldg(tris + 3 * (size_t)hit.slot + 1),
+                   q2 = __ldg(tris + 3 * (size_t)hit.slot + 2);
+      double vout[3];
+      reflect(q0, q1, q2, v, rc.sigma, cW, particle_block(rc, i, 2u + k), vout);
+      // O12: dp = w (v_in - v_out) on the fp32 values; hit point o + tau v in fp64
+      double hp[3], dp[3];
+      float vo[3];
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        vo[a] = (float)vout[a];
+        hp[a] = __dadd_rn((double)o[a], __dmul_rn(hit.tau, (double)v[a]));
+        dp[a] = w * ((double)v[a] - (double)vo[a]);
+        atomicAdd(&P[3 * (size_t)hit.facet + a], dp[a]);
+      }
+      const double rx = hp[0] - rc.x_ref[0], ry = hp[1] - rc.x_ref[1], rz = hp[2] - rc.x_ref[2];
+      tq[0] += ry * dp[2] - rz * dp[1];
+      tq[1] += rz * dp[0] - rx * dp[2];
+      tq[2] += rx * dp[1] - ry * dp[0];
+      // O13: next segment starts at the fp32-rounded hit point
+#pragma unroll
+      for (int a = 0; a < 3; ++a) { o[a] = (float)hp[a]; v[a] = vo[a]; }
+      f_prev = hit.facet;
+      ++k;
+      if (k >= rc.max_bounces) { ++trunc; break; }
+    }
+    if (dbg.hash) dbg.hash[j] = h;
+    if (dbg.bounces) dbg.bounces[j] = k;
+    if (dbg.first_facet) dbg.first_facet[j] = first;
+    nodes_tot += cnt.nodes; tris_tot += cnt.tris;
+    cnt.nodes = 0; cnt.tris = 0;
+  }
+  // block reduction of the torque and the counters, one atomic per block and quantity
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  unsigned long long c4[4] = {hits, trunc, tris_tot, nodes_tot};
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a) tq[a] += __shfl_down_sync(0xFFFFFFFFu, tq[a], off);
+#pragma unroll
+    for (int a = 0; a < 4; ++a) c4[a] += __shfl_down_sync(0xFFFFFFFFu, c4[a], off);
+  }
+  if (lane == 0) {
+    for (int a = 0; a < 3; ++a) sred[a][wid] = tq[a];
+    for (int a = 0; a < 4; ++a) scnt[a][wid] = c4[a];
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t3[3] = {0, 0, 0};
+    unsigned long long s4[4] = {0, 0, 0, 0};
+    for (int wv = 0; wv < kTraceBlock / 32; ++wv) {
+      for (int a = 0; a < 3; ++a) t3[a] += sred[a][wv];
+      for (int a = 0; a < 4; ++a) s4[a] += scnt[a][wv];
+    }
+    for (int a = 0; a < 3; ++a) if (t3[a] != 0.0) atomicAdd(&torque[a], t3[a]);
+    if (s4[0]) atomicAdd(&stats[ST_HITS], s4[0]);
+    if (s4[1]) atomicAdd(&stats[ST_TRUNC], s4[1]);
+    if (s4[2]) atomicAdd(&stats[ST_TRIS], s4[2]);
+    if (s4[3]) atomicAdd(&stats[ST_NODES], s4[3]);
+  }
+}
+
+// a7: F = sum_f P_f by a fixed-shape tree (deterministic for given P): parts -> one block.
+__global__ void __launch_bounds__(kReduceBlock) k_reduce_parts(const double* __restrict__ P, long long nt,
+                                                               double* __restrict__ parts) {
+  __shared__ double s[3][kReduceBlock];
+  const long long chunk = (nt + gridDim.x - 1) / gridDim.x;
+  const long long b = (long long)blockIdx.x * chunk, e = min(nt, b + chunk);
+  double acc[3] = {0, 0, 0};
+  for (long long f = b + threadIdx.x; f < e; f += kReduceBlock)
+    for (int a = 0; a < 3; ++a) acc[a] += P[3 * f + a];
+  for (int a = 0; a < 3; ++a) s[a][threadIdx.x] = acc[a];
+  __syncthreads();
+  for (int st = kReduceBlock / 2; st > 0; st >>= 1) {
+    if ((int)threadIdx.x < st)
+      for (int a = 0; a < 3; ++a) s[a][threadIdx.x] += s[a][threadIdx.x + st];
+    __syncthreads();
+  }
+  if (threadIdx.x < 3) parts[3 * blockIdx.x + threadIdx.x] = s[threadIdx.x][0];
+}
+
+__global__ void k_reduce_final(const double* __restrict__ parts, int nparts, const double* __restrict__ torque_acc,
+                               double* __restrict__ force, double* __restrict__ torque) {
+  const int a = threadIdx.x;
+  if (a < 3) {
+    double f = 0.0;
+    for (int p = 0; p < nparts; ++p) f += parts[3 * p + a];
+    force[a] = f;
+    torque[a] = torque_acc[a];
+  }
+}
+
+// ---- stand-alone steps for parity checks -----------------------------------------------------------
+__global__ void k_seed_only(const RunConst rc, double* __restrict__ x, double* __restrict__ v,
+                            int32_t* __restrict__ species) {
+  const unsigned long long j = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x;
+  if (j >= rc.count) return;
+  const SeedState s = seed_particle(rc, rc.first + j);
+  for (int k = 0; k < 3; ++k) { x[3 * j + k] = s.x[k]; v[3 * j + k] = s.v[k]; }
+  if (species) species[j] = s.species;
+}
+
+__global__ void __launch_bounds__(kTraceBlock) k_trace_only(const float4* __restrict__ nodes,
+                                                            const float4* __restrict__ tris,
+                                                            const float* __restrict__ o, const float* __restrict__ d,
+                                                            const int32_t* __restrict__ f_prev, long long n,
+                                                            int32_t* __restrict__ facet, double* __restrict__ tau) {
+  __shared__ int sstack[TPMC_STACK_SMEM * kTraceBlock];
+  const long long r = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (r >= n) return;
+  const float of[3] = {o[3 * r], o[3 * r + 1], o[3 * r + 2]};
+  const float df[3] = {d[3 * r], d[3 * r + 1], d[3 * r + 2]};
+  TraceCounters cnt;
+  cnt.nodes = 0; cnt.tris = 0;
+  const Hit h = closest_hit(nodes, tris, of, df, f_prev ? f_prev[r] : -1, sstack + threadIdx.x, kTraceBlock, cnt);
+  facet[r] = h.facet;
+  tau[r] = h.tau;
+}
+
+// ---- a1: per-run constants on the host, fp64 -------------------------------------------------------
+double host_Gt(double y) { return 0.25 * TPMC_SQRTPI * (1.0 + 2.0 * y * y) * erfc(-y) + 0.5 * y * exp(-y * y); }
+
+// Gamma / (c n r^2), eq. (10); erf(S)/S by series below 1e-4 (A19)
+double host_flux_bracket(double S) {
+  const double pi = 3.14159265358979323846;
+  const double erf_over_S = (S < 1e-4) ? (2.0 / TPMC_SQRTPI) * (1.0 - S * S / 3.0) : erf(S) / S;
+  return TPMC_SQRTPI * exp(-S * S) + 0.5 * pi * erf_over_S + pi * S * erf(S);
+}
+
+// eq. (15) P:207-209 (A5): R zhat = ztilde = -V/|V|, Rodrigues about (zhat x ztilde)/|.|
+void host_rotation(const double V[3], double R[9]) {
+  const double sp = sqrt(V[0] * V[0] + V[1] * V[1] + V[2] * V[2]);
+  double zt[3] = {0.0, 0.0, 1.0};
+  if (sp > 0.0) { zt[0] = -V[0] / sp; zt[1] = -V[1] / sp; zt[2] = -V[2] / sp; }
+  const double ax = -zt[1], ay = zt[0];
+  const double sb = sqrt(ax * ax + ay * ay), cb = zt[2];
+  for (int k = 0; k < 9; ++k) R[k] = 0.0;
+  if (sb < 1e-12) {
+    R[0] = 1.0;
+    R[4] = R[8] = (cb > 0.0) ? 1.0 : -1.0;
+    return;
+  }
+  const double ux = ax / sb, uy = ay / sb, uz = 0.0, omc = 1.0 - cb;
+  R[0] = cb + ux * ux * omc;      R[1] = ux * uy * omc - uz * sb; R[2] = ux * uz * omc + uy * sb;
+  R[3] = uy * ux * omc + uz * sb; R[4] = cb + uy * uy * omc;      R[5] = uy * uz * omc - ux * sb;
+  R[6] = uz * ux * omc - uy * sb; R[7] = uz * uy * omc + ux * sb; R[8] = cb + uz * uz * omc;
+}
+
+int make_run_const(const tpmc_mesh* m, const tpmc_params* p, RunConst* rc) {
+  if (!m || !p || !p->m || !p->x) return TPMC_EINVAL;
+  if (p->n_species < 1 || p->n_species > TPMC_MAX_SPECIES) return TPMC_EINVAL;
+  if (!(p->T_inf > 0.0) || !(p->T_W > 0.0) || !(p->n >= 0.0) || !isfinite(p->n)) return TPMC_EINVAL;
+  if (!(p->accommodation >= 0.0 && p->accommodation <= 1.0)) return TPMC_EINVAL;
+  if (!(p->cv_radius_factor >= 1.0) || !isfinite(p->cv_radius_factor)) return TPMC_EINVAL;
+  if (p->N == 0 || p->first > p->N || p->count > p->N - p->first) return TPMC_EINVAL;
+  if (p->max_bounces < 1 || p->max_bounces > 0x7FFFFFF0u) return TPMC_EINVAL;
+  double xs = 0.0;
+  for (int s = 0; s < p->n_species; ++s) {
+    if (!(p->m[s] > 0.0) || !(p->x[s] >= 0.0)) return TPMC_EINVAL;
+    xs += p->x[s];
+  }
+  if (fabs(xs - 1.0) > 1e-9) return TPMC_EINVAL;
+  for (int a = 0; a < 3; ++a)
+    if (!isfinite(p->V[a]) || !isfinite(p->x_ref[a])) return TPMC_EINVAL;
+  memset(rc, 0, sizeof(*rc));
+  const double speed = sqrt((p->V[0] * p->V[0] + p->V[1] * p->V[1]) + p->V[2] * p->V[2]);
+  const double r = p->cv_radius_factor * m->Rb;
+  double acc = 0.0;
+  for (int s = 0; s < p->n_species; ++s) {
+    SpeciesConst& sc = rc->sp[s];
+    sc.c = sqrt(2.0 * TPMC_KB * p->T_inf / p->m[s]);
+    sc.S = speed / sc.c;
+    sc.cW = sqrt(2.0 * TPMC_KB * p->T_W / p->m[s]);
+    sc.w = p->m[s] * (host_flux_bracket(sc.S) * sc.c * p->n * r * r) / (double)p->N;
+    sc.g0 = host_Gt(-sc.S);
+    sc.gI = host_Gt(sc.S) - sc.g0;
+    acc += p->x[s];
+    sc.cumx = acc;
+  }
+  rc->n_species = p->n_species;
+  host_rotation(p->V, rc->R);
+  for (int a = 0; a < 3; ++a) {
+    rc->centre[a] = m->centre[a];
+    rc->x_ref[a] = p->x_ref[a];
+    rc->aabb_lo[a] = m->aabb_lo[a];
+    rc->aabb_hi[a] = m->aabb_hi[a];
+  }
+  rc->r = r;
+  rc->sigma = p->accommodation;
+  rc->first = p->first;
+  rc->count = p->count;
+  rc->seed_lo = (unsigned int)p->seed;
+  rc->seed_hi = (unsigned int)(p->seed >> 32);
+  rc->max_bounces = p->max_bounces;
+  return TPMC_OK;
+}
+
+size_t wave_size() {
+  static size_t w = 0;
+  if (!w) {
+    const char* e = getenv("TPMC_WAVE");
+    long long v = e ? atoll(e) : 0;
+    w = (v >= 1024 && v <= (1ll << 28)) ? (size_t)v : ((size_t)1 << 22);
+  }
+  return w;
+}
+
+int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
+  if (!m->queue_count) {
+    TPMC_CUDA_TRY(cudaMalloc((void**)&m->queue_count, 4 * sizeof(unsigned int)));
+    TPMC_CUDA_TRY(cudaMalloc((void**)&m->stats, ST_COUNT * sizeof(unsigned long long)));
+    TPMC_CUDA_TRY(cudaMalloc((void**)&m->totals, 4 * sizeof(double)));
+    TPMC_CUDA_TRY(cudaMalloc((void**)&m->partials, 3 * kReduceParts * sizeof(double)));
+  }
+  if (m->wave_cap < wave) {
+    cudaFree(m->ray_o); cudaFree(m->ray_v);
+    m->ray_o = m->ray_v = nullptr; m->wave_cap = 0;
+    TPMC_CUDA_TRY(cudaMalloc((void**)&m->ray_o, wave * sizeof(float4)));
+    TPMC_CUDA_TRY(cudaMalloc((void**)&m->ray_v, wave * sizeof(float4)));
+    m->wave_cap = wave;
+  }
+  if (need_facets && !m->facet_scratch)
+    TPMC_CUDA_TRY(cudaMalloc((void**)&m->facet_scratch, 3 * sizeof(double) * (size_t)m->nt));
+  return TPMC_OK;
+}
+
+int trace_grid() {
+  static int g = 0;
+  if (!g) {
+    int dev = 0, sms = 148, per = 8;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_trace, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
+    g = sms * per;
+  }
+  return g;
+}
+
+int fill_stats(tpmc_mesh* m, const tpmc_params* params, tpmc_stats* h_stats) {
+  unsigned long long hs[ST_COUNT];
+  TPMC_CUDA_TRY(cudaMemcpy(hs, m->stats, sizeof(hs), cudaMemcpyDeviceToHost));
+  float ms = 0.0f;
+  TPMC_CUDA_TRY(cudaEventElapsedTime(&ms, m->ev0, m->ev1));
+  h_stats->hits = hs[ST_HITS];
+  h_stats->truncated = hs[ST_TRUNC];
+  h_stats->culled = hs[ST_CULLED];
+  h_stats->tri_tests = hs[ST_TRIS];
+  h_stats->node_visits = hs[ST_NODES];
+  h_stats->segments = params->count + hs[ST_HITS] - hs[ST_TRUNC];
+  h_stats->escaped = params->count - hs[ST_TRUNC];
+  h_stats->kernel_launches = m->last_launches;
+  h_stats->ms = ms;
+  h_stats->ms_seed = h_stats->ms_trace = 0.0;
+  h_stats->timed_waves = m->last_timed_waves;
+  for (unsigned long long w = 0; w < m->last_timed_waves; ++w) {
+    float a = 0.0f, b = 0.0f;
+    TPMC_CUDA_TRY(cudaEventElapsedTime(&a, m->wave_ev[2 * w], m->wave_ev[2 * w + 1]));
+    TPMC_CUDA_TRY(cudaEventElapsedTime(&b, m->wave_ev[2 * w + 1], m->wave_ev[2 * w + 2]));
+    h_stats->ms_seed += a;
+    h_stats->ms_trace += b;
+  }
+  return TPMC_OK;
+}
+
+}  // namespace
+
+extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* cuda_stream, double* d_force,
+                        double* d_torque, double* d_facet_momentum, tpmc_stats* h_stats, const tpmc_debug* debug) {
+  if (!mesh || !params || !d_force || !d_torque) return TPMC_EINVAL;
+  tpmc_mesh* m = const_cast<tpmc_mesh*>(mesh);   // the handle caches scratch
+  RunConst rc;
+  int rcode = make_run_const(m, params, &rc);
+  if (rcode != TPMC_OK) return rcode;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t wave = std::min<unsigned long long>(std::max<unsigned long long>(params->count, 1), wave_size());
+  rcode = ensure_scratch(m, wave, d_facet_momentum == nullptr);
+  if (rcode != TPMC_OK) return rcode;
+  double* P = d_facet_momentum ? d_facet_momentum : m->facet_scratch;
+  tpmc_debug dbg = {nullptr, nullptr, nullptr};
+  if (debug) dbg = *debug;
+
+  TPMC_CUDA_TRY(cudaEventRecord(m->ev0, st));
+  TPMC_CUDA_TRY(cudaMemsetAsync(P, 0, 3 * sizeof(double) * (size_t)m->nt, st));
+  TPMC_CUDA_TRY(cudaMemsetAsync(m->stats, 0, ST_COUNT * sizeof(unsigned long long), st));
+  TPMC_CUDA_TRY(cudaMemsetAsync(m->totals, 0, 4 * sizeof(double), st));
+  if ((dbg.hash || dbg.bounces || dbg.first_facet) && params->count)
+    k_init_debug<<<(unsigned)((params->count + 255) / 256), 256, 0, st>>>(dbg, params->count);
+  const int tgrid = trace_grid();
+  const bool timed = (h_stats != nullptr);   // per-kernel events only when the caller will read them
+  if (timed && !m->wave_ev) {
+    m->wave_ev = new (std::nothrow) cudaEvent_t[2 * kMaxTimedWaves + 1];
+    if (!m->wave_ev) return TPMC_ENOMEM;
+    for (int i = 0; i < 2 * kMaxTimedWaves + 1; ++i) TPMC_CUDA_TRY(cudaEventCreate(&m->wave_ev[i]));
+  }
+  unsigned long long launches = (dbg.hash || dbg.bounces || dbg.first_facet) && params->count ? 1 : 0, wi = 0;
+  for (unsigned long long w0 = 0; w0 < params->count; w0 += wave, ++wi) {
+    const unsigned int wn = (unsigned int)std::min<unsigned long long>(wave, params->count - w0);
+    TPMC_CUDA_TRY(cudaMemsetAsync(m->queue_count, 0, sizeof(unsigned int), st));
+    const bool tw = timed && wi < (unsigned long long)kMaxTimedWaves;
+    if (tw) TPMC_CUDA_TRY(cudaEventRecord(m->wave_ev[2 * wi], st));
+    k_seed<<<(wn + kSeedBlock - 1) / kSeedBlock, kSeedBlock, 0, st>>>(rc, w0, wn, m->ray_o, m->ray_v, m->queue_count,
+                                                                     m->stats);
+    if (tw) TPMC_CUDA_TRY(cudaEventRecord(m->wave_ev[2 * wi + 1], st));
+    k_trace<<<tgrid, kTraceBlock, 0, st>>>(rc, w0, m->nodes, m->tris, m->ray_o, m->ray_v, m->queue_count, P, m->totals,
+                                           m->stats, dbg);
+    if (tw) TPMC_CUDA_TRY(cudaEventRecord(m->wave_ev[2 * wi + 2], st));
+    launches += 2;
+  }
+  k_reduce_parts<<<kReduceParts, kReduceBlock, 0, st>>>(P, (long long)m->nt, m->partials);
+  k_reduce_final<<<1, 32, 0, st>>>(m->partials, kReduceParts, m->totals, d_force, d_torque);
+  launches += 2;
+  m->last_launches = launches;
+  m->last_timed_waves = timed ? std::min<unsigned long long>(wi, kMaxTimedWaves) : 0;
+  TPMC_CUDA_TRY(cudaGetLastError());
+  TPMC_CUDA_TRY(cudaEventRecord(m->ev1, st));
+  if (h_stats) {
+    TPMC_CUDA_TRY(cudaStreamSynchronize(st));
+    return fill_stats(m, params, h_stats);
+  }
+  return TPMC_OK;
+}
+
+extern "C" int tpmc_run_host(const tpmc_mesh* mesh, const tpmc_params* params, void* cuda_stream, double* h_force,
+                             double* h_torque, double* h_facet_momentum, tpmc_stats* h_stats) {
+  if (!mesh || !params || !h_force || !h_torque) return TPMC_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  tpmc_mesh* m = const_cast<tpmc_mesh*>(mesh);
+  double* d_ft = nullptr;
+  TPMC_CUDA_TRY(cudaMalloc((void**)&d_ft, 6 * sizeof(double)));
+  int rc = TPMC_OK;
+  if (h_facet_momentum && !m->facet_scratch) {
+    cudaError_t e = cudaMalloc((void**)&m->facet_scratch, 3 * sizeof(double) * (size_t)m->nt);
+    if (e != cudaSuccess) { cudaFree(d_ft); cudaGetLastError(); return TPMC_ENOMEM; }
+  }
+  tpmc_stats tmp_stats;
+  rc = tpmc_run(mesh, params, cuda_stream, d_ft, d_ft + 3, h_facet_momentum ? m->facet_scratch : nullptr,
+                h_stats ? &tmp_stats : nullptr, nullptr);
+  if (rc == TPMC_OK) {
+    double ft[6];
+    cudaError_t e = cudaMemcpyAsync(ft, d_ft, sizeof(ft), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && h_facet_momentum)
+      e = cudaMemcpyAsync(h_facet_momentum, m->facet_scratch, 3 * sizeof(double) * (size_t)m->nt,
+                          cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) {
+      snprintf(g_tpmc_cuda_error, sizeof(g_tpmc_cuda_error), "tpmc_run_host: %s", cudaGetErrorString(e));
+      rc = TPMC_ECUDA;
+    } else {
+      for (int a = 0; a < 3; ++a) { h_force[a] = ft[a]; h_torque[a] = ft[3 + a]; }
+      if (h_stats) *h_stats = tmp_stats;
+    }
+  }
+  cudaFree(d_ft);
+  return rc;
+}
+
+extern "C" int tpmc_seed(const tpmc_mesh* mesh, const tpmc_params* params, void* cuda_stream, double* d_x, double* d_v,
+                         int32_t* d_species) {
+  if (!mesh || !params || !d_x || !d_v) return TPMC_EINVAL;
+  RunConst rc;
+  const int rcode = make_run_const(mesh, params, &rc);
+  if (rcode != TPMC_OK) return rcode;
+  if (params->count == 0) return TPMC_OK;
+  k_seed_only<<<(unsigned)((params->count + 127) / 128), 128, 0, (cudaStream_t)cuda_stream>>>(rc, d_x, d_v, d_species);
+  TPMC_CUDA_TRY(cudaGetLastError());
+  return TPMC_OK;
+}
+
+extern "C" int tpmc_trace(const tpmc_mesh* mesh, const float* d_o, const float* d_d, const int32_t* d_f_prev, int64_t n,
+                          void* cuda_stream, int32_t* d_facet, double* d_tau) {
+  if (!mesh || !d_o || !d_d || !d_facet || !d_tau || n < 0) return TPMC_EINVAL;
+  if (n == 0) return TPMC_OK;
+  k_trace_only<<<(unsigned)((n + kTraceBlock - 1) / kTraceBlock), kTraceBlock, 0, (cudaStream_t)cuda_stream>>>(
+      mesh->nodes, mesh->tris, d_o, d_d, d_f_prev, (long long)n, d_facet, d_tau);
+  TPMC_CUDA_TRY(cudaGetLastError());
+  return TPMC_OK;
+}

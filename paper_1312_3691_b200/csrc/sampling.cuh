@@ -1,0 +1,121 @@
+// sampling.cuh -- step a2: consistent particle seeding on the spherical control volume
+// (eqs. 10, 11, 14a-c, 15; definitions O3-O8 of DESIGN.md).  Device code, fp64.
+//
+// Both random variates that the paper gives only as densities are drawn by INVERSE CDF (readings
+// A2/A3): one uniform per variate keeps the Philox counter layout fixed, and the result is a
+// mathematically defined function of the uniform, so any convergent root-finder gives the same value.
+#pragma once
+
+#include "common.cuh"
+
+// chi(s) = e^{-s^2} + sqrt(pi) s erfc(-s): bracket of eq. (8) P:143 written without cancellation (A4)
+TPMC_HD double chi_fn(double s) { return exp(-s * s) + TPMC_SQRTPI * s * erfc(-s); }
+
+// Position (eq. 11).  With t = sin(phi), y = S t:  dP ~ chi(y) dy, antiderivative
+//   Gt(y) = (sqrt(pi)/4)(1 + 2 y^2) erfc(-y) + (y/2) e^{-y^2},   Gt' = chi > 0,  Gt'' = sqrt(pi) erfc(-y) > 0.
+// Solve Gt(y) = Gt(-S) + u [Gt(S) - Gt(-S)].  Gt is convex and increasing, so Newton from any point is
+// to the right of the root after one step and then decreases monotonically: no bracket is needed.
+TPMC_HD double sample_sin_phi(double u, const SpeciesConst& sc) {
+  const double S = sc.S;
+  if (S < 1e-4) {
+    // A19: chi(s) = 1 + sqrt(pi) s + s^2 + O(s^4):  H(t) = [(t+1) + sqrt(pi) S (t^2-1)/2 + S^2 (t^3+1)/3] / (2 + 2S^2/3)
+    const double rhs = u * (2.0 + 2.0 * S * S / 3.0);
+    double t = 2.0 * u - 1.0;
+    for (int it = 0; it < 8; ++it) {
+      const double f = (t + 1.0) + 0.5 * TPMC_SQRTPI * S * (t * t - 1.0) + S * S * (t * t * t + 1.0) / 3.0 - rhs;
+      const double d = 1.0 + TPMC_SQRTPI * S * t + S * S * t * t;
+      t -= f / d;
+    }
+    return fmin(1.0, fmax(-1.0, t));
+  }
+  const double target = sc.g0 + u * sc.gI;
+  // large-y asymptote Gt ~ sqrt(pi) (y^2 + 1/2) as first guess; anything works (see above)
+  double y = sqrt(fmax(target / TPMC_SQRTPI - 0.5, 0.0));
+  y = fmin(y, S);
+  for (int it = 0; it < 64; ++it) {
+    const double e = exp(-y * y);
+    const double ec = erfc(-y);
+    const double g = 0.25 * TPMC_SQRTPI * (1.0 + 2.0 * y * y) * ec + 0.5 * y * e;
+    const double d = e + TPMC_SQRTPI * y * ec;
+    double yn = y - (g - target) / d;
+    yn = fmin(S, fmax(-S, yn));
+    const double step = fabs(yn - y);
+    y = yn;
+    if (step <= 4e-16 * fmax(1.0, fabs(y))) break;
+  }
+  return fmin(1.0, fmax(-1.0, y / S));
+}
+
+// Inward normal speed (eq. 14a, read in x = v_n / c_mp, G2): density 2x e^{-(x-s)^2} / chi(s), x >= 0.
+// Survival form (A4):  1 - F(x) = Q(x)/chi(s),  Q(x) = e^{-(x-s)^2} + sqrt(pi) s erfc(x-s),  Q' = -2x e^{-(x-s)^2}.
+// F is convex left of the mode x* = (s + sqrt(s^2+2))/2 and concave right of it, so Newton started at the
+// mode converges monotonically from either side.
+TPMC_HD double sample_normal_speed(double u, double s) {
+  const double target = (1.0 - u) * chi_fn(s);
+  const double xm = 0.5 * (s + sqrt(s * s + 2.0));
+  double x = xm;
+  {  // cheap improvement of the start on the low side, where F ~ x^2 e^{-s^2}/chi(s): stays right of the root
+    const double q0 = chi_fn(s) - target;            // = u chi(s)
+    const double xs = sqrt(q0) * exp(0.5 * s * s);   // root of the leading term
+    if (xs < 0.25 * xm) x = fmin(xm, 2.0 * xs);
+  }
+  for (int it = 0; it < 96; ++it) {
+    const double z = x - s;
+    const double e = exp(-z * z);
+    const double q = e + TPMC_SQRTPI * s * erfc(z);
+    const double d = -2.0 * x * e;
+    double xn = x - (q - target) / d;
+    if (!(xn > 0.0)) xn = 0.5 * x;
+    const double step = fabs(xn - x);
+    x = xn;
+    if (step <= 4e-16 * (1.0 + x)) break;
+  }
+  return x;
+}
+
+struct SeedState {
+  double x[3];
+  double v[3];
+  int species;
+};
+
+// O3-O8 for particle i.  Uniform usage: block 0 = (species, sin phi, theta, v_n), block 1 = (rho, angle, -, -).
+TPMC_HD SeedState seed_particle(const RunConst& rc, unsigned long long i) {
+  const uint4 b0 = particle_block(rc, i, 0u);
+  const uint4 b1 = particle_block(rc, i, 1u);
+  SeedState out;
+  // A8: species by number fraction
+  const double u0 = u01(b0.x);
+  int s = 0;
+  while (s < rc.n_species - 1 && u0 >= rc.sp[s].cumx) ++s;
+  out.species = s;
+  const SpeciesConst& sc = rc.sp[s];
+  // O5: position on the unit sphere, stream frame (pole = upstream, A1)
+  const double t = sample_sin_phi(u01(b0.y), sc);
+  const double cphi = sqrt(1.0 - t * t);
+  double st, ct;
+  sincospi(2.0 * u01(b0.z), &st, &ct);
+  const double xh[3] = {cphi * ct, cphi * st, t};
+  // O6: local frame: n = -xhat inward, t1 meridional (downstream), t2 = t1 x n
+  const double t1[3] = {t * ct, t * st, -cphi};
+  const double t2[3] = {-st, ct, 0.0};
+  // O7: velocity components in units of c_mp (eqs. 14a-c)
+  const double xn = sample_normal_speed(u01(b0.w), sc.S * t);
+  const double rho = sqrt(-log(u01(b1.x)));
+  double sa, ca;
+  sincospi(2.0 * u01(b1.y), &sa, &ca);
+  const double xt1 = sc.S * cphi + rho * ca;
+  const double xt2 = rho * sa;
+  double vl[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) vl[k] = (xn * -xh[k] + xt1 * t1[k]) + xt2 * t2[k];
+  // O8: rotate to the body frame (eq. 15), scale
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const double rx = (rc.R[3 * k] * xh[0] + rc.R[3 * k + 1] * xh[1]) + rc.R[3 * k + 2] * xh[2];
+    const double rv = (rc.R[3 * k] * vl[0] + rc.R[3 * k + 1] * vl[1]) + rc.R[3 * k + 2] * vl[2];
+    out.x[k] = rc.centre[k] + rc.r * rx;
+    out.v[k] = sc.c * rv;
+  }
+  return out;
+}

@@ -1,0 +1,347 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star): integer/index work bit-exact -- Philox
+stream, closest-hit facet and, since both sides evaluate O10 in the same fp64 order, tau;
+per-particle hit-facet sequences equal on >= 99.99 % of particles; total force within 1e-4
+relative; per-facet momentum within 1e-3 relative on facets untouched by a mismatched particle
+(reading A18); seeding within 1e-12 relative before the fp32 rounding."""
+import numpy as np
+import pytest
+
+import tpmc_inputs as ti
+
+pytestmark = pytest.mark.gpu
+
+SEQ_AGREE = 0.9999     # >= 99.99 % identical hit sequences
+FORCE_RTOL = 1e-4
+FACET_RTOL = 1e-3
+SEED_RTOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def T():
+    import paper_1312_3691_b200 as t
+    return t
+
+
+@pytest.fixture(scope="module")
+def O():
+    import oracle
+    return oracle
+
+
+_mesh_cache = {}
+
+
+def meshes(T, O, cfg):
+    key = cfg.name + cfg.mesh().name
+    if key not in _mesh_cache:
+        m = cfg.mesh()
+        _mesh_cache[key] = (T.Mesh(m.vertices, m.indices, m.flags), O.OracleMesh(m.vertices, m.indices, m.flags))
+    return _mesh_cache[key]
+
+
+def compare_run(T, O, cfg, first, count, use_bvh=True):
+    gm, om = meshes(T, O, cfg)
+    g = gm.run(cfg, first=first, count=count, debug=True)
+    o = om.run(cfg, first=first, count=count, use_bvh=use_bvh)
+    gh = g.hash.cpu().numpy().view(np.uint64)
+    same = gh == o.hash
+    frac = same.mean() if count else 1.0
+    assert frac >= SEQ_AGREE, f"{cfg.label}: only {frac:.6f} of hit sequences agree"
+    gb = g.bounces.cpu().numpy().astype(np.uint32)
+    assert np.array_equal(gb[same], o.bounces[same])
+    assert np.array_equal(g.first_facet.cpu().numpy()[same], o.first_facet[same])
+    F = g.force.cpu().numpy()
+    assert np.linalg.norm(F - o.force) <= FORCE_RTOL * np.linalg.norm(o.force), (cfg.label, F, o.force)
+    Tq = g.torque.cpu().numpy()
+    assert np.linalg.norm(Tq - o.torque) <= FORCE_RTOL * max(np.linalg.norm(o.torque), 1e-3 * np.linalg.norm(o.force))
+    fm = g.facet_momentum.cpu().numpy()
+    if same.all():
+        assert g.stats["hits"] == o.hits and g.stats["segments"] == o.segments
+        assert g.stats["truncated"] == o.truncated and g.stats["escaped"] == o.escaped
+        nrm = np.linalg.norm(o.facet_momentum, axis=1)
+        err = np.linalg.norm(fm - o.facet_momentum, axis=1)
+        assert np.all(err <= FACET_RTOL * nrm + 1e-300), (cfg.label, float((err / np.maximum(nrm, 1e-300)).max()))
+        assert np.array_equal(nrm == 0, np.linalg.norm(fm, axis=1) == 0)       # untouched facets stay exactly zero
+    assert np.allclose(fm.sum(0), F, rtol=1e-12, atol=1e-30)                    # a7: F = sum_f P_f
+    return g, o, frac
+
+
+# ------------------------------------------------------------------ a2: seeding
+@pytest.mark.parametrize("name,idx,first,N", [("C1", 0, 0, 100_000), ("C2", 0, 123_456, 10_000_000),
+                                               ("C3", 1, 99_990_000, 100_000_000),
+                                               ("C5", 7, 6_000_000_000, 10_000_000_000)])
+def test_seed_parity(T, O, name, idx, first, N):
+    cfg = ti.config(name)[idx]
+    if name == "C5":
+        cfg = cfg.with_(mesh_fn=lambda: ti.large_body(5, 16))
+        cfg._mesh_cache = []
+    gm, om = meshes(T, O, cfg)
+    cnt = 3000
+    x, v, s = gm.seed(cfg, first=first, count=cnt, N=N)
+    x, v, s = x.cpu().numpy(), v.cpu().numpy(), s.cpu().numpy()
+    xs = np.abs(x).max()
+    for j in range(cnt):
+        xo, vo, so = om.seed(cfg, first + j, N=N)
+        assert so == s[j]
+        assert np.abs(x[j] - xo).max() <= SEED_RTOL * xs
+        assert np.abs(v[j] - vo).max() <= SEED_RTOL * np.abs(vo).max() + 1e-9
+    info = gm.info()
+    ctr, Rb = om.bounds()
+    assert np.array_equal(info["centre"], ctr) and info["bounding_radius"] == Rb     # O1 bit-exact
+
+
+def test_seed_equilibrium_and_tiny_speed_ratio(T, O):
+    base = ti.RunConfig("eq", lambda: ti.box(h=0.5), T_inf=500.0, T_W=500.0, V=(0.0, 0.0, 0.0), N=5000)
+    for V in ((0.0, 0.0, 0.0), (0.0, 1e-3, 0.0), (0.02, 0.0, 0.01)):
+        cfg = base.with_(V=V)
+        gm, om = meshes(T, O, cfg)
+        x, v, s = (a.cpu().numpy() for a in gm.seed(cfg))
+        for j in range(0, cfg.N, 7):
+            xo, vo, _ = om.seed(cfg, j)
+            assert np.abs(x[j] - xo).max() <= 1e-11 and np.abs(v[j] - vo).max() <= 1e-9
+
+
+# ------------------------------------------------------------------ a0: LBVH
+@pytest.mark.parametrize("mesh_fn", [lambda: ti.plate(30.0), lambda: ti.box(h=1.0), lambda: ti.geodesic_sphere(8),
+                                      lambda: ti.satellite(4, 0.125), lambda: ti.cylinder(0.5, 2.0, 256, 3),
+                                      lambda: ti.large_body(5, 24)])
+def test_lbvh_topology_and_boxes(T, mesh_fn):
+    m = mesh_fn()
+    gm = T.Mesh(m.vertices, m.indices, m.flags)
+    nodes, leaf = gm.copy_bvh()
+    nt = m.nt
+    assert sorted(leaf.tolist()) == list(range(nt))                     # every facet in exactly one slot
+    kids = nodes[:, 12:14].copy().view(np.int32)
+    n_int = max(nt - 1, 1)
+    assert nodes.shape[0] == n_int
+    tri = m.vertices[m.indices[leaf]]                                   # [slot,3,3] fp32
+    tlo, thi = tri.min(1), tri.max(1)
+    seen_leaf = np.zeros(nt, int)
+    seen_node = np.zeros(n_int, int)
+    seen_node[0] = 1
+
+    def child_box(i, k):
+        b = nodes[i, 6 * k:6 * k + 6]
+        return b[:3], b[3:]
+
+    # bottom-up exact boxes
+    order, stack = [], [0]
+    while stack:
+        i = stack.pop()
+        order.append(i)
+        for k in range(2):
+            c = kids[i, k]
+            if c >= 0:
+                seen_node[c] += 1
+                stack.append(c)
+            elif nt > 1 or k == 0:
+                seen_leaf[~c] += 1
+    assert np.all(seen_leaf == 1) and np.all(seen_node == 1)           # a tree: each leaf/node reached once
+    lo = np.zeros((n_int, 3), np.float32)
+    hi = np.zeros((n_int, 3), np.float32)
+    for i in reversed(order):
+        l, h = [], []
+        for k in range(2):
+            c = kids[i, k]
+            if nt == 1 and k == 1:
+                continue
+            bl, bh = (lo[c], hi[c]) if c >= 0 else (tlo[~c], thi[~c])
+            cl, ch = child_box(i, k)
+            assert np.array_equal(cl, bl) and np.array_equal(ch, bh)   # stored child box = exact fp32 bounds
+            l.append(bl); h.append(bh)
+        lo[i], hi[i] = np.min(l, 0), np.max(h, 0)
+    info = gm.info()
+    assert np.array_equal(lo[0], info["aabb_lo"].astype(np.float32)) or nt == 1
+    assert info["build_ms"] > 0
+
+
+def test_mesh_create_from_device_tensors_and_errors(T):
+    import torch
+    m = ti.geodesic_sphere(4)
+    a = T.Mesh(m.vertices, m.indices, m.flags)
+    b = T.Mesh(torch.tensor(m.vertices).cuda(), torch.tensor(m.indices).cuda(), torch.tensor(m.flags).cuda())
+    na, la = a.copy_bvh()
+    nb, lb = b.copy_bvh()
+    assert np.array_equal(na.view(np.int32), nb.view(np.int32)) and np.array_equal(la, lb)
+    bad = m.indices.copy()
+    bad[3, 1] = m.nv + 5
+    with pytest.raises(T.TpmcError):
+        T.Mesh(m.vertices, bad)
+    with pytest.raises(T.TpmcError):
+        T.Mesh(m.vertices * np.float32("nan"), m.indices)
+    cfg = ti.RunConfig("bad", None)
+    for kw in (dict(T_inf=-1.0), dict(accommodation=1.5), dict(cv_radius_factor=0.5), dict(max_bounces=0),
+               dict(x=(0.5,)), dict(N=10, seed=1)):
+        c = cfg.with_(**kw)
+        if "N" in kw:
+            with pytest.raises(T.TpmcError):
+                a.run(c, first=5, count=6)
+        else:
+            with pytest.raises(T.TpmcError):
+                a.run(c)
+
+
+# ------------------------------------------------------------------ a3: closest hit, bit-exact
+def crafted_rays(m, om, rng, n_random=400):
+    V = m.vertices.astype(np.float64)
+    tri = m.triangles()
+    ctr, Rb = om.bounds()
+    tg = np.concatenate([V[:300], 0.5 * (tri[:300, 0] + tri[:300, 1]), 0.5 * (tri[:300, 1] + tri[:300, 2]),
+                         tri[:300].mean(1), ctr + rng.normal(size=(n_random, 3)) * Rb * 0.6])
+    dirs = rng.normal(size=tg.shape)
+    dirs /= np.linalg.norm(dirs, axis=1, keepdims=True)
+    o = (ctr + 2.5 * Rb * dirs).astype(np.float32)
+    d = (tg - o.astype(np.float64)).astype(np.float32)
+    # axis-parallel rays: zero direction components
+    cen = tri.mean(1)[:60]
+    for ax in range(3):
+        oo = cen.copy(); oo[:, ax] += 3 * Rb
+        dd = np.zeros_like(cen); dd[:, ax] = -1.0
+        o = np.concatenate([o, oo.astype(np.float32)]); d = np.concatenate([d, dd.astype(np.float32)])
+    # rays starting ON the surface (secondary-ray situation), leaving and grazing
+    st = tri.mean(1)[:200]
+    dd = rng.normal(size=st.shape)
+    o = np.concatenate([o, st.astype(np.float32)]); d = np.concatenate([d, dd.astype(np.float32)])
+    fprev = np.full(o.shape[0], -1, np.int32)
+    fprev[-200:] = np.arange(min(200, st.shape[0]))
+    return o, d, fprev
+
+
+@pytest.mark.parametrize("mesh_fn,bvh", [(lambda: ti.plate(30.0), False), (lambda: ti.box(h=0.5), False),
+                                          (lambda: ti.random_blob(1, 3), False), (lambda: ti.satellite(4, 0.125), True),
+                                          (lambda: ti.geodesic_sphere(32), True), (lambda: ti.large_body(5, 40), True)])
+def test_trace_parity_bit_exact(T, O, mesh_fn, bvh):
+    m = mesh_fn()
+    gm = T.Mesh(m.vertices, m.indices, m.flags)
+    om = O.OracleMesh(m.vertices, m.indices, m.flags)
+    o, d, fprev = crafted_rays(m, om, np.random.default_rng(5))
+    facet, tau = gm.trace(o, d, fprev)
+    facet, tau = facet.cpu().numpy(), tau.cpu().numpy()
+    nh = 0
+    for r in range(o.shape[0]):
+        fo, to = om.closest_hit(o[r], d[r], int(fprev[r]), use_bvh=bvh)
+        assert facet[r] == fo, (r, facet[r], fo)
+        if fo >= 0:
+            assert tau[r] == to                                           # same fp64 operations, same bits
+            nh += 1
+        else:
+            assert np.isinf(tau[r])
+    assert nh > 100
+
+
+def test_trace_tie_and_sidedness_rules(T):
+    pl = ti.plate(0.0)
+    gm = T.Mesh(pl.vertices, pl.indices, pl.flags)
+    o = np.float32([[2, 0, 0], [2, 0, 0], [-2, 0.1, 0.2]])
+    d = np.float32([[-1, 0, 0], [-1, 0, 0], [1, 0, 0]])
+    f, tau = gm.trace(o, d, np.int32([-1, 0, -1]))
+    f = f.cpu().numpy()
+    assert f[0] == 0 and f[1] == 1 and f[2] >= 0           # A12 tie -> smallest index; A11 source excluded; two-sided
+    bx = ti.box(h=1.0)
+    gb = T.Mesh(bx.vertices, bx.indices, bx.flags)
+    f, _ = gb.trace(np.float32([[0, 0, 0]]), np.float32([[1, 0.1, 0.2]]))
+    assert f.cpu().numpy()[0] == -1                         # one-sided facets are invisible from behind
+    one = T.Mesh(np.float32([[0, 0, 0], [1, 0, 0], [0, 1, 0]]), np.int32([[0, 1, 2]]))   # single-triangle mesh
+    f, tau = one.trace(np.float32([[0.2, 0.2, 1], [0.2, 0.2, -1], [2, 2, 1]]), np.float32([[0, 0, -1], [0, 0, 1], [0, 0, -1]]))
+    assert f.cpu().numpy().tolist() == [0, -1, -1] and tau.cpu().numpy()[0] == 1.0
+
+
+# ------------------------------------------------------------------ whole path on the five configs
+def test_run_parity_c1_plate_all_particles(T, O):
+    cfg = ti.config("C1")[0]
+    g, o, frac = compare_run(T, O, cfg, 0, cfg.N, use_bvh=False)
+    assert frac == 1.0
+    # and the physics: C_D within 4 sigma of the (corrected) Sentman value
+    F = g.force.cpu().numpy() / cfg.q_inf
+    se = o.force_stderr(cfg.N) / cfg.q_inf
+    assert abs(-F[0] - 1.847023) < 4 * se[0] and abs(-F[1] - 0.066379) < 4 * se[1]
+
+
+@pytest.mark.parametrize("idx", [0, 1, 2])
+def test_run_parity_c2_sphere(T, O, idx):
+    cfg = ti.config("C2")[idx]
+    compare_run(T, O, cfg, 1_000_000 * idx, 150_000)
+
+
+@pytest.mark.parametrize("idx", [0, 1, 2])
+def test_run_parity_c3_cylinder_maxwell(T, O, idx):
+    cfg = ti.config("C3")[idx]
+    g, o, _ = compare_run(T, O, cfg, 50_000_000, 150_000)
+    if idx == 0:                                             # config 3's invariant: zero lateral force at 0 deg
+        se = o.force_stderr(150_000)
+        F = g.force.cpu().numpy()
+        assert abs(F[0]) < 4 * se[0] and abs(F[1]) < 4 * se[1]
+
+
+@pytest.mark.parametrize("idx", [0, 5, 10, 15])
+def test_run_parity_c4_satellite_multiple_reflections(T, O, idx):
+    cfg = ti.config("C4")[idx]
+    g, o, _ = compare_run(T, O, cfg, 10_000_000 * idx, 200_000)
+    assert int(o.bounces.max()) >= 3 and o.truncated == 0
+
+
+@pytest.mark.parametrize("idx,first,count", [(0, 0, 200_000), (21, 500_000_000, 100_000), (63, 999_900_000, 100_000)])
+def test_run_parity_c5_large_body_full_size_stream(T, O, idx, first, count):
+    """Slices of the N = 1e9 stream on the ~1.0e6-facet body, in the configuration bench.py times."""
+    cfg = ti.config("C5")[idx]
+    g, o, _ = compare_run(T, O, cfg, first, count)
+    assert g.stats["truncated"] == 0
+
+
+def test_slices_are_additive_and_runs_repeat(T, O):
+    cfg = ti.config("C4")[3].with_(N=400_000)
+    gm, _ = meshes(T, O, cfg)
+    full = gm.run(cfg)
+    a = gm.run(cfg, first=0, count=150_000)
+    b = gm.run(cfg, first=150_000, count=250_000)
+    F = full.force.cpu().numpy()
+    assert np.allclose(a.force.cpu().numpy() + b.force.cpu().numpy(), F, rtol=1e-11)
+    assert np.allclose((a.facet_momentum + b.facet_momentum).cpu().numpy(), full.facet_momentum.cpu().numpy(), rtol=1e-9, atol=1e-25)
+    assert a.stats["hits"] + b.stats["hits"] == full.stats["hits"]
+    again = gm.run(cfg, debug=True)
+    assert np.allclose(again.force.cpu().numpy(), F, rtol=1e-12)        # fp64 atomic order only (A20)
+    # wave boundaries do not matter: a run spanning several waves equals its one-wave slices
+    assert full.stats["segments"] == cfg.N + full.stats["hits"] - full.stats["truncated"]
+
+
+def test_edge_cases_empty_truncated_host_buffers(T, O):
+    cfg = ti.config("C4")[0].with_(N=100_000)
+    gm, om = meshes(T, O, cfg)
+    z = gm.run(cfg, first=10, count=0, debug=True)
+    assert np.all(z.force.cpu().numpy() == 0) and z.stats["hits"] == 0 and z.stats["segments"] == 0
+    # bounce cap: particles cut off are counted, and both sides agree on them
+    c1 = cfg.with_(max_bounces=1)
+    g = gm.run(c1, debug=True)
+    o = om.run(c1)
+    assert g.stats["truncated"] == o.truncated > 0 and g.stats["hits"] == o.hits and g.stats["segments"] == o.segments
+    assert np.array_equal(g.hash.cpu().numpy().view(np.uint64), o.hash)
+    # host-buffer entry point gives the same numbers as the device one
+    d = gm.run(cfg)
+    F, Tq, fm, st = gm.run_host(cfg)
+    assert np.allclose(F, d.force.cpu().numpy(), rtol=1e-12) and np.allclose(Tq, d.torque.cpu().numpy(), rtol=1e-10, atol=1e-30)
+    assert np.allclose(fm, d.facet_momentum.cpu().numpy(), rtol=1e-9, atol=1e-25) and st["hits"] == d.stats["hits"]
+    # no per-facet buffer requested
+    nf = gm.run(cfg, facets=False)
+    assert np.allclose(nf.force.cpu().numpy(), d.force.cpu().numpy(), rtol=1e-12)
+
+
+def test_specular_and_mixture_parity(T, O):
+    cfg = ti.config("C3")[1].with_(accommodation=0.0, N=1_000_000)
+    compare_run(T, O, cfg, 0, 100_000)
+    mix = ti.config("C5")[9].with_(mesh_fn=lambda: ti.large_body(5, 24), N=1_000_000)
+    mix._mesh_cache = []
+    compare_run(T, O, mix, 300_000, 100_000)
+
+
+def test_run_on_side_stream(T, O):
+    import torch
+    cfg = ti.config("C2")[1].with_(N=200_000)
+    gm, _ = meshes(T, O, cfg)
+    ref = gm.run(cfg).force.cpu().numpy()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        r = gm.run(cfg, stream=s)
+    s.synchronize()
+    assert np.allclose(r.force.cpu().numpy(), ref, rtol=1e-12)
