@@ -76,8 +76,12 @@ typedef struct {
   uint64_t kernel_launches;/* kernels this run enqueued */
   double ms;               /* device time of this run, CUDA events on the caller's stream */
   double ms_seed;          /* summed device time of the seed-kernel launches (events around each launch) */
-  double ms_trace;         /* summed device time of the trace/reflect-kernel launches */
-  uint64_t timed_waves;    /* waves covered by ms_seed / ms_trace (all of them unless > 2048) */
+  double ms_trace;         /* ... of the wavefront traversal kernel launches */
+  double ms_reflect;       /* ... of the resolve/reflect/accumulate kernel launches */
+  double ms_finish;        /* ... of the straggler kernel launches */
+  uint64_t timed_waves;    /* waves covered by the per-kernel times (all of them unless > 512) */
+  uint64_t trace_launches; /* traversal-kernel launches covered by ms_trace */
+  uint64_t traced_rays;    /* rays those launches processed */
 } tpmc_stats;
 
 /* Optional per-particle outputs for parity checks; each pointer is device [count] or NULL. */

@@ -47,7 +47,8 @@ class tpmc_stats(C.Structure):
     _fields_ = [("hits", C.c_uint64), ("segments", C.c_uint64), ("escaped", C.c_uint64), ("truncated", C.c_uint64),
                 ("culled", C.c_uint64), ("tri_tests", C.c_uint64), ("node_visits", C.c_uint64),
                 ("kernel_launches", C.c_uint64), ("ms", C.c_double), ("ms_seed", C.c_double), ("ms_trace", C.c_double),
-                ("timed_waves", C.c_uint64)]
+                ("ms_reflect", C.c_double), ("ms_finish", C.c_double), ("timed_waves", C.c_uint64),
+                ("trace_launches", C.c_uint64), ("traced_rays", C.c_uint64)]
 
 
 class tpmc_debug(C.Structure):

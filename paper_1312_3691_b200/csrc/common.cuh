@@ -40,20 +40,28 @@ struct tpmc_mesh {
   int device;
   // per-run scratch, cached in the handle (one run at a time per handle)
   size_t wave_cap;
-  float4* ray_o;
-  float4* ray_v;
-  unsigned int* queue_count;       // [4] device counters
+  float4* q_o[2];                  // ray queues A/B (ping-pong between wavefront rounds)
+  float4* q_v[2];
+  int* q_f[2];
+  unsigned int* hit_ray;           // [wave_cap] ray index of every ray that ended with candidate facets
+  int4* hit_cand;                  // [wave_cap] its candidate slots
+  unsigned int* ctr;               // [kCtrWords] per-wave device counters (queue sizes, fetch heads, hit counts)
   double* facet_scratch;           // [nt][3] when the caller passes no per-facet buffer
   double* partials;                // reduction partials
   unsigned long long* stats;       // [8] device counters
   double* totals;                  // [3] torque accumulators
   cudaEvent_t ev0, ev1;
-  cudaEvent_t* wave_ev;            // [2*kMaxTimedWaves+1] per-kernel timing, created on first use
+  cudaEvent_t* wave_ev;            // [kEvPerWave*kMaxTimedWaves] per-kernel timing, created on first use
   unsigned long long last_launches;
   unsigned long long last_timed_waves;
 };
 
-constexpr int kMaxTimedWaves = 2048;
+constexpr int kMaxTimedWaves = 512;
+constexpr int kRounds = 3;                       // wavefront rounds before the straggler kernel
+constexpr int kEvPerWave = 2 + 2 * kRounds + 1;  // start, seed, (trace, reflect) x rounds, finish
+constexpr int kCtrWords = 32;
+// ctr layout: [0..kRounds] queue sizes, [8..] fetch heads of the trace rounds, [16..] hit counts
+constexpr int kCtrQueue = 0, kCtrFetch = 8, kCtrHits = 16;
 
 // Per-run constants (a1: host, fp64), passed to kernels by value.
 struct SpeciesConst {

@@ -308,10 +308,11 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
 extern "C" void tpmc_mesh_destroy(tpmc_mesh* m) {
   if (!m) return;
   cudaFree(m->nodes); cudaFree(m->tris);
-  cudaFree(m->ray_o); cudaFree(m->ray_v); cudaFree(m->queue_count);
+  for (int k = 0; k < 2; ++k) { cudaFree(m->q_o[k]); cudaFree(m->q_v[k]); cudaFree(m->q_f[k]); }
+  cudaFree(m->hit_ray); cudaFree(m->hit_cand); cudaFree(m->ctr);
   cudaFree(m->facet_scratch); cudaFree(m->partials); cudaFree(m->stats); cudaFree(m->totals);
   if (m->wave_ev) {
-    for (int i = 0; i < 2 * kMaxTimedWaves + 1; ++i) cudaEventDestroy(m->wave_ev[i]);
+    for (int i = 0; i < kEvPerWave * kMaxTimedWaves; ++i) cudaEventDestroy(m->wave_ev[i]);
     delete[] m->wave_ev;
   }
   if (m->ev0) cudaEventDestroy(m->ev0);

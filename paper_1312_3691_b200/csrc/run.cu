@@ -15,7 +15,7 @@ constexpr int kTraceBlock = 128;
 constexpr int kReduceBlock = 256;
 constexpr int kReduceParts = 296;   // 2 per SM
 
-enum { ST_HITS = 0, ST_TRUNC = 1, ST_CULLED = 2, ST_TRIS = 3, ST_NODES = 4, ST_COUNT = 8 };
+enum { ST_HITS = 0, ST_TRUNC = 1, ST_CULLED = 2, ST_TRIS = 3, ST_NODES = 4, ST_TRACED = 5, ST_COUNT = 8 };
 
 __device__ __forceinline__ unsigned lanemask_lt() {
   unsigned m;
@@ -65,79 +65,104 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
   if (keep) {
     const unsigned slot = base + __popc(m & lanemask_lt());
     ray_o[slot] = make_float4(o[0], o[1], o[2], __uint_as_float(j));
-    ray_v[slot] = make_float4(v[0], v[1], v[2], __int_as_float(species));
+    ray_v[slot] = make_float4(v[0], v[1], v[2], __uint_as_float((unsigned int)species));   // bounce 0
   }
 }
 
-// a3-a6: every queued particle is followed to escape: closest hit -> surface interaction ->
-// per-facet momentum (fp64 atomics) -> next segment.
-__global__ void __launch_bounds__(kTraceBlock) k_trace(const RunConst rc, unsigned long long wave_first,
-                                                       const float4* __restrict__ nodes,
-                                                       const float4* __restrict__ tris,
-                                                       const float4* __restrict__ ray_o,
-                                                       const float4* __restrict__ ray_v,
-                                                       const unsigned int* __restrict__ qcount,
-                                                       double* __restrict__ P, double* __restrict__ torque,
-                                                       unsigned long long* __restrict__ stats, tpmc_debug dbg) {
+// Ray queue record: o.xyz | particle index within the wave, v.xyz | (species | bounce << 4), source facet.
+struct RayQueue {
+  float4* o;
+  float4* v;
+  int* f;      // may be null for primary rays (f_prev = -1)
+};
+
+// a3: wavefront traversal.  Persistent warps; a lane whose ray has finished takes the next ray of the
+// queue (warp-aggregated fetch) as soon as fewer than kRefill lanes are busy, so rays of very different
+// length (misses vs. hits) do not idle the warp.  fp32 only: see trace.cuh.  Rays that end with at least
+// one candidate facet are appended to the hit list for the resolve/reflect kernel.
+constexpr int kRefill = 20;
+
+__global__ void __launch_bounds__(kTraceBlock, 8) k_trace_wf(const float4* __restrict__ nodes,
+                                                             const float4* __restrict__ tris, const RayQueue q,
+                                                             const unsigned int* __restrict__ n_rays,
+                                                             unsigned int* __restrict__ next_ray,
+                                                             unsigned int* __restrict__ hit_ray,
+                                                             int4* __restrict__ hit_cand,
+                                                             unsigned int* __restrict__ n_hits,
+                                                             unsigned long long* __restrict__ stats) {
   __shared__ int sstack[TPMC_STACK_SMEM * kTraceBlock];
-  __shared__ double sred[3][kTraceBlock / 32];
-  __shared__ unsigned long long scnt[4][kTraceBlock / 32];
-  const unsigned int n = *qcount;
-  double tq[3] = {0.0, 0.0, 0.0};
-  unsigned long long hits = 0, trunc = 0;
+  int* stk = sstack + threadIdx.x;
+  int lstack[TPMC_STACK_LOCAL];
+  const unsigned int n = *n_rays;
+  const int lane = threadIdx.x & 31;
+  const unsigned FULL = 0xFFFFFFFFu;
+  bool has = false, exhausted = false;
+  unsigned int r = 0;
+  Walk w;
+  w.cur = TPMC_SENTINEL; w.sp = 0; w.nc = 0; w.tmax = 0.0f; w.f_prev = -1;
   TraceCounters cnt;
   cnt.nodes = 0; cnt.tris = 0;
-  unsigned long long nodes_tot = 0, tris_tot = 0;
-  for (unsigned int r = blockIdx.x * blockDim.x + threadIdx.x; r < n; r += gridDim.x * blockDim.x) {
-    const float4 ro = ray_o[r], rv = ray_v[r];
-    float o[3] = {ro.x, ro.y, ro.z}, v[3] = {rv.x, rv.y, rv.z};
-    const unsigned long long j = wave_first + __float_as_uint(ro.w);
-    const unsigned long long i = rc.first + j;
-    const int species = __float_as_int(rv.w);
-    const double w = rc.sp[species].w, cW = rc.sp[species].cW;
-    int f_prev = -1, first = -1;
-    unsigned int k = 0;
-    unsigned long long h = 0xCBF29CE484222325ull;
-    for (;;) {
-      const Hit hit = closest_hit(nodes, tris, o, v, f_prev, sstack + threadIdx.x, kTraceBlock, cnt);
-      if (hit.facet < 0) break;
-      ++hits;
-      if (k == 0) first = hit.facet;
-      h = fnv1a_facet(h, hit.facet);
-      const float4 q0 = __ldg(tris + 3 * (size_t)hit.slot), q1 = __ldg(tris + 3 * (size_t)hit.slot + 1),
-                   q2 = __ldg(tris + 3 * (size_t)hit.slot + 2);
-      double vout[3];
-      reflect(q0, q1, q2, v, rc.sigma, cW, particle_block(rc, i, 2u + k), vout);
-      // O12: dp = w (v_in - v_out) on the fp32 values; hit point o + tau v in fp64
-      double hp[3], dp[3];
-      float vo[3];
-#pragma unroll
-      for (int a = 0; a < 3; ++a) {
-        vo[a] = (float)vout[a];
-        hp[a] = __dadd_rn((double)o[a], __dmul_rn(hit.tau, (double)v[a]));
-        dp[a] = w * ((double)v[a] - (double)vo[a]);
-        atomicAdd(&P[3 * (size_t)hit.facet + a], dp[a]);
+  for (;;) {
+    const unsigned need = __ballot_sync(FULL, !has && !exhausted);
+    if (need) {
+      const int leader = __ffs(need) - 1;
+      unsigned base = 0;
+      if (lane == leader) base = atomicAdd(next_ray, (unsigned)__popc(need));
+      base = __shfl_sync(FULL, base, leader);
+      if (!has && !exhausted) {
+        r = base + __popc(need & lanemask_lt());
+        if (r < n) {
+          walk_init(w, q.o[r], q.v[r], q.f ? q.f[r] : -1);
+          has = true;
+        } else {
+          exhausted = true;
+        }
       }
-      const double rx = hp[0] - rc.x_ref[0], ry = hp[1] - rc.x_ref[1], rz = hp[2] - rc.x_ref[2];
-      tq[0] += ry * dp[2] - rz * dp[1];
-      tq[1] += rz * dp[0] - rx * dp[2];
-      tq[2] += rx * dp[1] - ry * dp[0];
-      // O13: next segment starts at the fp32-rounded hit point
-#pragma unroll
-      for (int a = 0; a < 3; ++a) { o[a] = (float)hp[a]; v[a] = vo[a]; }
-      f_prev = hit.facet;
-      ++k;
-      if (k >= rc.max_bounces) { ++trunc; break; }
     }
-    if (dbg.hash) dbg.hash[j] = h;
-    if (dbg.bounces) dbg.bounces[j] = k;
-    if (dbg.first_facet) dbg.first_facet[j] = first;
-    nodes_tot += cnt.nodes; tris_tot += cnt.tris;
-    cnt.nodes = 0; cnt.tris = 0;
+    if (__ballot_sync(FULL, has) == 0u) break;
+    const int thresh = __any_sync(FULL, exhausted) ? 1 : kRefill;
+    unsigned busy;
+    do {
+      bool fin = false;
+      if (has) {
+        walk_step(w, nodes, tris, stk, kTraceBlock, lstack, cnt);
+        if (w.cur == TPMC_SENTINEL) { has = false; fin = w.nc > 0; }
+      }
+      const unsigned fm = __ballot_sync(FULL, fin);
+      if (fm) {   // append finished rays that have candidates to the hit list
+        const int leader = __ffs(fm) - 1;
+        unsigned base = 0;
+        if (lane == leader) base = atomicAdd(n_hits, (unsigned)__popc(fm));
+        base = __shfl_sync(FULL, base, leader);
+        if (fin) {
+          const unsigned h = base + __popc(fm & lanemask_lt());
+          hit_ray[h] = r;
+          hit_cand[h] = (w.nc > TPMC_MAX_CAND) ? make_int4(-1, -1, -1, TPMC_CAND_OVERFLOW)
+                                               : make_int4(w.cs[0], w.cs[1], w.cs[2], w.cs[3]);
+        }
+      }
+      busy = __ballot_sync(FULL, has);
+    } while (__popc(busy) >= thresh);
   }
-  // block reduction of the torque and the counters, one atomic per block and quantity
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  unsigned long long c4[4] = {hits, trunc, tris_tot, nodes_tot};
+  // counters: one atomic per warp
+  unsigned long long cn = cnt.nodes, ct = cnt.tris;
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    cn += __shfl_down_sync(FULL, cn, off);
+    ct += __shfl_down_sync(FULL, ct, off);
+  }
+  if (lane == 0) {
+    if (cn) atomicAdd(&stats[ST_NODES], cn);
+    if (ct) atomicAdd(&stats[ST_TRIS], ct);
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0 && n) atomicAdd(&stats[ST_TRACED], (unsigned long long)n);
+}
+
+// Block-level sum of per-thread torque and counters, one atomic per block and quantity.
+__device__ __forceinline__ void block_flush(double tq[3], unsigned long long c4[4], double* __restrict__ torque,
+                                            unsigned long long* __restrict__ stats, double (*sred)[8],
+                                            unsigned long long (*scnt)[8]) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) {
 #pragma unroll
@@ -153,7 +178,7 @@ __global__ void __launch_bounds__(kTraceBlock) k_trace(const RunConst rc, unsign
   if (threadIdx.x == 0) {
     double t3[3] = {0, 0, 0};
     unsigned long long s4[4] = {0, 0, 0, 0};
-    for (int wv = 0; wv < kTraceBlock / 32; ++wv) {
+    for (int wv = 0; wv < nw; ++wv) {
       for (int a = 0; a < 3; ++a) t3[a] += sred[a][wv];
       for (int a = 0; a < 4; ++a) s4[a] += scnt[a][wv];
     }
@@ -163,6 +188,154 @@ __global__ void __launch_bounds__(kTraceBlock) k_trace(const RunConst rc, unsign
     if (s4[2]) atomicAdd(&stats[ST_TRIS], s4[2]);
     if (s4[3]) atomicAdd(&stats[ST_NODES], s4[3]);
   }
+}
+
+// One surface interaction (O11-O13) of a particle whose closest hit is known: momentum and torque
+// accumulation, debug records, and the state of the next segment.  Returns false when the particle stops
+// here (bounce cap).
+struct Particle {
+  float o[3], v[3];
+  unsigned long long j;   // index within the slice
+  int species;
+  unsigned int k;         // reflections so far
+  int f_prev;
+};
+
+__device__ __forceinline__ bool interact(const RunConst& rc, const float4* __restrict__ tris, Particle& p, const Hit& hit,
+                                         double* __restrict__ P, double tq[3], const tpmc_debug& dbg,
+                                         unsigned long long& trunc) {
+  const float4 q0 = __ldg(tris + 3 * (size_t)hit.slot), q1 = __ldg(tris + 3 * (size_t)hit.slot + 1),
+               q2 = __ldg(tris + 3 * (size_t)hit.slot + 2);
+  const double w = rc.sp[p.species].w, cW = rc.sp[p.species].cW;
+  double vout[3];
+  reflect(q0, q1, q2, p.v, rc.sigma, cW, particle_block(rc, rc.first + p.j, 2u + p.k), vout);
+  // O12: dp = w (v_in - v_out) on the fp32 values; hit point o + tau v in fp64
+  double hp[3], dp[3];
+  float vo[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    vo[a] = (float)vout[a];
+    hp[a] = __dadd_rn((double)p.o[a], __dmul_rn(hit.tau, (double)p.v[a]));
+    dp[a] = w * ((double)p.v[a] - (double)vo[a]);
+    atomicAdd(&P[3 * (size_t)hit.facet + a], dp[a]);
+  }
+  const double rx = hp[0] - rc.x_ref[0], ry = hp[1] - rc.x_ref[1], rz = hp[2] - rc.x_ref[2];
+  tq[0] += ry * dp[2] - rz * dp[1];
+  tq[1] += rz * dp[0] - rx * dp[2];
+  tq[2] += rx * dp[1] - ry * dp[0];
+  if (dbg.hash) dbg.hash[p.j] = fnv1a_facet(dbg.hash[p.j], hit.facet);
+  if (dbg.bounces) dbg.bounces[p.j] = p.k + 1u;
+  if (dbg.first_facet && p.k == 0u) dbg.first_facet[p.j] = hit.facet;
+  // O13: next segment starts at the fp32-rounded hit point
+#pragma unroll
+  for (int a = 0; a < 3; ++a) { p.o[a] = (float)hp[a]; p.v[a] = vo[a]; }
+  p.f_prev = hit.facet;
+  ++p.k;
+  if (p.k >= rc.max_bounces) { ++trunc; return false; }
+  return true;
+}
+
+// a4-a6: resolve the candidates of every hit ray with the exact fp64 test, apply the surface interaction,
+// accumulate, and queue the reflected ray for the next wavefront round (compacted, warp-aggregated).
+__global__ void __launch_bounds__(kTraceBlock) k_reflect(const RunConst rc, unsigned long long wave_first,
+                                                         const float4* __restrict__ nodes,
+                                                         const float4* __restrict__ tris, const RayQueue qin,
+                                                         const unsigned int* __restrict__ hit_ray,
+                                                         const int4* __restrict__ hit_cand,
+                                                         const unsigned int* __restrict__ n_hits, const RayQueue qout,
+                                                         unsigned int* __restrict__ n_out, double* __restrict__ P,
+                                                         double* __restrict__ torque,
+                                                         unsigned long long* __restrict__ stats, tpmc_debug dbg) {
+  __shared__ double sred[3][8];
+  __shared__ unsigned long long scnt[4][8];
+  const unsigned int n = *n_hits;
+  const int lane = threadIdx.x & 31;
+  double tq[3] = {0.0, 0.0, 0.0};
+  unsigned long long hits = 0, trunc = 0;
+  unsigned int ntests = 0;
+  TraceCounters cnt;
+  cnt.nodes = 0; cnt.tris = 0;
+  const unsigned int stride = gridDim.x * blockDim.x;
+  const unsigned int nround = ((n + stride - 1) / stride) * stride;   // keep warps converged for the ballots
+  for (unsigned int h = blockIdx.x * blockDim.x + threadIdx.x; h < nround; h += stride) {
+    bool emit = false;
+    Particle p;
+    if (h < n) {
+      const unsigned int r = hit_ray[h];
+      const int4 cand = hit_cand[h];
+      const float4 ro = qin.o[r], rv = qin.v[r];
+      p.o[0] = ro.x; p.o[1] = ro.y; p.o[2] = ro.z;
+      p.v[0] = rv.x; p.v[1] = rv.y; p.v[2] = rv.z;
+      p.j = wave_first + __float_as_uint(ro.w);
+      const unsigned int pk = __float_as_uint(rv.w);
+      p.species = (int)(pk & 15u);
+      p.k = pk >> 4;
+      p.f_prev = qin.f ? qin.f[r] : -1;
+      Hit hit;
+      if (cand.w == TPMC_CAND_OVERFLOW) {
+        int tmp[TPMC_STACK_SMEM];
+        hit = closest_hit(nodes, tris, p.o, p.v, p.f_prev, tmp, 1, cnt);
+      } else {
+        hit = resolve_candidates(tris, cand, p.o, p.v, ntests);
+      }
+      if (hit.facet >= 0) {
+        ++hits;
+        emit = interact(rc, tris, p, hit, P, tq, dbg, trunc);
+      }
+    }
+    const unsigned em = __ballot_sync(0xFFFFFFFFu, emit);
+    if (em) {
+      const int leader = __ffs(em) - 1;
+      unsigned base = 0;
+      if (lane == leader) base = atomicAdd(n_out, (unsigned)__popc(em));
+      base = __shfl_sync(0xFFFFFFFFu, base, leader);
+      if (emit) {
+        const unsigned s = base + __popc(em & lanemask_lt());
+        qout.o[s] = make_float4(p.o[0], p.o[1], p.o[2], __uint_as_float((unsigned int)(p.j - wave_first)));
+        qout.v[s] = make_float4(p.v[0], p.v[1], p.v[2], __uint_as_float((unsigned int)p.species | (p.k << 4)));
+        qout.f[s] = p.f_prev;
+      }
+    }
+  }
+  unsigned long long c4[4] = {hits, trunc, (unsigned long long)ntests + cnt.tris, (unsigned long long)cnt.nodes};
+  block_flush(tq, c4, torque, stats, sred, scnt);
+}
+
+// Stragglers after the wavefront rounds: each remaining particle is followed to escape in one thread
+// (full fp64 traversal per segment).  Few particles get here; long multi-bounce paths live here.
+__global__ void __launch_bounds__(kTraceBlock) k_finish(const RunConst rc, unsigned long long wave_first,
+                                                        const float4* __restrict__ nodes,
+                                                        const float4* __restrict__ tris, const RayQueue q,
+                                                        const unsigned int* __restrict__ n_rays,
+                                                        double* __restrict__ P, double* __restrict__ torque,
+                                                        unsigned long long* __restrict__ stats, tpmc_debug dbg) {
+  __shared__ int sstack[TPMC_STACK_SMEM * kTraceBlock];
+  __shared__ double sred[3][8];
+  __shared__ unsigned long long scnt[4][8];
+  const unsigned int n = *n_rays;
+  double tq[3] = {0.0, 0.0, 0.0};
+  unsigned long long hits = 0, trunc = 0;
+  TraceCounters cnt;
+  cnt.nodes = 0; cnt.tris = 0;
+  for (unsigned int r = blockIdx.x * blockDim.x + threadIdx.x; r < n; r += gridDim.x * blockDim.x) {
+    const float4 ro = q.o[r], rv = q.v[r];
+    Particle p;
+    p.o[0] = ro.x; p.o[1] = ro.y; p.o[2] = ro.z;
+    p.v[0] = rv.x; p.v[1] = rv.y; p.v[2] = rv.z;
+    p.j = wave_first + __float_as_uint(ro.w);
+    const unsigned int pk = __float_as_uint(rv.w);
+    p.species = (int)(pk & 15u);
+    p.k = pk >> 4;
+    p.f_prev = q.f ? q.f[r] : -1;
+    for (;;) {
+      const Hit hit = closest_hit(nodes, tris, p.o, p.v, p.f_prev, sstack + threadIdx.x, kTraceBlock, cnt);
+      if (hit.facet < 0) break;
+      ++hits;
+      if (!interact(rc, tris, p, hit, P, tq, dbg, trunc)) break;
+    }
+  }
+  unsigned long long c4[4] = {hits, trunc, (unsigned long long)cnt.tris, (unsigned long long)cnt.nodes};
+  block_flush(tq, c4, torque, stats, sred, scnt);
 }
 
 // a7: F = sum_f P_f by a fixed-shape tree (deterministic for given P): parts -> one block.
@@ -205,21 +378,43 @@ __global__ void k_seed_only(const RunConst rc, double* __restrict__ x, double* _
   if (species) species[j] = s.species;
 }
 
-__global__ void __launch_bounds__(kTraceBlock) k_trace_only(const float4* __restrict__ nodes,
-                                                            const float4* __restrict__ tris,
-                                                            const float* __restrict__ o, const float* __restrict__ d,
-                                                            const int32_t* __restrict__ f_prev, long long n,
-                                                            int32_t* __restrict__ facet, double* __restrict__ tau) {
-  __shared__ int sstack[TPMC_STACK_SMEM * kTraceBlock];
-  const long long r = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+// tpmc_trace: user rays -> queue records; candidates -> (facet, tau)
+__global__ void k_pack_rays(const float* __restrict__ o, const float* __restrict__ d, const int32_t* __restrict__ f_prev,
+                            unsigned int n, RayQueue q, int32_t* __restrict__ facet, double* __restrict__ tau) {
+  const unsigned int r = blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= n) return;
-  const float of[3] = {o[3 * r], o[3 * r + 1], o[3 * r + 2]};
-  const float df[3] = {d[3 * r], d[3 * r + 1], d[3 * r + 2]};
+  q.o[r] = make_float4(o[3 * (size_t)r], o[3 * (size_t)r + 1], o[3 * (size_t)r + 2], __uint_as_float(r));
+  q.v[r] = make_float4(d[3 * (size_t)r], d[3 * (size_t)r + 1], d[3 * (size_t)r + 2], 0.0f);
+  q.f[r] = f_prev ? f_prev[r] : -1;
+  facet[r] = -1;
+  tau[r] = INFINITY;
+}
+
+__global__ void __launch_bounds__(kTraceBlock) k_resolve_only(const float4* __restrict__ nodes,
+                                                              const float4* __restrict__ tris, const RayQueue q,
+                                                              const unsigned int* __restrict__ hit_ray,
+                                                              const int4* __restrict__ hit_cand,
+                                                              const unsigned int* __restrict__ n_hits,
+                                                              int32_t* __restrict__ facet, double* __restrict__ tau) {
+  const unsigned int n = *n_hits;
   TraceCounters cnt;
   cnt.nodes = 0; cnt.tris = 0;
-  const Hit h = closest_hit(nodes, tris, of, df, f_prev ? f_prev[r] : -1, sstack + threadIdx.x, kTraceBlock, cnt);
-  facet[r] = h.facet;
-  tau[r] = h.tau;
+  unsigned int nt = 0;
+  for (unsigned int h = blockIdx.x * blockDim.x + threadIdx.x; h < n; h += gridDim.x * blockDim.x) {
+    const unsigned int r = hit_ray[h];
+    const int4 cand = hit_cand[h];
+    const float4 ro = q.o[r], rv = q.v[r];
+    const float of[3] = {ro.x, ro.y, ro.z}, df[3] = {rv.x, rv.y, rv.z};
+    Hit hit;
+    if (cand.w == TPMC_CAND_OVERFLOW) {
+      int tmp[TPMC_STACK_SMEM];
+      hit = closest_hit(nodes, tris, of, df, q.f[r], tmp, 1, cnt);
+    } else {
+      hit = resolve_candidates(tris, cand, of, df, nt);
+    }
+    facet[r] = hit.facet;
+    tau[r] = hit.tau;
+  }
 }
 
 // ---- a1: per-run constants on the host, fp64 -------------------------------------------------------
@@ -311,17 +506,27 @@ size_t wave_size() {
 }
 
 int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
-  if (!m->queue_count) {
-    TPMC_CUDA_TRY(cudaMalloc((void**)&m->queue_count, 4 * sizeof(unsigned int)));
+  if (!m->ctr) {
+    TPMC_CUDA_TRY(cudaMalloc((void**)&m->ctr, kCtrWords * sizeof(unsigned int)));
     TPMC_CUDA_TRY(cudaMalloc((void**)&m->stats, ST_COUNT * sizeof(unsigned long long)));
     TPMC_CUDA_TRY(cudaMalloc((void**)&m->totals, 4 * sizeof(double)));
     TPMC_CUDA_TRY(cudaMalloc((void**)&m->partials, 3 * kReduceParts * sizeof(double)));
   }
   if (m->wave_cap < wave) {
-    cudaFree(m->ray_o); cudaFree(m->ray_v);
-    m->ray_o = m->ray_v = nullptr; m->wave_cap = 0;
-    TPMC_CUDA_TRY(cudaMalloc((void**)&m->ray_o, wave * sizeof(float4)));
-    TPMC_CUDA_TRY(cudaMalloc((void**)&m->ray_v, wave * sizeof(float4)));
+    for (int k = 0; k < 2; ++k) {
+      cudaFree(m->q_o[k]); cudaFree(m->q_v[k]); cudaFree(m->q_f[k]);
+      m->q_o[k] = m->q_v[k] = nullptr; m->q_f[k] = nullptr;
+    }
+    cudaFree(m->hit_ray); cudaFree(m->hit_cand);
+    m->hit_ray = nullptr; m->hit_cand = nullptr;
+    m->wave_cap = 0;
+    for (int k = 0; k < 2; ++k) {
+      TPMC_CUDA_TRY(cudaMalloc((void**)&m->q_o[k], wave * sizeof(float4)));
+      TPMC_CUDA_TRY(cudaMalloc((void**)&m->q_v[k], wave * sizeof(float4)));
+      TPMC_CUDA_TRY(cudaMalloc((void**)&m->q_f[k], wave * sizeof(int)));
+    }
+    TPMC_CUDA_TRY(cudaMalloc((void**)&m->hit_ray, wave * sizeof(unsigned int)));
+    TPMC_CUDA_TRY(cudaMalloc((void**)&m->hit_cand, wave * sizeof(int4)));
     m->wave_cap = wave;
   }
   if (need_facets && !m->facet_scratch)
@@ -329,14 +534,19 @@ int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
   return TPMC_OK;
 }
 
-int trace_grid() {
-  static int g = 0;
-  if (!g) {
-    int dev = 0, sms = 148, per = 8;
+struct Grids { int trace, reflect, finish; };
+const Grids& grids() {
+  static Grids g = {0, 0, 0};
+  if (!g.trace) {
+    int dev = 0, sms = 148, per = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_trace, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
-    g = sms * per;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_trace_wf, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
+    g.trace = sms * per;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_reflect, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
+    g.reflect = sms * per;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_finish, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
+    g.finish = sms * per;
   }
   return g;
 }
@@ -355,14 +565,23 @@ int fill_stats(tpmc_mesh* m, const tpmc_params* params, tpmc_stats* h_stats) {
   h_stats->escaped = params->count - hs[ST_TRUNC];
   h_stats->kernel_launches = m->last_launches;
   h_stats->ms = ms;
-  h_stats->ms_seed = h_stats->ms_trace = 0.0;
+  h_stats->ms_seed = h_stats->ms_trace = h_stats->ms_reflect = h_stats->ms_finish = 0.0;
   h_stats->timed_waves = m->last_timed_waves;
+  h_stats->trace_launches = m->last_timed_waves * kRounds;
+  h_stats->traced_rays = hs[ST_TRACED];
   for (unsigned long long w = 0; w < m->last_timed_waves; ++w) {
-    float a = 0.0f, b = 0.0f;
-    TPMC_CUDA_TRY(cudaEventElapsedTime(&a, m->wave_ev[2 * w], m->wave_ev[2 * w + 1]));
-    TPMC_CUDA_TRY(cudaEventElapsedTime(&b, m->wave_ev[2 * w + 1], m->wave_ev[2 * w + 2]));
-    h_stats->ms_seed += a;
-    h_stats->ms_trace += b;
+    const cudaEvent_t* ev = m->wave_ev + kEvPerWave * w;
+    float t = 0.0f;
+    TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[0], ev[1]));
+    h_stats->ms_seed += t;
+    for (int r = 0; r < kRounds; ++r) {
+      TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[1 + 2 * r], ev[2 + 2 * r]));
+      h_stats->ms_trace += t;
+      TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[2 + 2 * r], ev[3 + 2 * r]));
+      h_stats->ms_reflect += t;
+    }
+    TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[1 + 2 * kRounds], ev[2 + 2 * kRounds]));
+    h_stats->ms_finish += t;
   }
   return TPMC_OK;
 }
@@ -390,26 +609,40 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
   TPMC_CUDA_TRY(cudaMemsetAsync(m->totals, 0, 4 * sizeof(double), st));
   if ((dbg.hash || dbg.bounces || dbg.first_facet) && params->count)
     k_init_debug<<<(unsigned)((params->count + 255) / 256), 256, 0, st>>>(dbg, params->count);
-  const int tgrid = trace_grid();
+  const Grids& g = grids();
   const bool timed = (h_stats != nullptr);   // per-kernel events only when the caller will read them
   if (timed && !m->wave_ev) {
-    m->wave_ev = new (std::nothrow) cudaEvent_t[2 * kMaxTimedWaves + 1];
+    m->wave_ev = new (std::nothrow) cudaEvent_t[kEvPerWave * kMaxTimedWaves];
     if (!m->wave_ev) return TPMC_ENOMEM;
-    for (int i = 0; i < 2 * kMaxTimedWaves + 1; ++i) TPMC_CUDA_TRY(cudaEventCreate(&m->wave_ev[i]));
+    for (int i = 0; i < kEvPerWave * kMaxTimedWaves; ++i) TPMC_CUDA_TRY(cudaEventCreate(&m->wave_ev[i]));
   }
   unsigned long long launches = (dbg.hash || dbg.bounces || dbg.first_facet) && params->count ? 1 : 0, wi = 0;
+  RayQueue Q[2] = {{m->q_o[0], m->q_v[0], m->q_f[0]}, {m->q_o[1], m->q_v[1], m->q_f[1]}};
   for (unsigned long long w0 = 0; w0 < params->count; w0 += wave, ++wi) {
     const unsigned int wn = (unsigned int)std::min<unsigned long long>(wave, params->count - w0);
-    TPMC_CUDA_TRY(cudaMemsetAsync(m->queue_count, 0, sizeof(unsigned int), st));
+    TPMC_CUDA_TRY(cudaMemsetAsync(m->ctr, 0, kCtrWords * sizeof(unsigned int), st));
     const bool tw = timed && wi < (unsigned long long)kMaxTimedWaves;
-    if (tw) TPMC_CUDA_TRY(cudaEventRecord(m->wave_ev[2 * wi], st));
-    k_seed<<<(wn + kSeedBlock - 1) / kSeedBlock, kSeedBlock, 0, st>>>(rc, w0, wn, m->ray_o, m->ray_v, m->queue_count,
+    cudaEvent_t* ev = tw ? m->wave_ev + kEvPerWave * wi : nullptr;
+    int e = 0;
+    if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[e++], st));
+    k_seed<<<(wn + kSeedBlock - 1) / kSeedBlock, kSeedBlock, 0, st>>>(rc, w0, wn, Q[0].o, Q[0].v, m->ctr + kCtrQueue,
                                                                      m->stats);
-    if (tw) TPMC_CUDA_TRY(cudaEventRecord(m->wave_ev[2 * wi + 1], st));
-    k_trace<<<tgrid, kTraceBlock, 0, st>>>(rc, w0, m->nodes, m->tris, m->ray_o, m->ray_v, m->queue_count, P, m->totals,
-                                           m->stats, dbg);
-    if (tw) TPMC_CUDA_TRY(cudaEventRecord(m->wave_ev[2 * wi + 2], st));
-    launches += 2;
+    if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[e++], st));
+    for (int r = 0; r < kRounds; ++r) {
+      RayQueue qin = Q[r & 1], qout = Q[(r + 1) & 1];
+      if (r == 0) qin.f = nullptr;   // primary rays have no source facet
+      k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(m->nodes, m->tris, qin, m->ctr + kCtrQueue + r, m->ctr + kCtrFetch + r,
+                                                  m->hit_ray, m->hit_cand, m->ctr + kCtrHits + r, m->stats);
+      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[e++], st));
+      k_reflect<<<g.reflect, kTraceBlock, 0, st>>>(rc, w0, m->nodes, m->tris, qin, m->hit_ray, m->hit_cand,
+                                                   m->ctr + kCtrHits + r, qout, m->ctr + kCtrQueue + r + 1, P,
+                                                   m->totals, m->stats, dbg);
+      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[e++], st));
+    }
+    k_finish<<<g.finish, kTraceBlock, 0, st>>>(rc, w0, m->nodes, m->tris, Q[kRounds & 1], m->ctr + kCtrQueue + kRounds, P,
+                                               m->totals, m->stats, dbg);
+    if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[e++], st));
+    launches += 2 + 2 * kRounds;
   }
   k_reduce_parts<<<kReduceParts, kReduceBlock, 0, st>>>(P, (long long)m->nt, m->partials);
   k_reduce_final<<<1, 32, 0, st>>>(m->partials, kReduceParts, m->totals, d_force, d_torque);
@@ -473,10 +706,25 @@ extern "C" int tpmc_seed(const tpmc_mesh* mesh, const tpmc_params* params, void*
 
 extern "C" int tpmc_trace(const tpmc_mesh* mesh, const float* d_o, const float* d_d, const int32_t* d_f_prev, int64_t n,
                           void* cuda_stream, int32_t* d_facet, double* d_tau) {
-  if (!mesh || !d_o || !d_d || !d_facet || !d_tau || n < 0) return TPMC_EINVAL;
+  if (!mesh || !d_o || !d_d || !d_facet || !d_tau || n < 0 || n > 0x7FFFFFFF) return TPMC_EINVAL;
   if (n == 0) return TPMC_OK;
-  k_trace_only<<<(unsigned)((n + kTraceBlock - 1) / kTraceBlock), kTraceBlock, 0, (cudaStream_t)cuda_stream>>>(
-      mesh->nodes, mesh->tris, d_o, d_d, d_f_prev, (long long)n, d_facet, d_tau);
+  tpmc_mesh* m = const_cast<tpmc_mesh*>(mesh);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rcode = ensure_scratch(m, std::max<size_t>((size_t)n, m->wave_cap), false);
+  if (rcode != TPMC_OK) return rcode;
+  const Grids& g = grids();
+  RayQueue q = {m->q_o[0], m->q_v[0], m->q_f[0]};
+  const unsigned int un = (unsigned int)n;
+  TPMC_CUDA_TRY(cudaMemsetAsync(m->ctr, 0, kCtrWords * sizeof(unsigned int), st));
+  TPMC_CUDA_TRY(cudaMemcpyAsync(m->ctr + kCtrQueue, &un, sizeof(un), cudaMemcpyHostToDevice, st));
+  TPMC_CUDA_TRY(cudaMemsetAsync(m->stats, 0, ST_COUNT * sizeof(unsigned long long), st));
+  k_pack_rays<<<(un + 255) / 256, 256, 0, st>>>(d_o, d_d, d_f_prev, un, q, d_facet, d_tau);
+  // the production traversal (fp32 wavefront + candidate lists), then the exact fp64 resolve
+  k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(m->nodes, m->tris, q, m->ctr + kCtrQueue, m->ctr + kCtrFetch, m->hit_ray,
+                                              m->hit_cand, m->ctr + kCtrHits, m->stats);
+  k_resolve_only<<<g.reflect, kTraceBlock, 0, st>>>(m->nodes, m->tris, q, m->hit_ray, m->hit_cand, m->ctr + kCtrHits,
+                                                    d_facet, d_tau);
   TPMC_CUDA_TRY(cudaGetLastError());
+  TPMC_CUDA_TRY(cudaStreamSynchronize(st));   // &un must outlive the copy
   return TPMC_OK;
 }

@@ -1,18 +1,30 @@
 // trace.cuh -- steps a3/a4 device code: closest-hit traversal of the LBVH and the surface interaction.
 //
 // Precision contract (reading A9): the mesh and the ray (o, d) are fp32 VALUES; which facet
-// is hit is decided as in exact arithmetic on those values.  The hierarchy is walked with fp32 slab
-// tests made conservative by an explicit rounding-error margin (a box is never wrongly skipped), and
-// every facet whose box the ray touches is decided by the fp64 edge functions below, evaluated with
-// separately rounded multiplies and adds (no FMA contraction): that keeps the shared-edge function of
-// two neighbouring facets exactly antisymmetric, i.e. the test watertight, and equal to DESIGN.md O10.
+// is hit is decided as in exact arithmetic on those values (concretely: by the fp64 edge functions of
+// O10, evaluated with separately rounded multiplies and adds so that the function of a shared edge is
+// exactly antisymmetric for the two facets that share it -- the test is watertight).
+//
+// The wavefront traversal never evaluates fp64.  It walks the hierarchy with fp32 slab tests made
+// conservative by an explicit rounding-error margin, and classifies each facet it reaches with an fp32
+// version of the same edge functions carrying a forward error bound:
+//     MISS       -- some pair of edge functions has provably opposite signs, or the facet is provably
+//                   back-facing / behind the origin: the exact test would reject it too;
+//     HIT        -- all three edge functions provably share a sign (and det, tau are provably admissible):
+//                   the exact test accepts it; its tau lies in [tlo, thi];
+//     UNCERTAIN  -- anything inside the error band.
+// HITs shrink the search interval (tmax = min thi); every HIT or UNCERTAIN facet whose tlo <= tmax stays
+// in a short candidate list.  The resolve step (k_reflect) evaluates the exact fp64 test on the
+// candidates only, and picks the smallest tau, ties to the smallest facet index (A12).
 #pragma once
 
 #include "common.cuh"
 
 #define TPMC_STACK_SMEM 24      // stack entries per thread kept in shared memory
 #define TPMC_STACK_LOCAL 80     // overflow entries (a Karras tree over 64-bit keys + index is <= 97 deep)
-#define TPMC_SENTINEL ((int)0x80000000)
+#define TPMC_SENTINEL ((int)0x7FFFFFFF)
+#define TPMC_MAX_CAND 4
+#define TPMC_CAND_OVERFLOW ((int)0x7FFFFFFE)   // in cand.w: more candidates than slots -> full fp64 traversal
 
 struct Hit {
   double tau;   // +inf: no hit
@@ -40,8 +52,10 @@ __device__ __forceinline__ void cross_nc(const double x[3], const double y[3], d
   z[2] = nc_sub(nc_mul(x[0], y[1]), nc_mul(x[1], y[0]));
 }
 
-__device__ __forceinline__ bool facet_test(const float4 q0, const float4 q1, const float4 q2, const double o[3],
-                                           const double d[3], double& tau) {
+__device__ __forceinline__ bool facet_test(const float4 q0, const float4 q1, const float4 q2, const float of[3],
+                                           const float df[3], double& tau) {
+  const double o[3] = {(double)of[0], (double)of[1], (double)of[2]};
+  const double d[3] = {(double)df[0], (double)df[1], (double)df[2]};
   const double p0[3] = {(double)q0.x, (double)q0.y, (double)q0.z};
   const double p1[3] = {(double)q1.x, (double)q1.y, (double)q1.z};
   const double p2[3] = {(double)q2.x, (double)q2.y, (double)q2.z};
@@ -70,6 +84,62 @@ __device__ __forceinline__ bool facet_test(const float4 q0, const float4 q1, con
   return true;
 }
 
+// ---- fp32 classification of the same test, with forward error bounds --------------------------------
+// Every monomial of a triple product d_i b_j c_k passes through at most 7 roundings (two corner
+// differences, product, difference, product with d, two sums): |computed - exact| <= ((1+u)^7 - 1) * M with
+// M the sum of the absolute monomials, u = 2^-24.  M is itself computed in fp32, so the band used is
+// 10 u M.  Magnitudes in this application (metres, m/s) are far from the fp32 under/overflow range.
+enum { TRI_MISS = 0, TRI_HIT = 1, TRI_UNCERTAIN = 2 };
+
+__device__ __forceinline__ void triple_f32(const float d[3], const float x[3], const float y[3], float& w, float& M) {
+  const float p0 = x[1] * y[2], p1 = x[2] * y[1];
+  const float p2 = x[2] * y[0], p3 = x[0] * y[2];
+  const float p4 = x[0] * y[1], p5 = x[1] * y[0];
+  w = fmaf(d[2], p4 - p5, fmaf(d[1], p2 - p3, d[0] * (p0 - p1)));
+  M = fmaf(fabsf(d[2]), fabsf(p4) + fabsf(p5), fmaf(fabsf(d[1]), fabsf(p2) + fabsf(p3), fabsf(d[0]) * (fabsf(p0) + fabsf(p1))));
+}
+
+__device__ __forceinline__ int tri_filter(const float4 q0, const float4 q1, const float4 q2, const float o[3],
+                                          const float d[3], float& tlo, float& thi) {
+  const float EPS = 5.9604645e-07f;   // 10 * 2^-24
+  const float a[3] = {q0.x - o[0], q0.y - o[1], q0.z - o[2]};
+  const float e1[3] = {q1.x - q0.x, q1.y - q0.y, q1.z - q0.z};
+  const float e2[3] = {q2.x - q0.x, q2.y - q0.y, q2.z - q0.z};
+  float det, Mdet;
+  triple_f32(d, e1, e2, det, Mdet);               // d . (e1 x e2)
+  const float Edet = EPS * Mdet;
+  const bool two_sided = (__float_as_uint(q1.w) & TPMC_FACET_TWO_SIDED) != 0u;
+  if (!two_sided && det > Edet) return TRI_MISS;  // provably back-facing
+  const float b[3] = {q1.x - o[0], q1.y - o[1], q1.z - o[2]};
+  const float c[3] = {q2.x - o[0], q2.y - o[1], q2.z - o[2]};
+  float w0, M0, w1, M1, w2, M2;
+  triple_f32(d, b, c, w0, M0);
+  triple_f32(d, c, a, w1, M1);
+  triple_f32(d, a, b, w2, M2);
+  const float E0 = EPS * M0, E1 = EPS * M1, E2 = EPS * M2;
+  const bool anypos = (w0 > E0) || (w1 > E1) || (w2 > E2);
+  const bool anyneg = (w0 < -E0) || (w1 < -E1) || (w2 < -E2);
+  if (anypos && anyneg) return TRI_MISS;          // two edge functions of provably opposite sign
+  float num, Mn;
+  triple_f32(a, e1, e2, num, Mn);                 // a . (e1 x e2)
+  const float En = EPS * Mn;
+  const float ad = fabsf(det), an = fabsf(num);
+  const bool det_ok = ad > Edet;                  // sign of det is certain
+  const bool num_ok = an > En;
+  if (det_ok && num_ok && ((num > 0.0f) != (det > 0.0f))) return TRI_MISS;   // provably behind the origin
+  tlo = 0.0f;
+  thi = INFINITY;
+  if (det_ok) {
+    tlo = fmaxf(an - En, 0.0f) / (ad + Edet) * 0.99999964f;
+    thi = (an + En) / (ad - Edet) * 1.00000036f;
+  }
+  const bool allpos = (w0 > E0) && (w1 > E1) && (w2 > E2);
+  const bool allneg = (w0 < -E0) && (w1 < -E1) && (w2 < -E2);
+  if ((allpos || allneg) && det_ok && num_ok) return TRI_HIT;   // (one-sided: det < -Edet follows from det_ok)
+  if (!(det_ok && num_ok)) tlo = 0.0f;
+  return TRI_UNCERTAIN;
+}
+
 // ---- conservative fp32 slab test -------------------------------------------------------------------
 // Each plane distance (lo - o) * (1/d) carries three roundings: relative error <= 3 * 2^-24.  min/max are
 // exact and x -> x -+ 4u|x| is monotone, so one margin on the entry and one on the exit make the test
@@ -88,23 +158,117 @@ __device__ __forceinline__ bool slab(float lx, float ly, float lz, float hx, flo
   return fmaxf(tn, 0.0f) <= fminf(tf, tmax);
 }
 
+// ---- per-ray traversal state of the wavefront kernel -------------------------------------------------
+struct Walk {
+  float o[3], d[3], id[3];
+  float tmax;          // min over provable hits of their thi
+  int f_prev;
+  int cur;             // node to visit next (>= 0 internal, < 0 leaf ~slot), TPMC_SENTINEL when finished
+  int sp;
+  int cs[TPMC_MAX_CAND];     // candidate slots
+  float cl[TPMC_MAX_CAND];   // their tlo
+  int nc;              // number of candidates; TPMC_MAX_CAND+1 = overflow
+};
+
+__device__ __forceinline__ void walk_init(Walk& w, const float4 ro, const float4 rv, int f_prev) {
+  w.o[0] = ro.x; w.o[1] = ro.y; w.o[2] = ro.z;
+  w.d[0] = rv.x; w.d[1] = rv.y; w.d[2] = rv.z;
+  w.id[0] = 1.0f / rv.x; w.id[1] = 1.0f / rv.y; w.id[2] = 1.0f / rv.z;
+  w.tmax = INFINITY;
+  w.f_prev = f_prev;
+  w.cur = 0;
+  w.sp = 0;
+  w.nc = 0;
+#pragma unroll
+  for (int k = 0; k < TPMC_MAX_CAND; ++k) { w.cs[k] = -1; w.cl[k] = 0.0f; }
+}
+
+__device__ __forceinline__ int walk_pop(Walk& w, const int* stk, int sstride, const int* lstack) {
+  if (w.sp == 0) return TPMC_SENTINEL;
+  --w.sp;
+  return (w.sp < TPMC_STACK_SMEM) ? stk[w.sp * sstride] : lstack[w.sp - TPMC_STACK_SMEM];
+}
+
+__device__ __forceinline__ void walk_add_candidate(Walk& w, int slot, int cls, float tlo, float thi) {
+  if (cls == TRI_HIT && thi < w.tmax) {
+    w.tmax = thi;
+    // drop candidates that can no longer be the closest
+    int n = 0;
+#pragma unroll
+    for (int k = 0; k < TPMC_MAX_CAND; ++k) {
+      const bool keep = (w.cs[k] >= 0) && (w.cl[k] <= w.tmax);
+      const int s = w.cs[k];
+      const float l = w.cl[k];
+      w.cs[k] = -1;
+      if (keep) {
+#pragma unroll
+        for (int j = 0; j < TPMC_MAX_CAND; ++j)
+          if (j == n) { w.cs[j] = s; w.cl[j] = l; }
+        ++n;
+      }
+    }
+    if (w.nc <= TPMC_MAX_CAND) w.nc = n;
+  }
+  if (tlo > w.tmax) return;
+  if (w.nc >= TPMC_MAX_CAND) { w.nc = TPMC_MAX_CAND + 1; return; }
+#pragma unroll
+  for (int j = 0; j < TPMC_MAX_CAND; ++j)
+    if (j == w.nc) { w.cs[j] = slot; w.cl[j] = tlo; }
+  ++w.nc;
+}
+
+// One traversal step: an internal node (two slab tests) or a leaf (one fp32 facet classification).
+__device__ __forceinline__ void walk_step(Walk& w, const float4* __restrict__ nodes, const float4* __restrict__ tris,
+                                          int* stk, int sstride, int* lstack, TraceCounters& cnt) {
+  if (w.cur >= 0) {
+    const float4* np = nodes + 4 * (size_t)w.cur;
+    const float4 n0 = __ldg(np + 0), n1 = __ldg(np + 1), n2 = __ldg(np + 2), n3 = __ldg(np + 3);
+    ++cnt.nodes;
+    float t0, t1;
+    const bool h0 = slab(n0.x, n0.y, n0.z, n0.w, n1.x, n1.y, w.o, w.id, w.tmax, t0);
+    const bool h1 = slab(n1.z, n1.w, n2.x, n2.y, n2.z, n2.w, w.o, w.id, w.tmax, t1);
+    int c0 = __float_as_int(n3.x), c1 = __float_as_int(n3.y);
+    if (h0 && h1) {
+      if (t1 < t0) { const int t = c0; c0 = c1; c1 = t; }
+      if (w.sp < TPMC_STACK_SMEM) stk[w.sp * sstride] = c1; else lstack[w.sp - TPMC_STACK_SMEM] = c1;
+      ++w.sp;
+      w.cur = c0;
+    } else if (h0) {
+      w.cur = c0;
+    } else if (h1) {
+      w.cur = c1;
+    } else {
+      w.cur = walk_pop(w, stk, sstride, lstack);
+    }
+  } else {
+    const int slot = ~w.cur;
+    const float4 q0 = __ldg(tris + 3 * (size_t)slot + 0);
+    if (__float_as_int(q0.w) != w.f_prev) {
+      const float4 q1 = __ldg(tris + 3 * (size_t)slot + 1);
+      const float4 q2 = __ldg(tris + 3 * (size_t)slot + 2);
+      ++cnt.tris;
+      float tlo, thi;
+      const int cls = tri_filter(q0, q1, q2, w.o, w.d, tlo, thi);
+      if (cls != TRI_MISS) walk_add_candidate(w, slot, cls, tlo, thi);
+    }
+    w.cur = walk_pop(w, stk, sstride, lstack);
+  }
+}
+
+// ---- exact closest hit by a full fp64 traversal (stragglers, candidate overflow) ----------------------
 // Closest hit ("the closest intersection point to the initial position becomes the first
 // collision"), ties to the smallest facet index (A12), source facet excluded (A11).
-// `sstack` points at this thread's column of the shared-memory stack (stride = blockDim.x).
 __device__ __forceinline__ Hit closest_hit(const float4* __restrict__ nodes, const float4* __restrict__ tris,
                                            const float of[3], const float df[3], int f_prev, int* sstack,
                                            int sstride, TraceCounters& cnt) {
   Hit best;
   best.tau = INFINITY; best.facet = -1; best.slot = -1;
-  const double o[3] = {(double)of[0], (double)of[1], (double)of[2]};
-  const double d[3] = {(double)df[0], (double)df[1], (double)df[2]};
   const float id[3] = {1.0f / df[0], 1.0f / df[1], 1.0f / df[2]};
   float tmax = INFINITY;
   int lstack[TPMC_STACK_LOCAL];
   int sp = 0;
   int node = 0;
   for (;;) {
-    // ---- internal node: test both child boxes
     const float4 n0 = __ldg(nodes + 4 * (size_t)node + 0);
     const float4 n1 = __ldg(nodes + 4 * (size_t)node + 1);
     const float4 n2 = __ldg(nodes + 4 * (size_t)node + 2);
@@ -129,7 +293,6 @@ __device__ __forceinline__ Hit closest_hit(const float4* __restrict__ nodes, con
       --sp;
       next = (sp < TPMC_STACK_SMEM) ? sstack[sp * sstride] : lstack[sp - TPMC_STACK_SMEM];
     }
-    // ---- leaves
     bool done = false;
     while (next < 0) {
       const int slot = ~next;
@@ -140,7 +303,7 @@ __device__ __forceinline__ Hit closest_hit(const float4* __restrict__ nodes, con
         const float4 q2 = __ldg(tris + 3 * (size_t)slot + 2);
         ++cnt.tris;
         double tau;
-        if (facet_test(q0, q1, q2, o, d, tau) && (tau < best.tau || (tau == best.tau && facet < best.facet))) {
+        if (facet_test(q0, q1, q2, of, df, tau) && (tau < best.tau || (tau == best.tau && facet < best.facet))) {
           best.tau = tau; best.facet = facet; best.slot = slot;
           tmax = __double2float_ru(tau);
         }
@@ -155,8 +318,30 @@ __device__ __forceinline__ Hit closest_hit(const float4* __restrict__ nodes, con
   return best;
 }
 
+// Resolve a candidate list with the exact test: smallest tau, ties to the smallest facet index.
+__device__ __forceinline__ Hit resolve_candidates(const float4* __restrict__ tris, const int4 cand, const float of[3],
+                                                  const float df[3], unsigned int& ntests) {
+  Hit best;
+  best.tau = INFINITY; best.facet = -1; best.slot = -1;
+  const int cs[4] = {cand.x, cand.y, cand.z, cand.w};
+#pragma unroll
+  for (int k = 0; k < TPMC_MAX_CAND; ++k) {
+    const int slot = cs[k];
+    if (slot < 0) continue;
+    const float4 q0 = __ldg(tris + 3 * (size_t)slot + 0), q1 = __ldg(tris + 3 * (size_t)slot + 1),
+                 q2 = __ldg(tris + 3 * (size_t)slot + 2);
+    const int facet = __float_as_int(q0.w);
+    double tau;
+    ++ntests;
+    if (facet_test(q0, q1, q2, of, df, tau) && (tau < best.tau || (tau == best.tau && facet < best.facet))) {
+      best.tau = tau; best.facet = facet; best.slot = slot;
+    }
+  }
+  return best;
+}
+
 // ---- O11: surface interaction (P:73 diffuse re-emission at T_W; P:53 specular; Maxwell mix A7) ------
-// u: the four uniforms of Philox block 2+k.  Returns v_out in fp64 (the caller rounds it to fp32, O9).
+// w: the four words of Philox block 2+k.  Returns v_out in fp64 (the caller rounds it to fp32, O9).
 __device__ __forceinline__ void reflect(const float4 q0, const float4 q1, const float4 q2, const float vf[3],
                                         double sigma, double cW, const uint4 w, double vout[3]) {
   const double p0[3] = {(double)q0.x, (double)q0.y, (double)q0.z};
