@@ -50,18 +50,16 @@ struct tpmc_mesh {
   double* partials;                // reduction partials
   unsigned long long* stats;       // [8] device counters
   double* totals;                  // [3] torque accumulators
-  cudaEvent_t ev0, ev1;
+  cudaEvent_t ev0, ev1, ev2, ev3;
   cudaEvent_t* wave_ev;            // [kEvPerWave*kMaxTimedWaves] per-kernel timing, created on first use
   unsigned long long last_launches;
   unsigned long long last_timed_waves;
 };
 
-constexpr int kMaxTimedWaves = 512;
-constexpr int kRounds = 3;                       // wavefront rounds before the straggler kernel
-constexpr int kEvPerWave = 2 + 2 * kRounds + 1;  // start, seed, (trace, reflect) x rounds, finish
-constexpr int kCtrWords = 32;
-// ctr layout: [0..kRounds] queue sizes, [8..] fetch heads of the trace rounds, [16..] hit counts
-constexpr int kCtrQueue = 0, kCtrFetch = 8, kCtrHits = 16;
+constexpr int kMaxTimedWaves = 1024;  // iterations covered by the per-kernel event times
+constexpr int kDrain = 3;             // trace/reflect iterations after the last wave, before the straggler kernel
+constexpr int kEvPerWave = 4;         // iteration start, after seed, after trace, after reflect
+constexpr int kCtrWords = 8;
 
 // Per-run constants (a1: host, fp64), passed to kernels by value.
 struct SpeciesConst {

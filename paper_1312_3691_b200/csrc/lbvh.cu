@@ -252,6 +252,7 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
   for (int a = 0; a < 3; ++a) { m->centre[a] = centre[a]; m->aabb_lo[a] = h.aabb[a]; m->aabb_hi[a] = h.aabb[3 + a]; }
   m->Rb = sqrt(h.r2);
   m->ev0 = e0; m->ev1 = e1;
+  cudaEventCreate(&m->ev2); cudaEventCreate(&m->ev3);
 
 #define MESH_TRY(expr)                       \
   do {                                       \
@@ -317,6 +318,8 @@ extern "C" void tpmc_mesh_destroy(tpmc_mesh* m) {
   }
   if (m->ev0) cudaEventDestroy(m->ev0);
   if (m->ev1) cudaEventDestroy(m->ev1);
+  if (m->ev2) cudaEventDestroy(m->ev2);
+  if (m->ev3) cudaEventDestroy(m->ev3);
   delete m;
 }
 

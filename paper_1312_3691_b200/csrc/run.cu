@@ -32,11 +32,31 @@ __global__ void k_init_debug(tpmc_debug dbg, unsigned long long count) {
   if (dbg.first_facet) dbg.first_facet[j] = -1;
 }
 
+// Ray queue: region A [0, cap) holds rays reflected in the previous iteration (any earlier wave), region B
+// [cap, 2 cap) the primaries of the current wave.  Record: o.xyz | particle index within the chunk,
+// v.xyz | (species | bounce << 4), source facet.
+struct RayQueue {
+  float4* o;
+  float4* v;
+  int* f;
+};
+
+// Per-iteration device counters: ctr[2p] = rays in region A of queue p, ctr[2p+1] = rays in region B,
+// ctr[4] = fetch head of the trace kernel, ctr[5] = hit-list length.
+__global__ void k_iter_begin(unsigned int* __restrict__ ctr, int out_parity) {
+  if (threadIdx.x == 0) {
+    ctr[2 * out_parity] = 0u;
+    ctr[2 * out_parity + 1] = 0u;
+    ctr[4] = 0u;
+    ctr[5] = 0u;
+  }
+}
+
 // a2: seed one wave of particles, round the state to fp32 (O9), drop the rays that cannot touch the
 // mesh AABB (their single segment is an escape) and append the rest to the ray queue.
-__global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned long long wave_first,
-                                                     unsigned int wave_n, float4* __restrict__ ray_o,
-                                                     float4* __restrict__ ray_v, unsigned int* __restrict__ qcount,
+__global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned int wave_first,
+                                                     unsigned int wave_n, const RayQueue q, unsigned int region_b,
+                                                     unsigned int* __restrict__ qcount,
                                                      unsigned long long* __restrict__ stats) {
   const unsigned int j = blockIdx.x * blockDim.x + threadIdx.x;
   const bool active = j < wave_n;
@@ -63,18 +83,13 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
   }
   base = __shfl_sync(0xFFFFFFFFu, base, 0);
   if (keep) {
-    const unsigned slot = base + __popc(m & lanemask_lt());
-    ray_o[slot] = make_float4(o[0], o[1], o[2], __uint_as_float(j));
-    ray_v[slot] = make_float4(v[0], v[1], v[2], __uint_as_float((unsigned int)species));   // bounce 0
+    const unsigned slot = region_b + base + __popc(m & lanemask_lt());
+    q.o[slot] = make_float4(o[0], o[1], o[2], __uint_as_float(wave_first + j));
+    q.v[slot] = make_float4(v[0], v[1], v[2], __uint_as_float((unsigned int)species));   // bounce 0
+    q.f[slot] = -1;
   }
 }
 
-// Ray queue record: o.xyz | particle index within the wave, v.xyz | (species | bounce << 4), source facet.
-struct RayQueue {
-  float4* o;
-  float4* v;
-  int* f;      // may be null for primary rays (f_prev = -1)
-};
 
 // a3: wavefront traversal.  Persistent warps; a lane whose ray has finished takes the next ray of the
 // queue (warp-aggregated fetch) as soon as fewer than kRefill lanes are busy, so rays of very different
@@ -84,7 +99,7 @@ constexpr int kRefill = 20;
 
 __global__ void __launch_bounds__(kTraceBlock, 8) k_trace_wf(const float4* __restrict__ nodes,
                                                              const float4* __restrict__ tris, const RayQueue q,
-                                                             const unsigned int* __restrict__ n_rays,
+                                                             unsigned int cap, const unsigned int* __restrict__ n_rays,
                                                              unsigned int* __restrict__ next_ray,
                                                              unsigned int* __restrict__ hit_ray,
                                                              int4* __restrict__ hit_cand,
@@ -93,7 +108,7 @@ __global__ void __launch_bounds__(kTraceBlock, 8) k_trace_wf(const float4* __res
   __shared__ int sstack[TPMC_STACK_SMEM * kTraceBlock];
   int* stk = sstack + threadIdx.x;
   int lstack[TPMC_STACK_LOCAL];
-  const unsigned int n = *n_rays;
+  const unsigned int na = min(n_rays[0], cap), n = na + n_rays[1];   // region A (reflected), region B (primaries)
   const int lane = threadIdx.x & 31;
   const unsigned FULL = 0xFFFFFFFFu;
   bool has = false, exhausted = false;
@@ -112,7 +127,8 @@ __global__ void __launch_bounds__(kTraceBlock, 8) k_trace_wf(const float4* __res
       if (!has && !exhausted) {
         r = base + __popc(need & lanemask_lt());
         if (r < n) {
-          walk_init(w, q.o[r], q.v[r], q.f ? q.f[r] : -1);
+          r = (r < na) ? r : cap + (r - na);   // physical slot
+          walk_init(w, q.o[r], q.v[r], q.f[r]);
           has = true;
         } else {
           exhausted = true;
@@ -195,7 +211,7 @@ __device__ __forceinline__ void block_flush(double tq[3], unsigned long long c4[
 // here (bounce cap).
 struct Particle {
   float o[3], v[3];
-  unsigned long long j;   // index within the slice
+  unsigned long long j;   // index within the chunk (rc.first = first particle of the chunk)
   int species;
   unsigned int k;         // reflections so far
   int f_prev;
@@ -237,7 +253,7 @@ __device__ __forceinline__ bool interact(const RunConst& rc, const float4* __res
 
 // a4-a6: resolve the candidates of every hit ray with the exact fp64 test, apply the surface interaction,
 // accumulate, and queue the reflected ray for the next wavefront round (compacted, warp-aggregated).
-__global__ void __launch_bounds__(kTraceBlock) k_reflect(const RunConst rc, unsigned long long wave_first,
+__global__ void __launch_bounds__(kTraceBlock) k_reflect(const RunConst rc, unsigned int cap,
                                                          const float4* __restrict__ nodes,
                                                          const float4* __restrict__ tris, const RayQueue qin,
                                                          const unsigned int* __restrict__ hit_ray,
@@ -266,11 +282,11 @@ __global__ void __launch_bounds__(kTraceBlock) k_reflect(const RunConst rc, unsi
       const float4 ro = qin.o[r], rv = qin.v[r];
       p.o[0] = ro.x; p.o[1] = ro.y; p.o[2] = ro.z;
       p.v[0] = rv.x; p.v[1] = rv.y; p.v[2] = rv.z;
-      p.j = wave_first + __float_as_uint(ro.w);
+      p.j = __float_as_uint(ro.w);
       const unsigned int pk = __float_as_uint(rv.w);
       p.species = (int)(pk & 15u);
       p.k = pk >> 4;
-      p.f_prev = qin.f ? qin.f[r] : -1;
+      p.f_prev = qin.f[r];
       Hit hit;
       if (cand.w == TPMC_CAND_OVERFLOW) {
         int tmp[TPMC_STACK_SMEM];
@@ -291,9 +307,21 @@ __global__ void __launch_bounds__(kTraceBlock) k_reflect(const RunConst rc, unsi
       base = __shfl_sync(0xFFFFFFFFu, base, leader);
       if (emit) {
         const unsigned s = base + __popc(em & lanemask_lt());
-        qout.o[s] = make_float4(p.o[0], p.o[1], p.o[2], __uint_as_float((unsigned int)(p.j - wave_first)));
-        qout.v[s] = make_float4(p.v[0], p.v[1], p.v[2], __uint_as_float((unsigned int)p.species | (p.k << 4)));
-        qout.f[s] = p.f_prev;
+        if (s < cap) {
+          qout.o[s] = make_float4(p.o[0], p.o[1], p.o[2], __uint_as_float((unsigned int)p.j));
+          qout.v[s] = make_float4(p.v[0], p.v[1], p.v[2], __uint_as_float((unsigned int)p.species | (p.k << 4)));
+          qout.f[s] = p.f_prev;
+        } else {
+          // region A of the next queue is full (possible only when most segments hit): follow this
+          // particle to escape here instead of dropping it
+          int tmp[TPMC_STACK_SMEM];
+          for (;;) {
+            const Hit hit = closest_hit(nodes, tris, p.o, p.v, p.f_prev, tmp, 1, cnt);
+            if (hit.facet < 0) break;
+            ++hits;
+            if (!interact(rc, tris, p, hit, P, tq, dbg, trunc)) break;
+          }
+        }
       }
     }
   }
@@ -303,7 +331,7 @@ __global__ void __launch_bounds__(kTraceBlock) k_reflect(const RunConst rc, unsi
 
 // Stragglers after the wavefront rounds: each remaining particle is followed to escape in one thread
 // (full fp64 traversal per segment).  Few particles get here; long multi-bounce paths live here.
-__global__ void __launch_bounds__(kTraceBlock) k_finish(const RunConst rc, unsigned long long wave_first,
+__global__ void __launch_bounds__(kTraceBlock) k_finish(const RunConst rc, unsigned int cap,
                                                         const float4* __restrict__ nodes,
                                                         const float4* __restrict__ tris, const RayQueue q,
                                                         const unsigned int* __restrict__ n_rays,
@@ -312,7 +340,7 @@ __global__ void __launch_bounds__(kTraceBlock) k_finish(const RunConst rc, unsig
   __shared__ int sstack[TPMC_STACK_SMEM * kTraceBlock];
   __shared__ double sred[3][8];
   __shared__ unsigned long long scnt[4][8];
-  const unsigned int n = *n_rays;
+  const unsigned int n = min(*n_rays, cap);
   double tq[3] = {0.0, 0.0, 0.0};
   unsigned long long hits = 0, trunc = 0;
   TraceCounters cnt;
@@ -322,11 +350,11 @@ __global__ void __launch_bounds__(kTraceBlock) k_finish(const RunConst rc, unsig
     Particle p;
     p.o[0] = ro.x; p.o[1] = ro.y; p.o[2] = ro.z;
     p.v[0] = rv.x; p.v[1] = rv.y; p.v[2] = rv.z;
-    p.j = wave_first + __float_as_uint(ro.w);
+    p.j = __float_as_uint(ro.w);
     const unsigned int pk = __float_as_uint(rv.w);
     p.species = (int)(pk & 15u);
     p.k = pk >> 4;
-    p.f_prev = q.f ? q.f[r] : -1;
+    p.f_prev = q.f[r];
     for (;;) {
       const Hit hit = closest_hit(nodes, tris, p.o, p.v, p.f_prev, sstack + threadIdx.x, kTraceBlock, cnt);
       if (hit.facet < 0) break;
@@ -500,7 +528,7 @@ size_t wave_size() {
   if (!w) {
     const char* e = getenv("TPMC_WAVE");
     long long v = e ? atoll(e) : 0;
-    w = (v >= 1024 && v <= (1ll << 28)) ? (size_t)v : ((size_t)1 << 22);
+    w = (v >= 1024 && v <= (1ll << 28)) ? (size_t)v : ((size_t)1 << 24);
   }
   return w;
 }
@@ -521,12 +549,12 @@ int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
     m->hit_ray = nullptr; m->hit_cand = nullptr;
     m->wave_cap = 0;
     for (int k = 0; k < 2; ++k) {
-      TPMC_CUDA_TRY(cudaMalloc((void**)&m->q_o[k], wave * sizeof(float4)));
-      TPMC_CUDA_TRY(cudaMalloc((void**)&m->q_v[k], wave * sizeof(float4)));
-      TPMC_CUDA_TRY(cudaMalloc((void**)&m->q_f[k], wave * sizeof(int)));
+      TPMC_CUDA_TRY(cudaMalloc((void**)&m->q_o[k], 2 * wave * sizeof(float4)));   // regions A and B
+      TPMC_CUDA_TRY(cudaMalloc((void**)&m->q_v[k], 2 * wave * sizeof(float4)));
+      TPMC_CUDA_TRY(cudaMalloc((void**)&m->q_f[k], 2 * wave * sizeof(int)));
     }
-    TPMC_CUDA_TRY(cudaMalloc((void**)&m->hit_ray, wave * sizeof(unsigned int)));
-    TPMC_CUDA_TRY(cudaMalloc((void**)&m->hit_cand, wave * sizeof(int4)));
+    TPMC_CUDA_TRY(cudaMalloc((void**)&m->hit_ray, 2 * wave * sizeof(unsigned int)));
+    TPMC_CUDA_TRY(cudaMalloc((void**)&m->hit_cand, 2 * wave * sizeof(int4)));
     m->wave_cap = wave;
   }
   if (need_facets && !m->facet_scratch)
@@ -567,21 +595,22 @@ int fill_stats(tpmc_mesh* m, const tpmc_params* params, tpmc_stats* h_stats) {
   h_stats->ms = ms;
   h_stats->ms_seed = h_stats->ms_trace = h_stats->ms_reflect = h_stats->ms_finish = 0.0;
   h_stats->timed_waves = m->last_timed_waves;
-  h_stats->trace_launches = m->last_timed_waves * kRounds;
+  h_stats->trace_launches = m->last_timed_waves;
   h_stats->traced_rays = hs[ST_TRACED];
   for (unsigned long long w = 0; w < m->last_timed_waves; ++w) {
     const cudaEvent_t* ev = m->wave_ev + kEvPerWave * w;
     float t = 0.0f;
     TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[0], ev[1]));
     h_stats->ms_seed += t;
-    for (int r = 0; r < kRounds; ++r) {
-      TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[1 + 2 * r], ev[2 + 2 * r]));
-      h_stats->ms_trace += t;
-      TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[2 + 2 * r], ev[3 + 2 * r]));
-      h_stats->ms_reflect += t;
-    }
-    TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[1 + 2 * kRounds], ev[2 + 2 * kRounds]));
-    h_stats->ms_finish += t;
+    TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[1], ev[2]));
+    h_stats->ms_trace += t;
+    TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[2], ev[3]));
+    h_stats->ms_reflect += t;
+  }
+  if (m->last_timed_waves) {
+    float t = 0.0f;
+    TPMC_CUDA_TRY(cudaEventElapsedTime(&t, m->ev2, m->ev3));
+    h_stats->ms_finish = t;
   }
   return TPMC_OK;
 }
@@ -599,16 +628,18 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
   const size_t wave = std::min<unsigned long long>(std::max<unsigned long long>(params->count, 1), wave_size());
   rcode = ensure_scratch(m, wave, d_facet_momentum == nullptr);
   if (rcode != TPMC_OK) return rcode;
+  const unsigned int cap = (unsigned int)m->wave_cap;   // region size of the queues
   double* P = d_facet_momentum ? d_facet_momentum : m->facet_scratch;
-  tpmc_debug dbg = {nullptr, nullptr, nullptr};
-  if (debug) dbg = *debug;
+  tpmc_debug dbg0 = {nullptr, nullptr, nullptr};
+  if (debug) dbg0 = *debug;
+  const bool any_dbg = dbg0.hash || dbg0.bounces || dbg0.first_facet;
 
   TPMC_CUDA_TRY(cudaEventRecord(m->ev0, st));
   TPMC_CUDA_TRY(cudaMemsetAsync(P, 0, 3 * sizeof(double) * (size_t)m->nt, st));
   TPMC_CUDA_TRY(cudaMemsetAsync(m->stats, 0, ST_COUNT * sizeof(unsigned long long), st));
   TPMC_CUDA_TRY(cudaMemsetAsync(m->totals, 0, 4 * sizeof(double), st));
-  if ((dbg.hash || dbg.bounces || dbg.first_facet) && params->count)
-    k_init_debug<<<(unsigned)((params->count + 255) / 256), 256, 0, st>>>(dbg, params->count);
+  if (any_dbg && params->count)
+    k_init_debug<<<(unsigned)((params->count + 255) / 256), 256, 0, st>>>(dbg0, params->count);
   const Grids& g = grids();
   const bool timed = (h_stats != nullptr);   // per-kernel events only when the caller will read them
   if (timed && !m->wave_ev) {
@@ -616,39 +647,58 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
     if (!m->wave_ev) return TPMC_ENOMEM;
     for (int i = 0; i < kEvPerWave * kMaxTimedWaves; ++i) TPMC_CUDA_TRY(cudaEventCreate(&m->wave_ev[i]));
   }
-  unsigned long long launches = (dbg.hash || dbg.bounces || dbg.first_facet) && params->count ? 1 : 0, wi = 0;
+  unsigned long long launches = (any_dbg && params->count) ? 1 : 0, it = 0;
   RayQueue Q[2] = {{m->q_o[0], m->q_v[0], m->q_f[0]}, {m->q_o[1], m->q_v[1], m->q_f[1]}};
-  for (unsigned long long w0 = 0; w0 < params->count; w0 += wave, ++wi) {
-    const unsigned int wn = (unsigned int)std::min<unsigned long long>(wave, params->count - w0);
+  // Particle indices inside the queues are 32-bit offsets into a chunk of the slice.
+  const unsigned long long kChunk = 0xF0000000ull;
+  for (unsigned long long c0 = 0; c0 < params->count; c0 += kChunk) {
+    const unsigned long long cn = std::min<unsigned long long>(kChunk, params->count - c0);
+    RunConst rcc = rc;
+    rcc.first = rc.first + c0;
+    rcc.count = cn;
+    tpmc_debug dbg = dbg0;
+    if (dbg.hash) dbg.hash += c0;
+    if (dbg.bounces) dbg.bounces += c0;
+    if (dbg.first_facet) dbg.first_facet += c0;
     TPMC_CUDA_TRY(cudaMemsetAsync(m->ctr, 0, kCtrWords * sizeof(unsigned int), st));
-    const bool tw = timed && wi < (unsigned long long)kMaxTimedWaves;
-    cudaEvent_t* ev = tw ? m->wave_ev + kEvPerWave * wi : nullptr;
-    int e = 0;
-    if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[e++], st));
-    k_seed<<<(wn + kSeedBlock - 1) / kSeedBlock, kSeedBlock, 0, st>>>(rc, w0, wn, Q[0].o, Q[0].v, m->ctr + kCtrQueue,
-                                                                     m->stats);
-    if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[e++], st));
-    for (int r = 0; r < kRounds; ++r) {
-      RayQueue qin = Q[r & 1], qout = Q[(r + 1) & 1];
-      if (r == 0) qin.f = nullptr;   // primary rays have no source facet
-      k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(m->nodes, m->tris, qin, m->ctr + kCtrQueue + r, m->ctr + kCtrFetch + r,
-                                                  m->hit_ray, m->hit_cand, m->ctr + kCtrHits + r, m->stats);
-      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[e++], st));
-      k_reflect<<<g.reflect, kTraceBlock, 0, st>>>(rc, w0, m->nodes, m->tris, qin, m->hit_ray, m->hit_cand,
-                                                   m->ctr + kCtrHits + r, qout, m->ctr + kCtrQueue + r + 1, P,
-                                                   m->totals, m->stats, dbg);
-      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[e++], st));
+    // One iteration per wave: seed the wave into region B of queue p (region A already holds the rays
+    // reflected in the previous iteration), trace the whole queue, reflect the hits into region A of the
+    // other queue.  Particles that keep bouncing ride along with the following waves.
+    const unsigned long long n_waves = (cn + wave - 1) / wave;
+    int p = 0;
+    for (unsigned long long wv = 0; wv < n_waves + kDrain; ++wv, ++it, p ^= 1) {
+      const bool tw = timed && it < (unsigned long long)kMaxTimedWaves;
+      cudaEvent_t* ev = tw ? m->wave_ev + kEvPerWave * it : nullptr;
+      k_iter_begin<<<1, 32, 0, st>>>(m->ctr, p ^ 1);
+      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[0], st));
+      if (wv < n_waves) {
+        const unsigned int w0 = (unsigned int)(wv * wave);
+        const unsigned int wn = (unsigned int)std::min<unsigned long long>(wave, cn - wv * wave);
+        k_seed<<<(wn + kSeedBlock - 1) / kSeedBlock, kSeedBlock, 0, st>>>(rcc, w0, wn, Q[p], cap, m->ctr + 2 * p + 1,
+                                                                         m->stats);
+        ++launches;
+      }
+      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[1], st));
+      k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(m->nodes, m->tris, Q[p], cap, m->ctr + 2 * p, m->ctr + 4, m->hit_ray,
+                                                  m->hit_cand, m->ctr + 5, m->stats);
+      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[2], st));
+      k_reflect<<<g.reflect, kTraceBlock, 0, st>>>(rcc, cap, m->nodes, m->tris, Q[p], m->hit_ray, m->hit_cand, m->ctr + 5,
+                                                   Q[p ^ 1], m->ctr + 2 * (p ^ 1), P, m->totals, m->stats, dbg);
+      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[3], st));
+      launches += 3;
     }
-    k_finish<<<g.finish, kTraceBlock, 0, st>>>(rc, w0, m->nodes, m->tris, Q[kRounds & 1], m->ctr + kCtrQueue + kRounds, P,
-                                               m->totals, m->stats, dbg);
-    if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[e++], st));
-    launches += 2 + 2 * kRounds;
+    // whatever still bounces after the drain iterations is followed to escape thread by thread
+    if (timed) TPMC_CUDA_TRY(cudaEventRecord(m->ev2, st));
+    k_finish<<<g.finish, kTraceBlock, 0, st>>>(rcc, cap, m->nodes, m->tris, Q[p], m->ctr + 2 * p, P, m->totals, m->stats,
+                                               dbg);
+    if (timed) TPMC_CUDA_TRY(cudaEventRecord(m->ev3, st));
+    ++launches;
   }
   k_reduce_parts<<<kReduceParts, kReduceBlock, 0, st>>>(P, (long long)m->nt, m->partials);
   k_reduce_final<<<1, 32, 0, st>>>(m->partials, kReduceParts, m->totals, d_force, d_torque);
   launches += 2;
   m->last_launches = launches;
-  m->last_timed_waves = timed ? std::min<unsigned long long>(wi, kMaxTimedWaves) : 0;
+  m->last_timed_waves = timed ? std::min<unsigned long long>(it, kMaxTimedWaves) : 0;
   TPMC_CUDA_TRY(cudaGetLastError());
   TPMC_CUDA_TRY(cudaEventRecord(m->ev1, st));
   if (h_stats) {
@@ -710,20 +760,20 @@ extern "C" int tpmc_trace(const tpmc_mesh* mesh, const float* d_o, const float* 
   if (n == 0) return TPMC_OK;
   tpmc_mesh* m = const_cast<tpmc_mesh*>(mesh);
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  int rcode = ensure_scratch(m, std::max<size_t>((size_t)n, m->wave_cap), false);
+  int rcode = ensure_scratch(m, std::max<size_t>(((size_t)n + 1) / 2, m->wave_cap), false);
   if (rcode != TPMC_OK) return rcode;
   const Grids& g = grids();
   RayQueue q = {m->q_o[0], m->q_v[0], m->q_f[0]};
   const unsigned int un = (unsigned int)n;
   TPMC_CUDA_TRY(cudaMemsetAsync(m->ctr, 0, kCtrWords * sizeof(unsigned int), st));
-  TPMC_CUDA_TRY(cudaMemcpyAsync(m->ctr + kCtrQueue, &un, sizeof(un), cudaMemcpyHostToDevice, st));
+  TPMC_CUDA_TRY(cudaMemcpyAsync(m->ctr, &un, sizeof(un), cudaMemcpyHostToDevice, st));   // region A holds the rays
   TPMC_CUDA_TRY(cudaMemsetAsync(m->stats, 0, ST_COUNT * sizeof(unsigned long long), st));
   k_pack_rays<<<(un + 255) / 256, 256, 0, st>>>(d_o, d_d, d_f_prev, un, q, d_facet, d_tau);
   // the production traversal (fp32 wavefront + candidate lists), then the exact fp64 resolve
-  k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(m->nodes, m->tris, q, m->ctr + kCtrQueue, m->ctr + kCtrFetch, m->hit_ray,
-                                              m->hit_cand, m->ctr + kCtrHits, m->stats);
-  k_resolve_only<<<g.reflect, kTraceBlock, 0, st>>>(m->nodes, m->tris, q, m->hit_ray, m->hit_cand, m->ctr + kCtrHits,
-                                                    d_facet, d_tau);
+  k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(m->nodes, m->tris, q, (unsigned int)(2 * m->wave_cap), m->ctr, m->ctr + 4,
+                                              m->hit_ray, m->hit_cand, m->ctr + 5, m->stats);
+  k_resolve_only<<<g.reflect, kTraceBlock, 0, st>>>(m->nodes, m->tris, q, m->hit_ray, m->hit_cand, m->ctr + 5, d_facet,
+                                                    d_tau);
   TPMC_CUDA_TRY(cudaGetLastError());
   TPMC_CUDA_TRY(cudaStreamSynchronize(st));   // &un must outlive the copy
   return TPMC_OK;
