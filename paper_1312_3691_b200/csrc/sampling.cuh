@@ -73,6 +73,114 @@ TPMC_HD double sample_normal_speed(double u, double s) {
   return x;
 }
 
+// ---- fast path: fp32 Newton to ~1e-6, two fp64 Newton steps, convergence check -----------------------
+// Root-finding in fp64 costs ~150 instructions per step and its iteration count differs from lane to
+// lane.  The first digits are therefore found in fp32 (erfcf/expf, a fixed number of steps), then two
+// fp64 steps square the error twice.  If the last fp64 step is not already below 1e-8 (ill-conditioned
+// tails, a poor start) the general solvers above take over from the current point: the result is the
+// same root either way.
+#define TPMC_SQRTPI_F 1.7724538509055160f
+
+TPMC_HD double sample_sin_phi_fast(double u, const SpeciesConst& sc) {
+  const double S = sc.S;
+  if (S < 1e-4) return sample_sin_phi(u, sc);
+  const double target = sc.g0 + u * sc.gI;
+  const float T = (float)target, Sf = (float)S;
+  float y;
+  if (T >= 2.0f) {
+    y = sqrtf(T * (1.0f / TPMC_SQRTPI_F) - 0.5f);            // Gt ~ sqrt(pi)(y^2 + 1/2)
+  } else if (T >= 0.004f) {
+    y = T - 0.4431135f;                                      // tangent at y = 0 (Gt(0) = sqrt(pi)/4, Gt' = 1)
+  } else {
+    const float L = -logf(4.0f * fmaxf(T, 1e-37f));          // Gt ~ e^{-y^2} / (4 |y|^3) for y << 0
+    y = -sqrtf(fmaxf(L - 1.5f * logf(L), 0.25f));
+  }
+  y = fminf(Sf, fmaxf(-Sf, y));
+#pragma unroll
+  for (int it = 0; it < 5; ++it) {
+    const float e = expf(-y * y);
+    const float ec = erfcf(-y);
+    const float g = 0.25f * TPMC_SQRTPI_F * (1.0f + 2.0f * y * y) * ec + 0.5f * y * e;
+    const float d = e + TPMC_SQRTPI_F * y * ec;
+    y = fminf(Sf, fmaxf(-Sf, y - (g - T) / d));
+  }
+  double yd = (double)y, step = 0.0;
+#pragma unroll
+  for (int it = 0; it < 2; ++it) {
+    const double e = exp(-yd * yd);
+    const double ec = erfc(-yd);
+    const double g = 0.25 * TPMC_SQRTPI * (1.0 + 2.0 * yd * yd) * ec + 0.5 * yd * e;
+    const double d = e + TPMC_SQRTPI * yd * ec;
+    const double yn = fmin(S, fmax(-S, yd - (g - target) / d));
+    step = fabs(yn - yd);
+    yd = yn;
+  }
+  if (!(step <= 1e-8 * fmax(1.0, fabs(yd)))) {
+    for (int it = 0; it < 64; ++it) {   // general solver, continued from yd
+      const double e = exp(-yd * yd);
+      const double ec = erfc(-yd);
+      const double g = 0.25 * TPMC_SQRTPI * (1.0 + 2.0 * yd * yd) * ec + 0.5 * yd * e;
+      const double d = e + TPMC_SQRTPI * yd * ec;
+      const double yn = fmin(S, fmax(-S, yd - (g - target) / d));
+      step = fabs(yn - yd);
+      yd = yn;
+      if (step <= 4e-16 * fmax(1.0, fabs(yd))) break;
+    }
+  }
+  return fmin(1.0, fmax(-1.0, yd / S));
+}
+
+TPMC_HD double sample_normal_speed_fast(double u, double s) {
+  const double chis = chi_fn(s);
+  const double target = (1.0 - u) * chis;
+  const float sf = (float)s, T = (float)target;
+  const float xm = 0.5f * (sf + sqrtf(sf * sf + 2.0f));
+  float x = xm;
+  if (sf >= 1.0f) {
+    // Q / (sqrt(pi) s) = erfc(z) + e^{-z^2} / (sqrt(pi) s), z = x - s: start from the erfc part alone
+    const float tau = fminf(fmaxf(T / (TPMC_SQRTPI_F * sf), 1e-30f), 1.9999f);
+    x = sf + erfcinvf(tau) + 0.5f / sf;
+  }
+  {
+    const float q0 = (float)(u * chis);
+    const float xs = sqrtf(q0) * expf(0.5f * sf * sf);       // root of the leading term of F near x = 0
+    if (xs < 0.25f * xm || !(x > 0.0f)) x = fminf(xm, 2.0f * xs);
+  }
+#pragma unroll
+  for (int it = 0; it < 5; ++it) {
+    const float z = x - sf;
+    const float e = expf(-z * z);
+    const float q = e + TPMC_SQRTPI_F * sf * erfcf(z);
+    float xn = x + (q - T) / (2.0f * x * e);
+    if (!(xn > 0.0f)) xn = 0.5f * x;
+    x = xn;
+  }
+  double xd = (double)x, step = 0.0;
+#pragma unroll
+  for (int it = 0; it < 2; ++it) {
+    const double z = xd - s;
+    const double e = exp(-z * z);
+    const double q = e + TPMC_SQRTPI * s * erfc(z);
+    double xn = xd + (q - target) / (2.0 * xd * e);
+    if (!(xn > 0.0)) xn = 0.5 * xd;
+    step = fabs(xn - xd);
+    xd = xn;
+  }
+  if (!(step <= 1e-8 * (1.0 + xd))) {
+    for (int it = 0; it < 96; ++it) {   // general solver, continued from xd
+      const double z = xd - s;
+      const double e = exp(-z * z);
+      const double q = e + TPMC_SQRTPI * s * erfc(z);
+      double xn = xd + (q - target) / (2.0 * xd * e);
+      if (!(xn > 0.0) || !(xn < 1e300)) xn = (xn > 0.0) ? 0.5 * (s > 0.0 ? s : 0.0) + 0.35 : 0.5 * xd;
+      step = fabs(xn - xd);
+      xd = xn;
+      if (step <= 4e-16 * (1.0 + xd)) break;
+    }
+  }
+  return xd;
+}
+
 struct SeedState {
   double x[3];
   double v[3];
@@ -91,7 +199,7 @@ TPMC_HD SeedState seed_particle(const RunConst& rc, unsigned long long i) {
   out.species = s;
   const SpeciesConst& sc = rc.sp[s];
   // O5: position on the unit sphere, stream frame (pole = upstream, A1)
-  const double t = sample_sin_phi(u01(b0.y), sc);
+  const double t = sample_sin_phi_fast(u01(b0.y), sc);
   const double cphi = sqrt(1.0 - t * t);
   double st, ct;
   sincospi(2.0 * u01(b0.z), &st, &ct);
@@ -100,7 +208,7 @@ TPMC_HD SeedState seed_particle(const RunConst& rc, unsigned long long i) {
   const double t1[3] = {t * ct, t * st, -cphi};
   const double t2[3] = {-st, ct, 0.0};
   // O7: velocity components in units of c_mp (eqs. 14a-c)
-  const double xn = sample_normal_speed(u01(b0.w), sc.S * t);
+  const double xn = sample_normal_speed_fast(u01(b0.w), sc.S * t);
   const double rho = sqrt(-log(u01(b1.x)));
   double sa, ca;
   sincospi(2.0 * u01(b1.y), &sa, &ca);
