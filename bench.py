@@ -73,6 +73,23 @@ class ClockSampler:
                 "reasons": reasons, "samples": len(sm)}
 
 
+def attitude_index(step: int, rank: int, world: int, n_attitudes: int) -> int:
+    """Which attitude of the sweep a rank runs at a step: ranks take disjoint attitudes (weak scaling)."""
+    return (step * world + rank) % n_attitudes
+
+
+def reduce_over_ranks(times, totals, world: int, device=None):
+    """MAX of the per-rank times and SUM of the per-rank totals (the only collective, after the timed region)."""
+    import torch
+    t = torch.tensor(list(times), dtype=torch.float64, device=device)
+    tot = torch.tensor(list(totals), dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    return t.tolist(), tot.tolist()
+
+
 def oracle_sample(cfgs, count_per_thread, threads):
     """The oracle, as it stands, on a bounded slice of the same workload, one slice per host thread."""
     import oracle
@@ -171,7 +188,7 @@ def main():
     import ctypes as C
 
     def step(k, stats=None):
-        cfg = cfgs[(k * world + rank) % len(cfgs)]
+        cfg = cfgs[attitude_index(k, rank, world, len(cfgs))]
         p, keep = tpmc.make_params(cfg)
         rc = L.tpmc_run(mesh._h, C.byref(p), stream.cuda_stream or None, force.data_ptr(), torque.data_ptr(),
                         facets.data_ptr(), None if stats is None else C.byref(stats), None)
@@ -219,7 +236,7 @@ def main():
         barrier()
         t0 = time.perf_counter()
         for k in range(args.steps):
-            cfg = cfgs[((args.warmup + k) * world + rank) % len(cfgs)]
+            cfg = cfgs[attitude_index(args.warmup + k, rank, world, len(cfgs))]
             p, keep = tpmc.make_params(cfg)
             rc = L.tpmc_run_host(mesh._h, C.byref(p), stream.cuda_stream or None, hF.ctypes.data, hT.ctypes.data,
                                  hP.ctypes.data, None)
@@ -230,13 +247,8 @@ def main():
         e2e = {"hits": hits, "s": e2e_s}
 
     # ---- max over ranks, totals over ranks
-    t = torch.tensor([ms_total, e2e["s"] if e2e else 0.0], dtype=torch.float64, device=dev)
-    tot = torch.tensor([hits, segs, N * args.steps], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-    ms_total_max, e2e_s_max = t.tolist()
-    hits_all, segs_all, parts_all = tot.tolist()
+    (ms_total_max, e2e_s_max), (hits_all, segs_all, parts_all) = reduce_over_ranks(
+        [ms_total, e2e["s"] if e2e else 0.0], [hits, segs, N * args.steps], world, dev)
 
     if rank == 0:
         value = hits_all / (ms_total_max * 1e-3)
