@@ -142,8 +142,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="tpmc", choices=["tpmc", "reference"])
     ap.add_argument("--particles", type=float, default=None, help="override N per step (default: the config's 1e9)")
-    ap.add_argument("--ref-particles", type=float, default=240_000, help="oracle particles per reference step")
-    ap.add_argument("--cpu-baseline-particles", type=float, default=400_000)
+    ap.add_argument("--ref-particles", type=float, default=4_000_000, help="oracle particles per reference step")
+    ap.add_argument("--cpu-baseline-particles", type=float, default=20_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()

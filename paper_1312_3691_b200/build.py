@@ -16,6 +16,7 @@ def nvcc_command(verbose: bool = False):
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
            "-Xcompiler", "-fPIC", "-shared", "-o", LIB]
+    cmd += os.environ.get("TPMC_NVCC_FLAGS", "").split()   # tuning experiments only
     if verbose:
         cmd += ["-Xptxas", "-v"]
     return cmd + [os.path.join(CSRC, s) for s in SOURCES]

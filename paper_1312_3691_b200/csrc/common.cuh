@@ -33,6 +33,8 @@ struct tpmc_mesh {
   int64_t n_nodes;
   float4* nodes;
   float4* tris;
+  float4* cull;                    // top of the hierarchy (<= kCullNodes nodes, breadth-first), for the seed-time cull
+  int n_cull;
   double centre[3];
   double Rb;
   float aabb_lo[3], aabb_hi[3];
@@ -51,6 +53,9 @@ struct tpmc_mesh {
   unsigned long long* stats;       // [8] device counters
   double* totals;                  // [3] torque accumulators
   cudaEvent_t ev0, ev1, ev2, ev3;
+  cudaStream_t seed_stream;        // the seed kernel of the next wave runs here, beside trace/reflect
+  cudaEvent_t ev_reset[4], ev_seeded[4];
+  unsigned long long last_seed_waves;
   cudaEvent_t* wave_ev;            // [kEvPerWave*kMaxTimedWaves] per-kernel timing, created on first use
   unsigned long long last_launches;
   unsigned long long last_timed_waves;
@@ -58,8 +63,9 @@ struct tpmc_mesh {
 
 constexpr int kMaxTimedWaves = 1024;  // iterations covered by the per-kernel event times
 constexpr int kDrain = 3;             // trace/reflect iterations after the last wave, before the straggler kernel
-constexpr int kEvPerWave = 4;         // iteration start, after seed, after trace, after reflect
+constexpr int kEvPerWave = 5;         // seed start/end (seed stream), trace start, after trace, after reflect
 constexpr int kCtrWords = 8;
+constexpr int kCullNodes = 1024;      // 64 KB: stays in L1 next to the shared-memory carve-out
 
 // Per-run constants (a1: host, fp64), passed to kernels by value.
 struct SpeciesConst {

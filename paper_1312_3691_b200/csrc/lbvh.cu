@@ -181,6 +181,29 @@ __global__ void k_single(const float* __restrict__ box_leaf, float4* __restrict_
   nodes[3] = make_float4(__int_as_float(~0), __int_as_float(~0), 0.0f, 0.0f);
 }
 
+// Top of the tree, breadth-first, cut at a node budget: child refs >= 0 index this array, -1 marks a
+// subtree (or triangle) that was cut off.  A ray that touches no cut-off box cannot hit the mesh.
+__global__ void k_build_cull(const float4* __restrict__ nodes, float4* __restrict__ cull, int* __restrict__ queue,
+                             int budget, int* __restrict__ out_count) {
+  if (blockIdx.x != 0 || threadIdx.x != 0) return;
+  int tail = 1;
+  queue[0] = 0;
+  for (int head = 0; head < tail; ++head) {
+    const float4* np = nodes + 4 * (size_t)queue[head];
+    const float4 n3 = np[3];
+    int ref[2] = {__float_as_int(n3.x), __float_as_int(n3.y)};
+    for (int k = 0; k < 2; ++k) {
+      if (ref[k] >= 0 && tail < budget) { queue[tail] = ref[k]; ref[k] = tail++; }
+      else ref[k] = -1;
+    }
+    cull[4 * head + 0] = np[0];
+    cull[4 * head + 1] = np[1];
+    cull[4 * head + 2] = np[2];
+    cull[4 * head + 3] = make_float4(__int_as_float(ref[0]), __int_as_float(ref[1]), 0.0f, 0.0f);
+  }
+  *out_count = tail;
+}
+
 struct DevBuf {  // frees on scope exit
   void* p = nullptr;
   ~DevBuf() { if (p) cudaFree(p); }
@@ -295,6 +318,11 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
                                                                                 kids.as<int2>(), par.as<int>());
     k_refit<<<gt, kBlock, 0, st>>>((int)nt, kids.as<int2>(), par.as<int>(), box.as<float>(), arr.as<int>(), m->nodes);
   }
+  DevBuf cq;
+  MESH_TRY(cudaMalloc((void**)&m->cull, sizeof(float4) * 4 * kCullNodes));
+  MESH_TRY(cudaMalloc(&cq.p, sizeof(int) * (kCullNodes + 1)));
+  k_build_cull<<<1, 32, 0, st>>>(m->nodes, m->cull, cq.as<int>(), kCullNodes, cq.as<int>() + kCullNodes);
+  MESH_TRY(cudaMemcpyAsync(&m->n_cull, cq.as<int>() + kCullNodes, sizeof(int), cudaMemcpyDeviceToHost, st));
   MESH_TRY(cudaGetLastError());
   MESH_TRY(cudaEventRecord(e1, st));
   MESH_TRY(cudaStreamSynchronize(st));
@@ -308,9 +336,14 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
 
 extern "C" void tpmc_mesh_destroy(tpmc_mesh* m) {
   if (!m) return;
-  cudaFree(m->nodes); cudaFree(m->tris);
+  cudaFree(m->nodes); cudaFree(m->tris); cudaFree(m->cull);
   for (int k = 0; k < 2; ++k) { cudaFree(m->q_o[k]); cudaFree(m->q_v[k]); cudaFree(m->q_f[k]); }
   cudaFree(m->hit_ray); cudaFree(m->hit_cand); cudaFree(m->ctr);
+  if (m->seed_stream) cudaStreamDestroy(m->seed_stream);
+  for (int k = 0; k < 4; ++k) {
+    if (m->ev_reset[k]) cudaEventDestroy(m->ev_reset[k]);
+    if (m->ev_seeded[k]) cudaEventDestroy(m->ev_seeded[k]);
+  }
   cudaFree(m->facet_scratch); cudaFree(m->partials); cudaFree(m->stats); cudaFree(m->totals);
   if (m->wave_ev) {
     for (int i = 0; i < kEvPerWave * kMaxTimedWaves; ++i) cudaEventDestroy(m->wave_ev[i]);

@@ -10,7 +10,7 @@
 
 namespace {
 
-constexpr int kSeedBlock = 256;
+constexpr int kSeedBlock = 128;
 constexpr int kTraceBlock = 128;
 constexpr int kReduceBlock = 256;
 constexpr int kReduceParts = 296;   // 2 per SM
@@ -53,9 +53,11 @@ __global__ void k_iter_begin(unsigned int* __restrict__ ctr, int out_parity) {
 }
 
 // a2: seed one wave of particles, round the state to fp32 (O9), drop the rays that cannot touch the
-// mesh AABB (their single segment is an escape) and append the rest to the ray queue.
+// mesh AABB or any box of the top of the hierarchy (their single segment is an escape; same conservative
+// slab test as the traversal) and append the rest to the ray queue.
 __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned int wave_first,
-                                                     unsigned int wave_n, const RayQueue q, unsigned int region_b,
+                                                     unsigned int wave_n, const float4* __restrict__ cull,
+                                                     const RayQueue q, unsigned int region_b,
                                                      unsigned int* __restrict__ qcount,
                                                      unsigned long long* __restrict__ stats) {
   const unsigned int j = blockIdx.x * blockDim.x + threadIdx.x;
@@ -70,8 +72,9 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
     for (int k = 0; k < 3; ++k) { o[k] = (float)s.x[k]; v[k] = (float)s.v[k]; }
     const float id[3] = {1.0f / v[0], 1.0f / v[1], 1.0f / v[2]};
     float tn;
+    float te;
     keep = slab(rc.aabb_lo[0], rc.aabb_lo[1], rc.aabb_lo[2], rc.aabb_hi[0], rc.aabb_hi[1], rc.aabb_hi[2], o, id,
-                INFINITY, tn);
+                INFINITY, tn) && cull_touch(cull, o, id, te);
   }
   const unsigned m = __ballot_sync(0xFFFFFFFFu, keep);
   const unsigned mc = __ballot_sync(0xFFFFFFFFu, active && !keep);
@@ -91,13 +94,26 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
 }
 
 
-// a3: wavefront traversal.  Persistent warps; a lane whose ray has finished takes the next ray of the
-// queue (warp-aggregated fetch) as soon as fewer than kRefill lanes are busy, so rays of very different
-// length (misses vs. hits) do not idle the warp.  fp32 only: see trace.cuh.  Rays that end with at least
-// one candidate facet are appended to the hit list for the resolve/reflect kernel.
-constexpr int kRefill = 20;
+// a3: wavefront traversal.  Persistent warps, one ray per lane, fp32 only (see trace.cuh).
+//  * node phase: lanes standing at an internal node step together; a lane that reaches a leaf waits;
+//  * leaf phase: once fewer than kNodeMin lanes are still at nodes, all waiting lanes classify their
+//    facet together (the ~120-instruction facet code then runs with many lanes active, not one);
+//  * a lane whose ray has finished takes the next ray of the queue as soon as kRefillIdle lanes are idle
+//    (one warp-aggregated atomic), so rays of very different length do not idle the warp.
+// Rays that end with at least one candidate facet are appended to the hit list for k_reflect.
+#ifndef TPMC_NODE_MIN
+#define TPMC_NODE_MIN 10
+#endif
+#ifndef TPMC_REFILL_IDLE
+#define TPMC_REFILL_IDLE 8
+#endif
+#ifndef TPMC_TRACE_MIN_BLOCKS
+#define TPMC_TRACE_MIN_BLOCKS 8
+#endif
+constexpr int kNodeMin = TPMC_NODE_MIN;
+constexpr int kRefillIdle = TPMC_REFILL_IDLE;
 
-__global__ void __launch_bounds__(kTraceBlock, 8) k_trace_wf(const float4* __restrict__ nodes,
+__global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf(const float4* __restrict__ nodes,
                                                              const float4* __restrict__ tris, const RayQueue q,
                                                              unsigned int cap, const unsigned int* __restrict__ n_rays,
                                                              unsigned int* __restrict__ next_ray,
@@ -111,21 +127,23 @@ __global__ void __launch_bounds__(kTraceBlock, 8) k_trace_wf(const float4* __res
   const unsigned int na = min(n_rays[0], cap), n = na + n_rays[1];   // region A (reflected), region B (primaries)
   const int lane = threadIdx.x & 31;
   const unsigned FULL = 0xFFFFFFFFu;
-  bool has = false, exhausted = false;
+  bool has = false, exhausted = false, fin = false;
   unsigned int r = 0;
   Walk w;
   w.cur = TPMC_SENTINEL; w.sp = 0; w.nc = 0; w.tmax = 0.0f; w.f_prev = -1;
   TraceCounters cnt;
   cnt.nodes = 0; cnt.tris = 0;
   for (;;) {
-    const unsigned need = __ballot_sync(FULL, !has && !exhausted);
-    if (need) {
-      const int leader = __ffs(need) - 1;
+    // ---- refill idle lanes
+    const unsigned idle = __ballot_sync(FULL, !has && !exhausted);
+    const unsigned busy0 = __ballot_sync(FULL, has);
+    if (idle && (__popc(idle) >= kRefillIdle || busy0 == 0u)) {
+      const int leader = __ffs(idle) - 1;
       unsigned base = 0;
-      if (lane == leader) base = atomicAdd(next_ray, (unsigned)__popc(need));
+      if (lane == leader) base = atomicAdd(next_ray, (unsigned)__popc(idle));
       base = __shfl_sync(FULL, base, leader);
       if (!has && !exhausted) {
-        r = base + __popc(need & lanemask_lt());
+        r = base + __popc(idle & lanemask_lt());
         if (r < n) {
           r = (r < na) ? r : cap + (r - na);   // physical slot
           walk_init(w, q.o[r], q.v[r], q.f[r]);
@@ -136,29 +154,37 @@ __global__ void __launch_bounds__(kTraceBlock, 8) k_trace_wf(const float4* __res
       }
     }
     if (__ballot_sync(FULL, has) == 0u) break;
-    const int thresh = __any_sync(FULL, exhausted) ? 1 : kRefill;
-    unsigned busy;
-    do {
-      bool fin = false;
-      if (has) {
-        walk_step(w, nodes, tris, stk, kTraceBlock, lstack, cnt);
+    // ---- node phase
+    for (;;) {
+      const bool at_node = has && w.cur >= 0;
+      const unsigned mn = __ballot_sync(FULL, at_node);
+      const unsigned ml = __ballot_sync(FULL, has && w.cur < 0);
+      if (!(__popc(mn) >= kNodeMin || (mn != 0u && ml == 0u))) break;
+      if (at_node) {
+        walk_node(w, nodes, stk, kTraceBlock, lstack, cnt);
         if (w.cur == TPMC_SENTINEL) { has = false; fin = w.nc > 0; }
       }
-      const unsigned fm = __ballot_sync(FULL, fin);
-      if (fm) {   // append finished rays that have candidates to the hit list
-        const int leader = __ffs(fm) - 1;
-        unsigned base = 0;
-        if (lane == leader) base = atomicAdd(n_hits, (unsigned)__popc(fm));
-        base = __shfl_sync(FULL, base, leader);
-        if (fin) {
-          const unsigned h = base + __popc(fm & lanemask_lt());
-          hit_ray[h] = r;
-          hit_cand[h] = (w.nc > TPMC_MAX_CAND) ? make_int4(-1, -1, -1, TPMC_CAND_OVERFLOW)
-                                               : make_int4(w.cs[0], w.cs[1], w.cs[2], w.cs[3]);
-        }
+    }
+    // ---- leaf phase
+    if (has && w.cur < 0) {
+      walk_leaf(w, tris, stk, kTraceBlock, lstack, cnt);
+      if (w.cur == TPMC_SENTINEL) { has = false; fin = w.nc > 0; }
+    }
+    // ---- finished rays with candidates -> hit list
+    const unsigned fm = __ballot_sync(FULL, fin);
+    if (fm) {
+      const int leader = __ffs(fm) - 1;
+      unsigned base = 0;
+      if (lane == leader) base = atomicAdd(n_hits, (unsigned)__popc(fm));
+      base = __shfl_sync(FULL, base, leader);
+      if (fin) {
+        const unsigned h = base + __popc(fm & lanemask_lt());
+        hit_ray[h] = r;
+        hit_cand[h] = (w.nc > TPMC_MAX_CAND) ? make_int4(-1, -1, -1, TPMC_CAND_OVERFLOW)
+                                             : make_int4(w.cs[0], w.cs[1], w.cs[2], w.cs[3]);
+        fin = false;
       }
-      busy = __ballot_sync(FULL, has);
-    } while (__popc(busy) >= thresh);
+    }
   }
   // counters: one atomic per warp
   unsigned long long cn = cnt.nodes, ct = cnt.tris;
@@ -535,6 +561,11 @@ size_t wave_size() {
 
 int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
   if (!m->ctr) {
+    TPMC_CUDA_TRY(cudaStreamCreateWithFlags(&m->seed_stream, cudaStreamNonBlocking));
+    for (int k = 0; k < 4; ++k) {
+      TPMC_CUDA_TRY(cudaEventCreateWithFlags(&m->ev_reset[k], cudaEventDisableTiming));
+      TPMC_CUDA_TRY(cudaEventCreateWithFlags(&m->ev_seeded[k], cudaEventDisableTiming));
+    }
     TPMC_CUDA_TRY(cudaMalloc((void**)&m->ctr, kCtrWords * sizeof(unsigned int)));
     TPMC_CUDA_TRY(cudaMalloc((void**)&m->stats, ST_COUNT * sizeof(unsigned long long)));
     TPMC_CUDA_TRY(cudaMalloc((void**)&m->totals, 4 * sizeof(double)));
@@ -570,6 +601,8 @@ const Grids& grids() {
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_trace_wf, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
+    if (const char* e = getenv("TPMC_TRACE_BLOCKS")) per = std::max(1, std::min(per, atoi(e)));
+    else per = std::max(1, per - 2);   // leave room for the seed kernel of the next wave
     g.trace = sms * per;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_reflect, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
     g.reflect = sms * per;
@@ -600,11 +633,13 @@ int fill_stats(tpmc_mesh* m, const tpmc_params* params, tpmc_stats* h_stats) {
   for (unsigned long long w = 0; w < m->last_timed_waves; ++w) {
     const cudaEvent_t* ev = m->wave_ev + kEvPerWave * w;
     float t = 0.0f;
-    TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[0], ev[1]));
-    h_stats->ms_seed += t;
-    TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[1], ev[2]));
-    h_stats->ms_trace += t;
+    if (w < m->last_seed_waves) {
+      TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[0], ev[1]));
+      h_stats->ms_seed += t;
+    }
     TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[2], ev[3]));
+    h_stats->ms_trace += t;
+    TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[3], ev[4]));
     h_stats->ms_reflect += t;
   }
   if (m->last_timed_waves) {
@@ -665,26 +700,36 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
     // reflected in the previous iteration), trace the whole queue, reflect the hits into region A of the
     // other queue.  Particles that keep bouncing ride along with the following waves.
     const unsigned long long n_waves = (cn + wave - 1) / wave;
+    // The seed kernel of wave w+1 (fp64/ALU bound) runs on a second stream next to the trace and reflect
+    // kernels of wave w (latency/L1 bound): it only touches region B of the other queue and its counter,
+    // which k_iter_begin(w) has reset.  ev_reset / ev_seeded order the two streams.
+    cudaStream_t s2 = m->seed_stream;
     int p = 0;
+    TPMC_CUDA_TRY(cudaEventRecord(m->ev_reset[0], st));
     for (unsigned long long wv = 0; wv < n_waves + kDrain; ++wv, ++it, p ^= 1) {
       const bool tw = timed && it < (unsigned long long)kMaxTimedWaves;
       cudaEvent_t* ev = tw ? m->wave_ev + kEvPerWave * it : nullptr;
-      k_iter_begin<<<1, 32, 0, st>>>(m->ctr, p ^ 1);
-      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[0], st));
       if (wv < n_waves) {
         const unsigned int w0 = (unsigned int)(wv * wave);
         const unsigned int wn = (unsigned int)std::min<unsigned long long>(wave, cn - wv * wave);
-        k_seed<<<(wn + kSeedBlock - 1) / kSeedBlock, kSeedBlock, 0, st>>>(rcc, w0, wn, Q[p], cap, m->ctr + 2 * p + 1,
-                                                                         m->stats);
+        TPMC_CUDA_TRY(cudaStreamWaitEvent(s2, m->ev_reset[wv & 3], 0));
+        if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[0], s2));
+        k_seed<<<(wn + kSeedBlock - 1) / kSeedBlock, kSeedBlock, 0, s2>>>(rcc, w0, wn, m->cull, Q[p], cap,
+                                                                         m->ctr + 2 * p + 1, m->stats);
+        if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[1], s2));
+        TPMC_CUDA_TRY(cudaEventRecord(m->ev_seeded[wv & 3], s2));
         ++launches;
       }
-      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[1], st));
+      k_iter_begin<<<1, 32, 0, st>>>(m->ctr, p ^ 1);
+      TPMC_CUDA_TRY(cudaEventRecord(m->ev_reset[(wv + 1) & 3], st));
+      if (wv < n_waves) TPMC_CUDA_TRY(cudaStreamWaitEvent(st, m->ev_seeded[wv & 3], 0));
+      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[2], st));
       k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(m->nodes, m->tris, Q[p], cap, m->ctr + 2 * p, m->ctr + 4, m->hit_ray,
                                                   m->hit_cand, m->ctr + 5, m->stats);
-      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[2], st));
+      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[3], st));
       k_reflect<<<g.reflect, kTraceBlock, 0, st>>>(rcc, cap, m->nodes, m->tris, Q[p], m->hit_ray, m->hit_cand, m->ctr + 5,
                                                    Q[p ^ 1], m->ctr + 2 * (p ^ 1), P, m->totals, m->stats, dbg);
-      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[3], st));
+      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[4], st));
       launches += 3;
     }
     // whatever still bounces after the drain iterations is followed to escape thread by thread
@@ -699,6 +744,7 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
   launches += 2;
   m->last_launches = launches;
   m->last_timed_waves = timed ? std::min<unsigned long long>(it, kMaxTimedWaves) : 0;
+  m->last_seed_waves = (params->count <= kChunk) ? (params->count + wave - 1) / wave : 0;   // seed events exist for these
   TPMC_CUDA_TRY(cudaGetLastError());
   TPMC_CUDA_TRY(cudaEventRecord(m->ev1, st));
   if (h_stats) {

@@ -73,12 +73,12 @@ TPMC_HD double sample_normal_speed(double u, double s) {
   return x;
 }
 
-// ---- fast path: fp32 Newton to ~1e-6, two fp64 Newton steps, convergence check -----------------------
+// ---- fast path: fp32 Newton to ~1e-7, one fp64 Halley step, convergence check -------------------------
 // Root-finding in fp64 costs ~150 instructions per step and its iteration count differs from lane to
-// lane.  The first digits are therefore found in fp32 (erfcf/expf, a fixed number of steps), then two
-// fp64 steps square the error twice.  If the last fp64 step is not already below 1e-8 (ill-conditioned
-// tails, a poor start) the general solvers above take over from the current point: the result is the
-// same root either way.
+// lane.  The first digits are therefore found in fp32 (erfcf/expf, a fixed number of steps), then one
+// cubically convergent fp64 step cubes the error.  If that step is longer than 3e-6 (ill-conditioned
+// tails, a poor start: 1-6 % of the variates) fp64 Newton continues from the current point until a step
+// falls below 1e-8: the result is the same root either way.
 #define TPMC_SQRTPI_F 1.7724538509055160f
 
 TPMC_HD double sample_sin_phi_fast(double u, const SpeciesConst& sc) {
@@ -104,28 +104,29 @@ TPMC_HD double sample_sin_phi_fast(double u, const SpeciesConst& sc) {
     const float d = e + TPMC_SQRTPI_F * y * ec;
     y = fminf(Sf, fmaxf(-Sf, y - (g - T) / d));
   }
-  double yd = (double)y, step = 0.0;
-#pragma unroll
-  for (int it = 0; it < 2; ++it) {
+  // one fp64 Halley step (cubic): from an fp32-converged start (error ~1e-7) it lands at rounding level.
+  // The step length measures the start error; if it is not small the Newton loop below finishes the job.
+  double yd = (double)y;
+  {
+    const double e = exp(-yd * yd);
+    const double ec = erfc(-yd);
+    const double f = 0.25 * TPMC_SQRTPI * (1.0 + 2.0 * yd * yd) * ec + 0.5 * yd * e - target;
+    const double d1 = e + TPMC_SQRTPI * yd * ec;       // G' = chi
+    const double d2 = TPMC_SQRTPI * ec;                // G''
+    const double yn = fmin(S, fmax(-S, yd - 2.0 * f * d1 / (2.0 * d1 * d1 - f * d2)));
+    const double step = fabs(yn - yd);
+    yd = yn;
+    if (step <= 3e-6 * fmax(1.0, fabs(yd))) return fmin(1.0, fmax(-1.0, yd / S));
+  }
+  for (int it = 0; it < 64; ++it) {   // general solver, continued from yd; a step below 1e-8 squares to < 1e-16
     const double e = exp(-yd * yd);
     const double ec = erfc(-yd);
     const double g = 0.25 * TPMC_SQRTPI * (1.0 + 2.0 * yd * yd) * ec + 0.5 * yd * e;
     const double d = e + TPMC_SQRTPI * yd * ec;
     const double yn = fmin(S, fmax(-S, yd - (g - target) / d));
-    step = fabs(yn - yd);
+    const double step = fabs(yn - yd);
     yd = yn;
-  }
-  if (!(step <= 1e-8 * fmax(1.0, fabs(yd)))) {
-    for (int it = 0; it < 64; ++it) {   // general solver, continued from yd
-      const double e = exp(-yd * yd);
-      const double ec = erfc(-yd);
-      const double g = 0.25 * TPMC_SQRTPI * (1.0 + 2.0 * yd * yd) * ec + 0.5 * yd * e;
-      const double d = e + TPMC_SQRTPI * yd * ec;
-      const double yn = fmin(S, fmax(-S, yd - (g - target) / d));
-      step = fabs(yn - yd);
-      yd = yn;
-      if (step <= 4e-16 * fmax(1.0, fabs(yd))) break;
-    }
+    if (step <= 1e-8 * fmax(1.0, fabs(yd))) break;
   }
   return fmin(1.0, fmax(-1.0, yd / S));
 }
@@ -155,28 +156,28 @@ TPMC_HD double sample_normal_speed_fast(double u, double s) {
     if (!(xn > 0.0f)) xn = 0.5f * x;
     x = xn;
   }
-  double xd = (double)x, step = 0.0;
-#pragma unroll
-  for (int it = 0; it < 2; ++it) {
+  double xd = (double)x;
+  {  // one fp64 Halley step, as above: f = Q - target, f' = -2x e^{-z^2}, f'' = -2 e^{-z^2} (1 - 2 x z)
+    const double z = xd - s;
+    const double e = exp(-z * z);
+    const double f = e + TPMC_SQRTPI * s * erfc(z) - target;
+    const double d1 = -2.0 * xd * e;
+    const double d2 = -2.0 * e * (1.0 - 2.0 * xd * z);
+    double xn = xd - 2.0 * f * d1 / (2.0 * d1 * d1 - f * d2);
+    if (!(xn > 0.0) || !(xn < 1e300)) xn = 0.5 * xd;
+    const double step = fabs(xn - xd);
+    xd = xn;
+    if (step <= 3e-6 * (1.0 + xd)) return xd;
+  }
+  for (int it = 0; it < 96; ++it) {   // general solver, continued from xd
     const double z = xd - s;
     const double e = exp(-z * z);
     const double q = e + TPMC_SQRTPI * s * erfc(z);
     double xn = xd + (q - target) / (2.0 * xd * e);
-    if (!(xn > 0.0)) xn = 0.5 * xd;
-    step = fabs(xn - xd);
+    if (!(xn > 0.0) || !(xn < 1e300)) xn = (xn > 0.0) ? 0.5 * (s > 0.0 ? s : 0.0) + 0.35 : 0.5 * xd;
+    const double step = fabs(xn - xd);
     xd = xn;
-  }
-  if (!(step <= 1e-8 * (1.0 + xd))) {
-    for (int it = 0; it < 96; ++it) {   // general solver, continued from xd
-      const double z = xd - s;
-      const double e = exp(-z * z);
-      const double q = e + TPMC_SQRTPI * s * erfc(z);
-      double xn = xd + (q - target) / (2.0 * xd * e);
-      if (!(xn > 0.0) || !(xn < 1e300)) xn = (xn > 0.0) ? 0.5 * (s > 0.0 ? s : 0.0) + 0.35 : 0.5 * xd;
-      step = fabs(xn - xd);
-      xd = xn;
-      if (step <= 4e-16 * (1.0 + xd)) break;
-    }
+    if (step <= 1e-8 * (1.0 + xd)) break;
   }
   return xd;
 }

@@ -20,11 +20,21 @@
 
 #include "common.cuh"
 
+#ifndef TPMC_STACK_SMEM
 #define TPMC_STACK_SMEM 24      // stack entries per thread kept in shared memory
+#endif
 #define TPMC_STACK_LOCAL 80     // overflow entries (a Karras tree over 64-bit keys + index is <= 97 deep)
 #define TPMC_SENTINEL ((int)0x7FFFFFFF)
 #define TPMC_MAX_CAND 4
 #define TPMC_CAND_OVERFLOW ((int)0x7FFFFFFE)   // in cand.w: more candidates than slots -> full fp64 traversal
+
+// 256-bit read-only load (sm_100: LDG.E.256): one L1 sector per lane per instruction instead of half a
+// sector -- the traversal is bound by L1 tag lookups of divergent 64-byte node fetches.
+__device__ __forceinline__ void ldg256(const float4* p, float4& a, float4& b) {
+  asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w), "=f"(b.x), "=f"(b.y), "=f"(b.z), "=f"(b.w)
+               : "l"(p));
+}
 
 struct Hit {
   double tau;   // +inf: no hit
@@ -158,6 +168,47 @@ __device__ __forceinline__ bool slab(float lx, float ly, float lz, float hx, flo
   return fmaxf(tn, 0.0f) <= fminf(tf, tmax);
 }
 
+// ---- seed-time cull: can the ray touch any cut-off subtree of the top tree? (conservative) ------------
+// Near child first, so the first cut-off box found is (nearly) the first along the ray; its entry
+// distance is returned and later gives the ray its sort key (a point close to where it will hit).
+__device__ __forceinline__ bool cull_touch(const float4* __restrict__ cull, const float o[3], const float id[3],
+                                           float& t_entry) {
+  int stack[24];
+  int sp = 0, node = 0;
+  t_entry = 0.0f;
+  for (;;) {
+    const float4* np = cull + 4 * node;
+    float4 n0, n1, n2, n3;
+    ldg256(np, n0, n1);
+    ldg256(np + 2, n2, n3);
+    float t0, t1;
+    bool h0 = slab(n0.x, n0.y, n0.z, n0.w, n1.x, n1.y, o, id, INFINITY, t0);
+    bool h1 = slab(n1.z, n1.w, n2.x, n2.y, n2.z, n2.w, o, id, INFINITY, t1);
+    int c0 = __float_as_int(n3.x), c1 = __float_as_int(n3.y);
+    if (h0 && h1 && t1 < t0) {
+      const int c = c0; c0 = c1; c1 = c;
+      const float t = t0; t0 = t1; t1 = t;
+    } else if (!h0 && h1) {
+      c0 = c1; t0 = t1; h0 = true; h1 = false;
+    }
+    if (h0 && c0 < 0) { t_entry = fmaxf(t0, 0.0f); return true; }
+    if (h0) {
+      if (h1) {
+        if (sp >= 24) { t_entry = fmaxf(t0, 0.0f); return true; }   // deeper than the stack: keep the ray
+        stack[sp++] = c1 < 0 ? (int)(0x80000000u | (__float_as_uint(fmaxf(t1, 0.0f)) >> 1)) : c1;
+      }
+      node = c0;
+    } else {
+      if (sp == 0) return false;
+      node = stack[--sp];
+    }
+    if (node < 0) {   // a cut-off box that was pushed as the far child: reached now
+      t_entry = __uint_as_float(((unsigned)node & 0x7FFFFFFFu) << 1);
+      return true;
+    }
+  }
+}
+
 // ---- per-ray traversal state of the wavefront kernel -------------------------------------------------
 struct Walk {
   float o[3], d[3], id[3];
@@ -217,42 +268,46 @@ __device__ __forceinline__ void walk_add_candidate(Walk& w, int slot, int cls, f
   ++w.nc;
 }
 
-// One traversal step: an internal node (two slab tests) or a leaf (one fp32 facet classification).
-__device__ __forceinline__ void walk_step(Walk& w, const float4* __restrict__ nodes, const float4* __restrict__ tris,
-                                          int* stk, int sstride, int* lstack, TraceCounters& cnt) {
-  if (w.cur >= 0) {
-    const float4* np = nodes + 4 * (size_t)w.cur;
-    const float4 n0 = __ldg(np + 0), n1 = __ldg(np + 1), n2 = __ldg(np + 2), n3 = __ldg(np + 3);
-    ++cnt.nodes;
-    float t0, t1;
-    const bool h0 = slab(n0.x, n0.y, n0.z, n0.w, n1.x, n1.y, w.o, w.id, w.tmax, t0);
-    const bool h1 = slab(n1.z, n1.w, n2.x, n2.y, n2.z, n2.w, w.o, w.id, w.tmax, t1);
-    int c0 = __float_as_int(n3.x), c1 = __float_as_int(n3.y);
-    if (h0 && h1) {
-      if (t1 < t0) { const int t = c0; c0 = c1; c1 = t; }
-      if (w.sp < TPMC_STACK_SMEM) stk[w.sp * sstride] = c1; else lstack[w.sp - TPMC_STACK_SMEM] = c1;
-      ++w.sp;
-      w.cur = c0;
-    } else if (h0) {
-      w.cur = c0;
-    } else if (h1) {
-      w.cur = c1;
-    } else {
-      w.cur = walk_pop(w, stk, sstride, lstack);
-    }
+// One internal-node step (two slab tests, push the far child) -- requires w.cur >= 0 and != SENTINEL.
+__device__ __forceinline__ void walk_node(Walk& w, const float4* __restrict__ nodes, int* stk, int sstride,
+                                          int* lstack, TraceCounters& cnt) {
+  const float4* np = nodes + 4 * (size_t)w.cur;
+  float4 n0, n1, n2, n3;
+  ldg256(np, n0, n1);
+  ldg256(np + 2, n2, n3);
+  ++cnt.nodes;
+  float t0, t1;
+  const bool h0 = slab(n0.x, n0.y, n0.z, n0.w, n1.x, n1.y, w.o, w.id, w.tmax, t0);
+  const bool h1 = slab(n1.z, n1.w, n2.x, n2.y, n2.z, n2.w, w.o, w.id, w.tmax, t1);
+  int c0 = __float_as_int(n3.x), c1 = __float_as_int(n3.y);
+  if (h0 && h1) {
+    if (t1 < t0) { const int t = c0; c0 = c1; c1 = t; }
+    if (w.sp < TPMC_STACK_SMEM) stk[w.sp * sstride] = c1; else lstack[w.sp - TPMC_STACK_SMEM] = c1;
+    ++w.sp;
+    w.cur = c0;
+  } else if (h0) {
+    w.cur = c0;
+  } else if (h1) {
+    w.cur = c1;
   } else {
-    const int slot = ~w.cur;
-    const float4 q0 = __ldg(tris + 3 * (size_t)slot + 0);
-    if (__float_as_int(q0.w) != w.f_prev) {
-      const float4 q1 = __ldg(tris + 3 * (size_t)slot + 1);
-      const float4 q2 = __ldg(tris + 3 * (size_t)slot + 2);
-      ++cnt.tris;
-      float tlo, thi;
-      const int cls = tri_filter(q0, q1, q2, w.o, w.d, tlo, thi);
-      if (cls != TRI_MISS) walk_add_candidate(w, slot, cls, tlo, thi);
-    }
     w.cur = walk_pop(w, stk, sstride, lstack);
   }
+}
+
+// One leaf step (fp32 facet classification) -- requires w.cur < 0.
+__device__ __forceinline__ void walk_leaf(Walk& w, const float4* __restrict__ tris, int* stk, int sstride,
+                                          int* lstack, TraceCounters& cnt) {
+  const int slot = ~w.cur;
+  const float4 q0 = __ldg(tris + 3 * (size_t)slot + 0);
+  if (__float_as_int(q0.w) != w.f_prev) {
+    const float4 q1 = __ldg(tris + 3 * (size_t)slot + 1);
+    const float4 q2 = __ldg(tris + 3 * (size_t)slot + 2);
+    ++cnt.tris;
+    float tlo, thi;
+    const int cls = tri_filter(q0, q1, q2, w.o, w.d, tlo, thi);
+    if (cls != TRI_MISS) walk_add_candidate(w, slot, cls, tlo, thi);
+  }
+  w.cur = walk_pop(w, stk, sstride, lstack);
 }
 
 // ---- exact closest hit by a full fp64 traversal (stragglers, candidate overflow) ----------------------
