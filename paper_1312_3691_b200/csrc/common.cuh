@@ -65,7 +65,7 @@ constexpr int kMaxTimedWaves = 1024;  // iterations covered by the per-kernel ev
 constexpr int kDrain = 3;             // trace/reflect iterations after the last wave, before the straggler kernel
 constexpr int kEvPerWave = 5;         // seed start/end (seed stream), trace start, after trace, after reflect
 constexpr int kCtrWords = 8;
-constexpr int kCullNodes = 1024;      // 64 KB: stays in L1 next to the shared-memory carve-out
+constexpr int kCullNodes = 64;        // 64 KB: stays in L1 next to the shared-memory carve-out
 
 // Per-run constants (a1: host, fp64), passed to kernels by value.
 struct SpeciesConst {

@@ -6,6 +6,9 @@
 // Everything runs on the device; there is no host build path.
 #include <cub/device/device_radix_sort.cuh>
 
+#include <algorithm>
+#include <cstdlib>
+
 #include "common.cuh"
 
 thread_local char g_tpmc_cuda_error[512] = "";
@@ -321,7 +324,9 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
   DevBuf cq;
   MESH_TRY(cudaMalloc((void**)&m->cull, sizeof(float4) * 4 * kCullNodes));
   MESH_TRY(cudaMalloc(&cq.p, sizeof(int) * (kCullNodes + 1)));
-  k_build_cull<<<1, 32, 0, st>>>(m->nodes, m->cull, cq.as<int>(), kCullNodes, cq.as<int>() + kCullNodes);
+  int cull_budget = kCullNodes;
+  if (const char* e = getenv("TPMC_CULL_NODES")) cull_budget = std::max(1, std::min(kCullNodes, atoi(e)));   // tuning aid
+  k_build_cull<<<1, 32, 0, st>>>(m->nodes, m->cull, cq.as<int>(), cull_budget, cq.as<int>() + kCullNodes);
   MESH_TRY(cudaMemcpyAsync(&m->n_cull, cq.as<int>() + kCullNodes, sizeof(int), cudaMemcpyDeviceToHost, st));
   MESH_TRY(cudaGetLastError());
   MESH_TRY(cudaEventRecord(e1, st));

@@ -703,7 +703,8 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
     // The seed kernel of wave w+1 (fp64/ALU bound) runs on a second stream next to the trace and reflect
     // kernels of wave w (latency/L1 bound): it only touches region B of the other queue and its counter,
     // which k_iter_begin(w) has reset.  ev_reset / ev_seeded order the two streams.
-    cudaStream_t s2 = m->seed_stream;
+    static const bool no_overlap = getenv("TPMC_NO_OVERLAP") != nullptr;   // diagnosis: everything on one stream
+    cudaStream_t s2 = no_overlap ? st : m->seed_stream;
     int p = 0;
     TPMC_CUDA_TRY(cudaEventRecord(m->ev_reset[0], st));
     for (unsigned long long wv = 0; wv < n_waves + kDrain; ++wv, ++it, p ^= 1) {

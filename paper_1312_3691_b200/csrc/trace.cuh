@@ -154,6 +154,9 @@ __device__ __forceinline__ int tri_filter(const float4 q0, const float4 q1, cons
 // Each plane distance (lo - o) * (1/d) carries three roundings: relative error <= 3 * 2^-24.  min/max are
 // exact and x -> x -+ 4u|x| is monotone, so one margin on the entry and one on the exit make the test
 // conservative.  NaN (0 * inf when d = 0 and o on the plane) is dropped by fminf/fmaxf.
+// (The one-FMA form fma(l, 1/d, -o/d) was tried and rejected: its error is absolute, ~u|o/d|, so a ray
+// with one tiny direction component needs a margin that inflates every box and walks thousands of nodes.
+// Carrying the entry distance on the stack to skip stale entries was tried too: no fewer node visits.)
 __device__ __forceinline__ bool slab(float lx, float ly, float lz, float hx, float hy, float hz, const float o[3],
                                      const float id[3], float tmax, float& tnear) {
   const float u4 = 2.384185791015625e-07f;  // 4 * 2^-24
