@@ -26,6 +26,24 @@ extern thread_local char g_tpmc_cuda_error[512];
   } while (0)
 
 // ---------------------------------------------------------------------------------------------
+// One wave pipeline: queues, hit list, counters, its two streams and the events that order them.
+// Waves are dealt round-robin to kPipes pipelines that run concurrently: every kernel of the path is
+// latency bound on its own, so a second, independent chain of kernels fills the idle issue slots.
+constexpr int kPipes = 1;   // two concurrent pipelines were measured: no gain once seeding overlaps trace/reflect
+struct Pipe {
+  float4* q_o[2];                  // ray queues (ping-pong between iterations), regions A|B of wave_cap rays each
+  float4* q_v[2];
+  int* q_f[2];
+  unsigned int* hit_ray;           // [2*wave_cap] queue slot of every ray that ended with candidate facets
+  int4* hit_cand;                  // [2*wave_cap] its candidate triangle slots
+  unsigned int* ctr;               // [kCtrWords] device counters (queue sizes, fetch head, hit count)
+  cudaStream_t main, seed;         // trace/reflect chain; seed kernel of the next wave (pipe 0: main = caller's)
+  cudaEvent_t ev_reset[4], ev_seeded[4], ev_done, ev_f0, ev_f1;
+  cudaEvent_t* wave_ev;            // [kEvPerWave*kMaxTimedWaves] per-kernel timing, created on first use
+  unsigned long long iters, seed_iters;   // of the last run: iterations / seeded iterations with timing events
+};
+
+// ---------------------------------------------------------------------------------------------
 // Device-resident body.  nodes: 4 float4 per internal node (two child boxes + two child refs);
 // tris: 3 float4 per triangle in Morton order: (p0, facet id), (p1, flags), (p2, 0).
 struct tpmc_mesh {
@@ -42,23 +60,13 @@ struct tpmc_mesh {
   int device;
   // per-run scratch, cached in the handle (one run at a time per handle)
   size_t wave_cap;
-  float4* q_o[2];                  // ray queues A/B (ping-pong between wavefront rounds)
-  float4* q_v[2];
-  int* q_f[2];
-  unsigned int* hit_ray;           // [wave_cap] ray index of every ray that ended with candidate facets
-  int4* hit_cand;                  // [wave_cap] its candidate slots
-  unsigned int* ctr;               // [kCtrWords] per-wave device counters (queue sizes, fetch heads, hit counts)
+  Pipe pipe[kPipes];
   double* facet_scratch;           // [nt][3] when the caller passes no per-facet buffer
   double* partials;                // reduction partials
   unsigned long long* stats;       // [8] device counters
   double* totals;                  // [3] torque accumulators
-  cudaEvent_t ev0, ev1, ev2, ev3;
-  cudaStream_t seed_stream;        // the seed kernel of the next wave runs here, beside trace/reflect
-  cudaEvent_t ev_reset[4], ev_seeded[4];
-  unsigned long long last_seed_waves;
-  cudaEvent_t* wave_ev;            // [kEvPerWave*kMaxTimedWaves] per-kernel timing, created on first use
+  cudaEvent_t ev0, ev1, ev_fork;
   unsigned long long last_launches;
-  unsigned long long last_timed_waves;
 };
 
 constexpr int kMaxTimedWaves = 1024;  // iterations covered by the per-kernel event times

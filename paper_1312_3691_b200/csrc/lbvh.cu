@@ -278,7 +278,6 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
   for (int a = 0; a < 3; ++a) { m->centre[a] = centre[a]; m->aabb_lo[a] = h.aabb[a]; m->aabb_hi[a] = h.aabb[3 + a]; }
   m->Rb = sqrt(h.r2);
   m->ev0 = e0; m->ev1 = e1;
-  cudaEventCreate(&m->ev2); cudaEventCreate(&m->ev3);
 
 #define MESH_TRY(expr)                       \
   do {                                       \
@@ -342,22 +341,28 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
 extern "C" void tpmc_mesh_destroy(tpmc_mesh* m) {
   if (!m) return;
   cudaFree(m->nodes); cudaFree(m->tris); cudaFree(m->cull);
-  for (int k = 0; k < 2; ++k) { cudaFree(m->q_o[k]); cudaFree(m->q_v[k]); cudaFree(m->q_f[k]); }
-  cudaFree(m->hit_ray); cudaFree(m->hit_cand); cudaFree(m->ctr);
-  if (m->seed_stream) cudaStreamDestroy(m->seed_stream);
-  for (int k = 0; k < 4; ++k) {
-    if (m->ev_reset[k]) cudaEventDestroy(m->ev_reset[k]);
-    if (m->ev_seeded[k]) cudaEventDestroy(m->ev_seeded[k]);
+  for (int pi = 0; pi < kPipes; ++pi) {
+    Pipe& pp = m->pipe[pi];
+    for (int k = 0; k < 2; ++k) { cudaFree(pp.q_o[k]); cudaFree(pp.q_v[k]); cudaFree(pp.q_f[k]); }
+    cudaFree(pp.hit_ray); cudaFree(pp.hit_cand); cudaFree(pp.ctr);
+    if (pi > 0 && pp.main) cudaStreamDestroy(pp.main);
+    if (pp.seed) cudaStreamDestroy(pp.seed);
+    for (int k = 0; k < 4; ++k) {
+      if (pp.ev_reset[k]) cudaEventDestroy(pp.ev_reset[k]);
+      if (pp.ev_seeded[k]) cudaEventDestroy(pp.ev_seeded[k]);
+    }
+    if (pp.ev_done) cudaEventDestroy(pp.ev_done);
+    if (pp.ev_f0) cudaEventDestroy(pp.ev_f0);
+    if (pp.ev_f1) cudaEventDestroy(pp.ev_f1);
+    if (pp.wave_ev) {
+      for (int i = 0; i < kEvPerWave * kMaxTimedWaves; ++i) cudaEventDestroy(pp.wave_ev[i]);
+      delete[] pp.wave_ev;
+    }
   }
   cudaFree(m->facet_scratch); cudaFree(m->partials); cudaFree(m->stats); cudaFree(m->totals);
-  if (m->wave_ev) {
-    for (int i = 0; i < kEvPerWave * kMaxTimedWaves; ++i) cudaEventDestroy(m->wave_ev[i]);
-    delete[] m->wave_ev;
-  }
   if (m->ev0) cudaEventDestroy(m->ev0);
   if (m->ev1) cudaEventDestroy(m->ev1);
-  if (m->ev2) cudaEventDestroy(m->ev2);
-  if (m->ev3) cudaEventDestroy(m->ev3);
+  if (m->ev_fork) cudaEventDestroy(m->ev_fork);
   delete m;
 }
 

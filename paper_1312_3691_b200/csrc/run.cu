@@ -560,32 +560,46 @@ size_t wave_size() {
 }
 
 int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
-  if (!m->ctr) {
-    TPMC_CUDA_TRY(cudaStreamCreateWithFlags(&m->seed_stream, cudaStreamNonBlocking));
-    for (int k = 0; k < 4; ++k) {
-      TPMC_CUDA_TRY(cudaEventCreateWithFlags(&m->ev_reset[k], cudaEventDisableTiming));
-      TPMC_CUDA_TRY(cudaEventCreateWithFlags(&m->ev_seeded[k], cudaEventDisableTiming));
-    }
-    TPMC_CUDA_TRY(cudaMalloc((void**)&m->ctr, kCtrWords * sizeof(unsigned int)));
+  if (!m->stats) {
     TPMC_CUDA_TRY(cudaMalloc((void**)&m->stats, ST_COUNT * sizeof(unsigned long long)));
     TPMC_CUDA_TRY(cudaMalloc((void**)&m->totals, 4 * sizeof(double)));
     TPMC_CUDA_TRY(cudaMalloc((void**)&m->partials, 3 * kReduceParts * sizeof(double)));
+    TPMC_CUDA_TRY(cudaEventCreateWithFlags(&m->ev_fork, cudaEventDisableTiming));
+    for (int pi = 0; pi < kPipes; ++pi) {
+      Pipe& pp = m->pipe[pi];
+      if (pi > 0) TPMC_CUDA_TRY(cudaStreamCreateWithFlags(&pp.main, cudaStreamNonBlocking));
+      TPMC_CUDA_TRY(cudaStreamCreateWithFlags(&pp.seed, cudaStreamNonBlocking));
+      for (int k = 0; k < 4; ++k) {
+        TPMC_CUDA_TRY(cudaEventCreateWithFlags(&pp.ev_reset[k], cudaEventDisableTiming));
+        TPMC_CUDA_TRY(cudaEventCreateWithFlags(&pp.ev_seeded[k], cudaEventDisableTiming));
+      }
+      TPMC_CUDA_TRY(cudaEventCreateWithFlags(&pp.ev_done, cudaEventDisableTiming));
+      TPMC_CUDA_TRY(cudaEventCreate(&pp.ev_f0));
+      TPMC_CUDA_TRY(cudaEventCreate(&pp.ev_f1));
+      TPMC_CUDA_TRY(cudaMalloc((void**)&pp.ctr, kCtrWords * sizeof(unsigned int)));
+    }
   }
   if (m->wave_cap < wave) {
-    for (int k = 0; k < 2; ++k) {
-      cudaFree(m->q_o[k]); cudaFree(m->q_v[k]); cudaFree(m->q_f[k]);
-      m->q_o[k] = m->q_v[k] = nullptr; m->q_f[k] = nullptr;
+    for (int pi = 0; pi < kPipes; ++pi) {
+      Pipe& pp = m->pipe[pi];
+      for (int k = 0; k < 2; ++k) {
+        cudaFree(pp.q_o[k]); cudaFree(pp.q_v[k]); cudaFree(pp.q_f[k]);
+        pp.q_o[k] = pp.q_v[k] = nullptr; pp.q_f[k] = nullptr;
+      }
+      cudaFree(pp.hit_ray); cudaFree(pp.hit_cand);
+      pp.hit_ray = nullptr; pp.hit_cand = nullptr;
     }
-    cudaFree(m->hit_ray); cudaFree(m->hit_cand);
-    m->hit_ray = nullptr; m->hit_cand = nullptr;
     m->wave_cap = 0;
-    for (int k = 0; k < 2; ++k) {
-      TPMC_CUDA_TRY(cudaMalloc((void**)&m->q_o[k], 2 * wave * sizeof(float4)));   // regions A and B
-      TPMC_CUDA_TRY(cudaMalloc((void**)&m->q_v[k], 2 * wave * sizeof(float4)));
-      TPMC_CUDA_TRY(cudaMalloc((void**)&m->q_f[k], 2 * wave * sizeof(int)));
+    for (int pi = 0; pi < kPipes; ++pi) {
+      Pipe& pp = m->pipe[pi];
+      for (int k = 0; k < 2; ++k) {
+        TPMC_CUDA_TRY(cudaMalloc((void**)&pp.q_o[k], 2 * wave * sizeof(float4)));   // regions A and B
+        TPMC_CUDA_TRY(cudaMalloc((void**)&pp.q_v[k], 2 * wave * sizeof(float4)));
+        TPMC_CUDA_TRY(cudaMalloc((void**)&pp.q_f[k], 2 * wave * sizeof(int)));
+      }
+      TPMC_CUDA_TRY(cudaMalloc((void**)&pp.hit_ray, 2 * wave * sizeof(unsigned int)));
+      TPMC_CUDA_TRY(cudaMalloc((void**)&pp.hit_cand, 2 * wave * sizeof(int4)));
     }
-    TPMC_CUDA_TRY(cudaMalloc((void**)&m->hit_ray, 2 * wave * sizeof(unsigned int)));
-    TPMC_CUDA_TRY(cudaMalloc((void**)&m->hit_cand, 2 * wave * sizeof(int4)));
     m->wave_cap = wave;
   }
   if (need_facets && !m->facet_scratch)
@@ -593,19 +607,22 @@ int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
   return TPMC_OK;
 }
 
-struct Grids { int trace, reflect, finish; };
+struct Grids { int trace, reflect, finish, pipes; };
 const Grids& grids() {
-  static Grids g = {0, 0, 0};
+  static Grids g = {0, 0, 0, 0};
   if (!g.trace) {
     int dev = 0, sms = 148, per = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    g.pipes = kPipes;
+    if (const char* e = getenv("TPMC_PIPES")) g.pipes = std::max(1, std::min(kPipes, atoi(e)));   // tuning aid
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_trace_wf, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
-    if (const char* e = getenv("TPMC_TRACE_BLOCKS")) per = std::max(1, std::min(per, atoi(e)));
-    else per = std::max(1, per - 2);   // leave room for the seed kernel of the next wave
-    g.trace = sms * per;
+    // resident trace CTAs per SM over all pipelines; the rest of the SM is left to the seed and reflect kernels
+    int tot = std::max(1, per - 2);
+    if (const char* e = getenv("TPMC_TRACE_BLOCKS")) tot = std::max(1, std::min(per, atoi(e)));
+    g.trace = sms * std::max(1, tot / g.pipes);
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_reflect, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
-    g.reflect = sms * per;
+    g.reflect = sms * std::max(1, per / g.pipes);
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_finish, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
     g.finish = sms * per;
   }
@@ -627,25 +644,32 @@ int fill_stats(tpmc_mesh* m, const tpmc_params* params, tpmc_stats* h_stats) {
   h_stats->kernel_launches = m->last_launches;
   h_stats->ms = ms;
   h_stats->ms_seed = h_stats->ms_trace = h_stats->ms_reflect = h_stats->ms_finish = 0.0;
-  h_stats->timed_waves = m->last_timed_waves;
-  h_stats->trace_launches = m->last_timed_waves;
+  h_stats->timed_waves = 0;
+  h_stats->trace_launches = 0;
   h_stats->traced_rays = hs[ST_TRACED];
-  for (unsigned long long w = 0; w < m->last_timed_waves; ++w) {
-    const cudaEvent_t* ev = m->wave_ev + kEvPerWave * w;
-    float t = 0.0f;
-    if (w < m->last_seed_waves) {
-      TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[0], ev[1]));
-      h_stats->ms_seed += t;
+  // Kernels of different pipelines and streams overlap: these are sums of per-launch durations, not a
+  // partition of `ms`.
+  for (int pi = 0; pi < kPipes; ++pi) {
+    const Pipe& pp = m->pipe[pi];
+    for (unsigned long long w = 0; w < pp.iters; ++w) {
+      const cudaEvent_t* ev = pp.wave_ev + kEvPerWave * w;
+      float t = 0.0f;
+      if (w < pp.seed_iters) {
+        TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[0], ev[1]));
+        h_stats->ms_seed += t;
+      }
+      TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[2], ev[3]));
+      h_stats->ms_trace += t;
+      TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[3], ev[4]));
+      h_stats->ms_reflect += t;
     }
-    TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[2], ev[3]));
-    h_stats->ms_trace += t;
-    TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[3], ev[4]));
-    h_stats->ms_reflect += t;
-  }
-  if (m->last_timed_waves) {
-    float t = 0.0f;
-    TPMC_CUDA_TRY(cudaEventElapsedTime(&t, m->ev2, m->ev3));
-    h_stats->ms_finish = t;
+    h_stats->timed_waves += pp.seed_iters;
+    h_stats->trace_launches += pp.iters;
+    if (pp.iters) {
+      float t = 0.0f;
+      TPMC_CUDA_TRY(cudaEventElapsedTime(&t, pp.ev_f0, pp.ev_f1));
+      h_stats->ms_finish += t;
+    }
   }
   return TPMC_OK;
 }
@@ -668,6 +692,20 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
   tpmc_debug dbg0 = {nullptr, nullptr, nullptr};
   if (debug) dbg0 = *debug;
   const bool any_dbg = dbg0.hash || dbg0.bounces || dbg0.first_facet;
+  const Grids& g = grids();
+  const int K = g.pipes;
+  static const bool no_overlap = getenv("TPMC_NO_OVERLAP") != nullptr;   // diagnosis: one stream only
+  const bool timed = (h_stats != nullptr);   // per-kernel events only when the caller will read them
+  m->pipe[0].main = st;
+  for (int pi = 0; pi < kPipes; ++pi) {
+    Pipe& pp = m->pipe[pi];
+    pp.iters = pp.seed_iters = 0;
+    if (timed && !pp.wave_ev) {
+      pp.wave_ev = new (std::nothrow) cudaEvent_t[kEvPerWave * kMaxTimedWaves];
+      if (!pp.wave_ev) return TPMC_ENOMEM;
+      for (int i = 0; i < kEvPerWave * kMaxTimedWaves; ++i) TPMC_CUDA_TRY(cudaEventCreate(&pp.wave_ev[i]));
+    }
+  }
 
   TPMC_CUDA_TRY(cudaEventRecord(m->ev0, st));
   TPMC_CUDA_TRY(cudaMemsetAsync(P, 0, 3 * sizeof(double) * (size_t)m->nt, st));
@@ -675,15 +713,8 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
   TPMC_CUDA_TRY(cudaMemsetAsync(m->totals, 0, 4 * sizeof(double), st));
   if (any_dbg && params->count)
     k_init_debug<<<(unsigned)((params->count + 255) / 256), 256, 0, st>>>(dbg0, params->count);
-  const Grids& g = grids();
-  const bool timed = (h_stats != nullptr);   // per-kernel events only when the caller will read them
-  if (timed && !m->wave_ev) {
-    m->wave_ev = new (std::nothrow) cudaEvent_t[kEvPerWave * kMaxTimedWaves];
-    if (!m->wave_ev) return TPMC_ENOMEM;
-    for (int i = 0; i < kEvPerWave * kMaxTimedWaves; ++i) TPMC_CUDA_TRY(cudaEventCreate(&m->wave_ev[i]));
-  }
-  unsigned long long launches = (any_dbg && params->count) ? 1 : 0, it = 0;
-  RayQueue Q[2] = {{m->q_o[0], m->q_v[0], m->q_f[0]}, {m->q_o[1], m->q_v[1], m->q_f[1]}};
+  unsigned long long launches = (any_dbg && params->count) ? 1 : 0;
+
   // Particle indices inside the queues are 32-bit offsets into a chunk of the slice.
   const unsigned long long kChunk = 0xF0000000ull;
   for (unsigned long long c0 = 0; c0 < params->count; c0 += kChunk) {
@@ -695,57 +726,75 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
     if (dbg.hash) dbg.hash += c0;
     if (dbg.bounces) dbg.bounces += c0;
     if (dbg.first_facet) dbg.first_facet += c0;
-    TPMC_CUDA_TRY(cudaMemsetAsync(m->ctr, 0, kCtrWords * sizeof(unsigned int), st));
-    // One iteration per wave: seed the wave into region B of queue p (region A already holds the rays
-    // reflected in the previous iteration), trace the whole queue, reflect the hits into region A of the
-    // other queue.  Particles that keep bouncing ride along with the following waves.
+    // fork: the other pipelines' streams start after everything enqueued so far on the caller's stream
+    TPMC_CUDA_TRY(cudaEventRecord(m->ev_fork, st));
+    for (int pi = 0; pi < K; ++pi) {
+      Pipe& pp = m->pipe[pi];
+      if (pi > 0) TPMC_CUDA_TRY(cudaStreamWaitEvent(pp.main, m->ev_fork, 0));
+      TPMC_CUDA_TRY(cudaMemsetAsync(pp.ctr, 0, kCtrWords * sizeof(unsigned int), pp.main));
+      TPMC_CUDA_TRY(cudaEventRecord(pp.ev_reset[0], pp.main));
+    }
+    // Waves are dealt round-robin to the pipelines.  In a pipeline, one iteration per wave: seed the wave
+    // into region B of queue p (region A already holds the rays reflected in the previous iteration),
+    // trace the whole queue, reflect the hits into region A of the other queue; particles that keep
+    // bouncing ride along with the following waves.  The seed kernel of the pipeline's next wave runs on
+    // its second stream beside trace/reflect: it only touches region B of the other queue and its counter,
+    // which k_iter_begin has reset (ev_reset / ev_seeded order the two streams).
     const unsigned long long n_waves = (cn + wave - 1) / wave;
-    // The seed kernel of wave w+1 (fp64/ALU bound) runs on a second stream next to the trace and reflect
-    // kernels of wave w (latency/L1 bound): it only touches region B of the other queue and its counter,
-    // which k_iter_begin(w) has reset.  ev_reset / ev_seeded order the two streams.
-    static const bool no_overlap = getenv("TPMC_NO_OVERLAP") != nullptr;   // diagnosis: everything on one stream
-    cudaStream_t s2 = no_overlap ? st : m->seed_stream;
-    int p = 0;
-    TPMC_CUDA_TRY(cudaEventRecord(m->ev_reset[0], st));
-    for (unsigned long long wv = 0; wv < n_waves + kDrain; ++wv, ++it, p ^= 1) {
-      const bool tw = timed && it < (unsigned long long)kMaxTimedWaves;
-      cudaEvent_t* ev = tw ? m->wave_ev + kEvPerWave * it : nullptr;
+    for (unsigned long long wv = 0; wv < n_waves + (unsigned long long)K * kDrain; ++wv) {
+      Pipe& pp = m->pipe[wv % K];
+      const unsigned long long li = wv / K;            // iteration index within the pipeline
+      const int p = (int)(li & 1);
+      cudaStream_t s1 = pp.main, s2 = no_overlap ? pp.main : pp.seed;
+      RayQueue Q[2] = {{pp.q_o[0], pp.q_v[0], pp.q_f[0]}, {pp.q_o[1], pp.q_v[1], pp.q_f[1]}};
+      const bool tw = timed && c0 == 0 && li < (unsigned long long)kMaxTimedWaves;
+      cudaEvent_t* ev = tw ? pp.wave_ev + kEvPerWave * li : nullptr;
       if (wv < n_waves) {
         const unsigned int w0 = (unsigned int)(wv * wave);
         const unsigned int wn = (unsigned int)std::min<unsigned long long>(wave, cn - wv * wave);
-        TPMC_CUDA_TRY(cudaStreamWaitEvent(s2, m->ev_reset[wv & 3], 0));
+        TPMC_CUDA_TRY(cudaStreamWaitEvent(s2, pp.ev_reset[li & 3], 0));
         if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[0], s2));
         k_seed<<<(wn + kSeedBlock - 1) / kSeedBlock, kSeedBlock, 0, s2>>>(rcc, w0, wn, m->cull, Q[p], cap,
-                                                                         m->ctr + 2 * p + 1, m->stats);
+                                                                         pp.ctr + 2 * p + 1, m->stats);
         if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[1], s2));
-        TPMC_CUDA_TRY(cudaEventRecord(m->ev_seeded[wv & 3], s2));
+        TPMC_CUDA_TRY(cudaEventRecord(pp.ev_seeded[li & 3], s2));
+        if (tw) pp.seed_iters = li + 1;
         ++launches;
       }
-      k_iter_begin<<<1, 32, 0, st>>>(m->ctr, p ^ 1);
-      TPMC_CUDA_TRY(cudaEventRecord(m->ev_reset[(wv + 1) & 3], st));
-      if (wv < n_waves) TPMC_CUDA_TRY(cudaStreamWaitEvent(st, m->ev_seeded[wv & 3], 0));
-      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[2], st));
-      k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(m->nodes, m->tris, Q[p], cap, m->ctr + 2 * p, m->ctr + 4, m->hit_ray,
-                                                  m->hit_cand, m->ctr + 5, m->stats);
-      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[3], st));
-      k_reflect<<<g.reflect, kTraceBlock, 0, st>>>(rcc, cap, m->nodes, m->tris, Q[p], m->hit_ray, m->hit_cand, m->ctr + 5,
-                                                   Q[p ^ 1], m->ctr + 2 * (p ^ 1), P, m->totals, m->stats, dbg);
-      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[4], st));
-      launches += 3;
+      k_iter_begin<<<1, 32, 0, s1>>>(pp.ctr, p ^ 1);
+      TPMC_CUDA_TRY(cudaEventRecord(pp.ev_reset[(li + 1) & 3], s1));
+      if (wv < n_waves) TPMC_CUDA_TRY(cudaStreamWaitEvent(s1, pp.ev_seeded[li & 3], 0));
+      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[2], s1));
+      k_trace_wf<<<g.trace, kTraceBlock, 0, s1>>>(m->nodes, m->tris, Q[p], cap, pp.ctr + 2 * p, pp.ctr + 4, pp.hit_ray,
+                                                  pp.hit_cand, pp.ctr + 5, m->stats);
+      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[3], s1));
+      k_reflect<<<g.reflect, kTraceBlock, 0, s1>>>(rcc, cap, m->nodes, m->tris, Q[p], pp.hit_ray, pp.hit_cand, pp.ctr + 5,
+                                                   Q[p ^ 1], pp.ctr + 2 * (p ^ 1), P, m->totals, m->stats, dbg);
+      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[4], s1));
+      if (tw) pp.iters = li + 1;
+      launches += 4;
     }
-    // whatever still bounces after the drain iterations is followed to escape thread by thread
-    if (timed) TPMC_CUDA_TRY(cudaEventRecord(m->ev2, st));
-    k_finish<<<g.finish, kTraceBlock, 0, st>>>(rcc, cap, m->nodes, m->tris, Q[p], m->ctr + 2 * p, P, m->totals, m->stats,
-                                               dbg);
-    if (timed) TPMC_CUDA_TRY(cudaEventRecord(m->ev3, st));
-    ++launches;
+    // whatever still bounces after the drain iterations is followed to escape thread by thread; then join
+    for (int pi = 0; pi < K; ++pi) {
+      Pipe& pp = m->pipe[pi];
+      const unsigned long long its = (n_waves + (unsigned long long)K * kDrain - pi + K - 1) / K;   // iterations it ran
+      const int p = (int)(its & 1);
+      RayQueue q = {pp.q_o[p], pp.q_v[p], pp.q_f[p]};
+      if (timed) TPMC_CUDA_TRY(cudaEventRecord(pp.ev_f0, pp.main));
+      k_finish<<<g.finish, kTraceBlock, 0, pp.main>>>(rcc, cap, m->nodes, m->tris, q, pp.ctr + 2 * p, P, m->totals,
+                                                     m->stats, dbg);
+      if (timed) TPMC_CUDA_TRY(cudaEventRecord(pp.ev_f1, pp.main));
+      ++launches;
+      if (pi > 0) {
+        TPMC_CUDA_TRY(cudaEventRecord(pp.ev_done, pp.main));
+        TPMC_CUDA_TRY(cudaStreamWaitEvent(st, pp.ev_done, 0));
+      }
+    }
   }
   k_reduce_parts<<<kReduceParts, kReduceBlock, 0, st>>>(P, (long long)m->nt, m->partials);
   k_reduce_final<<<1, 32, 0, st>>>(m->partials, kReduceParts, m->totals, d_force, d_torque);
   launches += 2;
   m->last_launches = launches;
-  m->last_timed_waves = timed ? std::min<unsigned long long>(it, kMaxTimedWaves) : 0;
-  m->last_seed_waves = (params->count <= kChunk) ? (params->count + wave - 1) / wave : 0;   // seed events exist for these
   TPMC_CUDA_TRY(cudaGetLastError());
   TPMC_CUDA_TRY(cudaEventRecord(m->ev1, st));
   if (h_stats) {
@@ -810,16 +859,17 @@ extern "C" int tpmc_trace(const tpmc_mesh* mesh, const float* d_o, const float* 
   int rcode = ensure_scratch(m, std::max<size_t>(((size_t)n + 1) / 2, m->wave_cap), false);
   if (rcode != TPMC_OK) return rcode;
   const Grids& g = grids();
-  RayQueue q = {m->q_o[0], m->q_v[0], m->q_f[0]};
+  Pipe& pp = m->pipe[0];
+  RayQueue q = {pp.q_o[0], pp.q_v[0], pp.q_f[0]};
   const unsigned int un = (unsigned int)n;
-  TPMC_CUDA_TRY(cudaMemsetAsync(m->ctr, 0, kCtrWords * sizeof(unsigned int), st));
-  TPMC_CUDA_TRY(cudaMemcpyAsync(m->ctr, &un, sizeof(un), cudaMemcpyHostToDevice, st));   // region A holds the rays
+  TPMC_CUDA_TRY(cudaMemsetAsync(pp.ctr, 0, kCtrWords * sizeof(unsigned int), st));
+  TPMC_CUDA_TRY(cudaMemcpyAsync(pp.ctr, &un, sizeof(un), cudaMemcpyHostToDevice, st));   // region A holds the rays
   TPMC_CUDA_TRY(cudaMemsetAsync(m->stats, 0, ST_COUNT * sizeof(unsigned long long), st));
   k_pack_rays<<<(un + 255) / 256, 256, 0, st>>>(d_o, d_d, d_f_prev, un, q, d_facet, d_tau);
   // the production traversal (fp32 wavefront + candidate lists), then the exact fp64 resolve
-  k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(m->nodes, m->tris, q, (unsigned int)(2 * m->wave_cap), m->ctr, m->ctr + 4,
-                                              m->hit_ray, m->hit_cand, m->ctr + 5, m->stats);
-  k_resolve_only<<<g.reflect, kTraceBlock, 0, st>>>(m->nodes, m->tris, q, m->hit_ray, m->hit_cand, m->ctr + 5, d_facet,
+  k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(m->nodes, m->tris, q, (unsigned int)(2 * m->wave_cap), pp.ctr, pp.ctr + 4,
+                                              pp.hit_ray, pp.hit_cand, pp.ctr + 5, m->stats);
+  k_resolve_only<<<g.reflect, kTraceBlock, 0, st>>>(m->nodes, m->tris, q, pp.hit_ray, pp.hit_cand, pp.ctr + 5, d_facet,
                                                     d_tau);
   TPMC_CUDA_TRY(cudaGetLastError());
   TPMC_CUDA_TRY(cudaStreamSynchronize(st));   // &un must outlive the copy
