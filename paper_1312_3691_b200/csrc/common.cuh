@@ -36,7 +36,8 @@ struct Pipe {
   int* q_f[2];
   unsigned int* hit_ray;           // [2*wave_cap] queue slot of every ray that ended with candidate facets
   int4* hit_cand;                  // [2*wave_cap] its candidate triangle slots
-  unsigned int* ctr;               // [kCtrWords] device counters (queue sizes, fetch head, hit count)
+  unsigned int* ctr;               // [kCtrWords] device counters (queue sizes, fetch head, hit count, survivors)
+  unsigned int* surv;              // [3][wave_cap] survivors of the fp32 pre-cull pass: wave offset, fp32 roots
   cudaStream_t main, seed;         // trace/reflect chain; seed kernel of the next wave (pipe 0: main = caller's)
   cudaEvent_t ev_reset[4], ev_seeded[4], ev_done, ev_f0, ev_f1;
   cudaEvent_t* wave_ev;            // [kEvPerWave*kMaxTimedWaves] per-kernel timing, created on first use
@@ -73,7 +74,8 @@ constexpr int kMaxTimedWaves = 1024;  // iterations covered by the per-kernel ev
 constexpr int kDrain = 3;             // trace/reflect iterations after the last wave, before the straggler kernel
 constexpr int kEvPerWave = 5;         // seed start/end (seed stream), trace start, after trace, after reflect
 constexpr int kCtrWords = 8;
-constexpr int kCullNodes = 64;        // 64 KB: stays in L1 next to the shared-memory carve-out
+constexpr int kCullNodes = 64;        // 4 KB: stays in L1 next to the shared-memory carve-out
+constexpr float kPrecullMargin = 2e-2f;   // box growth of the pre-cull pass, in bounding radii (sampling.cuh)
 
 // Per-run constants (a1: host, fp64), passed to kernels by value.
 struct SpeciesConst {

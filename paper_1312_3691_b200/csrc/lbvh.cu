@@ -344,7 +344,7 @@ extern "C" void tpmc_mesh_destroy(tpmc_mesh* m) {
   for (int pi = 0; pi < kPipes; ++pi) {
     Pipe& pp = m->pipe[pi];
     for (int k = 0; k < 2; ++k) { cudaFree(pp.q_o[k]); cudaFree(pp.q_v[k]); cudaFree(pp.q_f[k]); }
-    cudaFree(pp.hit_ray); cudaFree(pp.hit_cand); cudaFree(pp.ctr);
+    cudaFree(pp.hit_ray); cudaFree(pp.hit_cand); cudaFree(pp.ctr); cudaFree(pp.surv);
     if (pi > 0 && pp.main) cudaStreamDestroy(pp.main);
     if (pp.seed) cudaStreamDestroy(pp.seed);
     for (int k = 0; k < 4; ++k) {

@@ -52,21 +52,69 @@ __global__ void k_iter_begin(unsigned int* __restrict__ ctr, int out_parity) {
   }
 }
 
-// a2: seed one wave of particles, round the state to fp32 (O9), drop the rays that cannot touch the
+// a2, pre-cull pass (sampling.cuh): fp32 estimate of every particle's ray against the grown bounds.  Survivor
+// records (wave offset, fp32 roots) of certified estimates fill `surv` from the front, particles whose
+// estimate is not certified from the back; n_surv[0], n_surv[1] count them.  surv = [3][cap] words.
+__global__ void __launch_bounds__(kSeedBlock) k_seed_precull(const SeedConstF sf, unsigned int seed_lo,
+                                                             unsigned int seed_hi, unsigned long long first,
+                                                             unsigned int wave_n, unsigned int cap,
+                                                             unsigned int* __restrict__ surv,
+                                                             unsigned int* __restrict__ n_surv,
+                                                             unsigned long long* __restrict__ stats) {
+  const unsigned int j = blockIdx.x * blockDim.x + threadIdx.x;
+  const bool active = j < wave_n;
+  float o[3], v[3], root[2];
+  const bool ok = seed_particle_approx(sf, seed_lo, seed_hi, first + j, o, v, root);
+  const bool touch = precull_touch(sf, o, v);
+  const bool keep_c = active && ok && touch, keep_u = active && !ok;
+  const unsigned mcert = __ballot_sync(0xFFFFFFFFu, keep_c);
+  const unsigned munc = __ballot_sync(0xFFFFFFFFu, keep_u);
+  const unsigned mcull = __ballot_sync(0xFFFFFFFFu, active && ok && !touch);
+  const int lane = threadIdx.x & 31;
+  unsigned base_c = 0, base_u = 0;
+  if (lane == 0) {
+    if (mcert) base_c = atomicAdd(&n_surv[0], (unsigned)__popc(mcert));
+    if (munc) base_u = atomicAdd(&n_surv[1], (unsigned)__popc(munc));
+    if (mcull) atomicAdd(&stats[ST_CULLED], (unsigned long long)__popc(mcull));
+  }
+  base_c = __shfl_sync(0xFFFFFFFFu, base_c, 0);
+  base_u = __shfl_sync(0xFFFFFFFFu, base_u, 0);
+  if (keep_c) {
+    const unsigned slot = base_c + __popc(mcert & lanemask_lt());
+    surv[slot] = j;
+    surv[cap + slot] = __float_as_uint(root[0]);
+    surv[2 * cap + slot] = __float_as_uint(root[1]);
+  }
+  if (keep_u) surv[cap - 1u - (base_u + __popc(munc & lanemask_lt()))] = j;
+}
+
+// a2: seed particles of one wave in fp64, round the state to fp32 (O9), drop the rays that cannot touch the
 // mesh AABB or any box of the top of the hierarchy (their single segment is an escape; same conservative
 // slab test as the traversal) and append the rest to the ray queue.
+// surv != nullptr: dense over the survivors of the pre-cull pass; else over all wave_n particles.
 __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned int wave_first,
-                                                     unsigned int wave_n, const float4* __restrict__ cull,
+                                                     unsigned int wave_n, const unsigned int* __restrict__ surv,
+                                                     unsigned int cap_s, const unsigned int* __restrict__ n_surv,
+                                                     const float4* __restrict__ cull,
                                                      const RayQueue q, unsigned int region_b,
                                                      unsigned int* __restrict__ qcount,
                                                      unsigned long long* __restrict__ stats) {
-  const unsigned int j = blockIdx.x * blockDim.x + threadIdx.x;
-  const bool active = j < wave_n;
+  const unsigned int n1 = surv ? n_surv[0] : 0u;                 // certified survivors: fp32 roots available
+  const unsigned int n = surv ? n1 + n_surv[1] : wave_n;
+  const unsigned int stride = gridDim.x * blockDim.x;
+  const unsigned int nround = ((n + stride - 1) / stride) * stride;   // keep warps converged for the ballots
+  for (unsigned int kk = blockIdx.x * blockDim.x + threadIdx.x; kk < nround; kk += stride) {
+  const bool active = kk < n;
+  const bool hinted = kk < n1;
+  const unsigned int sl = hinted ? kk : cap_s - 1u - (kk - n1);
+  const unsigned int j = active ? (surv ? surv[sl] : kk) : 0u;
   bool keep = false;
   float o[3] = {0, 0, 0}, v[3] = {1, 1, 1};
   int species = 0;
   if (active) {
-    const SeedState s = seed_particle(rc, rc.first + wave_first + j);
+    float hint[2] = {0.0f, 0.0f};
+    if (hinted) { hint[0] = __uint_as_float(surv[cap_s + sl]); hint[1] = __uint_as_float(surv[2 * cap_s + sl]); }
+    const SeedState s = seed_particle(rc, rc.first + wave_first + j, hinted ? hint : nullptr);
     species = s.species;
 #pragma unroll
     for (int k = 0; k < 3; ++k) { o[k] = (float)s.x[k]; v[k] = (float)s.v[k]; }
@@ -90,6 +138,7 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
     q.o[slot] = make_float4(o[0], o[1], o[2], __uint_as_float(wave_first + j));
     q.v[slot] = make_float4(v[0], v[1], v[2], __uint_as_float((unsigned int)species));   // bounce 0
     q.f[slot] = -1;
+  }
   }
 }
 
@@ -549,6 +598,29 @@ int make_run_const(const tpmc_mesh* m, const tpmc_params* p, RunConst* rc) {
   return TPMC_OK;
 }
 
+// fp32 image of the per-run constants for the pre-cull pass
+void make_seed_const_f(const tpmc_mesh* m, const RunConst& rc, SeedConstF* sf) {
+  memset(sf, 0, sizeof(*sf));
+  sf->n_species = rc.n_species;
+  for (int s = 0; s < rc.n_species; ++s) {
+    SpeciesF& f = sf->sp[s];
+    f.S = (float)rc.sp[s].S; f.c = (float)rc.sp[s].c; f.g0 = (float)rc.sp[s].g0; f.gI = (float)rc.sp[s].gI;
+    // u01(w) = (w + 1/2) 2^-32 >= cumx  <=>  w >= cumx 2^32 - 1/2; all steps exact in fp64
+    const double t = ceil(rc.sp[s].cumx * 4294967296.0 - 0.5);
+    f.thr = t <= 0.0 ? 0ull : (t >= 4294967296.0 ? 4294967296ull : (unsigned long long)t);
+  }
+  const float mg = kPrecullMargin * (float)m->Rb;
+  for (int k = 0; k < 9; ++k) sf->R[k] = (float)rc.R[k];
+  for (int a = 0; a < 3; ++a) {
+    sf->centre[a] = (float)rc.centre[a];
+    sf->lo[a] = m->aabb_lo[a] - mg;
+    sf->hi[a] = m->aabb_hi[a] + mg;
+  }
+  sf->r = (float)rc.r;
+  const float Rg = (float)m->Rb * (1.0f + kPrecullMargin);
+  sf->Rg2 = Rg * Rg;
+}
+
 size_t wave_size() {
   static size_t w = 0;
   if (!w) {
@@ -586,8 +658,8 @@ int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
         cudaFree(pp.q_o[k]); cudaFree(pp.q_v[k]); cudaFree(pp.q_f[k]);
         pp.q_o[k] = pp.q_v[k] = nullptr; pp.q_f[k] = nullptr;
       }
-      cudaFree(pp.hit_ray); cudaFree(pp.hit_cand);
-      pp.hit_ray = nullptr; pp.hit_cand = nullptr;
+      cudaFree(pp.hit_ray); cudaFree(pp.hit_cand); cudaFree(pp.surv);
+      pp.hit_ray = nullptr; pp.hit_cand = nullptr; pp.surv = nullptr;
     }
     m->wave_cap = 0;
     for (int pi = 0; pi < kPipes; ++pi) {
@@ -599,6 +671,7 @@ int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
       }
       TPMC_CUDA_TRY(cudaMalloc((void**)&pp.hit_ray, 2 * wave * sizeof(unsigned int)));
       TPMC_CUDA_TRY(cudaMalloc((void**)&pp.hit_cand, 2 * wave * sizeof(int4)));
+      TPMC_CUDA_TRY(cudaMalloc((void**)&pp.surv, 3 * wave * sizeof(unsigned int)));
     }
     m->wave_cap = wave;
   }
@@ -607,9 +680,9 @@ int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
   return TPMC_OK;
 }
 
-struct Grids { int trace, reflect, finish, pipes; };
+struct Grids { int trace, reflect, finish, pipes, seed; };
 const Grids& grids() {
-  static Grids g = {0, 0, 0, 0};
+  static Grids g = {0, 0, 0, 0, 0};
   if (!g.trace) {
     int dev = 0, sms = 148, per = 0;
     cudaGetDevice(&dev);
@@ -625,6 +698,8 @@ const Grids& grids() {
     g.reflect = sms * std::max(1, per / g.pipes);
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_finish, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
     g.finish = sms * per;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_seed, kSeedBlock, 0) != cudaSuccess || per < 1) per = 4;
+    g.seed = sms * per;
   }
   return g;
 }
@@ -696,6 +771,10 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
   const int K = g.pipes;
   static const bool no_overlap = getenv("TPMC_NO_OVERLAP") != nullptr;   // diagnosis: one stream only
   const bool timed = (h_stats != nullptr);   // per-kernel events only when the caller will read them
+  const char* pc_env = getenv("TPMC_PRECULL");   // read per call: the parity tests switch the pass off and on
+  const bool precull = !(pc_env && pc_env[0] == '0');
+  SeedConstF sf;
+  make_seed_const_f(m, rc, &sf);
   m->pipe[0].main = st;
   for (int pi = 0; pi < kPipes; ++pi) {
     Pipe& pp = m->pipe[pi];
@@ -754,8 +833,15 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
         const unsigned int wn = (unsigned int)std::min<unsigned long long>(wave, cn - wv * wave);
         TPMC_CUDA_TRY(cudaStreamWaitEvent(s2, pp.ev_reset[li & 3], 0));
         if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[0], s2));
-        k_seed<<<(wn + kSeedBlock - 1) / kSeedBlock, kSeedBlock, 0, s2>>>(rcc, w0, wn, m->cull, Q[p], cap,
-                                                                         pp.ctr + 2 * p + 1, m->stats);
+        const unsigned int gfull = (wn + kSeedBlock - 1) / kSeedBlock;
+        if (precull) {
+          TPMC_CUDA_TRY(cudaMemsetAsync(pp.ctr + 6, 0, 2 * sizeof(unsigned int), s2));
+          k_seed_precull<<<gfull, kSeedBlock, 0, s2>>>(sf, rcc.seed_lo, rcc.seed_hi, rcc.first + w0, wn, cap, pp.surv,
+                                                       pp.ctr + 6, m->stats);
+          ++launches;
+        }
+        k_seed<<<std::min<unsigned int>(gfull, (unsigned int)g.seed), kSeedBlock, 0, s2>>>(
+            rcc, w0, wn, precull ? pp.surv : nullptr, cap, pp.ctr + 6, m->cull, Q[p], cap, pp.ctr + 2 * p + 1, m->stats);
         if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[1], s2));
         TPMC_CUDA_TRY(cudaEventRecord(pp.ev_seeded[li & 3], s2));
         if (tw) pp.seed_iters = li + 1;

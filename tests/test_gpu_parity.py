@@ -345,3 +345,26 @@ def test_run_on_side_stream(T, O):
         r = gm.run(cfg, stream=s)
     s.synchronize()
     assert np.allclose(r.force.cpu().numpy(), ref, rtol=1e-12)
+
+
+# ------------------------------------------------------------------ a2: the fp32 pre-cull pass drops only misses
+@pytest.mark.parametrize("name,idx,count", [("C1", 0, 100_000), ("C2", 0, 3_000_000), ("C2", 2, 3_000_000),
+                                             ("C3", 1, 3_000_000), ("C4", 5, 3_000_000), ("C5", 3, 20_000_000)])
+def test_precull_pass_changes_nothing(T, name, idx, count, monkeypatch):
+    """The pre-cull pass may only drop particles whose first segment misses the body: with the pass switched
+    off (TPMC_PRECULL=0, every particle through the fp64 sampler) hits, hashes and per-facet sums are identical."""
+    cfg = ti.config(name)[idx]
+    m = cfg.mesh()
+    gm = T.Mesh(m.vertices, m.indices, m.flags)
+    first = min(cfg.N - count, 777_777)
+    monkeypatch.setenv("TPMC_PRECULL", "1")
+    a = gm.run(cfg, first=first, count=count, debug=True)
+    monkeypatch.setenv("TPMC_PRECULL", "0")
+    b = gm.run(cfg, first=first, count=count, debug=True)
+    assert a.stats["hits"] == b.stats["hits"] and a.stats["hits"] > 0
+    assert a.stats["kernel_launches"] > b.stats["kernel_launches"]          # the pass really ran in `a` only
+    assert bool((a.hash == b.hash).all()) and bool((a.first_facet == b.first_facet).all())
+    Fa, Fb = a.force.cpu().numpy(), b.force.cpu().numpy()
+    assert np.linalg.norm(Fa - Fb) <= 1e-12 * np.linalg.norm(Fb)
+    assert a.stats["culled"] >= b.stats["culled"]     # the grown bounding sphere also drops rays the boxes keep
+    gm.close()
