@@ -52,6 +52,8 @@ struct tpmc_mesh {
   int64_t n_nodes;
   float4* nodes;
   float4* tris;
+  uint4* cnodes;                   // compact copy of `nodes` for the wavefront traversal: 2 uint4 = 32 B per node
+  float q_origin[3], q_scale[3];   // its quantisation grid: x = q_origin + q * q_scale, q in [0, 65535]
   float4* cull;                    // top of the hierarchy (<= kCullNodes nodes, breadth-first), for the seed-time cull
   int n_cull;
   double centre[3];
@@ -76,6 +78,12 @@ constexpr int kEvPerWave = 5;         // seed start/end (seed stream), trace sta
 constexpr int kCtrWords = 8;
 constexpr int kCullNodes = 64;        // 4 KB: stays in L1 next to the shared-memory carve-out
 constexpr float kPrecullMargin = 2e-2f;   // box growth of the pre-cull pass, in bounding radii (sampling.cuh)
+
+// Quantisation grid of the compact nodes, as the traversal kernel uses it (fp32).
+struct QuantGrid {
+  float origin[3];
+  float inv_scale[3];   // fp32(1 / q_scale)
+};
 
 // Per-run constants (a1: host, fp64), passed to kernels by value.
 struct SpeciesConst {

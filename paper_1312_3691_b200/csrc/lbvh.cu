@@ -184,6 +184,37 @@ __global__ void k_single(const float* __restrict__ box_leaf, float4* __restrict_
   nodes[3] = make_float4(__int_as_float(~0), __int_as_float(~0), 0.0f, 0.0f);
 }
 
+// Compact copy of the hierarchy for the wavefront traversal: 32 B per node = one 256-bit load.
+//   words 0-2: child 0 box, words 3-5: child 1 box, each (lo.x | lo.y << 16, lo.z | hi.x << 16, hi.y | hi.z << 16)
+//   as unsigned 16-bit grid coordinates, words 6-7: the two child refs.
+// Grid: x = origin + q * scale per axis.  lo is rounded down and hi up, then both are moved out by one more
+// grid step: the decoded box contains the fp32 box grown by `scale`, which covers the rounding of the ray's
+// transform into grid coordinates in the traversal (<= 0.012 steps, see slab_q in trace.cuh).
+__global__ void k_compact_nodes(const float4* __restrict__ nodes, int64_t n_nodes, double ox, double oy, double oz,
+                                double sx, double sy, double sz, uint4* __restrict__ cnodes) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n_nodes) return;
+  const float4 n0 = nodes[4 * i], n1 = nodes[4 * i + 1], n2 = nodes[4 * i + 2], n3 = nodes[4 * i + 3];
+  const float lo[2][3] = {{n0.x, n0.y, n0.z}, {n1.z, n1.w, n2.x}};
+  const float hi[2][3] = {{n0.w, n1.x, n1.y}, {n2.y, n2.z, n2.w}};
+  const double o[3] = {ox, oy, oz}, sc[3] = {sx, sy, sz};
+  unsigned int w[6];
+  for (int c = 0; c < 2; ++c) {
+    unsigned int ql[3], qh[3];
+    for (int a = 0; a < 3; ++a) {
+      if (lo[c][a] > hi[c][a]) { ql[a] = 65535u; qh[a] = 0u; continue; }   // empty box (single-triangle mesh)
+      const double l = floor(((double)lo[c][a] - o[a]) / sc[a]) - 1.0, h = ceil(((double)hi[c][a] - o[a]) / sc[a]) + 1.0;
+      ql[a] = (unsigned int)fmin(fmax(l, 0.0), 65535.0);
+      qh[a] = (unsigned int)fmin(fmax(h, 0.0), 65535.0);
+    }
+    w[3 * c + 0] = ql[0] | (ql[1] << 16);
+    w[3 * c + 1] = ql[2] | (qh[0] << 16);
+    w[3 * c + 2] = qh[1] | (qh[2] << 16);
+  }
+  cnodes[2 * i] = make_uint4(w[0], w[1], w[2], w[3]);
+  cnodes[2 * i + 1] = make_uint4(w[4], w[5], __float_as_uint(n3.x), __float_as_uint(n3.y));
+}
+
 // Top of the tree, breadth-first, cut at a node budget: child refs >= 0 index this array, -1 marks a
 // subtree (or triangle) that was cut off.  A ray that touches no cut-off box cannot hit the mesh.
 __global__ void k_build_cull(const float4* __restrict__ nodes, float4* __restrict__ cull, int* __restrict__ queue,
@@ -320,6 +351,19 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
                                                                                 kids.as<int2>(), par.as<int>());
     k_refit<<<gt, kBlock, 0, st>>>((int)nt, kids.as<int2>(), par.as<int>(), box.as<float>(), arr.as<int>(), m->nodes);
   }
+  {
+    // quantisation grid: the vertex AABB spans steps 100 .. 65100 of each axis (flat axes get a tiny step)
+    double ext[3], emax = 0.0;
+    for (int a = 0; a < 3; ++a) { ext[a] = (double)h.aabb[3 + a] - (double)h.aabb[a]; emax = std::max(emax, ext[a]); }
+    for (int a = 0; a < 3; ++a) {
+      m->q_scale[a] = (float)(std::max(ext[a], std::max(1e-6 * emax, 1e-30)) / 65000.0);
+      m->q_origin[a] = (float)((double)h.aabb[a] - 100.0 * (double)m->q_scale[a]);
+    }
+    MESH_TRY(cudaMalloc((void**)&m->cnodes, sizeof(uint4) * 2 * m->n_nodes));
+    k_compact_nodes<<<(unsigned)((m->n_nodes + kBlock - 1) / kBlock), kBlock, 0, st>>>(
+        m->nodes, m->n_nodes, (double)m->q_origin[0], (double)m->q_origin[1], (double)m->q_origin[2],
+        (double)m->q_scale[0], (double)m->q_scale[1], (double)m->q_scale[2], m->cnodes);
+  }
   DevBuf cq;
   MESH_TRY(cudaMalloc((void**)&m->cull, sizeof(float4) * 4 * kCullNodes));
   MESH_TRY(cudaMalloc(&cq.p, sizeof(int) * (kCullNodes + 1)));
@@ -340,7 +384,7 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
 
 extern "C" void tpmc_mesh_destroy(tpmc_mesh* m) {
   if (!m) return;
-  cudaFree(m->nodes); cudaFree(m->tris); cudaFree(m->cull);
+  cudaFree(m->nodes); cudaFree(m->tris); cudaFree(m->cull); cudaFree(m->cnodes);
   for (int pi = 0; pi < kPipes; ++pi) {
     Pipe& pp = m->pipe[pi];
     for (int k = 0; k < 2; ++k) { cudaFree(pp.q_o[k]); cudaFree(pp.q_v[k]); cudaFree(pp.q_f[k]); }

@@ -144,42 +144,45 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
 
 
 // a3: wavefront traversal.  Persistent warps, one ray per lane, fp32 only (see trace.cuh).
-//  * node phase: lanes standing at an internal node step together; a lane that reaches a leaf waits;
-//  * leaf phase: once fewer than kNodeMin lanes are still at nodes, all waiting lanes classify their
-//    facet together (the ~120-instruction facet code then runs with many lanes active, not one);
+//  * node phase: lanes standing at an internal node step together (two steps per warp vote, branch-free
+//    child selection).  A lane that reaches a leaf puts it aside and walks on speculatively; it waits only
+//    when it reaches a second leaf or its stack is empty;
+//  * leaf phase: once fewer than kNodeMin lanes can still step, every lane with a leaf put aside classifies
+//    its facet (the ~120-instruction facet code then runs with many lanes active, not one);
 //  * a lane whose ray has finished takes the next ray of the queue as soon as kRefillIdle lanes are idle
 //    (one warp-aggregated atomic), so rays of very different length do not idle the warp.
 // Rays that end with at least one candidate facet are appended to the hit list for k_reflect.
 #ifndef TPMC_NODE_MIN
-#define TPMC_NODE_MIN 10
+#define TPMC_NODE_MIN 20
 #endif
 #ifndef TPMC_REFILL_IDLE
-#define TPMC_REFILL_IDLE 8
+#define TPMC_REFILL_IDLE 4
 #endif
 #ifndef TPMC_TRACE_MIN_BLOCKS
 #define TPMC_TRACE_MIN_BLOCKS 8
 #endif
-constexpr int kNodeMin = TPMC_NODE_MIN;
-constexpr int kRefillIdle = TPMC_REFILL_IDLE;
+struct TraceTune { int node_min, refill_idle; };
 
-__global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf(const float4* __restrict__ nodes,
+__global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf(const uint4* __restrict__ cnodes,
+                                                             const QuantGrid grid,
                                                              const float4* __restrict__ tris, const RayQueue q,
                                                              unsigned int cap, const unsigned int* __restrict__ n_rays,
                                                              unsigned int* __restrict__ next_ray,
                                                              unsigned int* __restrict__ hit_ray,
                                                              int4* __restrict__ hit_cand,
                                                              unsigned int* __restrict__ n_hits,
-                                                             unsigned long long* __restrict__ stats) {
+                                                             unsigned long long* __restrict__ stats,
+                                                             const TraceTune tune) {
+  const int kNodeMin = tune.node_min, kRefillIdle = tune.refill_idle;
   __shared__ int sstack[TPMC_STACK_SMEM * kTraceBlock];
   int* stk = sstack + threadIdx.x;
-  int lstack[TPMC_STACK_LOCAL];
   const unsigned int na = min(n_rays[0], cap), n = na + n_rays[1];   // region A (reflected), region B (primaries)
   const int lane = threadIdx.x & 31;
   const unsigned FULL = 0xFFFFFFFFu;
   bool has = false, exhausted = false, fin = false;
   unsigned int r = 0;
   Walk w;
-  w.cur = TPMC_SENTINEL; w.sp = 0; w.nc = 0; w.tmax = 0.0f; w.f_prev = -1;
+  w.cur = TPMC_SENTINEL; w.stash = 0; w.sp = 0; w.nc = 0; w.tmax = 0.0f; w.f_prev = -1;
   TraceCounters cnt;
   cnt.nodes = 0; cnt.tris = 0;
   for (;;) {
@@ -195,7 +198,7 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
         r = base + __popc(idle & lanemask_lt());
         if (r < n) {
           r = (r < na) ? r : cap + (r - na);   // physical slot
-          walk_init(w, q.o[r], q.v[r], q.f[r]);
+          walk_init(w, grid, q.o[r], q.v[r], q.f[r]);
           has = true;
         } else {
           exhausted = true;
@@ -203,22 +206,26 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
       }
     }
     if (__ballot_sync(FULL, has) == 0u) break;
-    // ---- node phase
+    // ---- node phase: two node steps per vote
     for (;;) {
-      const bool at_node = has && w.cur >= 0;
+      const bool at_node = has && (unsigned)w.cur < (unsigned)TPMC_SENTINEL;
       const unsigned mn = __ballot_sync(FULL, at_node);
-      const unsigned ml = __ballot_sync(FULL, has && w.cur < 0);
-      if (!(__popc(mn) >= kNodeMin || (mn != 0u && ml == 0u))) break;
+      if (__popc(mn) < kNodeMin) {
+        const unsigned ml = __ballot_sync(FULL, has && w.stash != 0);
+        if (mn == 0u || ml != 0u) break;
+      }
       if (at_node) {
-        walk_node(w, nodes, stk, kTraceBlock, lstack, cnt);
-        if (w.cur == TPMC_SENTINEL) { has = false; fin = w.nc > 0; }
+        walk_node(w, cnodes, stk, kTraceBlock, cnt);
+        if ((unsigned)w.cur < (unsigned)TPMC_SENTINEL) walk_node(w, cnodes, stk, kTraceBlock, cnt);
       }
     }
-    // ---- leaf phase
-    if (has && w.cur < 0) {
-      walk_leaf(w, tris, stk, kTraceBlock, lstack, cnt);
-      if (w.cur == TPMC_SENTINEL) { has = false; fin = w.nc > 0; }
+    // ---- leaf phase: every lane that put a leaf aside classifies it
+    if (has && w.stash != 0) {
+      const float4 ro = q.o[r], rv = q.v[r];   // re-read (cache-resident): keeps six registers free during the node phase
+      const float o[3] = {ro.x, ro.y, ro.z}, d[3] = {rv.x, rv.y, rv.z};
+      walk_leaf(w, tris, o, d, stk, kTraceBlock, cnt);
     }
+    if (has && w.cur == TPMC_SENTINEL && w.stash == 0) { has = false; fin = w.nc > 0; }
     // ---- finished rays with candidates -> hit list
     const unsigned fm = __ballot_sync(FULL, fin);
     if (fm) {
@@ -621,6 +628,22 @@ void make_seed_const_f(const tpmc_mesh* m, const RunConst& rc, SeedConstF* sf) {
   sf->Rg2 = Rg * Rg;
 }
 
+TraceTune trace_tune() {
+  static TraceTune t = {0, 0};
+  if (!t.node_min) {
+    t.node_min = TPMC_NODE_MIN; t.refill_idle = TPMC_REFILL_IDLE;
+    if (const char* e = getenv("TPMC_NODE_MIN")) t.node_min = std::max(1, std::min(32, atoi(e)));        // tuning aids
+    if (const char* e = getenv("TPMC_REFILL_IDLE")) t.refill_idle = std::max(1, std::min(32, atoi(e)));
+  }
+  return t;
+}
+
+QuantGrid quant_grid(const tpmc_mesh* m) {
+  QuantGrid g;
+  for (int a = 0; a < 3; ++a) { g.origin[a] = m->q_origin[a]; g.inv_scale[a] = (float)(1.0 / (double)m->q_scale[a]); }
+  return g;
+}
+
 size_t wave_size() {
   static size_t w = 0;
   if (!w) {
@@ -690,8 +713,8 @@ const Grids& grids() {
     g.pipes = kPipes;
     if (const char* e = getenv("TPMC_PIPES")) g.pipes = std::max(1, std::min(kPipes, atoi(e)));   // tuning aid
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_trace_wf, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
-    // resident trace CTAs per SM over all pipelines; the rest of the SM is left to the seed and reflect kernels
-    int tot = std::max(1, per - 2);
+    // resident trace CTAs per SM over all pipelines (measured: leaving room for the seed kernel does not pay)
+    int tot = std::max(1, per);
     if (const char* e = getenv("TPMC_TRACE_BLOCKS")) tot = std::max(1, std::min(per, atoi(e)));
     g.trace = sms * std::max(1, tot / g.pipes);
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_reflect, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
@@ -775,6 +798,7 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
   const bool precull = !(pc_env && pc_env[0] == '0');
   SeedConstF sf;
   make_seed_const_f(m, rc, &sf);
+  const QuantGrid qg = quant_grid(m);
   m->pipe[0].main = st;
   for (int pi = 0; pi < kPipes; ++pi) {
     Pipe& pp = m->pipe[pi];
@@ -851,8 +875,8 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
       TPMC_CUDA_TRY(cudaEventRecord(pp.ev_reset[(li + 1) & 3], s1));
       if (wv < n_waves) TPMC_CUDA_TRY(cudaStreamWaitEvent(s1, pp.ev_seeded[li & 3], 0));
       if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[2], s1));
-      k_trace_wf<<<g.trace, kTraceBlock, 0, s1>>>(m->nodes, m->tris, Q[p], cap, pp.ctr + 2 * p, pp.ctr + 4, pp.hit_ray,
-                                                  pp.hit_cand, pp.ctr + 5, m->stats);
+      k_trace_wf<<<g.trace, kTraceBlock, 0, s1>>>(m->cnodes, qg, m->tris, Q[p], cap, pp.ctr + 2 * p, pp.ctr + 4, pp.hit_ray,
+                                                  pp.hit_cand, pp.ctr + 5, m->stats, trace_tune());
       if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[3], s1));
       k_reflect<<<g.reflect, kTraceBlock, 0, s1>>>(rcc, cap, m->nodes, m->tris, Q[p], pp.hit_ray, pp.hit_cand, pp.ctr + 5,
                                                    Q[p ^ 1], pp.ctr + 2 * (p ^ 1), P, m->totals, m->stats, dbg);
@@ -953,8 +977,8 @@ extern "C" int tpmc_trace(const tpmc_mesh* mesh, const float* d_o, const float* 
   TPMC_CUDA_TRY(cudaMemsetAsync(m->stats, 0, ST_COUNT * sizeof(unsigned long long), st));
   k_pack_rays<<<(un + 255) / 256, 256, 0, st>>>(d_o, d_d, d_f_prev, un, q, d_facet, d_tau);
   // the production traversal (fp32 wavefront + candidate lists), then the exact fp64 resolve
-  k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(m->nodes, m->tris, q, (unsigned int)(2 * m->wave_cap), pp.ctr, pp.ctr + 4,
-                                              pp.hit_ray, pp.hit_cand, pp.ctr + 5, m->stats);
+  k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(m->cnodes, quant_grid(m), m->tris, q, (unsigned int)(2 * m->wave_cap), pp.ctr, pp.ctr + 4,
+                                              pp.hit_ray, pp.hit_cand, pp.ctr + 5, m->stats, trace_tune());
   k_resolve_only<<<g.reflect, kTraceBlock, 0, st>>>(m->nodes, m->tris, q, pp.hit_ray, pp.hit_cand, pp.ctr + 5, d_facet,
                                                     d_tau);
   TPMC_CUDA_TRY(cudaGetLastError());

@@ -171,6 +171,41 @@ __device__ __forceinline__ bool slab(float lx, float ly, float lz, float hx, flo
   return fmaxf(tn, 0.0f) <= fminf(tf, tmax);
 }
 
+// ---- the same test on a box of the compact hierarchy (grid coordinates, see k_compact_nodes) ----------
+// The ray is carried in grid coordinates: o' = (o - origin) * inv_scale, 1/d' with d' = d * inv_scale; the ray
+// parameter t is unchanged.  o' carries three roundings (difference, the rounded inv_scale, product): it is
+// off by <= 3u|o'| grid steps, so the walk keeps o' + e and o' - e with e = 4u|o'| and measures the low planes
+// from the first and the high planes from the second -- the slab test of the box grown by e, which together
+// with the one-step growth applied at encoding contains the fp32 box for any origin.  Planes and origins both
+// carry an offset of 2^23 (q_lo16/q_hi16): their difference is exact while the origin is within ~2^23 steps of
+// the grid, and otherwise rounds once more (relative u, inside the margin); the outward rounding of the
+// shifted origin grows the box by less than one further step.  What is left is
+// relative: d' (2 roundings), its reciprocal, the difference and the product: <= 5u on each plane distance;
+// the margin on entry and exit is 8u.
+__device__ __forceinline__ bool slab_q(float lx, float ly, float lz, float hx, float hy, float hz, const float ol[3],
+                                       const float oh[3], const float id[3], float tmax, float& tnear) {
+  const float u8 = 4.76837158203125e-07f;  // 8 * 2^-24
+  const float ax = (lx - ol[0]) * id[0], bx = (hx - oh[0]) * id[0];
+  const float ay = (ly - ol[1]) * id[1], by = (hy - oh[1]) * id[1];
+  const float az = (lz - ol[2]) * id[2], bz = (hz - oh[2]) * id[2];
+  float tn = fmaxf(fmaxf(fminf(ax, bx), fminf(ay, by)), fminf(az, bz));
+  float tf = fminf(fminf(fmaxf(ax, bx), fmaxf(ay, by)), fmaxf(az, bz));
+  tn = fmaf(-u8, fabsf(tn), tn);
+  tf = fmaf(u8, fabsf(tf), tf);
+  tnear = tn;
+  return fmaxf(tn, 0.0f) <= fminf(tf, tmax);
+}
+
+__device__ __forceinline__ void ldg256u(const uint4* p, uint4& a, uint4& b) {
+  asm volatile("ld.global.nc.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w), "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w)
+               : "l"(p));
+}
+// 16-bit grid coordinate q -> the float 2^23 + q, by one byte permute (no integer-to-float conversion): the
+// walk keeps the ray origin shifted by 2^23 as well (rounded outwards), so plane - origin is exact.
+__device__ __forceinline__ float q_lo16(unsigned int w) { return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610)); }
+__device__ __forceinline__ float q_hi16(unsigned int w) { return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7632)); }
+
 // ---- seed-time cull: can the ray touch any cut-off subtree of the top tree? (conservative) ------------
 // Near child first, so the first cut-off box found is (nearly) the first along the ray; its entry
 // distance is returned and later gives the ray its sort key (a point close to where it will hit).
@@ -214,33 +249,51 @@ __device__ __forceinline__ bool cull_touch(const float4* __restrict__ cull, cons
 
 // ---- per-ray traversal state of the wavefront kernel -------------------------------------------------
 struct Walk {
-  float o[3], d[3], id[3];
+  float ol[3], oh[3], id[3];   // grid coordinates: 2^23 + o' + e (rounded up), 2^23 + o' - e (rounded down), 1/d'
   float tmax;          // min over provable hits of their thi
   int f_prev;
-  int cur;             // node to visit next (>= 0 internal, < 0 leaf ~slot), TPMC_SENTINEL when finished
+  int cur;             // node to visit next (>= 0 internal, < 0 leaf ~slot), TPMC_SENTINEL when the stack is empty
+  int stash;           // leaf put aside for the next leaf phase (< 0), 0 = none
   int sp;
   int cs[TPMC_MAX_CAND];     // candidate slots
   float cl[TPMC_MAX_CAND];   // their tlo
   int nc;              // number of candidates; TPMC_MAX_CAND+1 = overflow
 };
 
-__device__ __forceinline__ void walk_init(Walk& w, const float4 ro, const float4 rv, int f_prev) {
-  w.o[0] = ro.x; w.o[1] = ro.y; w.o[2] = ro.z;
-  w.d[0] = rv.x; w.d[1] = rv.y; w.d[2] = rv.z;
-  w.id[0] = 1.0f / rv.x; w.id[1] = 1.0f / rv.y; w.id[2] = 1.0f / rv.z;
+__device__ __forceinline__ void walk_init(Walk& w, const QuantGrid& g, const float4 ro, const float4 rv, int f_prev) {
+  const float o[3] = {ro.x, ro.y, ro.z}, d[3] = {rv.x, rv.y, rv.z};
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const float oq = (o[k] - g.origin[k]) * g.inv_scale[k];
+    const float e = 2.384185791015625e-07f * fabsf(oq);   // 4u |o'|
+    w.ol[k] = __fadd_ru(8388608.0f, oq + e);   // >= 2^23 + o' + e: low planes are measured from a point not below it
+    w.oh[k] = __fadd_rd(8388608.0f, oq - e);   // <= 2^23 + o' - e
+    w.id[k] = 1.0f / (d[k] * g.inv_scale[k]);
+  }
   w.tmax = INFINITY;
   w.f_prev = f_prev;
   w.cur = 0;
+  w.stash = 0;
   w.sp = 0;
   w.nc = 0;
 #pragma unroll
   for (int k = 0; k < TPMC_MAX_CAND; ++k) { w.cs[k] = -1; w.cl[k] = 0.0f; }
 }
 
-__device__ __forceinline__ int walk_pop(Walk& w, const int* stk, int sstride, const int* lstack) {
-  if (w.sp == 0) return TPMC_SENTINEL;
-  --w.sp;
-  return (w.sp < TPMC_STACK_SMEM) ? stk[w.sp * sstride] : lstack[w.sp - TPMC_STACK_SMEM];
+// Stack: TPMC_STACK_SMEM entries per thread in shared memory, [level][thread].  A ray that needs more gives
+// up and is flagged for the full fp64 traversal of the resolve step (which has a deep stack), like a ray
+// with too many candidates.
+__device__ __forceinline__ int walk_pop(Walk& w, const int* stk, int sstride) {
+  const bool some = w.sp > 0;
+  w.sp -= some ? 1 : 0;
+  return some ? stk[w.sp * sstride] : TPMC_SENTINEL;
+}
+
+__device__ __forceinline__ void walk_abort(Walk& w) {
+  w.nc = TPMC_MAX_CAND + 1;
+  w.cur = TPMC_SENTINEL;
+  w.stash = 0;
+  w.sp = 0;
 }
 
 __device__ __forceinline__ void walk_add_candidate(Walk& w, int slot, int cls, float tlo, float thi) {
@@ -272,45 +325,54 @@ __device__ __forceinline__ void walk_add_candidate(Walk& w, int slot, int cls, f
 }
 
 // One internal-node step (two slab tests, push the far child) -- requires w.cur >= 0 and != SENTINEL.
-__device__ __forceinline__ void walk_node(Walk& w, const float4* __restrict__ nodes, int* stk, int sstride,
-                                          int* lstack, TraceCounters& cnt) {
-  const float4* np = nodes + 4 * (size_t)w.cur;
-  float4 n0, n1, n2, n3;
-  ldg256(np, n0, n1);
-  ldg256(np + 2, n2, n3);
+__device__ __forceinline__ void walk_node(Walk& w, const uint4* __restrict__ cnodes, int* stk, int sstride,
+                                          TraceCounters& cnt) {
+  uint4 a, b;
+  ldg256u(cnodes + 2 * (size_t)w.cur, a, b);
   ++cnt.nodes;
   float t0, t1;
-  const bool h0 = slab(n0.x, n0.y, n0.z, n0.w, n1.x, n1.y, w.o, w.id, w.tmax, t0);
-  const bool h1 = slab(n1.z, n1.w, n2.x, n2.y, n2.z, n2.w, w.o, w.id, w.tmax, t1);
-  int c0 = __float_as_int(n3.x), c1 = __float_as_int(n3.y);
-  if (h0 && h1) {
-    if (t1 < t0) { const int t = c0; c0 = c1; c1 = t; }
-    if (w.sp < TPMC_STACK_SMEM) stk[w.sp * sstride] = c1; else lstack[w.sp - TPMC_STACK_SMEM] = c1;
+  const bool h0 = slab_q(q_lo16(a.x), q_hi16(a.x), q_lo16(a.y), q_hi16(a.y), q_lo16(a.z), q_hi16(a.z), w.ol, w.oh, w.id,
+                         w.tmax, t0);
+  const bool h1 = slab_q(q_lo16(a.w), q_hi16(a.w), q_lo16(b.x), q_hi16(b.x), q_lo16(b.y), q_hi16(b.y), w.ol, w.oh, w.id,
+                         w.tmax, t1);
+  // branch-free child selection: near child next, far child pushed when both boxes are hit, pop when none is
+  const bool both = h0 && h1, any = h0 || h1;
+  const bool second = both ? (t1 < t0) : !h0;
+  const int c0 = (int)b.z, c1 = (int)b.w;
+  const int nearc = second ? c1 : c0, farc = second ? c0 : c1;
+  if (both) {
+    if (w.sp >= TPMC_STACK_SMEM) { walk_abort(w); return; }
+    stk[w.sp * sstride] = farc;
     ++w.sp;
-    w.cur = c0;
-  } else if (h0) {
-    w.cur = c0;
-  } else if (h1) {
-    w.cur = c1;
-  } else {
-    w.cur = walk_pop(w, stk, sstride, lstack);
+  }
+  const int popped = any ? 0 : walk_pop(w, stk, sstride);
+  w.cur = any ? nearc : popped;
+  // speculation: a leaf is put aside and the walk goes on; it is tested in the next leaf phase
+  if (w.cur < 0 && w.stash == 0) {
+    w.stash = w.cur;
+    w.cur = walk_pop(w, stk, sstride);
   }
 }
 
-// One leaf step (fp32 facet classification) -- requires w.cur < 0.
-__device__ __forceinline__ void walk_leaf(Walk& w, const float4* __restrict__ tris, int* stk, int sstride,
-                                          int* lstack, TraceCounters& cnt) {
-  const int slot = ~w.cur;
+// One leaf step (fp32 facet classification of the leaf put aside), then the next leaf, if the walk stands at
+// one, is put aside in turn.
+__device__ __forceinline__ void walk_leaf(Walk& w, const float4* __restrict__ tris, const float o[3], const float d[3],
+                                          int* stk, int sstride, TraceCounters& cnt) {
+  const int slot = ~w.stash;
   const float4 q0 = __ldg(tris + 3 * (size_t)slot + 0);
   if (__float_as_int(q0.w) != w.f_prev) {
     const float4 q1 = __ldg(tris + 3 * (size_t)slot + 1);
     const float4 q2 = __ldg(tris + 3 * (size_t)slot + 2);
     ++cnt.tris;
     float tlo, thi;
-    const int cls = tri_filter(q0, q1, q2, w.o, w.d, tlo, thi);
+    const int cls = tri_filter(q0, q1, q2, o, d, tlo, thi);
     if (cls != TRI_MISS) walk_add_candidate(w, slot, cls, tlo, thi);
   }
-  w.cur = walk_pop(w, stk, sstride, lstack);
+  w.stash = 0;
+  if (w.cur < 0) {
+    w.stash = w.cur;
+    w.cur = walk_pop(w, stk, sstride);
+  }
 }
 
 // ---- exact closest hit by a full fp64 traversal (stragglers, candidate overflow) ----------------------
