@@ -37,9 +37,12 @@ struct Pipe {
   unsigned int* hit_ray;           // [2*wave_cap] queue slot of every ray that ended with candidate facets
   int4* hit_cand;                  // [2*wave_cap] its candidate triangle slots
   unsigned int* ctr;               // [kCtrWords] device counters (queue sizes, fetch head, hit count, survivors)
+  unsigned int* ovf;               // [2][2*wave_cap] queue slots of rays left to the straggler kernel (overflow lists)
   unsigned int* surv;              // [3][wave_cap] survivors of the fp32 pre-cull pass: wave offset, fp32 roots
-  cudaStream_t main, seed;         // trace/reflect chain; seed kernel of the next wave (pipe 0: main = caller's)
+  cudaStream_t main, seed, side;   // trace/reflect chain (pipe 0: the caller's); next wave's seed kernels; stragglers
   cudaEvent_t ev_reset[4], ev_seeded[4], ev_done, ev_f0, ev_f1;
+  cudaEvent_t ev_refl[2], ev_ovf[2];   // reflect step done / its overflow list processed (iteration parity)
+  unsigned long long last_iter;
   cudaEvent_t* wave_ev;            // [kEvPerWave*kMaxTimedWaves] per-kernel timing, created on first use
   unsigned long long iters, seed_iters;   // of the last run: iterations / seeded iterations with timing events
 };
@@ -75,7 +78,7 @@ struct tpmc_mesh {
 constexpr int kMaxTimedWaves = 1024;  // iterations covered by the per-kernel event times
 constexpr int kDrain = 3;             // trace/reflect iterations after the last wave, before the straggler kernel
 constexpr int kEvPerWave = 5;         // seed start/end (seed stream), trace start, after trace, after reflect
-constexpr int kCtrWords = 8;
+constexpr int kCtrWords = 16;
 constexpr int kCullNodes = 64;        // 4 KB: stays in L1 next to the shared-memory carve-out
 constexpr float kPrecullMargin = 2e-2f;   // box growth of the pre-cull pass, in bounding radii (sampling.cuh)
 

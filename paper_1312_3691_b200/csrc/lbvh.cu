@@ -388,9 +388,14 @@ extern "C" void tpmc_mesh_destroy(tpmc_mesh* m) {
   for (int pi = 0; pi < kPipes; ++pi) {
     Pipe& pp = m->pipe[pi];
     for (int k = 0; k < 2; ++k) { cudaFree(pp.q_o[k]); cudaFree(pp.q_v[k]); cudaFree(pp.q_f[k]); }
-    cudaFree(pp.hit_ray); cudaFree(pp.hit_cand); cudaFree(pp.ctr); cudaFree(pp.surv);
+    cudaFree(pp.hit_ray); cudaFree(pp.hit_cand); cudaFree(pp.ctr); cudaFree(pp.surv); cudaFree(pp.ovf);
     if (pi > 0 && pp.main) cudaStreamDestroy(pp.main);
     if (pp.seed) cudaStreamDestroy(pp.seed);
+    if (pp.side) cudaStreamDestroy(pp.side);
+    for (int k = 0; k < 2; ++k) {
+      if (pp.ev_refl[k]) cudaEventDestroy(pp.ev_refl[k]);
+      if (pp.ev_ovf[k]) cudaEventDestroy(pp.ev_ovf[k]);
+    }
     for (int k = 0; k < 4; ++k) {
       if (pp.ev_reset[k]) cudaEventDestroy(pp.ev_reset[k]);
       if (pp.ev_seeded[k]) cudaEventDestroy(pp.ev_seeded[k]);

@@ -42,13 +42,15 @@ struct RayQueue {
 };
 
 // Per-iteration device counters: ctr[2p] = rays in region A of queue p, ctr[2p+1] = rays in region B,
-// ctr[4] = fetch head of the trace kernel, ctr[5] = hit-list length.
-__global__ void k_iter_begin(unsigned int* __restrict__ ctr, int out_parity) {
+// ctr[4] = fetch head of the trace kernel, ctr[5] = hit-list length, ctr[6..7] = survivors of the pre-cull
+// pass (seed stream), ctr[8 + b] = length of the overflow list of iterations of parity b.
+__global__ void k_iter_begin(unsigned int* __restrict__ ctr, int out_parity, int iter_parity) {
   if (threadIdx.x == 0) {
     ctr[2 * out_parity] = 0u;
     ctr[2 * out_parity + 1] = 0u;
     ctr[4] = 0u;
     ctr[5] = 0u;
+    ctr[8 + iter_parity] = 0u;
   }
 }
 
@@ -335,99 +337,106 @@ __device__ __forceinline__ bool interact(const RunConst& rc, const float4* __res
 
 // a4-a6: resolve the candidates of every hit ray with the exact fp64 test, apply the surface interaction,
 // accumulate, and queue the reflected ray for the next wavefront round (compacted, warp-aggregated).
+// Rays the traversal gave up on (too many candidates, stack too deep) and rays whose reflected successor
+// finds region A of the next queue full go, untouched, to the overflow list: k_finish follows them to escape
+// with the full fp64 traversal, densely, instead of one lane doing so here while its warp waits.
 __global__ void __launch_bounds__(kTraceBlock) k_reflect(const RunConst rc, unsigned int cap,
-                                                         const float4* __restrict__ nodes,
                                                          const float4* __restrict__ tris, const RayQueue qin,
                                                          const unsigned int* __restrict__ hit_ray,
                                                          const int4* __restrict__ hit_cand,
                                                          const unsigned int* __restrict__ n_hits, const RayQueue qout,
-                                                         unsigned int* __restrict__ n_out, double* __restrict__ P,
-                                                         double* __restrict__ torque,
+                                                         unsigned int* __restrict__ n_out,
+                                                         unsigned int* __restrict__ ovf, unsigned int* __restrict__ n_ovf,
+                                                         double* __restrict__ P, double* __restrict__ torque,
                                                          unsigned long long* __restrict__ stats, tpmc_debug dbg) {
   __shared__ double sred[3][8];
   __shared__ unsigned long long scnt[4][8];
   const unsigned int n = *n_hits;
   const int lane = threadIdx.x & 31;
+  const unsigned FULL = 0xFFFFFFFFu;
   double tq[3] = {0.0, 0.0, 0.0};
   unsigned long long hits = 0, trunc = 0;
   unsigned int ntests = 0;
-  TraceCounters cnt;
-  cnt.nodes = 0; cnt.tris = 0;
   const unsigned int stride = gridDim.x * blockDim.x;
   const unsigned int nround = ((n + stride - 1) / stride) * stride;   // keep warps converged for the ballots
   for (unsigned int h = blockIdx.x * blockDim.x + threadIdx.x; h < nround; h += stride) {
-    bool emit = false;
+    bool spill = false, is_hit = false;
+    unsigned int r = 0;
     Particle p;
+    Hit hit;
+    hit.facet = -1;
     if (h < n) {
-      const unsigned int r = hit_ray[h];
+      r = hit_ray[h];
       const int4 cand = hit_cand[h];
-      const float4 ro = qin.o[r], rv = qin.v[r];
-      p.o[0] = ro.x; p.o[1] = ro.y; p.o[2] = ro.z;
-      p.v[0] = rv.x; p.v[1] = rv.y; p.v[2] = rv.z;
-      p.j = __float_as_uint(ro.w);
-      const unsigned int pk = __float_as_uint(rv.w);
-      p.species = (int)(pk & 15u);
-      p.k = pk >> 4;
-      p.f_prev = qin.f[r];
-      Hit hit;
       if (cand.w == TPMC_CAND_OVERFLOW) {
-        int tmp[TPMC_STACK_SMEM];
-        hit = closest_hit(nodes, tris, p.o, p.v, p.f_prev, tmp, 1, cnt);
+        spill = true;
       } else {
+        const float4 ro = qin.o[r], rv = qin.v[r];
+        p.o[0] = ro.x; p.o[1] = ro.y; p.o[2] = ro.z;
+        p.v[0] = rv.x; p.v[1] = rv.y; p.v[2] = rv.z;
+        p.j = __float_as_uint(ro.w);
+        const unsigned int pk = __float_as_uint(rv.w);
+        p.species = (int)(pk & 15u);
+        p.k = pk >> 4;
+        p.f_prev = qin.f[r];
         hit = resolve_candidates(tris, cand, p.o, p.v, ntests);
-      }
-      if (hit.facet >= 0) {
-        ++hits;
-        emit = interact(rc, tris, p, hit, P, tq, dbg, trunc);
+        is_hit = hit.facet >= 0;
       }
     }
-    const unsigned em = __ballot_sync(0xFFFFFFFFu, emit);
+    // reserve the successor's queue slot first: a particle that finds the region full is spilled untouched
+    const unsigned em = __ballot_sync(FULL, is_hit);
     if (em) {
       const int leader = __ffs(em) - 1;
       unsigned base = 0;
       if (lane == leader) base = atomicAdd(n_out, (unsigned)__popc(em));
-      base = __shfl_sync(0xFFFFFFFFu, base, leader);
-      if (emit) {
+      base = __shfl_sync(FULL, base, leader);
+      if (is_hit) {
         const unsigned s = base + __popc(em & lanemask_lt());
-        if (s < cap) {
-          qout.o[s] = make_float4(p.o[0], p.o[1], p.o[2], __uint_as_float((unsigned int)p.j));
+        if (s >= cap) {
+          spill = true;
+        } else {
+          ++hits;
+          const bool go_on = interact(rc, tris, p, hit, P, tq, dbg, trunc);
+          // a particle stopped by the bounce cap leaves a hole: a NaN origin fails every box test
+          qout.o[s] = make_float4(go_on ? p.o[0] : __int_as_float(0x7FC00000), p.o[1], p.o[2], __uint_as_float((unsigned int)p.j));
           qout.v[s] = make_float4(p.v[0], p.v[1], p.v[2], __uint_as_float((unsigned int)p.species | (p.k << 4)));
           qout.f[s] = p.f_prev;
-        } else {
-          // region A of the next queue is full (possible only when most segments hit): follow this
-          // particle to escape here instead of dropping it
-          int tmp[TPMC_STACK_SMEM];
-          for (;;) {
-            const Hit hit = closest_hit(nodes, tris, p.o, p.v, p.f_prev, tmp, 1, cnt);
-            if (hit.facet < 0) break;
-            ++hits;
-            if (!interact(rc, tris, p, hit, P, tq, dbg, trunc)) break;
-          }
         }
       }
     }
+    const unsigned sm = __ballot_sync(FULL, spill);
+    if (sm) {
+      const int leader = __ffs(sm) - 1;
+      unsigned base = 0;
+      if (lane == leader) base = atomicAdd(n_ovf, (unsigned)__popc(sm));
+      base = __shfl_sync(FULL, base, leader);
+      if (spill) ovf[base + __popc(sm & lanemask_lt())] = r;
+    }
   }
-  unsigned long long c4[4] = {hits, trunc, (unsigned long long)ntests + cnt.tris, (unsigned long long)cnt.nodes};
+  unsigned long long c4[4] = {hits, trunc, (unsigned long long)ntests, 0ull};
   block_flush(tq, c4, torque, stats, sred, scnt);
 }
 
-// Stragglers after the wavefront rounds: each remaining particle is followed to escape in one thread
-// (full fp64 traversal per segment).  Few particles get here; long multi-bounce paths live here.
+// Particles followed to escape thread by thread (full fp64 traversal per segment): the overflow list of an
+// iteration (list != nullptr: queue slots) and, after the wavefront rounds, the stragglers still in the
+// queue.  Few particles get here; long multi-bounce paths live here.
 __global__ void __launch_bounds__(kTraceBlock) k_finish(const RunConst rc, unsigned int cap,
                                                         const float4* __restrict__ nodes,
                                                         const float4* __restrict__ tris, const RayQueue q,
+                                                        const unsigned int* __restrict__ list,
                                                         const unsigned int* __restrict__ n_rays,
                                                         double* __restrict__ P, double* __restrict__ torque,
                                                         unsigned long long* __restrict__ stats, tpmc_debug dbg) {
   __shared__ int sstack[TPMC_STACK_SMEM * kTraceBlock];
   __shared__ double sred[3][8];
   __shared__ unsigned long long scnt[4][8];
-  const unsigned int n = min(*n_rays, cap);
+  const unsigned int n = list ? *n_rays : min(*n_rays, cap);
   double tq[3] = {0.0, 0.0, 0.0};
   unsigned long long hits = 0, trunc = 0;
   TraceCounters cnt;
   cnt.nodes = 0; cnt.tris = 0;
-  for (unsigned int r = blockIdx.x * blockDim.x + threadIdx.x; r < n; r += gridDim.x * blockDim.x) {
+  for (unsigned int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    const unsigned int r = list ? list[i] : i;
     const float4 ro = q.o[r], rv = q.v[r];
     Particle p;
     p.o[0] = ro.x; p.o[1] = ro.y; p.o[2] = ro.z;
@@ -664,6 +673,11 @@ int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
       Pipe& pp = m->pipe[pi];
       if (pi > 0) TPMC_CUDA_TRY(cudaStreamCreateWithFlags(&pp.main, cudaStreamNonBlocking));
       TPMC_CUDA_TRY(cudaStreamCreateWithFlags(&pp.seed, cudaStreamNonBlocking));
+      TPMC_CUDA_TRY(cudaStreamCreateWithFlags(&pp.side, cudaStreamNonBlocking));
+      for (int k = 0; k < 2; ++k) {
+        TPMC_CUDA_TRY(cudaEventCreateWithFlags(&pp.ev_refl[k], cudaEventDisableTiming));
+        TPMC_CUDA_TRY(cudaEventCreateWithFlags(&pp.ev_ovf[k], cudaEventDisableTiming));
+      }
       for (int k = 0; k < 4; ++k) {
         TPMC_CUDA_TRY(cudaEventCreateWithFlags(&pp.ev_reset[k], cudaEventDisableTiming));
         TPMC_CUDA_TRY(cudaEventCreateWithFlags(&pp.ev_seeded[k], cudaEventDisableTiming));
@@ -681,8 +695,8 @@ int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
         cudaFree(pp.q_o[k]); cudaFree(pp.q_v[k]); cudaFree(pp.q_f[k]);
         pp.q_o[k] = pp.q_v[k] = nullptr; pp.q_f[k] = nullptr;
       }
-      cudaFree(pp.hit_ray); cudaFree(pp.hit_cand); cudaFree(pp.surv);
-      pp.hit_ray = nullptr; pp.hit_cand = nullptr; pp.surv = nullptr;
+      cudaFree(pp.hit_ray); cudaFree(pp.hit_cand); cudaFree(pp.surv); cudaFree(pp.ovf);
+      pp.hit_ray = nullptr; pp.hit_cand = nullptr; pp.surv = nullptr; pp.ovf = nullptr;
     }
     m->wave_cap = 0;
     for (int pi = 0; pi < kPipes; ++pi) {
@@ -695,6 +709,7 @@ int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
       TPMC_CUDA_TRY(cudaMalloc((void**)&pp.hit_ray, 2 * wave * sizeof(unsigned int)));
       TPMC_CUDA_TRY(cudaMalloc((void**)&pp.hit_cand, 2 * wave * sizeof(int4)));
       TPMC_CUDA_TRY(cudaMalloc((void**)&pp.surv, 3 * wave * sizeof(unsigned int)));
+      TPMC_CUDA_TRY(cudaMalloc((void**)&pp.ovf, 4 * wave * sizeof(unsigned int)));   // two lists (iteration parity)
     }
     m->wave_cap = wave;
   }
@@ -848,7 +863,9 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
       Pipe& pp = m->pipe[wv % K];
       const unsigned long long li = wv / K;            // iteration index within the pipeline
       const int p = (int)(li & 1);
-      cudaStream_t s1 = pp.main, s2 = no_overlap ? pp.main : pp.seed;
+      cudaStream_t s1 = pp.main, s2 = no_overlap ? pp.main : pp.seed, s3 = no_overlap ? pp.main : pp.side;
+      const int b = (int)(li & 1);
+      unsigned int* ovf = pp.ovf + (size_t)b * 2 * cap;
       RayQueue Q[2] = {{pp.q_o[0], pp.q_v[0], pp.q_f[0]}, {pp.q_o[1], pp.q_v[1], pp.q_f[1]}};
       const bool tw = timed && c0 == 0 && li < (unsigned long long)kMaxTimedWaves;
       cudaEvent_t* ev = tw ? pp.wave_ev + kEvPerWave * li : nullptr;
@@ -856,6 +873,8 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
         const unsigned int w0 = (unsigned int)(wv * wave);
         const unsigned int wn = (unsigned int)std::min<unsigned long long>(wave, cn - wv * wave);
         TPMC_CUDA_TRY(cudaStreamWaitEvent(s2, pp.ev_reset[li & 3], 0));
+        // region B of this queue may still be read by the straggler kernel of iteration li - 2
+        if (li >= 2) TPMC_CUDA_TRY(cudaStreamWaitEvent(s2, pp.ev_ovf[b], 0));
         if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[0], s2));
         const unsigned int gfull = (wn + kSeedBlock - 1) / kSeedBlock;
         if (precull) {
@@ -871,18 +890,27 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
         if (tw) pp.seed_iters = li + 1;
         ++launches;
       }
-      k_iter_begin<<<1, 32, 0, s1>>>(pp.ctr, p ^ 1);
+      k_iter_begin<<<1, 32, 0, s1>>>(pp.ctr, p ^ 1, b);
       TPMC_CUDA_TRY(cudaEventRecord(pp.ev_reset[(li + 1) & 3], s1));
       if (wv < n_waves) TPMC_CUDA_TRY(cudaStreamWaitEvent(s1, pp.ev_seeded[li & 3], 0));
       if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[2], s1));
       k_trace_wf<<<g.trace, kTraceBlock, 0, s1>>>(m->cnodes, qg, m->tris, Q[p], cap, pp.ctr + 2 * p, pp.ctr + 4, pp.hit_ray,
                                                   pp.hit_cand, pp.ctr + 5, m->stats, trace_tune());
       if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[3], s1));
-      k_reflect<<<g.reflect, kTraceBlock, 0, s1>>>(rcc, cap, m->nodes, m->tris, Q[p], pp.hit_ray, pp.hit_cand, pp.ctr + 5,
-                                                   Q[p ^ 1], pp.ctr + 2 * (p ^ 1), P, m->totals, m->stats, dbg);
+      // the straggler kernel of the previous iteration reads the queue this reflect step writes
+      if (li >= 1) TPMC_CUDA_TRY(cudaStreamWaitEvent(s1, pp.ev_ovf[b ^ 1], 0));
+      k_reflect<<<g.reflect, kTraceBlock, 0, s1>>>(rcc, cap, m->tris, Q[p], pp.hit_ray, pp.hit_cand, pp.ctr + 5, Q[p ^ 1],
+                                                   pp.ctr + 2 * (p ^ 1), ovf, pp.ctr + 8 + b, P, m->totals, m->stats, dbg);
       if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[4], s1));
+      // overflow list of this iteration: followed to escape on the side stream, beside the next traversal
+      TPMC_CUDA_TRY(cudaEventRecord(pp.ev_refl[b], s1));
+      TPMC_CUDA_TRY(cudaStreamWaitEvent(s3, pp.ev_refl[b], 0));
+      k_finish<<<g.finish / 4, kTraceBlock, 0, s3>>>(rcc, cap, m->nodes, m->tris, Q[p], ovf, pp.ctr + 8 + b, P, m->totals,
+                                                     m->stats, dbg);
+      TPMC_CUDA_TRY(cudaEventRecord(pp.ev_ovf[b], s3));
+      pp.last_iter = li;
       if (tw) pp.iters = li + 1;
-      launches += 4;
+      launches += 5;
     }
     // whatever still bounces after the drain iterations is followed to escape thread by thread; then join
     for (int pi = 0; pi < K; ++pi) {
@@ -890,8 +918,10 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
       const unsigned long long its = (n_waves + (unsigned long long)K * kDrain - pi + K - 1) / K;   // iterations it ran
       const int p = (int)(its & 1);
       RayQueue q = {pp.q_o[p], pp.q_v[p], pp.q_f[p]};
+      TPMC_CUDA_TRY(cudaStreamWaitEvent(pp.main, pp.ev_ovf[0], 0));   // join the side stream
+      TPMC_CUDA_TRY(cudaStreamWaitEvent(pp.main, pp.ev_ovf[1], 0));
       if (timed) TPMC_CUDA_TRY(cudaEventRecord(pp.ev_f0, pp.main));
-      k_finish<<<g.finish, kTraceBlock, 0, pp.main>>>(rcc, cap, m->nodes, m->tris, q, pp.ctr + 2 * p, P, m->totals,
+      k_finish<<<g.finish, kTraceBlock, 0, pp.main>>>(rcc, cap, m->nodes, m->tris, q, nullptr, pp.ctr + 2 * p, P, m->totals,
                                                      m->stats, dbg);
       if (timed) TPMC_CUDA_TRY(cudaEventRecord(pp.ev_f1, pp.main));
       ++launches;
