@@ -27,6 +27,9 @@ import numpy as np
 
 import tpmc_inputs as ti
 
+# dram__bytes_read.sum + dram__bytes_write.sum of one steady-state k_trace_wf launch (6.9 M rays), from the
+# `ncu --set full` capture summarised in profiles/r1_ncu_full_pipeline_v3.md
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 803_000_000
 METRIC = "particle_bounces_per_s"
 UNIT = "bounces/s"
 WORKLOAD = "C5: ~1.0e6-facet noise-displaced geodesic body + 6 panels, O/He 70/30, 900 K, 7700 m/s"
@@ -260,6 +263,15 @@ def main():
         bytes_per_launch = traced * per_seg / launches_trace
         avg_ms = ms_trace / launches_trace
         achieved = bytes_per_launch / (avg_ms * 1e-3) / 1e9 if avg_ms > 0 else 0.0
+        # ncu shows the kernel bound by instruction issue (DRAM 1-4 %, L2 < 20 %, issue slots ~72 % busy; profiles/),
+        # so the binding roofline is the fp32 lane-instruction rate: SMs x 128 lanes x SM clock under this load.
+        # Algorithmic fp32 work per segment: ceil(log2 T) node visits x 2 slab tests x 18 ops + one
+        # watertight facet test of 60 ops; none of it pairs into FMAs, so one op = one lane-instruction.
+        ops_per_seg = int(np.ceil(np.log2(mesh.nt))) * 2 * 18 + 60
+        sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        clk_mhz = clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965.0
+        alu_peak = sms * 128 * clk_mhz * 1e6 / 1e12                      # T lane-op/s
+        alu_ach = (traced * ops_per_seg / launches_trace) / (avg_ms * 1e-3) / 1e12 if avg_ms > 0 else 0.0
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_total_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -271,9 +283,14 @@ def main():
             "clocks": clocks,
             "rates": {"segments_per_s": segs_all / (ms_total_max * 1e-3), "particles_per_s": parts_all / (ms_total_max * 1e-3),
                       "hits_per_particle": hits_all / parts_all},
-            "roofline": {"kernel": "k_trace_wf", "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                         "algorithmic_bytes_per_segment": per_seg, "segments_per_launch": traced / launches_trace,
+            "roofline": {"kernel": "k_trace_wf", "bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "TFLOP/s",
+                         "frac": alu_ach / alu_peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
+                         "peak_source": f"derived: {sms} SMs x 128 fp32 lanes x {clk_mhz:.0f} MHz sampled under this load "
+                                        "(one lane-instruction = 1 op; DESIGN.md section 7)",
+                         "algorithmic_ops_per_segment": ops_per_seg,
+                         "hbm_view": {"achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                                      "peak_source": peak_src, "algorithmic_bytes_per_segment": per_seg},
+                         "segments_per_launch": traced / launches_trace,
                          "avg_launch_ms": avg_ms, "launches_timed": int(launches_trace),
                          "share_of_step": {"k_seed": ms_seed / ms_stat if ms_stat else None,
                                            "k_trace_wf": ms_trace / ms_stat if ms_stat else None,

@@ -11,6 +11,7 @@
 namespace {
 
 constexpr int kSeedBlock = 128;
+constexpr int kPrecullBlock = 256;
 constexpr int kTraceBlock = 128;
 constexpr int kReduceBlock = 256;
 constexpr int kReduceParts = 296;   // 2 per SM
@@ -57,12 +58,12 @@ __global__ void k_iter_begin(unsigned int* __restrict__ ctr, int out_parity, int
 // a2, pre-cull pass (sampling.cuh): fp32 estimate of every particle's ray against the grown bounds.  Survivor
 // records (wave offset, fp32 roots) of certified estimates fill `surv` from the front, particles whose
 // estimate is not certified from the back; n_surv[0], n_surv[1] count them.  surv = [3][cap] words.
-__global__ void __launch_bounds__(kSeedBlock) k_seed_precull(const SeedConstF sf, unsigned int seed_lo,
-                                                             unsigned int seed_hi, unsigned long long first,
-                                                             unsigned int wave_n, unsigned int cap,
-                                                             unsigned int* __restrict__ surv,
-                                                             unsigned int* __restrict__ n_surv,
-                                                             unsigned long long* __restrict__ stats) {
+__global__ void __launch_bounds__(kPrecullBlock) k_seed_precull(const SeedConstF sf, unsigned int seed_lo,
+                                                                unsigned int seed_hi, unsigned long long first,
+                                                                unsigned int wave_n, unsigned int cap,
+                                                                unsigned int* __restrict__ surv,
+                                                                unsigned int* __restrict__ n_surv) {
+  __shared__ unsigned int s_cnt[2][kPrecullBlock / 32], s_base[2];
   const unsigned int j = blockIdx.x * blockDim.x + threadIdx.x;
   const bool active = j < wave_n;
   float o[3], v[3], root[2];
@@ -71,23 +72,23 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed_precull(const SeedConstF sf
   const bool keep_c = active && ok && touch, keep_u = active && !ok;
   const unsigned mcert = __ballot_sync(0xFFFFFFFFu, keep_c);
   const unsigned munc = __ballot_sync(0xFFFFFFFFu, keep_u);
-  const unsigned mcull = __ballot_sync(0xFFFFFFFFu, active && ok && !touch);
-  const int lane = threadIdx.x & 31;
-  unsigned base_c = 0, base_u = 0;
-  if (lane == 0) {
-    if (mcert) base_c = atomicAdd(&n_surv[0], (unsigned)__popc(mcert));
-    if (munc) base_u = atomicAdd(&n_surv[1], (unsigned)__popc(munc));
-    if (mcull) atomicAdd(&stats[ST_CULLED], (unsigned long long)__popc(mcull));
+  // one atomic per block and list (a per-warp atomic on one address was the kernel's bottleneck)
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (lane == 0) { s_cnt[0][wid] = __popc(mcert); s_cnt[1][wid] = __popc(munc); }
+  __syncthreads();
+  if (threadIdx.x < 2) {
+    unsigned int tot = 0;
+    for (int k = 0; k < kPrecullBlock / 32; ++k) { const unsigned int c = s_cnt[threadIdx.x][k]; s_cnt[threadIdx.x][k] = tot; tot += c; }
+    s_base[threadIdx.x] = tot ? atomicAdd(&n_surv[threadIdx.x], tot) : 0u;
   }
-  base_c = __shfl_sync(0xFFFFFFFFu, base_c, 0);
-  base_u = __shfl_sync(0xFFFFFFFFu, base_u, 0);
+  __syncthreads();
   if (keep_c) {
-    const unsigned slot = base_c + __popc(mcert & lanemask_lt());
+    const unsigned slot = s_base[0] + s_cnt[0][wid] + __popc(mcert & lanemask_lt());
     surv[slot] = j;
     surv[cap + slot] = __float_as_uint(root[0]);
     surv[2 * cap + slot] = __float_as_uint(root[1]);
   }
-  if (keep_u) surv[cap - 1u - (base_u + __popc(munc & lanemask_lt()))] = j;
+  if (keep_u) surv[cap - 1u - (s_base[1] + s_cnt[1][wid] + __popc(munc & lanemask_lt()))] = j;
 }
 
 // a2: seed particles of one wave in fp64, round the state to fp32 (O9), drop the rays that cannot touch the
@@ -97,12 +98,14 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed_precull(const SeedConstF sf
 __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned int wave_first,
                                                      unsigned int wave_n, const unsigned int* __restrict__ surv,
                                                      unsigned int cap_s, const unsigned int* __restrict__ n_surv,
-                                                     const float4* __restrict__ cull,
+                                                     const float4* __restrict__ cull, int walk,
                                                      const RayQueue q, unsigned int region_b,
                                                      unsigned int* __restrict__ qcount,
                                                      unsigned long long* __restrict__ stats) {
   const unsigned int n1 = surv ? n_surv[0] : 0u;                 // certified survivors: fp32 roots available
   const unsigned int n = surv ? n1 + n_surv[1] : wave_n;
+  if (blockIdx.x == 0 && threadIdx.x == 0 && n < wave_n)         // dropped by the pre-cull pass
+    atomicAdd(&stats[ST_CULLED], (unsigned long long)(wave_n - n));
   const unsigned int stride = gridDim.x * blockDim.x;
   const unsigned int nround = ((n + stride - 1) / stride) * stride;   // keep warps converged for the ballots
   for (unsigned int kk = blockIdx.x * blockDim.x + threadIdx.x; kk < nround; kk += stride) {
@@ -124,7 +127,7 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
     float tn;
     float te;
     keep = slab(rc.aabb_lo[0], rc.aabb_lo[1], rc.aabb_lo[2], rc.aabb_hi[0], rc.aabb_hi[1], rc.aabb_hi[2], o, id,
-                INFINITY, tn) && cull_touch(cull, o, id, te);
+                INFINITY, tn) && (!walk || cull_touch(cull, o, id, te));
   }
   const unsigned m = __ballot_sync(0xFFFFFFFFu, keep);
   const unsigned mc = __ballot_sync(0xFFFFFFFFu, active && !keep);
@@ -164,6 +167,7 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
 #define TPMC_TRACE_MIN_BLOCKS 8
 #endif
 struct TraceTune { int node_min, refill_idle; };
+constexpr int kFetchChunk = 64;   // rays a warp reserves per atomic on the queue head
 
 __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf(const uint4* __restrict__ cnodes,
                                                              const QuantGrid grid,
@@ -182,30 +186,36 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
   const int lane = threadIdx.x & 31;
   const unsigned FULL = 0xFFFFFFFFu;
   bool has = false, exhausted = false, fin = false;
-  unsigned int r = 0;
+  unsigned int r = 0, pool_next = 0, pool_end = 0;
   Walk w;
   w.cur = TPMC_SENTINEL; w.stash = 0; w.sp = 0; w.nc = 0; w.tmax = 0.0f; w.f_prev = -1;
   TraceCounters cnt;
   cnt.nodes = 0; cnt.tris = 0;
   for (;;) {
-    // ---- refill idle lanes
+    // ---- refill idle lanes from the warp's chunk of the queue (one atomic per kFetchChunk rays)
     const unsigned idle = __ballot_sync(FULL, !has && !exhausted);
     const unsigned busy0 = __ballot_sync(FULL, has);
     if (idle && (__popc(idle) >= kRefillIdle || busy0 == 0u)) {
-      const int leader = __ffs(idle) - 1;
-      unsigned base = 0;
-      if (lane == leader) base = atomicAdd(next_ray, (unsigned)__popc(idle));
-      base = __shfl_sync(FULL, base, leader);
+      if (pool_next == pool_end) {
+        unsigned base = 0;
+        if (lane == 0) base = atomicAdd(next_ray, (unsigned)kFetchChunk);
+        pool_next = __shfl_sync(FULL, base, 0);
+        pool_end = pool_next + kFetchChunk;
+      }
+      const unsigned avail = pool_end - pool_next, rank = __popc(idle & lanemask_lt());
       if (!has && !exhausted) {
-        r = base + __popc(idle & lanemask_lt());
-        if (r < n) {
-          r = (r < na) ? r : cap + (r - na);   // physical slot
-          walk_init(w, grid, q.o[r], q.v[r], q.f[r]);
-          has = true;
-        } else {
+        if (pool_next >= n) {
           exhausted = true;
+        } else if (rank < avail) {
+          r = pool_next + rank;
+          if (r < n) {
+            r = (r < na) ? r : cap + (r - na);   // physical slot
+            walk_init(w, grid, q.o[r], q.v[r], q.f[r]);
+            has = true;
+          }
         }
       }
+      pool_next += min((unsigned)__popc(idle), avail);
     }
     if (__ballot_sync(FULL, has) == 0u) break;
     // ---- node phase: two node steps per vote
@@ -730,7 +740,7 @@ const Grids& grids() {
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_trace_wf, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
     // resident trace CTAs per SM over all pipelines (measured: leaving room for the seed kernel does not pay)
     int tot = std::max(1, per);
-    if (const char* e = getenv("TPMC_TRACE_BLOCKS")) tot = std::max(1, std::min(per, atoi(e)));
+    if (const char* e = getenv("TPMC_TRACE_BLOCKS")) tot = std::max(1, std::min(4 * per, atoi(e)));
     g.trace = sms * std::max(1, tot / g.pipes);
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_reflect, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
     g.reflect = sms * std::max(1, per / g.pipes);
@@ -811,6 +821,7 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
   const bool timed = (h_stats != nullptr);   // per-kernel events only when the caller will read them
   const char* pc_env = getenv("TPMC_PRECULL");   // read per call: the parity tests switch the pass off and on
   const bool precull = !(pc_env && pc_env[0] == '0');
+  static const int seed_walk = (getenv("TPMC_SEED_WALK") && getenv("TPMC_SEED_WALK")[0] == '0') ? 0 : 1;   // tuning aid
   SeedConstF sf;
   make_seed_const_f(m, rc, &sf);
   const QuantGrid qg = quant_grid(m);
@@ -879,12 +890,13 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
         const unsigned int gfull = (wn + kSeedBlock - 1) / kSeedBlock;
         if (precull) {
           TPMC_CUDA_TRY(cudaMemsetAsync(pp.ctr + 6, 0, 2 * sizeof(unsigned int), s2));
-          k_seed_precull<<<gfull, kSeedBlock, 0, s2>>>(sf, rcc.seed_lo, rcc.seed_hi, rcc.first + w0, wn, cap, pp.surv,
-                                                       pp.ctr + 6, m->stats);
+          k_seed_precull<<<(wn + kPrecullBlock - 1) / kPrecullBlock, kPrecullBlock, 0, s2>>>(
+              sf, rcc.seed_lo, rcc.seed_hi, rcc.first + w0, wn, cap, pp.surv, pp.ctr + 6);
           ++launches;
         }
         k_seed<<<std::min<unsigned int>(gfull, (unsigned int)g.seed), kSeedBlock, 0, s2>>>(
-            rcc, w0, wn, precull ? pp.surv : nullptr, cap, pp.ctr + 6, m->cull, Q[p], cap, pp.ctr + 2 * p + 1, m->stats);
+            rcc, w0, wn, precull ? pp.surv : nullptr, cap, pp.ctr + 6, m->cull, seed_walk, Q[p], cap, pp.ctr + 2 * p + 1,
+            m->stats);
         if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[1], s2));
         TPMC_CUDA_TRY(cudaEventRecord(pp.ev_seeded[li & 3], s2));
         if (tw) pp.seed_iters = li + 1;

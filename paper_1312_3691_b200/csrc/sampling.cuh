@@ -270,6 +270,26 @@ struct SeedConstF {
 
 __device__ __forceinline__ float u01f(uint32_t w) { return ((float)w + 0.5f) * 2.3283064365386963e-10f; }
 
+// erfc(x) with fractional error ~2e-7 in ~20 instructions (the library erfcf costs ~45): the classical
+// Chebyshev fit erfc(z) = t exp(-z^2 + P(t)), t = 1/(1 + z/2), z >= 0 (Numerical Recipes' erfcc coefficients),
+// erfc(-z) = 2 - erfc(z).  Used by the pre-cull estimate only; its tolerances (1e-5, 1e-4) are far above this.
+__device__ __forceinline__ float erfc_fast(float x) {
+  const float z = fabsf(x);
+  const float t = __fdividef(1.0f, fmaf(0.5f, z, 1.0f));
+  float p = 0.17087277f;
+  p = fmaf(p, t, -0.82215223f);
+  p = fmaf(p, t, 1.48851587f);
+  p = fmaf(p, t, -1.13520398f);
+  p = fmaf(p, t, 0.27886807f);
+  p = fmaf(p, t, -0.18628806f);
+  p = fmaf(p, t, 0.09678418f);
+  p = fmaf(p, t, 0.37409196f);
+  p = fmaf(p, t, 1.00002368f);
+  p = fmaf(p, t, -1.26551223f);
+  const float r = t * __expf(fmaf(-z, z, p));
+  return x >= 0.0f ? r : 2.0f - r;
+}
+
 // y = S sin(phi) to ~1e-6 relative, ok = certified
 __device__ __forceinline__ float approx_y(float u, const SpeciesF& sc, bool& ok) {
   const float S = sc.S;
@@ -280,7 +300,7 @@ __device__ __forceinline__ float approx_y(float u, const SpeciesF& sc, bool& ok)
 #pragma unroll
   for (int it = 0; it < 3; ++it) {
     const float e = __expf(-y * y);
-    const float ec = erfcf(-y);
+    const float ec = erfc_fast(-y);
     const float g = 0.25f * TPMC_SQRTPI_F * fmaf(2.0f * y, y, 1.0f) * ec + 0.5f * y * e;
     const float d = fmaf(TPMC_SQRTPI_F * y, ec, e);
     const float yn = fminf(S, fmaxf(-S, y - __fdividef(g - T, d)));
@@ -294,7 +314,7 @@ __device__ __forceinline__ float approx_y(float u, const SpeciesF& sc, bool& ok)
 
 // x_n = v_n / c_mp to ~1e-4 relative, ok = certified.  omu = 1 - u
 __device__ __forceinline__ float approx_normal_speed(float omu, float s, bool& ok) {
-  const float chis = fmaf(TPMC_SQRTPI_F * s, erfcf(-s), __expf(-s * s));
+  const float chis = fmaf(TPMC_SQRTPI_F * s, erfc_fast(-s), __expf(-s * s));
   const float T = omu * chis;
   const float xm = 0.5f * (s + sqrtf(fmaf(s, s, 2.0f)));
   const float tau = fminf(fmaxf(__fdividef(T, TPMC_SQRTPI_F * s), 1e-30f), 1.9999f);
@@ -307,7 +327,7 @@ __device__ __forceinline__ float approx_normal_speed(float omu, float s, bool& o
   for (int it = 0; it < 3; ++it) {
     const float z = x - s;
     e = __expf(-z * z);
-    q = fmaf(TPMC_SQRTPI_F * s, erfcf(z), e);
+    q = fmaf(TPMC_SQRTPI_F * s, erfc_fast(z), e);
     float xn = x + __fdividef(q - T, 2.0f * x * e);
     xn = (xn > 0.0f) ? xn : 0.5f * x;
     step = fabsf(xn - x);

@@ -180,8 +180,8 @@ __device__ __forceinline__ bool slab(float lx, float ly, float lz, float hx, flo
 // carry an offset of 2^23 (q_lo16/q_hi16): their difference is exact while the origin is within ~2^23 steps of
 // the grid, and otherwise rounds once more (relative u, inside the margin); the outward rounding of the
 // shifted origin grows the box by less than one further step.  What is left is
-// relative: d' (2 roundings), its reciprocal, the difference and the product: <= 5u on each plane distance;
-// the margin on entry and exit is 8u.
+// relative: d' (2 roundings), its approximate reciprocal (2u), the difference and the product: <= 6u on each
+// plane distance; the margin on entry and exit is 8u.
 __device__ __forceinline__ bool slab_q(float lx, float ly, float lz, float hx, float hy, float hz, const float ol[3],
                                        const float oh[3], const float id[3], float tmax, float& tnear) {
   const float u8 = 4.76837158203125e-07f;  // 8 * 2^-24
@@ -268,7 +268,7 @@ __device__ __forceinline__ void walk_init(Walk& w, const QuantGrid& g, const flo
     const float e = 2.384185791015625e-07f * fabsf(oq);   // 4u |o'|
     w.ol[k] = __fadd_ru(8388608.0f, oq + e);   // >= 2^23 + o' + e: low planes are measured from a point not below it
     w.oh[k] = __fadd_rd(8388608.0f, oq - e);   // <= 2^23 + o' - e
-    w.id[k] = 1.0f / (d[k] * g.inv_scale[k]);
+    w.id[k] = __fdividef(1.0f, d[k] * g.inv_scale[k]);   // 2 ulp: the margin of slab_q has room for it
   }
   w.tmax = INFINITY;
   w.f_prev = f_prev;
@@ -335,23 +335,27 @@ __device__ __forceinline__ void walk_node(Walk& w, const uint4* __restrict__ cno
                          w.tmax, t0);
   const bool h1 = slab_q(q_lo16(a.w), q_hi16(a.w), q_lo16(b.x), q_hi16(b.x), q_lo16(b.y), q_hi16(b.y), w.ol, w.oh, w.id,
                          w.tmax, t1);
-  // branch-free child selection: near child next, far child pushed when both boxes are hit, pop when none is
+  // Branch-free child selection and stack traffic: the near child is next, the far child is stored above the
+  // top of the stack whether it is needed or not (it only counts when both boxes are hit), and the entry below
+  // the top is always read (it only counts when no box is hit).
   const bool both = h0 && h1, any = h0 || h1;
   const bool second = both ? (t1 < t0) : !h0;
   const int c0 = (int)b.z, c1 = (int)b.w;
   const int nearc = second ? c1 : c0, farc = second ? c0 : c1;
-  if (both) {
-    if (w.sp >= TPMC_STACK_SMEM) { walk_abort(w); return; }
-    stk[w.sp * sstride] = farc;
-    ++w.sp;
-  }
-  const int popped = any ? 0 : walk_pop(w, stk, sstride);
-  w.cur = any ? nearc : popped;
-  // speculation: a leaf is put aside and the walk goes on; it is tested in the next leaf phase
-  if (w.cur < 0 && w.stash == 0) {
-    w.stash = w.cur;
-    w.cur = walk_pop(w, stk, sstride);
-  }
+  if (both && w.sp >= TPMC_STACK_SMEM) { walk_abort(w); return; }   // rare
+  const int top = stk[max(w.sp - 1, 0) * sstride], top2 = stk[max(w.sp - 2, 0) * sstride];
+  stk[min(w.sp, TPMC_STACK_SMEM - 1) * sstride] = farc;
+  const bool pop1 = !any && w.sp > 0;
+  w.cur = any ? nearc : (pop1 ? top : TPMC_SENTINEL);
+  w.sp += (both ? 1 : 0) - (pop1 ? 1 : 0);
+  // speculation: a leaf is put aside and the walk goes on; it is tested in the next leaf phase.  The entry to
+  // pop is the far child just pushed, the old top (nothing pushed or popped), or the one below it (popped).
+  const bool take = w.cur < 0 && w.stash == 0;
+  const bool pop2 = take && w.sp > 0;
+  const int below = both ? farc : (any ? top : top2);
+  w.stash = take ? w.cur : w.stash;
+  w.cur = take ? (pop2 ? below : TPMC_SENTINEL) : w.cur;
+  w.sp -= pop2 ? 1 : 0;
 }
 
 // One leaf step (fp32 facet classification of the leaf put aside), then the next leaf, if the walk stands at
