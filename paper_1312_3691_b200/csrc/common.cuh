@@ -77,7 +77,7 @@ struct tpmc_mesh {
 
 constexpr int kMaxTimedWaves = 1024;  // iterations covered by the per-kernel event times
 constexpr int kDrain = 3;             // trace/reflect iterations after the last wave, before the straggler kernel
-constexpr int kEvPerWave = 5;         // seed start/end (seed stream), trace start, after trace, after reflect
+constexpr int kEvPerWave = 7;         // seed start/end (seed stream), trace start, after trace, after reflect, straggler start/end (side stream)
 constexpr int kCtrWords = 16;
 constexpr int kCullNodes = 64;        // 4 KB: stays in L1 next to the shared-memory carve-out
 constexpr float kPrecullMargin = 2e-2f;   // box growth of the pre-cull pass, in bounding radii (sampling.cuh)

@@ -185,11 +185,12 @@ __global__ void k_single(const float* __restrict__ box_leaf, float4* __restrict_
 }
 
 // Compact copy of the hierarchy for the wavefront traversal: 32 B per node = one 256-bit load.
-//   words 0-2: child 0 box, words 3-5: child 1 box, each (lo.x | lo.y << 16, lo.z | hi.x << 16, hi.y | hi.z << 16)
-//   as unsigned 16-bit grid coordinates, words 6-7: the two child refs.
-// Grid: x = origin + q * scale per axis.  lo is rounded down and hi up, then both are moved out by one more
-// grid step: the decoded box contains the fp32 box grown by `scale`, which covers the rounding of the ray's
-// transform into grid coordinates in the traversal (<= 0.012 steps, see slab_q in trace.cuh).
+//   words 0-2: child 0 box, words 3-5: child 1 box, one word per axis: lo | hi << 16 as unsigned 16-bit grid
+//   coordinates (so that one byte permute yields the near or the far plane of an axis, see trace.cuh);
+//   words 6-7: the two child refs.
+// Grid: x = origin + q * scale per axis.  lo is rounded down and hi up: the decoded box contains the fp32 box.
+// (The quotient is evaluated in fp64: a box corner within 1e-11 steps of a grid plane may land on the wrong
+// side of it, which the slack of the traversal's margin G covers.)
 __global__ void k_compact_nodes(const float4* __restrict__ nodes, int64_t n_nodes, double ox, double oy, double oz,
                                 double sx, double sy, double sz, uint4* __restrict__ cnodes) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
@@ -199,18 +200,16 @@ __global__ void k_compact_nodes(const float4* __restrict__ nodes, int64_t n_node
   const float hi[2][3] = {{n0.w, n1.x, n1.y}, {n2.y, n2.z, n2.w}};
   const double o[3] = {ox, oy, oz}, sc[3] = {sx, sy, sz};
   unsigned int w[6];
-  for (int c = 0; c < 2; ++c) {
-    unsigned int ql[3], qh[3];
+  for (int c = 0; c < 2; ++c)
     for (int a = 0; a < 3; ++a) {
-      if (lo[c][a] > hi[c][a]) { ql[a] = 65535u; qh[a] = 0u; continue; }   // empty box (single-triangle mesh)
-      const double l = floor(((double)lo[c][a] - o[a]) / sc[a]) - 1.0, h = ceil(((double)hi[c][a] - o[a]) / sc[a]) + 1.0;
-      ql[a] = (unsigned int)fmin(fmax(l, 0.0), 65535.0);
-      qh[a] = (unsigned int)fmin(fmax(h, 0.0), 65535.0);
+      unsigned int ql = 65535u, qh = 0u;   // empty box (single-triangle mesh): near plane beyond the far plane
+      if (lo[c][a] <= hi[c][a]) {
+        const double l = floor(((double)lo[c][a] - o[a]) / sc[a]), h = ceil(((double)hi[c][a] - o[a]) / sc[a]);
+        ql = (unsigned int)fmin(fmax(l, 0.0), 65535.0);
+        qh = (unsigned int)fmin(fmax(h, 0.0), 65535.0);
+      }
+      w[3 * c + a] = ql | (qh << 16);
     }
-    w[3 * c + 0] = ql[0] | (ql[1] << 16);
-    w[3 * c + 1] = ql[2] | (qh[0] << 16);
-    w[3 * c + 2] = qh[1] | (qh[2] << 16);
-  }
   cnodes[2 * i] = make_uint4(w[0], w[1], w[2], w[3]);
   cnodes[2 * i + 1] = make_uint4(w[4], w[5], __float_as_uint(n3.x), __float_as_uint(n3.y));
 }

@@ -180,8 +180,10 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
                                                              unsigned long long* __restrict__ stats,
                                                              const TraceTune tune) {
   const int kNodeMin = tune.node_min, kRefillIdle = tune.refill_idle;
-  __shared__ int sstack[TPMC_STACK_SMEM * kTraceBlock];
-  int* stk = sstack + threadIdx.x;
+  __shared__ int sstack[(TPMC_STACK_SMEM + 2) * kTraceBlock];
+  int* stk = sstack + 2 * kTraceBlock + threadIdx.x;   // level 0; levels -1, -2 are the guard entries (walk_pop)
+  stk[-kTraceBlock] = TPMC_SENTINEL;
+  stk[-2 * kTraceBlock] = TPMC_SENTINEL;
   const unsigned int na = min(n_rays[0], cap), n = na + n_rays[1];   // region A (reflected), region B (primaries)
   const int lane = threadIdx.x & 31;
   const unsigned FULL = 0xFFFFFFFFu;
@@ -785,6 +787,12 @@ int fill_stats(tpmc_mesh* m, const tpmc_params* params, tpmc_stats* h_stats) {
       h_stats->ms_trace += t;
       TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[3], ev[4]));
       h_stats->ms_reflect += t;
+      if (getenv("TPMC_TIMELINE") && w >= 20 && w < 26 && w < pp.seed_iters) {   // diagnosis: event times since the run began
+        float a[7];
+        for (int k = 0; k < 7; ++k) cudaEventElapsedTime(&a[k], m->ev0, ev[k]);
+        fprintf(stderr, "iter %llu: seed %.3f-%.3f trace %.3f-%.3f reflect -%.3f finish %.3f-%.3f\n", w, a[0], a[1], a[2], a[3], a[4],
+                a[5], a[6]);
+      }
     }
     h_stats->timed_waves += pp.seed_iters;
     h_stats->trace_launches += pp.iters;
@@ -917,8 +925,10 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
       // overflow list of this iteration: followed to escape on the side stream, beside the next traversal
       TPMC_CUDA_TRY(cudaEventRecord(pp.ev_refl[b], s1));
       TPMC_CUDA_TRY(cudaStreamWaitEvent(s3, pp.ev_refl[b], 0));
+      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[5], s3));
       k_finish<<<g.finish / 4, kTraceBlock, 0, s3>>>(rcc, cap, m->nodes, m->tris, Q[p], ovf, pp.ctr + 8 + b, P, m->totals,
                                                      m->stats, dbg);
+      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[6], s3));
       TPMC_CUDA_TRY(cudaEventRecord(pp.ev_ovf[b], s3));
       pp.last_iter = li;
       if (tw) pp.iters = li + 1;

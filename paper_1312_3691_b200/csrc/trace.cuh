@@ -172,28 +172,28 @@ __device__ __forceinline__ bool slab(float lx, float ly, float lz, float hx, flo
 }
 
 // ---- the same test on a box of the compact hierarchy (grid coordinates, see k_compact_nodes) ----------
-// The ray is carried in grid coordinates: o' = (o - origin) * inv_scale, 1/d' with d' = d * inv_scale; the ray
-// parameter t is unchanged.  o' carries three roundings (difference, the rounded inv_scale, product): it is
-// off by <= 3u|o'| grid steps, so the walk keeps o' + e and o' - e with e = 4u|o'| and measures the low planes
-// from the first and the high planes from the second -- the slab test of the box grown by e, which together
-// with the one-step growth applied at encoding contains the fp32 box for any origin.  Planes and origins both
-// carry an offset of 2^23 (q_lo16/q_hi16): their difference is exact while the origin is within ~2^23 steps of
-// the grid, and otherwise rounds once more (relative u, inside the margin); the outward rounding of the
-// shifted origin grows the box by less than one further step.  What is left is
-// relative: d' (2 roundings), its approximate reciprocal (2u), the difference and the product: <= 6u on each
-// plane distance; the margin on entry and exit is 8u.
-__device__ __forceinline__ bool slab_q(float lx, float ly, float lz, float hx, float hy, float hz, const float ol[3],
-                                       const float oh[3], const float id[3], float tmax, float& tnear) {
-  const float u8 = 4.76837158203125e-07f;  // 8 * 2^-24
-  const float ax = (lx - ol[0]) * id[0], bx = (hx - oh[0]) * id[0];
-  const float ay = (ly - ol[1]) * id[1], by = (hy - oh[1]) * id[1];
-  const float az = (lz - ol[2]) * id[2], bz = (hz - oh[2]) * id[2];
-  float tn = fmaxf(fmaxf(fminf(ax, bx), fminf(ay, by)), fminf(az, bz));
-  float tf = fminf(fminf(fmaxf(ax, bx), fmaxf(ay, by)), fmaxf(az, bz));
-  tn = fmaf(-u8, fabsf(tn), tn);
-  tf = fmaf(u8, fabsf(tf), tf);
-  tnear = tn;
-  return fmaxf(tn, 0.0f) <= fminf(tf, tmax);
+// The ray is carried in grid coordinates: o' = (o - origin) * inv_scale, d' = d * inv_scale; the ray
+// parameter t is unchanged.  A plane q (unsigned 16-bit grid coordinate) is crossed at
+//     t = (q - o') / d' = P * id - O * id,     P = 2^23 + q,  O = 2^23 + o',  id = 1 / d'.
+// P comes out of the node word by ONE byte permute (the float 0x4B00qqqq is exactly 2^23 + q), and the ray's
+// octant decides per axis which half of the word is the near plane and which the far one (sel_n, sel_f are
+// permute selectors fixed per ray), so a plane distance costs one PRMT and one FFMA and the slab test needs
+// no per-axis min/max:      t_near_k = fma(P_near, id_k, ncn_k),   t_far_k = fma(P_far, id_k, ncf_k).
+// ncn_k = -(O id) - G |id|,  ncf_k = -(O id) + G |id|: every error of this evaluation is bounded by a growth
+// of the box by G_k grid steps along axis k, so the test is conservative for the fp32 box the node encodes:
+//   * o' carries three roundings (difference, rounded inv_scale, product): <= 3u |o'| steps;
+//   * O = fl(2^23 + o') and the rounding of fma(-O, id, -+G|id|): <= u |O| steps each;
+//   * id = 1/d' carries <= 5u relative (rounded inv_scale, product, 2-ulp reciprocal), which scales the
+//     distance |P - O| <= |o'| + 2^16 steps; the final FFMA rounds once more, u relative;
+//   * the rounded inv_scale moves a plane by <= u q <= 0.004 steps.
+// Sum <= 2u|O| + 9u|o'| + 0.03; G_k = 2.5u|O| + 10u|o'| + 0.1 (about 1.4 steps of the 16-bit grid for an origin
+// inside or near the grid; it scales with the origin for a ray that starts far outside, e.g. on a flat axis).
+// A zero direction component gives id = inf and NaN plane distances, which fminf/fmaxf drop: the axis then
+// does not constrain the ray (conservative).
+__device__ __forceinline__ float q_plane(unsigned int w, unsigned int sel) {
+  unsigned int r;   // prmt.b32 directly: __byte_perm masks the selector first (one LOP3 per use)
+  asm("prmt.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(w), "r"(0x4B000000u), "r"(sel));
+  return __uint_as_float(r);
 }
 
 __device__ __forceinline__ void ldg256u(const uint4* p, uint4& a, uint4& b) {
@@ -201,10 +201,6 @@ __device__ __forceinline__ void ldg256u(const uint4* p, uint4& a, uint4& b) {
                : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w), "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w)
                : "l"(p));
 }
-// 16-bit grid coordinate q -> the float 2^23 + q, by one byte permute (no integer-to-float conversion): the
-// walk keeps the ray origin shifted by 2^23 as well (rounded outwards), so plane - origin is exact.
-__device__ __forceinline__ float q_lo16(unsigned int w) { return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610)); }
-__device__ __forceinline__ float q_hi16(unsigned int w) { return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7632)); }
 
 // ---- seed-time cull: can the ray touch any cut-off subtree of the top tree? (conservative) ------------
 // Near child first, so the first cut-off box found is (nearly) the first along the ray; its entry
@@ -249,7 +245,9 @@ __device__ __forceinline__ bool cull_touch(const float4* __restrict__ cull, cons
 
 // ---- per-ray traversal state of the wavefront kernel -------------------------------------------------
 struct Walk {
-  float ol[3], oh[3], id[3];   // grid coordinates: 2^23 + o' + e (rounded up), 2^23 + o' - e (rounded down), 1/d'
+  float id[3];         // 1/d' (grid coordinates)
+  float ncn[3], ncf[3];   // -(O id) -+ G |id|: offsets of the near and far plane distances (see above)
+  unsigned int sn[3], sf[3];   // byte-permute selectors of the near and far plane of each axis
   float tmax;          // min over provable hits of their thi
   int f_prev;
   int cur;             // node to visit next (>= 0 internal, < 0 leaf ~slot), TPMC_SENTINEL when the stack is empty
@@ -264,11 +262,18 @@ __device__ __forceinline__ void walk_init(Walk& w, const QuantGrid& g, const flo
   const float o[3] = {ro.x, ro.y, ro.z}, d[3] = {rv.x, rv.y, rv.z};
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
+    const float dq = d[k] * g.inv_scale[k];
+    const float idk = __fdividef(1.0f, dq);                  // 2 ulp
     const float oq = (o[k] - g.origin[k]) * g.inv_scale[k];
-    const float e = 2.384185791015625e-07f * fabsf(oq);   // 4u |o'|
-    w.ol[k] = __fadd_ru(8388608.0f, oq + e);   // >= 2^23 + o' + e: low planes are measured from a point not below it
-    w.oh[k] = __fadd_rd(8388608.0f, oq - e);   // <= 2^23 + o' - e
-    w.id[k] = __fdividef(1.0f, d[k] * g.inv_scale[k]);   // 2 ulp: the margin of slab_q has room for it
+    const float O = 8388608.0f + oq;
+    const float G = fmaf(1.4901161e-07f, fabsf(O), fmaf(5.9604645e-07f, fabsf(oq), 0.1f));   // 2.5u|O| + 10u|o'| + 0.1
+    const float mg = G * fabsf(idk);
+    w.id[k] = idk;
+    w.ncn[k] = fmaf(-O, idk, -mg);
+    w.ncf[k] = fmaf(-O, idk, mg);
+    const bool neg = dq < 0.0f;
+    w.sn[k] = neg ? 0x7632u : 0x7610u;
+    w.sf[k] = neg ? 0x7610u : 0x7632u;
   }
   w.tmax = INFINITY;
   w.f_prev = f_prev;
@@ -280,13 +285,14 @@ __device__ __forceinline__ void walk_init(Walk& w, const QuantGrid& g, const flo
   for (int k = 0; k < TPMC_MAX_CAND; ++k) { w.cs[k] = -1; w.cl[k] = 0.0f; }
 }
 
-// Stack: TPMC_STACK_SMEM entries per thread in shared memory, [level][thread].  A ray that needs more gives
-// up and is flagged for the full fp64 traversal of the resolve step (which has a deep stack), like a ray
-// with too many candidates.
+// Stack: TPMC_STACK_SMEM entries per thread in shared memory, [level][thread], above two guard entries that
+// hold TPMC_SENTINEL (`stk` points at level 0; levels -1 and -2 are the guards, so popping an empty stack needs
+// no test).  A ray that needs more gives up and is flagged for the full fp64 traversal of the resolve step
+// (which has a deep stack), like a ray with too many candidates.
 __device__ __forceinline__ int walk_pop(Walk& w, const int* stk, int sstride) {
-  const bool some = w.sp > 0;
-  w.sp -= some ? 1 : 0;
-  return some ? stk[w.sp * sstride] : TPMC_SENTINEL;
+  const int v = stk[(w.sp - 1) * sstride];
+  w.sp = max(w.sp - 1, 0);
+  return v;
 }
 
 __device__ __forceinline__ void walk_abort(Walk& w) {
@@ -325,37 +331,47 @@ __device__ __forceinline__ void walk_add_candidate(Walk& w, int slot, int cls, f
 }
 
 // One internal-node step (two slab tests, push the far child) -- requires w.cur >= 0 and != SENTINEL.
+// Node words: 0-2 = child 0 (x, y, z), 3-5 = child 1, each lo | hi << 16; 6-7 = the child refs.
 __device__ __forceinline__ void walk_node(Walk& w, const uint4* __restrict__ cnodes, int* stk, int sstride,
                                           TraceCounters& cnt) {
   uint4 a, b;
   ldg256u(cnodes + 2 * (size_t)w.cur, a, b);
   ++cnt.nodes;
-  float t0, t1;
-  const bool h0 = slab_q(q_lo16(a.x), q_hi16(a.x), q_lo16(a.y), q_hi16(a.y), q_lo16(a.z), q_hi16(a.z), w.ol, w.oh, w.id,
-                         w.tmax, t0);
-  const bool h1 = slab_q(q_lo16(a.w), q_hi16(a.w), q_lo16(b.x), q_hi16(b.x), q_lo16(b.y), q_hi16(b.y), w.ol, w.oh, w.id,
-                         w.tmax, t1);
-  // Branch-free child selection and stack traffic: the near child is next, the far child is stored above the
-  // top of the stack whether it is needed or not (it only counts when both boxes are hit), and the entry below
-  // the top is always read (it only counts when no box is hit).
+  const float n0 = fmaxf(fmaxf(fmaf(q_plane(a.x, w.sn[0]), w.id[0], w.ncn[0]), fmaf(q_plane(a.y, w.sn[1]), w.id[1], w.ncn[1])),
+                         fmaf(q_plane(a.z, w.sn[2]), w.id[2], w.ncn[2]));
+  const float f0 = fminf(fminf(fmaf(q_plane(a.x, w.sf[0]), w.id[0], w.ncf[0]), fmaf(q_plane(a.y, w.sf[1]), w.id[1], w.ncf[1])),
+                         fmaf(q_plane(a.z, w.sf[2]), w.id[2], w.ncf[2]));
+  const float n1 = fmaxf(fmaxf(fmaf(q_plane(a.w, w.sn[0]), w.id[0], w.ncn[0]), fmaf(q_plane(b.x, w.sn[1]), w.id[1], w.ncn[1])),
+                         fmaf(q_plane(b.y, w.sn[2]), w.id[2], w.ncn[2]));
+  const float f1 = fminf(fminf(fmaf(q_plane(a.w, w.sf[0]), w.id[0], w.ncf[0]), fmaf(q_plane(b.x, w.sf[1]), w.id[1], w.ncf[1])),
+                         fmaf(q_plane(b.y, w.sf[2]), w.id[2], w.ncf[2]));
+  // the clamps also drop a NaN that survived three NaN plane distances (zero direction)
+  const bool h0 = !(fmaxf(n0, 0.0f) > fminf(f0, w.tmax));
+  const bool h1 = !(fmaxf(n1, 0.0f) > fminf(f1, w.tmax));
+  // Branch-free child selection and stack traffic.  The near child is next and the far child is pushed; a leaf
+  // that becomes next while no leaf is put aside is put aside (speculation: it is tested in the next leaf
+  // phase) and the walk goes on with the far child, or with the top of the stack.  The two entries below the
+  // top are always read, the slot above it is written whenever both boxes are hit.
   const bool both = h0 && h1, any = h0 || h1;
-  const bool second = both ? (t1 < t0) : !h0;
+  const bool swp = h1 && (!h0 || n1 < n0);
   const int c0 = (int)b.z, c1 = (int)b.w;
-  const int nearc = second ? c1 : c0, farc = second ? c0 : c1;
+  const int nearc = swp ? c1 : c0, farc = swp ? c0 : c1;
   if (both && w.sp >= TPMC_STACK_SMEM) { walk_abort(w); return; }   // rare
-  const int top = stk[max(w.sp - 1, 0) * sstride], top2 = stk[max(w.sp - 2, 0) * sstride];
-  stk[min(w.sp, TPMC_STACK_SMEM - 1) * sstride] = farc;
-  const bool pop1 = !any && w.sp > 0;
-  w.cur = any ? nearc : (pop1 ? top : TPMC_SENTINEL);
-  w.sp += (both ? 1 : 0) - (pop1 ? 1 : 0);
-  // speculation: a leaf is put aside and the walk goes on; it is tested in the next leaf phase.  The entry to
-  // pop is the far child just pushed, the old top (nothing pushed or popped), or the one below it (popped).
-  const bool take = w.cur < 0 && w.stash == 0;
-  const bool pop2 = take && w.sp > 0;
-  const int below = both ? farc : (any ? top : top2);
-  w.stash = take ? w.cur : w.stash;
-  w.cur = take ? (pop2 ? below : TPMC_SENTINEL) : w.cur;
-  w.sp -= pop2 ? 1 : 0;
+  const int top = stk[(w.sp - 1) * sstride], top2 = stk[(w.sp - 2) * sstride];
+  if (both) stk[w.sp * sstride] = farc;
+  const bool empty = w.stash == 0;
+  const bool take = any && nearc < 0 && empty;       // the near child is a leaf: put it aside
+  const bool popleaf = !any && top < 0 && empty;     // nothing hit and the top of the stack is a leaf: likewise
+  const int x = both ? farc : top, y = popleaf ? top2 : top;
+  const int nx = take ? x : nearc;
+  w.cur = any ? nx : y;
+  if (popleaf) w.stash = top;
+  if (take) w.stash = nearc;
+  int sp = w.sp;
+  if (both) ++sp;
+  if (!any) --sp;
+  if (take || popleaf) --sp;
+  w.sp = max(sp, 0);
 }
 
 // One leaf step (fp32 facet classification of the leaf put aside), then the next leaf, if the walk stands at
