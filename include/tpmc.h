@@ -46,6 +46,7 @@ typedef struct {
   int64_t nt;              /* facets */
   int64_t n_nodes;         /* LBVH internal nodes (max(nt-1,1)), 64 B each */
   double build_ms;         /* device time of the LBVH build (Morton, sort, hierarchy, refit) */
+  double horizon_ms;       /* device time of the per-facet escape-horizon pass that follows it */
 } tpmc_mesh_info_t;
 
 /* Gas, control volume and run selection (Table 1). */

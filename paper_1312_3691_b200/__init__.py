@@ -31,7 +31,8 @@ class TpmcError(RuntimeError):
 
 class tpmc_mesh_info_t(C.Structure):
     _fields_ = [("centre", C.c_double * 3), ("bounding_radius", C.c_double), ("aabb_lo", C.c_float * 3),
-                ("aabb_hi", C.c_float * 3), ("nt", C.c_int64), ("n_nodes", C.c_int64), ("build_ms", C.c_double)]
+                ("aabb_hi", C.c_float * 3), ("nt", C.c_int64), ("n_nodes", C.c_int64), ("build_ms", C.c_double),
+                ("horizon_ms", C.c_double)]
 
 
 class tpmc_params(C.Structure):
@@ -188,7 +189,7 @@ class Mesh:
         _check(lib().tpmc_mesh_info(self._h, C.byref(out)), "tpmc_mesh_info")
         return {"centre": np.array(list(out.centre)), "bounding_radius": out.bounding_radius,
                 "aabb_lo": np.array(list(out.aabb_lo)), "aabb_hi": np.array(list(out.aabb_hi)),
-                "nt": int(out.nt), "n_nodes": int(out.n_nodes), "build_ms": out.build_ms}
+                "nt": int(out.nt), "n_nodes": int(out.n_nodes), "build_ms": out.build_ms, "horizon_ms": out.horizon_ms}
 
     def copy_bvh(self):
         n_nodes = self.info()["n_nodes"]

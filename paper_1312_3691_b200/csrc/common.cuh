@@ -57,6 +57,8 @@ struct tpmc_mesh {
   float4* tris;
   uint4* cnodes;                   // compact copy of `nodes` for the wavefront traversal: 2 uint4 = 32 B per node
   float q_origin[3], q_scale[3];   // its quantisation grid: x = q_origin + q * q_scale, q in [0, 65535]
+  uint4* horizon;                  // [nt] by sorted slot: escape horizon of each facet, 16 azimuth sectors x 1 byte (k_horizon, lbvh.cu)
+  double horizon_ms;
   float4* cull;                    // top of the hierarchy (<= kCullNodes nodes, breadth-first), for the seed-time cull
   int n_cull;
   double centre[3];

@@ -237,6 +237,170 @@ __global__ void k_build_cull(const float4* __restrict__ nodes, float4* __restric
   *out_count = tail;
 }
 
+// ---- escape horizon of every one-sided facet (a0, read by the reflect step) ------------------------------
+// A particle re-emitted from facet f leaves a point p of f with a direction d above f's plane.  In the facet
+// frame (e1 = first edge, e2 = n x e1, n = unit normal) let sin E = d.n / |d| be its elevation and
+// phi = atan2(d.e2, d.e1) its azimuth.  horizon[slot][k], k = 0..15, is an upper bound of sin E over every ray
+// from f with azimuth in sector k (22.5 deg each) that can hit the front of another facet: a ray above it
+// escapes (O10 finds no hit) and its traversal is skipped.  Stored as a byte b, bound = b / 254; 255 = never
+// skip.  Bounds used, all conservative, per other facet g or box B of the hierarchy:
+//   * orientation (facets): a front-face hit needs d.n_g < 0.  With gamma = angle(n, n_g) <= 90 deg,
+//     d.n_g >= |d| sin(E - gamma), so E >= gamma rules g out whatever the origin: sin E <= sin gamma.
+//     (Two-sided or degenerate g: no bound from this argument.)
+//   * position: a hit at x = p + tau d has sin E = n.(x - p) / |x - p|.  With c, rho the centre and radius
+//     of f's bounding sphere, for x in B:  n.(x - p) <= h(B) = max_B n.(x - a0) + delta  and
+//     |x - p| >= dist(c, B) - rho - delta,  delta covering the fp32 rounding of the ray origin (O13).
+//     h(B) <= 0: B lies below f's plane and cannot be reached.
+//   * azimuth: x - p lies in the ball of radius R = r_B + rho + delta about w = centre(B) - c, so d is within
+//     alpha = asin(R / |w|) of w; if that cone does not contain the pole its azimuths lie within
+//     asin(sin alpha / sin theta) of w's, theta = angle(w, n).  Otherwise, or when |w| <= R, all sectors.
+// The hierarchy is walked nearest child first; a subtree is skipped when its position bound is not above the
+// current value of any sector it can touch.  At a leaf the bound is the smaller of position and orientation.
+constexpr int kHorizonStack = 96;
+constexpr double kHorizonAzMargin = 2e-3;   // rad, covers the fp32 azimuth of the reflect step
+
+struct HorizonFacet {
+  double n[3], e1[3], e2[3], a0[3], c[3], rho, delta;
+};
+
+// position bound of a box, its distance from c, and the mask of azimuth sectors it can touch
+__device__ __forceinline__ double horizon_box(const HorizonFacet& f, const float lo[3], const float hi[3], double& dist,
+                                              unsigned int& mask) {
+  double h = f.delta, d2 = 0.0, w[3], r2 = 0.0;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    h += fmax(f.n[k] * ((double)lo[k] - f.a0[k]), f.n[k] * ((double)hi[k] - f.a0[k]));
+    const double e = fmax(fmax((double)lo[k] - f.c[k], f.c[k] - (double)hi[k]), 0.0);
+    d2 += e * e;
+    w[k] = 0.5 * ((double)lo[k] + (double)hi[k]) - f.c[k];
+    const double hw = 0.5 * ((double)hi[k] - (double)lo[k]);
+    r2 += hw * hw;
+  }
+  dist = sqrt(d2);
+  mask = 0xFFFFu;
+  if (!(h > 0.0)) return -1.0;                      // below the plane; empty boxes (lo > hi) end here as well
+  const double den = dist * (1.0 - 1e-12) - f.rho - f.delta;
+  const double R = (sqrt(r2) + f.rho + f.delta) * (1.0 + 1e-9);
+  const double L = sqrt(w[0] * w[0] + w[1] * w[1] + w[2] * w[2]);
+  if (L > R) {
+    const double x = w[0] * f.e1[0] + w[1] * f.e1[1] + w[2] * f.e1[2], y = w[0] * f.e2[0] + w[1] * f.e2[1] + w[2] * f.e2[2];
+    const double st = sqrt(x * x + y * y) / L, sa = R / L;
+    if (sa < st * (1.0 - 1e-9)) {
+      const double dphi = asin(sa / st) + kHorizonAzMargin, phi = atan2(y, x);
+      if (dphi < 3.0) {
+        const double q = 16.0 / 6.283185307179586476925;
+        const int k0 = (int)floor((phi - dphi + 3.14159265358979323846) * q), k1 = (int)floor((phi + dphi + 3.14159265358979323846) * q);
+        unsigned int m = 0u;
+        for (int k = k0; k <= k1; ++k) m |= 1u << ((k + 16) & 15);
+        mask = m;
+      }
+    }
+  }
+  return den > 0.0 ? h / den : INFINITY;
+}
+
+// 16 sector bounds packed as bytes in four words
+__device__ __forceinline__ unsigned int nibble_bytes(unsigned int nib) { return (((nib & 15u) * 0x00204081u) & 0x01010101u) * 0xFFu; }
+__device__ __forceinline__ unsigned int horizon_min(const unsigned int cur[4], unsigned int mask) {
+  unsigned int m = 0xFFFFFFFFu;
+#pragma unroll
+  for (int j = 0; j < 4; ++j) m = __vminu4(m, cur[j] | ~nibble_bytes(mask >> (4 * j)));
+  m = min(min(m & 0xFFu, (m >> 8) & 0xFFu), min((m >> 16) & 0xFFu, m >> 24));
+  return m;
+}
+__device__ __forceinline__ unsigned int horizon_quant(double b) {   // byte >= 254 b (with the safety factor), 255 = never skip
+  const double s = b * (1.0 + 1e-4) + 1e-4;
+  return s < 1.0 ? (unsigned int)ceil(s * 254.0) : 255u;
+}
+
+__global__ void __launch_bounds__(128) k_horizon(const float4* __restrict__ nodes, const float4* __restrict__ tris,
+                                                 int64_t nt, uint4* __restrict__ horizon) {
+  const int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (s >= nt) return;
+  const float4 q0 = tris[3 * s], q1 = tris[3 * s + 1], q2 = tris[3 * s + 2];
+  unsigned int cur[4] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
+  const bool two_sided = (__float_as_uint(q1.w) & TPMC_FACET_TWO_SIDED) != 0u;
+  HorizonFacet f;
+  const double a1[3] = {q1.x, q1.y, q1.z}, a2[3] = {q2.x, q2.y, q2.z};
+  f.a0[0] = q0.x; f.a0[1] = q0.y; f.a0[2] = q0.z;
+  double e2v[3];
+  for (int k = 0; k < 3; ++k) { f.e1[k] = a1[k] - f.a0[k]; e2v[k] = a2[k] - f.a0[k]; f.c[k] = (f.a0[k] + a1[k] + a2[k]) / 3.0; }
+  f.n[0] = f.e1[1] * e2v[2] - f.e1[2] * e2v[1];
+  f.n[1] = f.e1[2] * e2v[0] - f.e1[0] * e2v[2];
+  f.n[2] = f.e1[0] * e2v[1] - f.e1[1] * e2v[0];
+  const double nl = sqrt(f.n[0] * f.n[0] + f.n[1] * f.n[1] + f.n[2] * f.n[2]);
+  const double el = sqrt(f.e1[0] * f.e1[0] + f.e1[1] * f.e1[1] + f.e1[2] * f.e1[2]);
+  if (!two_sided && nl > 0.0 && el > 0.0 && nt > 1) {
+    double amax = 0.0;
+    f.rho = 0.0;
+    for (int k = 0; k < 3; ++k) {
+      f.n[k] /= nl;
+      f.e1[k] /= el;
+      amax = fmax(amax, fmax(fabs(f.a0[k]), fmax(fabs(a1[k]), fabs(a2[k]))));
+    }
+    f.e2[0] = f.n[1] * f.e1[2] - f.n[2] * f.e1[1];
+    f.e2[1] = f.n[2] * f.e1[0] - f.n[0] * f.e1[2];
+    f.e2[2] = f.n[0] * f.e1[1] - f.n[1] * f.e1[0];
+    for (int j = 0; j < 3; ++j) {
+      const double* a = j == 0 ? f.a0 : (j == 1 ? a1 : a2);
+      f.rho = fmax(f.rho, sqrt((a[0] - f.c[0]) * (a[0] - f.c[0]) + (a[1] - f.c[1]) * (a[1] - f.c[1]) + (a[2] - f.c[2]) * (a[2] - f.c[2])));
+    }
+    f.rho *= 1.0 + 1e-12;
+    f.delta = 4e-7 * amax + 1e-30;   // > sqrt(3) * 2^-24 * |coordinate|: rounding of the hit point to fp32
+    cur[0] = cur[1] = cur[2] = cur[3] = 0u;
+    int stack[kHorizonStack];
+    int sp = 0, node = 0;
+    bool give_up = false;
+    for (;;) {
+      const float4 n0 = __ldg(nodes + 4 * (size_t)node), n1 = __ldg(nodes + 4 * (size_t)node + 1),
+                   n2 = __ldg(nodes + 4 * (size_t)node + 2), n3 = __ldg(nodes + 4 * (size_t)node + 3);
+      const float lo[2][3] = {{n0.x, n0.y, n0.z}, {n1.z, n1.w, n2.x}};
+      const float hi[2][3] = {{n0.w, n1.x, n1.y}, {n2.y, n2.z, n2.w}};
+      const int ref[2] = {__float_as_int(n3.x), __float_as_int(n3.y)};
+      double dist[2];
+      bool go[2];
+      for (int ch = 0; ch < 2; ++ch) {
+        unsigned int mask;
+        const double bnd = horizon_box(f, lo[ch], hi[ch], dist[ch], mask);
+        go[ch] = bnd > 0.0 && horizon_quant(bnd) > horizon_min(cur, mask);
+        if (go[ch] && ref[ch] < 0) {        // leaf: the facet in it
+          go[ch] = false;
+          const int64_t g = ~ref[ch];
+          if (g == s) continue;
+          const float4 g0 = __ldg(tris + 3 * g), g1 = __ldg(tris + 3 * g + 1), g2 = __ldg(tris + 3 * g + 2);
+          double b = bnd;
+          if ((__float_as_uint(g1.w) & TPMC_FACET_TWO_SIDED) == 0u) {
+            const double f1[3] = {(double)g1.x - g0.x, (double)g1.y - g0.y, (double)g1.z - g0.z};
+            const double f2[3] = {(double)g2.x - g0.x, (double)g2.y - g0.y, (double)g2.z - g0.z};
+            const double m[3] = {f1[1] * f2[2] - f1[2] * f2[1], f1[2] * f2[0] - f1[0] * f2[2], f1[0] * f2[1] - f1[1] * f2[0]};
+            const double ml = sqrt(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
+            if (ml > 0.0) {
+              const double cg = (f.n[0] * m[0] + f.n[1] * m[1] + f.n[2] * m[2]) / ml;
+              if (cg > 0.0) b = fmin(b, sqrt(fmax(1.0 - cg * cg, 0.0)) + 1e-9);
+            }
+          }
+          const unsigned int qb = horizon_quant(b) * 0x01010101u;
+#pragma unroll
+          for (int j = 0; j < 4; ++j) cur[j] = __vmaxu4(cur[j], qb & nibble_bytes(mask >> (4 * j)));
+        }
+      }
+      if (go[0] && go[1]) {
+        const bool sw = dist[1] < dist[0];
+        if (sp >= kHorizonStack) { give_up = true; break; }
+        stack[sp++] = sw ? ref[0] : ref[1];
+        node = sw ? ref[1] : ref[0];
+      } else if (go[0] || go[1]) {
+        node = go[0] ? ref[0] : ref[1];
+      } else {
+        if (sp == 0) break;
+        node = stack[--sp];
+      }
+    }
+    if (give_up) cur[0] = cur[1] = cur[2] = cur[3] = 0xFFFFFFFFu;
+  }
+  horizon[s] = make_uint4(cur[0], cur[1], cur[2], cur[3]);
+}
+
 struct DevBuf {  // frees on scope exit
   void* p = nullptr;
   ~DevBuf() { if (p) cudaFree(p); }
@@ -372,10 +536,21 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
   MESH_TRY(cudaMemcpyAsync(&m->n_cull, cq.as<int>() + kCullNodes, sizeof(int), cudaMemcpyDeviceToHost, st));
   MESH_TRY(cudaGetLastError());
   MESH_TRY(cudaEventRecord(e1, st));
-  MESH_TRY(cudaStreamSynchronize(st));
-  float ms = 0.0f;
-  MESH_TRY(cudaEventElapsedTime(&ms, e0, e1));
-  m->build_ms = ms;
+  // escape horizons (timed apart from the hierarchy build)
+  MESH_TRY(cudaMalloc((void**)&m->horizon, sizeof(uint4) * nt));
+  cudaEvent_t e2;
+  MESH_TRY(cudaEventCreate(&e2));
+  k_horizon<<<(unsigned)((nt + 127) / 128), 128, 0, st>>>(m->nodes, m->tris, nt, m->horizon);
+  cudaEventRecord(e2, st);
+  {
+    const cudaError_t es = cudaStreamSynchronize(st);
+    float ms = 0.0f, ms2 = 0.0f;
+    if (es == cudaSuccess) { cudaEventElapsedTime(&ms, e0, e1); cudaEventElapsedTime(&ms2, e1, e2); }
+    cudaEventDestroy(e2);
+    MESH_TRY(es);
+    m->build_ms = ms;
+    m->horizon_ms = ms2;
+  }
 #undef MESH_TRY
   *out = m;
   return TPMC_OK;
@@ -383,7 +558,7 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
 
 extern "C" void tpmc_mesh_destroy(tpmc_mesh* m) {
   if (!m) return;
-  cudaFree(m->nodes); cudaFree(m->tris); cudaFree(m->cull); cudaFree(m->cnodes);
+  cudaFree(m->nodes); cudaFree(m->tris); cudaFree(m->cull); cudaFree(m->cnodes); cudaFree(m->horizon);
   for (int pi = 0; pi < kPipes; ++pi) {
     Pipe& pp = m->pipe[pi];
     for (int k = 0; k < 2; ++k) { cudaFree(pp.q_o[k]); cudaFree(pp.q_v[k]); cudaFree(pp.q_f[k]); }
@@ -421,6 +596,7 @@ extern "C" int tpmc_mesh_info(const tpmc_mesh* m, tpmc_mesh_info_t* out) {
   out->nt = m->nt;
   out->n_nodes = m->n_nodes;
   out->build_ms = m->build_ms;
+  out->horizon_ms = m->horizon_ms;
   return TPMC_OK;
 }
 

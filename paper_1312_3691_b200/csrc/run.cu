@@ -315,12 +315,13 @@ struct Particle {
 
 __device__ __forceinline__ bool interact(const RunConst& rc, const float4* __restrict__ tris, Particle& p, const Hit& hit,
                                          double* __restrict__ P, double tq[3], const tpmc_debug& dbg,
-                                         unsigned long long& trunc) {
+                                         unsigned long long& trunc, const uint4* __restrict__ horizon = nullptr) {
   const float4 q0 = __ldg(tris + 3 * (size_t)hit.slot), q1 = __ldg(tris + 3 * (size_t)hit.slot + 1),
                q2 = __ldg(tris + 3 * (size_t)hit.slot + 2);
   const double w = rc.sp[p.species].w, cW = rc.sp[p.species].cW;
   double vout[3];
-  reflect(q0, q1, q2, p.v, rc.sigma, cW, particle_block(rc, rc.first + p.j, 2u + p.k), vout);
+  float sin_e, phi;
+  reflect(q0, q1, q2, p.v, rc.sigma, cW, particle_block(rc, rc.first + p.j, 2u + p.k), vout, sin_e, phi);
   // O12: dp = w (v_in - v_out) on the fp32 values; hit point o + tau v in fp64
   double hp[3], dp[3];
   float vo[3];
@@ -344,6 +345,12 @@ __device__ __forceinline__ bool interact(const RunConst& rc, const float4* __res
   p.f_prev = hit.facet;
   ++p.k;
   if (p.k >= rc.max_bounces) { ++trunc; return false; }
+  // escape horizon of the facet (k_horizon, lbvh.cu): above it the next segment cannot hit anything
+  if (horizon) {
+    const int sector = min(max((int)floorf((phi + 3.14159265f) * 2.54647909f), 0), 15);   // 16 / (2 pi)
+    const unsigned int b = __ldg((const unsigned char*)horizon + 16 * (size_t)hit.slot + sector);
+    if (b < 255u && sin_e > (float)b * (1.0f / 254.0f)) return false;
+  }
   return true;
 }
 
@@ -360,7 +367,8 @@ __global__ void __launch_bounds__(kTraceBlock) k_reflect(const RunConst rc, unsi
                                                          unsigned int* __restrict__ n_out,
                                                          unsigned int* __restrict__ ovf, unsigned int* __restrict__ n_ovf,
                                                          double* __restrict__ P, double* __restrict__ torque,
-                                                         unsigned long long* __restrict__ stats, tpmc_debug dbg) {
+                                                         unsigned long long* __restrict__ stats, tpmc_debug dbg,
+                                                         const uint4* __restrict__ horizon) {
   __shared__ double sred[3][8];
   __shared__ unsigned long long scnt[4][8];
   const unsigned int n = *n_hits;
@@ -395,25 +403,28 @@ __global__ void __launch_bounds__(kTraceBlock) k_reflect(const RunConst rc, unsi
         is_hit = hit.facet >= 0;
       }
     }
-    // reserve the successor's queue slot first: a particle that finds the region full is spilled untouched
-    const unsigned em = __ballot_sync(FULL, is_hit);
+    // surface interaction, then a queue slot for every particle that goes on (warp-aggregated).  A particle
+    // that finds region A of the next queue full writes its new state back into its own slot of this queue
+    // and goes to the overflow list, like one the traversal gave up on.
+    bool go_on = false;
+    if (is_hit) {
+      ++hits;
+      go_on = interact(rc, tris, p, hit, P, tq, dbg, trunc, horizon);
+    }
+    const unsigned em = __ballot_sync(FULL, go_on);
     if (em) {
       const int leader = __ffs(em) - 1;
       unsigned base = 0;
       if (lane == leader) base = atomicAdd(n_out, (unsigned)__popc(em));
       base = __shfl_sync(FULL, base, leader);
-      if (is_hit) {
+      if (go_on) {
         const unsigned s = base + __popc(em & lanemask_lt());
-        if (s >= cap) {
-          spill = true;
-        } else {
-          ++hits;
-          const bool go_on = interact(rc, tris, p, hit, P, tq, dbg, trunc);
-          // a particle stopped by the bounce cap leaves a hole: a NaN origin fails every box test
-          qout.o[s] = make_float4(go_on ? p.o[0] : __int_as_float(0x7FC00000), p.o[1], p.o[2], __uint_as_float((unsigned int)p.j));
-          qout.v[s] = make_float4(p.v[0], p.v[1], p.v[2], __uint_as_float((unsigned int)p.species | (p.k << 4)));
-          qout.f[s] = p.f_prev;
-        }
+        const RayQueue& qd = (s >= cap) ? qin : qout;
+        const unsigned sd = (s >= cap) ? r : s;
+        spill = s >= cap;
+        qd.o[sd] = make_float4(p.o[0], p.o[1], p.o[2], __uint_as_float((unsigned int)p.j));
+        qd.v[sd] = make_float4(p.v[0], p.v[1], p.v[2], __uint_as_float((unsigned int)p.species | (p.k << 4)));
+        qd.f[sd] = p.f_prev;
       }
     }
     const unsigned sm = __ballot_sync(FULL, spill);
@@ -438,7 +449,8 @@ __global__ void __launch_bounds__(kTraceBlock) k_finish(const RunConst rc, unsig
                                                         const unsigned int* __restrict__ list,
                                                         const unsigned int* __restrict__ n_rays,
                                                         double* __restrict__ P, double* __restrict__ torque,
-                                                        unsigned long long* __restrict__ stats, tpmc_debug dbg) {
+                                                        unsigned long long* __restrict__ stats, tpmc_debug dbg,
+                                                        const uint4* __restrict__ horizon) {
   __shared__ int sstack[TPMC_STACK_SMEM * kTraceBlock];
   __shared__ double sred[3][8];
   __shared__ unsigned long long scnt[4][8];
@@ -462,7 +474,7 @@ __global__ void __launch_bounds__(kTraceBlock) k_finish(const RunConst rc, unsig
       const Hit hit = closest_hit(nodes, tris, p.o, p.v, p.f_prev, sstack + threadIdx.x, kTraceBlock, cnt);
       if (hit.facet < 0) break;
       ++hits;
-      if (!interact(rc, tris, p, hit, P, tq, dbg, trunc)) break;
+      if (!interact(rc, tris, p, hit, P, tq, dbg, trunc, horizon)) break;
     }
   }
   unsigned long long c4[4] = {hits, trunc, (unsigned long long)cnt.tris, (unsigned long long)cnt.nodes};
@@ -829,6 +841,8 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
   const bool timed = (h_stats != nullptr);   // per-kernel events only when the caller will read them
   const char* pc_env = getenv("TPMC_PRECULL");   // read per call: the parity tests switch the pass off and on
   const bool precull = !(pc_env && pc_env[0] == '0');
+  const char* hz_env = getenv("TPMC_HORIZON");   // likewise: "0" switches the escape-horizon test off
+  const bool use_horizon = !(hz_env && hz_env[0] == '0');
   static const int seed_walk = (getenv("TPMC_SEED_WALK") && getenv("TPMC_SEED_WALK")[0] == '0') ? 0 : 1;   // tuning aid
   SeedConstF sf;
   make_seed_const_f(m, rc, &sf);
@@ -920,14 +934,15 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
       // the straggler kernel of the previous iteration reads the queue this reflect step writes
       if (li >= 1) TPMC_CUDA_TRY(cudaStreamWaitEvent(s1, pp.ev_ovf[b ^ 1], 0));
       k_reflect<<<g.reflect, kTraceBlock, 0, s1>>>(rcc, cap, m->tris, Q[p], pp.hit_ray, pp.hit_cand, pp.ctr + 5, Q[p ^ 1],
-                                                   pp.ctr + 2 * (p ^ 1), ovf, pp.ctr + 8 + b, P, m->totals, m->stats, dbg);
+                                                   pp.ctr + 2 * (p ^ 1), ovf, pp.ctr + 8 + b, P, m->totals, m->stats, dbg,
+                                                   use_horizon ? m->horizon : nullptr);
       if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[4], s1));
       // overflow list of this iteration: followed to escape on the side stream, beside the next traversal
       TPMC_CUDA_TRY(cudaEventRecord(pp.ev_refl[b], s1));
       TPMC_CUDA_TRY(cudaStreamWaitEvent(s3, pp.ev_refl[b], 0));
       if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[5], s3));
       k_finish<<<g.finish / 4, kTraceBlock, 0, s3>>>(rcc, cap, m->nodes, m->tris, Q[p], ovf, pp.ctr + 8 + b, P, m->totals,
-                                                     m->stats, dbg);
+                                                     m->stats, dbg, use_horizon ? m->horizon : nullptr);
       if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[6], s3));
       TPMC_CUDA_TRY(cudaEventRecord(pp.ev_ovf[b], s3));
       pp.last_iter = li;
@@ -944,7 +959,7 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
       TPMC_CUDA_TRY(cudaStreamWaitEvent(pp.main, pp.ev_ovf[1], 0));
       if (timed) TPMC_CUDA_TRY(cudaEventRecord(pp.ev_f0, pp.main));
       k_finish<<<g.finish, kTraceBlock, 0, pp.main>>>(rcc, cap, m->nodes, m->tris, q, nullptr, pp.ctr + 2 * p, P, m->totals,
-                                                     m->stats, dbg);
+                                                     m->stats, dbg, use_horizon ? m->horizon : nullptr);
       if (timed) TPMC_CUDA_TRY(cudaEventRecord(pp.ev_f1, pp.main));
       ++launches;
       if (pi > 0) {

@@ -482,8 +482,11 @@ __device__ __forceinline__ Hit resolve_candidates(const float4* __restrict__ tri
 
 // ---- O11: surface interaction (P:73 diffuse re-emission at T_W; P:53 specular; Maxwell mix A7) ------
 // w: the four words of Philox block 2+k.  Returns v_out in fp64 (the caller rounds it to fp32, O9).
+// sin_e, phi: elevation (sin) above the facet plane and azimuth in the frame (e1, n_eff x e1) of fp32(v_out), for
+// the comparison with the facet's escape horizon (k_horizon, lbvh.cu); fp32 accuracy is enough (the stored
+// horizon carries a safety factor of 1e-4 and an azimuth margin of 2e-3 rad).
 __device__ __forceinline__ void reflect(const float4 q0, const float4 q1, const float4 q2, const float vf[3],
-                                        double sigma, double cW, const uint4 w, double vout[3]) {
+                                        double sigma, double cW, const uint4 w, double vout[3], float& sin_e, float& phi) {
   const double p0[3] = {(double)q0.x, (double)q0.y, (double)q0.z};
   double e1[3], e2[3], Ng[3];
 #pragma unroll
@@ -496,11 +499,11 @@ __device__ __forceinline__ void reflect(const float4 q0, const float4 q1, const 
   double ne[3] = {Ng[0] / nl, Ng[1] / nl, Ng[2] / nl};
   const double vn = (v[0] * ne[0] + v[1] * ne[1]) + v[2] * ne[2];
   if (!(vn < 0.0)) { ne[0] = -ne[0]; ne[1] = -ne[1]; ne[2] = -ne[2]; }   // n_eff faces the incoming particle
+  const double el = sqrt((e1[0] * e1[0] + e1[1] * e1[1]) + e1[2] * e1[2]);
+  const double t1[3] = {e1[0] / el, e1[1] / el, e1[2] / el};
+  const double t2[3] = {ne[1] * t1[2] - ne[2] * t1[1], ne[2] * t1[0] - ne[0] * t1[2], ne[0] * t1[1] - ne[1] * t1[0]};
   if (u01(w.x) < sigma) {
     // diffuse, fully accommodated: flux-weighted half-Maxwellian at T_W (A6); tangent basis A17
-    const double el = sqrt((e1[0] * e1[0] + e1[1] * e1[1]) + e1[2] * e1[2]);
-    const double t1[3] = {e1[0] / el, e1[1] / el, e1[2] / el};
-    const double t2[3] = {ne[1] * t1[2] - ne[2] * t1[1], ne[2] * t1[0] - ne[0] * t1[2], ne[0] * t1[1] - ne[1] * t1[0]};
     const double an = sqrt(-log(u01(w.y)));
     const double at = sqrt(-log(u01(w.z)));
     double sa, ca;
@@ -512,6 +515,12 @@ __device__ __forceinline__ void reflect(const float4 q0, const float4 q1, const 
 #pragma unroll
     for (int k = 0; k < 3; ++k) vout[k] = v[k] - 2.0 * vne * ne[k];
   }
+  const float r[3] = {(float)vout[0], (float)vout[1], (float)vout[2]};
+  const float rn = r[0] * (float)ne[0] + r[1] * (float)ne[1] + r[2] * (float)ne[2];
+  const float r1 = r[0] * (float)t1[0] + r[1] * (float)t1[1] + r[2] * (float)t1[2];
+  const float r2 = r[0] * (float)t2[0] + r[1] * (float)t2[1] + r[2] * (float)t2[2];
+  sin_e = rn * rsqrtf(r[0] * r[0] + r[1] * r[1] + r[2] * r[2]);   // NaN for a zero velocity: never above a horizon
+  phi = atan2f(r2, r1);
 }
 
 __device__ __forceinline__ unsigned long long fnv1a_facet(unsigned long long h, int facet) {

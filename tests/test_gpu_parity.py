@@ -368,3 +368,31 @@ def test_precull_pass_changes_nothing(T, name, idx, count, monkeypatch):
     assert np.linalg.norm(Fa - Fb) <= 1e-12 * np.linalg.norm(Fb)
     assert a.stats["culled"] >= b.stats["culled"]     # the grown bounding sphere also drops rays the boxes keep
     gm.close()
+
+
+# ------------------------------------------------------------------ a4: the escape-horizon test skips only escapes
+@pytest.mark.parametrize("name,idx,count", [("C1", 0, 100_000), ("C2", 1, 3_000_000), ("C3", 1, 3_000_000),
+                                             ("C4", 0, 3_000_000), ("C4", 9, 3_000_000), ("C5", 3, 20_000_000),
+                                             ("C5", 40, 20_000_000)])
+def test_escape_horizon_changes_nothing(T, name, idx, count, monkeypatch):
+    """A re-emitted ray above its facet's escape horizon (k_horizon, lbvh.cu) is not traced: with the test
+    switched off (TPMC_HORIZON=0, every reflected ray traced) hits, hashes, bounce counts and forces are identical,
+    and with it on fewer rays reach the traversal."""
+    cfg = ti.config(name)[idx]
+    m = cfg.mesh()
+    gm = T.Mesh(m.vertices, m.indices, m.flags)
+    first = min(cfg.N - count, 1_234_567)
+    monkeypatch.setenv("TPMC_HORIZON", "1")
+    a = gm.run(cfg, first=first, count=count, debug=True)
+    monkeypatch.setenv("TPMC_HORIZON", "0")
+    b = gm.run(cfg, first=first, count=count, debug=True)
+    assert a.stats["hits"] == b.stats["hits"] and a.stats["hits"] > 0
+    assert bool((a.hash == b.hash).all()) and bool((a.bounces == b.bounces).all())
+    Fa, Fb = a.force.cpu().numpy(), b.force.cpu().numpy()
+    assert np.linalg.norm(Fa - Fb) <= 1e-12 * np.linalg.norm(Fb)
+    assert a.stats["traced_rays"] <= b.stats["traced_rays"]
+    if name in ("C2", "C5"):                           # smooth bodies: most re-emitted rays are above the horizon
+        assert a.stats["traced_rays"] < b.stats["traced_rays"] - a.stats["hits"] // 4
+    elif name != "C1":                                 # C1 is two-sided (no horizon); facets at sharp edges have none either
+        assert a.stats["traced_rays"] < b.stats["traced_rays"]
+    gm.close()
