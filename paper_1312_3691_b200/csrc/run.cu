@@ -84,11 +84,13 @@ __global__ void __launch_bounds__(kPrecullBlock) k_seed_precull(const SeedConstF
   __syncthreads();
   if (keep_c) {
     const unsigned slot = s_base[0] + s_cnt[0][wid] + __popc(mcert & lanemask_lt());
-    surv[slot] = j;
-    surv[cap + slot] = __float_as_uint(root[0]);
-    surv[2 * cap + slot] = __float_as_uint(root[1]);
+    // streaming stores and loads (evict-first) for every list and queue of the path: the hierarchy and the
+    // facets (83 MB at C5) should stay in L2 while ~600 MB of lists and queues pass through it every wave
+    __stcs(surv + slot, j);
+    __stcs(surv + cap + slot, __float_as_uint(root[0]));
+    __stcs(surv + 2 * cap + slot, __float_as_uint(root[1]));
   }
-  if (keep_u) surv[cap - 1u - (s_base[1] + s_cnt[1][wid] + __popc(munc & lanemask_lt()))] = j;
+  if (keep_u) __stcs(surv + (cap - 1u - (s_base[1] + s_cnt[1][wid] + __popc(munc & lanemask_lt()))), j);
 }
 
 // a2: seed particles of one wave in fp64, round the state to fp32 (O9), drop the rays that cannot touch the
@@ -112,13 +114,13 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
   const bool active = kk < n;
   const bool hinted = kk < n1;
   const unsigned int sl = hinted ? kk : cap_s - 1u - (kk - n1);
-  const unsigned int j = active ? (surv ? surv[sl] : kk) : 0u;
+  const unsigned int j = active ? (surv ? __ldcs(surv + sl) : kk) : 0u;
   bool keep = false;
   float o[3] = {0, 0, 0}, v[3] = {1, 1, 1};
   int species = 0;
   if (active) {
     float hint[2] = {0.0f, 0.0f};
-    if (hinted) { hint[0] = __uint_as_float(surv[cap_s + sl]); hint[1] = __uint_as_float(surv[2 * cap_s + sl]); }
+    if (hinted) { hint[0] = __uint_as_float(__ldcs(surv + cap_s + sl)); hint[1] = __uint_as_float(__ldcs(surv + 2 * cap_s + sl)); }
     const SeedState s = seed_particle(rc, rc.first + wave_first + j, hinted ? hint : nullptr);
     species = s.species;
 #pragma unroll
@@ -140,9 +142,9 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
   base = __shfl_sync(0xFFFFFFFFu, base, 0);
   if (keep) {
     const unsigned slot = region_b + base + __popc(m & lanemask_lt());
-    q.o[slot] = make_float4(o[0], o[1], o[2], __uint_as_float(wave_first + j));
-    q.v[slot] = make_float4(v[0], v[1], v[2], __uint_as_float((unsigned int)species));   // bounce 0
-    q.f[slot] = -1;
+    __stcs(q.o + slot, make_float4(o[0], o[1], o[2], __uint_as_float(wave_first + j)));
+    __stcs(q.v + slot, make_float4(v[0], v[1], v[2], __uint_as_float((unsigned int)species)));   // bounce 0
+    __stcs(q.f + slot, -1);
   }
   }
 }
@@ -212,7 +214,7 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
           r = pool_next + rank;
           if (r < n) {
             r = (r < na) ? r : cap + (r - na);   // physical slot
-            walk_init(w, grid, q.o[r], q.v[r], q.f[r]);
+            walk_init(w, grid, __ldcs(q.o + r), __ldcs(q.v + r), __ldcs(q.f + r));
             has = true;
           }
         }
@@ -249,9 +251,9 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
       base = __shfl_sync(FULL, base, leader);
       if (fin) {
         const unsigned h = base + __popc(fm & lanemask_lt());
-        hit_ray[h] = r;
-        hit_cand[h] = (w.nc > TPMC_MAX_CAND) ? make_int4(-1, -1, -1, TPMC_CAND_OVERFLOW)
-                                             : make_int4(w.cs[0], w.cs[1], w.cs[2], w.cs[3]);
+        __stcs(hit_ray + h, r);
+        __stcs(hit_cand + h, (w.nc > TPMC_MAX_CAND) ? make_int4(-1, -1, -1, TPMC_CAND_OVERFLOW)
+                                                    : make_int4(w.cs[0], w.cs[1], w.cs[2], w.cs[3]));
         fin = false;
       }
     }
@@ -386,19 +388,19 @@ __global__ void __launch_bounds__(kTraceBlock) k_reflect(const RunConst rc, unsi
     Hit hit;
     hit.facet = -1;
     if (h < n) {
-      r = hit_ray[h];
-      const int4 cand = hit_cand[h];
+      r = __ldcs(hit_ray + h);
+      const int4 cand = __ldcs(hit_cand + h);
       if (cand.w == TPMC_CAND_OVERFLOW) {
         spill = true;
       } else {
-        const float4 ro = qin.o[r], rv = qin.v[r];
+        const float4 ro = __ldcs(qin.o + r), rv = __ldcs(qin.v + r);
         p.o[0] = ro.x; p.o[1] = ro.y; p.o[2] = ro.z;
         p.v[0] = rv.x; p.v[1] = rv.y; p.v[2] = rv.z;
         p.j = __float_as_uint(ro.w);
         const unsigned int pk = __float_as_uint(rv.w);
         p.species = (int)(pk & 15u);
         p.k = pk >> 4;
-        p.f_prev = qin.f[r];
+        p.f_prev = __ldcs(qin.f + r);
         hit = resolve_candidates(tris, cand, p.o, p.v, ntests);
         is_hit = hit.facet >= 0;
       }
@@ -422,9 +424,9 @@ __global__ void __launch_bounds__(kTraceBlock) k_reflect(const RunConst rc, unsi
         const RayQueue& qd = (s >= cap) ? qin : qout;
         const unsigned sd = (s >= cap) ? r : s;
         spill = s >= cap;
-        qd.o[sd] = make_float4(p.o[0], p.o[1], p.o[2], __uint_as_float((unsigned int)p.j));
-        qd.v[sd] = make_float4(p.v[0], p.v[1], p.v[2], __uint_as_float((unsigned int)p.species | (p.k << 4)));
-        qd.f[sd] = p.f_prev;
+        __stcs(qd.o + sd, make_float4(p.o[0], p.o[1], p.o[2], __uint_as_float((unsigned int)p.j)));
+        __stcs(qd.v + sd, make_float4(p.v[0], p.v[1], p.v[2], __uint_as_float((unsigned int)p.species | (p.k << 4))));
+        __stcs(qd.f + sd, p.f_prev);
       }
     }
     const unsigned sm = __ballot_sync(FULL, spill);
@@ -682,7 +684,7 @@ size_t wave_size() {
   if (!w) {
     const char* e = getenv("TPMC_WAVE");
     long long v = e ? atoll(e) : 0;
-    w = (v >= 1024 && v <= (1ll << 28)) ? (size_t)v : ((size_t)1 << 24);
+    w = (v >= 1024 && v <= (1ll << 28)) ? (size_t)v : ((size_t)1 << 26);
   }
   return w;
 }
