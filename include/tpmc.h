@@ -110,6 +110,14 @@ int tpmc_mesh_info(const tpmc_mesh* mesh, tpmc_mesh_info_t* out /* host */);
  * leaf_facet [nt] = facet id stored in each sorted triangle slot.  Either pointer may be NULL. */
 int tpmc_mesh_copy_bvh(const tpmc_mesh* mesh, float* h_nodes, int32_t* h_leaf_facet);
 
+/* Copy the escape horizons to the host for inspection: h_horizon [nt][16] bytes, indexed by sorted triangle
+ * slot (see leaf_facet above) and azimuth sector.  For a one-sided facet with unit normal n, first edge
+ * direction e1 and e2 = n x e1, a ray leaving the facet in direction d with azimuth atan2(d.e2, d.e1) in
+ * sector k = floor((azimuth + pi) * 16 / (2 pi)) and elevation sin E = d.n / |d| > byte / 254 cannot hit any
+ * facet (O10 finds no hit): the reflect step does not trace it.  255 = no such bound (two-sided facets, facets
+ * at sharp concave or convex edges).  Built on the device by tpmc_mesh_create after the LBVH. */
+int tpmc_mesh_copy_horizon(const tpmc_mesh* mesh, uint8_t* h_horizon);
+
 /* The hot path: seed particles [first, first+count) on the spherical control
  * volume from the drifting-Maxwellian number flux (eq. 10, 11, 14a-c, 15), trace each against the
  * body (closest hit), apply the surface interaction, follow reflections until

@@ -22,7 +22,7 @@ TPMC_MEM_HOST, TPMC_MEM_DEVICE = 0, 1
 TPMC_MAX_SPECIES = 8
 
 EXPORTS = ["tpmc_mesh_create", "tpmc_mesh_destroy", "tpmc_mesh_info", "tpmc_mesh_copy_bvh", "tpmc_run",
-           "tpmc_run_host", "tpmc_seed", "tpmc_trace", "tpmc_strerror", "tpmc_last_cuda_error", "tpmc_version"]
+           "tpmc_mesh_copy_horizon", "tpmc_run_host", "tpmc_seed", "tpmc_trace", "tpmc_strerror", "tpmc_last_cuda_error", "tpmc_version"]
 
 
 class TpmcError(RuntimeError):
@@ -76,6 +76,8 @@ def lib():
         L.tpmc_mesh_info.argtypes = [vp, C.POINTER(tpmc_mesh_info_t)]
         L.tpmc_mesh_copy_bvh.restype = C.c_int
         L.tpmc_mesh_copy_bvh.argtypes = [vp, vp, vp]
+        L.tpmc_mesh_copy_horizon.restype = C.c_int
+        L.tpmc_mesh_copy_horizon.argtypes = [vp, vp]
         L.tpmc_run.restype = C.c_int
         L.tpmc_run.argtypes = [vp, C.POINTER(tpmc_params), vp, vp, vp, vp, C.POINTER(tpmc_stats), C.POINTER(tpmc_debug)]
         L.tpmc_run_host.restype = C.c_int
@@ -198,6 +200,11 @@ class Mesh:
         _check(lib().tpmc_mesh_copy_bvh(self._h, nodes.ctypes.data, leaf.ctypes.data), "tpmc_mesh_copy_bvh")
         return nodes, leaf
 
+    def copy_horizon(self):
+        hz = np.zeros((self.nt, 16), dtype=np.uint8)
+        _check(lib().tpmc_mesh_copy_horizon(self._h, hz.ctypes.data), "tpmc_mesh_copy_horizon")
+        return hz
+
     # ------------------------------------------------------------------ the hot path
     def run(self, cfg, first=None, count=None, N=None, facets=True, debug=False, stats=True, stream=None) -> RunResult:
         torch = _torch()
@@ -283,6 +290,10 @@ def tpmc_mesh_info(mesh: Mesh) -> dict:
 
 def tpmc_mesh_copy_bvh(mesh: Mesh):
     return mesh.copy_bvh()
+
+
+def tpmc_mesh_copy_horizon(mesh: Mesh):
+    return mesh.copy_horizon()
 
 
 def tpmc_run(mesh: Mesh, cfg, **kw) -> RunResult:

@@ -619,6 +619,12 @@ extern "C" int tpmc_mesh_copy_bvh(const tpmc_mesh* m, float* h_nodes, int32_t* h
   return TPMC_OK;
 }
 
+extern "C" int tpmc_mesh_copy_horizon(const tpmc_mesh* m, uint8_t* h_horizon) {
+  if (!m || !h_horizon) return TPMC_EINVAL;
+  TPMC_CUDA_TRY(cudaMemcpy(h_horizon, m->horizon, sizeof(uint4) * m->nt, cudaMemcpyDeviceToHost));
+  return TPMC_OK;
+}
+
 extern "C" const char* tpmc_strerror(int code) {
   switch (code) {
     case TPMC_OK: return "ok";

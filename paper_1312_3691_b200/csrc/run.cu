@@ -801,7 +801,7 @@ int fill_stats(tpmc_mesh* m, const tpmc_params* params, tpmc_stats* h_stats) {
       h_stats->ms_trace += t;
       TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[3], ev[4]));
       h_stats->ms_reflect += t;
-      if (getenv("TPMC_TIMELINE") && w >= 20 && w < 26 && w < pp.seed_iters) {   // diagnosis: event times since the run began
+      if (getenv("TPMC_TIMELINE") && w >= 4 && w < 10 && w < pp.seed_iters) {   // diagnosis: event times since the run began
         float a[7];
         for (int k = 0; k < 7; ++k) cudaEventElapsedTime(&a[k], m->ev0, ev[k]);
         fprintf(stderr, "iter %llu: seed %.3f-%.3f trace %.3f-%.3f reflect -%.3f finish %.3f-%.3f\n", w, a[0], a[1], a[2], a[3], a[4],

@@ -396,3 +396,49 @@ def test_escape_horizon_changes_nothing(T, name, idx, count, monkeypatch):
     elif name != "C1":                                 # C1 is two-sided (no horizon); facets at sharp edges have none either
         assert a.stats["traced_rays"] < b.stats["traced_rays"]
     gm.close()
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5small"])
+def test_rays_above_the_escape_horizon_hit_nothing(T, O, name):
+    """Direct check of what the horizon promises (include/tpmc.h, tpmc_mesh_copy_horizon): a ray that leaves a
+    point of a one-sided facet above the stored bound of its azimuth sector has no hit in the ORACLE's closest-hit
+    search (brute force on the small meshes).  Also: smooth closed bodies do get bounds (the test is not vacuous)."""
+    if name == "C5small":
+        m = ti.large_body(5, 24)            # same recipe as C5, ~1.2e4 facets: displaced sphere + panels
+    else:
+        m = ti.config(name)[0].mesh()
+    gm = T.Mesh(m.vertices, m.indices, m.flags)
+    om = O.OracleMesh(m.vertices, m.indices, m.flags)
+    hz = gm.copy_horizon()
+    _, leaf = gm.copy_bvh()
+    rng = np.random.default_rng(7)
+    V = m.vertices.astype(np.float64)
+    tested = 0
+    for slot in rng.integers(0, m.nt, 1500):
+        f = int(leaf[slot])
+        a0, a1, a2 = (V[m.indices[f, k]] for k in range(3))
+        n = np.cross(a1 - a0, a2 - a0)
+        n /= np.linalg.norm(n)
+        e1 = (a1 - a0) / np.linalg.norm(a1 - a0)
+        e2 = np.cross(n, e1)
+        k = int(rng.integers(0, 16))
+        b = int(hz[slot, k])
+        if b == 255:
+            continue
+        w = rng.dirichlet([1.0, 1.0, 1.0])
+        p = (w[0] * a0 + w[1] * a1 + w[2] * a2).astype(np.float32)
+        phi = -np.pi + (k + rng.uniform(0.02, 0.98)) * (2 * np.pi / 16)
+        s_lo = b / 254.0
+        sin_e = min(s_lo + rng.uniform(1e-4, 1.0) ** 3 * (1.0 - s_lo) + 1e-5, 1.0)
+        cos_e = np.sqrt(max(1.0 - sin_e ** 2, 0.0))
+        d = (500.0 * (cos_e * (np.cos(phi) * e1 + np.sin(phi) * e2) + sin_e * n)).astype(np.float32)
+        dd = d.astype(np.float64)
+        if not (dd @ n / np.linalg.norm(dd) > s_lo + 1e-6):
+            continue
+        facet, tau = om.closest_hit(p, d, f_prev=f, use_bvh=(m.nt > 30000))
+        assert facet == -1, (name, slot, f, k, b, sin_e, facet, tau)
+        tested += 1
+    assert tested > 300
+    if name in ("C2", "C5small"):
+        assert (hz < 128).mean() > 0.5
+    gm.close()
