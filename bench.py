@@ -27,9 +27,10 @@ import numpy as np
 
 import tpmc_inputs as ti
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one steady-state k_trace_wf launch (6.9 M rays), from the
-# `ncu --set full` capture summarised in profiles/r1_ncu_full_pipeline_v3.md
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 803_000_000
+# dram__bytes_read.sum + dram__bytes_write.sum of one steady-state k_trace_wf launch in this launch configuration
+# (wave of 2^26 particles, ~1.7e7 rays per launch), from the `ncu --set full` capture summarised in
+# profiles/r1_ncu_full_pipeline_v4.md
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 3_138_545_152
 METRIC = "particle_bounces_per_s"
 UNIT = "bounces/s"
 WORKLOAD = "C5: ~1.0e6-facet noise-displaced geodesic body + 6 panels, O/He 70/30, 900 K, 7700 m/s"
@@ -146,7 +147,7 @@ def main():
     ap.add_argument("--impl", default="tpmc", choices=["tpmc", "reference"])
     ap.add_argument("--particles", type=float, default=None, help="override N per step (default: the config's 1e9)")
     ap.add_argument("--ref-particles", type=float, default=4_000_000, help="oracle particles per reference step")
-    ap.add_argument("--cpu-baseline-particles", type=float, default=20_000_000)
+    ap.add_argument("--cpu-baseline-particles", type=float, default=80_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -278,8 +279,9 @@ def main():
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": WORKLOAD, "particles_per_step": N, "facets": mesh.nt, "bvh_nodes": info["n_nodes"],
                        "attitudes": "fibonacci(64)[step*world+rank]", "cv_radius_factor": cfgs[0].cv_radius_factor,
-                       "l2": "working set > L2: BVH+triangles 114 MB, per-facet momentum 25 MB, ray queue rewritten each wave",
-                       "mesh_build_ms": info["build_ms"]},
+                       "l2": "inputs larger than L2: hierarchy + facets 149 MB (33 MB compact nodes, 66 MB fp32 nodes, 50 MB facets), per-facet momentum 25 MB, ~2 GB of lists and ray queues rewritten every wave",
+                       "mesh_build_ms": info["build_ms"], "horizon_build_ms": info["horizon_ms"],
+                       "wave_particles": 1 << 26},
             "clocks": clocks,
             "rates": {"segments_per_s": segs_all / (ms_total_max * 1e-3), "particles_per_s": parts_all / (ms_total_max * 1e-3),
                       "hits_per_particle": hits_all / parts_all},
