@@ -59,7 +59,7 @@ struct tpmc_mesh {
   float q_origin[3], q_scale[3];   // its quantisation grid: x = q_origin + q * q_scale, q in [0, 65535]
   uint4* horizon;                  // [nt] by sorted slot: escape horizon of each facet, 16 azimuth sectors x 1 byte (k_horizon, lbvh.cu)
   double horizon_ms;
-  float4* cull;                    // top of the hierarchy (<= kCullNodes nodes, breadth-first), for the seed-time cull
+  uint4* cull_c;                   // top of the hierarchy (<= kCullNodes nodes, breadth-first) in the compact format of `cnodes`: seed-time cull
   int n_cull;
   double centre[3];
   double Rb;

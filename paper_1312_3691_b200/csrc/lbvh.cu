@@ -216,8 +216,9 @@ __global__ void k_compact_nodes(const float4* __restrict__ nodes, int64_t n_node
 
 // Top of the tree, breadth-first, cut at a node budget: child refs >= 0 index this array, -1 marks a
 // subtree (or triangle) that was cut off.  A ray that touches no cut-off box cannot hit the mesh.
-__global__ void k_build_cull(const float4* __restrict__ nodes, float4* __restrict__ cull, int* __restrict__ queue,
-                             int budget, int* __restrict__ out_count) {
+// Nodes in the compact 32-byte format of k_compact_nodes (what the seed kernel walks).
+__global__ void k_build_cull(const float4* __restrict__ nodes, const uint4* __restrict__ cnodes,
+                             uint4* __restrict__ cull_c, int* __restrict__ queue, int budget, int* __restrict__ out_count) {
   if (blockIdx.x != 0 || threadIdx.x != 0) return;
   int tail = 1;
   queue[0] = 0;
@@ -229,10 +230,9 @@ __global__ void k_build_cull(const float4* __restrict__ nodes, float4* __restric
       if (ref[k] >= 0 && tail < budget) { queue[tail] = ref[k]; ref[k] = tail++; }
       else ref[k] = -1;
     }
-    cull[4 * head + 0] = np[0];
-    cull[4 * head + 1] = np[1];
-    cull[4 * head + 2] = np[2];
-    cull[4 * head + 3] = make_float4(__int_as_float(ref[0]), __int_as_float(ref[1]), 0.0f, 0.0f);
+    const uint4 ca = cnodes[2 * (size_t)queue[head]], cb = cnodes[2 * (size_t)queue[head] + 1];
+    cull_c[2 * head] = ca;
+    cull_c[2 * head + 1] = make_uint4(cb.x, cb.y, (unsigned int)ref[0], (unsigned int)ref[1]);
   }
   *out_count = tail;
 }
@@ -528,11 +528,11 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
         (double)m->q_scale[0], (double)m->q_scale[1], (double)m->q_scale[2], m->cnodes);
   }
   DevBuf cq;
-  MESH_TRY(cudaMalloc((void**)&m->cull, sizeof(float4) * 4 * kCullNodes));
+  MESH_TRY(cudaMalloc((void**)&m->cull_c, sizeof(uint4) * 2 * kCullNodes));
   MESH_TRY(cudaMalloc(&cq.p, sizeof(int) * (kCullNodes + 1)));
   int cull_budget = kCullNodes;
   if (const char* e = getenv("TPMC_CULL_NODES")) cull_budget = std::max(1, std::min(kCullNodes, atoi(e)));   // tuning aid
-  k_build_cull<<<1, 32, 0, st>>>(m->nodes, m->cull, cq.as<int>(), cull_budget, cq.as<int>() + kCullNodes);
+  k_build_cull<<<1, 32, 0, st>>>(m->nodes, m->cnodes, m->cull_c, cq.as<int>(), cull_budget, cq.as<int>() + kCullNodes);
   MESH_TRY(cudaMemcpyAsync(&m->n_cull, cq.as<int>() + kCullNodes, sizeof(int), cudaMemcpyDeviceToHost, st));
   MESH_TRY(cudaGetLastError());
   MESH_TRY(cudaEventRecord(e1, st));
@@ -558,7 +558,7 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
 
 extern "C" void tpmc_mesh_destroy(tpmc_mesh* m) {
   if (!m) return;
-  cudaFree(m->nodes); cudaFree(m->tris); cudaFree(m->cull); cudaFree(m->cnodes); cudaFree(m->horizon);
+  cudaFree(m->nodes); cudaFree(m->tris); cudaFree(m->cull_c); cudaFree(m->cnodes); cudaFree(m->horizon);
   for (int pi = 0; pi < kPipes; ++pi) {
     Pipe& pp = m->pipe[pi];
     for (int k = 0; k < 2; ++k) { cudaFree(pp.q_o[k]); cudaFree(pp.q_v[k]); cudaFree(pp.q_f[k]); }

@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(kPrecullBlock) k_seed_precull(const SeedConstF
 __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned int wave_first,
                                                      unsigned int wave_n, const unsigned int* __restrict__ surv,
                                                      unsigned int cap_s, const unsigned int* __restrict__ n_surv,
-                                                     const float4* __restrict__ cull, int walk,
+                                                     const uint4* __restrict__ cull_c, const QuantGrid grid, int walk,
                                                      const RayQueue q, unsigned int region_b,
                                                      unsigned int* __restrict__ qcount,
                                                      unsigned long long* __restrict__ stats) {
@@ -127,9 +127,8 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
     for (int k = 0; k < 3; ++k) { o[k] = (float)s.x[k]; v[k] = (float)s.v[k]; }
     const float id[3] = {1.0f / v[0], 1.0f / v[1], 1.0f / v[2]};
     float tn;
-    float te;
     keep = slab(rc.aabb_lo[0], rc.aabb_lo[1], rc.aabb_lo[2], rc.aabb_hi[0], rc.aabb_hi[1], rc.aabb_hi[2], o, id,
-                INFINITY, tn) && (!walk || cull_touch(cull, o, id, te));
+                INFINITY, tn) && (!walk || cull_touch_q(cull_c, grid, o, v));
   }
   const unsigned m = __ballot_sync(0xFFFFFFFFu, keep);
   const unsigned mc = __ballot_sync(0xFFFFFFFFu, active && !keep);
@@ -919,7 +918,7 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
           ++launches;
         }
         k_seed<<<std::min<unsigned int>(gfull, (unsigned int)g.seed), kSeedBlock, 0, s2>>>(
-            rcc, w0, wn, precull ? pp.surv : nullptr, cap, pp.ctr + 6, m->cull, seed_walk, Q[p], cap, pp.ctr + 2 * p + 1,
+            rcc, w0, wn, precull ? pp.surv : nullptr, cap, pp.ctr + 6, m->cull_c, qg, seed_walk, Q[p], cap, pp.ctr + 2 * p + 1,
             m->stats);
         if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[1], s2));
         TPMC_CUDA_TRY(cudaEventRecord(pp.ev_seeded[li & 3], s2));

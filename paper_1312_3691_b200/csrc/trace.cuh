@@ -202,52 +202,40 @@ __device__ __forceinline__ void ldg256u(const uint4* p, uint4& a, uint4& b) {
                : "l"(p));
 }
 
-// ---- seed-time cull: can the ray touch any cut-off subtree of the top tree? (conservative) ------------
-// Near child first, so the first cut-off box found is (nearly) the first along the ray; its entry
-// distance is returned and later gives the ray its sort key (a point close to where it will hit).
-__device__ __forceinline__ bool cull_touch(const float4* __restrict__ cull, const float o[3], const float id[3],
-                                           float& t_entry) {
-  int stack[24];
-  int sp = 0, node = 0;
-  t_entry = 0.0f;
-  for (;;) {
-    const float4* np = cull + 4 * node;
-    float4 n0, n1, n2, n3;
-    ldg256(np, n0, n1);
-    ldg256(np + 2, n2, n3);
-    float t0, t1;
-    bool h0 = slab(n0.x, n0.y, n0.z, n0.w, n1.x, n1.y, o, id, INFINITY, t0);
-    bool h1 = slab(n1.z, n1.w, n2.x, n2.y, n2.z, n2.w, o, id, INFINITY, t1);
-    int c0 = __float_as_int(n3.x), c1 = __float_as_int(n3.y);
-    if (h0 && h1 && t1 < t0) {
-      const int c = c0; c0 = c1; c1 = c;
-      const float t = t0; t0 = t1; t1 = t;
-    } else if (!h0 && h1) {
-      c0 = c1; t0 = t1; h0 = true; h1 = false;
-    }
-    if (h0 && c0 < 0) { t_entry = fmaxf(t0, 0.0f); return true; }
-    if (h0) {
-      if (h1) {
-        if (sp >= 24) { t_entry = fmaxf(t0, 0.0f); return true; }   // deeper than the stack: keep the ray
-        stack[sp++] = c1 < 0 ? (int)(0x80000000u | (__float_as_uint(fmaxf(t1, 0.0f)) >> 1)) : c1;
-      }
-      node = c0;
-    } else {
-      if (sp == 0) return false;
-      node = stack[--sp];
-    }
-    if (node < 0) {   // a cut-off box that was pushed as the far child: reached now
-      t_entry = __uint_as_float(((unsigned)node & 0x7FFFFFFFu) << 1);
-      return true;
-    }
+// Per-ray constants of the grid-coordinate slab test (see above): 1/d', the two offsets and the permute selectors.
+struct GridRay {
+  float id[3], ncn[3], ncf[3];
+  unsigned int sn[3], sf[3];
+};
+__device__ __forceinline__ void grid_ray(GridRay& r, const QuantGrid& g, const float o[3], const float d[3]) {
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const float dq = d[k] * g.inv_scale[k];
+    const float idk = __fdividef(1.0f, dq);                  // 2 ulp
+    const float oq = (o[k] - g.origin[k]) * g.inv_scale[k];
+    const float O = 8388608.0f + oq;
+    const float G = fmaf(1.4901161e-07f, fabsf(O), fmaf(5.9604645e-07f, fabsf(oq), 0.1f));   // 2.5u|O| + 10u|o'| + 0.1
+    const float mg = G * fabsf(idk);
+    r.id[k] = idk;
+    r.ncn[k] = fmaf(-O, idk, -mg);
+    r.ncf[k] = fmaf(-O, idk, mg);
+    const bool neg = dq < 0.0f;
+    r.sn[k] = neg ? 0x7632u : 0x7610u;
+    r.sf[k] = neg ? 0x7610u : 0x7632u;
   }
+}
+// entry and exit distance of the box stored in words (wx, wy, wz) of a compact node
+__device__ __forceinline__ void grid_slab(const GridRay& r, unsigned int wx, unsigned int wy, unsigned int wz, float& tn,
+                                          float& tf) {
+  tn = fmaxf(fmaxf(fmaf(q_plane(wx, r.sn[0]), r.id[0], r.ncn[0]), fmaf(q_plane(wy, r.sn[1]), r.id[1], r.ncn[1])),
+             fmaf(q_plane(wz, r.sn[2]), r.id[2], r.ncn[2]));
+  tf = fminf(fminf(fmaf(q_plane(wx, r.sf[0]), r.id[0], r.ncf[0]), fmaf(q_plane(wy, r.sf[1]), r.id[1], r.ncf[1])),
+             fmaf(q_plane(wz, r.sf[2]), r.id[2], r.ncf[2]));
 }
 
 // ---- per-ray traversal state of the wavefront kernel -------------------------------------------------
 struct Walk {
-  float id[3];         // 1/d' (grid coordinates)
-  float ncn[3], ncf[3];   // -(O id) -+ G |id|: offsets of the near and far plane distances (see above)
-  unsigned int sn[3], sf[3];   // byte-permute selectors of the near and far plane of each axis
+  GridRay g;           // the ray in grid coordinates
   float tmax;          // min over provable hits of their thi
   int f_prev;
   int cur;             // node to visit next (>= 0 internal, < 0 leaf ~slot), TPMC_SENTINEL when the stack is empty
@@ -260,21 +248,7 @@ struct Walk {
 
 __device__ __forceinline__ void walk_init(Walk& w, const QuantGrid& g, const float4 ro, const float4 rv, int f_prev) {
   const float o[3] = {ro.x, ro.y, ro.z}, d[3] = {rv.x, rv.y, rv.z};
-#pragma unroll
-  for (int k = 0; k < 3; ++k) {
-    const float dq = d[k] * g.inv_scale[k];
-    const float idk = __fdividef(1.0f, dq);                  // 2 ulp
-    const float oq = (o[k] - g.origin[k]) * g.inv_scale[k];
-    const float O = 8388608.0f + oq;
-    const float G = fmaf(1.4901161e-07f, fabsf(O), fmaf(5.9604645e-07f, fabsf(oq), 0.1f));   // 2.5u|O| + 10u|o'| + 0.1
-    const float mg = G * fabsf(idk);
-    w.id[k] = idk;
-    w.ncn[k] = fmaf(-O, idk, -mg);
-    w.ncf[k] = fmaf(-O, idk, mg);
-    const bool neg = dq < 0.0f;
-    w.sn[k] = neg ? 0x7632u : 0x7610u;
-    w.sf[k] = neg ? 0x7610u : 0x7632u;
-  }
+  grid_ray(w.g, g, o, d);
   w.tmax = INFINITY;
   w.f_prev = f_prev;
   w.cur = 0;
@@ -283,6 +257,37 @@ __device__ __forceinline__ void walk_init(Walk& w, const QuantGrid& g, const flo
   w.nc = 0;
 #pragma unroll
   for (int k = 0; k < TPMC_MAX_CAND; ++k) { w.cs[k] = -1; w.cl[k] = 0.0f; }
+}
+
+// ---- seed-time cull on the compact copy of the top of the hierarchy (k_build_cull): can the ray touch any
+// cut-off subtree?  Any-hit: true as soon as a box whose child ref is cut off (< 0) is touched.  Conservative
+// like the traversal (same slab test); a walk deeper than the stack keeps the ray.
+__device__ __forceinline__ bool cull_touch_q(const uint4* __restrict__ cc, const QuantGrid& g, const float o[3],
+                                             const float d[3]) {
+  GridRay r;
+  grid_ray(r, g, o, d);
+  int stack[16];
+  int sp = 0, node = 0;
+  for (;;) {
+    uint4 a, b;
+    ldg256u(cc + 2 * (size_t)node, a, b);
+    float n0, f0, n1, f1;
+    grid_slab(r, a.x, a.y, a.z, n0, f0);
+    grid_slab(r, a.w, b.x, b.y, n1, f1);
+    const bool h0 = !(fmaxf(n0, 0.0f) > f0), h1 = !(fmaxf(n1, 0.0f) > f1);
+    const int c0 = (int)b.z, c1 = (int)b.w;
+    if ((h0 && c0 < 0) || (h1 && c1 < 0)) return true;
+    if (h0 && h1) {
+      if (sp >= 16) return true;
+      stack[sp++] = c1;
+      node = c0;
+    } else if (h0 || h1) {
+      node = h0 ? c0 : c1;
+    } else {
+      if (sp == 0) return false;
+      node = stack[--sp];
+    }
+  }
 }
 
 // Stack: TPMC_STACK_SMEM entries per thread in shared memory, [level][thread], above two guard entries that
@@ -337,14 +342,9 @@ __device__ __forceinline__ void walk_node(Walk& w, const uint4* __restrict__ cno
   uint4 a, b;
   ldg256u(cnodes + 2 * (size_t)w.cur, a, b);
   ++cnt.nodes;
-  const float n0 = fmaxf(fmaxf(fmaf(q_plane(a.x, w.sn[0]), w.id[0], w.ncn[0]), fmaf(q_plane(a.y, w.sn[1]), w.id[1], w.ncn[1])),
-                         fmaf(q_plane(a.z, w.sn[2]), w.id[2], w.ncn[2]));
-  const float f0 = fminf(fminf(fmaf(q_plane(a.x, w.sf[0]), w.id[0], w.ncf[0]), fmaf(q_plane(a.y, w.sf[1]), w.id[1], w.ncf[1])),
-                         fmaf(q_plane(a.z, w.sf[2]), w.id[2], w.ncf[2]));
-  const float n1 = fmaxf(fmaxf(fmaf(q_plane(a.w, w.sn[0]), w.id[0], w.ncn[0]), fmaf(q_plane(b.x, w.sn[1]), w.id[1], w.ncn[1])),
-                         fmaf(q_plane(b.y, w.sn[2]), w.id[2], w.ncn[2]));
-  const float f1 = fminf(fminf(fmaf(q_plane(a.w, w.sf[0]), w.id[0], w.ncf[0]), fmaf(q_plane(b.x, w.sf[1]), w.id[1], w.ncf[1])),
-                         fmaf(q_plane(b.y, w.sf[2]), w.id[2], w.ncf[2]));
+  float n0, f0, n1, f1;
+  grid_slab(w.g, a.x, a.y, a.z, n0, f0);
+  grid_slab(w.g, a.w, b.x, b.y, n1, f1);
   // the clamps also drop a NaN that survived three NaN plane distances (zero direction)
   const bool h0 = !(fmaxf(n0, 0.0f) > fminf(f0, w.tmax));
   const bool h1 = !(fmaxf(n1, 0.0f) > fminf(f1, w.tmax));
