@@ -442,3 +442,40 @@ def test_rays_above_the_escape_horizon_hit_nothing(T, O, name):
     if name in ("C2", "C5small"):
         assert (hz < 128).mean() > 0.5
     gm.close()
+
+
+def test_c5_whole_stream_in_one_run_sampled_against_the_oracle(T, O):
+    """The launch configuration bench.py times: ONE tpmc_run of all N = 1e9 particles of a C5 attitude (15 waves of
+    2^26 particles, cross-wave queues, escape horizons, pre-cull), with the per-particle outputs kept (16 GB).
+    Windows of the stream are compared particle by particle with the oracle; properties that hold at any size
+    (F = sum of P_f, segment count, slices summing to the whole) are checked on the whole run."""
+    import torch
+    cfg = ti.config("C5")[7]
+    gm, om = meshes(T, O, cfg)
+    g = gm.run(cfg, debug=True)
+    st = g.stats
+    assert st["truncated"] == 0 and st["segments"] == cfg.N + st["hits"]
+    assert 0.15 * cfg.N < st["hits"] < 0.20 * cfg.N
+    fm = g.facet_momentum
+    F = g.force.cpu().numpy()
+    assert np.allclose(fm.sum(0).cpu().numpy(), F, rtol=1e-10)
+    assert int((g.bounces > 0).sum().item()) <= st["hits"] and int(g.bounces.sum(dtype=torch.int64).item()) == st["hits"]
+    worst = 1.0
+    for first, count in ((0, 100_000), (67_108_864 - 50_000, 100_000), (523_456_789, 100_000), (999_900_000, 100_000)):
+        o = om.run(cfg, first=first, count=count, facets=False)
+        gh = g.hash[first:first + count].cpu().numpy().view(np.uint64)
+        same = gh == o.hash
+        worst = min(worst, same.mean())
+        assert same.mean() >= SEQ_AGREE
+        assert np.array_equal(g.bounces[first:first + count].cpu().numpy().astype(np.uint32)[same], o.bounces[same])
+        assert np.array_equal(g.first_facet[first:first + count].cpu().numpy()[same], o.first_facet[same])
+    del g
+    torch.cuda.empty_cache()
+    # the whole run equals the sum of its quarters (different wave boundaries, different queue contents)
+    Fq, hq = np.zeros(3), 0
+    for k in range(4):
+        r = gm.run(cfg, first=k * 250_000_000, count=250_000_000, facets=False)
+        Fq += r.force.cpu().numpy()
+        hq += r.stats["hits"]
+    assert hq == st["hits"]
+    assert np.linalg.norm(Fq - F) <= 1e-11 * np.linalg.norm(F)
