@@ -250,7 +250,7 @@ __global__ void k_build_cull(const float4* __restrict__ nodes, const uint4* __re
 //   * position: a hit at x = p + tau d has sin E = n.(x - p) / |x - p|.  With c, rho the centre and radius
 //     of f's bounding sphere, for x in B:  n.(x - p) <= h(B) = max_B n.(x - a0) + delta  and
 //     |x - p| >= dist(c, B) - rho - delta,  delta covering the fp32 rounding of the ray origin (O13).
-//     h(B) <= 0: B lies below f's plane and cannot be reached.
+//     h(B) <= 0: B lies below f's plane and cannot be reached.  For a facet g, h is taken over its corners.
 //   * azimuth: x - p lies in the ball of radius R = r_B + rho + delta about w = centre(B) - c, so d is within
 //     alpha = asin(R / |w|) of w; if that cone does not contain the pole its azimuths lie within
 //     asin(sin alpha / sin theta) of w's, theta = angle(w, n).  Otherwise, or when |w| <= R, all sectors.
@@ -368,7 +368,13 @@ __global__ void __launch_bounds__(128) k_horizon(const float4* __restrict__ node
           const int64_t g = ~ref[ch];
           if (g == s) continue;
           const float4 g0 = __ldg(tris + 3 * g), g1 = __ldg(tris + 3 * g + 1), g2 = __ldg(tris + 3 * g + 2);
-          double b = bnd;
+          // height of the facet itself (a linear function: its maximum is at a corner), not of its box
+          const double hv = f.delta + fmax(fmax(f.n[0] * ((double)g0.x - f.a0[0]) + f.n[1] * ((double)g0.y - f.a0[1]) + f.n[2] * ((double)g0.z - f.a0[2]),
+                                               f.n[0] * ((double)g1.x - f.a0[0]) + f.n[1] * ((double)g1.y - f.a0[1]) + f.n[2] * ((double)g1.z - f.a0[2])),
+                                          f.n[0] * ((double)g2.x - f.a0[0]) + f.n[1] * ((double)g2.y - f.a0[1]) + f.n[2] * ((double)g2.z - f.a0[2]));
+          if (!(hv > 0.0)) continue;                 // wholly below the plane of f
+          const double den = dist[ch] * (1.0 - 1e-12) - f.rho - f.delta;
+          double b = den > 0.0 ? fmin(bnd, hv / den) : bnd;
           if ((__float_as_uint(g1.w) & TPMC_FACET_TWO_SIDED) == 0u) {
             const double f1[3] = {(double)g1.x - g0.x, (double)g1.y - g0.y, (double)g1.z - g0.z};
             const double f2[3] = {(double)g2.x - g0.x, (double)g2.y - g0.y, (double)g2.z - g0.z};
