@@ -91,6 +91,12 @@ def sphere_cd(S, S_W):
             + 2 * SQRTPI / (3 * S_W))
 
 
+def pratt_hemisphere_cd(S, Tw_over_Tinf, eps_d=1.05349):
+    """Concave hemispherical shell in hyperthermal flow, eq. (5) PAPER.md:100 with eps_D(90 deg) = 1.05349
+    (PAPER.md:103); A_ref = pi R^2.  An asymptote for S -> inf."""
+    return 2.0 + eps_d * np.sqrt(np.pi) / S * np.sqrt(Tw_over_Tinf)
+
+
 def cylinder_crossflow_cd(S, S_W):
     """Infinite cylinder normal to the stream, diffuse, A_ref = 2 R L (Schaaf & Chambre form)."""
     h = 0.5 * S * S

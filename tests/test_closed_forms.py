@@ -79,3 +79,9 @@ def test_cylinder_crossflow_closed_form():
     for S in (2.0, S1):
         F, _, _ = cf.panel_sum(tri[side], cy.flags[side], [1, 0, 0], S, SW1)
         assert -F[0] / 2.0 == pytest.approx(cf.cylinder_crossflow_cd(S, SW1), rel=1e-5)
+
+
+def test_pratt_concave_hemisphere_golden():
+    for S, v in cf.golden("shell_CD").items():
+        assert cf.pratt_hemisphere_cd(S, 300.0 / 922.0) == pytest.approx(v, abs=2e-6)
+    assert cf.pratt_hemisphere_cd(1e9, 0.3) == pytest.approx(2.0, abs=1e-8)

@@ -64,7 +64,9 @@ def compare_run(T, O, cfg, first, count, use_bvh=True):
         err = np.linalg.norm(fm - o.facet_momentum, axis=1)
         assert np.all(err <= FACET_RTOL * nrm + 1e-300), (cfg.label, float((err / np.maximum(nrm, 1e-300)).max()))
         assert np.array_equal(nrm == 0, np.linalg.norm(fm, axis=1) == 0)       # untouched facets stay exactly zero
-    assert np.allclose(fm.sum(0), F, rtol=1e-12, atol=1e-30)                    # a7: F = sum_f P_f
+    # a7: F = sum_f P_f, to the rounding of an fp64 sum of these terms (1e-12 of sum |P_f|: a component that
+    # cancels to ~0, like the side force of an axisymmetric body, has no relative accuracy of its own)
+    assert np.all(np.abs(fm.sum(0) - F) <= 1e-12 * np.abs(fm).sum(0) + 1e-30)
     return g, o, frac
 
 
@@ -479,3 +481,16 @@ def test_c5_whole_stream_in_one_run_sampled_against_the_oracle(T, O):
         hq += r.stats["hits"]
     assert hq == st["hits"]
     assert np.linalg.norm(Fq - F) <= 1e-11 * np.linalg.norm(F)
+
+
+@pytest.mark.parametrize("S", [5.0, 40.0])
+def test_run_parity_concave_shell(T, O, S):
+    """NEXT-2 workload: two-sided hemispherical shell, concave to the stream, at the paper's
+    verification temperatures; 0.7 hits per particle, two-sided facets (no escape horizon), hits from both sides."""
+    m = ti.hemisphere_shell(16)
+    mO = 16 * ti.AMU
+    speed = S * np.sqrt(2 * ti.K_B * 922.0 / mO)
+    cfg = ti.RunConfig("shell", lambda: m, T_inf=922.0, T_W=300.0, V=(-speed, 0.0, 0.0), N=300_000,
+                       A_ref=float(np.pi), seed=14, label=f"concave shell S={S:g}")
+    g, o, _ = compare_run(T, O, cfg, 0, 300_000)
+    assert g.stats["hits"] == o.hits > 0.6 * cfg.N
