@@ -61,6 +61,10 @@ struct tpmc_mesh {
   double horizon_ms;
   uint4* cull_c;                   // top of the hierarchy (<= kCullNodes nodes, breadth-first) in the compact format of `cnodes`: seed-time cull
   int n_cull;
+  // two-level cull volume of the pre-cull pass: all facets lie within cull_rin of the centre or in a box
+  float cull_rin;
+  int cull_nbox;                   // -1: not used (no gain over the bounding sphere)
+  float cull_box[8][6];            // lo.xyz, hi.xyz
   double centre[3];
   double Rb;
   float aabb_lo[3], aabb_hi[3];

@@ -407,12 +407,153 @@ __global__ void __launch_bounds__(128) k_horizon(const float4* __restrict__ node
   horizon[s] = make_uint4(cur[0], cur[1], cur[2], cur[3]);
 }
 
+// ---- two-level cull volume for the pre-cull pass (a0) --------------------------------------------------------
+// A body with a compact core and a few far-reaching parts (panels, booms) fills little of its bounding sphere or
+// box.  Every facet is put either in the sphere of radius R_in about the centre (its farthest corner is within
+// R_in) or, as an "outlier", in one of at most 8 boxes; a ray that misses the sphere and all boxes misses the
+// mesh.  R_in is chosen among quantiles of the facets' reach, the outliers are binned into 4^3 cells of the AABB
+// and the cell boxes merged greedily (smallest growth of surface area) on the host; the choice with the smallest
+// mean projected area wins, and the volume is not used when it is no better than the bounding sphere.
+constexpr int kReachBins = 1024;
+__device__ __forceinline__ float facet_reach(const float4* __restrict__ tris, int64_t s, float cx, float cy, float cz) {
+  float d2 = 0.0f;
+  for (int k = 0; k < 3; ++k) {
+    const float4 q = tris[3 * s + k];
+    const float dx = q.x - cx, dy = q.y - cy, dz = q.z - cz;
+    d2 = fmaxf(d2, __fadd_ru(__fadd_ru(__fmul_ru(dx, dx), __fmul_ru(dy, dy)), __fmul_ru(dz, dz)));
+  }
+  return __fsqrt_ru(d2) * 1.000001f;   // >= the true distance (the centre is rounded to fp32: 1e-6 covers it)
+}
+__global__ void k_reach_hist(const float4* __restrict__ tris, int64_t nt, float cx, float cy, float cz, float inv_bin,
+                             unsigned int* __restrict__ hist) {
+  const int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (s >= nt) return;
+  const int b = min(kReachBins - 1, (int)(facet_reach(tris, s, cx, cy, cz) * inv_bin));
+  atomicAdd(&hist[b], 1u);
+}
+__device__ __forceinline__ unsigned int float_order(float f) {   // monotone map float -> unsigned
+  const unsigned int u = __float_as_uint(f);
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+// boxes [64][6] as ordered unsigned: lo.xyz (atomicMin), hi.xyz (atomicMax) of the facets with reach > r_in
+__global__ void k_outlier_boxes(const float4* __restrict__ tris, int64_t nt, float cx, float cy, float cz, float r_in,
+                                float3 lo, float3 inv_ext, unsigned int* __restrict__ boxes) {
+  const int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (s >= nt) return;
+  if (!(facet_reach(tris, s, cx, cy, cz) > r_in)) return;
+  const float4 a = tris[3 * s], b = tris[3 * s + 1], c = tris[3 * s + 2];
+  const int ix = min(3, max(0, (int)(((a.x + b.x + c.x) * (1.0f / 3.0f) - lo.x) * inv_ext.x * 4.0f)));
+  const int iy = min(3, max(0, (int)(((a.y + b.y + c.y) * (1.0f / 3.0f) - lo.y) * inv_ext.y * 4.0f)));
+  const int iz = min(3, max(0, (int)(((a.z + b.z + c.z) * (1.0f / 3.0f) - lo.z) * inv_ext.z * 4.0f)));
+  unsigned int* bx = boxes + 6 * (16 * ix + 4 * iy + iz);
+  atomicMin(bx + 0, float_order(fminf(a.x, fminf(b.x, c.x))));
+  atomicMin(bx + 1, float_order(fminf(a.y, fminf(b.y, c.y))));
+  atomicMin(bx + 2, float_order(fminf(a.z, fminf(b.z, c.z))));
+  atomicMax(bx + 3, float_order(fmaxf(a.x, fmaxf(b.x, c.x))));
+  atomicMax(bx + 4, float_order(fmaxf(a.y, fmaxf(b.y, c.y))));
+  atomicMax(bx + 5, float_order(fmaxf(a.z, fmaxf(b.z, c.z))));
+}
+
 struct DevBuf {  // frees on scope exit
   void* p = nullptr;
   ~DevBuf() { if (p) cudaFree(p); }
   template <class T> T* as() { return (T*)p; }
 };
 
+}  // namespace
+
+
+namespace {
+float float_unorder(unsigned int u) {
+  const unsigned int b = (u & 0x80000000u) ? (u & 0x7FFFFFFFu) : ~u;
+  float f;
+  memcpy(&f, &b, 4);
+  return f;
+}
+struct HBox { float lo[3], hi[3]; };
+double half_area(const HBox& b, double g) {
+  const double e0 = (double)b.hi[0] - b.lo[0] + 2 * g, e1 = (double)b.hi[1] - b.lo[1] + 2 * g, e2 = (double)b.hi[2] - b.lo[2] + 2 * g;
+  return e0 * e1 + e1 * e2 + e0 * e2;   // = 2 x the mean projected area of a box (Cauchy: surface / 4)
+}
+HBox merged(const HBox& a, const HBox& b) {
+  HBox m;
+  for (int k = 0; k < 3; ++k) { m.lo[k] = std::min(a.lo[k], b.lo[k]); m.hi[k] = std::max(a.hi[k], b.hi[k]); }
+  return m;
+}
+
+// Choose the two-level cull volume (see k_reach_hist).  Leaves m->cull_nbox = -1 when it does not pay.
+int build_cull_volume(tpmc_mesh* m, cudaStream_t st) {
+  m->cull_nbox = -1;
+  m->cull_rin = (float)m->Rb;
+  const int64_t nt = m->nt;
+  if (nt < 64) return TPMC_OK;
+  DevBuf hist, boxes;
+  TPMC_CUDA_TRY(cudaMalloc(&hist.p, sizeof(unsigned int) * kReachBins));
+  TPMC_CUDA_TRY(cudaMalloc(&boxes.p, sizeof(unsigned int) * 64 * 6));
+  TPMC_CUDA_TRY(cudaMemsetAsync(hist.p, 0, sizeof(unsigned int) * kReachBins, st));
+  const float cx = (float)m->centre[0], cy = (float)m->centre[1], cz = (float)m->centre[2];
+  const float bin = (float)(m->Rb * 1.0001 / kReachBins);
+  const unsigned gt = (unsigned)((nt + kBlock - 1) / kBlock);
+  k_reach_hist<<<gt, kBlock, 0, st>>>(m->tris, nt, cx, cy, cz, 1.0f / bin, hist.as<unsigned int>());
+  unsigned int h[kReachBins];
+  TPMC_CUDA_TRY(cudaMemcpyAsync(h, hist.p, sizeof(h), cudaMemcpyDeviceToHost, st));
+  TPMC_CUDA_TRY(cudaStreamSynchronize(st));
+  const double g = (double)kPrecullMargin * m->Rb, pi = 3.14159265358979323846;
+  const double Rg = m->Rb + g;
+  double best = 0.8 * 2.0 * pi * Rg * Rg;   // must beat the bounding sphere (2 x projected area) by 20 %
+  float3 lo = make_float3(m->aabb_lo[0], m->aabb_lo[1], m->aabb_lo[2]);
+  float3 ie;
+  ie.x = m->aabb_hi[0] > m->aabb_lo[0] ? 1.0f / (m->aabb_hi[0] - m->aabb_lo[0]) : 0.0f;
+  ie.y = m->aabb_hi[1] > m->aabb_lo[1] ? 1.0f / (m->aabb_hi[1] - m->aabb_lo[1]) : 0.0f;
+  ie.z = m->aabb_hi[2] > m->aabb_lo[2] ? 1.0f / (m->aabb_hi[2] - m->aabb_lo[2]) : 0.0f;
+  const double quantiles[] = {0.80, 0.90, 0.95, 0.97, 0.98, 0.99, 0.995};
+  int last_bin = -1;
+  for (double q : quantiles) {
+    unsigned long long acc = 0;
+    int b = 0;
+    for (; b < kReachBins; ++b) { acc += h[b]; if ((double)acc >= q * (double)nt) break; }
+    if (b >= kReachBins - 1 || b == last_bin) continue;
+    last_bin = b;
+    const float r_in = (float)(b + 1) * bin;
+    unsigned int init[64 * 6];
+    for (int i = 0; i < 64; ++i)
+      for (int k = 0; k < 6; ++k) init[6 * i + k] = k < 3 ? 0xFFFFFFFFu : 0u;
+    TPMC_CUDA_TRY(cudaMemcpyAsync(boxes.p, init, sizeof(init), cudaMemcpyHostToDevice, st));
+    k_outlier_boxes<<<gt, kBlock, 0, st>>>(m->tris, nt, cx, cy, cz, r_in, lo, ie, boxes.as<unsigned int>());
+    unsigned int raw[64 * 6];
+    TPMC_CUDA_TRY(cudaMemcpyAsync(raw, boxes.p, sizeof(raw), cudaMemcpyDeviceToHost, st));
+    TPMC_CUDA_TRY(cudaStreamSynchronize(st));
+    HBox bx[64];
+    int nb = 0;
+    for (int i = 0; i < 64; ++i) {
+      if (raw[6 * i] == 0xFFFFFFFFu) continue;   // empty cell
+      for (int k = 0; k < 3; ++k) { bx[nb].lo[k] = float_unorder(raw[6 * i + k]); bx[nb].hi[k] = float_unorder(raw[6 * i + 3 + k]); }
+      ++nb;
+    }
+    while (nb > 8) {   // greedy merge: the pair whose union adds the least area
+      int bi = 0, bj = 1;
+      double bc = 1e300;
+      for (int i = 0; i < nb; ++i)
+        for (int j = i + 1; j < nb; ++j) {
+          const double c = half_area(merged(bx[i], bx[j]), g) - half_area(bx[i], g) - half_area(bx[j], g);
+          if (c < bc) { bc = c; bi = i; bj = j; }
+        }
+      bx[bi] = merged(bx[bi], bx[bj]);
+      bx[bj] = bx[--nb];
+    }
+    const double ri = (double)r_in + g;
+    double proxy = 2.0 * pi * ri * ri;
+    for (int i = 0; i < nb; ++i) proxy += half_area(bx[i], g);
+    if (proxy < best) {
+      best = proxy;
+      m->cull_rin = r_in;
+      m->cull_nbox = nb;
+      for (int i = 0; i < nb; ++i)
+        for (int k = 0; k < 3; ++k) { m->cull_box[i][k] = bx[i].lo[k]; m->cull_box[i][3 + k] = bx[i].hi[k]; }
+    }
+  }
+  return TPMC_OK;
+}
 }  // namespace
 
 extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t* indices, int64_t nt,
@@ -540,6 +681,10 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
   if (const char* e = getenv("TPMC_CULL_NODES")) cull_budget = std::max(1, std::min(kCullNodes, atoi(e)));   // tuning aid
   k_build_cull<<<1, 32, 0, st>>>(m->nodes, m->cnodes, m->cull_c, cq.as<int>(), cull_budget, cq.as<int>() + kCullNodes);
   MESH_TRY(cudaMemcpyAsync(&m->n_cull, cq.as<int>() + kCullNodes, sizeof(int), cudaMemcpyDeviceToHost, st));
+  {
+    const int rcv = build_cull_volume(m, st);
+    if (rcv != TPMC_OK) { tpmc_mesh_destroy(m); return rcv; }
+  }
   MESH_TRY(cudaGetLastError());
   MESH_TRY(cudaEventRecord(e1, st));
   // escape horizons (timed apart from the hierarchy build)

@@ -660,6 +660,17 @@ void make_seed_const_f(const tpmc_mesh* m, const RunConst& rc, SeedConstF* sf) {
   sf->r = (float)rc.r;
   const float Rg = (float)m->Rb * (1.0f + kPrecullMargin);
   sf->Rg2 = Rg * Rg;
+  static const bool no_two_level = getenv("TPMC_CULL_VOLUME") && getenv("TPMC_CULL_VOLUME")[0] == '0';   // tuning aid
+  sf->n_box = no_two_level ? -1 : m->cull_nbox;
+  if (sf->n_box >= 0) {
+    const float Ri = m->cull_rin + mg;
+    sf->Rin2 = Ri * Ri;
+    for (int j = 0; j < sf->n_box; ++j)
+      for (int a = 0; a < 3; ++a) {
+        sf->blo[j][a] = m->cull_box[j][a] - mg;
+        sf->bhi[j][a] = m->cull_box[j][3 + a] + mg;
+      }
+  }
 }
 
 TraceTune trace_tune() {
@@ -844,7 +855,10 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
   const bool precull = !(pc_env && pc_env[0] == '0');
   const char* hz_env = getenv("TPMC_HORIZON");   // likewise: "0" switches the escape-horizon test off
   const bool use_horizon = !(hz_env && hz_env[0] == '0');
-  static const int seed_walk = (getenv("TPMC_SEED_WALK") && getenv("TPMC_SEED_WALK")[0] == '0') ? 0 : 1;   // tuning aid
+  // seed-time walk of the top of the hierarchy: pays only while the pre-cull pass has no two-level cull volume
+  // (with it the pass is already tighter than the 64-node tree); TPMC_SEED_WALK=0/1 forces it (tuning aid)
+  const char* sw_env = getenv("TPMC_SEED_WALK");
+  const int seed_walk = sw_env ? (sw_env[0] != '0') : (m->cull_nbox < 0 || (getenv("TPMC_CULL_VOLUME") && getenv("TPMC_CULL_VOLUME")[0] == '0'));
   SeedConstF sf;
   make_seed_const_f(m, rc, &sf);
   const QuantGrid qg = quant_grid(m);

@@ -266,6 +266,11 @@ struct SeedConstF {
   float R[9], centre[3], r;
   float lo[3], hi[3];  // grown mesh AABB
   float Rg2;           // (grown bounding radius)^2
+  // two-level cull volume (k_reach_hist / k_outlier_boxes in lbvh.cu): every facet lies in the sphere of radius
+  // R_in about the centre or in one of n_box boxes; both grown like the AABB.  n_box < 0: not used.
+  float Rin2;
+  int n_box;
+  float blo[8][3], bhi[8][3];
 };
 
 __device__ __forceinline__ float u01f(uint32_t w) { return ((float)w + 0.5f) * 2.3283064365386963e-10f; }
@@ -387,15 +392,31 @@ __device__ __forceinline__ bool precull_touch(const SeedConstF& sf, const float 
   // closest approach to the centre: |oc|^2 - b^2/|v|^2 <= Rg^2, approached (b < 0); 1e-3 relative slack on the
   // cancelling difference (the terms are ~2.25 R_b^2, their rounding ~1e-7 of that)
   const bool sphere = (b < 0.0f) && (b * b >= vv * (cc - 1e-3f * sf.Rg2));
+  const float id[3] = {__frcp_rn(v[0]), __frcp_rn(v[1]), __frcp_rn(v[2])};
   float ax[3], bx[3];
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
-    const float id = __frcp_rn(v[k]);
-    ax[k] = (sf.lo[k] - o[k]) * id;
-    bx[k] = (sf.hi[k] - o[k]) * id;
+    ax[k] = (sf.lo[k] - o[k]) * id[k];
+    bx[k] = (sf.hi[k] - o[k]) * id[k];
   }
   const float tn = fmaxf(fmaxf(fminf(ax[0], bx[0]), fminf(ax[1], bx[1])), fminf(ax[2], bx[2]));
   const float tf = fminf(fminf(fmaxf(ax[0], bx[0]), fmaxf(ax[1], bx[1])), fmaxf(ax[2], bx[2]));
   const bool box = fmaxf(tn, 0.0f) * 0.999999f <= tf * 1.000001f;   // NaN planes (0 * inf) are dropped by min/max
+  if (sf.n_box >= 0) {   // uniform branch: the inner sphere (same slack as above) or any of the outlier boxes
+    const float cin = fmaf(oc[2], oc[2], fmaf(oc[1], oc[1], oc[0] * oc[0])) - sf.Rin2;
+    bool any = (b < 0.0f) && (b * b >= vv * (cin - 1e-3f * sf.Rg2));
+    for (int j = 0; j < sf.n_box; ++j) {
+      float a2[3], b2[3];
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        a2[k] = (sf.blo[j][k] - o[k]) * id[k];
+        b2[k] = (sf.bhi[j][k] - o[k]) * id[k];
+      }
+      const float un = fmaxf(fmaxf(fminf(a2[0], b2[0]), fminf(a2[1], b2[1])), fminf(a2[2], b2[2]));
+      const float uf = fminf(fminf(fmaxf(a2[0], b2[0]), fmaxf(a2[1], b2[1])), fmaxf(a2[2], b2[2]));
+      any = any || (fmaxf(un, 0.0f) * 0.999999f <= uf * 1.000001f);
+    }
+    return sphere && box && any;
+  }
   return sphere && box;
 }
