@@ -392,12 +392,18 @@ __device__ __forceinline__ bool precull_touch(const SeedConstF& sf, const float 
   // closest approach to the centre: |oc|^2 - b^2/|v|^2 <= Rg^2, approached (b < 0); 1e-3 relative slack on the
   // cancelling difference (the terms are ~2.25 R_b^2, their rounding ~1e-7 of that)
   const bool sphere = (b < 0.0f) && (b * b >= vv * (cc - 1e-3f * sf.Rg2));
-  const float id[3] = {__frcp_rn(v[0]), __frcp_rn(v[1]), __frcp_rn(v[2])};
+  // plane distances as fma(plane, 1/v, -o/v): one instruction each.  The absolute error u |o/v| of this form is,
+  // relative to the width of a slab in t, u |o| / extent < 1e-5 -- far inside the growth of the volumes.
+  // (a direction component below 1e-30 is replaced by 1e-30: no inf - inf; the ray stays parallel to the slab)
+  const float vs[3] = {fabsf(v[0]) < 1e-30f ? 1e-30f : v[0], fabsf(v[1]) < 1e-30f ? 1e-30f : v[1],
+                       fabsf(v[2]) < 1e-30f ? 1e-30f : v[2]};
+  const float id[3] = {__frcp_rn(vs[0]), __frcp_rn(vs[1]), __frcp_rn(vs[2])};
+  const float oi[3] = {-o[0] * id[0], -o[1] * id[1], -o[2] * id[2]};
   float ax[3], bx[3];
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
-    ax[k] = (sf.lo[k] - o[k]) * id[k];
-    bx[k] = (sf.hi[k] - o[k]) * id[k];
+    ax[k] = fmaf(sf.lo[k], id[k], oi[k]);
+    bx[k] = fmaf(sf.hi[k], id[k], oi[k]);
   }
   const float tn = fmaxf(fmaxf(fminf(ax[0], bx[0]), fminf(ax[1], bx[1])), fminf(ax[2], bx[2]));
   const float tf = fminf(fminf(fmaxf(ax[0], bx[0]), fmaxf(ax[1], bx[1])), fmaxf(ax[2], bx[2]));
@@ -409,8 +415,8 @@ __device__ __forceinline__ bool precull_touch(const SeedConstF& sf, const float 
       float a2[3], b2[3];
 #pragma unroll
       for (int k = 0; k < 3; ++k) {
-        a2[k] = (sf.blo[j][k] - o[k]) * id[k];
-        b2[k] = (sf.bhi[j][k] - o[k]) * id[k];
+        a2[k] = fmaf(sf.blo[j][k], id[k], oi[k]);
+        b2[k] = fmaf(sf.bhi[j][k], id[k], oi[k]);
       }
       const float un = fmaxf(fmaxf(fminf(a2[0], b2[0]), fminf(a2[1], b2[1])), fminf(a2[2], b2[2]));
       const float uf = fminf(fminf(fmaxf(a2[0], b2[0]), fmaxf(a2[1], b2[1])), fmaxf(a2[2], b2[2]));
