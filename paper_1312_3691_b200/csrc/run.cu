@@ -360,7 +360,7 @@ __device__ __forceinline__ bool interact(const RunConst& rc, const float4* __res
 // Rays the traversal gave up on (too many candidates, stack too deep) and rays whose reflected successor
 // finds region A of the next queue full go, untouched, to the overflow list: k_finish follows them to escape
 // with the full fp64 traversal, densely, instead of one lane doing so here while its warp waits.
-__global__ void __launch_bounds__(kTraceBlock) k_reflect(const RunConst rc, unsigned int cap,
+__global__ void __launch_bounds__(kTraceBlock, 6) k_reflect(const RunConst rc, unsigned int cap,
                                                          const float4* __restrict__ tris, const RayQueue qin,
                                                          const unsigned int* __restrict__ hit_ray,
                                                          const int4* __restrict__ hit_cand,
