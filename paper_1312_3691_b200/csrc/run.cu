@@ -55,42 +55,88 @@ __global__ void k_iter_begin(unsigned int* __restrict__ ctr, int out_parity, int
   }
 }
 
-// a2, pre-cull pass (sampling.cuh): fp32 estimate of every particle's ray against the grown bounds.  Survivor
-// records (wave offset, fp32 roots) of certified estimates fill `surv` from the front, particles whose
-// estimate is not certified from the back; n_surv[0], n_surv[1] count them.  surv = [3][cap] words.
+// a2, pre-cull pass (sampling.cuh): fp32 estimate of every particle's ray against the grown cull volumes, in two
+// stages with a compaction inside the block (precull_stage_a/b): stage A (everything but the normal speed, and a
+// threshold test against the bounding sphere) for every particle of the block's share, survivors queued in
+// shared memory; whenever a full block of them is waiting, stage B (normal speed, ray, cull volumes) runs
+// densely on those.  Survivor records (wave offset, fp32 roots) of certified estimates fill `surv` from the
+// front, particles whose estimate is not certified from the back; n_surv[0], n_surv[1] count them.
+// surv = [3][cap] words, written with streaming stores (evict-first) like every list and queue of the path: the
+// hierarchy and the facets (83 MB at C5) should stay in L2 while ~2 GB of lists and queues pass through it.
+constexpr int kPrecullQ = 2 * kPrecullBlock;
 __global__ void __launch_bounds__(kPrecullBlock) k_seed_precull(const SeedConstF sf, unsigned int seed_lo,
-                                                                unsigned int seed_hi, unsigned long long first,
-                                                                unsigned int wave_n, unsigned int cap,
-                                                                unsigned int* __restrict__ surv,
-                                                                unsigned int* __restrict__ n_surv) {
-  __shared__ unsigned int s_cnt[2][kPrecullBlock / 32], s_base[2];
-  const unsigned int j = blockIdx.x * blockDim.x + threadIdx.x;
-  const bool active = j < wave_n;
-  float o[3], v[3], root[2];
-  const bool ok = seed_particle_approx(sf, seed_lo, seed_hi, first + j, o, v, root);
-  const bool touch = precull_touch(sf, o, v);
-  const bool keep_c = active && ok && touch, keep_u = active && !ok;
-  const unsigned mcert = __ballot_sync(0xFFFFFFFFu, keep_c);
-  const unsigned munc = __ballot_sync(0xFFFFFFFFu, keep_u);
-  // one atomic per block and list (a per-warp atomic on one address was the kernel's bottleneck)
+                                                                 unsigned int seed_hi, unsigned long long first,
+                                                                 unsigned int wave_n, unsigned int cap,
+                                                                 unsigned int* __restrict__ surv,
+                                                                 unsigned int* __restrict__ n_surv) {
+  __shared__ float qf[8][kPrecullQ];
+  __shared__ unsigned int qj[kPrecullQ], qw[kPrecullQ];
+  __shared__ unsigned char qok[kPrecullQ];
+  __shared__ unsigned int q_n, s_cnt[2][kPrecullBlock / 32], s_base[2];
+  const unsigned int per = (((wave_n + gridDim.x - 1) / gridDim.x) + kPrecullBlock - 1) / kPrecullBlock * kPrecullBlock;
+  const unsigned long long b64 = (unsigned long long)blockIdx.x * per;
+  const unsigned int begin = (unsigned int)min(b64, (unsigned long long)wave_n);
+  const unsigned int end = (unsigned int)min(b64 + per, (unsigned long long)wave_n);
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  if (lane == 0) { s_cnt[0][wid] = __popc(mcert); s_cnt[1][wid] = __popc(munc); }
+  if (threadIdx.x == 0) q_n = 0u;
   __syncthreads();
-  if (threadIdx.x < 2) {
-    unsigned int tot = 0;
-    for (int k = 0; k < kPrecullBlock / 32; ++k) { const unsigned int c = s_cnt[threadIdx.x][k]; s_cnt[threadIdx.x][k] = tot; tot += c; }
-    s_base[threadIdx.x] = tot ? atomicAdd(&n_surv[threadIdx.x], tot) : 0u;
+  unsigned int base = begin;
+  for (;;) {
+    const bool more = base < end;
+    if (more) {
+      const unsigned int j = base + threadIdx.x;
+      PrecullA a;
+      const bool pass = precull_stage_a(sf, seed_lo, seed_hi, first + j, a) && (j < end);
+      const unsigned m = __ballot_sync(0xFFFFFFFFu, pass);
+      unsigned int pos = 0;
+      if (lane == 0 && m) pos = atomicAdd(&q_n, (unsigned)__popc(m));
+      pos = __shfl_sync(0xFFFFFFFFu, pos, 0);
+      if (pass) {
+        const unsigned int sl = pos + __popc(m & lanemask_lt());
+        qf[0][sl] = a.y; qf[1][sl] = a.t; qf[2][sl] = a.cphi; qf[3][sl] = a.st; qf[4][sl] = a.ct;
+        qf[5][sl] = a.xt1; qf[6][sl] = a.xt2; qf[7][sl] = a.s;
+        qj[sl] = j; qw[sl] = a.w3; qok[sl] = a.ok_t ? 1 : 0;
+      }
+      base += kPrecullBlock;
+      __syncthreads();
+    }
+    const unsigned int n = q_n;
+    if (n >= (unsigned)kPrecullBlock || (!more && n > 0u)) {
+      const unsigned int take = min(n, (unsigned)kPrecullBlock);
+      const bool active = threadIdx.x < take;
+      const unsigned int sl = n - take + (active ? threadIdx.x : 0u);
+      PrecullA a;
+      a.y = qf[0][sl]; a.t = qf[1][sl]; a.cphi = qf[2][sl]; a.st = qf[3][sl]; a.ct = qf[4][sl];
+      a.xt1 = qf[5][sl]; a.xt2 = qf[6][sl]; a.s = qf[7][sl];
+      a.w3 = qw[sl]; a.ok_t = qok[sl] != 0;
+      const unsigned int j = qj[sl];
+      float o[3], v[3], root[2];
+      const bool ok = precull_stage_b(sf, a, o, v, root);
+      const bool touch = precull_touch(sf, o, v);
+      const bool keep_c = active && ok && touch, keep_u = active && !ok;
+      const unsigned mcert = __ballot_sync(0xFFFFFFFFu, keep_c);
+      const unsigned munc = __ballot_sync(0xFFFFFFFFu, keep_u);
+      if (lane == 0) { s_cnt[0][wid] = __popc(mcert); s_cnt[1][wid] = __popc(munc); }
+      __syncthreads();                      // also: every read of the queue entries above is done
+      if (threadIdx.x == 0) q_n = n - take;
+      if (threadIdx.x < 2) {
+        unsigned int tot = 0;
+        for (int k = 0; k < kPrecullBlock / 32; ++k) { const unsigned int c = s_cnt[threadIdx.x][k]; s_cnt[threadIdx.x][k] = tot; tot += c; }
+        s_base[threadIdx.x] = tot ? atomicAdd(&n_surv[threadIdx.x], tot) : 0u;
+      }
+      __syncthreads();
+      if (keep_c) {
+        const unsigned slot = s_base[0] + s_cnt[0][wid] + __popc(mcert & lanemask_lt());
+        __stcs(surv + slot, j);
+        __stcs(surv + cap + slot, __float_as_uint(root[0]));
+        __stcs(surv + 2 * cap + slot, __float_as_uint(root[1]));
+      }
+      if (keep_u) __stcs(surv + (cap - 1u - (s_base[1] + s_cnt[1][wid] + __popc(munc & lanemask_lt()))), j);
+      __syncthreads();
+    } else if (!more) {
+      break;
+    }
   }
-  __syncthreads();
-  if (keep_c) {
-    const unsigned slot = s_base[0] + s_cnt[0][wid] + __popc(mcert & lanemask_lt());
-    // streaming stores and loads (evict-first) for every list and queue of the path: the hierarchy and the
-    // facets (83 MB at C5) should stay in L2 while ~600 MB of lists and queues pass through it every wave
-    __stcs(surv + slot, j);
-    __stcs(surv + cap + slot, __float_as_uint(root[0]));
-    __stcs(surv + 2 * cap + slot, __float_as_uint(root[1]));
-  }
-  if (keep_u) __stcs(surv + (cap - 1u - (s_base[1] + s_cnt[1][wid] + __popc(munc & lanemask_lt()))), j);
 }
 
 // a2: seed particles of one wave in fp64, round the state to fp32 (O9), drop the rays that cannot touch the
@@ -660,6 +706,10 @@ void make_seed_const_f(const tpmc_mesh* m, const RunConst& rc, SeedConstF* sf) {
   sf->r = (float)rc.r;
   const float Rg = (float)m->Rb * (1.0f + kPrecullMargin);
   sf->Rg2 = Rg * Rg;
+  {
+    const double sg = std::min(0.999999, (double)Rg / rc.r);   // sin(theta)
+    sf->cot_g = (float)(sqrt(1.0 - sg * sg) / sg * (1.0 - 1e-6));
+  }
   static const bool no_two_level = getenv("TPMC_CULL_VOLUME") && getenv("TPMC_CULL_VOLUME")[0] == '0';   // tuning aid
   sf->n_box = no_two_level ? -1 : m->cull_nbox;
   if (sf->n_box >= 0) {
@@ -754,9 +804,9 @@ int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
   return TPMC_OK;
 }
 
-struct Grids { int trace, reflect, finish, pipes, seed; };
+struct Grids { int trace, reflect, finish, pipes, seed, precull; };
 const Grids& grids() {
-  static Grids g = {0, 0, 0, 0, 0};
+  static Grids g = {0, 0, 0, 0, 0, 0};
   if (!g.trace) {
     int dev = 0, sms = 148, per = 0;
     cudaGetDevice(&dev);
@@ -774,6 +824,8 @@ const Grids& grids() {
     g.finish = sms * per;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_seed, kSeedBlock, 0) != cudaSuccess || per < 1) per = 4;
     g.seed = sms * per;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_seed_precull, kPrecullBlock, 0) != cudaSuccess || per < 1) per = 4;
+    g.precull = sms * per * 4;   // a few shares per resident block: evens out the tail
   }
   return g;
 }
@@ -927,8 +979,8 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
         const unsigned int gfull = (wn + kSeedBlock - 1) / kSeedBlock;
         if (precull) {
           TPMC_CUDA_TRY(cudaMemsetAsync(pp.ctr + 6, 0, 2 * sizeof(unsigned int), s2));
-          k_seed_precull<<<(wn + kPrecullBlock - 1) / kPrecullBlock, kPrecullBlock, 0, s2>>>(
-              sf, rcc.seed_lo, rcc.seed_hi, rcc.first + w0, wn, cap, pp.surv, pp.ctr + 6);
+          k_seed_precull<<<std::min<unsigned int>((wn + kPrecullBlock - 1) / kPrecullBlock, (unsigned int)g.precull),
+                           kPrecullBlock, 0, s2>>>(sf, rcc.seed_lo, rcc.seed_hi, rcc.first + w0, wn, cap, pp.surv, pp.ctr + 6);
           ++launches;
         }
         k_seed<<<std::min<unsigned int>(gfull, (unsigned int)g.seed), kSeedBlock, 0, s2>>>(

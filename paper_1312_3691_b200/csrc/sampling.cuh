@@ -266,6 +266,7 @@ struct SeedConstF {
   float R[9], centre[3], r;
   float lo[3], hi[3];  // grown mesh AABB
   float Rg2;           // (grown bounding radius)^2
+  float cot_g;         // cot(theta), sin(theta) = (grown bounding radius) / r: stage-A threshold
   // two-level cull volume (k_reach_hist / k_outlier_boxes in lbvh.cu): every facet lies in the sphere of radius
   // R_in about the centre or in one of n_box boxes; both grown like the AABB.  n_box < 0: not used.
   float Rin2;
@@ -345,42 +346,72 @@ __device__ __forceinline__ float approx_normal_speed(float omu, float s, bool& o
   return x;
 }
 
-// Estimated ray of particle i (o, v in the body frame) and the fp32 roots (root[0] = S sin phi, root[1] = x_n);
-// returns false when the estimate is not certified.  No divergent branch.
-__device__ __forceinline__ bool seed_particle_approx(const SeedConstF& sf, unsigned int seed_lo, unsigned int seed_hi,
-                                                     unsigned long long i, float o[3], float v[3], float root[2]) {
+// ---- the estimate in two stages (k_seed_precull) -------------------------------------------------------------
+// Stage A stops before the normal speed: with everything else known, the ray reaches the grown bounding sphere
+// iff its inward normal speed exceeds a threshold, x_n >= x_req = cot(theta) |x_t| with sin(theta) = R_g / r, and
+// x_n = F^-1(u) is increasing in u, so that is  1 - u <= Q(x_req) / chi(s)  -- ONE evaluation of the survival
+// function of eq. (14a) instead of its inversion.  Only particles that pass (44 % at r = 1.5 R_b) go on to
+// stage B (inversion, ray, cull volumes).  A particle is dropped here only when the comparison is certain:
+// Q and chi are evaluated to ~1e-5 relative under the conditions checked below, the slack is 2e-3, and x_req is
+// taken for the sphere grown by kPrecullMargin (a 3 % shift of x_req, against ~1e-4 of estimate error).
+struct PrecullA {
+  float y, t, cphi, st, ct, xt1, xt2, s;   // S sin(phi), sin(phi), cos(phi), sin/cos(theta), tangential speeds / c, S_n
+  unsigned int w3;                          // Philox word of the normal speed
+  bool ok_t;
+};
+
+__device__ __forceinline__ bool precull_stage_a(const SeedConstF& sf, unsigned int seed_lo, unsigned int seed_hi,
+                                                unsigned long long i, PrecullA& a) {
   const uint4 b0 = philox4x32_10(seed_lo, seed_hi, (uint32_t)i, (uint32_t)(i >> 32), 0u, 0u);
   const uint4 b1 = philox4x32_10(seed_lo, seed_hi, (uint32_t)i, (uint32_t)(i >> 32), 1u, 0u);
   SpeciesF sc = sf.sp[0];
   for (int s = 1; s < sf.n_species; ++s)
     if ((unsigned long long)b0.x >= sf.sp[s - 1].thr) sc = sf.sp[s];   // cumx is non-decreasing: the last hit wins
-  bool ok_t, ok_x;
-  const float y = approx_y(u01f(b0.y), sc, ok_t);
-  const float t = fminf(1.0f, fmaxf(-1.0f, __fdividef(y, sc.S)));
-  const float cphi = sqrtf(fmaxf((1.0f - t) * (1.0f + t), 0.0f));
-  float st, ct;
-  sincospif(2.0f * u01f(b0.z), &st, &ct);
-  const float xn = approx_normal_speed(u01f(~b0.w), sc.S * t, ok_x);   // 1 - u = (~w + 1/2) 2^-32
+  a.y = approx_y(u01f(b0.y), sc, a.ok_t);
+  a.t = fminf(1.0f, fmaxf(-1.0f, __fdividef(a.y, sc.S)));
+  a.cphi = sqrtf(fmaxf((1.0f - a.t) * (1.0f + a.t), 0.0f));
+  sincospif(2.0f * u01f(b0.z), &a.st, &a.ct);
   const float rho = sqrtf(-__logf(u01f(b1.x)));
   float sa, ca;
   sincospif(2.0f * u01f(b1.y), &sa, &ca);
-  const float xt1 = fmaf(sc.S, cphi, rho * ca), xt2 = rho * sa;
-  const float xh[3] = {cphi * ct, cphi * st, t};
-  const float t1[3] = {t * ct, t * st, -cphi};
-  const float t2[3] = {-st, ct, 0.0f};
+  a.xt1 = fmaf(sc.S, a.cphi, rho * ca);
+  a.xt2 = rho * sa;
+  a.s = sc.S * a.t;
+  a.w3 = b0.w;
+  // threshold on the normal speed for the grown bounding sphere
+  const float xr = sf.cot_g * sqrtf(fmaf(a.xt1, a.xt1, a.xt2 * a.xt2));
+  const float s = a.s, z = xr - s;
+  const float e = __expf(-z * z);
+  const float q = fmaf(TPMC_SQRTPI_F * s, erfc_fast(z), e);                        // Q(x_req)
+  const float chis = fmaf(TPMC_SQRTPI_F * s, erfc_fast(-s), __expf(-s * s));       // chi(s)
+  const float omu = u01f(~b0.w);                                                   // 1 - u
+  // certain only without heavy cancellation in Q or chi (lee side) and away from under/overflow
+  const bool sure = a.ok_t && (s > -2.0f) && (q >= 1e-3f * e) && (chis > 1e-30f) && (q == q);
+  const bool miss = sure && (omu * chis > q * 1.002f + 1e-37f);
+  return !miss;
+}
+
+// Stage B: the normal speed, the estimated ray, the fp32 roots.  Returns false when the estimate is not certified.
+__device__ __forceinline__ bool precull_stage_b(const SeedConstF& sf, const PrecullA& a, float o[3], float v[3],
+                                                float root[2]) {
+  bool ok_x;
+  const float xn = approx_normal_speed(u01f(~a.w3), a.s, ok_x);
+  const float xh[3] = {a.cphi * a.ct, a.cphi * a.st, a.t};
+  const float t1[3] = {a.t * a.ct, a.t * a.st, -a.cphi};
+  const float t2[3] = {-a.st, a.ct, 0.0f};
   float vl[3];
 #pragma unroll
-  for (int k = 0; k < 3; ++k) vl[k] = fmaf(xt2, t2[k], fmaf(xt1, t1[k], -xn * xh[k]));
+  for (int k = 0; k < 3; ++k) vl[k] = fmaf(a.xt2, t2[k], fmaf(a.xt1, t1[k], -xn * xh[k]));
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
     const float rx = fmaf(sf.R[3 * k + 2], xh[2], fmaf(sf.R[3 * k + 1], xh[1], sf.R[3 * k] * xh[0]));
     const float rv = fmaf(sf.R[3 * k + 2], vl[2], fmaf(sf.R[3 * k + 1], vl[1], sf.R[3 * k] * vl[0]));
     o[k] = fmaf(sf.r, rx, sf.centre[k]);
-    v[k] = rv;                      // direction only: the speed scale c_mp does not matter for the cull
+    v[k] = rv;
   }
-  root[0] = y;
+  root[0] = a.y;
   root[1] = xn;
-  return ok_t && ok_x;
+  return a.ok_t && ok_x;
 }
 
 // Can the estimated ray touch the grown bounding sphere and the grown AABB?  (branch-free)
