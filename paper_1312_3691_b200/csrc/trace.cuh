@@ -496,11 +496,13 @@ __device__ __forceinline__ void reflect(const float4 q0, const float4 q1, const 
   Ng[2] = e1[0] * e2[1] - e1[1] * e2[0];
   const double nl = sqrt((Ng[0] * Ng[0] + Ng[1] * Ng[1]) + Ng[2] * Ng[2]);
   const double v[3] = {(double)vf[0], (double)vf[1], (double)vf[2]};
-  double ne[3] = {Ng[0] / nl, Ng[1] / nl, Ng[2] / nl};
+  const double inl = 1.0 / nl;   // one division per frame vector (the unit vectors are within 1 ulp either way)
+  double ne[3] = {Ng[0] * inl, Ng[1] * inl, Ng[2] * inl};
   const double vn = (v[0] * ne[0] + v[1] * ne[1]) + v[2] * ne[2];
   if (!(vn < 0.0)) { ne[0] = -ne[0]; ne[1] = -ne[1]; ne[2] = -ne[2]; }   // n_eff faces the incoming particle
   const double el = sqrt((e1[0] * e1[0] + e1[1] * e1[1]) + e1[2] * e1[2]);
-  const double t1[3] = {e1[0] / el, e1[1] / el, e1[2] / el};
+  const double iel = 1.0 / el;
+  const double t1[3] = {e1[0] * iel, e1[1] * iel, e1[2] * iel};
   const double t2[3] = {ne[1] * t1[2] - ne[2] * t1[1], ne[2] * t1[0] - ne[0] * t1[2], ne[0] * t1[1] - ne[1] * t1[0]};
   if (u01(w.x) < sigma) {
     // diffuse, fully accommodated: flux-weighted half-Maxwellian at T_W (A6); tangent basis A17
