@@ -319,8 +319,7 @@ __device__ __forceinline__ float approx_y(float u, const SpeciesF& sc, bool& ok)
 }
 
 // x_n = v_n / c_mp to ~1e-4 relative, ok = certified.  omu = 1 - u
-__device__ __forceinline__ float approx_normal_speed(float omu, float s, bool& ok) {
-  const float chis = fmaf(TPMC_SQRTPI_F * s, erfc_fast(-s), __expf(-s * s));
+__device__ __forceinline__ float approx_normal_speed(float omu, float s, float chis, bool& ok) {
   const float T = omu * chis;
   const float xm = 0.5f * (s + sqrtf(fmaf(s, s, 2.0f)));
   const float tau = fminf(fmaxf(__fdividef(T, TPMC_SQRTPI_F * s), 1e-30f), 1.9999f);
@@ -356,6 +355,7 @@ __device__ __forceinline__ float approx_normal_speed(float omu, float s, bool& o
 // taken for the sphere grown by kPrecullMargin (a 3 % shift of x_req, against ~1e-4 of estimate error).
 struct PrecullA {
   float y, t, cphi, st, ct, xt1, xt2, s;   // S sin(phi), sin(phi), cos(phi), sin/cos(theta), tangential speeds / c, S_n
+  float chis;                               // chi(S_n)
   unsigned int w3;                          // Philox word of the normal speed
   bool ok_t;
 };
@@ -385,6 +385,7 @@ __device__ __forceinline__ bool precull_stage_a(const SeedConstF& sf, unsigned i
   const float q = fmaf(TPMC_SQRTPI_F * s, erfc_fast(z), e);                        // Q(x_req)
   const float chis = fmaf(TPMC_SQRTPI_F * s, erfc_fast(-s), __expf(-s * s));       // chi(s)
   const float omu = u01f(~b0.w);                                                   // 1 - u
+  a.chis = chis;
   // certain only without heavy cancellation in Q or chi (lee side) and away from under/overflow
   const bool sure = a.ok_t && (s > -2.0f) && (q >= 1e-3f * e) && (chis > 1e-30f) && (q == q);
   const bool miss = sure && (omu * chis > q * 1.002f + 1e-37f);
@@ -395,7 +396,7 @@ __device__ __forceinline__ bool precull_stage_a(const SeedConstF& sf, unsigned i
 __device__ __forceinline__ bool precull_stage_b(const SeedConstF& sf, const PrecullA& a, float o[3], float v[3],
                                                 float root[2]) {
   bool ok_x;
-  const float xn = approx_normal_speed(u01f(~a.w3), a.s, ok_x);
+  const float xn = approx_normal_speed(u01f(~a.w3), a.s, a.chis, ok_x);
   const float xh[3] = {a.cphi * a.ct, a.cphi * a.st, a.t};
   const float t1[3] = {a.t * a.ct, a.t * a.st, -a.cphi};
   const float t2[3] = {-a.st, a.ct, 0.0f};
