@@ -29,8 +29,8 @@ import tpmc_inputs as ti
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one steady-state k_trace_wf launch in this launch configuration
 # (wave of 2^26 particles, ~1.3e7 rays per launch), from the `ncu --set full` capture summarised in
-# profiles/r1_ncu_full_pipeline_v5.md
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 2_810_296_320
+# profiles/r1_ncu_full_pipeline_v6.md
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 2_793_646_504
 METRIC = "particle_bounces_per_s"
 UNIT = "bounces/s"
 WORKLOAD = "C5: ~1.0e6-facet noise-displaced geodesic body + 6 panels, O/He 70/30, 900 K, 7700 m/s"
