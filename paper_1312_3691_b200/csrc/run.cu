@@ -101,6 +101,7 @@ __global__ void __launch_bounds__(kPrecullBlock) k_seed_precull(const SeedConstF
       __syncthreads();
     }
     const unsigned int n = q_n;
+    __syncthreads();   // every warp has read q_n before any warp's next stage A (or stage B) changes it
     if (n >= (unsigned)kPrecullBlock || (!more && n > 0u)) {
       const unsigned int take = min(n, (unsigned)kPrecullBlock);
       const bool active = threadIdx.x < take;
