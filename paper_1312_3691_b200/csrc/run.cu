@@ -826,7 +826,11 @@ const Grids& grids() {
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_seed, kSeedBlock, 0) != cudaSuccess || per < 1) per = 4;
     g.seed = sms * per;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_seed_precull, kPrecullBlock, 0) != cudaSuccess || per < 1) per = 4;
-    g.precull = sms * per * 4;   // a few shares per resident block: evens out the tail
+    {
+      int f = 4;   // shares per resident block (evens out the tail); TPMC_PRECULL_SHARES: tuning aid
+      if (const char* e = getenv("TPMC_PRECULL_SHARES")) f = std::max(1, std::min(64, atoi(e)));
+      g.precull = sms * per * f;
+    }
   }
   return g;
 }
