@@ -55,6 +55,14 @@ struct tpmc_mesh {
   int64_t n_nodes;
   float4* nodes;
   float4* tris;
+  // flow-aligned copy of the compact hierarchy, refitted per run (tpmc_mesh_align in lbvh.cu)
+  int2* kids;                      // [nt-1] children of every internal node (topology of the LBVH)
+  int* parent;                     // [nt-1 | nt] parent of every internal node and leaf
+  int* arrive;                     // [nt-1] refit counters
+  float* rbox;                     // [(nt-1) + nt][6] boxes in the aligned frame
+  float4* nodes_r;                 // [nt-1][4] refit output in the aligned frame
+  uint4* cnodes_r;                 // [nt-1][2] its compact form
+  double* align_R;                 // [9] rotation of the current alignment (device copy)
   uint4* cnodes;                   // compact copy of `nodes` for the wavefront traversal: 2 uint4 = 32 B per node
   float q_origin[3], q_scale[3];   // its quantisation grid: x = q_origin + q * q_scale, q in [0, 65535]
   uint4* horizon;                  // [nt] by sorted slot: escape horizon of each facet, 16 azimuth sectors x 1 byte (k_horizon, lbvh.cu)
@@ -92,6 +100,7 @@ constexpr float kPrecullMargin = 2e-2f;   // box growth of the pre-cull pass, in
 struct QuantGrid {
   float origin[3];
   float inv_scale[3];   // fp32(1 / q_scale)
+  float R[9];           // frame of the grid: x' = R x (identity for the body-frame hierarchy, see tpmc_mesh_align)
 };
 
 // Per-run constants (a1: host, fp64), passed to kernels by value.
@@ -118,6 +127,8 @@ struct RunConst {
   unsigned int seed_lo, seed_hi;
   unsigned int max_bounces;
 };
+
+int tpmc_mesh_align(tpmc_mesh* m, const double R[9], cudaStream_t st, QuantGrid* grid, const uint4** cnodes_out);
 
 #define TPMC_HD __host__ __device__ __forceinline__
 

@@ -237,6 +237,33 @@ __global__ void k_build_cull(const float4* __restrict__ nodes, const uint4* __re
   *out_count = tail;
 }
 
+// ---- flow-aligned compact hierarchy (per run) ------------------------------------------------------------------
+// An axis-aligned box shows its smallest face to a ray that runs along one of its axes and up to sqrt(3) times
+// that area to a diagonal one, and nearly all primaries of a run travel along the free stream (S = 4..8).  So
+// each run refits the boxes of the SAME tree (topology, facet order, everything by slot unchanged) in a frame
+// whose z axis is the stream direction and hands that compact copy to the wavefront traversal (44 instead of up
+// to 75 node visits per ray on C5, whatever the attitude).  Leaf boxes are the bounds of the rotated corners,
+// evaluated in fp64 and rounded outwards; the traversal rotates the ray into the same frame (walk_init).
+__global__ void k_leaf_boxes_rot(const float4* __restrict__ tris, int64_t nt, int64_t n_int, const double* __restrict__ R,
+                                 float* __restrict__ box) {
+  const int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (s >= nt) return;
+  double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+  for (int k = 0; k < 3; ++k) {
+    const float4 q = tris[3 * s + k];
+    for (int a = 0; a < 3; ++a) {
+      const double x = (R[3 * a] * (double)q.x + R[3 * a + 1] * (double)q.y) + R[3 * a + 2] * (double)q.z;
+      lo[a] = fmin(lo[a], x);
+      hi[a] = fmax(hi[a], x);
+    }
+  }
+  float* b = box + 6 * (n_int + s);
+  for (int a = 0; a < 3; ++a) {   // fp64 rounding of the rotation: 1e-15 relative, far below one fp32 ulp
+    b[a] = __double2float_rd(lo[a] - 1e-14 * fabs(lo[a]));
+    b[3 + a] = __double2float_ru(hi[a] + 1e-14 * fabs(hi[a]));
+  }
+}
+
 // ---- escape horizon of every one-sided facet (a0, read by the reflect step) ------------------------------
 // A particle re-emitted from facet f leaves a point p of f with a direction d above f's plane.  In the facet
 // frame (e1 = first edge, e2 = n x e1, n = unit normal) let sin E = d.n / |d| be its elevation and
@@ -629,7 +656,7 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
   MESH_TRY(cudaMalloc((void**)&m->nodes, sizeof(float4) * 4 * m->n_nodes));
   MESH_TRY(cudaMalloc((void**)&m->tris, sizeof(float4) * 3 * nt));
 
-  DevBuf keys, keys2, ids, ids2, tmp, box, kids, par, arr;
+  DevBuf keys, keys2, ids, ids2, tmp, box;
   const int64_t n_int = nt - 1;
   MESH_TRY(cudaMalloc(&keys.p, sizeof(uint64_t) * nt));
   MESH_TRY(cudaMalloc(&keys2.p, sizeof(uint64_t) * nt));
@@ -653,13 +680,17 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
   if (nt == 1) {
     k_single<<<1, 1, 0, st>>>(box.as<float>(), m->nodes);
   } else {
-    MESH_TRY(cudaMalloc(&kids.p, sizeof(int2) * n_int));
-    MESH_TRY(cudaMalloc(&par.p, sizeof(int) * (size_t)(n_int + nt)));
-    MESH_TRY(cudaMalloc(&arr.p, sizeof(int) * n_int));
-    MESH_TRY(cudaMemsetAsync(arr.p, 0, sizeof(int) * n_int, st));
+    MESH_TRY(cudaMalloc((void**)&m->kids, sizeof(int2) * n_int));
+    MESH_TRY(cudaMalloc((void**)&m->parent, sizeof(int) * (size_t)(n_int + nt)));
+    MESH_TRY(cudaMalloc((void**)&m->arrive, sizeof(int) * n_int));
+    MESH_TRY(cudaMalloc((void**)&m->rbox, sizeof(float) * 6 * (size_t)(n_int + nt)));
+    MESH_TRY(cudaMalloc((void**)&m->nodes_r, sizeof(float4) * 4 * n_int));
+    MESH_TRY(cudaMalloc((void**)&m->cnodes_r, sizeof(uint4) * 2 * n_int));
+    MESH_TRY(cudaMalloc((void**)&m->align_R, sizeof(double) * 9));
+    MESH_TRY(cudaMemsetAsync(m->arrive, 0, sizeof(int) * n_int, st));
     k_hierarchy<<<(unsigned)((n_int + kBlock - 1) / kBlock), kBlock, 0, st>>>(keys2.as<uint64_t>(), (int)nt,
-                                                                                kids.as<int2>(), par.as<int>());
-    k_refit<<<gt, kBlock, 0, st>>>((int)nt, kids.as<int2>(), par.as<int>(), box.as<float>(), arr.as<int>(), m->nodes);
+                                                                                m->kids, m->parent);
+    k_refit<<<gt, kBlock, 0, st>>>((int)nt, m->kids, m->parent, box.as<float>(), m->arrive, m->nodes);
   }
   {
     // quantisation grid: the vertex AABB spans steps 100 .. 65100 of each axis (flat axes get a tiny step)
@@ -707,9 +738,51 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
   return TPMC_OK;
 }
 
+
+// Refit the compact hierarchy in the frame x' = R x (row-major 3x3, orthonormal) on `stream`; fills *grid.
+// Called by tpmc_run with the stream frame of the run.  nt == 1: the body-frame hierarchy is used.
+int tpmc_mesh_align(tpmc_mesh* m, const double R[9], cudaStream_t st, QuantGrid* grid, const uint4** cnodes_out) {
+  for (int k = 0; k < 9; ++k) grid->R[k] = (k % 4 == 0) ? 1.0f : 0.0f;
+  for (int a = 0; a < 3; ++a) { grid->origin[a] = m->q_origin[a]; grid->inv_scale[a] = (float)(1.0 / (double)m->q_scale[a]); }
+  *cnodes_out = m->cnodes;
+  if (m->nt < 2 || !m->kids) return TPMC_OK;
+  // bounds of the rotated body: box of the rotated corners of its AABB (a superset; costs < sqrt(3) in grid resolution)
+  double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+  for (int c = 0; c < 8; ++c) {
+    const double x[3] = {(c & 1) ? m->aabb_hi[0] : m->aabb_lo[0], (c & 2) ? m->aabb_hi[1] : m->aabb_lo[1],
+                         (c & 4) ? m->aabb_hi[2] : m->aabb_lo[2]};
+    for (int a = 0; a < 3; ++a) {
+      const double y = R[3 * a] * x[0] + R[3 * a + 1] * x[1] + R[3 * a + 2] * x[2];
+      lo[a] = std::min(lo[a], y);
+      hi[a] = std::max(hi[a], y);
+    }
+  }
+  double emax = 0.0;
+  for (int a = 0; a < 3; ++a) emax = std::max(emax, hi[a] - lo[a]);
+  float qs[3], qo[3];
+  for (int a = 0; a < 3; ++a) {
+    qs[a] = (float)(std::max(hi[a] - lo[a], std::max(1e-6 * emax, 1e-30)) / 65000.0);
+    qo[a] = (float)(lo[a] - 100.0 * (double)qs[a]);
+  }
+  const int64_t nt = m->nt, n_int = nt - 1;
+  const unsigned gt = (unsigned)((nt + kBlock - 1) / kBlock);
+  TPMC_CUDA_TRY(cudaMemcpyAsync(m->align_R, R, 9 * sizeof(double), cudaMemcpyHostToDevice, st));
+  TPMC_CUDA_TRY(cudaMemsetAsync(m->arrive, 0, sizeof(int) * n_int, st));
+  k_leaf_boxes_rot<<<gt, kBlock, 0, st>>>(m->tris, nt, n_int, m->align_R, m->rbox);
+  k_refit<<<gt, kBlock, 0, st>>>((int)nt, m->kids, m->parent, m->rbox, m->arrive, m->nodes_r);
+  k_compact_nodes<<<(unsigned)((n_int + kBlock - 1) / kBlock), kBlock, 0, st>>>(m->nodes_r, n_int, (double)qo[0], (double)qo[1],
+                                                                                (double)qo[2], (double)qs[0], (double)qs[1],
+                                                                                (double)qs[2], m->cnodes_r);
+  TPMC_CUDA_TRY(cudaGetLastError());
+  for (int k = 0; k < 9; ++k) grid->R[k] = (float)R[k];
+  for (int a = 0; a < 3; ++a) { grid->origin[a] = qo[a]; grid->inv_scale[a] = (float)(1.0 / (double)qs[a]); }
+  *cnodes_out = m->cnodes_r;
+  return TPMC_OK;
+}
+
 extern "C" void tpmc_mesh_destroy(tpmc_mesh* m) {
   if (!m) return;
-  cudaFree(m->nodes); cudaFree(m->tris); cudaFree(m->cull_c); cudaFree(m->cnodes); cudaFree(m->horizon);
+  cudaFree(m->nodes); cudaFree(m->tris); cudaFree(m->cull_c); cudaFree(m->kids); cudaFree(m->parent); cudaFree(m->arrive); cudaFree(m->rbox); cudaFree(m->nodes_r); cudaFree(m->cnodes_r); cudaFree(m->align_R); cudaFree(m->cnodes); cudaFree(m->horizon);
   for (int pi = 0; pi < kPipes; ++pi) {
     Pipe& pp = m->pipe[pi];
     for (int k = 0; k < 2; ++k) { cudaFree(pp.q_o[k]); cudaFree(pp.q_v[k]); cudaFree(pp.q_f[k]); }

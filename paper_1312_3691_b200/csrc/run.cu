@@ -734,9 +734,10 @@ TraceTune trace_tune() {
   return t;
 }
 
-QuantGrid quant_grid(const tpmc_mesh* m) {
+QuantGrid quant_grid(const tpmc_mesh* m) {   // the body-frame hierarchy
   QuantGrid g;
   for (int a = 0; a < 3; ++a) { g.origin[a] = m->q_origin[a]; g.inv_scale[a] = (float)(1.0 / (double)m->q_scale[a]); }
+  for (int k = 0; k < 9; ++k) g.R[k] = (k % 4 == 0) ? 1.0f : 0.0f;
   return g;
 }
 
@@ -918,7 +919,21 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
   const int seed_walk = sw_env ? (sw_env[0] != '0') : (m->cull_nbox < 0 || (getenv("TPMC_CULL_VOLUME") && getenv("TPMC_CULL_VOLUME")[0] == '0'));
   SeedConstF sf;
   make_seed_const_f(m, rc, &sf);
-  const QuantGrid qg = quant_grid(m);
+  const QuantGrid qg = quant_grid(m);   // seed-time cull (body frame)
+  TPMC_CUDA_TRY(cudaEventRecord(m->ev0, st));
+  // the traversal's hierarchy, refitted in the stream frame of this run (x' = R^T x: z' along the free stream)
+  QuantGrid qg_t = qg;
+  const uint4* cnodes_t = m->cnodes;
+  {
+    static const bool no_align = getenv("TPMC_ALIGN") && getenv("TPMC_ALIGN")[0] == '0';   // tuning aid
+    if (!no_align) {
+      double Rt[9];
+      for (int a = 0; a < 3; ++a)
+        for (int b2 = 0; b2 < 3; ++b2) Rt[3 * a + b2] = rc.R[3 * b2 + a];
+      rcode = tpmc_mesh_align(m, Rt, st, &qg_t, &cnodes_t);
+      if (rcode != TPMC_OK) return rcode;
+    }
+  }
   m->pipe[0].main = st;
   for (int pi = 0; pi < kPipes; ++pi) {
     Pipe& pp = m->pipe[pi];
@@ -930,7 +945,6 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
     }
   }
 
-  TPMC_CUDA_TRY(cudaEventRecord(m->ev0, st));
   TPMC_CUDA_TRY(cudaMemsetAsync(P, 0, 3 * sizeof(double) * (size_t)m->nt, st));
   TPMC_CUDA_TRY(cudaMemsetAsync(m->stats, 0, ST_COUNT * sizeof(unsigned long long), st));
   TPMC_CUDA_TRY(cudaMemsetAsync(m->totals, 0, 4 * sizeof(double), st));
@@ -1000,7 +1014,7 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
       TPMC_CUDA_TRY(cudaEventRecord(pp.ev_reset[(li + 1) & 3], s1));
       if (wv < n_waves) TPMC_CUDA_TRY(cudaStreamWaitEvent(s1, pp.ev_seeded[li & 3], 0));
       if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[2], s1));
-      k_trace_wf<<<g.trace, kTraceBlock, 0, s1>>>(m->cnodes, qg, m->tris, Q[p], cap, pp.ctr + 2 * p, pp.ctr + 4, pp.hit_ray,
+      k_trace_wf<<<g.trace, kTraceBlock, 0, s1>>>(cnodes_t, qg_t, m->tris, Q[p], cap, pp.ctr + 2 * p, pp.ctr + 4, pp.hit_ray,
                                                   pp.hit_cand, pp.ctr + 5, m->stats, trace_tune());
       if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[3], s1));
       // the straggler kernel of the previous iteration reads the queue this reflect step writes

@@ -186,7 +186,8 @@ __device__ __forceinline__ bool slab(float lx, float ly, float lz, float hx, flo
 //   * id = 1/d' carries <= 5u relative (rounded inv_scale, product, 2-ulp reciprocal), which scales the
 //     distance |P - O| <= |o'| + 2^16 steps; the final FFMA rounds once more, u relative;
 //   * the rounded inv_scale moves a plane by <= u q <= 0.004 steps.
-// Sum <= 2u|O| + 9u|o'| + 0.03; G_k = 2.5u|O| + 10u|o'| + 0.1 (about 1.4 steps of the 16-bit grid for an origin
+// Sum <= 2u|O| + 9u|o'| + 0.03 (+ 0.06 for the rotation into an aligned frame, see grid_ray);
+// G_k = 2.5u|O| + 10u|o'| + 0.25 (about 1.5 steps of the 16-bit grid for an origin
 // inside or near the grid; it scales with the origin for a ray that starts far outside, e.g. on a flat axis).
 // A zero direction component gives id = inf and NaN plane distances, which fminf/fmaxf drop: the axis then
 // does not constrain the ray (conservative).
@@ -208,13 +209,23 @@ struct GridRay {
   unsigned int sn[3], sf[3];
 };
 __device__ __forceinline__ void grid_ray(GridRay& r, const QuantGrid& g, const float o[3], const float d[3]) {
+  // into the frame of the grid (x' = R x; R = identity for the body-frame hierarchy, where this is exact).  The
+  // rotation adds an absolute error of <= 3u (|o|_1, |d|_1) to o' and d'.  For o' that is < 0.02 grid steps.  For d'
+  // it displaces the ray, over its whole path through the grid (< 1.2e5 steps), by < 3u * 1.2e5 * sqrt(3) = 0.04
+  // steps along any axis, however small that component of d' is.  Both are in the constant part of G below.
+  float og[3], dg[3];
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
-    const float dq = d[k] * g.inv_scale[k];
+    og[k] = fmaf(g.R[3 * k + 2], o[2], fmaf(g.R[3 * k + 1], o[1], g.R[3 * k] * o[0]));
+    dg[k] = fmaf(g.R[3 * k + 2], d[2], fmaf(g.R[3 * k + 1], d[1], g.R[3 * k] * d[0]));
+  }
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const float dq = dg[k] * g.inv_scale[k];
     const float idk = __fdividef(1.0f, dq);                  // 2 ulp
-    const float oq = (o[k] - g.origin[k]) * g.inv_scale[k];
+    const float oq = (og[k] - g.origin[k]) * g.inv_scale[k];
     const float O = 8388608.0f + oq;
-    const float G = fmaf(1.4901161e-07f, fabsf(O), fmaf(5.9604645e-07f, fabsf(oq), 0.1f));   // 2.5u|O| + 10u|o'| + 0.1
+    const float G = fmaf(1.4901161e-07f, fabsf(O), fmaf(5.9604645e-07f, fabsf(oq), 0.25f));   // 2.5u|O| + 10u|o'| + 0.25
     const float mg = G * fabsf(idk);
     r.id[k] = idk;
     r.ncn[k] = fmaf(-O, idk, -mg);
