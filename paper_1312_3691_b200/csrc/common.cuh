@@ -50,6 +50,7 @@ struct Pipe {
 // ---------------------------------------------------------------------------------------------
 // Device-resident body.  nodes: 4 float4 per internal node (two child boxes + two child refs);
 // tris: 3 float4 per triangle in Morton order: (p0, facet id), (p1, flags), (p2, 0).
+struct QuantGrid;
 struct tpmc_mesh {
   int64_t nv, nt;
   int64_t n_nodes;
@@ -62,7 +63,8 @@ struct tpmc_mesh {
   float* rbox;                     // [(nt-1) + nt][6] boxes in the aligned frame
   float4* nodes_r;                 // [nt-1][4] refit output in the aligned frame
   uint4* cnodes_r;                 // [nt-1][2] its compact form
-  double* align_R;                 // [9] rotation of the current alignment (device copy)
+  double* align_R;                 // [9] rotation of the current alignment, [6] its grid origin and scale (device)
+  QuantGrid* grid_dev;             // [2] device copies of the grids the traversal reads: body frame, aligned
   uint4* cnodes;                   // compact copy of `nodes` for the wavefront traversal: 2 uint4 = 32 B per node
   float q_origin[3], q_scale[3];   // its quantisation grid: x = q_origin + q * q_scale, q in [0, 65535]
   uint4* horizon;                  // [nt] by sorted slot: escape horizon of each facet, 16 azimuth sectors x 1 byte (k_horizon, lbvh.cu)
@@ -128,7 +130,7 @@ struct RunConst {
   unsigned int max_bounces;
 };
 
-int tpmc_mesh_align(tpmc_mesh* m, const double R[9], cudaStream_t st, QuantGrid* grid, const uint4** cnodes_out);
+int tpmc_mesh_align(tpmc_mesh* m, const double R[9], cudaStream_t st, const QuantGrid** grid_out, const uint4** cnodes_out);
 
 #define TPMC_HD __host__ __device__ __forceinline__
 

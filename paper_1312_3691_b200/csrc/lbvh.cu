@@ -192,9 +192,11 @@ __global__ void k_single(const float* __restrict__ box_leaf, float4* __restrict_
 // (The quotient is evaluated in fp64: a box corner within 1e-11 steps of a grid plane may land on the wrong
 // side of it, which the slack of the traversal's margin G covers.)
 __global__ void k_compact_nodes(const float4* __restrict__ nodes, int64_t n_nodes, double ox, double oy, double oz,
-                                double sx, double sy, double sz, uint4* __restrict__ cnodes) {
+                                double sx, double sy, double sz, uint4* __restrict__ cnodes,
+                                const double* __restrict__ dev_grid = nullptr) {
   const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n_nodes) return;
+  if (dev_grid) { ox = dev_grid[0]; oy = dev_grid[1]; oz = dev_grid[2]; sx = dev_grid[3]; sy = dev_grid[4]; sz = dev_grid[5]; }
   const float4 n0 = nodes[4 * i], n1 = nodes[4 * i + 1], n2 = nodes[4 * i + 2], n3 = nodes[4 * i + 3];
   const float lo[2][3] = {{n0.x, n0.y, n0.z}, {n1.z, n1.w, n2.x}};
   const float hi[2][3] = {{n0.w, n1.x, n1.y}, {n2.y, n2.z, n2.w}};
@@ -262,6 +264,24 @@ __global__ void k_leaf_boxes_rot(const float4* __restrict__ tris, int64_t nt, in
     b[a] = __double2float_rd(lo[a] - 1e-14 * fabs(lo[a]));
     b[3 + a] = __double2float_ru(hi[a] + 1e-14 * fabs(hi[a]));
   }
+}
+
+// Quantisation grid of the aligned hierarchy from the root box of the refit (device side: no host round trip).
+// out_d: origin xyz, scale xyz (fp32 values held as doubles, for k_compact_nodes); out_g: what the traversal reads.
+__global__ void k_align_grid(const float* __restrict__ root_box, const double* __restrict__ R, double* __restrict__ out_d,
+                             QuantGrid* __restrict__ out_g) {
+  if (blockIdx.x != 0 || threadIdx.x != 0) return;
+  double ext[3], emax = 0.0;
+  for (int a = 0; a < 3; ++a) { ext[a] = (double)root_box[3 + a] - (double)root_box[a]; emax = fmax(emax, ext[a]); }
+  for (int a = 0; a < 3; ++a) {
+    const float qs = (float)(fmax(ext[a], fmax(1e-6 * emax, 1e-30)) / 65000.0);
+    const float qo = (float)((double)root_box[a] - 100.0 * (double)qs);
+    out_d[a] = (double)qo;
+    out_d[3 + a] = (double)qs;
+    out_g->origin[a] = qo;
+    out_g->inv_scale[a] = (float)(1.0 / (double)qs);
+  }
+  for (int k = 0; k < 9; ++k) out_g->R[k] = (float)R[k];
 }
 
 // ---- escape horizon of every one-sided facet (a0, read by the reflect step) ------------------------------
@@ -686,7 +706,7 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
     MESH_TRY(cudaMalloc((void**)&m->rbox, sizeof(float) * 6 * (size_t)(n_int + nt)));
     MESH_TRY(cudaMalloc((void**)&m->nodes_r, sizeof(float4) * 4 * n_int));
     MESH_TRY(cudaMalloc((void**)&m->cnodes_r, sizeof(uint4) * 2 * n_int));
-    MESH_TRY(cudaMalloc((void**)&m->align_R, sizeof(double) * 9));
+    MESH_TRY(cudaMalloc((void**)&m->align_R, sizeof(double) * 16));
     MESH_TRY(cudaMemsetAsync(m->arrive, 0, sizeof(int) * n_int, st));
     k_hierarchy<<<(unsigned)((n_int + kBlock - 1) / kBlock), kBlock, 0, st>>>(keys2.as<uint64_t>(), (int)nt,
                                                                                 m->kids, m->parent);
@@ -704,6 +724,12 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
     k_compact_nodes<<<(unsigned)((m->n_nodes + kBlock - 1) / kBlock), kBlock, 0, st>>>(
         m->nodes, m->n_nodes, (double)m->q_origin[0], (double)m->q_origin[1], (double)m->q_origin[2],
         (double)m->q_scale[0], (double)m->q_scale[1], (double)m->q_scale[2], m->cnodes);
+    QuantGrid hg;
+    for (int a = 0; a < 3; ++a) { hg.origin[a] = m->q_origin[a]; hg.inv_scale[a] = (float)(1.0 / (double)m->q_scale[a]); }
+    for (int k = 0; k < 9; ++k) hg.R[k] = (k % 4 == 0) ? 1.0f : 0.0f;
+    MESH_TRY(cudaMalloc((void**)&m->grid_dev, 2 * sizeof(QuantGrid)));
+    MESH_TRY(cudaMemcpyAsync(m->grid_dev, &hg, sizeof(hg), cudaMemcpyHostToDevice, st));
+    MESH_TRY(cudaMemcpyAsync(m->grid_dev + 1, &hg, sizeof(hg), cudaMemcpyHostToDevice, st));
   }
   DevBuf cq;
   MESH_TRY(cudaMalloc((void**)&m->cull_c, sizeof(uint4) * 2 * kCullNodes));
@@ -741,48 +767,28 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
 
 // Refit the compact hierarchy in the frame x' = R x (row-major 3x3, orthonormal) on `stream`; fills *grid.
 // Called by tpmc_run with the stream frame of the run.  nt == 1: the body-frame hierarchy is used.
-int tpmc_mesh_align(tpmc_mesh* m, const double R[9], cudaStream_t st, QuantGrid* grid, const uint4** cnodes_out) {
-  for (int k = 0; k < 9; ++k) grid->R[k] = (k % 4 == 0) ? 1.0f : 0.0f;
-  for (int a = 0; a < 3; ++a) { grid->origin[a] = m->q_origin[a]; grid->inv_scale[a] = (float)(1.0 / (double)m->q_scale[a]); }
+int tpmc_mesh_align(tpmc_mesh* m, const double R[9], cudaStream_t st, const QuantGrid** grid_out, const uint4** cnodes_out) {
+  *grid_out = m->grid_dev;   // [0]: the body-frame grid, [1]: the aligned one
   *cnodes_out = m->cnodes;
   if (m->nt < 2 || !m->kids) return TPMC_OK;
-  // bounds of the rotated body: box of the rotated corners of its AABB (a superset; costs < sqrt(3) in grid resolution)
-  double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
-  for (int c = 0; c < 8; ++c) {
-    const double x[3] = {(c & 1) ? m->aabb_hi[0] : m->aabb_lo[0], (c & 2) ? m->aabb_hi[1] : m->aabb_lo[1],
-                         (c & 4) ? m->aabb_hi[2] : m->aabb_lo[2]};
-    for (int a = 0; a < 3; ++a) {
-      const double y = R[3 * a] * x[0] + R[3 * a + 1] * x[1] + R[3 * a + 2] * x[2];
-      lo[a] = std::min(lo[a], y);
-      hi[a] = std::max(hi[a], y);
-    }
-  }
-  double emax = 0.0;
-  for (int a = 0; a < 3; ++a) emax = std::max(emax, hi[a] - lo[a]);
-  float qs[3], qo[3];
-  for (int a = 0; a < 3; ++a) {
-    qs[a] = (float)(std::max(hi[a] - lo[a], std::max(1e-6 * emax, 1e-30)) / 65000.0);
-    qo[a] = (float)(lo[a] - 100.0 * (double)qs[a]);
-  }
   const int64_t nt = m->nt, n_int = nt - 1;
   const unsigned gt = (unsigned)((nt + kBlock - 1) / kBlock);
   TPMC_CUDA_TRY(cudaMemcpyAsync(m->align_R, R, 9 * sizeof(double), cudaMemcpyHostToDevice, st));
   TPMC_CUDA_TRY(cudaMemsetAsync(m->arrive, 0, sizeof(int) * n_int, st));
   k_leaf_boxes_rot<<<gt, kBlock, 0, st>>>(m->tris, nt, n_int, m->align_R, m->rbox);
   k_refit<<<gt, kBlock, 0, st>>>((int)nt, m->kids, m->parent, m->rbox, m->arrive, m->nodes_r);
-  k_compact_nodes<<<(unsigned)((n_int + kBlock - 1) / kBlock), kBlock, 0, st>>>(m->nodes_r, n_int, (double)qo[0], (double)qo[1],
-                                                                                (double)qo[2], (double)qs[0], (double)qs[1],
-                                                                                (double)qs[2], m->cnodes_r);
+  k_align_grid<<<1, 32, 0, st>>>(m->rbox, m->align_R, m->align_R + 9, m->grid_dev + 1);
+  k_compact_nodes<<<(unsigned)((n_int + kBlock - 1) / kBlock), kBlock, 0, st>>>(m->nodes_r, n_int, 0, 0, 0, 1, 1, 1, m->cnodes_r,
+                                                                                m->align_R + 9);
   TPMC_CUDA_TRY(cudaGetLastError());
-  for (int k = 0; k < 9; ++k) grid->R[k] = (float)R[k];
-  for (int a = 0; a < 3; ++a) { grid->origin[a] = qo[a]; grid->inv_scale[a] = (float)(1.0 / (double)qs[a]); }
   *cnodes_out = m->cnodes_r;
+  *grid_out = m->grid_dev + 1;
   return TPMC_OK;
 }
 
 extern "C" void tpmc_mesh_destroy(tpmc_mesh* m) {
   if (!m) return;
-  cudaFree(m->nodes); cudaFree(m->tris); cudaFree(m->cull_c); cudaFree(m->kids); cudaFree(m->parent); cudaFree(m->arrive); cudaFree(m->rbox); cudaFree(m->nodes_r); cudaFree(m->cnodes_r); cudaFree(m->align_R); cudaFree(m->cnodes); cudaFree(m->horizon);
+  cudaFree(m->nodes); cudaFree(m->tris); cudaFree(m->cull_c); cudaFree(m->kids); cudaFree(m->parent); cudaFree(m->arrive); cudaFree(m->rbox); cudaFree(m->nodes_r); cudaFree(m->cnodes_r); cudaFree(m->align_R); cudaFree(m->grid_dev); cudaFree(m->cnodes); cudaFree(m->horizon);
   for (int pi = 0; pi < kPipes; ++pi) {
     Pipe& pp = m->pipe[pi];
     for (int k = 0; k < 2; ++k) { cudaFree(pp.q_o[k]); cudaFree(pp.q_v[k]); cudaFree(pp.q_f[k]); }

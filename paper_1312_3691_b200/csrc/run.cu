@@ -218,7 +218,7 @@ struct TraceTune { int node_min, refill_idle; };
 constexpr int kFetchChunk = 64;   // rays a warp reserves per atomic on the queue head
 
 __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf(const uint4* __restrict__ cnodes,
-                                                             const QuantGrid grid,
+                                                             const QuantGrid* __restrict__ gridp,
                                                              const float4* __restrict__ tris, const RayQueue q,
                                                              unsigned int cap, const unsigned int* __restrict__ n_rays,
                                                              unsigned int* __restrict__ next_ray,
@@ -260,7 +260,7 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
           r = pool_next + rank;
           if (r < n) {
             r = (r < na) ? r : cap + (r - na);   // physical slot
-            walk_init(w, grid, __ldcs(q.o + r), __ldcs(q.v + r), __ldcs(q.f + r));
+            walk_init(w, *gridp, __ldcs(q.o + r), __ldcs(q.v + r), __ldcs(q.f + r));
             has = true;
           }
         }
@@ -922,11 +922,17 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
   const QuantGrid qg = quant_grid(m);   // seed-time cull (body frame)
   TPMC_CUDA_TRY(cudaEventRecord(m->ev0, st));
   // the traversal's hierarchy, refitted in the stream frame of this run (x' = R^T x: z' along the free stream)
-  QuantGrid qg_t = qg;
+  const QuantGrid* qg_t = m->grid_dev;
   const uint4* cnodes_t = m->cnodes;
   {
     static const bool no_align = getenv("TPMC_ALIGN") && getenv("TPMC_ALIGN")[0] == '0';   // tuning aid
-    if (!no_align) {
+    // Heuristic: bodies are usually modelled along their own axes (thin panels, flat faces), and a box refitted in a
+    // tilted frame is loose around such parts; with the stream within ~25 deg of a body axis the body-frame boxes
+    // are as good or better (measured on C5), so the refit is used only for the oblique attitudes.
+    const double vmax = std::max(std::fabs(params->V[0]), std::max(std::fabs(params->V[1]), std::fabs(params->V[2])));
+    const double vabs = std::sqrt(params->V[0] * params->V[0] + params->V[1] * params->V[1] + params->V[2] * params->V[2]);
+    static const bool force_align = getenv("TPMC_ALIGN") && getenv("TPMC_ALIGN")[0] == '2';
+    if (!no_align && (force_align || (vabs > 0.0 && vmax < 0.9 * vabs))) {
       double Rt[9];
       for (int a = 0; a < 3; ++a)
         for (int b2 = 0; b2 < 3; ++b2) Rt[3 * a + b2] = rc.R[3 * b2 + a];
@@ -1130,7 +1136,7 @@ extern "C" int tpmc_trace(const tpmc_mesh* mesh, const float* d_o, const float* 
   TPMC_CUDA_TRY(cudaMemsetAsync(m->stats, 0, ST_COUNT * sizeof(unsigned long long), st));
   k_pack_rays<<<(un + 255) / 256, 256, 0, st>>>(d_o, d_d, d_f_prev, un, q, d_facet, d_tau);
   // the production traversal (fp32 wavefront + candidate lists), then the exact fp64 resolve
-  k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(m->cnodes, quant_grid(m), m->tris, q, (unsigned int)(2 * m->wave_cap), pp.ctr, pp.ctr + 4,
+  k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(m->cnodes, m->grid_dev, m->tris, q, (unsigned int)(2 * m->wave_cap), pp.ctr, pp.ctr + 4,
                                               pp.hit_ray, pp.hit_cand, pp.ctr + 5, m->stats, trace_tune());
   k_resolve_only<<<g.reflect, kTraceBlock, 0, st>>>(m->nodes, m->tris, q, pp.hit_ray, pp.hit_cand, pp.ctr + 5, d_facet,
                                                     d_tau);
