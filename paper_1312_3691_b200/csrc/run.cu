@@ -956,7 +956,7 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
   TPMC_CUDA_TRY(cudaMemsetAsync(m->totals, 0, 4 * sizeof(double), st));
   if (any_dbg && params->count)
     k_init_debug<<<(unsigned)((params->count + 255) / 256), 256, 0, st>>>(dbg0, params->count);
-  unsigned long long launches = (any_dbg && params->count) ? 1 : 0;
+  unsigned long long launches = ((any_dbg && params->count) ? 1 : 0) + (cnodes_t != m->cnodes ? 4 : 0);   // + the refit kernels
 
   // Particle indices inside the queues are 32-bit offsets into a chunk of the slice.
   const unsigned long long kChunk = 0xF0000000ull;
