@@ -17,7 +17,9 @@
  * hit fraction (R/r)^2 (P5), facet counts (P6), convex-body force = panel sum (P7),
  * Sentman / sphere / cylinder closed forms (P8), symmetry (P9), equilibrium (P10),
  * control-volume invariance and rotation covariance (P11), BVH == brute force (P12),
- * specular limits (P13).  No function here is "parity unpinned".
+ * specular limits (P13), Pratt's concave hemisphere (P14), torque about an off-centre
+ * reference point = panel sum of (centroid - x_ref) x F_f, and the A14 shift identity (P16).
+ * No function here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>

@@ -389,3 +389,59 @@ def test_p14_concave_hemisphere_approaches_pratt():
     # the thermal excess over the hyperthermal asymptote shrinks with S
     assert dev[10.0][0] > dev[40.0][0] - 4 * (dev[10.0][1] + dev[40.0][1])
     assert dev[10.0][0] > 0.0
+
+
+# ------------------------------------------------------------------ O12 / A14: torque and its reference point
+def _batched_torque(om, cfg, nb=8):
+    """Force and torque of the whole stream with the standard error of the torque from nb disjoint slices."""
+    per = cfg.N // nb
+    rs = [om.run(cfg, first=k * per, count=per, debug=False, facets=False) for k in range(nb)]
+    Ts = np.array([r.torque for r in rs])
+    Fs = np.array([r.force for r in rs])
+    return Fs.sum(0), Ts.sum(0), Ts.std(0, ddof=1) * np.sqrt(nb)
+
+
+@pytest.mark.parametrize("body", ["sphere", "plate"])
+def test_p16_torque_about_an_off_centre_point_vs_panel_sum(body):
+    """O12: tau = sum (p - x_ref) x dp with p the HIT point (moments about a reference point).  On a
+    convex mesh every facet sees a uniform incident flux and a uniform re-emission, so the expected torque is
+    sum_f (centroid_f - x_ref) x F_f with F_f the panel force of the facet -- non-zero here because x_ref is off
+    the line of action.  A swapped cross product, the segment origin in place of the hit point, or an ignored
+    x_ref all move the result by many sigma."""
+    x_ref = np.array([0.3, -0.2, 0.5])
+    if body == "sphere":
+        m = ti.geodesic_sphere(4)
+        cfg = ti.RunConfig("tq", None, T_inf=1200.0, V=(-5200.0, 3100.0, -4300.0), N=160_000, seed=21,
+                           x_ref=tuple(x_ref))
+    else:
+        m = ti.plate(30.0)               # two-sided canted plate; reference point like a quarter-chord point, off the plate
+        cfg = ti.config("C1")[0].with_(N=240_000, seed=22, x_ref=tuple(x_ref))
+    om = omesh(m)
+    F, Tq, seT = _batched_torque(om, cfg)
+    up = -np.array(cfg.V) / cfg.speed
+    S = cfg.speed / cf.thermal_speed(cfg.T_inf, cfg.m[0])
+    SW = cfg.speed / cf.thermal_speed(cfg.T_W, cfg.m[0])
+    _, _, Fpf = cf.panel_sum(m.triangles(), m.flags, up, S, SW)
+    cen = m.triangles().mean(1)
+    want = np.cross(cen - x_ref, Fpf * cfg.q_inf).sum(0)
+    assert np.all(np.abs(Tq - want) < 4 * seT), (Tq, want, seT)
+    assert np.linalg.norm(want) > 30 * np.linalg.norm(seT)          # the pin has teeth: the expected torque is far from 0
+    # the mistakes it must catch, each evaluated from the same expectation
+    assert np.linalg.norm(-want - Tq) > 8 * np.linalg.norm(seT)                                   # dp x r
+    about_origin = np.cross(cen, Fpf * cfg.q_inf).sum(0)
+    assert np.linalg.norm(about_origin - Tq) > 8 * np.linalg.norm(seT)                            # x_ref ignored
+
+
+def test_a14_moving_the_reference_point():
+    """A14: tau(x_ref + dx) = tau(x_ref) - dx x F on the same particle stream, to rounding; per-facet momentum and
+    force do not depend on x_ref."""
+    m = ti.satellite(seed=2, h=0.25)
+    om = omesh(m)
+    base = ti.RunConfig("a14", None, T_inf=900.0, V=(-4000.0, 1500.0, -6000.0), N=40_000, seed=23)
+    a = om.run(base)
+    dx = np.array([0.7, -1.1, 0.4])
+    b = om.run(base.with_(x_ref=tuple(dx)))
+    assert np.array_equal(a.force, b.force) and np.array_equal(a.facet_momentum, b.facet_momentum)
+    scale = np.linalg.norm(dx) * np.linalg.norm(a.force) + np.linalg.norm(a.torque)
+    assert np.linalg.norm(b.torque - (a.torque - np.cross(dx, a.force))) <= 1e-11 * scale
+    assert np.linalg.norm(np.cross(dx, a.force)) > 1e-3 * scale       # the shift is not a no-op
