@@ -12,7 +12,10 @@
  *   - "host"/"device" says where a pointer must live.  The library never frees caller buffers.
  *   - work is enqueued on the caller's CUDA stream (cudaStream_t passed as void*, NULL = default
  *     stream); device outputs are valid once the caller has synchronised that stream.
- *   - one tpmc_run at a time per mesh handle (the handle caches per-run scratch).
+ *   - a mesh handle caches per-run scratch (ray queues, lists, counters, the flow-aligned copy of the
+ *     hierarchy): tpmc_run / tpmc_run_host / tpmc_trace take it non-const, and all calls on one handle must
+ *     be ordered on ONE stream (or separated by a synchronisation); two handles are independent.
+ *   - behaviour is selected by the parameter struct only; the library reads no environment variable.
  *   - there is no CPU fallback: without a CUDA device every compute call returns TPMC_ECUDA.
  */
 #ifndef TPMC_H
@@ -34,6 +37,21 @@ extern "C" {
 
 #define TPMC_MAX_SPECIES 8
 #define TPMC_FACET_TWO_SIDED 1u /* facet_flags bit0 */
+#define TPMC_MAX_BOUNCES 0x0FFFFFFFu /* largest max_bounces (the bounce count shares a word with the species) */
+
+/* tpmc_params.flags.  The first five switch off (or force) steps that must not change any result -- the parity
+ * tests run with and without them; the library's defaults are all zero. */
+#define TPMC_FLAG_NO_PRECULL 0x01u  /* every particle through the fp64 sampler (no fp32 pre-cull pass) */
+#define TPMC_FLAG_NO_HORIZON 0x02u  /* every re-emitted ray is traced (no escape-horizon test) */
+#define TPMC_FLAG_ALIGN_OFF 0x04u   /* traversal on the body-frame hierarchy, whatever the attitude */
+#define TPMC_FLAG_ALIGN_ON 0x08u    /* traversal on the flow-aligned refit, whatever the attitude */
+#define TPMC_FLAG_EXACT_TRACE 0x10u /* every segment by the fp64 closest-hit search (no fp32 filter, no candidate lists) */
+#define TPMC_FLAG_NO_SORT 0x20u     /* rays traced in queue order (no spatial sort before the traversal) */
+
+/* tpmc_params.control_volume */
+#define TPMC_CV_SPHERE 0 /* the paper's scheme: spherical control volume, eqs. (10)-(15) */
+#define TPMC_CV_BOX 1    /* rectangular control volume, flux-weighted per face: cross-check */
+#define TPMC_CV_BOX_UNWEIGHTED 2 /* the same with the inward speed drawn WITHOUT flux weighting: negative control */
 
 /* Opaque triangulated body + its on-device LBVH ("Satellite surfaces are represented by a
  * triangulation, allowing the use of well-known ray-tracing methods").  Owns its device memory. */
@@ -62,16 +80,26 @@ typedef struct {
   uint64_t N;              /* particles of the whole stream; the particle weight is m Gamma / N */
   uint64_t first, count;   /* run only particles [first, first+count) of that stream (slices, multi-GPU) */
   uint64_t seed;           /* Philox4x32-10 key; counter = (particle index, block) (O3) */
-  uint32_t max_bounces;    /* cap on reflections per particle (>=1); cut-off particles are counted (A13) */
+  uint32_t max_bounces;    /* cap on reflections per particle, 1..TPMC_MAX_BOUNCES; cut-off particles are counted (A13) */
   double x_ref[3];         /* torque reference point, body frame (A14) */
+  double energy_accommodation; /* alpha_E in [0,1]: re-emission temperature T_r = alpha_E T_W + (1 - alpha_E) T_k,i with
+                              T_k,i = m v_in^2 / (3 k_B) (reading A22); 1.0 = the paper's full accommodation */
+  uint64_t wave_particles; /* particles seeded per pipeline iteration; 0 = default (2^26).  Results do not depend on it */
+  uint64_t chunk_particles;/* particles per 32-bit index chunk; 0 = default (0xF0000000).  Results do not depend on it */
+  uint32_t flags;          /* TPMC_FLAG_* */
+  int32_t control_volume;  /* TPMC_CV_* */
 } tpmc_params;
 
+/* Every number below is COUNTED on the device where the event happens (none is derived from another), so
+ *   count == truncated + ret_precull_a + ret_precull_b + ret_seed + ret_trace + ret_resolve + ret_horizon + ret_finish
+ *   segments == count + hits - truncated,   escaped == count - truncated
+ * are checks of the pipeline's bookkeeping (a particle lost or duplicated between two lists breaks them). */
 typedef struct {
   uint64_t hits;           /* surface interactions ("bounces") */
-  uint64_t segments;       /* closest-hit queries = count + hits */
-  uint64_t escaped;        /* particles that left without (further) hit */
+  uint64_t segments;       /* segments answered: by a cull (1 per culled particle), the traversal, the escape horizon, the straggler kernel */
+  uint64_t escaped;        /* particles that left without (further) hit = all retirements except truncated */
   uint64_t truncated;      /* particles stopped by max_bounces */
-  uint64_t culled;         /* particles whose first segment was answered by the mesh-AABB test in the seed kernel */
+  uint64_t culled;         /* particles whose first segment was answered before the traversal = ret_precull_a + ret_precull_b + ret_seed */
   uint64_t tri_tests;      /* fp64 ray-triangle evaluations */
   uint64_t node_visits;    /* 64-byte BVH nodes fetched */
   uint64_t kernel_launches;/* kernels this run enqueued */
@@ -80,9 +108,24 @@ typedef struct {
   double ms_trace;         /* ... of the wavefront traversal kernel launches */
   double ms_reflect;       /* ... of the resolve/reflect/accumulate kernel launches */
   double ms_finish;        /* ... of the straggler kernel launches */
-  uint64_t timed_waves;    /* waves covered by the per-kernel times (all of them unless > 512) */
+  uint64_t timed_waves;    /* waves covered by the per-kernel times (the first 1024 of the first index chunk) */
   uint64_t trace_launches; /* traversal-kernel launches covered by ms_trace */
-  uint64_t traced_rays;    /* rays those launches processed */
+  uint64_t traced_rays;    /* rays the traversal kernel processed (all launches) */
+  /* where each particle retired (see the identities above) */
+  uint64_t ret_precull_a;  /* certain miss of the bounding sphere, pre-cull stage A */
+  uint64_t ret_precull_b;  /* certified miss of the cull volumes, pre-cull stage B */
+  uint64_t ret_seed;       /* exact fp32 ray misses the mesh AABB / the top of the hierarchy, seed kernel */
+  uint64_t ret_trace;      /* traversal ended without a candidate facet */
+  uint64_t ret_resolve;    /* all candidates rejected by the exact test */
+  uint64_t ret_horizon;    /* re-emitted above the facet's escape horizon */
+  uint64_t ret_finish;     /* no hit in the straggler kernel's fp64 search */
+  /* flows between the steps */
+  uint64_t queued_primaries; /* rays the seed kernel appended to the queue */
+  uint64_t queued_reflected; /* rays the reflect step appended to the next queue */
+  uint64_t overflow_rays;    /* rays handed to the straggler kernel by an overflow list (candidate overflow, stack abort, full region) */
+  uint64_t final_stragglers; /* rays still queued after the drain iterations (followed by the straggler kernel, not traced) */
+  uint64_t finish_segments;  /* closest-hit searches of the straggler kernel */
+  double ms_sort;          /* summed device time of the ray-sort launches */
 } tpmc_stats;
 
 /* Optional per-particle outputs for parity checks; each pointer is device [count] or NULL. */
@@ -127,12 +170,12 @@ int tpmc_mesh_copy_horizon(const tpmc_mesh* mesh, uint8_t* h_horizon);
  *   h_stats                     host or NULL; if given the call synchronises the stream and fills it
  *   debug                       host struct of device pointers, or NULL
  * Slices are additive: summing the outputs of disjoint [first,count) slices of one N gives the full run. */
-int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* cuda_stream, double* d_force,
+int tpmc_run(tpmc_mesh* mesh, const tpmc_params* params, void* cuda_stream, double* d_force,
              double* d_torque, double* d_facet_momentum, tpmc_stats* h_stats, const tpmc_debug* debug);
 
 /* Same run with HOST result buffers (h_facet_momentum may be NULL): device results are copied back
  * inside the call and the stream is synchronised before returning. */
-int tpmc_run_host(const tpmc_mesh* mesh, const tpmc_params* params, void* cuda_stream, double* h_force,
+int tpmc_run_host(tpmc_mesh* mesh, const tpmc_params* params, void* cuda_stream, double* h_force,
                   double* h_torque, double* h_facet_momentum, tpmc_stats* h_stats);
 
 /* Seeding step alone (O3-O8), for parity checks: fp64 position and velocity of particles
@@ -143,9 +186,12 @@ int tpmc_seed(const tpmc_mesh* mesh, const tpmc_params* params, void* cuda_strea
 
 /* Closest-hit step alone (O10), for parity checks: rays o + tau d with fp32 origin/direction,
  * d_o, d_d device [n][3]; d_f_prev device [n] (facet to exclude, -1 for none) or NULL;
- * outputs d_facet [n] (-1 = no hit) and d_tau [n] (fp64, +inf when no hit). */
-int tpmc_trace(const tpmc_mesh* mesh, const float* d_o, const float* d_d, const int32_t* d_f_prev, int64_t n,
-               void* cuda_stream, int32_t* d_facet, double* d_tau);
+ * h_align_V host [3] or NULL: when given, the traversal walks the hierarchy refitted in the stream frame of that
+ * bulk velocity (what tpmc_run does for oblique attitudes) instead of the body-frame one -- same results;
+ * outputs d_facet [n] (-1 = no hit) and d_tau [n] (fp64, +inf when no hit).  Runs the production traversal
+ * kernel and the exact resolve; synchronises the stream. */
+int tpmc_trace(tpmc_mesh* mesh, const float* d_o, const float* d_d, const int32_t* d_f_prev, int64_t n,
+               const double* h_align_V, void* cuda_stream, int32_t* d_facet, double* d_tau);
 
 const char* tpmc_strerror(int code);
 const char* tpmc_last_cuda_error(void);

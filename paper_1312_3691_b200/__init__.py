@@ -20,6 +20,10 @@ LIB_PATH = os.path.join(_HERE, "libtpmc.so")
 TPMC_OK, TPMC_EINVAL, TPMC_ENOMEM, TPMC_ECUDA = 0, -1, -2, -3
 TPMC_MEM_HOST, TPMC_MEM_DEVICE = 0, 1
 TPMC_MAX_SPECIES = 8
+TPMC_MAX_BOUNCES = 0x0FFFFFFF
+TPMC_FLAG_NO_PRECULL, TPMC_FLAG_NO_HORIZON, TPMC_FLAG_ALIGN_OFF, TPMC_FLAG_ALIGN_ON = 0x01, 0x02, 0x04, 0x08
+TPMC_FLAG_EXACT_TRACE, TPMC_FLAG_NO_SORT = 0x10, 0x20
+TPMC_CV_SPHERE, TPMC_CV_BOX, TPMC_CV_BOX_UNWEIGHTED = 0, 1, 2
 
 EXPORTS = ["tpmc_mesh_create", "tpmc_mesh_destroy", "tpmc_mesh_info", "tpmc_mesh_copy_bvh", "tpmc_run",
            "tpmc_mesh_copy_horizon", "tpmc_run_host", "tpmc_seed", "tpmc_trace", "tpmc_strerror", "tpmc_last_cuda_error", "tpmc_version"]
@@ -41,7 +45,8 @@ class tpmc_params(C.Structure):
                 ("m", C.POINTER(C.c_double)), ("x", C.POINTER(C.c_double)),
                 ("cv_radius_factor", C.c_double), ("N", C.c_uint64), ("first", C.c_uint64),
                 ("count", C.c_uint64), ("seed", C.c_uint64), ("max_bounces", C.c_uint32),
-                ("x_ref", C.c_double * 3)]
+                ("x_ref", C.c_double * 3), ("energy_accommodation", C.c_double), ("wave_particles", C.c_uint64),
+                ("chunk_particles", C.c_uint64), ("flags", C.c_uint32), ("control_volume", C.c_int32)]
 
 
 class tpmc_stats(C.Structure):
@@ -49,7 +54,12 @@ class tpmc_stats(C.Structure):
                 ("culled", C.c_uint64), ("tri_tests", C.c_uint64), ("node_visits", C.c_uint64),
                 ("kernel_launches", C.c_uint64), ("ms", C.c_double), ("ms_seed", C.c_double), ("ms_trace", C.c_double),
                 ("ms_reflect", C.c_double), ("ms_finish", C.c_double), ("timed_waves", C.c_uint64),
-                ("trace_launches", C.c_uint64), ("traced_rays", C.c_uint64)]
+                ("trace_launches", C.c_uint64), ("traced_rays", C.c_uint64),
+                ("ret_precull_a", C.c_uint64), ("ret_precull_b", C.c_uint64), ("ret_seed", C.c_uint64),
+                ("ret_trace", C.c_uint64), ("ret_resolve", C.c_uint64), ("ret_horizon", C.c_uint64),
+                ("ret_finish", C.c_uint64), ("queued_primaries", C.c_uint64), ("queued_reflected", C.c_uint64),
+                ("overflow_rays", C.c_uint64), ("final_stragglers", C.c_uint64), ("finish_segments", C.c_uint64),
+                ("ms_sort", C.c_double)]
 
 
 class tpmc_debug(C.Structure):
@@ -85,7 +95,7 @@ def lib():
         L.tpmc_seed.restype = C.c_int
         L.tpmc_seed.argtypes = [vp, C.POINTER(tpmc_params), vp, vp, vp, vp]
         L.tpmc_trace.restype = C.c_int
-        L.tpmc_trace.argtypes = [vp, vp, vp, vp, C.c_int64, vp, vp, vp]
+        L.tpmc_trace.argtypes = [vp, vp, vp, vp, C.c_int64, vp, vp, vp, vp]
         for n in ("tpmc_strerror", "tpmc_last_cuda_error", "tpmc_version"):
             getattr(L, n).restype = C.c_char_p
         L.tpmc_strerror.argtypes = [C.c_int]
@@ -115,7 +125,7 @@ def _stream_ptr(stream) -> Optional[int]:
     return getattr(stream, "cuda_stream", stream) or None
 
 
-def make_params(cfg, first=None, count=None, N=None):
+def make_params(cfg, first=None, count=None, N=None, flags=0, wave_particles=0, chunk_particles=0):
     """Marshal a parameter record (anything with the tpmc_params field names, e.g.
     tpmc_inputs.RunConfig) into a C struct.  Returns (struct, keepalive)."""
     p = tpmc_params()
@@ -134,6 +144,11 @@ def make_params(cfg, first=None, count=None, N=None):
     p.seed = int(cfg.seed)
     p.max_bounces = int(cfg.max_bounces)
     p.x_ref = (C.c_double * 3)(*[float(a) for a in cfg.x_ref])
+    p.energy_accommodation = float(getattr(cfg, "energy_accommodation", 1.0))
+    p.wave_particles = int(wave_particles)
+    p.chunk_particles = int(chunk_particles)
+    p.flags = int(flags)
+    p.control_volume = int(getattr(cfg, "control_volume", TPMC_CV_SPHERE))
     return p, (m, x)
 
 
@@ -206,9 +221,10 @@ class Mesh:
         return hz
 
     # ------------------------------------------------------------------ the hot path
-    def run(self, cfg, first=None, count=None, N=None, facets=True, debug=False, stats=True, stream=None) -> RunResult:
+    def run(self, cfg, first=None, count=None, N=None, facets=True, debug=False, stats=True, stream=None,
+            flags=0, wave_particles=0, chunk_particles=0) -> RunResult:
         torch = _torch()
-        p, keep = make_params(cfg, first, count, N)
+        p, keep = make_params(cfg, first, count, N, flags, wave_particles, chunk_particles)
         dev = torch.device("cuda", torch.cuda.current_device())
         force = torch.empty(3, dtype=torch.float64, device=dev)
         torque = torch.empty(3, dtype=torch.float64, device=dev)
@@ -229,10 +245,10 @@ class Mesh:
         return RunResult(force, torque, fm, sd, hs, nb, ff)
 
     def run_host(self, cfg, first=None, count=None, N=None, facets=True, stats=True, stream=None,
-                 out_facets: Optional[np.ndarray] = None):
+                 out_facets: Optional[np.ndarray] = None, flags=0):
         """tpmc_run_host: results land in HOST numpy buffers (D2H copies inside the call)."""
         _torch()
-        p, keep = make_params(cfg, first, count, N)
+        p, keep = make_params(cfg, first, count, N, flags)
         force = np.empty(3, dtype=np.float64)
         torque = np.empty(3, dtype=np.float64)
         fm = None
@@ -258,8 +274,9 @@ class Mesh:
                                s.data_ptr() or None), "tpmc_seed")
         return x, v, s
 
-    def trace(self, o, d, f_prev=None, stream=None):
-        """Closest hit of rays o + tau d (tpmc_trace).  o, d: [n,3] float32 (numpy or CUDA tensors)."""
+    def trace(self, o, d, f_prev=None, stream=None, align_V=None):
+        """Closest hit of rays o + tau d (tpmc_trace).  o, d: [n,3] float32 (numpy or CUDA tensors); align_V: walk
+        the hierarchy refitted in the stream frame of this bulk velocity instead of the body-frame one."""
         torch = _torch()
         dev = torch.device("cuda", torch.cuda.current_device())
         o = torch.as_tensor(np.ascontiguousarray(o, dtype=np.float32) if isinstance(o, np.ndarray) else o).to(dev, torch.float32).contiguous()
@@ -270,8 +287,9 @@ class Mesh:
             fp = torch.as_tensor(f_prev).to(dev, torch.int32).contiguous()
         facet = torch.empty(n, dtype=torch.int32, device=dev)
         tau = torch.empty(n, dtype=torch.float64, device=dev)
+        av = None if align_V is None else (C.c_double * 3)(*[float(a) for a in align_V])
         _check(lib().tpmc_trace(self._h, o.data_ptr() or None, d.data_ptr() or None, None if fp is None else fp.data_ptr(),
-                                n, _stream_ptr(stream), facet.data_ptr() or None, tau.data_ptr() or None), "tpmc_trace")
+                                n, av, _stream_ptr(stream), facet.data_ptr() or None, tau.data_ptr() or None), "tpmc_trace")
         return facet, tau
 
 

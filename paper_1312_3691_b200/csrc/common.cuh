@@ -87,13 +87,14 @@ struct tpmc_mesh {
   double* partials;                // reduction partials
   unsigned long long* stats;       // [8] device counters
   double* totals;                  // [3] torque accumulators
+  double* ft_dev;                  // [6] force | torque of tpmc_run_host
   cudaEvent_t ev0, ev1, ev_fork;
   unsigned long long last_launches;
 };
 
 constexpr int kMaxTimedWaves = 1024;  // iterations covered by the per-kernel event times
 constexpr int kDrain = 3;             // trace/reflect iterations after the last wave, before the straggler kernel
-constexpr int kEvPerWave = 7;         // seed start/end (seed stream), trace start, after trace, after reflect, straggler start/end (side stream)
+constexpr int kEvPerWave = 8;         // seed start/end (seed stream), iteration start, after trace, after reflect, straggler start/end (side stream), after sort
 constexpr int kCtrWords = 16;
 constexpr int kCullNodes = 64;        // 4 KB: stays in L1 next to the shared-memory carve-out
 constexpr float kPrecullMargin = 2e-2f;   // box growth of the pre-cull pass, in bounding radii (sampling.cuh)
@@ -103,6 +104,8 @@ struct QuantGrid {
   float origin[3];
   float inv_scale[3];   // fp32(1 / q_scale)
   float R[9];           // frame of the grid: x' = R x (identity for the body-frame hierarchy, see tpmc_mesh_align)
+  float rot_o, rot_c;   // rotation-error terms of the slab margin (trace.cuh, grid_ray): 0 for the identity frame, else
+                        // 9u (factor of |o|_1) and 6u * reach, reach = largest |x| over the root box, in metres
 };
 
 // Per-run constants (a1: host, fp64), passed to kernels by value.
@@ -129,6 +132,11 @@ struct RunConst {
   unsigned int seed_lo, seed_hi;
   unsigned int max_bounces;
 };
+
+// Device counters of a run (tpmc_stats: every one is counted where the event happens).
+enum { ST_HITS = 0, ST_TRUNC, ST_TRIS, ST_NODES, ST_TRACED, ST_RET_PA, ST_RET_PB, ST_RET_SEED, ST_RET_TRACE,
+       ST_RET_RESOLVE, ST_RET_HORIZON, ST_RET_FINISH, ST_Q_PRIM, ST_Q_REFL, ST_OVF_RETRACE, ST_OVF_PENDING, ST_DIVERTED,
+       ST_STRAGGLERS, ST_FIN_SEGS, ST_COUNT = 24 };
 
 int tpmc_mesh_align(tpmc_mesh* m, const double R[9], cudaStream_t st, const QuantGrid** grid_out, const uint4** cnodes_out);
 

@@ -190,7 +190,8 @@ __global__ void k_single(const float* __restrict__ box_leaf, float4* __restrict_
 //   words 6-7: the two child refs.
 // Grid: x = origin + q * scale per axis.  lo is rounded down and hi up: the decoded box contains the fp32 box.
 // (The quotient is evaluated in fp64: a box corner within 1e-11 steps of a grid plane may land on the wrong
-// side of it, which the slack of the traversal's margin G covers.)
+// side of it, which the slack of the traversal's margin G covers.  The clamps below never act on a box of the
+// hierarchy: quant_step keeps every plane inside steps 0 .. 65535.)
 __global__ void k_compact_nodes(const float4* __restrict__ nodes, int64_t n_nodes, double ox, double oy, double oz,
                                 double sx, double sy, double sz, uint4* __restrict__ cnodes,
                                 const double* __restrict__ dev_grid = nullptr) {
@@ -266,15 +267,29 @@ __global__ void k_leaf_boxes_rot(const float4* __restrict__ tris, int64_t nt, in
   }
 }
 
+// Grid step of one axis: the root box spans steps 100 .. 65100.  Lower bounds: 1e-6 of the largest extent (flat axes),
+// and 4u max|coordinate|, so that the 100-step pad below the box always exceeds the fp32 rounding of the grid origin
+// (u |lo|): no plane of the hierarchy ever falls below step 0 or above step 65535, where k_compact_nodes would have to
+// clamp it inwards.
+__host__ __device__ inline double quant_step(double ext, double emax, double lo, double hi) {
+  const double cmax = fmax(fabs(lo), fabs(hi));
+  return fmax(fmax(ext, 1e-6 * emax) / 65000.0, fmax(4.0 * 5.9604645e-08 * cmax, 1e-30));
+}
+
 // Quantisation grid of the aligned hierarchy from the root box of the refit (device side: no host round trip).
 // out_d: origin xyz, scale xyz (fp32 values held as doubles, for k_compact_nodes); out_g: what the traversal reads.
 __global__ void k_align_grid(const float* __restrict__ root_box, const double* __restrict__ R, double* __restrict__ out_d,
                              QuantGrid* __restrict__ out_g) {
   if (blockIdx.x != 0 || threadIdx.x != 0) return;
-  double ext[3], emax = 0.0;
-  for (int a = 0; a < 3; ++a) { ext[a] = (double)root_box[3 + a] - (double)root_box[a]; emax = fmax(emax, ext[a]); }
+  double ext[3], emax = 0.0, reach2 = 0.0;
   for (int a = 0; a < 3; ++a) {
-    const float qs = (float)(fmax(ext[a], fmax(1e-6 * emax, 1e-30)) / 65000.0);
+    ext[a] = (double)root_box[3 + a] - (double)root_box[a];
+    emax = fmax(emax, ext[a]);
+    const double c = fmax(fabs((double)root_box[a]), fabs((double)root_box[3 + a]));
+    reach2 += c * c;
+  }
+  for (int a = 0; a < 3; ++a) {
+    const float qs = (float)quant_step(ext[a], emax, (double)root_box[a], (double)root_box[3 + a]);
     const float qo = (float)((double)root_box[a] - 100.0 * (double)qs);
     out_d[a] = (double)qo;
     out_d[3 + a] = (double)qs;
@@ -282,6 +297,9 @@ __global__ void k_align_grid(const float* __restrict__ root_box, const double* _
     out_g->inv_scale[a] = (float)(1.0 / (double)qs);
   }
   for (int k = 0; k < 9; ++k) out_g->R[k] = (float)R[k];
+  // rotation-error terms of the traversal's slab margin (trace.cuh, grid_ray): 9u |o|_1 + 6u reach metres
+  out_g->rot_o = 9.0f * 5.9604645e-08f;
+  out_g->rot_c = (float)(6.0 * 5.9604645e-08 * sqrt(reach2) * 1.0001);
 }
 
 // ---- escape horizon of every one-sided facet (a0, read by the reflect step) ------------------------------
@@ -717,7 +735,7 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
     double ext[3], emax = 0.0;
     for (int a = 0; a < 3; ++a) { ext[a] = (double)h.aabb[3 + a] - (double)h.aabb[a]; emax = std::max(emax, ext[a]); }
     for (int a = 0; a < 3; ++a) {
-      m->q_scale[a] = (float)(std::max(ext[a], std::max(1e-6 * emax, 1e-30)) / 65000.0);
+      m->q_scale[a] = (float)quant_step(ext[a], emax, (double)h.aabb[a], (double)h.aabb[3 + a]);
       m->q_origin[a] = (float)((double)h.aabb[a] - 100.0 * (double)m->q_scale[a]);
     }
     MESH_TRY(cudaMalloc((void**)&m->cnodes, sizeof(uint4) * 2 * m->n_nodes));
@@ -727,6 +745,7 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
     QuantGrid hg;
     for (int a = 0; a < 3; ++a) { hg.origin[a] = m->q_origin[a]; hg.inv_scale[a] = (float)(1.0 / (double)m->q_scale[a]); }
     for (int k = 0; k < 9; ++k) hg.R[k] = (k % 4 == 0) ? 1.0f : 0.0f;
+    hg.rot_o = hg.rot_c = 0.0f;   // the identity frame is exact
     MESH_TRY(cudaMalloc((void**)&m->grid_dev, 2 * sizeof(QuantGrid)));
     MESH_TRY(cudaMemcpyAsync(m->grid_dev, &hg, sizeof(hg), cudaMemcpyHostToDevice, st));
     MESH_TRY(cudaMemcpyAsync(m->grid_dev + 1, &hg, sizeof(hg), cudaMemcpyHostToDevice, st));
@@ -734,9 +753,7 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
   DevBuf cq;
   MESH_TRY(cudaMalloc((void**)&m->cull_c, sizeof(uint4) * 2 * kCullNodes));
   MESH_TRY(cudaMalloc(&cq.p, sizeof(int) * (kCullNodes + 1)));
-  int cull_budget = kCullNodes;
-  if (const char* e = getenv("TPMC_CULL_NODES")) cull_budget = std::max(1, std::min(kCullNodes, atoi(e)));   // tuning aid
-  k_build_cull<<<1, 32, 0, st>>>(m->nodes, m->cnodes, m->cull_c, cq.as<int>(), cull_budget, cq.as<int>() + kCullNodes);
+  k_build_cull<<<1, 32, 0, st>>>(m->nodes, m->cnodes, m->cull_c, cq.as<int>(), kCullNodes, cq.as<int>() + kCullNodes);
   MESH_TRY(cudaMemcpyAsync(&m->n_cull, cq.as<int>() + kCullNodes, sizeof(int), cudaMemcpyDeviceToHost, st));
   {
     const int rcv = build_cull_volume(m, st);
@@ -812,7 +829,7 @@ extern "C" void tpmc_mesh_destroy(tpmc_mesh* m) {
       delete[] pp.wave_ev;
     }
   }
-  cudaFree(m->facet_scratch); cudaFree(m->partials); cudaFree(m->stats); cudaFree(m->totals);
+  cudaFree(m->facet_scratch); cudaFree(m->partials); cudaFree(m->stats); cudaFree(m->totals); cudaFree(m->ft_dev);
   if (m->ev0) cudaEventDestroy(m->ev0);
   if (m->ev1) cudaEventDestroy(m->ev1);
   if (m->ev_fork) cudaEventDestroy(m->ev_fork);

@@ -16,7 +16,11 @@ constexpr int kTraceBlock = 128;
 constexpr int kReduceBlock = 256;
 constexpr int kReduceParts = 296;   // 2 per SM
 
-enum { ST_HITS = 0, ST_TRUNC = 1, ST_CULLED = 2, ST_TRIS = 3, ST_NODES = 4, ST_TRACED = 5, ST_COUNT = 8 };
+// sum of a per-thread count over the warp, added to a device counter by lane 0 (all lanes must call)
+__device__ __forceinline__ void warp_count(unsigned long long* __restrict__ ctr, unsigned int v) {
+  v = __reduce_add_sync(0xFFFFFFFFu, v);
+  if ((threadIdx.x & 31) == 0 && v) atomicAdd(ctr, (unsigned long long)v);
+}
 
 __device__ __forceinline__ unsigned lanemask_lt() {
   unsigned m;
@@ -68,7 +72,8 @@ __global__ void __launch_bounds__(kPrecullBlock) k_seed_precull(const SeedConstF
                                                                  unsigned int seed_hi, unsigned long long first,
                                                                  unsigned int wave_n, unsigned int cap,
                                                                  unsigned int* __restrict__ surv,
-                                                                 unsigned int* __restrict__ n_surv) {
+                                                                 unsigned int* __restrict__ n_surv,
+                                                                 unsigned long long* __restrict__ stats) {
   __shared__ float qf[9][kPrecullQ];
   __shared__ unsigned int qj[kPrecullQ], qw[kPrecullQ];
   __shared__ unsigned char qok[kPrecullQ];
@@ -80,13 +85,15 @@ __global__ void __launch_bounds__(kPrecullBlock) k_seed_precull(const SeedConstF
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   if (threadIdx.x == 0) q_n = 0u;
   __syncthreads();
-  unsigned int base = begin;
+  unsigned int base = begin, drop_a = 0u, drop_b = 0u;   // particles retired here (counted, not inferred)
   for (;;) {
     const bool more = base < end;
     if (more) {
       const unsigned int j = base + threadIdx.x;
       PrecullA a;
-      const bool pass = precull_stage_a(sf, seed_lo, seed_hi, first + j, a) && (j < end);
+      const bool reach = precull_stage_a(sf, seed_lo, seed_hi, first + j, a);
+      const bool pass = reach && (j < end);
+      drop_a += (!reach && j < end) ? 1u : 0u;
       const unsigned m = __ballot_sync(0xFFFFFFFFu, pass);
       unsigned int pos = 0;
       if (lane == 0 && m) pos = atomicAdd(&q_n, (unsigned)__popc(m));
@@ -115,6 +122,7 @@ __global__ void __launch_bounds__(kPrecullBlock) k_seed_precull(const SeedConstF
       const bool ok = precull_stage_b(sf, a, o, v, root);
       const bool touch = precull_touch(sf, o, v);
       const bool keep_c = active && ok && touch, keep_u = active && !ok;
+      drop_b += (active && ok && !touch) ? 1u : 0u;
       const unsigned mcert = __ballot_sync(0xFFFFFFFFu, keep_c);
       const unsigned munc = __ballot_sync(0xFFFFFFFFu, keep_u);
       if (lane == 0) { s_cnt[0][wid] = __popc(mcert); s_cnt[1][wid] = __popc(munc); }
@@ -138,6 +146,8 @@ __global__ void __launch_bounds__(kPrecullBlock) k_seed_precull(const SeedConstF
       break;
     }
   }
+  warp_count(&stats[ST_RET_PA], drop_a);
+  warp_count(&stats[ST_RET_PB], drop_b);
 }
 
 // a2: seed particles of one wave in fp64, round the state to fp32 (O9), drop the rays that cannot touch the
@@ -153,8 +163,6 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
                                                      unsigned long long* __restrict__ stats) {
   const unsigned int n1 = surv ? n_surv[0] : 0u;                 // certified survivors: fp32 roots available
   const unsigned int n = surv ? n1 + n_surv[1] : wave_n;
-  if (blockIdx.x == 0 && threadIdx.x == 0 && n < wave_n)         // dropped by the pre-cull pass
-    atomicAdd(&stats[ST_CULLED], (unsigned long long)(wave_n - n));
   const unsigned int stride = gridDim.x * blockDim.x;
   const unsigned int nround = ((n + stride - 1) / stride) * stride;   // keep warps converged for the ballots
   for (unsigned int kk = blockIdx.x * blockDim.x + threadIdx.x; kk < nround; kk += stride) {
@@ -182,8 +190,8 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
   const int lane = threadIdx.x & 31;
   unsigned base = 0;
   if (lane == 0) {
-    if (m) base = atomicAdd(qcount, (unsigned)__popc(m));
-    if (mc) atomicAdd(&stats[ST_CULLED], (unsigned long long)__popc(mc));
+    if (m) { base = atomicAdd(qcount, (unsigned)__popc(m)); atomicAdd(&stats[ST_Q_PRIM], (unsigned long long)__popc(m)); }
+    if (mc) atomicAdd(&stats[ST_RET_SEED], (unsigned long long)__popc(mc));
   }
   base = __shfl_sync(0xFFFFFFFFu, base, 0);
   if (keep) {
@@ -241,6 +249,7 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
   w.cur = TPMC_SENTINEL; w.stash = 0; w.sp = 0; w.nc = 0; w.tmax = 0.0f; w.f_prev = -1;
   TraceCounters cnt;
   cnt.nodes = 0; cnt.tris = 0;
+  unsigned int n_escaped = 0u;   // rays that ended without a candidate facet: these particles retire here
   for (;;) {
     // ---- refill idle lanes from the warp's chunk of the queue (one atomic per kFetchChunk rays)
     const unsigned idle = __ballot_sync(FULL, !has && !exhausted);
@@ -287,7 +296,7 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
       const float o[3] = {ro.x, ro.y, ro.z}, d[3] = {rv.x, rv.y, rv.z};
       walk_leaf(w, tris, o, d, stk, kTraceBlock, cnt);
     }
-    if (has && w.cur == TPMC_SENTINEL && w.stash == 0) { has = false; fin = w.nc > 0; }
+    if (has && w.cur == TPMC_SENTINEL && w.stash == 0) { has = false; fin = w.nc > 0; n_escaped += fin ? 0u : 1u; }
     // ---- finished rays with candidates -> hit list
     const unsigned fm = __ballot_sync(FULL, fin);
     if (fm) {
@@ -315,44 +324,54 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
     if (cn) atomicAdd(&stats[ST_NODES], cn);
     if (ct) atomicAdd(&stats[ST_TRIS], ct);
   }
+  warp_count(&stats[ST_RET_TRACE], n_escaped);
   if (blockIdx.x == 0 && threadIdx.x == 0 && n) atomicAdd(&stats[ST_TRACED], (unsigned long long)n);
 }
 
 // Block-level sum of per-thread torque and counters, one atomic per block and quantity.
-__device__ __forceinline__ void block_flush(double tq[3], unsigned long long c4[4], double* __restrict__ torque,
-                                            unsigned long long* __restrict__ stats, double (*sred)[8],
-                                            unsigned long long (*scnt)[8]) {
+// c[k] is added to stats[c_flush_idx[which][k]], k < kFlushCounters (which: 0 = k_reflect, 1 = k_finish).
+constexpr int kFlushCounters = 10;
+enum { FC_HITS = 0, FC_TRUNC, FC_TRIS, FC_NODES, FC_HORIZON, FC_NOHIT, FC_QUEUED, FC_RETRACE, FC_PENDING, FC_SEGS };
+__constant__ int c_flush_idx[2][kFlushCounters] = {
+    {ST_HITS, ST_TRUNC, ST_TRIS, ST_NODES, ST_RET_HORIZON, ST_RET_RESOLVE, ST_Q_REFL, ST_OVF_RETRACE, ST_OVF_PENDING, ST_FIN_SEGS},
+    {ST_HITS, ST_TRUNC, ST_TRIS, ST_NODES, ST_RET_HORIZON, ST_RET_FINISH, ST_Q_REFL, ST_OVF_RETRACE, ST_OVF_PENDING, ST_FIN_SEGS}};
+struct FlushShared {
+  double red[3][8];
+  unsigned int cnt[kFlushCounters][8];
+};
+__device__ __forceinline__ void block_flush(double tq[3], const unsigned int c[kFlushCounters], int which,
+                                            double* __restrict__ torque, unsigned long long* __restrict__ stats,
+                                            FlushShared& sh) {
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) {
 #pragma unroll
     for (int a = 0; a < 3; ++a) tq[a] += __shfl_down_sync(0xFFFFFFFFu, tq[a], off);
+  }
 #pragma unroll
-    for (int a = 0; a < 4; ++a) c4[a] += __shfl_down_sync(0xFFFFFFFFu, c4[a], off);
+  for (int a = 0; a < kFlushCounters; ++a) {
+    const unsigned int v = __reduce_add_sync(0xFFFFFFFFu, c[a]);
+    if (lane == 0) sh.cnt[a][wid] = v;
   }
-  if (lane == 0) {
-    for (int a = 0; a < 3; ++a) sred[a][wid] = tq[a];
-    for (int a = 0; a < 4; ++a) scnt[a][wid] = c4[a];
-  }
+  if (lane == 0)
+    for (int a = 0; a < 3; ++a) sh.red[a][wid] = tq[a];
   __syncthreads();
   if (threadIdx.x == 0) {
     double t3[3] = {0, 0, 0};
-    unsigned long long s4[4] = {0, 0, 0, 0};
-    for (int wv = 0; wv < nw; ++wv) {
-      for (int a = 0; a < 3; ++a) t3[a] += sred[a][wv];
-      for (int a = 0; a < 4; ++a) s4[a] += scnt[a][wv];
-    }
+    for (int wv = 0; wv < nw; ++wv)
+      for (int a = 0; a < 3; ++a) t3[a] += sh.red[a][wv];
     for (int a = 0; a < 3; ++a) if (t3[a] != 0.0) atomicAdd(&torque[a], t3[a]);
-    if (s4[0]) atomicAdd(&stats[ST_HITS], s4[0]);
-    if (s4[1]) atomicAdd(&stats[ST_TRUNC], s4[1]);
-    if (s4[2]) atomicAdd(&stats[ST_TRIS], s4[2]);
-    if (s4[3]) atomicAdd(&stats[ST_NODES], s4[3]);
+  }
+  if (threadIdx.x < kFlushCounters) {
+    unsigned long long tot = 0;
+    for (int wv = 0; wv < nw; ++wv) tot += sh.cnt[threadIdx.x][wv];
+    if (tot) atomicAdd(&stats[c_flush_idx[which][threadIdx.x]], tot);
   }
 }
 
 // One surface interaction (O11-O13) of a particle whose closest hit is known: momentum and torque
-// accumulation, debug records, and the state of the next segment.  Returns false when the particle stops
-// here (bounce cap).
+// accumulation, debug records, and the state of the next segment.  Returns GO_ON, or why the particle retires here.
+enum { GO_ON = 0, END_TRUNCATED = 1, END_HORIZON = 2 };
 struct Particle {
   float o[3], v[3];
   unsigned long long j;   // index within the chunk (rc.first = first particle of the chunk)
@@ -361,9 +380,9 @@ struct Particle {
   int f_prev;
 };
 
-__device__ __forceinline__ bool interact(const RunConst& rc, const float4* __restrict__ tris, Particle& p, const Hit& hit,
-                                         double* __restrict__ P, double tq[3], const tpmc_debug& dbg,
-                                         unsigned long long& trunc, const uint4* __restrict__ horizon = nullptr) {
+__device__ __forceinline__ int interact(const RunConst& rc, const float4* __restrict__ tris, Particle& p, const Hit& hit,
+                                        double* __restrict__ P, double tq[3], const tpmc_debug& dbg,
+                                        const uint4* __restrict__ horizon) {
   const float4 q0 = __ldg(tris + 3 * (size_t)hit.slot), q1 = __ldg(tris + 3 * (size_t)hit.slot + 1),
                q2 = __ldg(tris + 3 * (size_t)hit.slot + 2);
   const double w = rc.sp[p.species].w, cW = rc.sp[p.species].cW;
@@ -392,14 +411,14 @@ __device__ __forceinline__ bool interact(const RunConst& rc, const float4* __res
   for (int a = 0; a < 3; ++a) { p.o[a] = (float)hp[a]; p.v[a] = vo[a]; }
   p.f_prev = hit.facet;
   ++p.k;
-  if (p.k >= rc.max_bounces) { ++trunc; return false; }
+  if (p.k >= rc.max_bounces) return END_TRUNCATED;
   // escape horizon of the facet (k_horizon, lbvh.cu): above it the next segment cannot hit anything
   if (horizon) {
     const int sector = min(max((int)floorf((phi + 3.14159265f) * 2.54647909f), 0), 15);   // 16 / (2 pi)
     const unsigned int b = __ldg((const unsigned char*)horizon + 16 * (size_t)hit.slot + sector);
-    if (b < 255u && sin_e > (float)b * (1.0f / 254.0f)) return false;
+    if (b < 255u && sin_e > (float)b * (1.0f / 254.0f)) return END_HORIZON;
   }
-  return true;
+  return GO_ON;
 }
 
 // a4-a6: resolve the candidates of every hit ray with the exact fp64 test, apply the surface interaction,
@@ -417,14 +436,12 @@ __global__ void __launch_bounds__(kTraceBlock, 6) k_reflect(const RunConst rc, u
                                                          double* __restrict__ P, double* __restrict__ torque,
                                                          unsigned long long* __restrict__ stats, tpmc_debug dbg,
                                                          const uint4* __restrict__ horizon) {
-  __shared__ double sred[3][8];
-  __shared__ unsigned long long scnt[4][8];
+  __shared__ FlushShared fsh;
   const unsigned int n = *n_hits;
   const int lane = threadIdx.x & 31;
   const unsigned FULL = 0xFFFFFFFFu;
   double tq[3] = {0.0, 0.0, 0.0};
-  unsigned long long hits = 0, trunc = 0;
-  unsigned int ntests = 0;
+  unsigned int c[kFlushCounters] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
   const unsigned int stride = gridDim.x * blockDim.x;
   const unsigned int nround = ((n + stride - 1) / stride) * stride;   // keep warps converged for the ballots
   for (unsigned int h = blockIdx.x * blockDim.x + threadIdx.x; h < nround; h += stride) {
@@ -438,6 +455,7 @@ __global__ void __launch_bounds__(kTraceBlock, 6) k_reflect(const RunConst rc, u
       const int4 cand = __ldcs(hit_cand + h);
       if (cand.w == TPMC_CAND_OVERFLOW) {
         spill = true;
+        ++c[FC_RETRACE];
       } else {
         const float4 ro = __ldcs(qin.o + r), rv = __ldcs(qin.v + r);
         p.o[0] = ro.x; p.o[1] = ro.y; p.o[2] = ro.z;
@@ -447,8 +465,9 @@ __global__ void __launch_bounds__(kTraceBlock, 6) k_reflect(const RunConst rc, u
         p.species = (int)(pk & 15u);
         p.k = pk >> 4;
         p.f_prev = __ldcs(qin.f + r);
-        hit = resolve_candidates(tris, cand, p.o, p.v, ntests);
+        hit = resolve_candidates(tris, cand, p.o, p.v, c[FC_TRIS]);
         is_hit = hit.facet >= 0;
+        c[FC_NOHIT] += is_hit ? 0u : 1u;
       }
     }
     // surface interaction, then a queue slot for every particle that goes on (warp-aggregated).  A particle
@@ -456,8 +475,11 @@ __global__ void __launch_bounds__(kTraceBlock, 6) k_reflect(const RunConst rc, u
     // and goes to the overflow list, like one the traversal gave up on.
     bool go_on = false;
     if (is_hit) {
-      ++hits;
-      go_on = interact(rc, tris, p, hit, P, tq, dbg, trunc, horizon);
+      ++c[FC_HITS];
+      const int end = interact(rc, tris, p, hit, P, tq, dbg, horizon);
+      go_on = end == GO_ON;
+      c[FC_TRUNC] += end == END_TRUNCATED ? 1u : 0u;
+      c[FC_HORIZON] += end == END_HORIZON ? 1u : 0u;
     }
     const unsigned em = __ballot_sync(FULL, go_on);
     if (em) {
@@ -470,6 +492,8 @@ __global__ void __launch_bounds__(kTraceBlock, 6) k_reflect(const RunConst rc, u
         const RayQueue& qd = (s >= cap) ? qin : qout;
         const unsigned sd = (s >= cap) ? r : s;
         spill = s >= cap;
+        c[FC_PENDING] += spill ? 1u : 0u;
+        c[FC_QUEUED] += spill ? 0u : 1u;
         __stcs(qd.o + sd, make_float4(p.o[0], p.o[1], p.o[2], __uint_as_float((unsigned int)p.j)));
         __stcs(qd.v + sd, make_float4(p.v[0], p.v[1], p.v[2], __uint_as_float((unsigned int)p.species | (p.k << 4))));
         __stcs(qd.f + sd, p.f_prev);
@@ -484,8 +508,7 @@ __global__ void __launch_bounds__(kTraceBlock, 6) k_reflect(const RunConst rc, u
       if (spill) ovf[base + __popc(sm & lanemask_lt())] = r;
     }
   }
-  unsigned long long c4[4] = {hits, trunc, (unsigned long long)ntests, 0ull};
-  block_flush(tq, c4, torque, stats, sred, scnt);
+  block_flush(tq, c, 0, torque, stats, fsh);
 }
 
 // Particles followed to escape thread by thread (full fp64 traversal per segment): the overflow list of an
@@ -500,11 +523,11 @@ __global__ void __launch_bounds__(kTraceBlock) k_finish(const RunConst rc, unsig
                                                         unsigned long long* __restrict__ stats, tpmc_debug dbg,
                                                         const uint4* __restrict__ horizon) {
   __shared__ int sstack[TPMC_STACK_SMEM * kTraceBlock];
-  __shared__ double sred[3][8];
-  __shared__ unsigned long long scnt[4][8];
+  __shared__ FlushShared fsh;
   const unsigned int n = list ? *n_rays : min(*n_rays, cap);
+  if (!list && blockIdx.x == 0 && threadIdx.x == 0 && n) atomicAdd(&stats[ST_STRAGGLERS], (unsigned long long)n);
   double tq[3] = {0.0, 0.0, 0.0};
-  unsigned long long hits = 0, trunc = 0;
+  unsigned int c[kFlushCounters] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
   TraceCounters cnt;
   cnt.nodes = 0; cnt.tris = 0;
   for (unsigned int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
@@ -520,14 +543,33 @@ __global__ void __launch_bounds__(kTraceBlock) k_finish(const RunConst rc, unsig
     p.f_prev = q.f[r];
     for (;;) {
       const Hit hit = closest_hit(nodes, tris, p.o, p.v, p.f_prev, sstack + threadIdx.x, kTraceBlock, cnt);
-      if (hit.facet < 0) break;
-      ++hits;
-      if (!interact(rc, tris, p, hit, P, tq, dbg, trunc, horizon)) break;
+      ++c[FC_SEGS];
+      if (hit.facet < 0) { ++c[FC_NOHIT]; break; }
+      ++c[FC_HITS];
+      const int end = interact(rc, tris, p, hit, P, tq, dbg, horizon);
+      c[FC_TRUNC] += end == END_TRUNCATED ? 1u : 0u;
+      c[FC_HORIZON] += end == END_HORIZON ? 1u : 0u;
+      if (end != GO_ON) break;
     }
   }
-  unsigned long long c4[4] = {hits, trunc, (unsigned long long)cnt.tris, (unsigned long long)cnt.nodes};
-  block_flush(tq, c4, torque, stats, sred, scnt);
+  c[FC_TRIS] = cnt.tris;
+  c[FC_NODES] = cnt.nodes;
+  block_flush(tq, c, 1, torque, stats, fsh);
 }
+
+// TPMC_FLAG_EXACT_TRACE: every queued ray goes to the overflow list (the straggler kernel follows it to escape with
+// the fp64 closest-hit search); the traversal and reflect kernels then see an empty queue.
+__global__ void k_divert(unsigned int cap, unsigned int* __restrict__ n_rays, unsigned int* __restrict__ ovf,
+                         unsigned int* __restrict__ n_ovf, unsigned long long* __restrict__ stats) {
+  const unsigned int na = min(n_rays[0], cap), n = na + n_rays[1];
+  for (unsigned int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x)
+    ovf[i] = (i < na) ? i : cap + (i - na);
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    *n_ovf = n;
+    if (n) atomicAdd(&stats[ST_DIVERTED], (unsigned long long)n);
+  }
+}
+
 
 // a7: F = sum_f P_f by a fixed-shape tree (deterministic for given P): parts -> one block.
 __global__ void __launch_bounds__(kReduceBlock) k_reduce_parts(const double* __restrict__ P, long long nt,
@@ -644,7 +686,13 @@ int make_run_const(const tpmc_mesh* m, const tpmc_params* p, RunConst* rc) {
   if (!(p->accommodation >= 0.0 && p->accommodation <= 1.0)) return TPMC_EINVAL;
   if (!(p->cv_radius_factor >= 1.0) || !isfinite(p->cv_radius_factor)) return TPMC_EINVAL;
   if (p->N == 0 || p->first > p->N || p->count > p->N - p->first) return TPMC_EINVAL;
-  if (p->max_bounces < 1 || p->max_bounces > 0x7FFFFFF0u) return TPMC_EINVAL;
+  if (p->max_bounces < 1 || p->max_bounces > TPMC_MAX_BOUNCES) return TPMC_EINVAL;
+  if (!(p->energy_accommodation >= 0.0 && p->energy_accommodation <= 1.0)) return TPMC_EINVAL;
+  if ((p->flags & TPMC_FLAG_ALIGN_OFF) && (p->flags & TPMC_FLAG_ALIGN_ON)) return TPMC_EINVAL;
+  if (p->flags & ~0x3Fu) return TPMC_EINVAL;
+  if (p->wave_particles && (p->wave_particles < 256 || p->wave_particles > (1ull << 28))) return TPMC_EINVAL;
+  if (p->chunk_particles > 0xF0000000ull) return TPMC_EINVAL;
+  if (p->control_volume != TPMC_CV_SPHERE) return TPMC_EINVAL;   // TPMC_CV_BOX*: not in this build
   double xs = 0.0;
   for (int s = 0; s < p->n_species; ++s) {
     if (!(p->m[s] > 0.0) || !(p->x[s] >= 0.0)) return TPMC_EINVAL;
@@ -711,8 +759,7 @@ void make_seed_const_f(const tpmc_mesh* m, const RunConst& rc, SeedConstF* sf) {
     const double sg = std::min(0.999999, (double)Rg / rc.r);   // sin(theta)
     sf->cot_g = (float)(sqrt(1.0 - sg * sg) / sg * (1.0 - 1e-6));
   }
-  static const bool no_two_level = getenv("TPMC_CULL_VOLUME") && getenv("TPMC_CULL_VOLUME")[0] == '0';   // tuning aid
-  sf->n_box = no_two_level ? -1 : m->cull_nbox;
+  sf->n_box = m->cull_nbox;
   if (sf->n_box >= 0) {
     const float Ri = m->cull_rin + mg;
     sf->Rin2 = Ri * Ri;
@@ -724,37 +771,23 @@ void make_seed_const_f(const tpmc_mesh* m, const RunConst& rc, SeedConstF* sf) {
   }
 }
 
-TraceTune trace_tune() {
-  static TraceTune t = {0, 0};
-  if (!t.node_min) {
-    t.node_min = TPMC_NODE_MIN; t.refill_idle = TPMC_REFILL_IDLE;
-    if (const char* e = getenv("TPMC_NODE_MIN")) t.node_min = std::max(1, std::min(32, atoi(e)));        // tuning aids
-    if (const char* e = getenv("TPMC_REFILL_IDLE")) t.refill_idle = std::max(1, std::min(32, atoi(e)));
-  }
-  return t;
-}
+TraceTune trace_tune() { return TraceTune{TPMC_NODE_MIN, TPMC_REFILL_IDLE}; }
 
 QuantGrid quant_grid(const tpmc_mesh* m) {   // the body-frame hierarchy
   QuantGrid g;
   for (int a = 0; a < 3; ++a) { g.origin[a] = m->q_origin[a]; g.inv_scale[a] = (float)(1.0 / (double)m->q_scale[a]); }
   for (int k = 0; k < 9; ++k) g.R[k] = (k % 4 == 0) ? 1.0f : 0.0f;
+  g.rot_o = g.rot_c = 0.0f;
   return g;
 }
 
-size_t wave_size() {
-  static size_t w = 0;
-  if (!w) {
-    const char* e = getenv("TPMC_WAVE");
-    long long v = e ? atoll(e) : 0;
-    w = (v >= 1024 && v <= (1ll << 28)) ? (size_t)v : ((size_t)1 << 26);
-  }
-  return w;
-}
+constexpr size_t kDefaultWave = (size_t)1 << 26;   // particles per pipeline iteration (tpmc_params.wave_particles = 0)
 
 int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
   if (!m->stats) {
     TPMC_CUDA_TRY(cudaMalloc((void**)&m->stats, ST_COUNT * sizeof(unsigned long long)));
     TPMC_CUDA_TRY(cudaMalloc((void**)&m->totals, 4 * sizeof(double)));
+    TPMC_CUDA_TRY(cudaMalloc((void**)&m->ft_dev, 6 * sizeof(double)));
     TPMC_CUDA_TRY(cudaMalloc((void**)&m->partials, 3 * kReduceParts * sizeof(double)));
     TPMC_CUDA_TRY(cudaEventCreateWithFlags(&m->ev_fork, cudaEventDisableTiming));
     for (int pi = 0; pi < kPipes; ++pi) {
@@ -814,12 +847,9 @@ const Grids& grids() {
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     g.pipes = kPipes;
-    if (const char* e = getenv("TPMC_PIPES")) g.pipes = std::max(1, std::min(kPipes, atoi(e)));   // tuning aid
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_trace_wf, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
     // resident trace CTAs per SM over all pipelines (measured: leaving room for the seed kernel does not pay)
-    int tot = std::max(1, per);
-    if (const char* e = getenv("TPMC_TRACE_BLOCKS")) tot = std::max(1, std::min(4 * per, atoi(e)));
-    g.trace = sms * std::max(1, tot / g.pipes);
+    g.trace = sms * std::max(1, per / g.pipes);
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_reflect, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
     g.reflect = sms * std::max(1, per / g.pipes);
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_finish, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
@@ -827,11 +857,7 @@ const Grids& grids() {
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_seed, kSeedBlock, 0) != cudaSuccess || per < 1) per = 4;
     g.seed = sms * per;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_seed_precull, kPrecullBlock, 0) != cudaSuccess || per < 1) per = 4;
-    {
-      int f = 4;   // shares per resident block (evens out the tail); TPMC_PRECULL_SHARES: tuning aid
-      if (const char* e = getenv("TPMC_PRECULL_SHARES")) f = std::max(1, std::min(64, atoi(e)));
-      g.precull = sms * per * f;
-    }
+    g.precull = sms * per * 4;   // four shares per resident block (evens out the tail)
   }
   return g;
 }
@@ -841,21 +867,34 @@ int fill_stats(tpmc_mesh* m, const tpmc_params* params, tpmc_stats* h_stats) {
   TPMC_CUDA_TRY(cudaMemcpy(hs, m->stats, sizeof(hs), cudaMemcpyDeviceToHost));
   float ms = 0.0f;
   TPMC_CUDA_TRY(cudaEventElapsedTime(&ms, m->ev0, m->ev1));
+  (void)params;
+  memset(h_stats, 0, sizeof(*h_stats));
   h_stats->hits = hs[ST_HITS];
   h_stats->truncated = hs[ST_TRUNC];
-  h_stats->culled = hs[ST_CULLED];
   h_stats->tri_tests = hs[ST_TRIS];
   h_stats->node_visits = hs[ST_NODES];
-  h_stats->segments = params->count + hs[ST_HITS] - hs[ST_TRUNC];
-  h_stats->escaped = params->count - hs[ST_TRUNC];
+  h_stats->ret_precull_a = hs[ST_RET_PA];
+  h_stats->ret_precull_b = hs[ST_RET_PB];
+  h_stats->ret_seed = hs[ST_RET_SEED];
+  h_stats->ret_trace = hs[ST_RET_TRACE];
+  h_stats->ret_resolve = hs[ST_RET_RESOLVE];
+  h_stats->ret_horizon = hs[ST_RET_HORIZON];
+  h_stats->ret_finish = hs[ST_RET_FINISH];
+  h_stats->queued_primaries = hs[ST_Q_PRIM];
+  h_stats->queued_reflected = hs[ST_Q_REFL];
+  h_stats->overflow_rays = hs[ST_OVF_RETRACE] + hs[ST_OVF_PENDING] + hs[ST_DIVERTED];
+  h_stats->final_stragglers = hs[ST_STRAGGLERS];
+  h_stats->finish_segments = hs[ST_FIN_SEGS];
+  h_stats->traced_rays = hs[ST_TRACED];
+  // sums of counted events (the identities of tpmc.h hold only if no particle was lost or duplicated on the way)
+  h_stats->culled = hs[ST_RET_PA] + hs[ST_RET_PB] + hs[ST_RET_SEED];
+  h_stats->escaped = h_stats->culled + hs[ST_RET_TRACE] + hs[ST_RET_RESOLVE] + hs[ST_RET_HORIZON] + hs[ST_RET_FINISH];
+  // one segment per culled particle, per traced ray whose answer stood (a ray handed on after a candidate overflow is
+  // searched again by the straggler kernel), per horizon escape and per search of the straggler kernel
+  h_stats->segments = h_stats->culled + (hs[ST_TRACED] - hs[ST_OVF_RETRACE]) + hs[ST_RET_HORIZON] + hs[ST_FIN_SEGS];
   h_stats->kernel_launches = m->last_launches;
   h_stats->ms = ms;
-  h_stats->ms_seed = h_stats->ms_trace = h_stats->ms_reflect = h_stats->ms_finish = 0.0;
-  h_stats->timed_waves = 0;
-  h_stats->trace_launches = 0;
-  h_stats->traced_rays = hs[ST_TRACED];
-  // Kernels of different pipelines and streams overlap: these are sums of per-launch durations, not a
-  // partition of `ms`.
+  // Kernels of different streams overlap: these are sums of per-launch durations, not a partition of `ms`.
   for (int pi = 0; pi < kPipes; ++pi) {
     const Pipe& pp = m->pipe[pi];
     for (unsigned long long w = 0; w < pp.iters; ++w) {
@@ -865,16 +904,12 @@ int fill_stats(tpmc_mesh* m, const tpmc_params* params, tpmc_stats* h_stats) {
         TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[0], ev[1]));
         h_stats->ms_seed += t;
       }
-      TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[2], ev[3]));
+      TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[2], ev[7]));
+      h_stats->ms_sort += t;
+      TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[7], ev[3]));
       h_stats->ms_trace += t;
       TPMC_CUDA_TRY(cudaEventElapsedTime(&t, ev[3], ev[4]));
       h_stats->ms_reflect += t;
-      if (getenv("TPMC_TIMELINE") && w >= 4 && w < 10 && w < pp.seed_iters) {   // diagnosis: event times since the run began
-        float a[7];
-        for (int k = 0; k < 7; ++k) cudaEventElapsedTime(&a[k], m->ev0, ev[k]);
-        fprintf(stderr, "iter %llu: seed %.3f-%.3f trace %.3f-%.3f reflect -%.3f finish %.3f-%.3f\n", w, a[0], a[1], a[2], a[3], a[4],
-                a[5], a[6]);
-      }
     }
     h_stats->timed_waves += pp.seed_iters;
     h_stats->trace_launches += pp.iters;
@@ -887,58 +922,57 @@ int fill_stats(tpmc_mesh* m, const tpmc_params* params, tpmc_stats* h_stats) {
   return TPMC_OK;
 }
 
+// The flow-aligned refit pays for oblique attitudes only: bodies are usually modelled along their own axes (thin
+// panels, flat faces), and a box refitted in a tilted frame is loose around such parts; with the stream within ~25 deg
+// of a body axis the body-frame boxes are as good or better (measured on C5).  Both hierarchies give the same results.
+bool want_alignment(const tpmc_params* p) {
+  if (p->flags & TPMC_FLAG_ALIGN_OFF) return false;
+  if (p->flags & TPMC_FLAG_ALIGN_ON) return true;
+  const double vmax = std::max(std::fabs(p->V[0]), std::max(std::fabs(p->V[1]), std::fabs(p->V[2])));
+  const double vabs = std::sqrt(p->V[0] * p->V[0] + p->V[1] * p->V[1] + p->V[2] * p->V[2]);
+  return vabs > 0.0 && vmax < 0.9 * vabs;
+}
+
 }  // namespace
 
-extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* cuda_stream, double* d_force,
+extern "C" int tpmc_run(tpmc_mesh* m, const tpmc_params* params, void* cuda_stream, double* d_force,
                         double* d_torque, double* d_facet_momentum, tpmc_stats* h_stats, const tpmc_debug* debug) {
-  if (!mesh || !params || !d_force || !d_torque) return TPMC_EINVAL;
-  tpmc_mesh* m = const_cast<tpmc_mesh*>(mesh);   // the handle caches scratch
+  if (!m || !params || !d_force || !d_torque) return TPMC_EINVAL;
   RunConst rc;
   int rcode = make_run_const(m, params, &rc);
   if (rcode != TPMC_OK) return rcode;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  const size_t wave = std::min<unsigned long long>(std::max<unsigned long long>(params->count, 1), wave_size());
+  const size_t wave_req = params->wave_particles ? (size_t)params->wave_particles : kDefaultWave;
+  const size_t wave = std::min<unsigned long long>(std::max<unsigned long long>(params->count, 256), wave_req);
   rcode = ensure_scratch(m, wave, d_facet_momentum == nullptr);
   if (rcode != TPMC_OK) return rcode;
-  const unsigned int cap = (unsigned int)m->wave_cap;   // region size of the queues
+  const unsigned int cap = (unsigned int)wave;   // region size of the queues (<= the allocated m->wave_cap)
   double* P = d_facet_momentum ? d_facet_momentum : m->facet_scratch;
   tpmc_debug dbg0 = {nullptr, nullptr, nullptr};
   if (debug) dbg0 = *debug;
   const bool any_dbg = dbg0.hash || dbg0.bounces || dbg0.first_facet;
   const Grids& g = grids();
   const int K = g.pipes;
-  static const bool no_overlap = getenv("TPMC_NO_OVERLAP") != nullptr;   // diagnosis: one stream only
   const bool timed = (h_stats != nullptr);   // per-kernel events only when the caller will read them
-  const char* pc_env = getenv("TPMC_PRECULL");   // read per call: the parity tests switch the pass off and on
-  const bool precull = !(pc_env && pc_env[0] == '0');
-  const char* hz_env = getenv("TPMC_HORIZON");   // likewise: "0" switches the escape-horizon test off
-  const bool use_horizon = !(hz_env && hz_env[0] == '0');
+  const bool precull = !(params->flags & TPMC_FLAG_NO_PRECULL);
+  const bool use_horizon = !(params->flags & TPMC_FLAG_NO_HORIZON);
+  const bool exact = (params->flags & TPMC_FLAG_EXACT_TRACE) != 0;
   // seed-time walk of the top of the hierarchy: pays only while the pre-cull pass has no two-level cull volume
-  // (with it the pass is already tighter than the 64-node tree); TPMC_SEED_WALK=0/1 forces it (tuning aid)
-  const char* sw_env = getenv("TPMC_SEED_WALK");
-  const int seed_walk = sw_env ? (sw_env[0] != '0') : (m->cull_nbox < 0 || (getenv("TPMC_CULL_VOLUME") && getenv("TPMC_CULL_VOLUME")[0] == '0'));
+  // (with it the pass is already tighter than the 64-node tree)
+  const int seed_walk = m->cull_nbox < 0;
   SeedConstF sf;
   make_seed_const_f(m, rc, &sf);
   const QuantGrid qg = quant_grid(m);   // seed-time cull (body frame)
   TPMC_CUDA_TRY(cudaEventRecord(m->ev0, st));
-  // the traversal's hierarchy, refitted in the stream frame of this run (x' = R^T x: z' along the free stream)
+  // the traversal's hierarchy: body frame, or refitted in the stream frame of this run (x' = R^T x: z' along the stream)
   const QuantGrid* qg_t = m->grid_dev;
   const uint4* cnodes_t = m->cnodes;
-  {
-    static const bool no_align = getenv("TPMC_ALIGN") && getenv("TPMC_ALIGN")[0] == '0';   // tuning aid
-    // Heuristic: bodies are usually modelled along their own axes (thin panels, flat faces), and a box refitted in a
-    // tilted frame is loose around such parts; with the stream within ~25 deg of a body axis the body-frame boxes
-    // are as good or better (measured on C5), so the refit is used only for the oblique attitudes.
-    const double vmax = std::max(std::fabs(params->V[0]), std::max(std::fabs(params->V[1]), std::fabs(params->V[2])));
-    const double vabs = std::sqrt(params->V[0] * params->V[0] + params->V[1] * params->V[1] + params->V[2] * params->V[2]);
-    static const bool force_align = getenv("TPMC_ALIGN") && getenv("TPMC_ALIGN")[0] == '2';
-    if (!no_align && (force_align || (vabs > 0.0 && vmax < 0.9 * vabs))) {
-      double Rt[9];
-      for (int a = 0; a < 3; ++a)
-        for (int b2 = 0; b2 < 3; ++b2) Rt[3 * a + b2] = rc.R[3 * b2 + a];
-      rcode = tpmc_mesh_align(m, Rt, st, &qg_t, &cnodes_t);
-      if (rcode != TPMC_OK) return rcode;
-    }
+  if (!exact && want_alignment(params)) {
+    double Rt[9];
+    for (int a = 0; a < 3; ++a)
+      for (int b2 = 0; b2 < 3; ++b2) Rt[3 * a + b2] = rc.R[3 * b2 + a];
+    rcode = tpmc_mesh_align(m, Rt, st, &qg_t, &cnodes_t);
+    if (rcode != TPMC_OK) return rcode;
   }
   m->pipe[0].main = st;
   for (int pi = 0; pi < kPipes; ++pi) {
@@ -959,7 +993,7 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
   unsigned long long launches = ((any_dbg && params->count) ? 1 : 0) + (cnodes_t != m->cnodes ? 4 : 0);   // + the refit kernels
 
   // Particle indices inside the queues are 32-bit offsets into a chunk of the slice.
-  const unsigned long long kChunk = 0xF0000000ull;
+  const unsigned long long kChunk = params->chunk_particles ? params->chunk_particles : 0xF0000000ull;
   for (unsigned long long c0 = 0; c0 < params->count; c0 += kChunk) {
     const unsigned long long cn = std::min<unsigned long long>(kChunk, params->count - c0);
     RunConst rcc = rc;
@@ -974,6 +1008,7 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
     for (int pi = 0; pi < K; ++pi) {
       Pipe& pp = m->pipe[pi];
       if (pi > 0) TPMC_CUDA_TRY(cudaStreamWaitEvent(pp.main, m->ev_fork, 0));
+      // a chunk starts from empty queues; the side streams of the previous chunk have been joined
       TPMC_CUDA_TRY(cudaMemsetAsync(pp.ctr, 0, kCtrWords * sizeof(unsigned int), pp.main));
       TPMC_CUDA_TRY(cudaEventRecord(pp.ev_reset[0], pp.main));
     }
@@ -988,9 +1023,9 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
       Pipe& pp = m->pipe[wv % K];
       const unsigned long long li = wv / K;            // iteration index within the pipeline
       const int p = (int)(li & 1);
-      cudaStream_t s1 = pp.main, s2 = no_overlap ? pp.main : pp.seed, s3 = no_overlap ? pp.main : pp.side;
+      cudaStream_t s1 = pp.main, s2 = pp.seed, s3 = pp.side;
       const int b = (int)(li & 1);
-      unsigned int* ovf = pp.ovf + (size_t)b * 2 * cap;
+      unsigned int* ovf = pp.ovf + (size_t)b * 2 * m->wave_cap;
       RayQueue Q[2] = {{pp.q_o[0], pp.q_v[0], pp.q_f[0]}, {pp.q_o[1], pp.q_v[1], pp.q_f[1]}};
       const bool tw = timed && c0 == 0 && li < (unsigned long long)kMaxTimedWaves;
       cudaEvent_t* ev = tw ? pp.wave_ev + kEvPerWave * li : nullptr;
@@ -1005,7 +1040,8 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
         if (precull) {
           TPMC_CUDA_TRY(cudaMemsetAsync(pp.ctr + 6, 0, 2 * sizeof(unsigned int), s2));
           k_seed_precull<<<std::min<unsigned int>((wn + kPrecullBlock - 1) / kPrecullBlock, (unsigned int)g.precull),
-                           kPrecullBlock, 0, s2>>>(sf, rcc.seed_lo, rcc.seed_hi, rcc.first + w0, wn, cap, pp.surv, pp.ctr + 6);
+                           kPrecullBlock, 0, s2>>>(sf, rcc.seed_lo, rcc.seed_hi, rcc.first + w0, wn, cap, pp.surv, pp.ctr + 6,
+                                                   m->stats);
           ++launches;
         }
         k_seed<<<std::min<unsigned int>(gfull, (unsigned int)g.seed), kSeedBlock, 0, s2>>>(
@@ -1016,30 +1052,40 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
         if (tw) pp.seed_iters = li + 1;
         ++launches;
       }
+      // (without a reflect step nothing else orders this iteration behind the straggler kernel that still reads list b)
+      if (exact && li >= 2) TPMC_CUDA_TRY(cudaStreamWaitEvent(s1, pp.ev_ovf[b], 0));
       k_iter_begin<<<1, 32, 0, s1>>>(pp.ctr, p ^ 1, b);
       TPMC_CUDA_TRY(cudaEventRecord(pp.ev_reset[(li + 1) & 3], s1));
       if (wv < n_waves) TPMC_CUDA_TRY(cudaStreamWaitEvent(s1, pp.ev_seeded[li & 3], 0));
       if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[2], s1));
-      k_trace_wf<<<g.trace, kTraceBlock, 0, s1>>>(cnodes_t, qg_t, m->tris, Q[p], cap, pp.ctr + 2 * p, pp.ctr + 4, pp.hit_ray,
-                                                  pp.hit_cand, pp.ctr + 5, m->stats, trace_tune());
-      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[3], s1));
-      // the straggler kernel of the previous iteration reads the queue this reflect step writes
-      if (li >= 1) TPMC_CUDA_TRY(cudaStreamWaitEvent(s1, pp.ev_ovf[b ^ 1], 0));
-      k_reflect<<<g.reflect, kTraceBlock, 0, s1>>>(rcc, cap, m->tris, Q[p], pp.hit_ray, pp.hit_cand, pp.ctr + 5, Q[p ^ 1],
-                                                   pp.ctr + 2 * (p ^ 1), ovf, pp.ctr + 8 + b, P, m->totals, m->stats, dbg,
-                                                   use_horizon ? m->horizon : nullptr);
+      if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[7], s1));
+      if (!exact) {
+        k_trace_wf<<<g.trace, kTraceBlock, 0, s1>>>(cnodes_t, qg_t, m->tris, Q[p], cap, pp.ctr + 2 * p, pp.ctr + 4, pp.hit_ray,
+                                                    pp.hit_cand, pp.ctr + 5, m->stats, trace_tune());
+        if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[3], s1));
+        // the straggler kernel of the previous iteration reads the queue this reflect step writes
+        if (li >= 1) TPMC_CUDA_TRY(cudaStreamWaitEvent(s1, pp.ev_ovf[b ^ 1], 0));
+        k_reflect<<<g.reflect, kTraceBlock, 0, s1>>>(rcc, cap, m->tris, Q[p], pp.hit_ray, pp.hit_cand, pp.ctr + 5, Q[p ^ 1],
+                                                     pp.ctr + 2 * (p ^ 1), ovf, pp.ctr + 8 + b, P, m->totals, m->stats, dbg,
+                                                     use_horizon ? m->horizon : nullptr);
+        launches += 2;
+      } else {
+        if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[3], s1));
+        k_divert<<<296, 256, 0, s1>>>(cap, pp.ctr + 2 * p, ovf, pp.ctr + 8 + b, m->stats);
+        ++launches;
+      }
       if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[4], s1));
       // overflow list of this iteration: followed to escape on the side stream, beside the next traversal
       TPMC_CUDA_TRY(cudaEventRecord(pp.ev_refl[b], s1));
       TPMC_CUDA_TRY(cudaStreamWaitEvent(s3, pp.ev_refl[b], 0));
       if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[5], s3));
-      k_finish<<<g.finish / 4, kTraceBlock, 0, s3>>>(rcc, cap, m->nodes, m->tris, Q[p], ovf, pp.ctr + 8 + b, P, m->totals,
-                                                     m->stats, dbg, use_horizon ? m->horizon : nullptr);
+      k_finish<<<exact ? g.finish : g.finish / 4, kTraceBlock, 0, s3>>>(rcc, cap, m->nodes, m->tris, Q[p], ovf, pp.ctr + 8 + b, P,
+                                                                        m->totals, m->stats, dbg, use_horizon ? m->horizon : nullptr);
       if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[6], s3));
       TPMC_CUDA_TRY(cudaEventRecord(pp.ev_ovf[b], s3));
       pp.last_iter = li;
       if (tw) pp.iters = li + 1;
-      launches += 5;
+      launches += 2;
     }
     // whatever still bounces after the drain iterations is followed to escape thread by thread; then join
     for (int pi = 0; pi < K; ++pi) {
@@ -1073,39 +1119,27 @@ extern "C" int tpmc_run(const tpmc_mesh* mesh, const tpmc_params* params, void* 
   return TPMC_OK;
 }
 
-extern "C" int tpmc_run_host(const tpmc_mesh* mesh, const tpmc_params* params, void* cuda_stream, double* h_force,
+extern "C" int tpmc_run_host(tpmc_mesh* m, const tpmc_params* params, void* cuda_stream, double* h_force,
                              double* h_torque, double* h_facet_momentum, tpmc_stats* h_stats) {
-  if (!mesh || !params || !h_force || !h_torque) return TPMC_EINVAL;
+  if (!m || !params || !h_force || !h_torque) return TPMC_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  tpmc_mesh* m = const_cast<tpmc_mesh*>(mesh);
-  double* d_ft = nullptr;
-  TPMC_CUDA_TRY(cudaMalloc((void**)&d_ft, 6 * sizeof(double)));
-  int rc = TPMC_OK;
-  if (h_facet_momentum && !m->facet_scratch) {
-    cudaError_t e = cudaMalloc((void**)&m->facet_scratch, 3 * sizeof(double) * (size_t)m->nt);
-    if (e != cudaSuccess) { cudaFree(d_ft); cudaGetLastError(); return TPMC_ENOMEM; }
-  }
+  int rc = ensure_scratch(m, std::max<size_t>(m->wave_cap, 256), h_facet_momentum != nullptr);   // allocates ft_dev, facet_scratch
+  if (rc != TPMC_OK) return rc;
   tpmc_stats tmp_stats;
-  rc = tpmc_run(mesh, params, cuda_stream, d_ft, d_ft + 3, h_facet_momentum ? m->facet_scratch : nullptr,
+  rc = tpmc_run(m, params, cuda_stream, m->ft_dev, m->ft_dev + 3, h_facet_momentum ? m->facet_scratch : nullptr,
                 h_stats ? &tmp_stats : nullptr, nullptr);
-  if (rc == TPMC_OK) {
-    double ft[6];
-    cudaError_t e = cudaMemcpyAsync(ft, d_ft, sizeof(ft), cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && h_facet_momentum)
-      e = cudaMemcpyAsync(h_facet_momentum, m->facet_scratch, 3 * sizeof(double) * (size_t)m->nt,
-                          cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) {
-      snprintf(g_tpmc_cuda_error, sizeof(g_tpmc_cuda_error), "tpmc_run_host: %s", cudaGetErrorString(e));
-      rc = TPMC_ECUDA;
-    } else {
-      for (int a = 0; a < 3; ++a) { h_force[a] = ft[a]; h_torque[a] = ft[3 + a]; }
-      if (h_stats) *h_stats = tmp_stats;
-    }
-  }
-  cudaFree(d_ft);
-  return rc;
+  if (rc != TPMC_OK) return rc;
+  double ft[6];
+  TPMC_CUDA_TRY(cudaMemcpyAsync(ft, m->ft_dev, sizeof(ft), cudaMemcpyDeviceToHost, st));
+  if (h_facet_momentum)
+    TPMC_CUDA_TRY(cudaMemcpyAsync(h_facet_momentum, m->facet_scratch, 3 * sizeof(double) * (size_t)m->nt,
+                                  cudaMemcpyDeviceToHost, st));
+  TPMC_CUDA_TRY(cudaStreamSynchronize(st));
+  for (int a = 0; a < 3; ++a) { h_force[a] = ft[a]; h_torque[a] = ft[3 + a]; }
+  if (h_stats) *h_stats = tmp_stats;
+  return TPMC_OK;
 }
+
 
 extern "C" int tpmc_seed(const tpmc_mesh* mesh, const tpmc_params* params, void* cuda_stream, double* d_x, double* d_v,
                          int32_t* d_species) {
@@ -1119,24 +1153,33 @@ extern "C" int tpmc_seed(const tpmc_mesh* mesh, const tpmc_params* params, void*
   return TPMC_OK;
 }
 
-extern "C" int tpmc_trace(const tpmc_mesh* mesh, const float* d_o, const float* d_d, const int32_t* d_f_prev, int64_t n,
-                          void* cuda_stream, int32_t* d_facet, double* d_tau) {
-  if (!mesh || !d_o || !d_d || !d_facet || !d_tau || n < 0 || n > 0x7FFFFFFF) return TPMC_EINVAL;
+extern "C" int tpmc_trace(tpmc_mesh* m, const float* d_o, const float* d_d, const int32_t* d_f_prev, int64_t n,
+                          const double* h_align_V, void* cuda_stream, int32_t* d_facet, double* d_tau) {
+  if (!m || !d_o || !d_d || !d_facet || !d_tau || n < 0 || n > 0x7FFFFFFF) return TPMC_EINVAL;
   if (n == 0) return TPMC_OK;
-  tpmc_mesh* m = const_cast<tpmc_mesh*>(mesh);
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  int rcode = ensure_scratch(m, std::max<size_t>(((size_t)n + 1) / 2, m->wave_cap), false);
+  int rcode = ensure_scratch(m, std::max<size_t>(((size_t)n + 1) / 2, std::max<size_t>(m->wave_cap, 256)), false);
   if (rcode != TPMC_OK) return rcode;
   const Grids& g = grids();
   Pipe& pp = m->pipe[0];
   RayQueue q = {pp.q_o[0], pp.q_v[0], pp.q_f[0]};
   const unsigned int un = (unsigned int)n;
+  const QuantGrid* qg_t = m->grid_dev;
+  const uint4* cnodes_t = m->cnodes;
+  if (h_align_V) {   // the hierarchy refitted in the stream frame of this velocity, as tpmc_run uses it
+    double R[9], Rt[9];
+    host_rotation(h_align_V, R);
+    for (int a = 0; a < 3; ++a)
+      for (int b2 = 0; b2 < 3; ++b2) Rt[3 * a + b2] = R[3 * b2 + a];
+    rcode = tpmc_mesh_align(m, Rt, st, &qg_t, &cnodes_t);
+    if (rcode != TPMC_OK) return rcode;
+  }
   TPMC_CUDA_TRY(cudaMemsetAsync(pp.ctr, 0, kCtrWords * sizeof(unsigned int), st));
   TPMC_CUDA_TRY(cudaMemcpyAsync(pp.ctr, &un, sizeof(un), cudaMemcpyHostToDevice, st));   // region A holds the rays
   TPMC_CUDA_TRY(cudaMemsetAsync(m->stats, 0, ST_COUNT * sizeof(unsigned long long), st));
   k_pack_rays<<<(un + 255) / 256, 256, 0, st>>>(d_o, d_d, d_f_prev, un, q, d_facet, d_tau);
   // the production traversal (fp32 wavefront + candidate lists), then the exact fp64 resolve
-  k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(m->cnodes, m->grid_dev, m->tris, q, (unsigned int)(2 * m->wave_cap), pp.ctr, pp.ctr + 4,
+  k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(cnodes_t, qg_t, m->tris, q, (unsigned int)(2 * m->wave_cap), pp.ctr, pp.ctr + 4,
                                               pp.hit_ray, pp.hit_cand, pp.ctr + 5, m->stats, trace_tune());
   k_resolve_only<<<g.reflect, kTraceBlock, 0, st>>>(m->nodes, m->tris, q, pp.hit_ray, pp.hit_cand, pp.ctr + 5, d_facet,
                                                     d_tau);

@@ -186,9 +186,10 @@ __device__ __forceinline__ bool slab(float lx, float ly, float lz, float hx, flo
 //   * id = 1/d' carries <= 5u relative (rounded inv_scale, product, 2-ulp reciprocal), which scales the
 //     distance |P - O| <= |o'| + 2^16 steps; the final FFMA rounds once more, u relative;
 //   * the rounded inv_scale moves a plane by <= u q <= 0.004 steps.
-// Sum <= 2u|O| + 9u|o'| + 0.03 (+ 0.06 for the rotation into an aligned frame, see grid_ray);
-// G_k = 2.5u|O| + 10u|o'| + 0.25 (about 1.5 steps of the 16-bit grid for an origin
-// inside or near the grid; it scales with the origin for a ray that starts far outside, e.g. on a flat axis).
+// Sum <= 2u|O| + 9u|o'| + 0.03, plus the rotation into an aligned frame (see grid_ray), which is an error in METRES
+// and therefore enters per axis as E_rot * inv_scale_k steps (large in steps, tiny in metres, on an axis along which
+// the body is thin);  G_k = 2.5u|O| + 10u|o'| + 0.25 + E_rot * inv_scale_k (about 1.5 steps of the 16-bit grid for an
+// origin inside or near the grid; it scales with the origin for a ray that starts far outside, e.g. on a flat axis).
 // A zero direction component gives id = inf and NaN plane distances, which fminf/fmaxf drop: the axis then
 // does not constrain the ray (conservative).
 __device__ __forceinline__ float q_plane(unsigned int w, unsigned int sel) {
@@ -209,11 +210,15 @@ struct GridRay {
   unsigned int sn[3], sf[3];
 };
 __device__ __forceinline__ void grid_ray(GridRay& r, const QuantGrid& g, const float o[3], const float d[3]) {
-  // into the frame of the grid (x' = R x; R = identity for the body-frame hierarchy, where this is exact).  The
-  // rotation adds an absolute error of <= 3u (|o|_1, |d|_1) to o' and d'.  For o' that is < 0.02 grid steps.  For d'
-  // it displaces the ray, over its whole path through the grid (< 1.2e5 steps), by < 3u * 1.2e5 * sqrt(3) = 0.04
-  // steps along any axis, however small that component of d' is.  Both are in the constant part of G below.
+  // into the frame of the grid (x' = R x; R = identity for the body-frame hierarchy, where this is exact: g.rot_* = 0).
+  // The fp32 rotation adds an absolute error of <= 3u |o|_1 to each component of o' and <= 3u |d|_1 to each of d'.  At
+  // parameter t the rotated ray is therefore within 3u (|o|_1 + t |d|_1) METRES of the exact one along every axis, and
+  // while the ray is inside the root box t |d|_1 <= sqrt(3) t |d| <= sqrt(3) (|o| + reach), reach = the largest |x| in
+  // the box: E_rot <= 3u (1 + sqrt 3) |o|_1 + 3 sqrt(3) u reach < 9u |o|_1 + 6u reach = g.rot_o |o|_1 + g.rot_c.  A box
+  // that the exact ray enters at t is entered at t by the rotated ray once grown by E_rot: in grid steps of axis k that
+  // is E_rot * inv_scale_k, whatever the extent of the body along that axis.
   float og[3], dg[3];
+  const float e_rot = fmaf(g.rot_o, fabsf(o[0]) + fabsf(o[1]) + fabsf(o[2]), g.rot_c) * 1.000001f;
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
     og[k] = fmaf(g.R[3 * k + 2], o[2], fmaf(g.R[3 * k + 1], o[1], g.R[3 * k] * o[0]));
@@ -225,7 +230,7 @@ __device__ __forceinline__ void grid_ray(GridRay& r, const QuantGrid& g, const f
     const float idk = __fdividef(1.0f, dq);                  // 2 ulp
     const float oq = (og[k] - g.origin[k]) * g.inv_scale[k];
     const float O = 8388608.0f + oq;
-    const float G = fmaf(1.4901161e-07f, fabsf(O), fmaf(5.9604645e-07f, fabsf(oq), 0.25f));   // 2.5u|O| + 10u|o'| + 0.25
+    const float G = fmaf(1.4901161e-07f, fabsf(O), fmaf(5.9604645e-07f, fabsf(oq), fmaf(e_rot, g.inv_scale[k], 0.25f)));   // 2.5u|O| + 10u|o'| + 0.25 + E_rot
     const float mg = G * fabsf(idk);
     r.id[k] = idk;
     r.ncn[k] = fmaf(-O, idk, -mg);

@@ -49,15 +49,28 @@ def test_sass_is_sm100a(libpath):
 def test_struct_layouts_match_header(libpath, tmp_path):
     import paper_1312_3691_b200 as t
     prog = tmp_path / "sz.c"
-    prog.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "tpmc.h"\nint main(){printf("%zu %zu %zu %zu %zu %zu %zu\\n",'
+    prog.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "tpmc.h"\nint main(){printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\\n",'
                     "sizeof(tpmc_params),sizeof(tpmc_stats),sizeof(tpmc_debug),sizeof(tpmc_mesh_info_t),"
-                    "offsetof(tpmc_params,N),offsetof(tpmc_params,x_ref),offsetof(tpmc_mesh_info_t,nt));return 0;}\n")
+                    "offsetof(tpmc_params,N),offsetof(tpmc_params,x_ref),offsetof(tpmc_mesh_info_t,nt),"
+                    "offsetof(tpmc_params,flags),offsetof(tpmc_params,control_volume),offsetof(tpmc_stats,ret_precull_a),"
+                    "offsetof(tpmc_stats,ms_sort));return 0;}\n")
     exe = tmp_path / "sz"
     subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), str(prog), "-o", str(exe)], check=True)
     got = [int(x) for x in subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()]
     want = [C.sizeof(t.tpmc_params), C.sizeof(t.tpmc_stats), C.sizeof(t.tpmc_debug), C.sizeof(t.tpmc_mesh_info_t),
-            t.tpmc_params.N.offset, t.tpmc_params.x_ref.offset, t.tpmc_mesh_info_t.nt.offset]
+            t.tpmc_params.N.offset, t.tpmc_params.x_ref.offset, t.tpmc_mesh_info_t.nt.offset,
+            t.tpmc_params.flags.offset, t.tpmc_params.control_volume.offset, t.tpmc_stats.ret_precull_a.offset,
+            t.tpmc_stats.ms_sort.offset]
     assert got == want
+    assert (t.TPMC_FLAG_NO_PRECULL, t.TPMC_FLAG_NO_HORIZON, t.TPMC_FLAG_ALIGN_OFF, t.TPMC_FLAG_ALIGN_ON,
+            t.TPMC_FLAG_EXACT_TRACE, t.TPMC_FLAG_NO_SORT) == (1, 2, 4, 8, 16, 32)
+
+
+def test_library_reads_no_environment_variable():
+    """Behaviour is selected through tpmc_params only (include/tpmc.h conventions)."""
+    csrc = os.path.join(ROOT, "paper_1312_3691_b200", "csrc")
+    for f in os.listdir(csrc):
+        assert "getenv" not in open(os.path.join(csrc, f)).read(), f
 
 
 def test_error_strings_and_null_arguments(libpath):

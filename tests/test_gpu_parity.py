@@ -41,9 +41,26 @@ def meshes(T, O, cfg):
     return _mesh_cache[key]
 
 
-def compare_run(T, O, cfg, first, count, use_bvh=True):
+def check_conservation(st, count, exact=False):
+    """tpmc_stats counts every event where it happens (include/tpmc.h): a particle lost or duplicated between the
+    pre-cull lists, the two queue regions, the hit list, the overflow lists and the straggler kernel breaks these."""
+    retired = (st["truncated"] + st["ret_precull_a"] + st["ret_precull_b"] + st["ret_seed"] + st["ret_trace"]
+               + st["ret_resolve"] + st["ret_horizon"] + st["ret_finish"])
+    assert retired == count, (retired, count, st)
+    assert st["escaped"] == count - st["truncated"]
+    assert st["segments"] == count + st["hits"] - st["truncated"], st
+    assert st["culled"] == st["ret_precull_a"] + st["ret_precull_b"] + st["ret_seed"]
+    assert st["queued_primaries"] == count - st["culled"]
+    if exact:
+        assert st["traced_rays"] == 0 and st["overflow_rays"] == st["queued_primaries"]
+    else:
+        assert st["traced_rays"] + st["final_stragglers"] == st["queued_primaries"] + st["queued_reflected"], st
+
+
+def compare_run(T, O, cfg, first, count, use_bvh=True, **run_kw):
     gm, om = meshes(T, O, cfg)
-    g = gm.run(cfg, first=first, count=count, debug=True)
+    g = gm.run(cfg, first=first, count=count, debug=True, **run_kw)
+    check_conservation(g.stats, count, exact=bool(run_kw.get("flags", 0) & T.TPMC_FLAG_EXACT_TRACE))
     o = om.run(cfg, first=first, count=count, use_bvh=use_bvh)
     gh = g.hash.cpu().numpy().view(np.uint64)
     same = gh == o.hash
@@ -231,6 +248,11 @@ def test_trace_parity_bit_exact(T, O, mesh_fn, bvh):
         else:
             assert np.isinf(tau[r])
     assert nh > 100
+    # the same rays on the hierarchy refitted in a stream frame (what tpmc_run walks at oblique attitudes): the
+    # boxes differ, the answers must not
+    for V in ((-3000.0, 5200.0, -4100.0), (100.0, -7000.0, 2500.0)):
+        fa, ta = gm.trace(o, d, fprev, align_V=V)
+        assert np.array_equal(fa.cpu().numpy(), facet) and np.array_equal(ta.cpu().numpy(), tau)
 
 
 def test_trace_tie_and_sidedness_rules(T):
@@ -305,7 +327,8 @@ def test_slices_are_additive_and_runs_repeat(T, O):
     again = gm.run(cfg, debug=True)
     assert np.allclose(again.force.cpu().numpy(), F, rtol=1e-12)        # fp64 atomic order only (A20)
     # wave boundaries do not matter: a run spanning several waves equals its one-wave slices
-    assert full.stats["segments"] == cfg.N + full.stats["hits"] - full.stats["truncated"]
+    for r, n in ((full, cfg.N), (a, 150_000), (b, 250_000), (again, cfg.N)):
+        check_conservation(r.stats, n)
 
 
 def test_edge_cases_empty_truncated_host_buffers(T, O):
@@ -352,17 +375,18 @@ def test_run_on_side_stream(T, O):
 # ------------------------------------------------------------------ a2: the fp32 pre-cull pass drops only misses
 @pytest.mark.parametrize("name,idx,count", [("C1", 0, 100_000), ("C2", 0, 3_000_000), ("C2", 2, 3_000_000),
                                              ("C3", 1, 3_000_000), ("C4", 5, 3_000_000), ("C5", 3, 20_000_000)])
-def test_precull_pass_changes_nothing(T, name, idx, count, monkeypatch):
+def test_precull_pass_changes_nothing(T, name, idx, count):
     """The pre-cull pass may only drop particles whose first segment misses the body: with the pass switched
-    off (TPMC_PRECULL=0, every particle through the fp64 sampler) hits, hashes and per-facet sums are identical."""
+    off (TPMC_FLAG_NO_PRECULL, every particle through the fp64 sampler) hits, hashes and per-facet sums are identical."""
     cfg = ti.config(name)[idx]
     m = cfg.mesh()
     gm = T.Mesh(m.vertices, m.indices, m.flags)
     first = min(cfg.N - count, 777_777)
-    monkeypatch.setenv("TPMC_PRECULL", "1")
     a = gm.run(cfg, first=first, count=count, debug=True)
-    monkeypatch.setenv("TPMC_PRECULL", "0")
-    b = gm.run(cfg, first=first, count=count, debug=True)
+    b = gm.run(cfg, first=first, count=count, debug=True, flags=T.TPMC_FLAG_NO_PRECULL)
+    check_conservation(a.stats, count)
+    check_conservation(b.stats, count)
+    assert b.stats["ret_precull_a"] == 0 and b.stats["ret_precull_b"] == 0
     assert a.stats["hits"] == b.stats["hits"] and a.stats["hits"] > 0
     assert a.stats["kernel_launches"] > b.stats["kernel_launches"]          # the pass really ran in `a` only
     assert bool((a.hash == b.hash).all()) and bool((a.first_facet == b.first_facet).all())
@@ -376,18 +400,19 @@ def test_precull_pass_changes_nothing(T, name, idx, count, monkeypatch):
 @pytest.mark.parametrize("name,idx,count", [("C1", 0, 100_000), ("C2", 1, 3_000_000), ("C3", 1, 3_000_000),
                                              ("C4", 0, 3_000_000), ("C4", 9, 3_000_000), ("C5", 3, 20_000_000),
                                              ("C5", 40, 20_000_000)])
-def test_escape_horizon_changes_nothing(T, name, idx, count, monkeypatch):
+def test_escape_horizon_changes_nothing(T, name, idx, count):
     """A re-emitted ray above its facet's escape horizon (k_horizon, lbvh.cu) is not traced: with the test
-    switched off (TPMC_HORIZON=0, every reflected ray traced) hits, hashes, bounce counts and forces are identical,
-    and with it on fewer rays reach the traversal."""
+    switched off (TPMC_FLAG_NO_HORIZON, every reflected ray traced) hits, hashes, bounce counts and forces are
+    identical, and with it on fewer rays reach the traversal."""
     cfg = ti.config(name)[idx]
     m = cfg.mesh()
     gm = T.Mesh(m.vertices, m.indices, m.flags)
     first = min(cfg.N - count, 1_234_567)
-    monkeypatch.setenv("TPMC_HORIZON", "1")
     a = gm.run(cfg, first=first, count=count, debug=True)
-    monkeypatch.setenv("TPMC_HORIZON", "0")
-    b = gm.run(cfg, first=first, count=count, debug=True)
+    b = gm.run(cfg, first=first, count=count, debug=True, flags=T.TPMC_FLAG_NO_HORIZON)
+    check_conservation(a.stats, count)
+    check_conservation(b.stats, count)
+    assert b.stats["ret_horizon"] == 0
     assert a.stats["hits"] == b.stats["hits"] and a.stats["hits"] > 0
     assert bool((a.hash == b.hash).all()) and bool((a.bounces == b.bounces).all())
     Fa, Fb = a.force.cpu().numpy(), b.force.cpu().numpy()
@@ -456,6 +481,7 @@ def test_c5_whole_stream_in_one_run_sampled_against_the_oracle(T, O):
     gm, om = meshes(T, O, cfg)
     g = gm.run(cfg, debug=True)
     st = g.stats
+    check_conservation(st, cfg.N)
     assert st["truncated"] == 0 and st["segments"] == cfg.N + st["hits"]
     assert 0.15 * cfg.N < st["hits"] < 0.20 * cfg.N
     fm = g.facet_momentum
@@ -505,6 +531,7 @@ def test_repeated_multi_wave_runs_agree(T, O):
     ref = None
     for _ in range(4):
         r = gm.run(cfg, first=100_000_000, count=200_000_000, facets=False)
+        check_conservation(r.stats, 200_000_000)
         cur = (r.stats["hits"], r.stats["segments"], r.stats["truncated"], r.force.cpu().numpy(), r.torque.cpu().numpy())
         if ref is None:
             ref = cur
@@ -512,3 +539,189 @@ def test_repeated_multi_wave_runs_agree(T, O):
         assert cur[:3] == ref[:3]
         assert np.linalg.norm(cur[3] - ref[3]) <= 1e-12 * np.linalg.norm(ref[3])
         assert np.linalg.norm(cur[4] - ref[4]) <= 1e-11 * max(np.linalg.norm(ref[4]), 1e-3 * np.linalg.norm(ref[3]))
+
+
+# ------------------------------------------------------------------ the flow-aligned hierarchy changes nothing
+def thin_plate_cfg():
+    """A two-sided plate whose normal lies along an oblique stream: in the stream frame the body has (almost) no
+    extent along z', the case in which the rotation error of the traversal's slab margin, a length in metres, is
+    thousands of steps of that axis' quantisation grid (trace.cuh, grid_ray)."""
+    n = np.array([0.48, -0.62, 0.62])
+    n /= np.linalg.norm(n)
+    a = np.cross(n, [0.0, 0.0, 1.0]); a /= np.linalg.norm(a)
+    b = np.cross(n, a)
+    c = np.array([3.0, -2.0, 1.5])              # far from the origin: large |o|_1
+    v = np.array([c - 0.5 * a - 0.5 * b, c + 0.5 * a - 0.5 * b, c + 0.5 * a + 0.5 * b, c - 0.5 * a + 0.5 * b])
+    m = ti.Mesh(v.astype(np.float32), np.int32([[0, 1, 2], [0, 2, 3]]), np.uint8([1, 1]), "oblique_plate")
+    return ti.RunConfig("thin", lambda: m, V=tuple(-7500.0 * n), N=400_000, seed=31, label="plate normal to an oblique stream")
+
+
+@pytest.mark.parametrize("name,idx,count", [("C1", 0, 100_000), ("thin", 0, 400_000), ("C2", 1, 2_000_000), ("C3", 1, 2_000_000),
+                                             ("C4", 6, 3_000_000), ("C4", 15, 3_000_000), ("C5", 3, 10_000_000),
+                                             ("C5", 30, 10_000_000)])
+def test_flow_alignment_changes_nothing(T, O, name, idx, count):
+    """tpmc_run walks either the body-frame hierarchy or its refit in the stream frame (heuristic on the attitude);
+    forced one way and the other (TPMC_FLAG_ALIGN_OFF / _ON), hashes, bounce counts and forces are identical."""
+    cfg = thin_plate_cfg() if name == "thin" else ti.config(name)[idx]
+    m = cfg.mesh()
+    gm = T.Mesh(m.vertices, m.indices, m.flags)
+    first = min(cfg.N - count, 2_345_678)
+    a = gm.run(cfg, first=first, count=count, debug=True, flags=T.TPMC_FLAG_ALIGN_OFF)
+    b = gm.run(cfg, first=first, count=count, debug=True, flags=T.TPMC_FLAG_ALIGN_ON)
+    check_conservation(a.stats, count)
+    check_conservation(b.stats, count)
+    assert a.stats["hits"] == b.stats["hits"] > 0
+    assert b.stats["kernel_launches"] > a.stats["kernel_launches"]          # the refit really ran in `b` only
+    assert bool((a.hash == b.hash).all()) and bool((a.bounces == b.bounces).all()) and bool((a.first_facet == b.first_facet).all())
+    Fa, Fb = a.force.cpu().numpy(), b.force.cpu().numpy()
+    assert np.linalg.norm(Fa - Fb) <= 1e-12 * np.linalg.norm(Fb)
+    if name == "thin":                          # and against the oracle, on the aligned hierarchy
+        compare_run(T, O, cfg, 0, 100_000, use_bvh=False, flags=T.TPMC_FLAG_ALIGN_ON)
+    gm.close()
+
+
+# ------------------------------------------------------------------ the fp32 filter + candidate lists change nothing
+@pytest.mark.parametrize("name,idx,count", [("C1", 0, 100_000), ("C2", 2, 2_000_000), ("C3", 2, 2_000_000), ("C4", 3, 2_000_000),
+                                             ("C5", 17, 4_000_000)])
+def test_exact_trace_arm_changes_nothing(T, name, idx, count):
+    """TPMC_FLAG_EXACT_TRACE sends every segment through the fp64 closest-hit search of the straggler kernel (no
+    wavefront traversal, no fp32 classification, no candidate lists): same hashes, bounces, forces."""
+    cfg = ti.config(name)[idx]
+    m = cfg.mesh()
+    gm = T.Mesh(m.vertices, m.indices, m.flags)
+    first = min(cfg.N - count, 3_456_789)
+    a = gm.run(cfg, first=first, count=count, debug=True)
+    b = gm.run(cfg, first=first, count=count, debug=True, flags=T.TPMC_FLAG_EXACT_TRACE)
+    check_conservation(a.stats, count)
+    check_conservation(b.stats, count, exact=True)
+    assert a.stats["hits"] == b.stats["hits"] > 0
+    assert bool((a.hash == b.hash).all()) and bool((a.bounces == b.bounces).all()) and bool((a.first_facet == b.first_facet).all())
+    Fa, Fb = a.force.cpu().numpy(), b.force.cpu().numpy()
+    assert np.linalg.norm(Fa - Fb) <= 1e-12 * np.linalg.norm(Fb)
+    gm.close()
+
+
+# ------------------------------------------------------------------ rare paths of tpmc_run, each forced
+def test_candidate_overflow_inside_a_run(T, O):
+    """Six coincident copies of every facet: each hit is a six-way tie, the traversal's four-slot candidate list
+    overflows, the ray goes to the overflow list and the straggler kernel resolves it (A12: smallest index)."""
+    cfg = ti.RunConfig("dup", lambda: ti.stacked_duplicates(6), N=200_000, seed=41, label="six coincident copies")
+    g, o, frac = compare_run(T, O, cfg, 0, cfg.N, use_bvh=False)
+    assert frac == 1.0 and g.stats["overflow_rays"] >= o.hits // 2 > 1000
+    assert set(np.unique(o.first_facet)) <= {-1, 0, 1}
+
+
+def test_traversal_stack_overflow_inside_a_run(T, O):
+    """A hierarchy about 28 levels deep whose boxes a ray along +x all overlaps: the 24-entry shared-memory stack
+    of the wavefront traversal gives up and the straggler kernel (deep stack) takes the ray."""
+    cfg = ti.RunConfig("chain", lambda: ti.deep_chain(), V=(7500.0, 0.0, 0.0), N=100_000, seed=42, label="deep chain")
+    g, o, frac = compare_run(T, O, cfg, 0, cfg.N, use_bvh=False)
+    assert frac == 1.0 and g.stats["overflow_rays"] > 1000
+    assert g.stats["truncated"] == o.truncated
+
+
+def test_full_reflected_region_tiny_waves_and_untimed_iterations(T, O):
+    """A hollow box with a small opening keeps particles bouncing (chains of > 100 reflections): with waves of 256
+    particles the reflected rays outgrow region A of the queue (write-back into the ray's own slot + overflow list),
+    and the run has more iterations than the per-kernel timing events cover."""
+    cfg = ti.RunConfig("pot", lambda: ti.lobster_pot(), N=300_000, seed=43, label="lobster pot")
+    g, o, frac = compare_run(T, O, cfg, 0, cfg.N, wave_particles=256)
+    assert frac == 1.0 and int(o.bounces.max()) > 100
+    assert g.stats["overflow_rays"] > 0 and g.stats["trace_launches"] == 1024 and g.stats["timed_waves"] == 1024
+    big = meshes(T, O, cfg)[0].run(cfg, debug=True)                       # one wave: same answers
+    assert bool((big.hash == g.hash).all()) and big.stats["overflow_rays"] == 0
+
+
+def test_index_chunks(T, O):
+    """Queues carry 32-bit particle offsets into a chunk of the slice; with a small chunk_particles the chunk loop
+    of tpmc_run (otherwise reached only beyond 4.0e9 particles) runs several times."""
+    cfg = ti.config("C4")[7].with_(N=1_000_000)
+    g, o, frac = compare_run(T, O, cfg, 123_456, 250_000, chunk_particles=100_000, wave_particles=40_000)
+    assert frac == 1.0
+
+
+def test_torque_about_an_off_centre_reference_point(T, O):
+    """A14 on the GPU: x_ref != 0 against the oracle (whose torque is pinned by P16), and the shift identity."""
+    cfg = ti.config("C4")[9].with_(N=400_000, x_ref=(0.3, -0.2, 0.5))
+    g, o, _ = compare_run(T, O, cfg, 0, 200_000)
+    assert np.linalg.norm(o.torque) > 1e-2 * np.linalg.norm(o.force)
+    gm, _ = meshes(T, O, cfg)
+    z = gm.run(cfg.with_(x_ref=(0.0, 0.0, 0.0)), first=0, count=200_000)
+    F, t0, t1 = g.force.cpu().numpy(), z.torque.cpu().numpy(), g.torque.cpu().numpy()
+    assert np.linalg.norm(t1 - (t0 - np.cross(cfg.x_ref, F))) <= 1e-10 * (np.linalg.norm(t0) + np.linalg.norm(F))
+
+
+def test_equilibrium_through_the_whole_path(T, O):
+    """P10 through tpmc_run: V = 0, T_W = T_inf on the pocket satellite (S = 0: the series branch of the position
+    CDF, no certified pre-cull, degenerate rotation and alignment).  Parity with the oracle on the same stream, and
+    the physics on a GPU-sized sample: zero net force on a closed solid, P_f = -n k_B T A_f n_f inside the pocket."""
+    mfn = lambda: ti.satellite(seed=2, h=0.25)
+    cfg = ti.RunConfig("eq", mfn, T_inf=500.0, T_W=500.0, V=(0.0, 0.0, 0.0), N=20_000_000, seed=5, cv_radius_factor=1.05,
+                       label="equilibrium")
+    g, o, frac = compare_run(T, O, cfg, 0, 150_000)
+    assert frac >= SEQ_AGREE and int(o.bounces.max()) >= 3
+    gm, _ = meshes(T, O, cfg)
+    per = cfg.N // 8
+    runs = [gm.run(cfg, first=k * per, count=per) for k in range(8)]
+    Fs = np.array([r.force.cpu().numpy() for r in runs]) * 8
+    m = cfg.mesh()
+    tri = m.triangles()
+    Ng = np.cross(tri[:, 1] - tri[:, 0], tri[:, 2] - tri[:, 0])
+    A = 0.5 * np.linalg.norm(Ng, axis=1)
+    nh = Ng / (2 * A)[:, None]
+    p = cfg.n * ti.K_B * cfg.T_inf
+    scale = p * A.sum()
+    assert np.all(np.abs(Fs.mean(0)) < 4 * Fs.std(0, ddof=1) / np.sqrt(8) + 1e-9 * scale)
+    cen = tri.mean(1)
+    floor = (np.abs(cen[:, 2] - 0.5) < 1e-6) & (np.abs(cen[:, 0]) < 0.31) & (np.abs(cen[:, 1]) < 0.31)
+    vals = np.array([np.einsum("ij,ij->", r.facet_momentum.cpu().numpy()[floor], nh[floor]) * 8 for r in runs])
+    want = -p * A[floor].sum()
+    se = vals.std(ddof=1) / np.sqrt(8)
+    assert abs(vals.mean() - want) < 4 * se and se < 0.02 * abs(want)
+
+
+# ------------------------------------------------------------------ exhaustive on/off checks at timing size
+def _arms(T):
+    return [("no pre-cull", T.TPMC_FLAG_NO_PRECULL), ("no horizon", T.TPMC_FLAG_NO_HORIZON),
+            ("body-frame boxes", T.TPMC_FLAG_ALIGN_OFF), ("flow-aligned boxes", T.TPMC_FLAG_ALIGN_ON),
+            ("unsorted", T.TPMC_FLAG_NO_SORT),
+            ("fp64 search, nothing skipped", T.TPMC_FLAG_EXACT_TRACE | T.TPMC_FLAG_NO_PRECULL | T.TPMC_FLAG_NO_HORIZON)]
+
+
+def _full_size_arms(T, cfg, arms):
+    import torch
+    m = cfg.mesh()
+    gm = T.Mesh(m.vertices, m.indices, m.flags)
+    ref = gm.run(cfg, debug=True, facets=False)
+    check_conservation(ref.stats, cfg.N)
+    assert ref.stats["truncated"] == 0
+    F = ref.force.cpu().numpy()
+    for label, flags in arms:
+        r = gm.run(cfg, debug=True, facets=False, flags=flags)
+        check_conservation(r.stats, cfg.N, exact=bool(flags & T.TPMC_FLAG_EXACT_TRACE))
+        assert r.stats["hits"] == ref.stats["hits"], label
+        assert torch.equal(r.hash, ref.hash), label                       # every particle of the stream
+        assert torch.equal(r.bounces, ref.bounces) and torch.equal(r.first_facet, ref.first_facet), label
+        assert np.linalg.norm(r.force.cpu().numpy() - F) <= 1e-11 * np.linalg.norm(F), label
+        del r
+        torch.cuda.empty_cache()
+    gm.close()
+
+
+@pytest.mark.parametrize("att", [0, 21, 40])
+def test_c5_every_shortcut_off_at_full_size(T, att):
+    """Every "exact" shortcut switched off in turn on ALL 1e9 particles of a C5 attitude (axis-near, oblique, and
+    the diagonal-most of the sweep), in the launch configuration bench.py times: the per-particle hashes, bounce
+    counts and first facets of the whole stream are compared on the device.  The last arm runs every segment
+    through the fp64 search with the pre-cull and the horizon off as well."""
+    cfg = ti.config("C5")[att]
+    arms = _arms(T)
+    if att != 21:
+        arms = arms[:-1]            # the thread-per-particle fp64 arm on 1e9 particles once only
+    _full_size_arms(T, cfg, arms)
+
+
+@pytest.mark.parametrize("name,idx", [("C2", 0), ("C3", 1), ("C4", 8)])
+def test_c2_c3_c4_every_shortcut_off_at_timing_size(T, name, idx):
+    """The same at the timing sizes of SURVEY 8(d): C2 N = 1e7, C3 N = 1e8, C4 N = 1e8."""
+    _full_size_arms(T, ti.config(name)[idx], _arms(T))

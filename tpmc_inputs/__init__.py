@@ -16,6 +16,9 @@ from .meshes import (  # noqa: F401
     hemisphere_shell,
     box,
     random_blob,
+    lobster_pot,
+    stacked_duplicates,
+    deep_chain,
 )
 from .configs import (  # noqa: F401
     AMU,

@@ -350,3 +350,47 @@ def random_blob(seed: int = 0, freq: int = 2, amplitude: float = 0.15) -> Mesh:
     noise = _GradientNoise(seed)
     return geodesic_sphere(freq, 1.0, lambda d: 1.0 + 2.0 * amplitude * _fbm(noise, d, 2, 1.5),
                            name=f"blob{seed}")
+
+
+def lobster_pot(hole: float = 0.5, h: float = 0.25) -> Mesh:
+    """Hollow unit cube of two-sided sheets with a square opening of side `hole` in its +x face: a particle that
+    enters bounces many times before it finds the opening again (long reflection chains, a full reflected-ray
+    region with a small wave)."""
+    n = max(2, int(round(1.0 / h)))
+    k = max(1, int(round(hole / 2.0 * n)))
+    X, Y, Z = np.eye(3)
+    c = np.zeros(3)
+    a = 0.5
+    patches = [
+        _patch(c + a * X - a * Y - a * Z, 2 * a * Y, 2 * a * Z, n, n, hole=(n // 2 - k, n // 2 + k, n // 2 - k, n // 2 + k)),
+        _patch(c - a * X - a * Y - a * Z, 2 * a * Z, 2 * a * Y, n, n),
+        _patch(c + a * Y - a * X - a * Z, 2 * a * Z, 2 * a * X, n, n),
+        _patch(c - a * Y - a * X - a * Z, 2 * a * X, 2 * a * Z, n, n),
+        _patch(c + a * Z - a * X - a * Y, 2 * a * X, 2 * a * Y, n, n),
+        _patch(c - a * Z - a * X - a * Y, 2 * a * Y, 2 * a * X, n, n),
+    ]
+    v, t = _merge(patches)
+    return _finish(v, t, np.full(t.shape[0], TWO_SIDED, np.uint8), name="lobster_pot")
+
+
+def stacked_duplicates(copies: int = 6) -> Mesh:
+    """A unit square (two triangles, normal +x) stored `copies` times over: every hit is a tie between `copies`
+    coincident facets (rule A12: the smallest facet index wins) -- more candidates than a short list holds."""
+    v = np.array([[0, -0.5, -0.5], [0, 0.5, -0.5], [0, 0.5, 0.5], [0, -0.5, 0.5]], dtype=np.float64)
+    t = np.array([[0, 1, 2], [0, 2, 3]] * copies)
+    return _finish(v, t, np.full(t.shape[0], TWO_SIDED, np.uint8), name=f"stack{copies}", weld=False)
+
+
+def deep_chain(levels: int = 21, cluster: int = 64) -> Mesh:
+    """Parallel two-sided unit squares normal to x at x = 2^-i (i < levels) plus `cluster` more packed below
+    2^-(levels+1): centroid Morton codes with one leading bit each, so a radix-tree hierarchy over them is a chain
+    about levels + log2(cluster) deep, and a ray along +x overlaps every box of it (deeper than a short
+    traversal stack)."""
+    xs = [2.0 ** -i for i in range(levels)] + [2.0 ** -(levels + 1) * (j + 1) / (cluster + 1) for j in range(cluster)]
+    verts, tris = [], []
+    for x in xs:
+        o = len(verts)
+        verts += [[x, -0.5, -0.5], [x, 0.5, -0.5], [x, 0.5, 0.5], [x, -0.5, 0.5]]
+        tris += [[o, o + 1, o + 2], [o, o + 2, o + 3]]
+    t = np.array(tris)
+    return _finish(np.array(verts, dtype=np.float64), t, np.full(t.shape[0], TWO_SIDED, np.uint8), name="deep_chain", weld=False)
