@@ -34,6 +34,9 @@ struct Pipe {
   float4* q_o[2];                  // ray queues (ping-pong between iterations), regions A|B of wave_cap rays each
   float4* q_v[2];
   int* q_f[2];
+  unsigned int* q_key[2];          // sort key of every queued ray (sort.cuh)
+  unsigned int* hist[2];           // [kSortBins] histogram of the keys of queue p, then their offsets
+  unsigned int* order;             // [2*wave_cap] queue slots in key order
   unsigned int* hit_ray;           // [2*wave_cap] queue slot of every ray that ended with candidate facets
   int4* hit_cand;                  // [2*wave_cap] its candidate triangle slots
   unsigned int* ctr;               // [kCtrWords] device counters (queue sizes, fetch head, hit count, survivors)
@@ -131,6 +134,7 @@ struct RunConst {
   unsigned long long first, count;
   unsigned int seed_lo, seed_hi;
   unsigned int max_bounces;
+  float key_c[3], key_r2;   // sort key of a ray (sort.cuh): body centre, (radius of the key sphere)^2
 };
 
 // Device counters of a run (tpmc_stats: every one is counted where the event happens).

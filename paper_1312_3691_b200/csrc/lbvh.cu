@@ -808,8 +808,8 @@ extern "C" void tpmc_mesh_destroy(tpmc_mesh* m) {
   cudaFree(m->nodes); cudaFree(m->tris); cudaFree(m->cull_c); cudaFree(m->kids); cudaFree(m->parent); cudaFree(m->arrive); cudaFree(m->rbox); cudaFree(m->nodes_r); cudaFree(m->cnodes_r); cudaFree(m->align_R); cudaFree(m->grid_dev); cudaFree(m->cnodes); cudaFree(m->horizon);
   for (int pi = 0; pi < kPipes; ++pi) {
     Pipe& pp = m->pipe[pi];
-    for (int k = 0; k < 2; ++k) { cudaFree(pp.q_o[k]); cudaFree(pp.q_v[k]); cudaFree(pp.q_f[k]); }
-    cudaFree(pp.hit_ray); cudaFree(pp.hit_cand); cudaFree(pp.ctr); cudaFree(pp.surv); cudaFree(pp.ovf);
+    for (int k = 0; k < 2; ++k) { cudaFree(pp.q_o[k]); cudaFree(pp.q_v[k]); cudaFree(pp.q_f[k]); cudaFree(pp.q_key[k]); cudaFree(pp.hist[k]); }
+    cudaFree(pp.hit_ray); cudaFree(pp.hit_cand); cudaFree(pp.ctr); cudaFree(pp.surv); cudaFree(pp.ovf); cudaFree(pp.order);
     if (pi > 0 && pp.main) cudaStreamDestroy(pp.main);
     if (pp.seed) cudaStreamDestroy(pp.seed);
     if (pp.side) cudaStreamDestroy(pp.side);

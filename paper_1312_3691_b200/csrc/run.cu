@@ -6,6 +6,7 @@
 
 #include "common.cuh"
 #include "sampling.cuh"
+#include "sort.cuh"
 #include "trace.cuh"
 
 namespace {
@@ -44,6 +45,8 @@ struct RayQueue {
   float4* o;
   float4* v;
   int* f;
+  unsigned int* key;    // sort key (sort.cuh)
+  unsigned int* hist;   // histogram of the keys of this queue, or nullptr (no sort)
 };
 
 // Per-iteration device counters: ctr[2p] = rays in region A of queue p, ctr[2p+1] = rays in region B,
@@ -199,6 +202,12 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
     __stcs(q.o + slot, make_float4(o[0], o[1], o[2], __uint_as_float(wave_first + j)));
     __stcs(q.v + slot, make_float4(v[0], v[1], v[2], __uint_as_float((unsigned int)species)));   // bounce 0
     __stcs(q.f + slot, -1);
+    if (q.hist) {
+      const SortKeyConst kc = {{rc.key_c[0], rc.key_c[1], rc.key_c[2]}, rc.key_r2};
+      const unsigned int key = primary_key(kc, o, v);
+      __stcs(q.key + slot, key);
+      atomicAdd(q.hist + key, 1u);
+    }
   }
   }
 }
@@ -228,6 +237,7 @@ constexpr int kFetchChunk = 64;   // rays a warp reserves per atomic on the queu
 __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf(const uint4* __restrict__ cnodes,
                                                              const QuantGrid* __restrict__ gridp,
                                                              const float4* __restrict__ tris, const RayQueue q,
+                                                             const unsigned int* __restrict__ order,
                                                              unsigned int cap, const unsigned int* __restrict__ n_rays,
                                                              unsigned int* __restrict__ next_ray,
                                                              unsigned int* __restrict__ hit_ray,
@@ -268,7 +278,7 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
         } else if (rank < avail) {
           r = pool_next + rank;
           if (r < n) {
-            r = (r < na) ? r : cap + (r - na);   // physical slot
+            r = order ? __ldcs(order + r) : ((r < na) ? r : cap + (r - na));   // physical slot (in key order when sorted)
             walk_init(w, *gridp, __ldcs(q.o + r), __ldcs(q.v + r), __ldcs(q.f + r));
             has = true;
           }
@@ -497,6 +507,12 @@ __global__ void __launch_bounds__(kTraceBlock, 6) k_reflect(const RunConst rc, u
         __stcs(qd.o + sd, make_float4(p.o[0], p.o[1], p.o[2], __uint_as_float((unsigned int)p.j)));
         __stcs(qd.v + sd, make_float4(p.v[0], p.v[1], p.v[2], __uint_as_float((unsigned int)p.species | (p.k << 4))));
         __stcs(qd.f + sd, p.f_prev);
+        if (qout.hist && !spill) {
+          const SortKeyConst kc = {{rc.key_c[0], rc.key_c[1], rc.key_c[2]}, rc.key_r2};
+          const unsigned int key = origin_key(kc, p.o);
+          __stcs(qout.key + s, key);
+          atomicAdd(qout.hist + key, 1u);
+        }
       }
     }
     const unsigned sm = __ballot_sync(FULL, spill);
@@ -725,6 +741,11 @@ int make_run_const(const tpmc_mesh* m, const tpmc_params* p, RunConst* rc) {
     rc->aabb_hi[a] = m->aabb_hi[a];
   }
   rc->r = r;
+  for (int a = 0; a < 3; ++a) rc->key_c[a] = (float)m->centre[a];
+  {
+    const float rk = m->cull_nbox >= 0 ? m->cull_rin : (float)m->Rb;
+    rc->key_r2 = rk * rk;
+  }
   rc->sigma = p->accommodation;
   rc->first = p->first;
   rc->count = p->count;
@@ -807,17 +828,18 @@ int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
       TPMC_CUDA_TRY(cudaEventCreate(&pp.ev_f0));
       TPMC_CUDA_TRY(cudaEventCreate(&pp.ev_f1));
       TPMC_CUDA_TRY(cudaMalloc((void**)&pp.ctr, kCtrWords * sizeof(unsigned int)));
+      for (int k = 0; k < 2; ++k) TPMC_CUDA_TRY(cudaMalloc((void**)&pp.hist[k], kSortBins * sizeof(unsigned int)));
     }
   }
   if (m->wave_cap < wave) {
     for (int pi = 0; pi < kPipes; ++pi) {
       Pipe& pp = m->pipe[pi];
       for (int k = 0; k < 2; ++k) {
-        cudaFree(pp.q_o[k]); cudaFree(pp.q_v[k]); cudaFree(pp.q_f[k]);
-        pp.q_o[k] = pp.q_v[k] = nullptr; pp.q_f[k] = nullptr;
+        cudaFree(pp.q_o[k]); cudaFree(pp.q_v[k]); cudaFree(pp.q_f[k]); cudaFree(pp.q_key[k]);
+        pp.q_o[k] = pp.q_v[k] = nullptr; pp.q_f[k] = nullptr; pp.q_key[k] = nullptr;
       }
-      cudaFree(pp.hit_ray); cudaFree(pp.hit_cand); cudaFree(pp.surv); cudaFree(pp.ovf);
-      pp.hit_ray = nullptr; pp.hit_cand = nullptr; pp.surv = nullptr; pp.ovf = nullptr;
+      cudaFree(pp.hit_ray); cudaFree(pp.hit_cand); cudaFree(pp.surv); cudaFree(pp.ovf); cudaFree(pp.order);
+      pp.hit_ray = nullptr; pp.hit_cand = nullptr; pp.surv = nullptr; pp.ovf = nullptr; pp.order = nullptr;
     }
     m->wave_cap = 0;
     for (int pi = 0; pi < kPipes; ++pi) {
@@ -826,7 +848,9 @@ int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
         TPMC_CUDA_TRY(cudaMalloc((void**)&pp.q_o[k], 2 * wave * sizeof(float4)));   // regions A and B
         TPMC_CUDA_TRY(cudaMalloc((void**)&pp.q_v[k], 2 * wave * sizeof(float4)));
         TPMC_CUDA_TRY(cudaMalloc((void**)&pp.q_f[k], 2 * wave * sizeof(int)));
+        TPMC_CUDA_TRY(cudaMalloc((void**)&pp.q_key[k], 2 * wave * sizeof(unsigned int)));
       }
+      TPMC_CUDA_TRY(cudaMalloc((void**)&pp.order, 2 * wave * sizeof(unsigned int)));
       TPMC_CUDA_TRY(cudaMalloc((void**)&pp.hit_ray, 2 * wave * sizeof(unsigned int)));
       TPMC_CUDA_TRY(cudaMalloc((void**)&pp.hit_cand, 2 * wave * sizeof(int4)));
       TPMC_CUDA_TRY(cudaMalloc((void**)&pp.surv, 3 * wave * sizeof(unsigned int)));
@@ -839,9 +863,9 @@ int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
   return TPMC_OK;
 }
 
-struct Grids { int trace, reflect, finish, pipes, seed, precull; };
+struct Grids { int trace, reflect, finish, pipes, seed, precull, scatter; };
 const Grids& grids() {
-  static Grids g = {0, 0, 0, 0, 0, 0};
+  static Grids g = {0, 0, 0, 0, 0, 0, 0};
   if (!g.trace) {
     int dev = 0, sms = 148, per = 0;
     cudaGetDevice(&dev);
@@ -858,6 +882,7 @@ const Grids& grids() {
     g.seed = sms * per;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_seed_precull, kPrecullBlock, 0) != cudaSuccess || per < 1) per = 4;
     g.precull = sms * per * 4;   // four shares per resident block (evens out the tail)
+    g.scatter = sms * 8;
   }
   return g;
 }
@@ -957,6 +982,7 @@ extern "C" int tpmc_run(tpmc_mesh* m, const tpmc_params* params, void* cuda_stre
   const bool precull = !(params->flags & TPMC_FLAG_NO_PRECULL);
   const bool use_horizon = !(params->flags & TPMC_FLAG_NO_HORIZON);
   const bool exact = (params->flags & TPMC_FLAG_EXACT_TRACE) != 0;
+  const bool sorted = !exact && !(params->flags & TPMC_FLAG_NO_SORT);
   // seed-time walk of the top of the hierarchy: pays only while the pre-cull pass has no two-level cull volume
   // (with it the pass is already tighter than the 64-node tree)
   const int seed_walk = m->cull_nbox < 0;
@@ -1010,6 +1036,8 @@ extern "C" int tpmc_run(tpmc_mesh* m, const tpmc_params* params, void* cuda_stre
       if (pi > 0) TPMC_CUDA_TRY(cudaStreamWaitEvent(pp.main, m->ev_fork, 0));
       // a chunk starts from empty queues; the side streams of the previous chunk have been joined
       TPMC_CUDA_TRY(cudaMemsetAsync(pp.ctr, 0, kCtrWords * sizeof(unsigned int), pp.main));
+      if (sorted)
+        for (int k = 0; k < 2; ++k) TPMC_CUDA_TRY(cudaMemsetAsync(pp.hist[k], 0, kSortBins * sizeof(unsigned int), pp.main));
       TPMC_CUDA_TRY(cudaEventRecord(pp.ev_reset[0], pp.main));
     }
     // Waves are dealt round-robin to the pipelines.  In a pipeline, one iteration per wave: seed the wave
@@ -1026,7 +1054,8 @@ extern "C" int tpmc_run(tpmc_mesh* m, const tpmc_params* params, void* cuda_stre
       cudaStream_t s1 = pp.main, s2 = pp.seed, s3 = pp.side;
       const int b = (int)(li & 1);
       unsigned int* ovf = pp.ovf + (size_t)b * 2 * m->wave_cap;
-      RayQueue Q[2] = {{pp.q_o[0], pp.q_v[0], pp.q_f[0]}, {pp.q_o[1], pp.q_v[1], pp.q_f[1]}};
+      RayQueue Q[2] = {{pp.q_o[0], pp.q_v[0], pp.q_f[0], pp.q_key[0], sorted ? pp.hist[0] : nullptr},
+                       {pp.q_o[1], pp.q_v[1], pp.q_f[1], pp.q_key[1], sorted ? pp.hist[1] : nullptr}};
       const bool tw = timed && c0 == 0 && li < (unsigned long long)kMaxTimedWaves;
       cudaEvent_t* ev = tw ? pp.wave_ev + kEvPerWave * li : nullptr;
       if (wv < n_waves) {
@@ -1054,13 +1083,22 @@ extern "C" int tpmc_run(tpmc_mesh* m, const tpmc_params* params, void* cuda_stre
       }
       // (without a reflect step nothing else orders this iteration behind the straggler kernel that still reads list b)
       if (exact && li >= 2) TPMC_CUDA_TRY(cudaStreamWaitEvent(s1, pp.ev_ovf[b], 0));
+      // the histogram of the OTHER queue (offsets of the previous iteration's sort by now) starts from zero: the seed
+      // kernel of the next wave and this iteration's reflect step both count into it
+      if (sorted && li >= 1) TPMC_CUDA_TRY(cudaMemsetAsync(pp.hist[p ^ 1], 0, kSortBins * sizeof(unsigned int), s1));
       k_iter_begin<<<1, 32, 0, s1>>>(pp.ctr, p ^ 1, b);
       TPMC_CUDA_TRY(cudaEventRecord(pp.ev_reset[(li + 1) & 3], s1));
       if (wv < n_waves) TPMC_CUDA_TRY(cudaStreamWaitEvent(s1, pp.ev_seeded[li & 3], 0));
       if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[2], s1));
+      if (sorted) {   // counting sort of the queue by key (sort.cuh)
+        k_sort_scan<<<1, kScanBlock, 0, s1>>>(pp.hist[p]);
+        k_sort_scatter<<<g.scatter, 256, 0, s1>>>(pp.q_key[p], cap, pp.ctr + 2 * p, pp.hist[p], pp.order);
+        launches += 2;
+      }
       if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[7], s1));
       if (!exact) {
-        k_trace_wf<<<g.trace, kTraceBlock, 0, s1>>>(cnodes_t, qg_t, m->tris, Q[p], cap, pp.ctr + 2 * p, pp.ctr + 4, pp.hit_ray,
+        k_trace_wf<<<g.trace, kTraceBlock, 0, s1>>>(cnodes_t, qg_t, m->tris, Q[p], sorted ? pp.order : nullptr, cap,
+                                                    pp.ctr + 2 * p, pp.ctr + 4, pp.hit_ray,
                                                     pp.hit_cand, pp.ctr + 5, m->stats, trace_tune());
         if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[3], s1));
         // the straggler kernel of the previous iteration reads the queue this reflect step writes
@@ -1092,7 +1130,7 @@ extern "C" int tpmc_run(tpmc_mesh* m, const tpmc_params* params, void* cuda_stre
       Pipe& pp = m->pipe[pi];
       const unsigned long long its = (n_waves + (unsigned long long)K * kDrain - pi + K - 1) / K;   // iterations it ran
       const int p = (int)(its & 1);
-      RayQueue q = {pp.q_o[p], pp.q_v[p], pp.q_f[p]};
+      RayQueue q = {pp.q_o[p], pp.q_v[p], pp.q_f[p], pp.q_key[p], nullptr};
       TPMC_CUDA_TRY(cudaStreamWaitEvent(pp.main, pp.ev_ovf[0], 0));   // join the side stream
       TPMC_CUDA_TRY(cudaStreamWaitEvent(pp.main, pp.ev_ovf[1], 0));
       if (timed) TPMC_CUDA_TRY(cudaEventRecord(pp.ev_f0, pp.main));
@@ -1162,7 +1200,7 @@ extern "C" int tpmc_trace(tpmc_mesh* m, const float* d_o, const float* d_d, cons
   if (rcode != TPMC_OK) return rcode;
   const Grids& g = grids();
   Pipe& pp = m->pipe[0];
-  RayQueue q = {pp.q_o[0], pp.q_v[0], pp.q_f[0]};
+  RayQueue q = {pp.q_o[0], pp.q_v[0], pp.q_f[0], pp.q_key[0], nullptr};
   const unsigned int un = (unsigned int)n;
   const QuantGrid* qg_t = m->grid_dev;
   const uint4* cnodes_t = m->cnodes;
@@ -1179,7 +1217,7 @@ extern "C" int tpmc_trace(tpmc_mesh* m, const float* d_o, const float* d_d, cons
   TPMC_CUDA_TRY(cudaMemsetAsync(m->stats, 0, ST_COUNT * sizeof(unsigned long long), st));
   k_pack_rays<<<(un + 255) / 256, 256, 0, st>>>(d_o, d_d, d_f_prev, un, q, d_facet, d_tau);
   // the production traversal (fp32 wavefront + candidate lists), then the exact fp64 resolve
-  k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(cnodes_t, qg_t, m->tris, q, (unsigned int)(2 * m->wave_cap), pp.ctr, pp.ctr + 4,
+  k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(cnodes_t, qg_t, m->tris, q, nullptr, (unsigned int)(2 * m->wave_cap), pp.ctr, pp.ctr + 4,
                                               pp.hit_ray, pp.hit_cand, pp.ctr + 5, m->stats, trace_tune());
   k_resolve_only<<<g.reflect, kTraceBlock, 0, st>>>(m->nodes, m->tris, q, pp.hit_ray, pp.hit_cand, pp.ctr + 5, d_facet,
                                                     d_tau);

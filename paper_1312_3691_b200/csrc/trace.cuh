@@ -95,10 +95,26 @@ __device__ __forceinline__ bool facet_test(const float4 q0, const float4 q1, con
 }
 
 // ---- fp32 classification of the same test, with forward error bounds --------------------------------
-// Every monomial of a triple product d_i b_j c_k passes through at most 7 roundings (two corner
-// differences, product, difference, product with d, two sums): |computed - exact| <= ((1+u)^7 - 1) * M with
-// M the sum of the absolute monomials, u = 2^-24.  M is itself computed in fp32, so the band used is
-// 10 u M.  Magnitudes in this application (metres, m/s) are far from the fp32 under/overflow range.
+// The edge functions d.(b x c) with b = p1 - o, c = p2 - o do not change when the origin slides along the ray
+// (exact arithmetic: d.((b - t d) x (c - t d)) = d.(b x c)), but their fp32 evaluation does: with the origin on the
+// control sphere, metres away, the rounding band 10u * sum|d_i b_j c_k| is as wide as a millimetre-sized facet and
+// nothing is ever certain.  So the origin is first moved next to the facet, o' = fl(o + t0 d) with t0 the
+// parameter of the ray point closest to p0 (any t0 is valid; this one makes |p - o'| facet-sized for a hit), and
+// the rounding of that move is carried as a perturbation of the inputs:
+//   x = o + t0 d exactly;  o'_k = fma(t0, d_k, o_k) = x_k + e,  |e| <= u |o'_k|         (one rounding)
+//   a'_k = fl(p0_k - o'_k) = (p0_k - x_k) + eps_k,  |eps_k| <= u |o'_k| + u |a'_k| <= eta    (likewise b', c')
+//   eta  = u (1 + 2^-10) max_k (|o'_k| + max(|a'_k|, |b'_k|, |c'_k|))
+//   d.(b' x c') - d.(B x C) = d.(eps_b x c') + d.(b' x eps_c) - d.(eps_b x eps_c),  and
+//   |d.(e x c)| = |e.(c x d)| <= |e|_inf |c x d|_1 <= |e|_inf |c|_1 |d|_1,  so the perturbation is bounded by
+//   P(b', c') = eta |d|_1 (|b'|_1 + |c'|_1 + 3 eta).
+// On top of it the evaluation itself: every monomial d_i b'_j c'_k passes through at most 5 roundings (product,
+// difference, product with d, two sums; 7 for det and the numerator, whose edge vectors are rounded differences of
+// corners): |computed - exact| <= ((1+u)^7 - 1) M with M the sum of the absolute monomials, itself computed in fp32:
+// band 10u M.  The bounds are sums of positive terms evaluated in fp32 (relative error < 1e-6): a factor 1.0001
+// covers that.  tau: the shifted ray hits at tau - t0 = (A.Ng)/det with A = p0 - x; the numerator's perturbation is
+// |eps_a.(e1 x e2)| <= eta |e1 x e2|_1 <= eta sum|e1_j e2_k|; quotient and sum are rounded outwards by directed
+// roundings.  Magnitudes in this application (metres, m/s) are far from the fp32 under/overflow range; a NaN (zero
+// direction) fails every comparison and ends as UNCERTAIN.
 enum { TRI_MISS = 0, TRI_HIT = 1, TRI_UNCERTAIN = 2 };
 
 __device__ __forceinline__ void triple_f32(const float d[3], const float x[3], const float y[3], float& w, float& M) {
@@ -108,11 +124,11 @@ __device__ __forceinline__ void triple_f32(const float d[3], const float x[3], c
   w = fmaf(d[2], p4 - p5, fmaf(d[1], p2 - p3, d[0] * (p0 - p1)));
   M = fmaf(fabsf(d[2]), fabsf(p4) + fabsf(p5), fmaf(fabsf(d[1]), fabsf(p2) + fabsf(p3), fabsf(d[0]) * (fabsf(p0) + fabsf(p1))));
 }
+__device__ __forceinline__ float norm1(const float x[3]) { return fabsf(x[0]) + fabsf(x[1]) + fabsf(x[2]); }
 
 __device__ __forceinline__ int tri_filter(const float4 q0, const float4 q1, const float4 q2, const float o[3],
                                           const float d[3], float& tlo, float& thi) {
   const float EPS = 5.9604645e-07f;   // 10 * 2^-24
-  const float a[3] = {q0.x - o[0], q0.y - o[1], q0.z - o[2]};
   const float e1[3] = {q1.x - q0.x, q1.y - q0.y, q1.z - q0.z};
   const float e2[3] = {q2.x - q0.x, q2.y - q0.y, q2.z - q0.z};
   float det, Mdet;
@@ -120,33 +136,51 @@ __device__ __forceinline__ int tri_filter(const float4 q0, const float4 q1, cons
   const float Edet = EPS * Mdet;
   const bool two_sided = (__float_as_uint(q1.w) & TPMC_FACET_TWO_SIDED) != 0u;
   if (!two_sided && det > Edet) return TRI_MISS;  // provably back-facing
-  const float b[3] = {q1.x - o[0], q1.y - o[1], q1.z - o[2]};
-  const float c[3] = {q2.x - o[0], q2.y - o[1], q2.z - o[2]};
+  // origin moved next to the facet
+  const float dd = fmaf(d[2], d[2], fmaf(d[1], d[1], d[0] * d[0]));
+  const float t0 = __fdividef(fmaf(q0.z - o[2], d[2], fmaf(q0.y - o[1], d[1], (q0.x - o[0]) * d[0])), dd);
+  const float os[3] = {fmaf(t0, d[0], o[0]), fmaf(t0, d[1], o[1]), fmaf(t0, d[2], o[2])};
+  const float a[3] = {q0.x - os[0], q0.y - os[1], q0.z - os[2]};
+  const float b[3] = {q1.x - os[0], q1.y - os[1], q1.z - os[2]};
+  const float c[3] = {q2.x - os[0], q2.y - os[1], q2.z - os[2]};
+  float eta = 0.0f;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) eta = fmaxf(eta, fabsf(os[k]) + fmaxf(fabsf(a[k]), fmaxf(fabsf(b[k]), fabsf(c[k]))));
+  eta *= 5.9662852e-08f;                          // u (1 + 2^-10)
+  const float d1 = norm1(d) * 1.0001f, na = norm1(a), nb = norm1(b), nc = norm1(c), e3 = 3.0f * eta;
   float w0, M0, w1, M1, w2, M2;
   triple_f32(d, b, c, w0, M0);
   triple_f32(d, c, a, w1, M1);
   triple_f32(d, a, b, w2, M2);
-  const float E0 = EPS * M0, E1 = EPS * M1, E2 = EPS * M2;
+  const float pd = eta * d1;
+  const float E0 = fmaf(EPS, M0, pd * (nb + nc + e3)), E1 = fmaf(EPS, M1, pd * (nc + na + e3)), E2 = fmaf(EPS, M2, pd * (na + nb + e3));
   const bool anypos = (w0 > E0) || (w1 > E1) || (w2 > E2);
   const bool anyneg = (w0 < -E0) || (w1 < -E1) || (w2 < -E2);
   if (anypos && anyneg) return TRI_MISS;          // two edge functions of provably opposite sign
   float num, Mn;
-  triple_f32(a, e1, e2, num, Mn);                 // a . (e1 x e2)
-  const float En = EPS * Mn;
-  const float ad = fabsf(det), an = fabsf(num);
+  triple_f32(a, e1, e2, num, Mn);                 // a' . (e1 x e2) = (tau - t0) det, up to the bands
+  const float Mx = (fabsf(e1[1] * e2[2]) + fabsf(e1[2] * e2[1])) + (fabsf(e1[2] * e2[0]) + fabsf(e1[0] * e2[2])) +
+                   (fabsf(e1[0] * e2[1]) + fabsf(e1[1] * e2[0]));
+  const float En = fmaf(EPS, Mn, 1.0001f * eta * Mx);
+  const float ad = fabsf(det);
   const bool det_ok = ad > Edet;                  // sign of det is certain
-  const bool num_ok = an > En;
-  if (det_ok && num_ok && ((num > 0.0f) != (det > 0.0f))) return TRI_MISS;   // provably behind the origin
   tlo = 0.0f;
   thi = INFINITY;
-  if (det_ok) {
-    tlo = fmaxf(an - En, 0.0f) / (ad + Edet) * 0.99999964f;
-    thi = (an + En) / (ad - Edet) * 1.00000036f;
-  }
+  if (!det_ok) return TRI_UNCERTAIN;
+  // tau - t0 = N / |det| with N = sign(det) num in [nl, nh], |det| in [dl, dh]: quotient and sum rounded outwards
+  const float ns = det < 0.0f ? -num : num;
+  const float nl = __fadd_rd(ns, -En), nh = __fadd_ru(ns, En);
+  const float dl = __fadd_rd(ad, -Edet), dh = __fadd_ru(ad, Edet);
+  const float ql = __fdiv_rd(nl, nl >= 0.0f ? dh : dl), qh = __fdiv_ru(nh, nh >= 0.0f ? dl : dh);
+  const float tl = __fadd_rd(t0, ql), th = __fadd_ru(t0, qh);
+  if (th < 0.0f) return TRI_MISS;                 // provably behind the origin
+  tlo = fmaxf(tl, 0.0f);
   const bool allpos = (w0 > E0) && (w1 > E1) && (w2 > E2);
   const bool allneg = (w0 < -E0) && (w1 < -E1) && (w2 < -E2);
-  if ((allpos || allneg) && det_ok && num_ok) return TRI_HIT;   // (one-sided: det < -Edet follows from det_ok)
-  if (!(det_ok && num_ok)) tlo = 0.0f;
+  if ((allpos || allneg) && tl > 0.0f) {          // (one-sided: det < -Edet follows from det_ok)
+    thi = th;
+    return TRI_HIT;
+  }
   return TRI_UNCERTAIN;
 }
 
