@@ -1,12 +1,14 @@
 #!/usr/bin/env python
-"""bench.py -- particle-bounces/s of the TPMC hot path (seed -> trace -> reflect -> accumulate ->
-reduce) on synthetic config C5 of BASELINE.json: the ~1.0e6-facet procedural body, 70 % O / 30 % He,
-T_inf = 900 K, |V| = 7700 m/s, N = 1e9 particles per attitude of the 64-attitude sweep.
+"""bench.py -- particle-bounces/s of the TPMC hot path (seed -> trace -> reflect -> accumulate -> reduce).
 
-One "step" = one tpmc_run of N particles at one attitude (the whole hot path over one batch).
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl tpmc|reference] [--particles N]
-N > 1: launched by torchrun, one rank per GPU; rank r runs attitudes r, r+N, ... (weak scaling, no
-data-path collective: attitudes are independent problems); value = all ranks' bounces / max time.
+Headline (default, `--config C5`): synthetic config C5 of BASELINE.json, the ~1.0e6-facet procedural body, 70 % O /
+30 % He, T_inf = 900 K, |V| = 7700 m/s, N = 1e9 particles per attitude of the 64-attitude sweep.  `--config C1..C4`
+times the other four configs at the sizes of SURVEY 8(d) (their bench lines are recorded in DESIGN.md section 7).
+
+One "step" = one tpmc_run of N particles at one point of the config's sweep (the whole hot path over one batch).
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl tpmc|reference] [--config C5] [--particles N]
+N > 1: launched by torchrun, one rank per GPU; rank r runs sweep points r, r+N, ... (weak scaling, no data-path
+collective: sweep points are independent problems); value = all ranks' bounces / max time.
 Prints ONE JSON line on rank 0 (contract in DESIGN.md "Measurement").
 """
 from __future__ import annotations
@@ -27,21 +29,34 @@ import numpy as np
 
 import tpmc_inputs as ti
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one steady-state k_trace_wf launch in this launch configuration
-# (wave of 2^26 particles, ~1.3e7 rays per launch), from the `ncu --set full` capture summarised in
-# profiles/r1_ncu_full_pipeline_v6.md
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 2_793_646_504
 METRIC = "particle_bounces_per_s"
 UNIT = "bounces/s"
-WORKLOAD = "C5: ~1.0e6-facet noise-displaced geodesic body + 6 panels, O/He 70/30, 900 K, 7700 m/s"
+WORKLOADS = {
+    "C1": "C1: flat plate, 2 two-sided facets, normal 30 deg to the stream, O, 1000 K, 7500 m/s, N = 1e5",
+    "C2": "C2: geodesic sphere, 20480 facets, O, 7500 m/s, S in {2, 5, 8}, N = 1e7 per run",
+    "C3": "C3: capped cylinder, 2048 facets, Maxwell sigma = 0.8, axis at 0/45/90 deg, N = 1e8 per run",
+    "C4": "C4: concave satellite (bus + pocket + 2 canted panels), 50160 facets, 16 pitch angles, N = 1e8 per run",
+    "C5": "C5: ~1.0e6-facet noise-displaced geodesic body + 6 panels, O/He 70/30, 900 K, 7700 m/s",
+}
 
 
-def peaks():
+def hbm_peak():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
         d = json.load(open(p))
         return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json, copy)"
     return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(config: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one steady-state k_trace_wf launch, from the tracked summary of
+    the latest `ncu --set full` capture in this launch configuration (profiles/trace_traffic.json names the capture)."""
+    p = os.path.join(ROOT, "profiles", "trace_traffic.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        if config in d:
+            return d[config]["dram_bytes_per_launch"], d[config]["source"]
+    return None, None
 
 
 class ClockSampler:
@@ -55,7 +70,7 @@ class ClockSampler:
              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits",
-                                          "-i", str(self.index), "-lms", "200"], stdout=subprocess.PIPE, text=True)
+                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
             threading.Thread(target=self._read, daemon=True).start()
         except Exception:
             self.proc = None
@@ -78,7 +93,7 @@ class ClockSampler:
 
 
 def attitude_index(step: int, rank: int, world: int, n_attitudes: int) -> int:
-    """Which attitude of the sweep a rank runs at a step: ranks take disjoint attitudes (weak scaling)."""
+    """Which point of the sweep a rank runs at a step: ranks take disjoint points (weak scaling)."""
     return (step * world + rank) % n_attitudes
 
 
@@ -94,6 +109,25 @@ def reduce_over_ranks(times, totals, world: int, device=None):
     return t.tolist(), tot.tolist()
 
 
+def sum_slices(parts, world: int, device=None):
+    """The other split of SURVEY 8(e): ranks run disjoint (first, count) slices of ONE run and the outputs (force,
+    torque, per-facet momentum: slices are additive) are summed across ranks.  parts: list of tensors."""
+    import torch
+    out = [torch.as_tensor(p, dtype=torch.float64, device=device).clone() for p in parts]
+    if world > 1:
+        import torch.distributed as dist
+        for t in out:
+            dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return out
+
+
+def slice_of(rank: int, world: int, N: int):
+    """Contiguous particle range of a rank: (first, count), covering [0, N) without overlap."""
+    per = N // world
+    first = rank * per
+    return first, (N - first if rank == world - 1 else per)
+
+
 def oracle_sample(cfgs, count_per_thread, threads):
     """The oracle, as it stands, on a bounded slice of the same workload, one slice per host thread."""
     import oracle
@@ -101,6 +135,7 @@ def oracle_sample(cfgs, count_per_thread, threads):
     m = cfgs[0].mesh()
     om = oracle.OracleMesh(m.vertices, m.indices, m.flags)
     cfg = cfgs[0]
+    count_per_thread = max(1, min(count_per_thread, cfg.N // threads))
 
     def work(k):
         return om.run(cfg, first=k * count_per_thread, count=count_per_thread, debug=False, facets=False)
@@ -122,17 +157,17 @@ def run_reference(args, cfgs, rank):
     oracle_sample(cfgs, 2000, threads)                       # builds the oracle mesh, warms caches
     for _ in range(max(args.warmup, 0)):
         oracle_sample(cfgs, max(per // 10, 1000), threads)
-    tot_hits, tot_t = 0, 0.0
+    tot_hits, tot_t, n = 0, 0.0, 0
     for _ in range(args.steps):
         h, dt, n = oracle_sample(cfgs, per, threads)
         tot_hits += h
         tot_t += dt
     val = tot_hits / tot_t
-    sample = f"{per * threads} particles per step ({threads} slices of {per}) of the N={cfgs[0].N:.0e} stream, attitude 0"
+    sample = f"{n} particles per step ({threads} slices) of the N={cfgs[0].N:.0e} stream, sweep point 0"
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": WORKLOAD, "particles_per_step": per * threads, "facets": cfgs[0].mesh().nt},
+            "config": {"workload": WORKLOADS[args.config], "particles_per_step": n, "facets": cfgs[0].mesh().nt},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -145,17 +180,19 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="tpmc", choices=["tpmc", "reference"])
-    ap.add_argument("--particles", type=float, default=None, help="override N per step (default: the config's 1e9)")
+    ap.add_argument("--config", default="C5", choices=sorted(WORKLOADS))
+    ap.add_argument("--particles", type=float, default=None, help="override N per step (default: the config's)")
     ap.add_argument("--ref-particles", type=float, default=4_000_000, help="oracle particles per reference step")
     ap.add_argument("--cpu-baseline-particles", type=float, default=80_000_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-peaks", action="store_true")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
-    cfgs = ti.config("C5")
+    cfgs = ti.config(args.config)
     if args.particles:
         cfgs = [c.with_(N=int(args.particles)) for c in cfgs]
 
@@ -191,6 +228,10 @@ def main():
     L = tpmc.lib()
     import ctypes as C
 
+    # C5's structure (149 MB) and its per-wave lists exceed the 126 MB L2; the small configs fit, so their L2 is flushed
+    # between steps by writing a 512 MB buffer (outside the per-step event pairs).
+    flush = None if args.config == "C5" else torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+
     def step(k, stats=None):
         cfg = cfgs[attitude_index(k, rank, world, len(cfgs))]
         p, keep = tpmc.make_params(cfg)
@@ -207,36 +248,49 @@ def main():
     # ---- timed: exactly K steps, device-resident, CUDA events on the launching stream
     sampler = ClockSampler(local_rank)
     sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
-    e0.record(stream)
-    for k in range(args.steps):
-        step(args.warmup + k)
-    e1.record(stream)
-    barrier()
+    if flush is None:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for k in range(args.steps):
+            step(args.warmup + k)
+        e1.record(stream)
+        barrier()
+        ms_total = e0.elapsed_time(e1)
+    else:
+        evs = []
+        for k in range(args.steps):
+            flush.fill_(k & 0xFF)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            step(args.warmup + k)
+            b.record(stream)
+            evs.append((a, b))
+        barrier()
+        ms_total = sum(a.elapsed_time(b) for a, b in evs)
     clocks = sampler.stop()
-    ms_total = e0.elapsed_time(e1)
 
-    # ---- one more pass per timed attitude with stats on: hits (the metric's numerator) and the
+    # ---- one more pass per timed sweep point with stats on: hits (the metric's numerator) and the
     #      per-kernel event times for the roofline.  Same work, same stream; not part of `value`'s clock.
-    hits = segs = launches = 0
-    ms_seed = ms_trace = ms_reflect = ms_finish = ms_stat = 0.0
-    waves = nodes = tris = culled = tr_launches = traced = 0
+    tot = {}
+    keys = ["hits", "segments", "kernel_launches", "ms_seed", "ms_trace", "ms_reflect", "ms_finish", "ms_sort", "ms",
+            "timed_waves", "node_visits", "tri_tests", "culled", "trace_launches", "traced_rays", "overflow_rays"]
     for k in range(args.steps):
         st = tpmc.tpmc_stats()
         step(args.warmup + k, st)
-        hits += st.hits; segs += st.segments; launches += st.kernel_launches
-        ms_seed += st.ms_seed; ms_trace += st.ms_trace; ms_stat += st.ms
-        ms_reflect += st.ms_reflect; ms_finish += st.ms_finish
-        waves += st.timed_waves; nodes += st.node_visits; tris += st.tri_tests; culled += st.culled
-        tr_launches += st.trace_launches; traced += st.traced_rays
+        for f in keys:
+            tot[f] = tot.get(f, 0) + getattr(st, f)
     barrier()
+    hits, segs, launches = tot["hits"], tot["segments"], tot["kernel_launches"]
 
     # ---- end to end: host buffers through tpmc_run_host (params H2D, results D2H inside the region)
     e2e = None
     if not args.no_e2e:
         hF, hT = np.empty(3), np.empty(3)
         hP = torch.empty((mesh.nt, 3), dtype=torch.float64).pin_memory().numpy()
+        cfg0 = cfgs[attitude_index(args.warmup, rank, world, len(cfgs))]
+        p0, keep0 = tpmc.make_params(cfg0)
+        L.tpmc_run_host(mesh._h, C.byref(p0), stream.cuda_stream or None, hF.ctypes.data, hT.ctypes.data, hP.ctypes.data, None)
         barrier()
         t0 = time.perf_counter()
         for k in range(args.steps):
@@ -250,59 +304,78 @@ def main():
         e2e_s = time.perf_counter() - t0
         e2e = {"hits": hits, "s": e2e_s}
 
+    peaks = None
+    if rank == 0 and not args.no_peaks:
+        peaks = tpmc.tpmc_measure_peaks()
+
     # ---- max over ranks, totals over ranks
     (ms_total_max, e2e_s_max), (hits_all, segs_all, parts_all) = reduce_over_ranks(
         [ms_total, e2e["s"] if e2e else 0.0], [hits, segs, N * args.steps], world, dev)
 
     if rank == 0:
         value = hits_all / (ms_total_max * 1e-3)
-        peak, peak_src = peaks()
-        # dominant kernel = trace/reflect.  Algorithmic bytes per segment:
-        # ceil(log2 T) nodes * 64 B + 1 triangle * 48 B + 32 B ray in + 8 B result out.
-        per_seg = int(np.ceil(np.log2(mesh.nt))) * 64 + 48 + 32 + 8
-        launches_trace = max(tr_launches, 1)         # k_trace_wf launches (rounds x waves), rays they processed
-        bytes_per_launch = traced * per_seg / launches_trace
-        avg_ms = ms_trace / launches_trace
-        achieved = bytes_per_launch / (avg_ms * 1e-3) / 1e9 if avg_ms > 0 else 0.0
-        # ncu shows the kernel bound by instruction issue (DRAM 1-4 %, L2 < 20 %, issue slots ~72 % busy; profiles/),
-        # so the binding roofline is the fp32 lane-instruction rate: SMs x 128 lanes x SM clock under this load.
-        # Algorithmic fp32 work per segment: ceil(log2 T) node visits x 2 slab tests x 18 ops + one
-        # watertight facet test of 60 ops; none of it pairs into FMAs, so one op = one lane-instruction.
-        ops_per_seg = int(np.ceil(np.log2(mesh.nt))) * 2 * 18 + 60
-        sms = torch.cuda.get_device_properties(dev).multi_processor_count
-        clk_mhz = clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965.0
-        alu_peak = sms * 128 * clk_mhz * 1e6 / 1e12                      # T lane-op/s
-        alu_ach = (traced * ops_per_seg / launches_trace) / (avg_ms * 1e-3) / 1e12 if avg_ms > 0 else 0.0
+        hbm, hbm_src = hbm_peak()
+        traced, nodes, tris = tot["traced_rays"], tot["node_visits"], tot["tri_tests"]
+        launches_trace = max(tot["trace_launches"], 1)         # k_trace_wf launches, rays they processed
+        avg_ms = tot["ms_trace"] / launches_trace
+        depth = int(np.ceil(np.log2(max(mesh.nt, 2))))
+        # Algorithmic work per segment: ceil(log2 T) nodes x 64 B + one triangle of
+        # 48 B + 32 B ray in + 8 B result out; ceil(log2 T) node visits x 2 slab tests x 18 ops + one facet test of 60 ops.
+        per_seg_bytes = depth * 64 + 48 + 32 + 8
+        per_seg_ops = depth * 2 * 18 + 60
+        rays_per_launch = traced / launches_trace
+        t = avg_ms * 1e-3
+        alg_bw = rays_per_launch * per_seg_bytes / t / 1e9 if t > 0 else 0.0                  # GB/s
+        alg_ops = rays_per_launch * per_seg_ops / t / 1e12 if t > 0 else 0.0                  # T lane-op/s
+        fetched_bw = (nodes * 32 + tris * 48) / launches_trace / t / 1e9 if t > 0 else 0.0    # what the kernel really gathers
+        ms_stat = tot["ms"]
+        traffic, traffic_src = ncu_traffic(args.config)
+        roof = {"kernel": "k_trace_wf", "segments_per_launch": rays_per_launch, "avg_launch_ms": avg_ms,
+                "launches_timed": int(launches_trace), "traffic": traffic, "traffic_source": traffic_src,
+                "algorithmic_bytes_per_segment": per_seg_bytes, "algorithmic_ops_per_segment": per_seg_ops,
+                "nodes_per_traced_segment": nodes / max(traced, 1), "tri_tests_per_traced_segment": tris / max(traced, 1),
+                "share_of_step": {k: (tot[f] / ms_stat if ms_stat else None) for k, f in
+                                  (("seed+precull", "ms_seed"), ("sort", "ms_sort"), ("k_trace_wf", "ms_trace"),
+                                   ("k_reflect", "ms_reflect"), ("k_finish_final", "ms_finish"))}}
+        if peaks:
+            # ncu (profiles/) shows the L1TEX data pipe as the busiest unit of k_trace_wf (scattered 32-byte gathers that
+            # hit L2), then instruction issue; DRAM is a few per cent.  Binding roofline: the gather path, against the
+            # measured rate of independent 32-byte gathers over an array of the structure's size at this kernel's
+            # residency.  The fp32-issue and HBM views are reported beside it.
+            gpk = peaks["gather32_bytes_per_s"] / 1e9
+            roof.update({"bound": "l2-gather", "achieved": alg_bw, "peak": gpk, "unit": "GB/s", "frac": alg_bw / gpk,
+                         "peak_source": "measured in this run (tpmc_measure_peaks): independent 32-byte ld.global.nc gathers over "
+                                        "83 MB, 8 x 128 threads per SM",
+                         "fetched_view": {"achieved": fetched_bw, "peak": gpk, "unit": "GB/s", "frac": fetched_bw / gpk,
+                                          "what": "nodes x 32 B + facets x 48 B the kernel really fetched"},
+                         "alu_view": {"achieved": alg_ops, "peak": peaks["fp32_lane_ops_per_s"] / 1e12, "unit": "T lane-op/s",
+                                      "frac": alg_ops / (peaks["fp32_lane_ops_per_s"] / 1e12),
+                                      "peak_source": "measured in this run: FFMA lane-instructions/s at full occupancy"}})
+        else:
+            roof.update({"bound": "hbm", "achieved": alg_bw, "peak": hbm, "unit": "GB/s", "frac": alg_bw / hbm, "peak_source": hbm_src})
+        roof["hbm_view"] = {"achieved": alg_bw, "peak": hbm, "unit": "GB/s", "frac": alg_bw / hbm, "peak_source": hbm_src}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_total_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": WORKLOAD, "particles_per_step": N, "facets": mesh.nt, "bvh_nodes": info["n_nodes"],
-                       "attitudes": "fibonacci(64)[step*world+rank]", "cv_radius_factor": cfgs[0].cv_radius_factor,
-                       "l2": "inputs larger than L2: hierarchy + facets 149 MB (33 MB compact nodes, 66 MB fp32 nodes, 50 MB facets), per-facet momentum 25 MB, ~2 GB of lists and ray queues rewritten every wave",
+            "config": {"workload": WORKLOADS[args.config], "particles_per_step": N, "facets": mesh.nt, "bvh_nodes": info["n_nodes"],
+                       "sweep": f"{len(cfgs)} points, point (step*world+rank) mod {len(cfgs)}", "cv_radius_factor": cfgs[0].cv_radius_factor,
+                       "l2": ("inputs larger than L2: hierarchy + facets 149 MB, per-facet momentum 25 MB, ~2 GB of lists and ray "
+                              "queues rewritten every wave" if flush is None else
+                              "L2 flushed between steps (512 MB written); each step timed by its own event pair"),
                        "mesh_build_ms": info["build_ms"], "horizon_build_ms": info["horizon_ms"],
-                       "wave_particles": 1 << 26},
+                       "wave_particles": min(1 << 26, max(N, 256))},
             "clocks": clocks,
             "rates": {"segments_per_s": segs_all / (ms_total_max * 1e-3), "particles_per_s": parts_all / (ms_total_max * 1e-3),
                       "hits_per_particle": hits_all / parts_all},
-            "roofline": {"kernel": "k_trace_wf", "bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "TFLOP/s",
-                         "frac": alu_ach / alu_peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
-                         "peak_source": f"derived: {sms} SMs x 128 fp32 lanes x {clk_mhz:.0f} MHz sampled under this load "
-                                        "(one lane-instruction = 1 op; DESIGN.md section 7)",
-                         "algorithmic_ops_per_segment": ops_per_seg,
-                         "hbm_view": {"achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                                      "peak_source": peak_src, "algorithmic_bytes_per_segment": per_seg},
-                         "segments_per_launch": traced / launches_trace,
-                         "avg_launch_ms": avg_ms, "launches_timed": int(launches_trace),
-                         "share_of_step": {"k_seed": ms_seed / ms_stat if ms_stat else None,
-                                           "k_trace_wf": ms_trace / ms_stat if ms_stat else None,
-                                           "k_reflect": ms_reflect / ms_stat if ms_stat else None,
-                                           "k_finish": ms_finish / ms_stat if ms_stat else None},
-                         "nodes_per_traced_segment": nodes / max(traced, 1), "tri_tests_per_traced_segment": tris / max(traced, 1)},
+            "roofline": roof,
             "gpu_launches": int(launches),
         }
+        if peaks:
+            line["peaks"] = peaks
         if e2e:
-            line["e2e"] = {"value": hits_all / e2e_s_max, "unit": UNIT, "h2d_bytes_per_step": int(C.sizeof(tpmc.tpmc_params) + 16 * len(cfgs[0].m)),
+            line["e2e"] = {"value": hits_all / e2e_s_max, "unit": UNIT,
+                           "h2d_bytes_per_step": int(C.sizeof(tpmc.tpmc_params) + 16 * len(cfgs[0].m)),
                            "d2h_bytes_per_step": int(mesh.nt * 24 + 48), "api": "tpmc_run_host"}
         if world == 1 and not args.no_cpu_baseline:
             threads = os.cpu_count() or 1
@@ -310,7 +383,7 @@ def main():
             oracle_sample(cfgs, 1000, threads)
             h, dt, n = oracle_sample(cfgs, per, threads)
             line["cpu_baseline"] = {"value": h / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
-                                    "sample": f"{n} particles ({threads} slices of {per}) of the same N={N:.0e} stream, attitude 0, {dt:.1f} s"}
+                                    "sample": f"{n} particles ({threads} slices) of the same N={N:.0e} stream, sweep point 0, {dt:.1f} s"}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -39,14 +39,15 @@ extern "C" {
 #define TPMC_FACET_TWO_SIDED 1u /* facet_flags bit0 */
 #define TPMC_MAX_BOUNCES 0x0FFFFFFFu /* largest max_bounces (the bounce count shares a word with the species) */
 
-/* tpmc_params.flags.  The first five switch off (or force) steps that must not change any result -- the parity
- * tests run with and without them; the library's defaults are all zero. */
+/* tpmc_params.flags.  Each switches off, forces or adds a step that must not change any result -- the parity tests
+ * run with and without them; the library's defaults are all zero. */
 #define TPMC_FLAG_NO_PRECULL 0x01u  /* every particle through the fp64 sampler (no fp32 pre-cull pass) */
 #define TPMC_FLAG_NO_HORIZON 0x02u  /* every re-emitted ray is traced (no escape-horizon test) */
 #define TPMC_FLAG_ALIGN_OFF 0x04u   /* traversal on the body-frame hierarchy, whatever the attitude */
 #define TPMC_FLAG_ALIGN_ON 0x08u    /* traversal on the flow-aligned refit, whatever the attitude */
 #define TPMC_FLAG_EXACT_TRACE 0x10u /* every segment by the fp64 closest-hit search (no fp32 filter, no candidate lists) */
-#define TPMC_FLAG_NO_SORT 0x20u     /* rays traced in queue order (no spatial sort before the traversal) */
+#define TPMC_FLAG_NO_AGGREGATION 0x40u /* one fp64 atomic per hit and component even on bodies with few facets */
+#define TPMC_FLAG_SORT_RAYS 0x20u   /* rays traced in the order of a spatial key (counting sort before the traversal) */
 
 /* tpmc_params.control_volume */
 #define TPMC_CV_SPHERE 0 /* the paper's scheme: spherical control volume, eqs. (10)-(15) */
@@ -192,6 +193,26 @@ int tpmc_seed(const tpmc_mesh* mesh, const tpmc_params* params, void* cuda_strea
  * kernel and the exact resolve; synchronises the stream. */
 int tpmc_trace(tpmc_mesh* mesh, const float* d_o, const float* d_d, const int32_t* d_f_prev, int64_t n,
                const double* h_align_V, void* cuda_stream, int32_t* d_facet, double* d_tau);
+
+/* Measured peaks of the units that bound the kernels of the path (roofline denominators are measured,
+ * not nominal).  Hand-written micro-kernels, each timed once after a warm-up launch (about 0.1 s in all):
+ *   fp32 FFMA lane-instruction rate at full occupancy; fp64 FMA rate; 32-byte read-only gathers (one 256-bit load per
+ *   lane, every lane its own record) over an 83 MB array with the traversal kernel's residency (8 blocks of 128
+ *   threads per SM), with independent addresses and as a pointer chase; fp64 red.global.add at 1, 2048 and 1e6
+ *   accumulators laid out like the per-facet momentum.  out: host.  Synchronises the stream. */
+typedef struct {
+  int32_t sms;
+  double sm_clock_mhz_nominal;      /* cudaDevAttrClockRate */
+  double sm_clock_mhz_fp32;         /* fp32_lane_ops_per_s / (sms * 128): the clock if every lane issued every cycle */
+  double fp32_lane_ops_per_s;       /* FFMA lane-instructions per second (1 FFMA = 1 op here, 2 flops) */
+  double fp64_fma_per_s;            /* DFMA lane-instructions per second */
+  double gather32_bytes_per_s;      /* independent 32-byte gathers */
+  double gather32_dependent_bytes_per_s; /* pointer chase, same residency */
+  double gather_array_bytes;
+  double red_f64_per_s[3];          /* fp64 atomic adds per second ... */
+  double red_f64_addresses[3];      /* ... over this many accumulators */
+} tpmc_peaks;
+int tpmc_measure_peaks(tpmc_peaks* out, void* cuda_stream);
 
 const char* tpmc_strerror(int code);
 const char* tpmc_last_cuda_error(void);

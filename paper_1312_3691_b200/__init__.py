@@ -22,11 +22,12 @@ TPMC_MEM_HOST, TPMC_MEM_DEVICE = 0, 1
 TPMC_MAX_SPECIES = 8
 TPMC_MAX_BOUNCES = 0x0FFFFFFF
 TPMC_FLAG_NO_PRECULL, TPMC_FLAG_NO_HORIZON, TPMC_FLAG_ALIGN_OFF, TPMC_FLAG_ALIGN_ON = 0x01, 0x02, 0x04, 0x08
-TPMC_FLAG_EXACT_TRACE, TPMC_FLAG_NO_SORT = 0x10, 0x20
+TPMC_FLAG_EXACT_TRACE, TPMC_FLAG_SORT_RAYS, TPMC_FLAG_NO_AGGREGATION = 0x10, 0x20, 0x40
 TPMC_CV_SPHERE, TPMC_CV_BOX, TPMC_CV_BOX_UNWEIGHTED = 0, 1, 2
 
 EXPORTS = ["tpmc_mesh_create", "tpmc_mesh_destroy", "tpmc_mesh_info", "tpmc_mesh_copy_bvh", "tpmc_run",
-           "tpmc_mesh_copy_horizon", "tpmc_run_host", "tpmc_seed", "tpmc_trace", "tpmc_strerror", "tpmc_last_cuda_error", "tpmc_version"]
+           "tpmc_mesh_copy_horizon", "tpmc_run_host", "tpmc_seed", "tpmc_trace", "tpmc_strerror", "tpmc_last_cuda_error", "tpmc_version",
+           "tpmc_measure_peaks"]
 
 
 class TpmcError(RuntimeError):
@@ -60,6 +61,13 @@ class tpmc_stats(C.Structure):
                 ("ret_finish", C.c_uint64), ("queued_primaries", C.c_uint64), ("queued_reflected", C.c_uint64),
                 ("overflow_rays", C.c_uint64), ("final_stragglers", C.c_uint64), ("finish_segments", C.c_uint64),
                 ("ms_sort", C.c_double)]
+
+
+class tpmc_peaks(C.Structure):
+    _fields_ = [("sms", C.c_int32), ("sm_clock_mhz_nominal", C.c_double), ("sm_clock_mhz_fp32", C.c_double),
+                ("fp32_lane_ops_per_s", C.c_double), ("fp64_fma_per_s", C.c_double), ("gather32_bytes_per_s", C.c_double),
+                ("gather32_dependent_bytes_per_s", C.c_double), ("gather_array_bytes", C.c_double),
+                ("red_f64_per_s", C.c_double * 3), ("red_f64_addresses", C.c_double * 3)]
 
 
 class tpmc_debug(C.Structure):
@@ -96,6 +104,8 @@ def lib():
         L.tpmc_seed.argtypes = [vp, C.POINTER(tpmc_params), vp, vp, vp, vp]
         L.tpmc_trace.restype = C.c_int
         L.tpmc_trace.argtypes = [vp, vp, vp, vp, C.c_int64, vp, vp, vp, vp]
+        L.tpmc_measure_peaks.restype = C.c_int
+        L.tpmc_measure_peaks.argtypes = [C.POINTER(tpmc_peaks), vp]
         for n in ("tpmc_strerror", "tpmc_last_cuda_error", "tpmc_version"):
             getattr(L, n).restype = C.c_char_p
         L.tpmc_strerror.argtypes = [C.c_int]
@@ -328,6 +338,17 @@ def tpmc_seed(mesh: Mesh, cfg, **kw):
 
 def tpmc_trace(mesh: Mesh, o, d, f_prev=None, **kw):
     return mesh.trace(o, d, f_prev, **kw)
+
+
+def tpmc_measure_peaks(stream=None) -> dict:
+    """Measured peaks of the binding units (tpmc_measure_peaks): plain dict of the C struct's fields."""
+    _torch()
+    out = tpmc_peaks()
+    _check(lib().tpmc_measure_peaks(C.byref(out), _stream_ptr(stream)), "tpmc_measure_peaks")
+    d = {k: getattr(out, k) for k, _ in tpmc_peaks._fields_}
+    d["red_f64_per_s"] = list(out.red_f64_per_s)
+    d["red_f64_addresses"] = list(out.red_f64_addresses)
+    return d
 
 
 def tpmc_version() -> str:

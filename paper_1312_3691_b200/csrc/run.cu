@@ -390,9 +390,10 @@ struct Particle {
   int f_prev;
 };
 
+// P != nullptr: dp goes straight to the facet's accumulators (fp64 atomics); else the caller adds dp_out (a5).
 __device__ __forceinline__ int interact(const RunConst& rc, const float4* __restrict__ tris, Particle& p, const Hit& hit,
                                         double* __restrict__ P, double tq[3], const tpmc_debug& dbg,
-                                        const uint4* __restrict__ horizon) {
+                                        const uint4* __restrict__ horizon, double dp_out[3] = nullptr) {
   const float4 q0 = __ldg(tris + 3 * (size_t)hit.slot), q1 = __ldg(tris + 3 * (size_t)hit.slot + 1),
                q2 = __ldg(tris + 3 * (size_t)hit.slot + 2);
   const double w = rc.sp[p.species].w, cW = rc.sp[p.species].cW;
@@ -407,7 +408,8 @@ __device__ __forceinline__ int interact(const RunConst& rc, const float4* __rest
     vo[a] = (float)vout[a];
     hp[a] = __dadd_rn((double)p.o[a], __dmul_rn(hit.tau, (double)p.v[a]));
     dp[a] = w * ((double)p.v[a] - (double)vo[a]);
-    atomicAdd(&P[3 * (size_t)hit.facet + a], dp[a]);
+    if (P) atomicAdd(&P[3 * (size_t)hit.facet + a], dp[a]);
+    else dp_out[a] = dp[a];
   }
   const double rx = hp[0] - rc.x_ref[0], ry = hp[1] - rc.x_ref[1], rz = hp[2] - rc.x_ref[2];
   tq[0] += ry * dp[2] - rz * dp[1];
@@ -431,6 +433,44 @@ __device__ __forceinline__ int interact(const RunConst& rc, const float4* __rest
   return GO_ON;
 }
 
+// a5: per-facet momentum, warp-aggregated.  Lanes of a (converged) warp that hit the same facet are summed with
+// shuffles and their leader issues one fp64 atomic per component: one loop iteration per DISTINCT facet among the
+// warp's hits.  That pays when a body has few facets (C1: 2, C3: 2048 -- many lanes per facet, hot accumulators)
+// and costs when every lane has its own (C5), so the caller decides per run (aggregate = nt <= kAggregateMaxFacets).
+constexpr long long kAggregateMaxFacets = 4096;
+__device__ __forceinline__ void accumulate_warp(double* __restrict__ P, bool is_hit, int facet, const double dp[3],
+                                                bool aggregate) {
+  const unsigned FULL = 0xFFFFFFFFu;
+  if (!aggregate) {
+    if (is_hit)
+      for (int a = 0; a < 3; ++a) atomicAdd(&P[3 * (size_t)facet + a], dp[a]);
+    return;
+  }
+  const int lane = threadIdx.x & 31;
+  unsigned todo = __ballot_sync(FULL, is_hit);
+  while (todo) {
+    const int src = __ffs(todo) - 1;
+    const int f = __shfl_sync(FULL, facet, src);
+    const bool mine = is_hit && facet == f;
+    const unsigned grp = __ballot_sync(FULL, mine);
+    double s0 = mine ? dp[0] : 0.0, s1 = mine ? dp[1] : 0.0, s2 = mine ? dp[2] : 0.0;
+    if (grp != (1u << src)) {   // more than one lane on this facet: butterfly sum (zeros elsewhere)
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) {
+        s0 += __shfl_xor_sync(FULL, s0, off);
+        s1 += __shfl_xor_sync(FULL, s1, off);
+        s2 += __shfl_xor_sync(FULL, s2, off);
+      }
+    }
+    if (lane == src) {
+      atomicAdd(&P[3 * (size_t)f], s0);
+      atomicAdd(&P[3 * (size_t)f + 1], s1);
+      atomicAdd(&P[3 * (size_t)f + 2], s2);
+    }
+    todo &= ~grp;
+  }
+}
+
 // a4-a6: resolve the candidates of every hit ray with the exact fp64 test, apply the surface interaction,
 // accumulate, and queue the reflected ray for the next wavefront round (compacted, warp-aggregated).
 // Rays the traversal gave up on (too many candidates, stack too deep) and rays whose reflected successor
@@ -445,7 +485,7 @@ __global__ void __launch_bounds__(kTraceBlock, 6) k_reflect(const RunConst rc, u
                                                          unsigned int* __restrict__ ovf, unsigned int* __restrict__ n_ovf,
                                                          double* __restrict__ P, double* __restrict__ torque,
                                                          unsigned long long* __restrict__ stats, tpmc_debug dbg,
-                                                         const uint4* __restrict__ horizon) {
+                                                         const uint4* __restrict__ horizon, int aggregate) {
   __shared__ FlushShared fsh;
   const unsigned int n = *n_hits;
   const int lane = threadIdx.x & 31;
@@ -484,13 +524,15 @@ __global__ void __launch_bounds__(kTraceBlock, 6) k_reflect(const RunConst rc, u
     // that finds region A of the next queue full writes its new state back into its own slot of this queue
     // and goes to the overflow list, like one the traversal gave up on.
     bool go_on = false;
+    double dp[3] = {0.0, 0.0, 0.0};
     if (is_hit) {
       ++c[FC_HITS];
-      const int end = interact(rc, tris, p, hit, P, tq, dbg, horizon);
+      const int end = interact(rc, tris, p, hit, nullptr, tq, dbg, horizon, dp);
       go_on = end == GO_ON;
       c[FC_TRUNC] += end == END_TRUNCATED ? 1u : 0u;
       c[FC_HORIZON] += end == END_HORIZON ? 1u : 0u;
     }
+    accumulate_warp(P, is_hit, hit.facet, dp, aggregate != 0);
     const unsigned em = __ballot_sync(FULL, go_on);
     if (em) {
       const int leader = __ffs(em) - 1;
@@ -705,7 +747,7 @@ int make_run_const(const tpmc_mesh* m, const tpmc_params* p, RunConst* rc) {
   if (p->max_bounces < 1 || p->max_bounces > TPMC_MAX_BOUNCES) return TPMC_EINVAL;
   if (!(p->energy_accommodation >= 0.0 && p->energy_accommodation <= 1.0)) return TPMC_EINVAL;
   if ((p->flags & TPMC_FLAG_ALIGN_OFF) && (p->flags & TPMC_FLAG_ALIGN_ON)) return TPMC_EINVAL;
-  if (p->flags & ~0x3Fu) return TPMC_EINVAL;
+  if (p->flags & ~0x7Fu) return TPMC_EINVAL;
   if (p->wave_particles && (p->wave_particles < 256 || p->wave_particles > (1ull << 28))) return TPMC_EINVAL;
   if (p->chunk_particles > 0xF0000000ull) return TPMC_EINVAL;
   if (p->control_volume != TPMC_CV_SPHERE) return TPMC_EINVAL;   // TPMC_CV_BOX*: not in this build
@@ -982,7 +1024,8 @@ extern "C" int tpmc_run(tpmc_mesh* m, const tpmc_params* params, void* cuda_stre
   const bool precull = !(params->flags & TPMC_FLAG_NO_PRECULL);
   const bool use_horizon = !(params->flags & TPMC_FLAG_NO_HORIZON);
   const bool exact = (params->flags & TPMC_FLAG_EXACT_TRACE) != 0;
-  const bool sorted = !exact && !(params->flags & TPMC_FLAG_NO_SORT);
+  const bool sorted = !exact && (params->flags & TPMC_FLAG_SORT_RAYS);
+  const int aggregate = (m->nt <= kAggregateMaxFacets && !(params->flags & TPMC_FLAG_NO_AGGREGATION)) ? 1 : 0;
   // seed-time walk of the top of the hierarchy: pays only while the pre-cull pass has no two-level cull volume
   // (with it the pass is already tighter than the 64-node tree)
   const int seed_walk = m->cull_nbox < 0;
@@ -1105,7 +1148,7 @@ extern "C" int tpmc_run(tpmc_mesh* m, const tpmc_params* params, void* cuda_stre
         if (li >= 1) TPMC_CUDA_TRY(cudaStreamWaitEvent(s1, pp.ev_ovf[b ^ 1], 0));
         k_reflect<<<g.reflect, kTraceBlock, 0, s1>>>(rcc, cap, m->tris, Q[p], pp.hit_ray, pp.hit_cand, pp.ctr + 5, Q[p ^ 1],
                                                      pp.ctr + 2 * (p ^ 1), ovf, pp.ctr + 8 + b, P, m->totals, m->stats, dbg,
-                                                     use_horizon ? m->horizon : nullptr);
+                                                     use_horizon ? m->horizon : nullptr, aggregate);
         launches += 2;
       } else {
         if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[3], s1));

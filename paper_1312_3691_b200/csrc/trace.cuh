@@ -403,6 +403,9 @@ __device__ __forceinline__ void walk_node(Walk& w, const uint4* __restrict__ cno
   // phase) and the walk goes on with the far child, or with the top of the stack.  The two entries below the
   // top are always read, the slot above it is written whenever both boxes are hit.
   const bool both = h0 && h1, any = h0 || h1;
+#ifdef TPMC_COUNT_STALE
+  if (!any) ++cnt.tris;   // experiment: visits that hit neither child
+#endif
   const bool swp = h1 && (!h0 || n1 < n0);
   const int c0 = (int)b.z, c1 = (int)b.w;
   const int nearc = swp ? c1 : c0, farc = swp ? c0 : c1;

@@ -63,7 +63,7 @@ def test_struct_layouts_match_header(libpath, tmp_path):
             t.tpmc_stats.ms_sort.offset]
     assert got == want
     assert (t.TPMC_FLAG_NO_PRECULL, t.TPMC_FLAG_NO_HORIZON, t.TPMC_FLAG_ALIGN_OFF, t.TPMC_FLAG_ALIGN_ON,
-            t.TPMC_FLAG_EXACT_TRACE, t.TPMC_FLAG_NO_SORT) == (1, 2, 4, 8, 16, 32)
+            t.TPMC_FLAG_EXACT_TRACE, t.TPMC_FLAG_SORT_RAYS) == (1, 2, 4, 8, 16, 32)
 
 
 def test_library_reads_no_environment_variable():

@@ -44,3 +44,57 @@ def test_single_rank_is_identity():
     import bench
     assert bench.reduce_over_ranks([3.0], [4.0, 5.0], 1) == ([3.0], [4.0, 5.0])
     assert [bench.attitude_index(k, 0, 1, 64) for k in (0, 1, 63, 64)] == [0, 1, 63, 0]
+
+
+def _slice_worker(rank, world, port, out):
+    """SURVEY 8(e), the particle-range split: each rank runs its (first, count) slice of ONE run and the outputs are
+    summed across ranks.  On the CPU box the slice results come from the oracle (slices are additive on both sides)."""
+    sys.path.insert(0, ROOT)
+    import numpy as np
+    import bench
+    import oracle
+    import tpmc_inputs as ti
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    cfg = ti.config("C4")[5].with_(N=30_000, mesh_fn=lambda: ti.satellite(4, 0.25))
+    cfg._mesh_cache = []
+    m = cfg.mesh()
+    om = oracle.OracleMesh(m.vertices, m.indices, m.flags)
+    first, count = bench.slice_of(rank, world, cfg.N)
+    r = om.run(cfg, first=first, count=count, debug=False)
+    F, Tq, P, hits = bench.sum_slices([r.force, r.torque, r.facet_momentum, np.array([float(r.hits)])], world)
+    res = None
+    if rank == 0:
+        full = om.run(cfg, debug=False)
+        res = (float(np.abs(F.numpy() - full.force).max() / np.abs(full.force).max()),
+               float(np.abs(Tq.numpy() - full.torque).max() / max(np.abs(full.torque).max(), 1e-30)),
+               float(np.abs(P.numpy() - full.facet_momentum).max() / np.abs(full.facet_momentum).max()),
+               int(hits.item()) == full.hits, (first, count))
+    out.put((rank, (first, count), res))
+    dist.destroy_process_group()
+
+
+def test_two_ranks_sum_particle_slices_of_one_run():
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 31500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_slice_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=180) for _ in procs)
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    (_, s0, r0), (_, s1, _) = res
+    assert s0 == (0, 15_000) and s1 == (15_000, 15_000)                       # disjoint cover of [0, N)
+    eF, eT, eP, same_hits, _ = r0
+    assert eF < 1e-12 and eT < 1e-11 and eP < 1e-12 and same_hits
+
+
+def test_slices_cover_the_stream():
+    sys.path.insert(0, ROOT)
+    import bench
+    for N, world in ((10, 3), (1_000_000_007, 8), (5, 8)):
+        s = [bench.slice_of(r, world, N) for r in range(world)]
+        assert s[0][0] == 0 and sum(c for _, c in s) == N
+        assert all(s[k][0] + s[k][1] == s[k + 1][0] for k in range(world - 1))

@@ -684,7 +684,7 @@ def test_equilibrium_through_the_whole_path(T, O):
 def _arms(T):
     return [("no pre-cull", T.TPMC_FLAG_NO_PRECULL), ("no horizon", T.TPMC_FLAG_NO_HORIZON),
             ("body-frame boxes", T.TPMC_FLAG_ALIGN_OFF), ("flow-aligned boxes", T.TPMC_FLAG_ALIGN_ON),
-            ("unsorted", T.TPMC_FLAG_NO_SORT),
+            ("rays sorted by key", T.TPMC_FLAG_SORT_RAYS),
             ("fp64 search, nothing skipped", T.TPMC_FLAG_EXACT_TRACE | T.TPMC_FLAG_NO_PRECULL | T.TPMC_FLAG_NO_HORIZON)]
 
 
