@@ -33,7 +33,7 @@ class _Params(C.Structure):
                 ("m", C.POINTER(C.c_double)), ("x", C.POINTER(C.c_double)),
                 ("cv_radius_factor", C.c_double), ("N", C.c_uint64), ("first", C.c_uint64),
                 ("count", C.c_uint64), ("seed", C.c_uint64), ("max_bounces", C.c_uint32),
-                ("x_ref", C.c_double * 3)]
+                ("x_ref", C.c_double * 3), ("energy_accommodation", C.c_double)]
 
 
 class _Stats(C.Structure):
@@ -61,6 +61,7 @@ def lib():
         L.oracle_mesh_create.argtypes = [vp, C.c_int64, vp, C.c_int64, vp]
         L.oracle_mesh_destroy.argtypes = [vp]
         L.oracle_mesh_bounds.argtypes = [vp, dp, dp]
+        L.oracle_mesh_set_surface.argtypes = [vp, vp, vp]
         L.oracle_closest_hit.restype = C.c_int32
         L.oracle_closest_hit.argtypes = [vp, vp, vp, C.c_int32, C.c_int, dp]
         L.oracle_seed.restype = C.c_int
@@ -152,6 +153,14 @@ class OracleMesh:
         except Exception:
             pass
 
+    def set_surface(self, T_W=None, sigma=None):
+        """Per-facet wall temperature and accommodation (A23); None = the run's scalar."""
+        tw = None if T_W is None else np.ascontiguousarray(T_W, dtype=np.float64)
+        sg = None if sigma is None else np.ascontiguousarray(sigma, dtype=np.float64)
+        assert tw is None or tw.shape == (self.nt,)
+        assert sg is None or sg.shape == (self.nt,)
+        lib().oracle_mesh_set_surface(self._h, None if tw is None else tw.ctypes.data, None if sg is None else sg.ctypes.data)
+
     def bounds(self):
         c = (C.c_double * 3)()
         r = C.c_double()
@@ -182,6 +191,7 @@ class OracleMesh:
         p.seed = int(cfg.seed)
         p.max_bounces = int(cfg.max_bounces)
         p.x_ref = (C.c_double * 3)(*[float(a) for a in cfg.x_ref])
+        p.energy_accommodation = float(getattr(cfg, "energy_accommodation", 1.0))
         return p, (m, x)
 
     def seed(self, cfg, i, N=None):

@@ -19,6 +19,9 @@
  * control-volume invariance and rotation covariance (P11), BVH == brute force (P12),
  * specular limits (P13), Pratt's concave hemisphere (P14), torque about an off-centre
  * reference point = panel sum of (centroid - x_ref) x F_f, and the A14 shift identity (P16).
+ * Per-facet wall temperature / accommodation and partial energy accommodation (NEXT-3, readings A22/A23 of
+ * DESIGN.md): panel sum with per-facet S_W and sigma, quadrature of the re-emission momentum flux with
+ * T_r = alpha_E T_W + (1 - alpha_E) m v_in^2 / (3 k_B), and alpha_E = 1 / uniform arrays reproducing the scalar run (P17).
  * No function here is "parity unpinned".
  */
 #include <math.h>
@@ -164,6 +167,8 @@ typedef struct oracle_mesh {
   bvh_node* nodes;
   int32_t n_nodes;
   int32_t* perm;
+  double* surf_TW;    /* [nt] wall temperature per facet, or NULL: the run's T_W (A23) */
+  double* surf_sigma; /* [nt] accommodation per facet, or NULL: the run's sigma (A23) */
 } oracle_mesh;
 
 static void tri_corner(const oracle_mesh* m, int64_t f, int k, double p[3]) {
@@ -250,7 +255,15 @@ oracle_mesh* oracle_mesh_create(const float* v, int64_t nv, const int32_t* idx, 
 }
 void oracle_mesh_destroy(oracle_mesh* m) {
   if (!m) return;
-  free(m->v); free(m->idx); free(m->flags); free(m->nodes); free(m->perm); free(m);
+  free(m->v); free(m->idx); free(m->flags); free(m->nodes); free(m->perm); free(m->surf_TW); free(m->surf_sigma); free(m);
+}
+/* A23: surface properties per facet ("arbitrary surface interaction"; re-emission "determined by the satellite
+ * surface temperature").  Either array may be NULL (back to the run's scalar). */
+void oracle_mesh_set_surface(oracle_mesh* m, const double* T_W, const double* sigma) {
+  free(m->surf_TW); free(m->surf_sigma);
+  m->surf_TW = NULL; m->surf_sigma = NULL;
+  if (T_W) { m->surf_TW = (double*)malloc(sizeof(double) * (size_t)m->nt); memcpy(m->surf_TW, T_W, sizeof(double) * (size_t)m->nt); }
+  if (sigma) { m->surf_sigma = (double*)malloc(sizeof(double) * (size_t)m->nt); memcpy(m->surf_sigma, sigma, sizeof(double) * (size_t)m->nt); }
 }
 void oracle_mesh_bounds(const oracle_mesh* m, double centre[3], double* Rb) {
   for (int a = 0; a < 3; ++a) centre[a] = m->centre[a];
@@ -355,6 +368,7 @@ typedef struct {
   uint64_t N, first, count, seed;
   uint32_t max_bounces;
   double x_ref[3];
+  double energy_accommodation; /* alpha_E (A22); 1 = full accommodation to T_W */
 } oracle_params;
 
 typedef struct { uint64_t hits, segments, escaped, truncated; } oracle_stats;
@@ -416,9 +430,15 @@ void oracle_reflect(const oracle_mesh* mesh, const oracle_params* p, int32_t f, 
   double vn = dot3(v, nf);
   double sgn = (vn < 0.0) ? 1.0 : -1.0;
   double ne[3] = {sgn * nf[0], sgn * nf[1], sgn * nf[2]}; /* n_eff faces the incoming particle */
-  if (u[0] < p->accommodation) {
-    /* diffuse, fully accommodated to T_W: flux-weighted half-Maxwellian (A6) */
-    double cw = sqrt(2.0 * ORACLE_KB * p->T_W / p->m[species]);
+  double sigma = mesh->surf_sigma ? mesh->surf_sigma[f] : p->accommodation; /* A23 */
+  if (u[0] < sigma) {
+    /* diffuse: flux-weighted half-Maxwellian (A6) at the re-emission temperature
+     *   T_r = alpha_E T_W + (1 - alpha_E) T_k,i,   T_k,i = m v_in^2 / (3 k_B)   (A22; alpha_E = 1: T_r = T_W exactly) */
+    double TW = mesh->surf_TW ? mesh->surf_TW[f] : p->T_W;
+    double aE = p->energy_accommodation;
+    double Tki = p->m[species] * dot3(v, v) / (3.0 * ORACLE_KB);
+    double Tr = aE * TW + (1.0 - aE) * Tki;
+    double cw = sqrt(2.0 * ORACLE_KB * Tr / p->m[species]);
     double el = sqrt(dot3(e1, e1));
     double t1[3] = {e1[0] / el, e1[1] / el, e1[2] / el};
     double t2[3];

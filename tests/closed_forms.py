@@ -146,3 +146,28 @@ def panel_sum(tri, flags, upstream, S, S_W, sigma=1.0):
 
 def thermal_speed(T, m):
     return np.sqrt(2 * K_B * T / m)
+
+
+# ------------------------------------------------------------------ partial energy accommodation (reading A22)
+def reemission_pressure_alpha_e(S, S_W, gamma, alpha_e):
+    """Normal momentum flux of diffuse re-emission from a one-sided flat element, in units of q = rho V^2 / 2, when a
+    molecule arriving with velocity v leaves as a flux-weighted half-Maxwellian at
+        T_r = alpha_E T_W + (1 - alpha_E) m |v|^2 / (3 k_B)        (reading A22 of DESIGN.md).
+    With x = v / c_mp:  c_r(x)^2 / c_mp^2 = alpha_E (S/S_W)^2 + (1 - alpha_E) (2/3) |x|^2,  each re-emitted molecule
+    carries the mean normal momentum m (sqrt(pi)/2) c_r, and the incident flux density is n c_mp x_n f(x):
+        p_r = (sqrt(pi) / S^2) int_{x_n > 0} x_n pi^{-3/2} exp(-|x - S_vec|^2) (c_r(x) / c_mp) d^3x .
+    alpha_E = 1 gives chi(s) / (2 S S_W), the standard panel term.  Gauss-Hermite in the two tangential components,
+    adaptive quadrature in the normal one."""
+    s, st = S * gamma, S * np.sqrt(max(0.0, 1.0 - gamma * gamma))
+    xh, wh = np.polynomial.hermite.hermgauss(64)          # int e^{-x^2} g(x) dx ~ sum w g(x)
+    T1, T2 = np.meshgrid(xh + st, xh, indexing="ij")
+    W = np.outer(wh, wh)
+    r2t = T1 ** 2 + T2 ** 2
+
+    def inner(xn):
+        cr = np.sqrt(alpha_e * (S / S_W) ** 2 + (1.0 - alpha_e) * (2.0 / 3.0) * (xn * xn + r2t))
+        return xn * np.exp(-(xn - s) ** 2) * float((W * cr).sum())
+
+    lo = max(0.0, s - 7.0)
+    val, _ = integrate.quad(inner, lo, max(s, 0.0) + 7.0, epsabs=1e-13, epsrel=1e-11, limit=200)
+    return SQRTPI / S ** 2 * np.pi ** -1.5 * val

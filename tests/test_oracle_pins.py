@@ -445,3 +445,92 @@ def test_a14_moving_the_reference_point():
     scale = np.linalg.norm(dx) * np.linalg.norm(a.force) + np.linalg.norm(a.torque)
     assert np.linalg.norm(b.torque - (a.torque - np.cross(dx, a.force))) <= 1e-11 * scale
     assert np.linalg.norm(np.cross(dx, a.force)) > 1e-3 * scale       # the shift is not a no-op
+
+
+# ------------------------------------------------------------------ P17: surface models beyond one global T_W, sigma (NEXT-3)
+def test_p17_quadrature_reduces_to_the_panel_term():
+    # the reference of the alpha_E pin is itself pinned: alpha_E = 1 must give chi(s) / (2 S S_W)
+    for S, SW, g in ((7.356804, 13.431624, 0.8660254), (2.0, 5.0, 0.3), (5.0, 9.0, -0.2)):
+        want = float(cf.chi(S * g)) / (2 * S * SW)
+        assert cf.reemission_pressure_alpha_e(S, SW, g, 1.0) == pytest.approx(want, rel=1e-9)
+
+
+def test_p17_per_facet_wall_temperature_and_accommodation_vs_panel_sum():
+    """A23: T_W and sigma per facet.  On a convex body the expectation is still the panel sum, now with S_W,f and
+    sigma_f per facet; hot/cold halves give a side force that a global T_W cannot."""
+    m = ti.geodesic_sphere(4)
+    cen = m.triangles().mean(1)
+    TW = np.where(cen[:, 1] > 0, 200.0, 1500.0)
+    sg = np.where(cen[:, 2] > 0, 1.0, 0.5)
+    om = omesh(m)
+    om.set_surface(TW, sg)
+    cfg = ti.RunConfig("surf", None, T_inf=1000.0, T_W=300.0, accommodation=1.0, N=200_000, seed=51)
+    r = om.run(cfg, use_bvh=False)
+    se = r.force_stderr(cfg.N) / cfg.q_inf
+    F = r.force / cfg.q_inf
+    S = cfg.speed / cf.thermal_speed(cfg.T_inf, cfg.m[0])
+    SWf = cfg.speed / cf.thermal_speed(TW, cfg.m[0])
+    Fp, _, _ = cf.panel_sum(m.triangles(), m.flags, [1, 0, 0], S, SWf, sigma=sg)
+    assert np.all(np.abs(F - Fp) < 4 * se), (F, Fp, se)
+    Fu, _, _ = cf.panel_sum(m.triangles(), m.flags, [1, 0, 0], S, cfg.speed / cf.thermal_speed(300.0, cfg.m[0]), sigma=1.0)
+    assert abs(Fp[1] - Fu[1]) > 8 * se[1] and abs(Fp[2] - Fu[2]) > 8 * se[2]     # the arrays matter: side forces appear
+    # NULL arrays fall back to the run's scalars; uniform arrays equal to the scalars change nothing, bit for bit
+    om.set_surface(None, None)
+    a = om.run(cfg.with_(N=20_000), use_bvh=False)
+    om.set_surface(np.full(m.nt, 300.0), np.full(m.nt, 1.0))
+    b = om.run(cfg.with_(N=20_000), use_bvh=False)
+    assert np.array_equal(a.force, b.force) and np.array_equal(a.hash, b.hash) and np.array_equal(a.facet_momentum, b.facet_momentum)
+
+
+@pytest.mark.parametrize("alpha_e", [0.5, 0.0])
+def test_p17_energy_accommodation_vs_quadrature(alpha_e):
+    """A22: re-emission at T_r = alpha_E T_W + (1 - alpha_E) m v_in^2 / (3 k_B), per particle.  On the C1 plate the
+    expected force is the incident part of the panel sum plus the re-emission pressure integrated over the incident
+    flux (closed_forms.reemission_pressure_alpha_e); full accommodation (the paper's case) is many sigma away."""
+    cfg = ti.config("C1")[0].with_(N=240_000, seed=52, energy_accommodation=alpha_e)
+    m = cfg.mesh()
+    r = omesh(m).run(cfg, use_bvh=False)
+    se = r.force_stderr(cfg.N) / cfg.q_inf
+    F = r.force / cfg.q_inf
+    up = -np.array(cfg.V) / cfg.speed
+    tri = m.triangles()
+    Ng = np.cross(tri[:, 1] - tri[:, 0], tri[:, 2] - tri[:, 0])
+    A = 0.5 * np.linalg.norm(Ng, axis=1)
+    n0 = Ng / (2 * A)[:, None]
+    Finc, _, _ = cf.panel_sum(tri, m.flags, up, S1, 1e30)              # incident momentum only (no re-emission term)
+    want = Finc.copy()
+    for side in (+1.0, -1.0):                                          # two-sided sheet: both faces re-emit
+        for f in range(m.nt):
+            g = float(side * n0[f] @ up)
+            want += -A[f] * cf.reemission_pressure_alpha_e(S1, SW1, g, alpha_e) * side * n0[f]
+    assert np.all(np.abs(F - want) < 4 * se), (F, want, se)
+    Ffull, _, _ = cf.panel_sum(tri, m.flags, up, S1, SW1)
+    assert abs(want[0] - Ffull[0]) > 30 * se[0]
+    # alpha_E = 1 is the scalar model, bit for bit
+    a = omesh(m).run(cfg.with_(N=20_000, energy_accommodation=1.0), use_bvh=False)
+    b = omesh(m).run(ti.config("C1")[0].with_(N=20_000, seed=52), use_bvh=False)
+    assert np.array_equal(a.force, b.force) and np.array_equal(a.hash, b.hash)
+
+
+def test_p17_equilibrium_with_per_facet_arrays():
+    """P10 again with the wall temperature given per facet (all equal to T_inf) and alpha_E = 1: per-facet pressure
+    -n k_B T A_f n_f on the pocket floor and zero net force, through any number of reflections."""
+    m = ti.satellite(seed=2, h=0.25)
+    om = omesh(m)
+    T = 500.0
+    om.set_surface(np.full(m.nt, T), np.ones(m.nt))
+    cfg = ti.RunConfig("eq", None, T_inf=T, T_W=123.0, accommodation=0.3, V=(0.0, 0.0, 0.0), N=240_000, seed=5, cv_radius_factor=1.05)
+    per = cfg.N // 8
+    runs = [om.run(cfg, first=k * per, count=per) for k in range(8)]
+    tri = m.triangles()
+    Ng = np.cross(tri[:, 1] - tri[:, 0], tri[:, 2] - tri[:, 0])
+    A = 0.5 * np.linalg.norm(Ng, axis=1)
+    nh = Ng / (2 * A)[:, None]
+    cen = tri.mean(1)
+    g = (np.abs(cen[:, 2] - 0.5) < 1e-6) & (np.abs(cen[:, 0]) < 0.31) & (np.abs(cen[:, 1]) < 0.31)
+    vals = np.array([np.einsum("ij,ij->", r.facet_momentum[g], nh[g]) * 8 for r in runs])
+    want = -cfg.n * cf.K_B * T * A[g].sum()
+    se = vals.std(ddof=1) / np.sqrt(8)
+    assert abs(vals.mean() - want) < 4 * se and se < 0.2 * abs(want)
+    Fs = np.array([r.force for r in runs]) * 8
+    assert np.all(np.abs(Fs.mean(0)) < 4 * Fs.std(0, ddof=1) / np.sqrt(8))
