@@ -148,6 +148,13 @@ int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t* indices, 
 void tpmc_mesh_destroy(tpmc_mesh* mesh);
 int tpmc_mesh_info(const tpmc_mesh* mesh, tpmc_mesh_info_t* out /* host */);
 
+/* Surface properties per facet (reading A23; "arbitrary surface interaction"; re-emission "determined by the
+ * satellite surface temperature"): T_W [nt] wall temperature (K, > 0) and sigma [nt] accommodation in [0,1],
+ * indexed by facet id as in `indices`, both where mem_space says; either may be NULL, which restores the run's scalar
+ * (tpmc_params.T_W / .accommodation).  The arrays are copied; they apply to every later run on this handle.
+ * Synchronises the stream (before replacing arrays a run may still read, and after the copy). */
+int tpmc_mesh_set_surface(tpmc_mesh* mesh, const double* T_W, const double* sigma, int mem_space, void* cuda_stream);
+
 /* Copy the built hierarchy to the host for inspection: nodes [n_nodes][16] floats
  * (lo0.xyz hi0.xyz lo1.xyz hi1.xyz, then child0, child1 as int32 bit patterns, 2 pad words;
  * child >= 0: internal node, child < 0: leaf holding sorted triangle ~child),

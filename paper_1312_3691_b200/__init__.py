@@ -27,7 +27,7 @@ TPMC_CV_SPHERE, TPMC_CV_BOX, TPMC_CV_BOX_UNWEIGHTED = 0, 1, 2
 
 EXPORTS = ["tpmc_mesh_create", "tpmc_mesh_destroy", "tpmc_mesh_info", "tpmc_mesh_copy_bvh", "tpmc_run",
            "tpmc_mesh_copy_horizon", "tpmc_run_host", "tpmc_seed", "tpmc_trace", "tpmc_strerror", "tpmc_last_cuda_error", "tpmc_version",
-           "tpmc_measure_peaks"]
+           "tpmc_measure_peaks", "tpmc_mesh_set_surface"]
 
 
 class TpmcError(RuntimeError):
@@ -92,6 +92,8 @@ def lib():
         L.tpmc_mesh_destroy.argtypes = [vp]
         L.tpmc_mesh_info.restype = C.c_int
         L.tpmc_mesh_info.argtypes = [vp, C.POINTER(tpmc_mesh_info_t)]
+        L.tpmc_mesh_set_surface.restype = C.c_int
+        L.tpmc_mesh_set_surface.argtypes = [vp, vp, vp, C.c_int, vp]
         L.tpmc_mesh_copy_bvh.restype = C.c_int
         L.tpmc_mesh_copy_bvh.argtypes = [vp, vp, vp]
         L.tpmc_mesh_copy_horizon.restype = C.c_int
@@ -218,6 +220,16 @@ class Mesh:
                 "aabb_lo": np.array(list(out.aabb_lo)), "aabb_hi": np.array(list(out.aabb_hi)),
                 "nt": int(out.nt), "n_nodes": int(out.n_nodes), "build_ms": out.build_ms, "horizon_ms": out.horizon_ms}
 
+    def set_surface(self, T_W=None, sigma=None, stream=None):
+        """Per-facet wall temperature / accommodation (tpmc_mesh_set_surface); None restores the run's scalar."""
+        tw = None if T_W is None else np.ascontiguousarray(T_W, dtype=np.float64)
+        sg = None if sigma is None else np.ascontiguousarray(sigma, dtype=np.float64)
+        for a in (tw, sg):
+            if a is not None and a.shape != (self.nt,):
+                raise TpmcError("surface arrays must have one entry per facet")
+        _check(lib().tpmc_mesh_set_surface(self._h, None if tw is None else tw.ctypes.data, None if sg is None else sg.ctypes.data,
+                                           TPMC_MEM_HOST, _stream_ptr(stream)), "tpmc_mesh_set_surface")
+
     def copy_bvh(self):
         n_nodes = self.info()["n_nodes"]
         nodes = np.zeros((n_nodes, 16), dtype=np.float32)
@@ -314,6 +326,10 @@ def tpmc_mesh_destroy(mesh: Mesh) -> None:
 
 def tpmc_mesh_info(mesh: Mesh) -> dict:
     return mesh.info()
+
+
+def tpmc_mesh_set_surface(mesh: Mesh, T_W=None, sigma=None, **kw) -> None:
+    mesh.set_surface(T_W, sigma, **kw)
 
 
 def tpmc_mesh_copy_bvh(mesh: Mesh):

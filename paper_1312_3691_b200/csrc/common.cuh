@@ -70,6 +70,8 @@ struct tpmc_mesh {
   QuantGrid* grid_dev;             // [2] device copies of the grids the traversal reads: body frame, aligned
   uint4* cnodes;                   // compact copy of `nodes` for the wavefront traversal: 2 uint4 = 32 B per node
   float q_origin[3], q_scale[3];   // its quantisation grid: x = q_origin + q * q_scale, q in [0, 65535]
+  double* surf_TW;                 // [nt] by facet id: wall temperature per facet, or nullptr (tpmc_mesh_set_surface, A23)
+  double* surf_sigma;              // [nt] by facet id: accommodation per facet, or nullptr
   uint4* horizon;                  // [nt] by sorted slot: escape horizon of each facet, 16 azimuth sectors x 1 byte (k_horizon, lbvh.cu)
   double horizon_ms;
   uint4* cull_c;                   // top of the hierarchy (<= kCullNodes nodes, breadth-first) in the compact format of `cnodes`: seed-time cull
@@ -113,6 +115,7 @@ struct QuantGrid {
 
 // Per-run constants (a1: host, fp64), passed to kernels by value.
 struct SpeciesConst {
+  double m;      // molecular mass, kg
   double c;      // c_mp = sqrt(2 k_B T_inf / m)
   double S;      // speed ratio |V| / c_mp
   double cW;     // sqrt(2 k_B T_W / m)
@@ -129,6 +132,10 @@ struct RunConst {
   double centre[3];
   double r;             // control-sphere radius
   double sigma;
+  double T_W, alpha_E;              // wall temperature and energy accommodation of the run (A22)
+  const double* surf_TW;            // per-facet overrides by facet id, or nullptr (A23)
+  const double* surf_sigma;
+  int simple_surface;               // alpha_E == 1 and no per-facet T_W: c_W is the per-species constant
   double x_ref[3];
   float aabb_lo[3], aabb_hi[3];
   unsigned long long first, count;

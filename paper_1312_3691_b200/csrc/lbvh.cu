@@ -805,7 +805,7 @@ int tpmc_mesh_align(tpmc_mesh* m, const double R[9], cudaStream_t st, const Quan
 
 extern "C" void tpmc_mesh_destroy(tpmc_mesh* m) {
   if (!m) return;
-  cudaFree(m->nodes); cudaFree(m->tris); cudaFree(m->cull_c); cudaFree(m->kids); cudaFree(m->parent); cudaFree(m->arrive); cudaFree(m->rbox); cudaFree(m->nodes_r); cudaFree(m->cnodes_r); cudaFree(m->align_R); cudaFree(m->grid_dev); cudaFree(m->cnodes); cudaFree(m->horizon);
+  cudaFree(m->nodes); cudaFree(m->tris); cudaFree(m->cull_c); cudaFree(m->kids); cudaFree(m->parent); cudaFree(m->arrive); cudaFree(m->rbox); cudaFree(m->nodes_r); cudaFree(m->cnodes_r); cudaFree(m->align_R); cudaFree(m->grid_dev); cudaFree(m->cnodes); cudaFree(m->horizon); cudaFree(m->surf_TW); cudaFree(m->surf_sigma);
   for (int pi = 0; pi < kPipes; ++pi) {
     Pipe& pp = m->pipe[pi];
     for (int k = 0; k < 2; ++k) { cudaFree(pp.q_o[k]); cudaFree(pp.q_v[k]); cudaFree(pp.q_f[k]); cudaFree(pp.q_key[k]); cudaFree(pp.hist[k]); }
@@ -834,6 +834,30 @@ extern "C" void tpmc_mesh_destroy(tpmc_mesh* m) {
   if (m->ev1) cudaEventDestroy(m->ev1);
   if (m->ev_fork) cudaEventDestroy(m->ev_fork);
   delete m;
+}
+
+// A23: per-facet wall temperature and accommodation, by facet id; either may be NULL (the run's scalar is used).
+extern "C" int tpmc_mesh_set_surface(tpmc_mesh* m, const double* T_W, const double* sigma, int mem_space, void* cuda_stream) {
+  if (!m || (mem_space != TPMC_MEM_HOST && mem_space != TPMC_MEM_DEVICE)) return TPMC_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t bytes = sizeof(double) * (size_t)m->nt;
+  const cudaMemcpyKind kind = mem_space == TPMC_MEM_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+  if (mem_space == TPMC_MEM_HOST) {   // validate what can be read here: T_W > 0, 0 <= sigma <= 1
+    for (int64_t f = 0; f < m->nt; ++f) {
+      if (T_W && !(T_W[f] > 0.0 && isfinite(T_W[f]))) return TPMC_EINVAL;
+      if (sigma && !(sigma[f] >= 0.0 && sigma[f] <= 1.0)) return TPMC_EINVAL;
+    }
+  }
+  TPMC_CUDA_TRY(cudaStreamSynchronize(st));   // no run may still read the arrays being replaced
+  const double* src[2] = {T_W, sigma};
+  double** dst[2] = {&m->surf_TW, &m->surf_sigma};
+  for (int k = 0; k < 2; ++k) {
+    if (!src[k]) { cudaFree(*dst[k]); *dst[k] = nullptr; continue; }
+    if (!*dst[k]) TPMC_CUDA_TRY(cudaMalloc((void**)dst[k], bytes));
+    TPMC_CUDA_TRY(cudaMemcpyAsync(*dst[k], src[k], bytes, kind, st));
+  }
+  TPMC_CUDA_TRY(cudaStreamSynchronize(st));
+  return TPMC_OK;
 }
 
 extern "C" int tpmc_mesh_info(const tpmc_mesh* m, tpmc_mesh_info_t* out) {

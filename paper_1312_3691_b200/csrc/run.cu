@@ -396,10 +396,23 @@ __device__ __forceinline__ int interact(const RunConst& rc, const float4* __rest
                                         const uint4* __restrict__ horizon, double dp_out[3] = nullptr) {
   const float4 q0 = __ldg(tris + 3 * (size_t)hit.slot), q1 = __ldg(tris + 3 * (size_t)hit.slot + 1),
                q2 = __ldg(tris + 3 * (size_t)hit.slot + 2);
-  const double w = rc.sp[p.species].w, cW = rc.sp[p.species].cW;
+  const double w = rc.sp[p.species].w;
+  // A23: accommodation and wall temperature of the facet hit; A22: re-emission temperature of this particle,
+  // T_r = alpha_E T_W + (1 - alpha_E) m v_in^2 / (3 k_B), every operation rounded separately (the definition fixes the order)
+  const double sigma = rc.surf_sigma ? __ldg(rc.surf_sigma + hit.facet) : rc.sigma;
+  double cW = rc.sp[p.species].cW;
+  if (!rc.simple_surface) {
+    const double ms = rc.sp[p.species].m;
+    const double TW = rc.surf_TW ? __ldg(rc.surf_TW + hit.facet) : rc.T_W;
+    const double vx = (double)p.v[0], vy = (double)p.v[1], vz = (double)p.v[2];
+    const double v2 = __dadd_rn(__dadd_rn(__dmul_rn(vx, vx), __dmul_rn(vy, vy)), __dmul_rn(vz, vz));
+    const double Tki = __ddiv_rn(__dmul_rn(ms, v2), __dmul_rn(3.0, TPMC_KB));
+    const double Tr = __dadd_rn(__dmul_rn(rc.alpha_E, TW), __dmul_rn(__dsub_rn(1.0, rc.alpha_E), Tki));
+    cW = sqrt(__ddiv_rn(__dmul_rn(__dmul_rn(2.0, TPMC_KB), Tr), ms));
+  }
   double vout[3];
   float sin_e, phi;
-  reflect(q0, q1, q2, p.v, rc.sigma, cW, particle_block(rc, rc.first + p.j, 2u + p.k), vout, sin_e, phi);
+  reflect(q0, q1, q2, p.v, sigma, cW, particle_block(rc, rc.first + p.j, 2u + p.k), vout, sin_e, phi);
   // O12: dp = w (v_in - v_out) on the fp32 values; hit point o + tau v in fp64
   double hp[3], dp[3];
   float vo[3];
@@ -765,6 +778,7 @@ int make_run_const(const tpmc_mesh* m, const tpmc_params* p, RunConst* rc) {
   double acc = 0.0;
   for (int s = 0; s < p->n_species; ++s) {
     SpeciesConst& sc = rc->sp[s];
+    sc.m = p->m[s];
     sc.c = sqrt(2.0 * TPMC_KB * p->T_inf / p->m[s]);
     sc.S = speed / sc.c;
     sc.cW = sqrt(2.0 * TPMC_KB * p->T_W / p->m[s]);
@@ -789,6 +803,11 @@ int make_run_const(const tpmc_mesh* m, const tpmc_params* p, RunConst* rc) {
     rc->key_r2 = rk * rk;
   }
   rc->sigma = p->accommodation;
+  rc->T_W = p->T_W;
+  rc->alpha_E = p->energy_accommodation;
+  rc->surf_TW = m->surf_TW;
+  rc->surf_sigma = m->surf_sigma;
+  rc->simple_surface = (p->energy_accommodation == 1.0 && !m->surf_TW) ? 1 : 0;
   rc->first = p->first;
   rc->count = p->count;
   rc->seed_lo = (unsigned int)p->seed;

@@ -57,8 +57,8 @@ def check_conservation(st, count, exact=False):
         assert st["traced_rays"] + st["final_stragglers"] == st["queued_primaries"] + st["queued_reflected"], st
 
 
-def compare_run(T, O, cfg, first, count, use_bvh=True, **run_kw):
-    gm, om = meshes(T, O, cfg)
+def compare_run(T, O, cfg, first, count, use_bvh=True, pair=None, **run_kw):
+    gm, om = pair if pair is not None else meshes(T, O, cfg)
     g = gm.run(cfg, first=first, count=count, debug=True, **run_kw)
     check_conservation(g.stats, count, exact=bool(run_kw.get("flags", 0) & T.TPMC_FLAG_EXACT_TRACE))
     o = om.run(cfg, first=first, count=count, use_bvh=use_bvh)
@@ -725,3 +725,60 @@ def test_c5_every_shortcut_off_at_full_size(T, att):
 def test_c2_c3_c4_every_shortcut_off_at_timing_size(T, name, idx):
     """The same at the timing sizes of SURVEY 8(d): C2 N = 1e7, C3 N = 1e8, C4 N = 1e8."""
     _full_size_arms(T, ti.config(name)[idx], _arms(T))
+
+
+# ------------------------------------------------------------------ NEXT-3: surface models beyond one global T_W, sigma
+def test_per_facet_surface_and_energy_accommodation_parity(T, O):
+    """Readings A22 / A23 against the oracle (whose versions are pinned by P17): wall temperature and accommodation
+    per facet, partial energy accommodation, both together on a concave body with a gas mixture; and alpha_E = 1 with
+    uniform arrays equal to the scalars reproduces the scalar run."""
+    m = ti.satellite(4, 0.1)
+    gm = T.Mesh(m.vertices, m.indices, m.flags)
+    om = O.OracleMesh(m.vertices, m.indices, m.flags)
+    cen = m.triangles().mean(1)
+    TW = np.where(cen[:, 1] > 0, 200.0, 1500.0) + 50.0 * np.sin(7.0 * cen[:, 0])
+    sg = np.where(cen[:, 2] > 0, 1.0, 0.5)
+    base = ti.config("C4")[6].with_(N=1_000_000, mesh_fn=lambda: m, m=(16.0 * ti.AMU, 4.0 * ti.AMU), x=(0.6, 0.4))
+    base._mesh_cache = [m]
+    ref = gm.run(base, first=0, count=150_000, debug=True)
+    # (1) alpha_E < 1, scalar surface
+    g1, o1, _ = compare_run(T, O, base.with_(energy_accommodation=0.4), 0, 150_000, pair=(gm, om))
+    assert not np.allclose(g1.force.cpu().numpy(), ref.force.cpu().numpy(), rtol=1e-3)        # the model does act
+    # (2) per-facet arrays, alpha_E = 1
+    gm.set_surface(TW, sg)
+    om.set_surface(TW, sg)
+    g2, o2, _ = compare_run(T, O, base, 0, 150_000, pair=(gm, om))
+    assert not np.allclose(g2.force.cpu().numpy(), ref.force.cpu().numpy(), rtol=1e-3)
+    # (3) both
+    compare_run(T, O, base.with_(energy_accommodation=0.7), 300_000, 150_000, pair=(gm, om))
+    # (4) only sigma per facet; T_W from the run
+    gm.set_surface(None, sg)
+    om.set_surface(None, sg)
+    compare_run(T, O, base, 0, 100_000, pair=(gm, om))
+    # (5) uniform arrays equal to the run's scalars: the scalar run again (same hashes; sums to the atomics' order)
+    gm.set_surface(np.full(m.nt, base.T_W), np.full(m.nt, base.accommodation))
+    u = gm.run(base, first=0, count=150_000, debug=True)
+    assert bool((u.hash == ref.hash).all())
+    assert np.linalg.norm(u.force.cpu().numpy() - ref.force.cpu().numpy()) <= 1e-12 * np.linalg.norm(ref.force.cpu().numpy())
+    gm.set_surface(None, None)
+    z = gm.run(base, first=0, count=150_000, debug=True)
+    assert bool((z.hash == ref.hash).all())
+    with pytest.raises(T.TpmcError):
+        gm.set_surface(np.full(m.nt, -1.0), None)
+    with pytest.raises(T.TpmcError):
+        gm.run(base.with_(energy_accommodation=1.5))
+    gm.close()
+
+
+def test_warp_aggregated_accumulation_changes_nothing(T, O):
+    """a5: on bodies with few facets the reflect step sums the lanes of a warp that hit the same facet before its fp64
+    atomics; with TPMC_FLAG_NO_AGGREGATION every hit issues its own.  Same per-facet sums to the order of the additions."""
+    for name, idx, count in (("C1", 0, 100_000), ("C3", 1, 3_000_000)):
+        cfg = ti.config(name)[idx]
+        gm, om = meshes(T, O, cfg)
+        a = gm.run(cfg, first=0, count=count, debug=True)
+        b = gm.run(cfg, first=0, count=count, debug=True, flags=T.TPMC_FLAG_NO_AGGREGATION)
+        assert a.stats["hits"] == b.stats["hits"] > 0 and bool((a.hash == b.hash).all())
+        fa, fb = a.facet_momentum.cpu().numpy(), b.facet_momentum.cpu().numpy()
+        assert np.all(np.abs(fa - fb) <= 1e-11 * np.abs(fb).max(0))
+        assert np.array_equal(np.linalg.norm(fa, axis=1) == 0, np.linalg.norm(fb, axis=1) == 0)
