@@ -33,7 +33,8 @@ class _Params(C.Structure):
                 ("m", C.POINTER(C.c_double)), ("x", C.POINTER(C.c_double)),
                 ("cv_radius_factor", C.c_double), ("N", C.c_uint64), ("first", C.c_uint64),
                 ("count", C.c_uint64), ("seed", C.c_uint64), ("max_bounces", C.c_uint32),
-                ("x_ref", C.c_double * 3), ("energy_accommodation", C.c_double)]
+                ("x_ref", C.c_double * 3), ("energy_accommodation", C.c_double),
+                ("control_volume", C.c_int32), ("pad_", C.c_int32)]
 
 
 class _Stats(C.Structure):
@@ -53,7 +54,7 @@ def lib():
         L.oracle_flux_bracket.argtypes = [C.c_double]
         L.oracle_flux.restype = C.c_double
         L.oracle_flux.argtypes = [C.c_double] * 4
-        for name in ("oracle_position_cdf", "oracle_position_inv", "oracle_vn_cdf", "oracle_vn_inv"):
+        for name in ("oracle_position_cdf", "oracle_position_inv", "oracle_vn_cdf", "oracle_vn_inv", "oracle_vn_unweighted_inv"):
             getattr(L, name).restype = C.c_double
             getattr(L, name).argtypes = [C.c_double, C.c_double]
         L.oracle_rotation.argtypes = [dp, dp]
@@ -104,6 +105,10 @@ def vn_cdf(x, s):
 
 def vn_inv(u, s):
     return lib().oracle_vn_inv(float(u), float(s))
+
+
+def vn_unweighted_inv(u, s):
+    return lib().oracle_vn_unweighted_inv(float(u), float(s))
 
 
 def rotation(V):
@@ -192,6 +197,7 @@ class OracleMesh:
         p.max_bounces = int(cfg.max_bounces)
         p.x_ref = (C.c_double * 3)(*[float(a) for a in cfg.x_ref])
         p.energy_accommodation = float(getattr(cfg, "energy_accommodation", 1.0))
+        p.control_volume = int(getattr(cfg, "control_volume", 0))
         return p, (m, x)
 
     def seed(self, cfg, i, N=None):

@@ -164,6 +164,7 @@ typedef struct oracle_mesh {
   int32_t* idx;   /* [nt][3] */
   uint8_t* flags; /* [nt] */
   double centre[3], Rb;
+  double lo[3], hi[3]; /* AABB of the vertices */
   bvh_node* nodes;
   int32_t n_nodes;
   int32_t* perm;
@@ -230,7 +231,7 @@ oracle_mesh* oracle_mesh_create(const float* v, int64_t nv, const int32_t* idx, 
   double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
   for (int64_t i = 0; i < nv; ++i)
     for (int a = 0; a < 3; ++a) { double p = (double)v[3 * i + a]; if (p < lo[a]) lo[a] = p; if (p > hi[a]) hi[a] = p; }
-  for (int a = 0; a < 3; ++a) m->centre[a] = 0.5 * (lo[a] + hi[a]);
+  for (int a = 0; a < 3; ++a) { m->centre[a] = 0.5 * (lo[a] + hi[a]); m->lo[a] = lo[a]; m->hi[a] = hi[a]; }
   double r2 = 0.0;
   for (int64_t i = 0; i < nv; ++i) {
     double dx = (double)v[3 * i] - m->centre[0], dy = (double)v[3 * i + 1] - m->centre[1], dz = (double)v[3 * i + 2] - m->centre[2];
@@ -369,13 +370,88 @@ typedef struct {
   uint32_t max_bounces;
   double x_ref[3];
   double energy_accommodation; /* alpha_E (A22); 1 = full accommodation to T_W */
+  int32_t control_volume;      /* 0 sphere (the paper's scheme); 1 box, flux-weighted; 2 box, inward speed NOT flux-weighted (A24, A25) */
+  int32_t pad_;
 } oracle_params;
 
 typedef struct { uint64_t hits, segments, escaped, truncated; } oracle_stats;
 
+/* ------------------------------------------------------------------ rectangular control volume (A24, A25) */
+/* "placing particles with a random uniform distribution on the six faces of a rectangular control volume.  The number
+ * of particles to cross each face derives from the analytical molecular flux across a flat plate with given normal
+ * velocity component of the free stream".  Box: the AABB of the vertices scaled by cv_radius_factor about its
+ * centre (half-extent at least 0.05 R_b per axis).  Face k = 2a + side: side 0 at -h_a with inward normal +e_a, side 1
+ * at +h_a with inward normal -e_a.  Flux through a face with inward bulk component s_k = V.n_k / c:
+ * Gamma_k = A_k n c chi(s_k) / (2 sqrt(pi))  (the integrand of eq. (8) on a plane). */
+typedef struct { double h[3], area[6], sn[6], cum[6], total; } box_cv;
+static void box_setup(const oracle_mesh* mesh, const oracle_params* p, int s, box_cv* b) {
+  double c = sqrt(2.0 * ORACLE_KB * p->T_inf / p->m[s]);
+  for (int a = 0; a < 3; ++a) {
+    double h = 0.5 * (mesh->hi[a] - mesh->lo[a]);
+    if (h < 0.05 * mesh->Rb) h = 0.05 * mesh->Rb;
+    b->h[a] = p->cv_radius_factor * h;
+  }
+  double acc = 0.0;
+  for (int k = 0; k < 6; ++k) {
+    int a = k / 2, side = k % 2;
+    b->area[k] = 4.0 * b->h[(a + 1) % 3] * b->h[(a + 2) % 3];
+    b->sn[k] = (side ? -p->V[a] : p->V[a]) / c;
+    acc += b->area[k] * chi(b->sn[k]);
+    b->cum[k] = acc;
+  }
+  b->total = acc; /* Gamma / (n c / (2 sqrt(pi))) */
+}
+double oracle_box_flux(const oracle_mesh* mesh, const oracle_params* p, int s) {
+  box_cv b;
+  box_setup(mesh, p, s, &b);
+  double c = sqrt(2.0 * ORACLE_KB * p->T_inf / p->m[s]);
+  return b.total * p->n * c / (2.0 * SQRTPI);
+}
+/* A25 (negative control): inward speed from the half-range Maxwellian WITHOUT the flux weight, density
+ * ~ e^{-(x-s)^2} on x > 0: survival 1 - F = erfc(x - s) / erfc(-s).  Bracketed Newton like the other inverses. */
+double oracle_vn_unweighted_inv(double u, double s) {
+  double target = (1.0 - u) * erfc(-s);
+  double lo = 0.0, hi = (s > 0.0 ? s : 0.0) + 8.0, x = (s > 0.0 ? s : 0.0) + 0.5;
+  for (int it = 0; it < 400; ++it) {
+    double f = erfc(x - s) - target; /* decreasing in x */
+    if (f > 0.0) lo = x; else hi = x;
+    double z = x - s;
+    double d = -2.0 / SQRTPI * exp(-z * z);
+    double xn = (d < 0.0) ? x - f / d : 0.5 * (lo + hi);
+    if (!(xn > lo && xn < hi)) xn = 0.5 * (lo + hi);
+    if (fabs(xn - x) <= 1e-16 * (1.0 + x) || hi - lo <= 1e-16 * (1.0 + x)) { x = xn; break; }
+    x = xn;
+  }
+  return x;
+}
+static int seed_box(const oracle_mesh* mesh, const oracle_params* p, uint64_t i, double x[3], double v[3]) {
+  double ub0[4], ub1[4];
+  particle_block(p->seed, i, 0u, ub0);
+  particle_block(p->seed, i, 1u, ub1);
+  int s = 0; double acc = p->x[0];
+  while (s < p->n_species - 1 && ub0[0] >= acc) { ++s; acc += p->x[s]; }
+  double c = sqrt(2.0 * ORACLE_KB * p->T_inf / p->m[s]);
+  box_cv b;
+  box_setup(mesh, p, s, &b);
+  int k = 0;
+  while (k < 5 && ub0[1] * b.total >= b.cum[k]) ++k;   /* face with probability Gamma_k / Gamma */
+  int a = k / 2, side = k % 2, e1 = (a + 1) % 3, e2 = (a + 2) % 3;
+  x[a] = mesh->centre[a] + (side ? b.h[a] : -b.h[a]);
+  x[e1] = mesh->centre[e1] + (2.0 * ub0[2] - 1.0) * b.h[e1];     /* uniform on the face */
+  x[e2] = mesh->centre[e2] + (2.0 * ub0[3] - 1.0) * b.h[e2];
+  double xn = (p->control_volume == 2) ? oracle_vn_unweighted_inv(ub1[0], b.sn[k]) : oracle_vn_inv(ub1[0], b.sn[k]);
+  double rho = sqrt(-log(ub1[1]));
+  double ang = TWOPI * ub1[2];
+  v[a] = c * (side ? -xn : xn);                                   /* inward */
+  v[e1] = c * (p->V[e1] / c + rho * cos(ang));                    /* Maxwellian about the bulk tangential components */
+  v[e2] = c * (p->V[e2] / c + rho * sin(ang));
+  return s;
+}
+
 /* ------------------------------------------------------------------ O4-O8: seed one particle */
 /* Returns the species; x[3], v[3] are the fp64 values BEFORE the fp32 rounding of O9. */
 int oracle_seed(const oracle_mesh* mesh, const oracle_params* p, uint64_t i, double x[3], double v[3]) {
+  if (p->control_volume != 0) return seed_box(mesh, p, i, x, v);
   double ub0[4], ub1[4];
   particle_block(p->seed, i, 0u, ub0);
   particle_block(p->seed, i, 1u, ub1);
@@ -479,7 +555,8 @@ int oracle_run(const oracle_mesh* mesh, const oracle_params* p, int use_bvh,
     int s = oracle_seed(mesh, p, i, x64, v64);
     /* O2: weight w_s = m_s Gamma_s / N ("effective mass") */
     double c = sqrt(2.0 * ORACLE_KB * p->T_inf / p->m[s]);
-    double w = p->m[s] * oracle_flux(speed / c, c, p->n, r) / (double)p->N;
+    double flux = (p->control_volume != 0) ? oracle_box_flux(mesh, p, s) : oracle_flux(speed / c, c, p->n, r);
+    double w = p->m[s] * flux / (double)p->N;
     /* O9: the particle IS the ray defined by these fp32 values */
     float o[3] = {(float)x64[0], (float)x64[1], (float)x64[2]};
     float v[3] = {(float)v64[0], (float)v64[1], (float)v64[2]};

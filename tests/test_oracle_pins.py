@@ -534,3 +534,54 @@ def test_p17_equilibrium_with_per_facet_arrays():
     assert abs(vals.mean() - want) < 4 * se and se < 0.2 * abs(want)
     Fs = np.array([r.force for r in runs]) * 8
     assert np.all(np.abs(Fs.mean(0)) < 4 * Fs.std(0, ddof=1) / np.sqrt(8))
+
+
+# ------------------------------------------------------------------ P18: rectangular control volume (NEXT-4)
+def test_p18_unweighted_normal_speed_inverse():
+    from scipy import special
+    for s in (-3.0, -0.5, 0.0, 1.0, 7.4):
+        for u in (1e-6, 0.01, 0.3, 0.77, 0.999):
+            want = s + special.erfcinv((1.0 - u) * special.erfc(-s))
+            assert oracle.vn_unweighted_inv(u, s) == pytest.approx(want, rel=1e-9, abs=1e-12)
+
+
+def _drag_over_q(om, cfg):
+    r = om.run(cfg, use_bvh=True, facets=False)
+    up = -np.array(cfg.V) / cfg.speed
+    return r, (r.force / cfg.q_inf) @ (-up), np.linalg.norm(r.force_stderr(cfg.N) / cfg.q_inf)
+
+
+def test_p18_box_control_volume_exact_and_negative_control():
+    """The scheme the paper replaces: uniform seeding on the six faces of a box, the share of each face from the
+    flat-plate flux.  Done consistently (inward speed from the flux-weighted law (14a), reading A24) it is exact: the
+    force on a convex body is the panel sum at any attitude, the hit count is N Gamma_body / Gamma_box, and it agrees
+    with the spherical scheme.  With the inward speed drawn WITHOUT the flux weight (reading A25, the negative
+    control) the drag depends on the attitude of the stream to the box, as in the paper's Fig. 1."""
+    m = ti.geodesic_sphere(4)
+    om = omesh(m)
+    dev = {}
+    for ang in (0.0, 45.0):
+        a = np.deg2rad(ang)
+        V = (-7500.0 * np.cos(a), -7500.0 * np.sin(a), 0.0)
+        up = -np.array(V) / 7500.0
+        Fp, flux, _ = cf.panel_sum(m.triangles(), m.flags, up, S1, SW1)
+        want = Fp @ (-up)
+        cfg = ti.RunConfig("box", None, V=V, N=400_000, seed=61, control_volume=1)
+        r, drag, se = _drag_over_q(om, cfg)
+        assert abs(drag - want) < 4 * se, (ang, drag, want, se)
+        # share of the box flux that reaches the body: sum_f Gamma_f / Gamma_box (every hit is a first hit: convex)
+        h = 1.5 * 0.5 * (m.vertices.max(0) - m.vertices.min(0)).astype(np.float64)
+        gbox = 0.0
+        for ax in range(3):
+            area = 4.0 * h[(ax + 1) % 3] * h[(ax + 2) % 3]
+            for sgn in (+1.0, -1.0):
+                gbox += area * float(cf.chi(S1 * sgn * V[ax] / 7500.0)) / (2 * np.sqrt(np.pi))
+        pin = flux.sum() / gbox
+        assert abs(r.hits - cfg.N * pin) < 4 * np.sqrt(cfg.N * pin * (1 - pin))
+        rs, drag_s, se_s = _drag_over_q(om, cfg.with_(control_volume=0))
+        assert abs(drag - drag_s) < 4 * np.hypot(se, se_s)               # box and sphere schemes agree
+        ru, drag_u, se_u = _drag_over_q(om, cfg.with_(control_volume=2))
+        dev[ang] = ((drag_u - want) / want, se_u / want)
+    # negative control: biased at 45 deg by several sigma, and the bias changes with the attitude
+    assert abs(dev[45.0][0]) > 5 * dev[45.0][1]
+    assert abs(dev[45.0][0] - dev[0.0][0]) > 4 * np.hypot(dev[45.0][1], dev[0.0][1])

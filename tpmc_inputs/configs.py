@@ -34,6 +34,7 @@ class RunConfig:
     max_bounces: int = 1024
     x_ref: Tuple[float, float, float] = (0.0, 0.0, 0.0)
     energy_accommodation: float = 1.0      # alpha_E: 1 = re-emission at T_W (the paper's case)
+    control_volume: int = 0                # 0 sphere (the paper's scheme), 1 box, 2 box with unweighted inward speed
     A_ref: float = 1.0                     # m^2, for coefficients only
     label: str = ""
     _mesh_cache: list = field(default_factory=list, repr=False, compare=False)
