@@ -181,6 +181,14 @@ int tpmc_mesh_copy_horizon(const tpmc_mesh* mesh, uint8_t* h_horizon);
 int tpmc_run(tpmc_mesh* mesh, const tpmc_params* params, void* cuda_stream, double* d_force,
              double* d_torque, double* d_facet_momentum, tpmc_stats* h_stats, const tpmc_debug* debug);
 
+/* An attitude sweep in one call (the paper's application: force and moment coefficients over a range of attitudes,
+ * P:243, Figs. 8-9): run k (k < n_attitudes) is `params` with V replaced by h_V[k] (host [n_attitudes][3];
+ * sweeps rotate V, not the mesh).  d_force, d_torque device [n_attitudes][3]; d_facet_momentum device
+ * [n_attitudes][nt][3] or NULL; h_stats host [n_attitudes] or NULL (when given, the stream is synchronised after every
+ * attitude).  Stops at the first failing attitude and returns its code. */
+int tpmc_run_sweep(tpmc_mesh* mesh, const tpmc_params* params, int32_t n_attitudes, const double* h_V, void* cuda_stream,
+                   double* d_force, double* d_torque, double* d_facet_momentum, tpmc_stats* h_stats);
+
 /* Same run with HOST result buffers (h_facet_momentum may be NULL): device results are copied back
  * inside the call and the stream is synchronised before returning. */
 int tpmc_run_host(tpmc_mesh* mesh, const tpmc_params* params, void* cuda_stream, double* h_force,

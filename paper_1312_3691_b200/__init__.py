@@ -27,7 +27,7 @@ TPMC_CV_SPHERE, TPMC_CV_BOX, TPMC_CV_BOX_UNWEIGHTED = 0, 1, 2
 
 EXPORTS = ["tpmc_mesh_create", "tpmc_mesh_destroy", "tpmc_mesh_info", "tpmc_mesh_copy_bvh", "tpmc_run",
            "tpmc_mesh_copy_horizon", "tpmc_run_host", "tpmc_seed", "tpmc_trace", "tpmc_strerror", "tpmc_last_cuda_error", "tpmc_version",
-           "tpmc_measure_peaks", "tpmc_mesh_set_surface"]
+           "tpmc_measure_peaks", "tpmc_mesh_set_surface", "tpmc_run_sweep"]
 
 
 class TpmcError(RuntimeError):
@@ -100,6 +100,8 @@ def lib():
         L.tpmc_mesh_copy_horizon.argtypes = [vp, vp]
         L.tpmc_run.restype = C.c_int
         L.tpmc_run.argtypes = [vp, C.POINTER(tpmc_params), vp, vp, vp, vp, C.POINTER(tpmc_stats), C.POINTER(tpmc_debug)]
+        L.tpmc_run_sweep.restype = C.c_int
+        L.tpmc_run_sweep.argtypes = [vp, C.POINTER(tpmc_params), C.c_int32, vp, vp, vp, vp, vp, vp]
         L.tpmc_run_host.restype = C.c_int
         L.tpmc_run_host.argtypes = [vp, C.POINTER(tpmc_params), vp, vp, vp, vp, C.POINTER(tpmc_stats)]
         L.tpmc_seed.restype = C.c_int
@@ -266,6 +268,25 @@ class Mesh:
         sd = None if st is None else {k: getattr(st, k) for k, _ in tpmc_stats._fields_}
         return RunResult(force, torque, fm, sd, hs, nb, ff)
 
+    def sweep(self, cfg, velocities, facets=False, stats=False, stream=None, flags=0):
+        """tpmc_run_sweep: one run per row of `velocities` [K,3]; returns (force [K,3], torque [K,3], facet momentum
+        [K,nt,3] or None, list of stats dicts or None), device tensors."""
+        torch = _torch()
+        p, keep = make_params(cfg, flags=flags)
+        V = np.ascontiguousarray(velocities, dtype=np.float64).reshape(-1, 3)
+        K = int(V.shape[0])
+        dev = torch.device("cuda", torch.cuda.current_device())
+        force = torch.empty((K, 3), dtype=torch.float64, device=dev)
+        torque = torch.empty((K, 3), dtype=torch.float64, device=dev)
+        fm = torch.empty((K, self.nt, 3), dtype=torch.float64, device=dev) if facets else None
+        st = (tpmc_stats * K)() if stats else None
+        rc = lib().tpmc_run_sweep(self._h, C.byref(p), K, V.ctypes.data, _stream_ptr(stream), force.data_ptr() or None,
+                                  torque.data_ptr() or None, None if fm is None else fm.data_ptr(),
+                                  None if st is None else C.cast(st, C.c_void_p))
+        _check(rc, "tpmc_run_sweep")
+        sd = None if st is None else [{k: getattr(s, k) for k, _ in tpmc_stats._fields_} for s in st]
+        return force, torque, fm, sd
+
     def run_host(self, cfg, first=None, count=None, N=None, facets=True, stats=True, stream=None,
                  out_facets: Optional[np.ndarray] = None, flags=0):
         """tpmc_run_host: results land in HOST numpy buffers (D2H copies inside the call)."""
@@ -342,6 +363,10 @@ def tpmc_mesh_copy_horizon(mesh: Mesh):
 
 def tpmc_run(mesh: Mesh, cfg, **kw) -> RunResult:
     return mesh.run(cfg, **kw)
+
+
+def tpmc_run_sweep(mesh: Mesh, cfg, velocities, **kw):
+    return mesh.sweep(cfg, velocities, **kw)
 
 
 def tpmc_run_host(mesh: Mesh, cfg, **kw):

@@ -123,6 +123,8 @@ struct SpeciesConst {
   double g0;     // Gt(-S)                                  (position CDF constants, O5)
   double gI;     // Gt(S) - Gt(-S)
   double cumx;   // cumulative number fraction
+  // rectangular control volume (A24): per face k = 2 axis + side, inward bulk component / c, cumulative A_k chi(s_k)
+  double bsn[6], bcum[6];
 };
 
 struct RunConst {
@@ -142,6 +144,9 @@ struct RunConst {
   unsigned int seed_lo, seed_hi;
   unsigned int max_bounces;
   float key_c[3], key_r2;   // sort key of a ray (sort.cuh): body centre, (radius of the key sphere)^2
+  int control_volume;       // TPMC_CV_*
+  double box_h[3];          // half-extents of the rectangular control volume (A24)
+  double V[3];              // bulk velocity (the box scheme needs its components, not only the stream frame)
 };
 
 // Device counters of a run (tpmc_stats: every one is counted where the event happens).

@@ -179,7 +179,8 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
   if (active) {
     float hint[2] = {0.0f, 0.0f};
     if (hinted) { hint[0] = __uint_as_float(__ldcs(surv + cap_s + sl)); hint[1] = __uint_as_float(__ldcs(surv + 2 * cap_s + sl)); }
-    const SeedState s = seed_particle(rc, rc.first + wave_first + j, hinted ? hint : nullptr);
+    const SeedState s = rc.control_volume == TPMC_CV_SPHERE ? seed_particle(rc, rc.first + wave_first + j, hinted ? hint : nullptr)
+                                                            : seed_particle_box(rc, rc.first + wave_first + j);
     species = s.species;
 #pragma unroll
     for (int k = 0; k < 3; ++k) { o[k] = (float)s.x[k]; v[k] = (float)s.v[k]; }
@@ -677,7 +678,7 @@ __global__ void k_seed_only(const RunConst rc, double* __restrict__ x, double* _
                             int32_t* __restrict__ species) {
   const unsigned long long j = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x;
   if (j >= rc.count) return;
-  const SeedState s = seed_particle(rc, rc.first + j);
+  const SeedState s = rc.control_volume == TPMC_CV_SPHERE ? seed_particle(rc, rc.first + j) : seed_particle_box(rc, rc.first + j);
   for (int k = 0; k < 3; ++k) { x[3 * j + k] = s.x[k]; v[3 * j + k] = s.v[k]; }
   if (species) species[j] = s.species;
 }
@@ -763,7 +764,7 @@ int make_run_const(const tpmc_mesh* m, const tpmc_params* p, RunConst* rc) {
   if (p->flags & ~0x7Fu) return TPMC_EINVAL;
   if (p->wave_particles && (p->wave_particles < 256 || p->wave_particles > (1ull << 28))) return TPMC_EINVAL;
   if (p->chunk_particles > 0xF0000000ull) return TPMC_EINVAL;
-  if (p->control_volume != TPMC_CV_SPHERE) return TPMC_EINVAL;   // TPMC_CV_BOX*: not in this build
+  if (p->control_volume < TPMC_CV_SPHERE || p->control_volume > TPMC_CV_BOX_UNWEIGHTED) return TPMC_EINVAL;
   double xs = 0.0;
   for (int s = 0; s < p->n_species; ++s) {
     if (!(p->m[s] > 0.0) || !(p->x[s] >= 0.0)) return TPMC_EINVAL;
@@ -775,6 +776,12 @@ int make_run_const(const tpmc_mesh* m, const tpmc_params* p, RunConst* rc) {
   memset(rc, 0, sizeof(*rc));
   const double speed = sqrt((p->V[0] * p->V[0] + p->V[1] * p->V[1]) + p->V[2] * p->V[2]);
   const double r = p->cv_radius_factor * m->Rb;
+  rc->control_volume = p->control_volume;
+  for (int a = 0; a < 3; ++a) {   // A24: the vertex AABB scaled about its centre, at least 0.05 R_b per axis
+    const double h = std::max(0.5 * ((double)m->aabb_hi[a] - (double)m->aabb_lo[a]), 0.05 * m->Rb);
+    rc->box_h[a] = p->cv_radius_factor * h;
+    rc->V[a] = p->V[a];
+  }
   double acc = 0.0;
   for (int s = 0; s < p->n_species; ++s) {
     SpeciesConst& sc = rc->sp[s];
@@ -782,7 +789,19 @@ int make_run_const(const tpmc_mesh* m, const tpmc_params* p, RunConst* rc) {
     sc.c = sqrt(2.0 * TPMC_KB * p->T_inf / p->m[s]);
     sc.S = speed / sc.c;
     sc.cW = sqrt(2.0 * TPMC_KB * p->T_W / p->m[s]);
-    sc.w = p->m[s] * (host_flux_bracket(sc.S) * sc.c * p->n * r * r) / (double)p->N;
+    double flux = host_flux_bracket(sc.S) * sc.c * p->n * r * r;   // eq. (10)
+    {
+      double bacc = 0.0;
+      for (int k = 0; k < 6; ++k) {
+        const int a = k / 2, side = k % 2;
+        const double area = 4.0 * rc->box_h[(a + 1) % 3] * rc->box_h[(a + 2) % 3];
+        sc.bsn[k] = (side ? -p->V[a] : p->V[a]) / sc.c;
+        bacc += area * (exp(-sc.bsn[k] * sc.bsn[k]) + TPMC_SQRTPI * sc.bsn[k] * erfc(-sc.bsn[k]));
+        sc.bcum[k] = bacc;
+      }
+      if (p->control_volume != TPMC_CV_SPHERE) flux = bacc * p->n * sc.c / (2.0 * TPMC_SQRTPI);   // sum of the face fluxes
+    }
+    sc.w = p->m[s] * flux / (double)p->N;
     sc.g0 = host_Gt(-sc.S);
     sc.gI = host_Gt(sc.S) - sc.g0;
     acc += p->x[s];
@@ -1040,7 +1059,7 @@ extern "C" int tpmc_run(tpmc_mesh* m, const tpmc_params* params, void* cuda_stre
   const Grids& g = grids();
   const int K = g.pipes;
   const bool timed = (h_stats != nullptr);   // per-kernel events only when the caller will read them
-  const bool precull = !(params->flags & TPMC_FLAG_NO_PRECULL);
+  const bool precull = !(params->flags & TPMC_FLAG_NO_PRECULL) && params->control_volume == TPMC_CV_SPHERE;
   const bool use_horizon = !(params->flags & TPMC_FLAG_NO_HORIZON);
   const bool exact = (params->flags & TPMC_FLAG_EXACT_TRACE) != 0;
   const bool sorted = !exact && (params->flags & TPMC_FLAG_SORT_RAYS);
@@ -1215,6 +1234,23 @@ extern "C" int tpmc_run(tpmc_mesh* m, const tpmc_params* params, void* cuda_stre
   if (h_stats) {
     TPMC_CUDA_TRY(cudaStreamSynchronize(st));
     return fill_stats(m, params, h_stats);
+  }
+  return TPMC_OK;
+}
+
+// K attitudes of a sweep in one call: run k is `params` with V = h_V[k].  The handle's scratch, streams and events are
+// shared by all of them; nothing is read back between attitudes unless statistics are asked for.
+extern "C" int tpmc_run_sweep(tpmc_mesh* m, const tpmc_params* params, int32_t n_attitudes, const double* h_V,
+                              void* cuda_stream, double* d_force, double* d_torque, double* d_facet_momentum,
+                              tpmc_stats* h_stats) {
+  if (!m || !params || !h_V || !d_force || !d_torque || n_attitudes < 0) return TPMC_EINVAL;
+  for (int32_t k = 0; k < n_attitudes; ++k) {
+    tpmc_params p = *params;
+    for (int a = 0; a < 3; ++a) p.V[a] = h_V[3 * (size_t)k + a];
+    const int rc = tpmc_run(m, &p, cuda_stream, d_force + 3 * (size_t)k, d_torque + 3 * (size_t)k,
+                            d_facet_momentum ? d_facet_momentum + 3 * (size_t)m->nt * (size_t)k : nullptr,
+                            h_stats ? h_stats + k : nullptr, nullptr);
+    if (rc != TPMC_OK) return rc;
   }
   return TPMC_OK;
 }

@@ -243,6 +243,42 @@ TPMC_HD SeedState seed_particle(const RunConst& rc, unsigned long long i, const 
   return out;
 }
 
+// ---- rectangular control volume (readings A24, A25) ------------------------------------------
+// The scheme the paper replaces, as a cross-check (TPMC_CV_BOX: exact) and as a negative control
+// (TPMC_CV_BOX_UNWEIGHTED: inward speed without the flux weight).  Face k = 2 axis + side (side 0 at -h with inward
+// normal +e_axis).  Uniforms: block 0 = (species, face, position, position), block 1 = (v_n, rho, angle, -).
+TPMC_HD SeedState seed_particle_box(const RunConst& rc, unsigned long long i) {
+  const uint4 b0 = particle_block(rc, i, 0u);
+  const uint4 b1 = particle_block(rc, i, 1u);
+  SeedState out;
+  const double u0 = u01(b0.x);
+  int s = 0;
+  while (s < rc.n_species - 1 && u0 >= rc.sp[s].cumx) ++s;
+  out.species = s;
+  const SpeciesConst& sc = rc.sp[s];
+  const double uf = u01(b0.y) * sc.bcum[5];
+  int k = 0;
+  while (k < 5 && uf >= sc.bcum[k]) ++k;
+  const int a = k >> 1, side = k & 1, e1 = (a + 1) % 3, e2 = (a + 2) % 3;
+  const double sn = sc.bsn[k];
+  double xn;
+  if (rc.control_volume == TPMC_CV_BOX_UNWEIGHTED) xn = sn + erfcinv((1.0 - u01(b1.x)) * erfc(-sn));
+  else xn = sample_normal_speed_fast(u01(b1.x), sn);
+  const double rho = sqrt(-log(u01(b1.y)));
+  double sa, ca;
+  sincospi(2.0 * u01(b1.z), &sa, &ca);
+  double x[3], v[3];
+  x[a] = rc.centre[a] + (side ? rc.box_h[a] : -rc.box_h[a]);
+  x[e1] = rc.centre[e1] + (2.0 * u01(b0.z) - 1.0) * rc.box_h[e1];
+  x[e2] = rc.centre[e2] + (2.0 * u01(b0.w) - 1.0) * rc.box_h[e2];
+  v[a] = sc.c * (side ? -xn : xn);
+  v[e1] = sc.c * (rc.V[e1] / sc.c + rho * ca);
+  v[e2] = sc.c * (rc.V[e2] / sc.c + rho * sa);
+#pragma unroll
+  for (int j = 0; j < 3; ++j) { out.x[j] = x[j]; out.v[j] = v[j]; }
+  return out;
+}
+
 // ---- a2, pre-cull pass: fp32 ESTIMATE of the seeded ray ------------------------------------------------
 // Most particles of the spherical control volume never come near the body (hit fraction of the bounding
 // sphere = (R_b/r)^2, P5), and a particle whose first segment misses the body contributes nothing (O10:

@@ -782,3 +782,69 @@ def test_warp_aggregated_accumulation_changes_nothing(T, O):
         fa, fb = a.facet_momentum.cpu().numpy(), b.facet_momentum.cpu().numpy()
         assert np.all(np.abs(fa - fb) <= 1e-11 * np.abs(fb).max(0))
         assert np.array_equal(np.linalg.norm(fa, axis=1) == 0, np.linalg.norm(fb, axis=1) == 0)
+
+
+# ------------------------------------------------------------------ NEXT-4: rectangular control volume, sweeps, moment maps
+@pytest.mark.parametrize("cv", [1, 2])
+def test_box_control_volume_parity(T, O, cv):
+    """The rectangular scheme the paper replaces (readings A24 / A25; oracle pins P18), flux-weighted and as the
+    unweighted negative control: seeding within 1e-12 of the oracle, then the whole path on a concave body."""
+    cfg = ti.config("C4")[4].with_(N=600_000, mesh_fn=lambda: ti.satellite(4, 0.1), control_volume=cv, seed=71,
+                                   m=(16.0 * ti.AMU, 4.0 * ti.AMU), x=(0.5, 0.5))
+    cfg._mesh_cache = []
+    gm, om = meshes(T, O, cfg)
+    x, v, s = (a.cpu().numpy() for a in gm.seed(cfg, first=1000, count=2000))
+    for j in range(0, 2000, 3):
+        xo, vo, so = om.seed(cfg, 1000 + j)
+        assert so == s[j] and np.abs(x[j] - xo).max() <= 1e-12 * np.abs(xo).max() + 1e-300
+        assert np.abs(v[j] - vo).max() <= SEED_RTOL * np.abs(vo).max() + 1e-9
+    g, o, frac = compare_run(T, O, cfg, 100_000, 200_000)
+    assert g.stats["ret_precull_a"] == 0 and g.stats["ret_precull_b"] == 0      # the fp32 pre-cull is the sphere scheme's
+
+
+def test_box_scheme_agrees_with_sphere_scheme_and_its_negative_control_does_not(T):
+    """Fig. 1 of the paper on the GPU: sphere drag at 2e7 particles per point.  The spherical scheme and
+    the flux-weighted box agree at both attitudes; the unweighted box is off by ~2 % at 45 deg to the box."""
+    m = ti.geodesic_sphere(16)
+    gm = T.Mesh(m.vertices, m.indices, m.flags)
+    N, nb = 24_000_000, 8
+    cd = {}
+    for ang in (0.0, 45.0):
+        a = np.deg2rad(ang)
+        V = (-7500.0 * np.cos(a), -7500.0 * np.sin(a), 0.0)
+        up = -np.array(V) / 7500.0
+        for cv in (0, 1, 2):
+            cfg = ti.RunConfig("fig1", None, V=V, N=N, seed=72, control_volume=cv)
+            Fs = np.array([gm.run(cfg, first=k * (N // nb), count=N // nb, facets=False, stats=False).force.cpu().numpy()
+                           for k in range(nb)])
+            d = (Fs @ (-up)) * nb / cfg.q_inf / np.pi
+            cd[(ang, cv)] = (d.mean(), d.std(ddof=1) / np.sqrt(nb))
+    for ang in (0.0, 45.0):
+        s, b, u = cd[(ang, 0)], cd[(ang, 1)], cd[(ang, 2)]
+        assert abs(s[0] - b[0]) < 4 * np.hypot(s[1], b[1]), (ang, s, b)
+    s, u = cd[(45.0, 0)], cd[(45.0, 2)]
+    assert abs(u[0] - s[0]) > 10 * np.hypot(s[1], u[1]) and abs(u[0] / s[0] - 1.0) > 0.01
+    assert abs(cd[(0.0, 0)][0] - cd[(45.0, 0)][0]) < 4 * np.hypot(cd[(0.0, 0)][1], cd[(45.0, 0)][1])   # sphere scheme: no attitude dependence
+    gm.close()
+
+
+def test_attitude_sweep_in_one_call_and_moment_map(T, O):
+    """tpmc_run_sweep: K attitudes in one call equal K separate runs, and the pitching-moment map about a reference
+    point (Figs. 8-9) agrees with the oracle's at the sampled pitch angles."""
+    cfgs = [c.with_(N=200_000, x_ref=(0.0, 0.0, -0.5), mesh_fn=lambda: ti.satellite(4, 0.1)) for c in ti.config("C4")[::5]]
+    for c in cfgs:
+        c._mesh_cache = cfgs[0]._mesh_cache
+    gm, om = meshes(T, O, cfgs[0])
+    V = np.array([c.V for c in cfgs])
+    F, Tq, fm, st = gm.sweep(cfgs[0], V, facets=True, stats=True)
+    F, Tq = F.cpu().numpy(), Tq.cpu().numpy()
+    assert F.shape == (len(cfgs), 3) and fm.shape == (len(cfgs), gm.nt, 3)
+    for k, c in enumerate(cfgs):
+        one = gm.run(c)
+        assert np.allclose(one.force.cpu().numpy(), F[k], rtol=1e-11) and st[k]["hits"] == one.stats["hits"]
+        assert np.allclose(fm[k].sum(0).cpu().numpy(), F[k], rtol=1e-9)
+        o = om.run(c, debug=False, facets=False)
+        q = c.q_inf
+        cm_gpu, cm_cpu = Tq[k, 1] / (q * 1.0 * 2.0), o.torque[1] / (q * 1.0 * 2.0)      # pitch axis y, A_ref 1 m^2, L_ref 2 m
+        assert abs(cm_gpu - cm_cpu) <= 1e-4 * max(abs(cm_cpu), 1e-3 * np.linalg.norm(o.force) / q)
+    assert np.ptp(Tq[:, 1]) > 0.0                                     # the map is not flat
