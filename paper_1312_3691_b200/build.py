@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtpmc.so")
 SOURCES = ["lbvh.cu", "run.cu", "peaks.cu"]
-HEADERS = ["common.cuh", "sampling.cuh", "sort.cuh", "trace.cuh", os.path.join("..", "..", "include", "tpmc.h")]
+HEADERS = ["common.cuh", "radix.cuh", "sampling.cuh", "sort.cuh", "trace.cuh", os.path.join("..", "..", "include", "tpmc.h")]
 
 
 def nvcc_command(verbose: bool = False):

@@ -2,14 +2,13 @@
 //
 // "Satellite surfaces are represented by a triangulation, allowing the use of well-known
 // ray-tracing methods"; the paper names no acceleration structure.  Here: 63-bit Morton
-// codes of facet centroids -> radix sort -> Karras (2012) binary radix tree -> bottom-up refit.
+// codes of facet centroids -> radix sort (radix.cuh) -> Karras (2012) binary radix tree -> bottom-up refit.
 // Everything runs on the device; there is no host build path.
-#include <cub/device/device_radix_sort.cuh>
-
 #include <algorithm>
 #include <cstdlib>
 
 #include "common.cuh"
+#include "radix.cuh"
 
 thread_local char g_tpmc_cuda_error[512] = "";
 
@@ -501,11 +500,12 @@ __device__ __forceinline__ unsigned int float_order(float f) {   // monotone map
   return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
 }
 // boxes [64][6] as ordered unsigned: lo.xyz (atomicMin), hi.xyz (atomicMax) of the facets with reach > r_in
-__global__ void k_outlier_boxes(const float4* __restrict__ tris, int64_t nt, float cx, float cy, float cz, float r_in,
-                                float3 lo, float3 inv_ext, unsigned int* __restrict__ boxes) {
+__global__ void k_outlier_boxes(const float4* __restrict__ tris, int64_t nt, float cx, float cy, float cz,
+                                const float* __restrict__ r_in_dev, float3 lo, float3 inv_ext, unsigned int* __restrict__ boxes) {
   const int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (s >= nt) return;
-  if (!(facet_reach(tris, s, cx, cy, cz) > r_in)) return;
+  const float r_in = *r_in_dev;
+  if (!(r_in >= 0.0f) || !(facet_reach(tris, s, cx, cy, cz) > r_in)) return;   // r_in < 0: candidate not in use
   const float4 a = tris[3 * s], b = tris[3 * s + 1], c = tris[3 * s + 2];
   const int ix = min(3, max(0, (int)(((a.x + b.x + c.x) * (1.0f / 3.0f) - lo.x) * inv_ext.x * 4.0f)));
   const int iy = min(3, max(0, (int)(((a.y + b.y + c.y) * (1.0f / 3.0f) - lo.y) * inv_ext.y * 4.0f)));
@@ -519,106 +519,129 @@ __global__ void k_outlier_boxes(const float4* __restrict__ tris, int64_t nt, flo
   atomicMax(bx + 5, float_order(fmaxf(a.z, fmaxf(b.z, c.z))));
 }
 
+// The choice itself, on the device: candidate radii from the histogram, then per candidate a greedy merge of the
+// outlier cells (<= 64 boxes: one thread) and the comparison of mean projected areas.
+constexpr int kCullCandidates = 7;
+struct CullChoice {
+  float r_in[kCullCandidates];   // candidate inner radii, < 0: not in use
+  double best;                   // smallest proxy so far (2 x mean projected area)
+  float rin;
+  int nbox;                      // -1: the bounding sphere stays
+  float box[8][6];
+};
+__device__ __forceinline__ float float_unorder(unsigned int u) {
+  return __uint_as_float((u & 0x80000000u) ? (u & 0x7FFFFFFFu) : ~u);
+}
+__global__ void k_cull_candidates(const unsigned int* __restrict__ hist, int64_t nt, float bin, double Rg, CullChoice* __restrict__ ch) {
+  if (blockIdx.x != 0 || threadIdx.x != 0) return;
+  const double quantiles[kCullCandidates] = {0.80, 0.90, 0.95, 0.97, 0.98, 0.99, 0.995};
+  int last_bin = -1;
+  for (int q = 0; q < kCullCandidates; ++q) {
+    unsigned long long acc = 0;
+    int b = 0;
+    for (; b < kReachBins; ++b) { acc += hist[b]; if ((double)acc >= quantiles[q] * (double)nt) break; }
+    const bool use = !(b >= kReachBins - 1 || b == last_bin);
+    if (use) last_bin = b;
+    ch->r_in[q] = use ? (float)(b + 1) * bin : -1.0f;
+  }
+  ch->best = 0.8 * 2.0 * 3.14159265358979323846 * Rg * Rg;   // must beat the bounding sphere (2 x projected area) by 20 %
+  ch->nbox = -1;
+  ch->rin = 0.0f;
+}
+__global__ void k_cull_init(unsigned int* __restrict__ boxes) {
+  const int i = threadIdx.x;
+  if (i < 64 * 6) boxes[i] = (i % 6) < 3 ? 0xFFFFFFFFu : 0u;
+}
+struct HBox { float lo[3], hi[3]; };
+__device__ __forceinline__ double half_area(const HBox& b, double g) {
+  const double e0 = (double)b.hi[0] - b.lo[0] + 2 * g, e1 = (double)b.hi[1] - b.lo[1] + 2 * g, e2 = (double)b.hi[2] - b.lo[2] + 2 * g;
+  return e0 * e1 + e1 * e2 + e0 * e2;   // = 2 x the mean projected area of a box (Cauchy: surface / 4)
+}
+__device__ __forceinline__ HBox merged(const HBox& a, const HBox& b) {
+  HBox m;
+  for (int k = 0; k < 3; ++k) { m.lo[k] = fminf(a.lo[k], b.lo[k]); m.hi[k] = fmaxf(a.hi[k], b.hi[k]); }
+  return m;
+}
+__global__ void k_cull_merge(const unsigned int* __restrict__ raw, int q, double g, CullChoice* __restrict__ ch) {
+  if (blockIdx.x != 0 || threadIdx.x != 0) return;
+  const float r_in = ch->r_in[q];
+  if (!(r_in >= 0.0f)) return;
+  HBox bx[64];
+  int nb = 0;
+  for (int i = 0; i < 64; ++i) {
+    if (raw[6 * i] == 0xFFFFFFFFu) continue;   // empty cell
+    for (int k = 0; k < 3; ++k) { bx[nb].lo[k] = float_unorder(raw[6 * i + k]); bx[nb].hi[k] = float_unorder(raw[6 * i + 3 + k]); }
+    ++nb;
+  }
+  while (nb > 8) {   // greedy merge: the pair whose union adds the least area
+    int bi = 0, bj = 1;
+    double bc = 1e300;
+    for (int i = 0; i < nb; ++i)
+      for (int j = i + 1; j < nb; ++j) {
+        const double c = half_area(merged(bx[i], bx[j]), g) - half_area(bx[i], g) - half_area(bx[j], g);
+        if (c < bc) { bc = c; bi = i; bj = j; }
+      }
+    bx[bi] = merged(bx[bi], bx[bj]);
+    bx[bj] = bx[--nb];
+  }
+  const double ri = (double)r_in + g;
+  double proxy = 2.0 * 3.14159265358979323846 * ri * ri;
+  for (int i = 0; i < nb; ++i) proxy += half_area(bx[i], g);
+  if (proxy < ch->best) {
+    ch->best = proxy;
+    ch->rin = r_in;
+    ch->nbox = nb;
+    for (int i = 0; i < nb; ++i)
+      for (int k = 0; k < 3; ++k) { ch->box[i][k] = bx[i].lo[k]; ch->box[i][3 + k] = bx[i].hi[k]; }
+  }
+}
+
 struct DevBuf {  // frees on scope exit
   void* p = nullptr;
   ~DevBuf() { if (p) cudaFree(p); }
   template <class T> T* as() { return (T*)p; }
 };
 
-}  // namespace
-
-
-namespace {
-float float_unorder(unsigned int u) {
-  const unsigned int b = (u & 0x80000000u) ? (u & 0x7FFFFFFFu) : ~u;
-  float f;
-  memcpy(&f, &b, 4);
-  return f;
-}
-struct HBox { float lo[3], hi[3]; };
-double half_area(const HBox& b, double g) {
-  const double e0 = (double)b.hi[0] - b.lo[0] + 2 * g, e1 = (double)b.hi[1] - b.lo[1] + 2 * g, e2 = (double)b.hi[2] - b.lo[2] + 2 * g;
-  return e0 * e1 + e1 * e2 + e0 * e2;   // = 2 x the mean projected area of a box (Cauchy: surface / 4)
-}
-HBox merged(const HBox& a, const HBox& b) {
-  HBox m;
-  for (int k = 0; k < 3; ++k) { m.lo[k] = std::min(a.lo[k], b.lo[k]); m.hi[k] = std::max(a.hi[k], b.hi[k]); }
-  return m;
-}
-
-// Choose the two-level cull volume (see k_reach_hist).  Leaves m->cull_nbox = -1 when it does not pay.
+// Choose the two-level cull volume (see k_reach_hist).  Leaves m->cull_nbox = -1 when it does not pay.  Everything is
+// computed on the device; the host reads the chosen volume once (the per-run constants are assembled there).
 int build_cull_volume(tpmc_mesh* m, cudaStream_t st) {
   m->cull_nbox = -1;
   m->cull_rin = (float)m->Rb;
   const int64_t nt = m->nt;
   if (nt < 64) return TPMC_OK;
-  DevBuf hist, boxes;
+  DevBuf hist, boxes, choice;
   TPMC_CUDA_TRY(cudaMalloc(&hist.p, sizeof(unsigned int) * kReachBins));
   TPMC_CUDA_TRY(cudaMalloc(&boxes.p, sizeof(unsigned int) * 64 * 6));
+  TPMC_CUDA_TRY(cudaMalloc(&choice.p, sizeof(CullChoice)));
   TPMC_CUDA_TRY(cudaMemsetAsync(hist.p, 0, sizeof(unsigned int) * kReachBins, st));
   const float cx = (float)m->centre[0], cy = (float)m->centre[1], cz = (float)m->centre[2];
   const float bin = (float)(m->Rb * 1.0001 / kReachBins);
   const unsigned gt = (unsigned)((nt + kBlock - 1) / kBlock);
+  const double g = (double)kPrecullMargin * m->Rb;
   k_reach_hist<<<gt, kBlock, 0, st>>>(m->tris, nt, cx, cy, cz, 1.0f / bin, hist.as<unsigned int>());
-  unsigned int h[kReachBins];
-  TPMC_CUDA_TRY(cudaMemcpyAsync(h, hist.p, sizeof(h), cudaMemcpyDeviceToHost, st));
-  TPMC_CUDA_TRY(cudaStreamSynchronize(st));
-  const double g = (double)kPrecullMargin * m->Rb, pi = 3.14159265358979323846;
-  const double Rg = m->Rb + g;
-  double best = 0.8 * 2.0 * pi * Rg * Rg;   // must beat the bounding sphere (2 x projected area) by 20 %
+  k_cull_candidates<<<1, 32, 0, st>>>(hist.as<unsigned int>(), nt, bin, m->Rb + g, choice.as<CullChoice>());
   float3 lo = make_float3(m->aabb_lo[0], m->aabb_lo[1], m->aabb_lo[2]);
   float3 ie;
   ie.x = m->aabb_hi[0] > m->aabb_lo[0] ? 1.0f / (m->aabb_hi[0] - m->aabb_lo[0]) : 0.0f;
   ie.y = m->aabb_hi[1] > m->aabb_lo[1] ? 1.0f / (m->aabb_hi[1] - m->aabb_lo[1]) : 0.0f;
   ie.z = m->aabb_hi[2] > m->aabb_lo[2] ? 1.0f / (m->aabb_hi[2] - m->aabb_lo[2]) : 0.0f;
-  const double quantiles[] = {0.80, 0.90, 0.95, 0.97, 0.98, 0.99, 0.995};
-  int last_bin = -1;
-  for (double q : quantiles) {
-    unsigned long long acc = 0;
-    int b = 0;
-    for (; b < kReachBins; ++b) { acc += h[b]; if ((double)acc >= q * (double)nt) break; }
-    if (b >= kReachBins - 1 || b == last_bin) continue;
-    last_bin = b;
-    const float r_in = (float)(b + 1) * bin;
-    unsigned int init[64 * 6];
-    for (int i = 0; i < 64; ++i)
-      for (int k = 0; k < 6; ++k) init[6 * i + k] = k < 3 ? 0xFFFFFFFFu : 0u;
-    TPMC_CUDA_TRY(cudaMemcpyAsync(boxes.p, init, sizeof(init), cudaMemcpyHostToDevice, st));
-    k_outlier_boxes<<<gt, kBlock, 0, st>>>(m->tris, nt, cx, cy, cz, r_in, lo, ie, boxes.as<unsigned int>());
-    unsigned int raw[64 * 6];
-    TPMC_CUDA_TRY(cudaMemcpyAsync(raw, boxes.p, sizeof(raw), cudaMemcpyDeviceToHost, st));
-    TPMC_CUDA_TRY(cudaStreamSynchronize(st));
-    HBox bx[64];
-    int nb = 0;
-    for (int i = 0; i < 64; ++i) {
-      if (raw[6 * i] == 0xFFFFFFFFu) continue;   // empty cell
-      for (int k = 0; k < 3; ++k) { bx[nb].lo[k] = float_unorder(raw[6 * i + k]); bx[nb].hi[k] = float_unorder(raw[6 * i + 3 + k]); }
-      ++nb;
-    }
-    while (nb > 8) {   // greedy merge: the pair whose union adds the least area
-      int bi = 0, bj = 1;
-      double bc = 1e300;
-      for (int i = 0; i < nb; ++i)
-        for (int j = i + 1; j < nb; ++j) {
-          const double c = half_area(merged(bx[i], bx[j]), g) - half_area(bx[i], g) - half_area(bx[j], g);
-          if (c < bc) { bc = c; bi = i; bj = j; }
-        }
-      bx[bi] = merged(bx[bi], bx[bj]);
-      bx[bj] = bx[--nb];
-    }
-    const double ri = (double)r_in + g;
-    double proxy = 2.0 * pi * ri * ri;
-    for (int i = 0; i < nb; ++i) proxy += half_area(bx[i], g);
-    if (proxy < best) {
-      best = proxy;
-      m->cull_rin = r_in;
-      m->cull_nbox = nb;
-      for (int i = 0; i < nb; ++i)
-        for (int k = 0; k < 3; ++k) { m->cull_box[i][k] = bx[i].lo[k]; m->cull_box[i][3 + k] = bx[i].hi[k]; }
-    }
+  for (int q = 0; q < kCullCandidates; ++q) {
+    k_cull_init<<<1, 384, 0, st>>>(boxes.as<unsigned int>());
+    k_outlier_boxes<<<gt, kBlock, 0, st>>>(m->tris, nt, cx, cy, cz, choice.as<CullChoice>()->r_in + q, lo, ie, boxes.as<unsigned int>());
+    k_cull_merge<<<1, 32, 0, st>>>(boxes.as<unsigned int>(), q, g, choice.as<CullChoice>());
+  }
+  CullChoice h;
+  TPMC_CUDA_TRY(cudaMemcpyAsync(&h, choice.p, sizeof(h), cudaMemcpyDeviceToHost, st));
+  TPMC_CUDA_TRY(cudaStreamSynchronize(st));
+  if (h.nbox >= 0) {
+    m->cull_rin = h.rin;
+    m->cull_nbox = h.nbox;
+    for (int i = 0; i < h.nbox; ++i)
+      for (int k = 0; k < 6; ++k) m->cull_box[i][k] = h.box[i][k];
   }
   return TPMC_OK;
 }
+
 }  // namespace
 
 extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t* indices, int64_t nt,
@@ -708,13 +731,13 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
   ie.y = h.aabb[4] > h.aabb[1] ? 1.0f / (h.aabb[4] - h.aabb[1]) : 0.0f;
   ie.z = h.aabb[5] > h.aabb[2] ? 1.0f / (h.aabb[5] - h.aabb[2]) : 0.0f;
   k_morton<<<gt, kBlock, 0, st>>>(d_v, d_i, nt, lo, ie, keys.as<uint64_t>(), ids.as<int32_t>());
-  size_t tmp_bytes = 0;
-  MESH_TRY(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys.as<uint64_t>(), keys2.as<uint64_t>(),
-                                           ids.as<int32_t>(), ids2.as<int32_t>(), (int)nt, 0, 63, st));
-  MESH_TRY(cudaMalloc(&tmp.p, tmp_bytes ? tmp_bytes : 16));
-  MESH_TRY(cub::DeviceRadixSort::SortPairs(tmp.p, tmp_bytes, keys.as<uint64_t>(), keys2.as<uint64_t>(),
-                                           ids.as<int32_t>(), ids2.as<int32_t>(), (int)nt, 0, 63, st));
-  k_gather<<<gt, kBlock, 0, st>>>(d_v, d_i, d_f, ids2.as<int32_t>(), nt, m->tris, box.as<float>(), n_int);
+  MESH_TRY(cudaMalloc(&tmp.p, radix::scratch_bytes(nt)));
+  // 63-bit codes: 16 passes of 4 bits, stable, so equal codes keep the facet order (the hierarchy's tie-break)
+  const int where = radix::sort_pairs(keys.as<uint64_t>(), ids.as<int32_t>(), keys2.as<uint64_t>(), ids2.as<int32_t>(), nt, 64,
+                                      tmp.as<unsigned int>(), st);
+  const uint64_t* keys_sorted = where ? keys2.as<uint64_t>() : keys.as<uint64_t>();
+  const int32_t* ids_sorted = where ? ids2.as<int32_t>() : ids.as<int32_t>();
+  k_gather<<<gt, kBlock, 0, st>>>(d_v, d_i, d_f, ids_sorted, nt, m->tris, box.as<float>(), n_int);
   if (nt == 1) {
     k_single<<<1, 1, 0, st>>>(box.as<float>(), m->nodes);
   } else {
@@ -726,8 +749,7 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
     MESH_TRY(cudaMalloc((void**)&m->cnodes_r, sizeof(uint4) * 2 * n_int));
     MESH_TRY(cudaMalloc((void**)&m->align_R, sizeof(double) * 16));
     MESH_TRY(cudaMemsetAsync(m->arrive, 0, sizeof(int) * n_int, st));
-    k_hierarchy<<<(unsigned)((n_int + kBlock - 1) / kBlock), kBlock, 0, st>>>(keys2.as<uint64_t>(), (int)nt,
-                                                                                m->kids, m->parent);
+    k_hierarchy<<<(unsigned)((n_int + kBlock - 1) / kBlock), kBlock, 0, st>>>(keys_sorted, (int)nt, m->kids, m->parent);
     k_refit<<<gt, kBlock, 0, st>>>((int)nt, m->kids, m->parent, box.as<float>(), m->arrive, m->nodes);
   }
   {
