@@ -318,8 +318,12 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
       if (fin) {
         const unsigned h = base + __popc(fm & lanemask_lt());
         __stcs(hit_ray + h, r);
-        __stcs(hit_cand + h, (w.nc > TPMC_MAX_CAND) ? make_int4(-1, -1, -1, TPMC_CAND_OVERFLOW)
-                                                    : make_int4(w.cs[0], w.cs[1], w.cs[2], w.cs[3]));
+        int4 cd = make_int4(-1, -1, -1, -1);
+        cd.x = w.cs[0];
+        if (TPMC_MAX_CAND > 1) cd.y = w.cs[TPMC_MAX_CAND > 1 ? 1 : 0];
+        if (TPMC_MAX_CAND > 2) cd.z = w.cs[TPMC_MAX_CAND > 2 ? 2 : 0];
+        if (TPMC_MAX_CAND > 3) cd.w = w.cs[TPMC_MAX_CAND > 3 ? 3 : 0];
+        __stcs(hit_cand + h, (w.nc > TPMC_MAX_CAND) ? make_int4(-1, -1, -1, TPMC_CAND_OVERFLOW) : cd);
         fin = false;
       }
     }

@@ -25,7 +25,9 @@
 #endif
 #define TPMC_STACK_LOCAL 80     // overflow entries (a Karras tree over 64-bit keys + index is <= 97 deep)
 #define TPMC_SENTINEL ((int)0x7FFFFFFF)
+#ifndef TPMC_MAX_CAND
 #define TPMC_MAX_CAND 4
+#endif
 #define TPMC_CAND_OVERFLOW ((int)0x7FFFFFFE)   // in cand.w: more candidates than slots -> full fp64 traversal
 
 // 256-bit read-only load (sm_100: LDG.E.256): one L1 sector per lane per instruction instead of half a
@@ -518,7 +520,7 @@ __device__ __forceinline__ Hit resolve_candidates(const float4* __restrict__ tri
   best.tau = INFINITY; best.facet = -1; best.slot = -1;
   const int cs[4] = {cand.x, cand.y, cand.z, cand.w};
 #pragma unroll
-  for (int k = 0; k < TPMC_MAX_CAND; ++k) {
+  for (int k = 0; k < 4; ++k) {
     const int slot = cs[k];
     if (slot < 0) continue;
     const float4 q0 = __ldg(tris + 3 * (size_t)slot + 0), q1 = __ldg(tris + 3 * (size_t)slot + 1),
