@@ -77,8 +77,8 @@ __global__ void __launch_bounds__(kPrecullBlock) k_seed_precull(const SeedConstF
                                                                  unsigned int* __restrict__ surv,
                                                                  unsigned int* __restrict__ n_surv,
                                                                  unsigned long long* __restrict__ stats) {
-  __shared__ float qf[9][kPrecullQ];
-  __shared__ unsigned int qj[kPrecullQ], qw[kPrecullQ];
+  __shared__ float qf[7][kPrecullQ];
+  __shared__ unsigned int qj[kPrecullQ], qw[kPrecullQ], qw2[kPrecullQ];
   __shared__ unsigned char qok[kPrecullQ];
   __shared__ unsigned int q_n, s_cnt[2][kPrecullBlock / 32], s_base[2];
   const unsigned int per = (((wave_n + gridDim.x - 1) / gridDim.x) + kPrecullBlock - 1) / kPrecullBlock * kPrecullBlock;
@@ -103,9 +103,9 @@ __global__ void __launch_bounds__(kPrecullBlock) k_seed_precull(const SeedConstF
       pos = __shfl_sync(0xFFFFFFFFu, pos, 0);
       if (pass) {
         const unsigned int sl = pos + __popc(m & lanemask_lt());
-        qf[0][sl] = a.y; qf[1][sl] = a.t; qf[2][sl] = a.cphi; qf[3][sl] = a.st; qf[4][sl] = a.ct;
-        qf[5][sl] = a.xt1; qf[6][sl] = a.xt2; qf[7][sl] = a.s; qf[8][sl] = a.chis;
-        qj[sl] = j; qw[sl] = a.w3; qok[sl] = a.ok_t ? 1 : 0;
+        qf[0][sl] = a.y; qf[1][sl] = a.t; qf[2][sl] = a.cphi;
+        qf[3][sl] = a.xt1; qf[4][sl] = a.xt2; qf[5][sl] = a.s; qf[6][sl] = a.chis;
+        qj[sl] = j; qw[sl] = a.w3; qw2[sl] = a.w2; qok[sl] = a.ok_t ? 1 : 0;
       }
       base += kPrecullBlock;
       __syncthreads();
@@ -117,9 +117,9 @@ __global__ void __launch_bounds__(kPrecullBlock) k_seed_precull(const SeedConstF
       const bool active = threadIdx.x < take;
       const unsigned int sl = n - take + (active ? threadIdx.x : 0u);
       PrecullA a;
-      a.y = qf[0][sl]; a.t = qf[1][sl]; a.cphi = qf[2][sl]; a.st = qf[3][sl]; a.ct = qf[4][sl];
-      a.xt1 = qf[5][sl]; a.xt2 = qf[6][sl]; a.s = qf[7][sl]; a.chis = qf[8][sl];
-      a.w3 = qw[sl]; a.ok_t = qok[sl] != 0;
+      a.y = qf[0][sl]; a.t = qf[1][sl]; a.cphi = qf[2][sl];
+      a.xt1 = qf[3][sl]; a.xt2 = qf[4][sl]; a.s = qf[5][sl]; a.chis = qf[6][sl];
+      a.w3 = qw[sl]; a.w2 = qw2[sl]; a.ok_t = qok[sl] != 0;
       const unsigned int j = qj[sl];
       float o[3], v[3], root[2];
       const bool ok = precull_stage_b(sf, a, o, v, root);
