@@ -127,6 +127,7 @@ typedef struct {
   uint64_t final_stragglers; /* rays still queued after the drain iterations (followed by the straggler kernel, not traced) */
   uint64_t finish_segments;  /* closest-hit searches of the straggler kernel */
   double ms_sort;          /* summed device time of the ray-sort launches */
+  uint64_t precull_uncertified; /* particles whose fp32 pre-cull estimate was not certified (they take the fp64 sampler whatever their ray does) */
 } tpmc_stats;
 
 /* Optional per-particle outputs for parity checks; each pointer is device [count] or NULL. */

@@ -60,7 +60,7 @@ class tpmc_stats(C.Structure):
                 ("ret_trace", C.c_uint64), ("ret_resolve", C.c_uint64), ("ret_horizon", C.c_uint64),
                 ("ret_finish", C.c_uint64), ("queued_primaries", C.c_uint64), ("queued_reflected", C.c_uint64),
                 ("overflow_rays", C.c_uint64), ("final_stragglers", C.c_uint64), ("finish_segments", C.c_uint64),
-                ("ms_sort", C.c_double)]
+                ("ms_sort", C.c_double), ("precull_uncertified", C.c_uint64)]
 
 
 class tpmc_peaks(C.Structure):

@@ -152,7 +152,7 @@ struct RunConst {
 // Device counters of a run (tpmc_stats: every one is counted where the event happens).
 enum { ST_HITS = 0, ST_TRUNC, ST_TRIS, ST_NODES, ST_TRACED, ST_RET_PA, ST_RET_PB, ST_RET_SEED, ST_RET_TRACE,
        ST_RET_RESOLVE, ST_RET_HORIZON, ST_RET_FINISH, ST_Q_PRIM, ST_Q_REFL, ST_OVF_RETRACE, ST_OVF_PENDING, ST_DIVERTED,
-       ST_STRAGGLERS, ST_FIN_SEGS, ST_COUNT = 24 };
+       ST_STRAGGLERS, ST_FIN_SEGS, ST_UNCERT, ST_COUNT = 24 };
 
 int tpmc_mesh_align(tpmc_mesh* m, const double R[9], cudaStream_t st, const QuantGrid** grid_out, const uint4** cnodes_out);
 

@@ -166,6 +166,7 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
                                                      unsigned long long* __restrict__ stats) {
   const unsigned int n1 = surv ? n_surv[0] : 0u;                 // certified survivors: fp32 roots available
   const unsigned int n = surv ? n1 + n_surv[1] : wave_n;
+  if (surv && blockIdx.x == 0 && threadIdx.x == 0 && n_surv[1]) atomicAdd(&stats[ST_UNCERT], (unsigned long long)n_surv[1]);
   const unsigned int stride = gridDim.x * blockDim.x;
   const unsigned int nround = ((n + stride - 1) / stride) * stride;   // keep warps converged for the ballots
   for (unsigned int kk = blockIdx.x * blockDim.x + threadIdx.x; kk < nround; kk += stride) {
@@ -994,6 +995,7 @@ int fill_stats(tpmc_mesh* m, const tpmc_params* params, tpmc_stats* h_stats) {
   h_stats->overflow_rays = hs[ST_OVF_RETRACE] + hs[ST_OVF_PENDING] + hs[ST_DIVERTED];
   h_stats->final_stragglers = hs[ST_STRAGGLERS];
   h_stats->finish_segments = hs[ST_FIN_SEGS];
+  h_stats->precull_uncertified = hs[ST_UNCERT];
   h_stats->traced_rays = hs[ST_TRACED];
   // sums of counted events (the identities of tpmc.h hold only if no particle was lost or duplicated on the way)
   h_stats->culled = hs[ST_RET_PA] + hs[ST_RET_PB] + hs[ST_RET_SEED];
