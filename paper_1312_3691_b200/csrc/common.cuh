@@ -64,8 +64,12 @@ struct tpmc_mesh {
   int* parent;                     // [nt-1 | nt] parent of every internal node and leaf
   int* arrive;                     // [nt-1] refit counters
   float* rbox;                     // [(nt-1) + nt][6] boxes in the aligned frame
-  float4* nodes_r;                 // [nt-1][4] refit output in the aligned frame
-  uint4* cnodes_r;                 // [nt-1][2] its compact form
+  // wide (4-ary) hierarchy of the wavefront traversal: the binary tree collapsed breadth-first (k_wide_*), 64 B per node
+  int64_t n_wide;                  // wide nodes
+  int4* wkids_bin;                 // [n_wide] children as refs of the BINARY tree (>= 0 internal node, < 0 leaf ~slot, TPMC_WIDE_EMPTY)
+  int4* wkids;                     // [n_wide] the same children as refs of the WIDE tree (>= 0 wide node, < 0 leaf ~slot)
+  uint4* wnodes;                   // [n_wide][4] body-frame boxes on the 16-bit grid + refs (k_compact_wide)
+  uint4* wnodes_r;                 // [n_wide][4] the flow-aligned copy, refitted per run
   double* align_R;                 // [9] rotation of the current alignment, [6] its grid origin and scale (device)
   QuantGrid* grid_dev;             // [2] device copies of the grids the traversal reads: body frame, aligned
   uint4* cnodes;                   // compact copy of `nodes` for the wavefront traversal: 2 uint4 = 32 B per node
@@ -154,7 +158,8 @@ enum { ST_HITS = 0, ST_TRUNC, ST_TRIS, ST_NODES, ST_TRACED, ST_RET_PA, ST_RET_PB
        ST_RET_RESOLVE, ST_RET_HORIZON, ST_RET_FINISH, ST_Q_PRIM, ST_Q_REFL, ST_OVF_RETRACE, ST_OVF_PENDING, ST_DIVERTED,
        ST_STRAGGLERS, ST_FIN_SEGS, ST_UNCERT, ST_COUNT = 24 };
 
-int tpmc_mesh_align(tpmc_mesh* m, const double R[9], cudaStream_t st, const QuantGrid** grid_out, const uint4** cnodes_out);
+int tpmc_mesh_align(tpmc_mesh* m, const double R[9], cudaStream_t st, const QuantGrid** grid_out, const uint4** wnodes_out);
+#define TPMC_WIDE_EMPTY ((int)0x7FFFFFFD)   // wkids_bin: no child in this slot
 
 #define TPMC_HD __host__ __device__ __forceinline__
 

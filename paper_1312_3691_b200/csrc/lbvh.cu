@@ -166,10 +166,12 @@ __global__ void k_refit(int n, const int2* __restrict__ children, const int* __r
     for (int a = 0; a < 3; ++a) { l0[a] = b0[a]; h0[a] = b0[3 + a]; l1[a] = b1[a]; h1[a] = b1[3 + a]; }
     float* b = box + 6 * (size_t)cur;
     for (int a = 0; a < 3; ++a) { b[a] = fminf(l0[a], l1[a]); b[3 + a] = fmaxf(h0[a], h1[a]); }
-    nodes[4 * (size_t)cur + 0] = make_float4(l0[0], l0[1], l0[2], h0[0]);
-    nodes[4 * (size_t)cur + 1] = make_float4(h0[1], h0[2], l1[0], l1[1]);
-    nodes[4 * (size_t)cur + 2] = make_float4(l1[2], h1[0], h1[1], h1[2]);
-    nodes[4 * (size_t)cur + 3] = make_float4(__int_as_float(ch.x), __int_as_float(ch.y), 0.0f, 0.0f);
+    if (nodes) {   // (the per-run refit in the stream frame only needs the boxes)
+      nodes[4 * (size_t)cur + 0] = make_float4(l0[0], l0[1], l0[2], h0[0]);
+      nodes[4 * (size_t)cur + 1] = make_float4(h0[1], h0[2], l1[0], l1[1]);
+      nodes[4 * (size_t)cur + 2] = make_float4(l1[2], h1[0], h1[1], h1[2]);
+      nodes[4 * (size_t)cur + 3] = make_float4(__int_as_float(ch.x), __int_as_float(ch.y), 0.0f, 0.0f);
+    }
     cur = parent[cur];
   }
 }
@@ -237,6 +239,164 @@ __global__ void k_build_cull(const float4* __restrict__ nodes, const uint4* __re
     cull_c[2 * head + 1] = make_uint4(cb.x, cb.y, (unsigned int)ref[0], (unsigned int)ref[1]);
   }
   *out_count = tail;
+}
+
+// ---- wide (4-ary) hierarchy for the wavefront traversal --------------------------------------------------------
+// The binary radix tree is collapsed breadth-first: a wide node starts from the two children of a binary node and
+// replaces, up to twice, its internal child with the largest box surface by that child's two children (greedy by
+// area; TPMC_WIDE_GREEDY=0 opens the two original children instead: every second level of the binary tree).  A ray
+// then fetches one 64-byte node where it fetched two or three 32-byte nodes one after the other: the chain of
+// dependent loads per ray, which bounds the traversal kernel, gets about half as long.  Topology only (which binary
+// nodes/leaves are the children of each wide node, and the breadth-first numbering); the boxes are filled in per
+// frame by k_compact_wide from the per-node boxes of the refit.  Numbering is deterministic: per level an expand
+// pass, a one-block exclusive scan of the internal-child counts, and an assign pass.
+#ifndef TPMC_WIDE_GREEDY
+#define TPMC_WIDE_GREEDY 1
+#endif
+constexpr int kWideLevels = 100;   // >= depth of a Karras tree over 63-bit keys with a 30-bit index tie-break
+__device__ __forceinline__ float box_half_area(const float* __restrict__ b) {
+  const float ex = b[3] - b[0], ey = b[4] - b[1], ez = b[5] - b[2];
+  return ex * ey + ey * ez + ez * ex;
+}
+// lvl[0], lvl[1]: wide nodes [begin, end) of the current level; lvl[2]: internal children found on it
+__global__ void k_wide_expand(const int2* __restrict__ kids, const float* __restrict__ box, const int* __restrict__ lvl,
+                              const int* __restrict__ wroot, int4* __restrict__ wkids_bin, unsigned int* __restrict__ cnt) {
+  const int begin = lvl[0], end = lvl[1];
+  for (int w = begin + blockIdx.x * blockDim.x + threadIdx.x; w < end; w += gridDim.x * blockDim.x) {
+    const int2 k0 = kids[wroot[w]];
+    int c[4] = {k0.x, k0.y, TPMC_WIDE_EMPTY, TPMC_WIDE_EMPTY};
+    int nc = 2;
+#if TPMC_WIDE_GREEDY
+    for (int round = 0; round < 2; ++round) {
+      int best = -1;
+      float ba = -1.0f;
+      for (int j = 0; j < nc; ++j)
+        if (c[j] >= 0) {
+          const float a = box_half_area(box + 6 * (size_t)c[j]);
+          if (a > ba) { ba = a; best = j; }
+        }
+      if (best < 0) break;
+      const int2 kk = kids[c[best]];
+      for (int j = nc; j > best + 1; --j) c[j] = c[j - 1];   // keep the children in Morton order
+      c[best] = kk.x;
+      c[best + 1] = kk.y;
+      ++nc;
+    }
+#else
+    if (k0.y >= 0) { const int2 kk = kids[k0.y]; c[1] = kk.x; c[2] = kk.y; nc = 3; }
+    if (k0.x >= 0) { const int2 kk = kids[k0.x]; for (int j = nc; j > 1; --j) c[j] = c[j - 1]; c[0] = kk.x; c[1] = kk.y; ++nc; }
+#endif
+    unsigned int ni = 0u;
+    for (int j = 0; j < 4; ++j) ni += (c[j] >= 0 && c[j] != TPMC_WIDE_EMPTY) ? 1u : 0u;
+    wkids_bin[w] = make_int4(c[0], c[1], c[2], c[3]);
+    cnt[w] = ni;
+  }
+}
+// exclusive scan of cnt[begin, end) in place by one block; lvl[2] = total
+__global__ void __launch_bounds__(1024) k_wide_scan(unsigned int* __restrict__ cnt, int* __restrict__ lvl) {
+  __shared__ unsigned int wsum[32];
+  __shared__ unsigned int carry;
+  const int begin = lvl[0], end = lvl[1];
+  if (threadIdx.x == 0) carry = 0u;
+  __syncthreads();
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  for (int c0 = begin; c0 < end; c0 += 1024) {
+    const int i = c0 + threadIdx.x;
+    const unsigned int v = i < end ? cnt[i] : 0u;
+    unsigned int inc = v;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+      const unsigned int t = __shfl_up_sync(0xFFFFFFFFu, inc, off);
+      if (lane >= off) inc += t;
+    }
+    if (lane == 31) wsum[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+      unsigned int x = wsum[lane];
+#pragma unroll
+      for (int off = 1; off < 32; off <<= 1) {
+        const unsigned int t = __shfl_up_sync(0xFFFFFFFFu, x, off);
+        if (lane >= off) x += t;
+      }
+      wsum[lane] = x;
+    }
+    __syncthreads();
+    const unsigned int before = carry + (wid ? wsum[wid - 1] : 0u);
+    if (i < end) cnt[i] = before + inc - v;
+    __syncthreads();
+    if (threadIdx.x == 1023) carry = before + inc;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) lvl[2] = (int)carry;
+}
+__global__ void k_wide_assign(const int* __restrict__ lvl, const int4* __restrict__ wkids_bin, const unsigned int* __restrict__ off,
+                              int* __restrict__ wroot, int4* __restrict__ wkids) {
+  const int begin = lvl[0], end = lvl[1];
+  for (int w = begin + blockIdx.x * blockDim.x + threadIdx.x; w < end; w += gridDim.x * blockDim.x) {
+    const int4 kb = wkids_bin[w];
+    const int c[4] = {kb.x, kb.y, kb.z, kb.w};
+    int r[4];
+    int next = end + (int)off[w];
+    for (int j = 0; j < 4; ++j) {
+      r[j] = c[j];                                    // leaf (< 0) or empty: unchanged
+      if (c[j] >= 0 && c[j] != TPMC_WIDE_EMPTY) { wroot[next] = c[j]; r[j] = next++; }
+    }
+    wkids[w] = make_int4(r[0], r[1], r[2], r[3]);
+  }
+}
+__global__ void k_wide_next(int* __restrict__ lvl) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) { lvl[0] = lvl[1]; lvl[1] += lvl[2]; lvl[2] = 0; }
+}
+__global__ void k_wide_init(int* __restrict__ lvl, int* __restrict__ wroot, int4* __restrict__ wkids_bin, int4* __restrict__ wkids, int single) {
+  if (blockIdx.x != 0 || threadIdx.x != 0) return;
+  if (single) {   // one triangle: one wide node holding the leaf
+    wkids_bin[0] = make_int4(~0, TPMC_WIDE_EMPTY, TPMC_WIDE_EMPTY, TPMC_WIDE_EMPTY);
+    wkids[0] = wkids_bin[0];
+    lvl[0] = 1; lvl[1] = 1; lvl[2] = 0;
+  } else {
+    wroot[0] = 0;
+    lvl[0] = 0; lvl[1] = 1; lvl[2] = 0;
+  }
+}
+
+// Boxes of the wide nodes in one frame: 64 B per node = two 256-bit loads.
+//   words 3k .. 3k+2: box of child k (x, y, z), one word per axis: lo | hi << 16 as unsigned 16-bit grid coordinates
+//   (one byte permute yields the near or the far plane of an axis, see trace.cuh); words 12-15: the four child refs
+//   (>= 0: wide node, < 0: leaf holding sorted triangle ~ref).  An empty slot has the box lo = 65535, hi = 0 on every
+//   axis, which no ray enters (near plane 65535 steps beyond the far plane), and repeats the ref of child 0, so that
+//   even a margin of absurd size (a ray far outside along a flat axis) would only repeat work, never read a bad ref.
+// Grid: x = origin + q * scale per axis.  lo is rounded down and hi up: the decoded box contains the fp32 box.
+// (The quotient is evaluated in fp64: a box corner within 1e-11 steps of a grid plane may land on the wrong side of it,
+// which the slack of the traversal's margin G covers.  The clamps never act: quant_step keeps every plane inside
+// steps 0 .. 65535.)  box: [(n_int + nt)][6], the per-node boxes of the refit in this frame.
+__global__ void k_compact_wide(const float* __restrict__ box, int64_t n_int, const int4* __restrict__ wkids_bin,
+                               const int4* __restrict__ wkids, int64_t n_wide, double ox, double oy, double oz, double sx,
+                               double sy, double sz, uint4* __restrict__ wnodes, const double* __restrict__ dev_grid = nullptr) {
+  const int64_t w = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (w >= n_wide) return;
+  if (dev_grid) { ox = dev_grid[0]; oy = dev_grid[1]; oz = dev_grid[2]; sx = dev_grid[3]; sy = dev_grid[4]; sz = dev_grid[5]; }
+  const double o[3] = {ox, oy, oz}, sc[3] = {sx, sy, sz};
+  const int4 kb = wkids_bin[w], kw = wkids[w];
+  const int cb[4] = {kb.x, kb.y, kb.z, kb.w};
+  unsigned int ref[4] = {(unsigned int)kw.x, (unsigned int)kw.y, (unsigned int)kw.z, (unsigned int)kw.w};
+  unsigned int q[12];
+  for (int k = 0; k < 4; ++k) {
+    if (cb[k] == TPMC_WIDE_EMPTY) {
+      q[3 * k] = q[3 * k + 1] = q[3 * k + 2] = 0x0000FFFFu;
+      ref[k] = ref[0];
+      continue;
+    }
+    const float* b = box + 6 * (size_t)(cb[k] >= 0 ? (int64_t)cb[k] : n_int + (int64_t)~cb[k]);
+    for (int a = 0; a < 3; ++a) {
+      const double l = floor(((double)b[a] - o[a]) / sc[a]), h = ceil(((double)b[3 + a] - o[a]) / sc[a]);
+      const unsigned int ql = (unsigned int)fmin(fmax(l, 0.0), 65535.0), qh = (unsigned int)fmin(fmax(h, 0.0), 65535.0);
+      q[3 * k + a] = ql | (qh << 16);
+    }
+  }
+  wnodes[4 * w + 0] = make_uint4(q[0], q[1], q[2], q[3]);
+  wnodes[4 * w + 1] = make_uint4(q[4], q[5], q[6], q[7]);
+  wnodes[4 * w + 2] = make_uint4(q[8], q[9], q[10], q[11]);
+  wnodes[4 * w + 3] = make_uint4(ref[0], ref[1], ref[2], ref[3]);
 }
 
 // ---- flow-aligned compact hierarchy (per run) ------------------------------------------------------------------
@@ -745,8 +905,6 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
     MESH_TRY(cudaMalloc((void**)&m->parent, sizeof(int) * (size_t)(n_int + nt)));
     MESH_TRY(cudaMalloc((void**)&m->arrive, sizeof(int) * n_int));
     MESH_TRY(cudaMalloc((void**)&m->rbox, sizeof(float) * 6 * (size_t)(n_int + nt)));
-    MESH_TRY(cudaMalloc((void**)&m->nodes_r, sizeof(float4) * 4 * n_int));
-    MESH_TRY(cudaMalloc((void**)&m->cnodes_r, sizeof(uint4) * 2 * n_int));
     MESH_TRY(cudaMalloc((void**)&m->align_R, sizeof(double) * 16));
     MESH_TRY(cudaMemsetAsync(m->arrive, 0, sizeof(int) * n_int, st));
     k_hierarchy<<<(unsigned)((n_int + kBlock - 1) / kBlock), kBlock, 0, st>>>(keys_sorted, (int)nt, m->kids, m->parent);
@@ -771,6 +929,36 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
     MESH_TRY(cudaMalloc((void**)&m->grid_dev, 2 * sizeof(QuantGrid)));
     MESH_TRY(cudaMemcpyAsync(m->grid_dev, &hg, sizeof(hg), cudaMemcpyHostToDevice, st));
     MESH_TRY(cudaMemcpyAsync(m->grid_dev + 1, &hg, sizeof(hg), cudaMemcpyHostToDevice, st));
+  }
+  {
+    // wide hierarchy of the traversal: topology breadth-first (k_wide_*), then the body-frame boxes
+    DevBuf lvl, wroot, wcnt;
+    const int64_t cap_w = std::max<int64_t>(n_int, 1);
+    MESH_TRY(cudaMalloc((void**)&m->wkids_bin, sizeof(int4) * cap_w));
+    MESH_TRY(cudaMalloc((void**)&m->wkids, sizeof(int4) * cap_w));
+    MESH_TRY(cudaMalloc(&wroot.p, sizeof(int) * cap_w));
+    MESH_TRY(cudaMalloc(&wcnt.p, sizeof(unsigned int) * cap_w));
+    MESH_TRY(cudaMalloc(&lvl.p, sizeof(int) * 4));
+    k_wide_init<<<1, 32, 0, st>>>(lvl.as<int>(), wroot.as<int>(), m->wkids_bin, m->wkids, nt == 1 ? 1 : 0);
+    if (nt > 1) {
+      const unsigned gw = (unsigned)std::min<int64_t>((cap_w + kBlock - 1) / kBlock, 592);
+      for (int L = 0; L < kWideLevels; ++L) {
+        k_wide_expand<<<gw, kBlock, 0, st>>>(m->kids, box.as<float>(), lvl.as<int>(), wroot.as<int>(), m->wkids_bin, wcnt.as<unsigned int>());
+        k_wide_scan<<<1, 1024, 0, st>>>(wcnt.as<unsigned int>(), lvl.as<int>());
+        k_wide_assign<<<gw, kBlock, 0, st>>>(lvl.as<int>(), m->wkids_bin, wcnt.as<unsigned int>(), wroot.as<int>(), m->wkids);
+        k_wide_next<<<1, 32, 0, st>>>(lvl.as<int>());
+      }
+    }
+    int hl[4] = {0, 0, 0, 0};
+    MESH_TRY(cudaMemcpyAsync(hl, lvl.p, sizeof(hl), cudaMemcpyDeviceToHost, st));
+    MESH_TRY(cudaStreamSynchronize(st));
+    if (hl[0] != hl[1] || hl[1] < 1 || hl[1] > cap_w) { tpmc_mesh_destroy(m); return TPMC_ECUDA; }   // the frontier must be empty
+    m->n_wide = hl[1];
+    MESH_TRY(cudaMalloc((void**)&m->wnodes, sizeof(uint4) * 4 * m->n_wide));
+    if (nt > 1) MESH_TRY(cudaMalloc((void**)&m->wnodes_r, sizeof(uint4) * 4 * m->n_wide));
+    k_compact_wide<<<(unsigned)((m->n_wide + kBlock - 1) / kBlock), kBlock, 0, st>>>(
+        box.as<float>(), n_int, m->wkids_bin, m->wkids, m->n_wide, (double)m->q_origin[0], (double)m->q_origin[1],
+        (double)m->q_origin[2], (double)m->q_scale[0], (double)m->q_scale[1], (double)m->q_scale[2], m->wnodes);
   }
   DevBuf cq;
   MESH_TRY(cudaMalloc((void**)&m->cull_c, sizeof(uint4) * 2 * kCullNodes));
@@ -806,28 +994,28 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
 
 // Refit the compact hierarchy in the frame x' = R x (row-major 3x3, orthonormal) on `stream`; fills *grid.
 // Called by tpmc_run with the stream frame of the run.  nt == 1: the body-frame hierarchy is used.
-int tpmc_mesh_align(tpmc_mesh* m, const double R[9], cudaStream_t st, const QuantGrid** grid_out, const uint4** cnodes_out) {
+int tpmc_mesh_align(tpmc_mesh* m, const double R[9], cudaStream_t st, const QuantGrid** grid_out, const uint4** wnodes_out) {
   *grid_out = m->grid_dev;   // [0]: the body-frame grid, [1]: the aligned one
-  *cnodes_out = m->cnodes;
+  *wnodes_out = m->wnodes;
   if (m->nt < 2 || !m->kids) return TPMC_OK;
   const int64_t nt = m->nt, n_int = nt - 1;
   const unsigned gt = (unsigned)((nt + kBlock - 1) / kBlock);
   TPMC_CUDA_TRY(cudaMemcpyAsync(m->align_R, R, 9 * sizeof(double), cudaMemcpyHostToDevice, st));
   TPMC_CUDA_TRY(cudaMemsetAsync(m->arrive, 0, sizeof(int) * n_int, st));
   k_leaf_boxes_rot<<<gt, kBlock, 0, st>>>(m->tris, nt, n_int, m->align_R, m->rbox);
-  k_refit<<<gt, kBlock, 0, st>>>((int)nt, m->kids, m->parent, m->rbox, m->arrive, m->nodes_r);
+  k_refit<<<gt, kBlock, 0, st>>>((int)nt, m->kids, m->parent, m->rbox, m->arrive, nullptr);
   k_align_grid<<<1, 32, 0, st>>>(m->rbox, m->align_R, m->align_R + 9, m->grid_dev + 1);
-  k_compact_nodes<<<(unsigned)((n_int + kBlock - 1) / kBlock), kBlock, 0, st>>>(m->nodes_r, n_int, 0, 0, 0, 1, 1, 1, m->cnodes_r,
-                                                                                m->align_R + 9);
+  k_compact_wide<<<(unsigned)((m->n_wide + kBlock - 1) / kBlock), kBlock, 0, st>>>(m->rbox, n_int, m->wkids_bin, m->wkids, m->n_wide, 0, 0,
+                                                                                   0, 1, 1, 1, m->wnodes_r, m->align_R + 9);
   TPMC_CUDA_TRY(cudaGetLastError());
-  *cnodes_out = m->cnodes_r;
+  *wnodes_out = m->wnodes_r;
   *grid_out = m->grid_dev + 1;
   return TPMC_OK;
 }
 
 extern "C" void tpmc_mesh_destroy(tpmc_mesh* m) {
   if (!m) return;
-  cudaFree(m->nodes); cudaFree(m->tris); cudaFree(m->cull_c); cudaFree(m->kids); cudaFree(m->parent); cudaFree(m->arrive); cudaFree(m->rbox); cudaFree(m->nodes_r); cudaFree(m->cnodes_r); cudaFree(m->align_R); cudaFree(m->grid_dev); cudaFree(m->cnodes); cudaFree(m->horizon); cudaFree(m->surf_TW); cudaFree(m->surf_sigma);
+  cudaFree(m->nodes); cudaFree(m->tris); cudaFree(m->cull_c); cudaFree(m->kids); cudaFree(m->parent); cudaFree(m->arrive); cudaFree(m->rbox); cudaFree(m->wkids_bin); cudaFree(m->wkids); cudaFree(m->wnodes); cudaFree(m->wnodes_r); cudaFree(m->align_R); cudaFree(m->grid_dev); cudaFree(m->cnodes); cudaFree(m->horizon); cudaFree(m->surf_TW); cudaFree(m->surf_sigma);
   for (int pi = 0; pi < kPipes; ++pi) {
     Pipe& pp = m->pipe[pi];
     for (int k = 0; k < 2; ++k) { cudaFree(pp.q_o[k]); cudaFree(pp.q_v[k]); cudaFree(pp.q_f[k]); cudaFree(pp.q_key[k]); cudaFree(pp.hist[k]); }

@@ -233,10 +233,14 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
 #ifndef TPMC_TRACE_MIN_BLOCKS
 #define TPMC_TRACE_MIN_BLOCKS 8
 #endif
+#ifndef TPMC_NODE_STEPS
+#define TPMC_NODE_STEPS 1   // wide-node steps per warp vote
+#endif
 struct TraceTune { int node_min, refill_idle; };
-constexpr int kFetchChunk = 64;   // rays a warp reserves per atomic on the queue head
+constexpr int kFetchChunk = 32;   // rays a warp reserves per atomic on the queue head: one per lane (set up together, see k_trace_wf)
+constexpr int kChunkWords = 11;   // per ray of the chunk: 1/d', the two slab offsets per axis, the octant, the queue slot
 
-__global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf(const uint4* __restrict__ cnodes,
+__global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf(const uint4* __restrict__ wnodes,
                                                              const QuantGrid* __restrict__ gridp,
                                                              const float4* __restrict__ tris, const RayQueue q,
                                                              const unsigned int* __restrict__ order,
@@ -248,12 +252,13 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
                                                              unsigned long long* __restrict__ stats,
                                                              const TraceTune tune) {
   const int kNodeMin = tune.node_min, kRefillIdle = tune.refill_idle;
-  __shared__ int sstack[(TPMC_STACK_SMEM + 2) * kTraceBlock];
+  __shared__ int sstack[(TPMC_STACK_SMEM + 6) * kTraceBlock];      // two guard rows, TPMC_STACK_SMEM rows, four of headroom
+  __shared__ unsigned int schunk[kChunkWords][kTraceBlock];        // the warp's current chunk of rays, set up for the walk
   int* stk = sstack + 2 * kTraceBlock + threadIdx.x;   // level 0; levels -1, -2 are the guard entries (walk_pop)
   stk[-kTraceBlock] = TPMC_SENTINEL;
   stk[-2 * kTraceBlock] = TPMC_SENTINEL;
   const unsigned int na = min(n_rays[0], cap), n = na + n_rays[1];   // region A (reflected), region B (primaries)
-  const int lane = threadIdx.x & 31;
+  const int lane = threadIdx.x & 31, wbase = threadIdx.x & ~31;
   const unsigned FULL = 0xFFFFFFFFu;
   bool has = false, exhausted = false, fin = false;
   unsigned int r = 0, pool_next = 0, pool_end = 0;
@@ -263,7 +268,11 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
   cnt.nodes = 0; cnt.tris = 0;
   unsigned int n_escaped = 0u;   // rays that ended without a candidate facet: these particles retire here
   for (;;) {
-    // ---- refill idle lanes from the warp's chunk of the queue (one atomic per kFetchChunk rays)
+    // ---- refill idle lanes from the warp's chunk of the queue.  A chunk is kFetchChunk = 32 consecutive rays (one
+    // atomic on the queue head); when a warp takes one, ALL its lanes set up one ray each for the walk (rotation into the
+    // grid's frame, reciprocal direction, slab offsets: grid_ray) and park the result in shared memory, so that the
+    // ~150 instructions of set-up run with 32 lanes active instead of the handful that happen to be idle; a lane that
+    // runs out of work later picks its ray up from there.
     const unsigned idle = __ballot_sync(FULL, !has && !exhausted);
     const unsigned busy0 = __ballot_sync(FULL, has);
     if (idle && (__popc(idle) >= kRefillIdle || busy0 == 0u)) {
@@ -272,21 +281,51 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
         if (lane == 0) base = atomicAdd(next_ray, (unsigned)kFetchChunk);
         pool_next = __shfl_sync(FULL, base, 0);
         pool_end = pool_next + kFetchChunk;
+        const unsigned int rr = pool_next + lane;
+        if (rr < n) {
+          const unsigned int phys = order ? __ldcs(order + rr) : ((rr < na) ? rr : cap + (rr - na));   // physical slot (in key order when sorted)
+          const float4 ro = __ldcs(q.o + phys), rv = __ldcs(q.v + phys);
+          const float o[3] = {ro.x, ro.y, ro.z}, d[3] = {rv.x, rv.y, rv.z};
+          GridRay g;
+          grid_ray(g, *gridp, o, d);
+          unsigned int* c = &schunk[0][wbase + lane];
+#pragma unroll
+          for (int k = 0; k < 3; ++k) {
+            c[k * kTraceBlock] = __float_as_uint(g.id[k]);
+            c[(3 + k) * kTraceBlock] = __float_as_uint(g.ncn[k]);
+            c[(6 + k) * kTraceBlock] = __float_as_uint(g.ncf[k]);
+          }
+          c[9 * kTraceBlock] = (g.sn[0] == 0x7632u ? 1u : 0u) | (g.sn[1] == 0x7632u ? 2u : 0u) | (g.sn[2] == 0x7632u ? 4u : 0u);
+          c[10 * kTraceBlock] = phys;
+        }
+        __syncwarp();
       }
       const unsigned avail = pool_end - pool_next, rank = __popc(idle & lanemask_lt());
       if (!has && !exhausted) {
         if (pool_next >= n) {
           exhausted = true;
-        } else if (rank < avail) {
-          r = pool_next + rank;
-          if (r < n) {
-            r = order ? __ldcs(order + r) : ((r < na) ? r : cap + (r - na));   // physical slot (in key order when sorted)
-            walk_init(w, *gridp, __ldcs(q.o + r), __ldcs(q.v + r), __ldcs(q.f + r));
-            has = true;
+        } else if (rank < avail && pool_next + rank < n) {
+          const unsigned int* c = &schunk[0][wbase + (kFetchChunk - avail) + rank];
+#pragma unroll
+          for (int k = 0; k < 3; ++k) {
+            w.g.id[k] = __uint_as_float(c[k * kTraceBlock]);
+            w.g.ncn[k] = __uint_as_float(c[(3 + k) * kTraceBlock]);
+            w.g.ncf[k] = __uint_as_float(c[(6 + k) * kTraceBlock]);
           }
+          const unsigned int oct = c[9 * kTraceBlock];
+#pragma unroll
+          for (int k = 0; k < 3; ++k) {
+            const bool neg = (oct >> k) & 1u;
+            w.g.sn[k] = neg ? 0x7632u : 0x7610u;
+            w.g.sf[k] = neg ? 0x7610u : 0x7632u;
+          }
+          r = c[10 * kTraceBlock];
+          walk_reset(w, __ldcs(q.f + r));
+          has = true;
         }
       }
       pool_next += min((unsigned)__popc(idle), avail);
+      __syncwarp();   // every read of the chunk is done before a later iteration may replace it
     }
     if (__ballot_sync(FULL, has) == 0u) break;
     // ---- node phase: two node steps per vote
@@ -298,8 +337,10 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
         if (mn == 0u || ml != 0u) break;
       }
       if (at_node) {
-        walk_node(w, cnodes, stk, kTraceBlock, cnt);
-        if ((unsigned)w.cur < (unsigned)TPMC_SENTINEL) walk_node(w, cnodes, stk, kTraceBlock, cnt);
+        walk_node(w, wnodes, stk, kTraceBlock, cnt);
+#if TPMC_NODE_STEPS > 1
+        if ((unsigned)w.cur < (unsigned)TPMC_SENTINEL) walk_node(w, wnodes, stk, kTraceBlock, cnt);
+#endif
       }
     }
     // ---- leaf phase: every lane that put a leaf aside classifies it
@@ -1079,12 +1120,12 @@ extern "C" int tpmc_run(tpmc_mesh* m, const tpmc_params* params, void* cuda_stre
   TPMC_CUDA_TRY(cudaEventRecord(m->ev0, st));
   // the traversal's hierarchy: body frame, or refitted in the stream frame of this run (x' = R^T x: z' along the stream)
   const QuantGrid* qg_t = m->grid_dev;
-  const uint4* cnodes_t = m->cnodes;
+  const uint4* wnodes_t = m->wnodes;
   if (!exact && want_alignment(params)) {
     double Rt[9];
     for (int a = 0; a < 3; ++a)
       for (int b2 = 0; b2 < 3; ++b2) Rt[3 * a + b2] = rc.R[3 * b2 + a];
-    rcode = tpmc_mesh_align(m, Rt, st, &qg_t, &cnodes_t);
+    rcode = tpmc_mesh_align(m, Rt, st, &qg_t, &wnodes_t);
     if (rcode != TPMC_OK) return rcode;
   }
   m->pipe[0].main = st;
@@ -1103,7 +1144,7 @@ extern "C" int tpmc_run(tpmc_mesh* m, const tpmc_params* params, void* cuda_stre
   TPMC_CUDA_TRY(cudaMemsetAsync(m->totals, 0, 4 * sizeof(double), st));
   if (any_dbg && params->count)
     k_init_debug<<<(unsigned)((params->count + 255) / 256), 256, 0, st>>>(dbg0, params->count);
-  unsigned long long launches = ((any_dbg && params->count) ? 1 : 0) + (cnodes_t != m->cnodes ? 4 : 0);   // + the refit kernels
+  unsigned long long launches = ((any_dbg && params->count) ? 1 : 0) + (wnodes_t != m->wnodes ? 4 : 0);   // + the refit kernels
 
   // Particle indices inside the queues are 32-bit offsets into a chunk of the slice.
   const unsigned long long kChunk = params->chunk_particles ? params->chunk_particles : 0xF0000000ull;
@@ -1184,7 +1225,7 @@ extern "C" int tpmc_run(tpmc_mesh* m, const tpmc_params* params, void* cuda_stre
       }
       if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[7], s1));
       if (!exact) {
-        k_trace_wf<<<g.trace, kTraceBlock, 0, s1>>>(cnodes_t, qg_t, m->tris, Q[p], sorted ? pp.order : nullptr, cap,
+        k_trace_wf<<<g.trace, kTraceBlock, 0, s1>>>(wnodes_t, qg_t, m->tris, Q[p], sorted ? pp.order : nullptr, cap,
                                                     pp.ctr + 2 * p, pp.ctr + 4, pp.hit_ray,
                                                     pp.hit_cand, pp.ctr + 5, m->stats, trace_tune());
         if (tw) TPMC_CUDA_TRY(cudaEventRecord(ev[3], s1));
@@ -1307,13 +1348,13 @@ extern "C" int tpmc_trace(tpmc_mesh* m, const float* d_o, const float* d_d, cons
   RayQueue q = {pp.q_o[0], pp.q_v[0], pp.q_f[0], pp.q_key[0], nullptr};
   const unsigned int un = (unsigned int)n;
   const QuantGrid* qg_t = m->grid_dev;
-  const uint4* cnodes_t = m->cnodes;
+  const uint4* wnodes_t = m->wnodes;
   if (h_align_V) {   // the hierarchy refitted in the stream frame of this velocity, as tpmc_run uses it
     double R[9], Rt[9];
     host_rotation(h_align_V, R);
     for (int a = 0; a < 3; ++a)
       for (int b2 = 0; b2 < 3; ++b2) Rt[3 * a + b2] = R[3 * b2 + a];
-    rcode = tpmc_mesh_align(m, Rt, st, &qg_t, &cnodes_t);
+    rcode = tpmc_mesh_align(m, Rt, st, &qg_t, &wnodes_t);
     if (rcode != TPMC_OK) return rcode;
   }
   TPMC_CUDA_TRY(cudaMemsetAsync(pp.ctr, 0, kCtrWords * sizeof(unsigned int), st));
@@ -1321,7 +1362,7 @@ extern "C" int tpmc_trace(tpmc_mesh* m, const float* d_o, const float* d_d, cons
   TPMC_CUDA_TRY(cudaMemsetAsync(m->stats, 0, ST_COUNT * sizeof(unsigned long long), st));
   k_pack_rays<<<(un + 255) / 256, 256, 0, st>>>(d_o, d_d, d_f_prev, un, q, d_facet, d_tau);
   // the production traversal (fp32 wavefront + candidate lists), then the exact fp64 resolve
-  k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(cnodes_t, qg_t, m->tris, q, nullptr, (unsigned int)(2 * m->wave_cap), pp.ctr, pp.ctr + 4,
+  k_trace_wf<<<g.trace, kTraceBlock, 0, st>>>(wnodes_t, qg_t, m->tris, q, nullptr, (unsigned int)(2 * m->wave_cap), pp.ctr, pp.ctr + 4,
                                               pp.hit_ray, pp.hit_cand, pp.ctr + 5, m->stats, trace_tune());
   k_resolve_only<<<g.reflect, kTraceBlock, 0, st>>>(m->nodes, m->tris, q, pp.hit_ray, pp.hit_cand, pp.ctr + 5, d_facet,
                                                     d_tau);

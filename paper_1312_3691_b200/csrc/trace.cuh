@@ -21,7 +21,7 @@
 #include "common.cuh"
 
 #ifndef TPMC_STACK_SMEM
-#define TPMC_STACK_SMEM 24      // stack entries per thread kept in shared memory
+#define TPMC_STACK_SMEM 24      // stack entries per thread kept in shared memory (+ 3 rows of headroom in the wavefront kernel)
 #endif
 #define TPMC_STACK_LOCAL 80     // overflow entries (a Karras tree over 64-bit keys + index is <= 97 deep)
 #define TPMC_SENTINEL ((int)0x7FFFFFFF)
@@ -298,9 +298,8 @@ struct Walk {
   int nc;              // number of candidates; TPMC_MAX_CAND+1 = overflow
 };
 
-__device__ __forceinline__ void walk_init(Walk& w, const QuantGrid& g, const float4 ro, const float4 rv, int f_prev) {
-  const float o[3] = {ro.x, ro.y, ro.z}, d[3] = {rv.x, rv.y, rv.z};
-  grid_ray(w.g, g, o, d);
+// start of a walk: everything but the ray in grid coordinates (w.g, set up when the warp fetched its chunk of rays)
+__device__ __forceinline__ void walk_reset(Walk& w, int f_prev) {
   w.tmax = INFINITY;
   w.f_prev = f_prev;
   w.cur = 0;
@@ -387,46 +386,60 @@ __device__ __forceinline__ void walk_add_candidate(Walk& w, int slot, int cls, f
   ++w.nc;
 }
 
-// One internal-node step (two slab tests, push the far child) -- requires w.cur >= 0 and != SENTINEL.
-// Node words: 0-2 = child 0 (x, y, z), 3-5 = child 1, each lo | hi << 16; 6-7 = the child refs.
-__device__ __forceinline__ void walk_node(Walk& w, const uint4* __restrict__ cnodes, int* stk, int sstride,
+// One step at a wide node (four slab tests; the children the ray enters are taken nearest first) -- requires
+// w.cur >= 0 and != SENTINEL.  Node words (k_compact_wide, lbvh.cu): 3k .. 3k+2 = box of child k (x, y, z), each
+// lo | hi << 16; 12-15 = the four child refs.
+__device__ __forceinline__ void ce_sort(float& ka, int& ra, float& kb, int& rb) {   // compare-exchange: ka <= kb after
+  const bool sw = kb < ka;
+  const float k0 = fminf(ka, kb), k1 = fmaxf(ka, kb);
+  const int r0 = sw ? rb : ra, r1 = sw ? ra : rb;
+  ka = k0; kb = k1; ra = r0; rb = r1;
+}
+__device__ __forceinline__ void walk_node(Walk& w, const uint4* __restrict__ wnodes, int* stk, int sstride,
                                           TraceCounters& cnt) {
-  uint4 a, b;
-  ldg256u(cnodes + 2 * (size_t)w.cur, a, b);
+  uint4 a, b, c, d;
+  ldg256u(wnodes + 4 * (size_t)w.cur, a, b);
+  ldg256u(wnodes + 4 * (size_t)w.cur + 2, c, d);
   ++cnt.nodes;
-  float n0, f0, n1, f1;
+  float n0, f0, n1, f1, n2, f2, n3, f3;
   grid_slab(w.g, a.x, a.y, a.z, n0, f0);
   grid_slab(w.g, a.w, b.x, b.y, n1, f1);
-  // the clamps also drop a NaN that survived three NaN plane distances (zero direction)
-  const bool h0 = !(fmaxf(n0, 0.0f) > fminf(f0, w.tmax));
-  const bool h1 = !(fmaxf(n1, 0.0f) > fminf(f1, w.tmax));
-  // Branch-free child selection and stack traffic.  The near child is next and the far child is pushed; a leaf
-  // that becomes next while no leaf is put aside is put aside (speculation: it is tested in the next leaf
-  // phase) and the walk goes on with the far child, or with the top of the stack.  The two entries below the
-  // top are always read, the slot above it is written whenever both boxes are hit.
-  const bool both = h0 && h1, any = h0 || h1;
-#ifdef TPMC_COUNT_STALE
-  if (!any) ++cnt.tris;   // experiment: visits that hit neither child
-#endif
-  const bool swp = h1 && (!h0 || n1 < n0);
-  const int c0 = (int)b.z, c1 = (int)b.w;
-  const int nearc = swp ? c1 : c0, farc = swp ? c0 : c1;
-  if (both && w.sp >= TPMC_STACK_SMEM) { walk_abort(w); return; }   // rare
-  const int top = stk[(w.sp - 1) * sstride], top2 = stk[(w.sp - 2) * sstride];
-  if (both) stk[w.sp * sstride] = farc;
-  const bool empty = w.stash == 0;
-  const bool take = any && nearc < 0 && empty;       // the near child is a leaf: put it aside
-  const bool popleaf = !any && top < 0 && empty;     // nothing hit and the top of the stack is a leaf: likewise
-  const int x = both ? farc : top, y = popleaf ? top2 : top;
-  const int nx = take ? x : nearc;
-  w.cur = any ? nx : y;
-  if (popleaf) w.stash = top;
-  if (take) w.stash = nearc;
-  int sp = w.sp;
-  if (both) ++sp;
-  if (!any) --sp;
-  if (take || popleaf) --sp;
-  w.sp = max(sp, 0);
+  grid_slab(w.g, b.z, b.w, c.x, n2, f2);
+  grid_slab(w.g, c.y, c.z, c.w, n3, f3);
+  // entered iff !(max(near, 0) > min(far, tmax)); the clamps also drop a NaN that survived three NaN plane distances
+  // (zero direction).  Sort key: the entry distance (finite) of an entered child, +inf of a missed one.
+  // (Whatever the keys, each of the four refs is safe to visit: a box at infinity sorted among the missed ones costs work, not a hit.)
+  const float INF = __int_as_float(0x7F800000);
+  float k0 = fmaxf(n0, 0.0f), k1 = fmaxf(n1, 0.0f), k2 = fmaxf(n2, 0.0f), k3 = fmaxf(n3, 0.0f);
+  const bool h0 = !(k0 > fminf(f0, w.tmax)), h1 = !(k1 > fminf(f1, w.tmax)), h2 = !(k2 > fminf(f2, w.tmax)),
+             h3 = !(k3 > fminf(f3, w.tmax));
+  k0 = h0 ? k0 : INF; k1 = h1 ? k1 : INF; k2 = h2 ? k2 : INF; k3 = h3 ? k3 : INF;
+  const int cnt_h = (int)h0 + (int)h1 + (int)h2 + (int)h3;
+  int r0 = (int)d.x, r1 = (int)d.y, r2 = (int)d.z, r3 = (int)d.w;
+  ce_sort(k0, r0, k1, r1);
+  ce_sort(k2, r2, k3, r3);
+  ce_sort(k0, r0, k2, r2);
+  ce_sort(k1, r1, k3, r3);
+  ce_sort(k1, r1, k2, r2);
+  // Branch-free stack traffic.  The virtual sequence of what comes next is [r0 .. r_{cnt-1}, top, top2, ...]: the
+  // entered children nearest first, then the stack.  Its first entry is next; if that is a leaf and no leaf is put
+  // aside it is put aside (speculation: it is tested in the next leaf phase) and the second entry is next.  Children
+  // r1 .. r_{cnt-1} are written above the top of the stack, the farthest lowest; the two entries below the top are
+  // always read.  The stack has TPMC_STACK_SMEM + 3 rows above the two guard rows.
+  const int sp = w.sp;
+  if (sp > TPMC_STACK_SMEM) { walk_abort(w); return; }   // rare; three rows of headroom above TPMC_STACK_SMEM
+  const int top = stk[(sp - 1) * sstride], top2 = stk[(sp - 2) * sstride];
+  // r_j (j = 1..3) goes to row sp + ((cnt - 1 - j) & 3): an entered child lands at sp + cnt - 1 - j, a missed one
+  // (j >= cnt) above the new top, where it is never read -- three unconditional stores, no branch
+  stk[(sp + ((cnt_h - 2) & 3)) * sstride] = r1;
+  stk[(sp + ((cnt_h - 3) & 3)) * sstride] = r2;
+  stk[(sp + (cnt_h & 3)) * sstride] = r3;
+  const int e0 = cnt_h >= 1 ? r0 : top;
+  const int e1 = cnt_h >= 2 ? r1 : (cnt_h == 1 ? top : top2);
+  const bool take = e0 < 0 && w.stash == 0;
+  if (take) w.stash = e0;
+  w.cur = take ? e1 : e0;
+  w.sp = max(sp + cnt_h - (take ? 2 : 1), 0);
 }
 
 // One leaf step (fp32 facet classification of the leaf put aside), then the next leaf, if the walk stands at
