@@ -327,7 +327,7 @@ def main():
         t = avg_ms * 1e-3
         alg_bw = rays_per_launch * per_seg_bytes / t / 1e9 if t > 0 else 0.0                  # GB/s
         alg_ops = rays_per_launch * per_seg_ops / t / 1e12 if t > 0 else 0.0                  # T lane-op/s
-        fetched_bw = (nodes * 32 + tris * 48) / launches_trace / t / 1e9 if t > 0 else 0.0    # what the kernel really gathers
+        fetched_bw = (nodes * 64 + tris * 48) / launches_trace / t / 1e9 if t > 0 else 0.0    # what the kernel really gathers (64-byte wide nodes)
         ms_stat = tot["ms"]
         traffic, traffic_src = ncu_traffic(args.config)
         roof = {"kernel": "k_trace_wf", "segments_per_launch": rays_per_launch, "avg_launch_ms": avg_ms,
@@ -347,7 +347,7 @@ def main():
                          "peak_source": "measured in this run (tpmc_measure_peaks): independent 32-byte ld.global.nc gathers over "
                                         "83 MB, 8 x 128 threads per SM",
                          "fetched_view": {"achieved": fetched_bw, "peak": gpk, "unit": "GB/s", "frac": fetched_bw / gpk,
-                                          "what": "nodes x 32 B + facets x 48 B the kernel really fetched"},
+                                          "what": "wide nodes x 64 B + facets x 48 B the kernel really fetched"},
                          "alu_view": {"achieved": alg_ops, "peak": peaks["fp32_lane_ops_per_s"] / 1e12, "unit": "T lane-op/s",
                                       "frac": alg_ops / (peaks["fp32_lane_ops_per_s"] / 1e12),
                                       "peak_source": "measured in this run: FFMA lane-instructions/s at full occupancy"}})
