@@ -232,9 +232,9 @@ def main():
     # between steps by writing a 512 MB buffer (outside the per-step event pairs).
     flush = None if args.config == "C5" else torch.empty(512 << 20, dtype=torch.uint8, device=dev)
 
-    def step(k, stats=None):
+    def step(k, stats=None, flags=0):
         cfg = cfgs[attitude_index(k, rank, world, len(cfgs))]
-        p, keep = tpmc.make_params(cfg)
+        p, keep = tpmc.make_params(cfg, flags=flags)
         rc = L.tpmc_run(mesh._h, C.byref(p), stream.cuda_stream or None, force.data_ptr(), torque.data_ptr(),
                         facets.data_ptr(), None if stats is None else C.byref(stats), None)
         if rc != 0:
@@ -281,6 +281,17 @@ def main():
         for f in keys:
             tot[f] = tot.get(f, 0) + getattr(st, f)
     barrier()
+    # ---- and once more with the seed kernels of the next wave BEHIND trace/reflect instead of beside them
+    #      (TPMC_FLAG_SERIAL_SEED; same kernels, same grids, same arguments): the event pair around a launch then
+    #      brackets that kernel alone, not the kernel plus whatever share of the SMs the other stream took meanwhile.
+    #      The roofline's launch duration is taken from this pass; the overlapped one is reported beside it.
+    ser = {}
+    for k in range(args.steps):
+        st = tpmc.tpmc_stats()
+        step(args.warmup + k, st, flags=tpmc.TPMC_FLAG_SERIAL_SEED)
+        for f in ("ms", "ms_seed", "ms_trace", "ms_reflect", "ms_finish", "ms_sort", "trace_launches", "traced_rays"):
+            ser[f] = ser.get(f, 0) + getattr(st, f)
+    barrier()
     hits, segs, launches = tot["hits"], tot["segments"], tot["kernel_launches"]
 
     # ---- end to end: host buffers through tpmc_run_host (params H2D, results D2H inside the region)
@@ -317,7 +328,8 @@ def main():
         hbm, hbm_src = hbm_peak()
         traced, nodes, tris = tot["traced_rays"], tot["node_visits"], tot["tri_tests"]
         launches_trace = max(tot["trace_launches"], 1)         # k_trace_wf launches, rays they processed
-        avg_ms = tot["ms_trace"] / launches_trace
+        avg_ms_overlapped = tot["ms_trace"] / launches_trace   # seed kernels of the next wave share the SMs meanwhile
+        avg_ms = ser["ms_trace"] / max(ser["trace_launches"], 1)   # the kernel alone (serialised pass)
         depth = int(np.ceil(np.log2(max(mesh.nt, 2))))
         # Algorithmic work per segment: ceil(log2 T) nodes x 64 B + one triangle of
         # 48 B + 32 B ray in + 8 B result out; ceil(log2 T) node visits x 2 slab tests x 18 ops + one facet test of 60 ops.
@@ -331,6 +343,14 @@ def main():
         ms_stat = tot["ms"]
         traffic, traffic_src = ncu_traffic(args.config)
         roof = {"kernel": "k_trace_wf", "segments_per_launch": rays_per_launch, "avg_launch_ms": avg_ms,
+                "avg_launch_ms_overlapped": avg_ms_overlapped,
+                "timing": "CUDA events around every k_trace_wf launch on its stream, in a pass with the seed kernels of the next "
+                          "wave enqueued behind trace/reflect (TPMC_FLAG_SERIAL_SEED) so that the bracket holds this kernel alone; "
+                          "avg_launch_ms_overlapped is the same bracket in the normal, overlapped schedule",
+                "ms_per_step_serialised": ser["ms"] / args.steps,
+                "share_of_step_serialised": {k: (ser[f] / ser["ms"] if ser.get("ms") else None) for k, f in
+                                             (("seed+precull", "ms_seed"), ("k_trace_wf", "ms_trace"), ("k_reflect", "ms_reflect"),
+                                              ("k_finish_final", "ms_finish"))},
                 "launches_timed": int(launches_trace), "traffic": traffic, "traffic_source": traffic_src,
                 "algorithmic_bytes_per_segment": per_seg_bytes, "algorithmic_ops_per_segment": per_seg_ops,
                 "nodes_per_traced_segment": nodes / max(traced, 1), "tri_tests_per_traced_segment": tris / max(traced, 1),

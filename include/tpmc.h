@@ -48,6 +48,8 @@ extern "C" {
 #define TPMC_FLAG_EXACT_TRACE 0x10u /* every segment by the fp64 closest-hit search (no fp32 filter, no candidate lists) */
 #define TPMC_FLAG_NO_AGGREGATION 0x40u /* one fp64 atomic per hit and component even on bodies with few facets */
 #define TPMC_FLAG_SORT_RAYS 0x20u   /* rays traced in the order of a spatial key (counting sort before the traversal) */
+#define TPMC_FLAG_SERIAL_SEED 0x80u /* the seed kernels of the next wave run on the caller's stream, behind trace/reflect, not beside
+                                      * them: the per-kernel times of tpmc_stats are then each kernel's own (measurement aid) */
 
 /* tpmc_params.control_volume */
 #define TPMC_CV_SPHERE 0 /* the paper's scheme: spherical control volume, eqs. (10)-(15) */
@@ -161,6 +163,14 @@ int tpmc_mesh_set_surface(tpmc_mesh* mesh, const double* T_W, const double* sigm
  * child >= 0: internal node, child < 0: leaf holding sorted triangle ~child),
  * leaf_facet [nt] = facet id stored in each sorted triangle slot.  Either pointer may be NULL. */
 int tpmc_mesh_copy_bvh(const tpmc_mesh* mesh, float* h_nodes, int32_t* h_leaf_facet);
+
+/* Copy the wide (4-ary) hierarchy the wavefront traversal walks, body frame, to the host for inspection.
+ * *n_wide = number of wide nodes (always written); h_wnodes [n_wide][16] uint32 or NULL: words 3k .. 3k+2 = box of child
+ * k (x, y, z), each lo | hi << 16 in unsigned 16-bit grid coordinates (lo rounded down, hi up; an empty slot has
+ * lo = 65535, hi = 0), words 12-15 = the child refs (>= 0: wide node, < 0: leaf holding sorted triangle ~ref);
+ * h_grid [6] float or NULL: origin xyz and step xyz of the grid, x = origin + q * step.  The radix tree is collapsed
+ * breadth-first (wide node 0 is the root): every sorted triangle is a leaf of exactly one wide node. */
+int tpmc_mesh_copy_wide(const tpmc_mesh* mesh, int64_t* n_wide, uint32_t* h_wnodes, float* h_grid);
 
 /* Copy the escape horizons to the host for inspection: h_horizon [nt][16] bytes, indexed by sorted triangle
  * slot (see leaf_facet above) and azimuth sector.  For a one-sided facet with unit normal n, first edge

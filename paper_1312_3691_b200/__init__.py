@@ -22,12 +22,12 @@ TPMC_MEM_HOST, TPMC_MEM_DEVICE = 0, 1
 TPMC_MAX_SPECIES = 8
 TPMC_MAX_BOUNCES = 0x0FFFFFFF
 TPMC_FLAG_NO_PRECULL, TPMC_FLAG_NO_HORIZON, TPMC_FLAG_ALIGN_OFF, TPMC_FLAG_ALIGN_ON = 0x01, 0x02, 0x04, 0x08
-TPMC_FLAG_EXACT_TRACE, TPMC_FLAG_SORT_RAYS, TPMC_FLAG_NO_AGGREGATION = 0x10, 0x20, 0x40
+TPMC_FLAG_EXACT_TRACE, TPMC_FLAG_SORT_RAYS, TPMC_FLAG_NO_AGGREGATION, TPMC_FLAG_SERIAL_SEED = 0x10, 0x20, 0x40, 0x80
 TPMC_CV_SPHERE, TPMC_CV_BOX, TPMC_CV_BOX_UNWEIGHTED = 0, 1, 2
 
 EXPORTS = ["tpmc_mesh_create", "tpmc_mesh_destroy", "tpmc_mesh_info", "tpmc_mesh_copy_bvh", "tpmc_run",
            "tpmc_mesh_copy_horizon", "tpmc_run_host", "tpmc_seed", "tpmc_trace", "tpmc_strerror", "tpmc_last_cuda_error", "tpmc_version",
-           "tpmc_measure_peaks", "tpmc_mesh_set_surface", "tpmc_run_sweep"]
+           "tpmc_measure_peaks", "tpmc_mesh_set_surface", "tpmc_run_sweep", "tpmc_mesh_copy_wide"]
 
 
 class TpmcError(RuntimeError):
@@ -94,6 +94,8 @@ def lib():
         L.tpmc_mesh_info.argtypes = [vp, C.POINTER(tpmc_mesh_info_t)]
         L.tpmc_mesh_set_surface.restype = C.c_int
         L.tpmc_mesh_set_surface.argtypes = [vp, vp, vp, C.c_int, vp]
+        L.tpmc_mesh_copy_wide.restype = C.c_int
+        L.tpmc_mesh_copy_wide.argtypes = [vp, vp, vp, vp]
         L.tpmc_mesh_copy_bvh.restype = C.c_int
         L.tpmc_mesh_copy_bvh.argtypes = [vp, vp, vp]
         L.tpmc_mesh_copy_horizon.restype = C.c_int
@@ -239,6 +241,14 @@ class Mesh:
         _check(lib().tpmc_mesh_copy_bvh(self._h, nodes.ctypes.data, leaf.ctypes.data), "tpmc_mesh_copy_bvh")
         return nodes, leaf
 
+    def copy_wide(self):
+        n = C.c_int64(0)
+        _check(lib().tpmc_mesh_copy_wide(self._h, C.byref(n), None, None), "tpmc_mesh_copy_wide")
+        wn = np.zeros((n.value, 16), dtype=np.uint32)
+        grid = np.zeros(6, dtype=np.float32)
+        _check(lib().tpmc_mesh_copy_wide(self._h, C.byref(n), wn.ctypes.data, grid.ctypes.data), "tpmc_mesh_copy_wide")
+        return wn, grid
+
     def copy_horizon(self):
         hz = np.zeros((self.nt, 16), dtype=np.uint8)
         _check(lib().tpmc_mesh_copy_horizon(self._h, hz.ctypes.data), "tpmc_mesh_copy_horizon")
@@ -355,6 +365,10 @@ def tpmc_mesh_set_surface(mesh: Mesh, T_W=None, sigma=None, **kw) -> None:
 
 def tpmc_mesh_copy_bvh(mesh: Mesh):
     return mesh.copy_bvh()
+
+
+def tpmc_mesh_copy_wide(mesh: Mesh):
+    return mesh.copy_wide()
 
 
 def tpmc_mesh_copy_horizon(mesh: Mesh):

@@ -1100,6 +1100,15 @@ extern "C" int tpmc_mesh_copy_bvh(const tpmc_mesh* m, float* h_nodes, int32_t* h
   return TPMC_OK;
 }
 
+extern "C" int tpmc_mesh_copy_wide(const tpmc_mesh* m, int64_t* n_wide, uint32_t* h_wnodes, float* h_grid) {
+  if (!m || !n_wide) return TPMC_EINVAL;
+  *n_wide = m->n_wide;
+  if (h_wnodes) TPMC_CUDA_TRY(cudaMemcpy(h_wnodes, m->wnodes, sizeof(uint4) * 4 * m->n_wide, cudaMemcpyDeviceToHost));
+  if (h_grid)
+    for (int a = 0; a < 3; ++a) { h_grid[a] = m->q_origin[a]; h_grid[3 + a] = m->q_scale[a]; }
+  return TPMC_OK;
+}
+
 extern "C" int tpmc_mesh_copy_horizon(const tpmc_mesh* m, uint8_t* h_horizon) {
   if (!m || !h_horizon) return TPMC_EINVAL;
   TPMC_CUDA_TRY(cudaMemcpy(h_horizon, m->horizon, sizeof(uint4) * m->nt, cudaMemcpyDeviceToHost));

@@ -824,7 +824,7 @@ int make_run_const(const tpmc_mesh* m, const tpmc_params* p, RunConst* rc) {
   if (p->max_bounces < 1 || p->max_bounces > TPMC_MAX_BOUNCES) return TPMC_EINVAL;
   if (!(p->energy_accommodation >= 0.0 && p->energy_accommodation <= 1.0)) return TPMC_EINVAL;
   if ((p->flags & TPMC_FLAG_ALIGN_OFF) && (p->flags & TPMC_FLAG_ALIGN_ON)) return TPMC_EINVAL;
-  if (p->flags & ~0x7Fu) return TPMC_EINVAL;
+  if (p->flags & ~0xFFu) return TPMC_EINVAL;
   if (p->wave_particles && (p->wave_particles < 256 || p->wave_particles > (1ull << 28))) return TPMC_EINVAL;
   if (p->chunk_particles > 0xF0000000ull) return TPMC_EINVAL;
   if (p->control_volume < TPMC_CV_SPHERE || p->control_volume > TPMC_CV_BOX_UNWEIGHTED) return TPMC_EINVAL;
@@ -1196,7 +1196,7 @@ extern "C" int tpmc_run(tpmc_mesh* m, const tpmc_params* params, void* cuda_stre
       Pipe& pp = m->pipe[wv % K];
       const unsigned long long li = wv / K;            // iteration index within the pipeline
       const int p = (int)(li & 1);
-      cudaStream_t s1 = pp.main, s2 = pp.seed, s3 = pp.side;
+      cudaStream_t s1 = pp.main, s2 = (params->flags & TPMC_FLAG_SERIAL_SEED) ? pp.main : pp.seed, s3 = pp.side;
       const int b = (int)(li & 1);
       unsigned int* ovf = pp.ovf + (size_t)b * 2 * m->wave_cap;
       RayQueue Q[2] = {{pp.q_o[0], pp.q_v[0], pp.q_f[0], pp.q_key[0], sorted ? pp.hist[0] : nullptr},

@@ -176,6 +176,61 @@ def test_lbvh_topology_and_boxes(T, mesh_fn):
     assert info["build_ms"] > 0
 
 
+@pytest.mark.parametrize("mesh_fn", [lambda: ti.plate(30.0), lambda: ti.box(h=1.0), lambda: ti.meshes.Mesh(np.float32([[0, 0, 0], [1, 0, 0], [0, 1, 0]]), np.int32([[0, 1, 2]]), np.zeros(1, np.uint8), "one"),
+                                      lambda: ti.satellite(4, 0.125), lambda: ti.deep_chain(), lambda: ti.large_body(5, 24)])
+def test_wide_hierarchy_topology_and_boxes(T, mesh_fn):
+    """The 4-ary hierarchy the wavefront traversal walks (tpmc_mesh_copy_wide): a tree over the same sorted facets as the
+    radix tree, every facet in exactly one leaf, every node reached once from the root, and every stored child box --
+    16-bit grid coordinates, decoded as the traversal decodes them -- contains the exact fp32 bounds of everything below it."""
+    m = mesh_fn()
+    gm = T.Mesh(m.vertices, m.indices, m.flags)
+    _, leaf = gm.copy_bvh()
+    wn, grid = gm.copy_wide()
+    nt, nw = m.nt, wn.shape[0]
+    assert 1 <= nw <= max(nt - 1, 1)
+    refs = wn[:, 12:16].view(np.int32)
+    q = wn[:, :12].reshape(nw, 4, 3)
+    qlo, qhi = (q & 0xFFFF).astype(np.float64), (q >> 16).astype(np.float64)
+    org, step = grid[:3].astype(np.float64), grid[3:].astype(np.float64)
+    blo, bhi = org + qlo * step, org + qhi * step                       # decoded boxes [node, child, axis]
+    empty = (qlo == 65535).all(2) & (qhi == 0).all(2)
+    tri = m.vertices[m.indices[leaf]].astype(np.float64)                # [slot,3,3]
+    tlo, thi = tri.min(1), tri.max(1)
+    seen_leaf, seen_node = np.zeros(nt, int), np.zeros(nw, int)
+    seen_node[0] = 1
+    order, stack = [], [0]
+    while stack:
+        i = stack.pop()
+        order.append(i)
+        assert not empty[i, 0]
+        for k in range(4):
+            if empty[i, k]:
+                assert refs[i, k] == refs[i, 0]                           # an empty slot repeats the first ref
+                continue
+            c = refs[i, k]
+            if c >= 0:
+                assert c < nw and c > i                                   # breadth-first numbering
+                seen_node[c] += 1
+                stack.append(c)
+            else:
+                seen_leaf[~c] += 1
+    assert np.all(seen_leaf == 1) and np.all(seen_node == 1)
+    lo, hi = np.zeros((nw, 3)), np.zeros((nw, 3))
+    tol = 1e-9 * np.abs(grid[:3]).max() + 1e-12                           # the fp64 quotient of the quantisation (see k_compact_wide)
+    for i in reversed(order):
+        l, h = [], []
+        for k in range(4):
+            if empty[i, k]:
+                continue
+            c = refs[i, k]
+            el, eh = (lo[c], hi[c]) if c >= 0 else (tlo[~c], thi[~c])
+            assert np.all(blo[i, k] <= el + tol) and np.all(bhi[i, k] >= eh - tol)
+            assert np.all(el - blo[i, k] <= 1.001 * step + tol) and np.all(bhi[i, k] - eh <= 1.001 * step + tol)   # and is tight: < 1 step
+            l.append(el); h.append(eh)
+        lo[i], hi[i] = np.min(l, 0), np.max(h, 0)
+    gm.close()
+
+
 def test_mesh_create_from_device_tensors_and_errors(T):
     import torch
     m = ti.geodesic_sphere(4)
@@ -603,7 +658,7 @@ def test_exact_trace_arm_changes_nothing(T, name, idx, count):
 
 # ------------------------------------------------------------------ rare paths of tpmc_run, each forced
 def test_candidate_overflow_inside_a_run(T, O):
-    """Six coincident copies of every facet: each hit is a six-way tie, the traversal's four-slot candidate list
+    """Six coincident copies of every facet: each hit is a six-way tie, the traversal's three-slot candidate list
     overflows, the ray goes to the overflow list and the straggler kernel resolves it (A12: smallest index)."""
     cfg = ti.RunConfig("dup", lambda: ti.stacked_duplicates(6), N=200_000, seed=41, label="six coincident copies")
     g, o, frac = compare_run(T, O, cfg, 0, cfg.N, use_bvh=False)
@@ -612,8 +667,8 @@ def test_candidate_overflow_inside_a_run(T, O):
 
 
 def test_traversal_stack_overflow_inside_a_run(T, O):
-    """A hierarchy about 28 levels deep whose boxes a ray along +x all overlaps: the 24-entry shared-memory stack
-    of the wavefront traversal gives up and the straggler kernel (deep stack) takes the ray."""
+    """A hierarchy about 28 levels deep whose boxes a ray along +x all overlaps: the shared-memory stack of the wavefront
+    traversal (24 entries of the 4-wide hierarchy) gives up and the straggler kernel (deep stack) takes the ray."""
     cfg = ti.RunConfig("chain", lambda: ti.deep_chain(), V=(7500.0, 0.0, 0.0), N=100_000, seed=42, label="deep chain")
     g, o, frac = compare_run(T, O, cfg, 0, cfg.N, use_bvh=False)
     assert frac == 1.0 and g.stats["overflow_rays"] > 1000
@@ -684,7 +739,7 @@ def test_equilibrium_through_the_whole_path(T, O):
 def _arms(T):
     return [("no pre-cull", T.TPMC_FLAG_NO_PRECULL), ("no horizon", T.TPMC_FLAG_NO_HORIZON),
             ("body-frame boxes", T.TPMC_FLAG_ALIGN_OFF), ("flow-aligned boxes", T.TPMC_FLAG_ALIGN_ON),
-            ("rays sorted by key", T.TPMC_FLAG_SORT_RAYS),
+            ("rays sorted by key", T.TPMC_FLAG_SORT_RAYS), ("seed kernels behind the traversal", T.TPMC_FLAG_SERIAL_SEED),
             ("fp64 search, nothing skipped", T.TPMC_FLAG_EXACT_TRACE | T.TPMC_FLAG_NO_PRECULL | T.TPMC_FLAG_NO_HORIZON)]
 
 
