@@ -102,7 +102,10 @@ struct tpmc_mesh {
 };
 
 constexpr int kMaxTimedWaves = 1024;  // iterations covered by the per-kernel event times
-constexpr int kDrain = 3;             // trace/reflect iterations after the last wave, before the straggler kernel
+#ifndef TPMC_DRAIN
+#define TPMC_DRAIN 3
+#endif
+constexpr int kDrain = TPMC_DRAIN;    // trace/reflect iterations after the last wave, before the straggler kernel
 constexpr int kEvPerWave = 8;         // seed start/end (seed stream), iteration start, after trace, after reflect, straggler start/end (side stream), after sort
 constexpr int kCtrWords = 16;
 constexpr int kCullNodes = 64;        // 4 KB: stays in L1 next to the shared-memory carve-out

@@ -488,8 +488,11 @@ struct HorizonFacet {
 };
 
 // position bound of a box, its distance from c, and the mask of azimuth sectors it can touch
+__device__ __forceinline__ unsigned int horizon_quant(double b);
+// (min_all: the smallest of the 16 sector bounds so far -- a box that cannot raise even that one is skipped before its
+// azimuth range is worked out)
 __device__ __forceinline__ double horizon_box(const HorizonFacet& f, const float lo[3], const float hi[3], double& dist,
-                                              unsigned int& mask) {
+                                              unsigned int& mask, unsigned int min_all) {
   double h = f.delta, d2 = 0.0, w[3], r2 = 0.0;
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
@@ -504,23 +507,27 @@ __device__ __forceinline__ double horizon_box(const HorizonFacet& f, const float
   mask = 0xFFFFu;
   if (!(h > 0.0)) return -1.0;                      // below the plane; empty boxes (lo > hi) end here as well
   const double den = dist * (1.0 - 1e-12) - f.rho - f.delta;
+  const double bound = den > 0.0 ? h / den : INFINITY;
+  if (horizon_quant(bound) <= min_all) return -1.0;
   const double R = (sqrt(r2) + f.rho + f.delta) * (1.0 + 1e-9);
   const double L = sqrt(w[0] * w[0] + w[1] * w[1] + w[2] * w[2]);
   if (L > R) {
     const double x = w[0] * f.e1[0] + w[1] * f.e1[1] + w[2] * f.e1[2], y = w[0] * f.e2[0] + w[1] * f.e2[1] + w[2] * f.e2[2];
     const double st = sqrt(x * x + y * y) / L, sa = R / L;
-    if (sa < st * (1.0 - 1e-9)) {
-      const double dphi = asin(sa / st) + kHorizonAzMargin, phi = atan2(y, x);
-      if (dphi < 3.0) {
-        const double q = 16.0 / 6.283185307179586476925;
-        const int k0 = (int)floor((phi - dphi + 3.14159265358979323846) * q), k1 = (int)floor((phi + dphi + 3.14159265358979323846) * q);
+    if (sa < st * (1.0 - 1e-6)) {
+      // the two angles in fp32 (asinf, atan2f: a few ulp; the argument's rounding moves asin by at most 1e-7 / sqrt(2e-6));
+      // 2e-4 rad on top of the margin covers both
+      const float dphi = asinf(fminf((float)(sa / st), 1.0f)) + (float)kHorizonAzMargin + 2e-4f, phi = atan2f((float)y, (float)x);
+      if (dphi < 3.0f) {
+        const float q = 2.5464790894703255f;   // 16 / (2 pi)
+        const int k0 = (int)floorf((phi - dphi + 3.14159265f) * q - 1e-4f), k1 = (int)floorf((phi + dphi + 3.14159265f) * q + 1e-4f);
         unsigned int m = 0u;
         for (int k = k0; k <= k1; ++k) m |= 1u << ((k + 16) & 15);
         mask = m;
       }
     }
   }
-  return den > 0.0 ? h / den : INFINITY;
+  return bound;
 }
 
 // 16 sector bounds packed as bytes in four words
@@ -585,7 +592,7 @@ __global__ void __launch_bounds__(128) k_horizon(const float4* __restrict__ node
       bool go[2];
       for (int ch = 0; ch < 2; ++ch) {
         unsigned int mask;
-        const double bnd = horizon_box(f, lo[ch], hi[ch], dist[ch], mask);
+        const double bnd = horizon_box(f, lo[ch], hi[ch], dist[ch], mask, horizon_min(cur, 0xFFFFu));
         go[ch] = bnd > 0.0 && horizon_quant(bnd) > horizon_min(cur, mask);
         if (go[ch] && ref[ch] < 0) {        // leaf: the facet in it
           go[ch] = false;
@@ -940,18 +947,20 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
     MESH_TRY(cudaMalloc(&wcnt.p, sizeof(unsigned int) * cap_w));
     MESH_TRY(cudaMalloc(&lvl.p, sizeof(int) * 4));
     k_wide_init<<<1, 32, 0, st>>>(lvl.as<int>(), wroot.as<int>(), m->wkids_bin, m->wkids, nt == 1 ? 1 : 0);
-    if (nt > 1) {
-      const unsigned gw = (unsigned)std::min<int64_t>((cap_w + kBlock - 1) / kBlock, 592);
-      for (int L = 0; L < kWideLevels; ++L) {
-        k_wide_expand<<<gw, kBlock, 0, st>>>(m->kids, box.as<float>(), lvl.as<int>(), wroot.as<int>(), m->wkids_bin, wcnt.as<unsigned int>());
-        k_wide_scan<<<1, 1024, 0, st>>>(wcnt.as<unsigned int>(), lvl.as<int>());
-        k_wide_assign<<<gw, kBlock, 0, st>>>(lvl.as<int>(), m->wkids_bin, wcnt.as<unsigned int>(), wroot.as<int>(), m->wkids);
-        k_wide_next<<<1, 32, 0, st>>>(lvl.as<int>());
-      }
-    }
     int hl[4] = {0, 0, 0, 0};
-    MESH_TRY(cudaMemcpyAsync(hl, lvl.p, sizeof(hl), cudaMemcpyDeviceToHost, st));
-    MESH_TRY(cudaStreamSynchronize(st));
+    const unsigned gw = (unsigned)std::min<int64_t>((cap_w + kBlock - 1) / kBlock, 592);
+    for (int L = 0; L < kWideLevels; L += 8) {   // eight levels per read-back of the frontier (a 1e6-facet body has ~12)
+      if (nt > 1)
+        for (int l8 = 0; l8 < 8; ++l8) {
+          k_wide_expand<<<gw, kBlock, 0, st>>>(m->kids, box.as<float>(), lvl.as<int>(), wroot.as<int>(), m->wkids_bin, wcnt.as<unsigned int>());
+          k_wide_scan<<<1, 1024, 0, st>>>(wcnt.as<unsigned int>(), lvl.as<int>());
+          k_wide_assign<<<gw, kBlock, 0, st>>>(lvl.as<int>(), m->wkids_bin, wcnt.as<unsigned int>(), wroot.as<int>(), m->wkids);
+          k_wide_next<<<1, 32, 0, st>>>(lvl.as<int>());
+        }
+      MESH_TRY(cudaMemcpyAsync(hl, lvl.p, sizeof(hl), cudaMemcpyDeviceToHost, st));
+      MESH_TRY(cudaStreamSynchronize(st));
+      if (hl[0] == hl[1]) break;   // the frontier is empty
+    }
     if (hl[0] != hl[1] || hl[1] < 1 || hl[1] > cap_w) { tpmc_mesh_destroy(m); return TPMC_ECUDA; }   // the frontier must be empty
     m->n_wide = hl[1];
     MESH_TRY(cudaMalloc((void**)&m->wnodes, sizeof(uint4) * 4 * m->n_wide));
