@@ -18,8 +18,19 @@ _SRC = os.path.join(_HERE, "tpmc_oracle.c")
 _LIB = os.path.join(_HERE, "liboracle_tpmc.so")
 
 
+def build_sanitized(path: str) -> str:
+    """The same source with -fsanitize=address,undefined (tests/test_oracle_pins.py runs a few workloads through it)."""
+    cmd = ["gcc", "-O1", "-g", "-std=c11", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared",
+           "-fsanitize=address,undefined", "-fno-sanitize-recover=all", "-o", path, _SRC, "-lm"]
+    subprocess.run(cmd, check=True)
+    return path
+
+
 def build(force: bool = False) -> str:
-    """Compile the oracle with gcc (strict IEEE evaluation: no contraction, no fast-math)."""
+    """Compile the oracle with gcc (strict IEEE evaluation: no contraction, no fast-math).
+    TPMC_ORACLE_LIB names an already built library to load instead (the sanitizer test)."""
+    if os.environ.get("TPMC_ORACLE_LIB"):
+        return os.environ["TPMC_ORACLE_LIB"]
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared",
                "-o", _LIB, _SRC, "-lm"]

@@ -585,3 +585,44 @@ def test_p18_box_control_volume_exact_and_negative_control():
     # negative control: biased at 45 deg by several sigma, and the bias changes with the attitude
     assert abs(dev[45.0][0]) > 5 * dev[45.0][1]
     assert abs(dev[45.0][0] - dev[0.0][0]) > 4 * np.hypot(dev[45.0][1], dev[0.0][1])
+
+
+# ------------------------------------------------------------------ the oracle under AddressSanitizer + UBSan
+def test_oracle_under_address_and_undefined_behaviour_sanitizers(tmp_path):
+    """oracle/tpmc_oracle.c rebuilt with -fsanitize=address,undefined -fno-sanitize-recover=all and run, in a child
+    process with the sanitizer runtime preloaded, through every entry point on small workloads (plate, two-sided shell
+    with multiple reflections, mixture, per-facet surface arrays, both box schemes, brute force and BVH): any
+    out-of-bounds access, use after free, signed overflow, misaligned access or invalid shift aborts the child."""
+    import subprocess, sys, os, textwrap
+    import oracle as orc
+    asan = subprocess.run(["gcc", "-print-file-name=libasan.so"], capture_output=True, text=True).stdout.strip()
+    if not os.path.isabs(asan) or not os.path.exists(asan):
+        pytest.skip("no libasan in this toolchain")
+    lib = orc.build_sanitized(str(tmp_path / "liboracle_san.so"))
+    code = textwrap.dedent("""
+        import numpy as np, oracle, tpmc_inputs as ti
+        assert oracle.philox4x32_10((1, 2), (3, 4, 5, 6))
+        oracle.flux_bracket(5.0); oracle.position_inv(0.3, 7.0); oracle.vn_inv(0.9, -1.5); oracle.vn_unweighted_inv(0.2, 2.0)
+        oracle.rotation((1.0, 2.0, -3.0))
+        cases = [ti.config("C1")[0].with_(N=4000),
+                 ti.RunConfig("shell", lambda: ti.hemisphere_shell(4), N=4000, seed=3, label="shell"),
+                 ti.config("C5")[5].with_(N=3000, mesh_fn=lambda: ti.large_body(5, 6)),
+                 ti.config("C4")[3].with_(N=3000, mesh_fn=lambda: ti.satellite(4, 0.25), control_volume=1),
+                 ti.config("C2")[0].with_(N=3000, mesh_fn=lambda: ti.geodesic_sphere(3), control_volume=2, energy_accommodation=0.5)]
+        for k, cfg in enumerate(cases):
+            cfg._mesh_cache = []
+            m = cfg.mesh()
+            om = oracle.OracleMesh(m.vertices, m.indices, m.flags)
+            if k == 4:
+                om.set_surface(np.full(m.nt, 350.0), np.linspace(0.0, 1.0, m.nt))
+            a = om.run(cfg, first=0, count=cfg.N, use_bvh=True)
+            b = om.run(cfg, first=0, count=cfg.N, use_bvh=False)
+            assert a.hits == b.hits and np.array_equal(a.hash, b.hash)
+            om.seed(cfg, 0, 16)
+            del om
+        print("sanitized ok")
+    """)
+    env = dict(os.environ, LD_PRELOAD=asan, ASAN_OPTIONS="detect_leaks=0:abort_on_error=1", UBSAN_OPTIONS="halt_on_error=1:print_stacktrace=1",
+               TPMC_ORACLE_LIB=lib, PYTHONPATH=os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, env=env, timeout=600)
+    assert r.returncode == 0 and "sanitized ok" in r.stdout, r.stdout[-2000:] + r.stderr[-4000:]
