@@ -241,6 +241,9 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
 #endif
 struct TraceTune { int node_min, refill_idle; };
 constexpr int kFetchChunk = 32;   // rays a warp reserves per atomic on the queue head: one per lane (set up together, see k_trace_wf)
+constexpr int kHitBlock = 64;     // hit-list slots a warp reserves per atomic
+constexpr unsigned int kNoRay = 0xFFFFFFFFu;   // hit_ray: reserved slot without a ray
+constexpr size_t kHitSlack = (size_t)1 << 19;   // >= resident warps x kHitBlock: slots reserved but not used
 constexpr int kChunkWords = 11;   // per ray of the chunk: 1/d', the two slab offsets per axis, the octant, the queue slot
 
 __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf(const uint4* __restrict__ wnodes,
@@ -267,7 +270,7 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
   const int lane = threadIdx.x & 31, wbase = threadIdx.x & ~31;
   const unsigned FULL = 0xFFFFFFFFu;
   bool has = false, exhausted = false, fin = false;
-  unsigned int r = 0, pool_next = 0, pool_end = 0;
+  unsigned int r = 0, pool_next = 0, pool_end = 0, hpool_next = 0, hpool_end = 0;
   Walk w;
   w.cur = TPMC_SENTINEL; w.stash = 0; w.sp = 0; w.nc = 0; w.tmax = 0.0f; w.f_prev = -1;
   TraceCounters cnt;
@@ -367,15 +370,22 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
       walk_leaf(w, tris, o, d, stk, kTraceBlock, cnt);
     }
     if (has && w.cur == TPMC_SENTINEL && w.stash == 0) { has = false; fin = w.nc > 0; n_escaped += fin ? 0u : 1u; }
-    // ---- finished rays with candidates -> hit list
+    // ---- finished rays with candidates -> hit list.  A warp reserves hit-list slots kHitBlock at a time (one atomic per
+    // block instead of one per finish event of ~5 rays, and no round trip to the counter on the common path); slots it
+    // does not use are marked empty (kNoRay) and skipped by the reflect step.
     const unsigned fm = __ballot_sync(FULL, fin);
     if (fm) {
-      const int leader = __ffs(fm) - 1;
-      unsigned base = 0;
-      if (lane == leader) base = atomicAdd(n_hits, (unsigned)__popc(fm));
-      base = __shfl_sync(FULL, base, leader);
+      const unsigned nf = __popc(fm);
+      if (hpool_next + nf > hpool_end) {
+        const unsigned rest = hpool_end - hpool_next;   // < nf <= 32
+        if ((unsigned)lane < rest) __stcs(hit_ray + hpool_next + lane, kNoRay);
+        unsigned base = 0;
+        if (lane == 0) base = atomicAdd(n_hits, (unsigned)kHitBlock);
+        hpool_next = __shfl_sync(FULL, base, 0);
+        hpool_end = hpool_next + kHitBlock;
+      }
       if (fin) {
-        const unsigned h = base + __popc(fm & lanemask_lt());
+        const unsigned h = hpool_next + __popc(fm & lanemask_lt());
         __stcs(hit_ray + h, r);
         int4 cd = make_int4(-1, -1, -1, -1);
         cd.x = w.cs[0];
@@ -385,8 +395,10 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
         __stcs(hit_cand + h, (w.nc > TPMC_MAX_CAND) ? make_int4(-1, -1, -1, TPMC_CAND_OVERFLOW) : cd);
         fin = false;
       }
+      hpool_next += nf;
     }
   }
+  for (unsigned int h = hpool_next + lane; h < hpool_end; h += 32u) __stcs(hit_ray + h, kNoRay);   // the unused rest of the last block
   // counters: one atomic per warp
   unsigned long long cn = cnt.nodes, ct = cnt.tris;
 #pragma unroll
@@ -577,8 +589,8 @@ __global__ void __launch_bounds__(kTraceBlock, 6) k_reflect(const RunConst rc, u
     Particle p;
     Hit hit;
     hit.facet = -1;
-    if (h < n) {
-      r = __ldcs(hit_ray + h);
+    if (h < n) r = __ldcs(hit_ray + h);
+    if (h < n && r != kNoRay) {
       const int4 cand = __ldcs(hit_cand + h);
       if (cand.w == TPMC_CAND_OVERFLOW) {
         spill = true;
@@ -770,6 +782,7 @@ __global__ void __launch_bounds__(kTraceBlock) k_resolve_only(const float4* __re
   unsigned int nt = 0;
   for (unsigned int h = blockIdx.x * blockDim.x + threadIdx.x; h < n; h += gridDim.x * blockDim.x) {
     const unsigned int r = hit_ray[h];
+    if (r == kNoRay) continue;
     const int4 cand = hit_cand[h];
     const float4 ro = q.o[r], rv = q.v[r];
     const float of[3] = {ro.x, ro.y, ro.z}, df[3] = {rv.x, rv.y, rv.z};
@@ -994,8 +1007,8 @@ int ensure_scratch(tpmc_mesh* m, size_t wave, bool need_facets) {
         TPMC_CUDA_TRY(cudaMalloc((void**)&pp.q_key[k], 2 * wave * sizeof(unsigned int)));
       }
       TPMC_CUDA_TRY(cudaMalloc((void**)&pp.order, 2 * wave * sizeof(unsigned int)));
-      TPMC_CUDA_TRY(cudaMalloc((void**)&pp.hit_ray, 2 * wave * sizeof(unsigned int)));
-      TPMC_CUDA_TRY(cudaMalloc((void**)&pp.hit_cand, 2 * wave * sizeof(int4)));
+      TPMC_CUDA_TRY(cudaMalloc((void**)&pp.hit_ray, (2 * wave + kHitSlack) * sizeof(unsigned int)));
+      TPMC_CUDA_TRY(cudaMalloc((void**)&pp.hit_cand, (2 * wave + kHitSlack) * sizeof(int4)));
       TPMC_CUDA_TRY(cudaMalloc((void**)&pp.surv, 3 * wave * sizeof(unsigned int)));
       TPMC_CUDA_TRY(cudaMalloc((void**)&pp.ovf, 4 * wave * sizeof(unsigned int)));   // two lists (iteration parity)
     }
