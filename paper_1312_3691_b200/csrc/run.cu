@@ -1030,6 +1030,7 @@ const Grids& grids() {
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_trace_wf, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
     // resident trace CTAs per SM over all pipelines (measured: leaving room for the seed kernel does not pay)
     g.trace = sms * std::max(1, per / g.pipes);
+    g.trace = std::min<int>(g.trace, (int)(kHitSlack / ((kTraceBlock / 32) * kHitBlock)));   // every warp may leave a hit-list block partly unused
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_reflect, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
     g.reflect = sms * std::max(1, per / g.pipes);
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_finish, kTraceBlock, 0) != cudaSuccess || per < 1) per = 4;
