@@ -173,7 +173,10 @@ __device__ __forceinline__ int tri_filter(const float4 q0, const float4 q1, cons
   const float ns = det < 0.0f ? -num : num;
   const float nl = __fadd_rd(ns, -En), nh = __fadd_ru(ns, En);
   const float dl = __fadd_rd(ad, -Edet), dh = __fadd_ru(ad, Edet);
-  const float ql = __fdiv_rd(nl, nl >= 0.0f ? dh : dl), qh = __fdiv_ru(nh, nh >= 0.0f ? dl : dh);
+  // quotients by the fast division (2 ulp for a denominator in [2^-126, 2^126], here |det| of metres x m/s), pushed
+  // outwards by 4 ulp and a denormal's worth: still directed bounds, at a fifth of the instructions of __fdiv_rd/ru
+  const float qa = __fdividef(nl, nl >= 0.0f ? dh : dl), qb = __fdividef(nh, nh >= 0.0f ? dl : dh);
+  const float ql = fmaf(-2.4e-7f, fabsf(qa), qa) - 1e-37f, qh = fmaf(2.4e-7f, fabsf(qb), qb) + 1e-37f;
   const float tl = __fadd_rd(t0, ql), th = __fadd_ru(t0, qh);
   if (th < 0.0f) return TRI_MISS;                 // provably behind the origin
   tlo = fmaxf(tl, 0.0f);
