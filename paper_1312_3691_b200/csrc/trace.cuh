@@ -361,31 +361,24 @@ __device__ __forceinline__ void walk_abort(Walk& w) {
   w.sp = 0;
 }
 
+// Candidate list: up to TPMC_MAX_CAND live entries in any of the slots (cs[k] < 0: free), w.nc of them; a provable hit
+// that shrinks tmax frees the entries that start beyond it.  (Kept short: this runs with the few lanes whose facet was
+// not a miss, and every instruction there costs the warp a full issue slot.)
 __device__ __forceinline__ void walk_add_candidate(Walk& w, int slot, int cls, float tlo, float thi) {
   if (cls == TRI_HIT && thi < w.tmax) {
     w.tmax = thi;
-    // drop candidates that can no longer be the closest
-    int n = 0;
+    if (w.nc <= TPMC_MAX_CAND) {   // (an overflowed list stays overflowed)
 #pragma unroll
-    for (int k = 0; k < TPMC_MAX_CAND; ++k) {
-      const bool keep = (w.cs[k] >= 0) && (w.cl[k] <= w.tmax);
-      const int s = w.cs[k];
-      const float l = w.cl[k];
-      w.cs[k] = -1;
-      if (keep) {
-#pragma unroll
-        for (int j = 0; j < TPMC_MAX_CAND; ++j)
-          if (j == n) { w.cs[j] = s; w.cl[j] = l; }
-        ++n;
-      }
+      for (int k = 0; k < TPMC_MAX_CAND; ++k)
+        if (w.cs[k] >= 0 && w.cl[k] > thi) { w.cs[k] = -1; --w.nc; }
     }
-    if (w.nc <= TPMC_MAX_CAND) w.nc = n;
   }
   if (tlo > w.tmax) return;
   if (w.nc >= TPMC_MAX_CAND) { w.nc = TPMC_MAX_CAND + 1; return; }
+  bool placed = false;
 #pragma unroll
-  for (int j = 0; j < TPMC_MAX_CAND; ++j)
-    if (j == w.nc) { w.cs[j] = slot; w.cl[j] = tlo; }
+  for (int k = 0; k < TPMC_MAX_CAND; ++k)
+    if (!placed && w.cs[k] < 0) { w.cs[k] = slot; w.cl[k] = tlo; placed = true; }
   ++w.nc;
 }
 
