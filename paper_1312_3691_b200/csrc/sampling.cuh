@@ -311,6 +311,10 @@ struct SeedConstF {
 };
 
 __device__ __forceinline__ float u01f(uint32_t w) { return ((float)w + 0.5f) * 2.3283064365386963e-10f; }
+// square root and reciprocal to ~2 ulp without the range checks and fix-up steps of sqrtf / __frcp_rn (one MUFU + one
+// multiply): the estimate's own error budget is 1e-4 and its margin 2e-2 R_b.  sqrt_fast(0) = 0; arguments are >= 0.
+__device__ __forceinline__ float sqrt_fast(float x) { return x * rsqrtf(fmaxf(x, 1e-36f)); }
+__device__ __forceinline__ float rcp_fast(float x) { return __fdividef(1.0f, x); }
 
 // erfc(x) with fractional error ~2e-7 in ~20 instructions (the library erfcf costs ~45): the classical
 // Chebyshev fit erfc(z) = t exp(-z^2 + P(t)), t = 1/(1 + z/2), z >= 0 (Numerical Recipes' erfcc coefficients),
@@ -349,7 +353,7 @@ __device__ __forceinline__ float approx_y(float u, const SpeciesF& sc, bool& ok)
   pl = fmaf(pl, L, 7.322245522e-02f);
   pl = fmaf(pl, L, 5.387478773e-01f);
   pl = fmaf(pl, L, 3.962664050e-01f);
-  float y = (T >= 5.0f) ? sqrtf(fmaf(T, 1.0f / TPMC_SQRTPI_F, -0.5f)) : pl;
+  float y = (T >= 5.0f) ? sqrt_fast(fmaf(T, 1.0f / TPMC_SQRTPI_F, -0.5f)) : pl;
   y = fminf(S, fmaxf(-S, y));
   float step = 1.0f;
 #pragma unroll
@@ -370,11 +374,11 @@ __device__ __forceinline__ float approx_y(float u, const SpeciesF& sc, bool& ok)
 // x_n = v_n / c_mp to ~1e-4 relative, ok = certified.  omu = 1 - u
 __device__ __forceinline__ float approx_normal_speed(float omu, float s, float chis, bool& ok) {
   const float T = omu * chis;
-  const float xm = 0.5f * (s + sqrtf(fmaf(s, s, 2.0f)));
+  const float xm = 0.5f * (s + sqrt_fast(fmaf(s, s, 2.0f)));
   const float tau = fminf(fmaxf(__fdividef(T, TPMC_SQRTPI_F * s), 1e-30f), 1.9999f);
   const float xa = s + erfcinvf(tau) + __fdividef(0.5f, s);
   float x = (s >= 1.0f) ? xa : xm;
-  const float xs = sqrtf(fmaxf(chis - T, 0.0f)) * __expf(0.5f * s * s);   // chis - T = u chi(s)
+  const float xs = sqrt_fast(fmaxf(chis - T, 0.0f)) * __expf(0.5f * s * s);   // chis - T = u chi(s)
   x = (xs < 0.25f * xm || !(x > 0.0f)) ? fminf(xm, 2.0f * xs) : x;
   float step = 1.0f, q = 0.0f, e = 0.0f;
 #pragma unroll
@@ -418,9 +422,9 @@ __device__ __forceinline__ bool precull_stage_a(const SeedConstF& sf, unsigned i
     if ((unsigned long long)b0.x >= sf.sp[s - 1].thr) sc = sf.sp[s];   // cumx is non-decreasing: the last hit wins
   a.y = approx_y(u01f(b0.y), sc, a.ok_t);
   a.t = fminf(1.0f, fmaxf(-1.0f, __fdividef(a.y, sc.S)));
-  a.cphi = sqrtf(fmaxf((1.0f - a.t) * (1.0f + a.t), 0.0f));
+  a.cphi = sqrt_fast(fmaxf((1.0f - a.t) * (1.0f + a.t), 0.0f));
   a.w2 = b0.z;
-  const float rho = sqrtf(-__logf(u01f(b1.x)));
+  const float rho = sqrt_fast(-__logf(u01f(b1.x)));
   float sa, ca;
   sincospif(2.0f * u01f(b1.y), &sa, &ca);
   a.xt1 = fmaf(sc.S, a.cphi, rho * ca);
@@ -428,7 +432,7 @@ __device__ __forceinline__ bool precull_stage_a(const SeedConstF& sf, unsigned i
   a.s = sc.S * a.t;
   a.w3 = b0.w;
   // threshold on the normal speed for the grown bounding sphere
-  const float xr = sf.cot_g * sqrtf(fmaf(a.xt1, a.xt1, a.xt2 * a.xt2));
+  const float xr = sf.cot_g * sqrt_fast(fmaf(a.xt1, a.xt1, a.xt2 * a.xt2));
   const float s = a.s, z = xr - s;
   const float e = __expf(-z * z);
   const float q = fmaf(TPMC_SQRTPI_F * s, erfc_fast(z), e);                        // Q(x_req)
@@ -480,7 +484,7 @@ __device__ __forceinline__ bool precull_touch(const SeedConstF& sf, const float 
   // (a direction component below 1e-30 is replaced by 1e-30: no inf - inf; the ray stays parallel to the slab)
   const float vs[3] = {fabsf(v[0]) < 1e-30f ? 1e-30f : v[0], fabsf(v[1]) < 1e-30f ? 1e-30f : v[1],
                        fabsf(v[2]) < 1e-30f ? 1e-30f : v[2]};
-  const float id[3] = {__frcp_rn(vs[0]), __frcp_rn(vs[1]), __frcp_rn(vs[2])};
+  const float id[3] = {rcp_fast(vs[0]), rcp_fast(vs[1]), rcp_fast(vs[2])};
   const float oi[3] = {-o[0] * id[0], -o[1] * id[1], -o[2] * id[2]};
   float ax[3], bx[3];
 #pragma unroll
