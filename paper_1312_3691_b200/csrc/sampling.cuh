@@ -315,6 +315,13 @@ __device__ __forceinline__ float u01f(uint32_t w) { return ((float)w + 0.5f) * 2
 // multiply): the estimate's own error budget is 1e-4 and its margin 2e-2 R_b.  sqrt_fast(0) = 0; arguments are >= 0.
 __device__ __forceinline__ float sqrt_fast(float x) { return x * rsqrtf(fmaxf(x, 1e-36f)); }
 __device__ __forceinline__ float rcp_fast(float x) { return __fdividef(1.0f, x); }
+// sin and cos of 2 pi u, u in (0, 1), by the hardware approximations on an argument folded into [-pi, pi) (absolute
+// error ~5e-7: as good as the estimate needs; sincospif costs six times as many instructions)
+__device__ __forceinline__ void sincos_2pi_fast(float u, float& s, float& c) {
+  const float x = 6.2831853071795865f * (u - (u >= 0.5f ? 1.0f : 0.0f));
+  s = __sinf(x);
+  c = __cosf(x);
+}
 
 // erfc(x) with fractional error ~2e-7 in ~20 instructions (the library erfcf costs ~45): the classical
 // Chebyshev fit erfc(z) = t exp(-z^2 + P(t)), t = 1/(1 + z/2), z >= 0 (Numerical Recipes' erfcc coefficients),
@@ -426,7 +433,7 @@ __device__ __forceinline__ bool precull_stage_a(const SeedConstF& sf, unsigned i
   a.w2 = b0.z;
   const float rho = sqrt_fast(-__logf(u01f(b1.x)));
   float sa, ca;
-  sincospif(2.0f * u01f(b1.y), &sa, &ca);
+  sincos_2pi_fast(u01f(b1.y), sa, ca);
   a.xt1 = fmaf(sc.S, a.cphi, rho * ca);
   a.xt2 = rho * sa;
   a.s = sc.S * a.t;
@@ -451,7 +458,7 @@ __device__ __forceinline__ bool precull_stage_b(const SeedConstF& sf, const Prec
   bool ok_x;
   const float xn = approx_normal_speed(u01f(~a.w3), a.s, a.chis, ok_x);
   float st, ct;
-  sincospif(2.0f * u01f(a.w2), &st, &ct);
+  sincos_2pi_fast(u01f(a.w2), st, ct);
   const float xh[3] = {a.cphi * ct, a.cphi * st, a.t};
   const float t1[3] = {a.t * ct, a.t * st, -a.cphi};
   const float t2[3] = {-st, ct, 0.0f};
