@@ -118,6 +118,11 @@ __device__ __forceinline__ bool facet_test(const float4 q0, const float4 q1, con
 // roundings.  Magnitudes in this application (metres, m/s) are far from the fp32 under/overflow range; a NaN (zero
 // direction) fails every comparison and ends as UNCERTAIN.
 enum { TRI_MISS = 0, TRI_HIT = 1, TRI_UNCERTAIN = 2 };
+__device__ __forceinline__ float rcp_approx(float x) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
 
 __device__ __forceinline__ void triple_f32(const float d[3], const float x[3], const float y[3], float& w, float& M) {
   const float p0 = x[1] * y[2], p1 = x[2] * y[1];
@@ -140,7 +145,7 @@ __device__ __forceinline__ int tri_filter(const float4 q0, const float4 q1, cons
   if (!two_sided && det > Edet) return TRI_MISS;  // provably back-facing
   // origin moved next to the facet
   const float dd = fmaf(d[2], d[2], fmaf(d[1], d[1], d[0] * d[0]));
-  const float t0 = __fdividef(fmaf(q0.z - o[2], d[2], fmaf(q0.y - o[1], d[1], (q0.x - o[0]) * d[0])), dd);
+  const float t0 = fmaf(q0.z - o[2], d[2], fmaf(q0.y - o[1], d[1], (q0.x - o[0]) * d[0])) * rcp_approx(dd);   // (any t0 is valid)
   const float os[3] = {fmaf(t0, d[0], o[0]), fmaf(t0, d[1], o[1]), fmaf(t0, d[2], o[2])};
   const float a[3] = {q0.x - os[0], q0.y - os[1], q0.z - os[2]};
   const float b[3] = {q1.x - os[0], q1.y - os[1], q1.z - os[2]};
@@ -173,9 +178,10 @@ __device__ __forceinline__ int tri_filter(const float4 q0, const float4 q1, cons
   const float ns = det < 0.0f ? -num : num;
   const float nl = __fadd_rd(ns, -En), nh = __fadd_ru(ns, En);
   const float dl = __fadd_rd(ad, -Edet), dh = __fadd_ru(ad, Edet);
-  // quotients by the fast division (2 ulp for a denominator in [2^-126, 2^126], here |det| of metres x m/s), pushed
-  // outwards by 4 ulp and a denormal's worth: still directed bounds, at a fifth of the instructions of __fdiv_rd/ru
-  const float qa = __fdividef(nl, nl >= 0.0f ? dh : dl), qb = __fdividef(nh, nh >= 0.0f ? dl : dh);
+  // quotients as numerator x approximate reciprocal (1 ulp + the product's rounding; a denormal denominator flushes to an
+  // infinite or NaN quotient, which never shrinks tmax), pushed outwards by 4 ulp and a denormal's worth: still directed
+  // bounds, at a tenth of the instructions of __fdiv_rd/ru
+  const float qa = nl * rcp_approx(nl >= 0.0f ? dh : dl), qb = nh * rcp_approx(nh >= 0.0f ? dl : dh);
   const float ql = fmaf(-2.4e-7f, fabsf(qa), qa) - 1e-37f, qh = fmaf(2.4e-7f, fabsf(qb), qb) + 1e-37f;
   const float tl = __fadd_rd(t0, ql), th = __fadd_ru(t0, qh);
   if (th < 0.0f) return TRI_MISS;                 // provably behind the origin
