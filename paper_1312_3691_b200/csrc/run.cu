@@ -240,6 +240,10 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
 #define TPMC_SRAY 1
 #endif
 struct TraceTune { int node_min, refill_idle; };
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  const unsigned int sa = (unsigned int)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gmem) : "memory");
+}
 constexpr int kFetchChunk = 32;   // rays a warp reserves per atomic on the queue head: one per lane (set up together, see k_trace_wf)
 constexpr int kHitBlock = 64;     // hit-list slots a warp reserves per atomic
 constexpr unsigned int kNoRay = 0xFFFFFFFFu;   // hit_ray: reserved slot without a ray
@@ -261,7 +265,7 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
   __shared__ int sstack[(TPMC_STACK_SMEM + 6) * kTraceBlock];      // two guard rows, TPMC_STACK_SMEM rows, four of headroom
   __shared__ unsigned int schunk[kChunkWords][kTraceBlock];        // the warp's current chunk of rays, set up for the walk
 #if TPMC_SRAY
-  __shared__ float sray[6][kTraceBlock];                           // the lane's ray (o, d) for the leaf phases
+  __shared__ float4 sray[2][kTraceBlock];                          // the lane's ray (o | index, d | species) for the leaf phases
 #endif
   int* stk = sstack + 2 * kTraceBlock + threadIdx.x;   // level 0; levels -1, -2 are the guard entries (walk_pop)
   stk[-kTraceBlock] = TPMC_SENTINEL;
@@ -331,9 +335,10 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
           r = c[10 * kTraceBlock];
           walk_reset(w, __ldcs(q.f + r));
 #if TPMC_SRAY
-          const float4 ro = __ldcs(q.o + r), rv = __ldcs(q.v + r);   // (just read by the lane that set the ray up: cache-resident)
-          sray[0][threadIdx.x] = ro.x; sray[1][threadIdx.x] = ro.y; sray[2][threadIdx.x] = ro.z;
-          sray[3][threadIdx.x] = rv.x; sray[4][threadIdx.x] = rv.y; sray[5][threadIdx.x] = rv.z;
+          // asynchronous copies global -> shared (the records were just read by the lane that set the ray up): the lane
+          // does not wait for them here; the first leaf phase does (cp.async.wait_all), long after they have landed
+          cp_async16(&sray[0][threadIdx.x], q.o + r);
+          cp_async16(&sray[1][threadIdx.x], q.v + r);
 #endif
           has = true;
         }
@@ -361,8 +366,9 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
     if (has && w.stash != 0) {
 #if TPMC_SRAY
       // the ray lives in shared memory: six registers stay free during the node phase
-      const float o[3] = {sray[0][threadIdx.x], sray[1][threadIdx.x], sray[2][threadIdx.x]};
-      const float d[3] = {sray[3][threadIdx.x], sray[4][threadIdx.x], sray[5][threadIdx.x]};
+      asm volatile("cp.async.wait_all;" ::: "memory");
+      const float4 ro = sray[0][threadIdx.x], rv = sray[1][threadIdx.x];
+      const float o[3] = {ro.x, ro.y, ro.z}, d[3] = {rv.x, rv.y, rv.z};
 #else
       const float4 ro = q.o[r], rv = q.v[r];   // re-read (cache-resident): keeps six registers free during the node phase
       const float o[3] = {ro.x, ro.y, ro.z}, d[3] = {rv.x, rv.y, rv.z};
