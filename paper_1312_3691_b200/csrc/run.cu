@@ -225,7 +225,7 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
 //    (one warp-aggregated atomic), so rays of very different length do not idle the warp.
 // Rays that end with at least one candidate facet are appended to the hit list for k_reflect.
 #ifndef TPMC_NODE_MIN
-#define TPMC_NODE_MIN 16
+#define TPMC_NODE_MIN 20
 #endif
 #ifndef TPMC_REFILL_IDLE
 #define TPMC_REFILL_IDLE 4
@@ -234,7 +234,7 @@ __global__ void __launch_bounds__(kSeedBlock) k_seed(const RunConst rc, unsigned
 #define TPMC_TRACE_MIN_BLOCKS 7   // 72 registers: the wide node step spills at 64 (measured: 7 x 72 is 1.6 % faster than 8 x 64)
 #endif
 #ifndef TPMC_NODE_STEPS
-#define TPMC_NODE_STEPS 1   // wide-node steps per warp vote
+#define TPMC_NODE_STEPS 2   // wide-node steps per warp vote (a loop over one copy of the step: the votes are 8 % of the issue slots at 1)
 #endif
 #ifndef TPMC_SRAY
 #define TPMC_SRAY 1
@@ -355,12 +355,13 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
         const unsigned ml = __ballot_sync(FULL, has && w.stash != 0);
         if (mn == 0u || ml != 0u) break;
       }
-      if (at_node) {
-        walk_node(w, wnodes, stk, kTraceBlock, cnt);
 #if TPMC_NODE_STEPS > 1
-        if ((unsigned)w.cur < (unsigned)TPMC_SENTINEL) walk_node(w, wnodes, stk, kTraceBlock, cnt);
+#pragma unroll 1
+      for (int rep = 0; rep < TPMC_NODE_STEPS; ++rep)   // (one copy of the step's code: unrolled, it spills)
+        if (has && (unsigned)w.cur < (unsigned)TPMC_SENTINEL) walk_node(w, wnodes, stk, kTraceBlock, cnt);
+#else
+      if (at_node) walk_node(w, wnodes, stk, kTraceBlock, cnt);
 #endif
-      }
     }
     // ---- leaf phase: every lane that put a leaf aside classifies it
     if (has && w.stash != 0) {
