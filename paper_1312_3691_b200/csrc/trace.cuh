@@ -450,10 +450,11 @@ __device__ __forceinline__ void walk_node(Walk& w, const uint4* __restrict__ wno
 __device__ __forceinline__ void walk_leaf(Walk& w, const float4* __restrict__ tris, const float o[3], const float d[3],
                                           int* stk, int sstride, TraceCounters& cnt) {
   const int slot = ~w.stash;
+  // all three loads at once (the source facet is rare: waiting for q0 before asking for q1, q2 cost a second round trip)
   const float4 q0 = __ldg(tris + 3 * (size_t)slot + 0);
+  const float4 q1 = __ldg(tris + 3 * (size_t)slot + 1);
+  const float4 q2 = __ldg(tris + 3 * (size_t)slot + 2);
   if (__float_as_int(q0.w) != w.f_prev) {
-    const float4 q1 = __ldg(tris + 3 * (size_t)slot + 1);
-    const float4 q2 = __ldg(tris + 3 * (size_t)slot + 2);
     ++cnt.tris;
     float tlo, thi;
     const int cls = tri_filter(q0, q1, q2, o, d, tlo, thi);
