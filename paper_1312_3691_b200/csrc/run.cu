@@ -567,12 +567,15 @@ __device__ __forceinline__ void accumulate_warp(double* __restrict__ P, bool is_
   }
 }
 
+#ifndef TPMC_REFLECT_MIN_BLOCKS
+#define TPMC_REFLECT_MIN_BLOCKS 6
+#endif
 // a4-a6: resolve the candidates of every hit ray with the exact fp64 test, apply the surface interaction,
 // accumulate, and queue the reflected ray for the next wavefront round (compacted, warp-aggregated).
 // Rays the traversal gave up on (too many candidates, stack too deep) and rays whose reflected successor
 // finds region A of the next queue full go, untouched, to the overflow list: k_finish follows them to escape
 // with the full fp64 traversal, densely, instead of one lane doing so here while its warp waits.
-__global__ void __launch_bounds__(kTraceBlock, 6) k_reflect(const RunConst rc, unsigned int cap,
+__global__ void __launch_bounds__(kTraceBlock, TPMC_REFLECT_MIN_BLOCKS) k_reflect(const RunConst rc, unsigned int cap,
                                                          const float4* __restrict__ tris, const RayQueue qin,
                                                          const unsigned int* __restrict__ hit_ray,
                                                          const int4* __restrict__ hit_cand,
