@@ -337,6 +337,7 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
 #if TPMC_SRAY
           // asynchronous copies global -> shared (the records were just read by the lane that set the ray up): the lane
           // does not wait for them here; the first leaf phase does (cp.async.wait_all), long after they have landed
+          asm volatile("cp.async.wait_all;" ::: "memory");   // (a previous ray's copy that was never waited for must not land after this one)
           cp_async16(&sray[0][threadIdx.x], q.o + r);
           cp_async16(&sray[1][threadIdx.x], q.v + r);
 #endif
