@@ -255,6 +255,11 @@ def test_mesh_create_from_device_tensors_and_errors(T):
         else:
             with pytest.raises(T.TpmcError):
                 a.run(c)
+    good = ti.config("C2")[0].with_(N=1000)
+    for flags in (0x100, T.TPMC_FLAG_ALIGN_OFF | T.TPMC_FLAG_ALIGN_ON):      # unknown bit; contradictory pair
+        with pytest.raises(T.TpmcError):
+            a.run(good, flags=flags)
+    a.run(good, flags=T.TPMC_FLAG_SERIAL_SEED | T.TPMC_FLAG_NO_AGGREGATION)  # every defined bit is accepted
 
 
 # ------------------------------------------------------------------ a3: closest hit, bit-exact
