@@ -31,6 +31,7 @@ extern "C" {
 #define TPMC_EINVAL (-1) /* bad argument / degenerate mesh / bad parameter */
 #define TPMC_ENOMEM (-2) /* host or device allocation failed */
 #define TPMC_ECUDA (-3)  /* a CUDA call failed; see tpmc_last_cuda_error() */
+#define TPMC_ECAPACITY (-4) /* input larger than a fixed-capacity entry point takes; tpmc_last_cuda_error() has the numbers */
 
 #define TPMC_MEM_HOST 0
 #define TPMC_MEM_DEVICE 1
@@ -239,6 +240,32 @@ typedef struct {
   double red_f64_addresses[3];      /* ... over this many accumulators */
 } tpmc_peaks;
 int tpmc_measure_peaks(tpmc_peaks* out, void* cuda_stream);
+
+/* F = sum over facets of the per-facet momentum-transfer rate (the last step of tpmc_run), as a
+ * call of its own that ALLOCATES NOTHING.  It is meant for callers that must not, or cannot, obtain device memory at the
+ * time of the call: a program that gave all of the GPU's memory to its own pool (a cudaMalloc from inside a library would
+ * fail or break its budget), a loop with a deadline (cudaMalloc and cudaFree take driver locks and may wait for the
+ * device to drain), code running while another thread holds a global-mode stream capture open (the runtime refuses
+ * cudaMalloc then).  Such a caller sums a facet-momentum array it already holds -- one written by tpmc_run, or the sum
+ * of several slices -- without libtpmc touching an allocator: no cudaMalloc, cudaFree or allocating library routine is
+ * called, on any path.
+ *   d_facet_momentum  device [nt][3] fp64, read only (may be NULL when nt == 0)
+ *   nt                0 .. TPMC_STATIC_MAX_FACETS; more returns TPMC_ECAPACITY and enqueues nothing (the call does not
+ *                     split or fall back to allocating)
+ *   d_force           device [3], overwritten (zeros for nt == 0); valid once `cuda_stream` has been synchronised
+ * The partial sums live in a fixed array inside the library image (49 408 bytes; every GPU that loads libtpmc.so holds
+ * its copy until the process exits).  Consequences the caller must know:
+ *   - one array per GPU, shared by all calls, threads and streams: two calls that may overlap on the same GPU race on
+ *     it and give wrong sums.  Order them on one stream or with events.  Calls on different GPUs are independent.
+ *   - the array keeps what the previous call left; the call clears the one word that has to start at zero itself
+ *     (a 4-byte cudaMemsetAsync on `cuda_stream` ahead of the kernel), so nothing needs resetting between calls.
+ *   - the first call on each GPU looks up that GPU's address of the array (cudaGetSymbolAddress, with the caller's
+ *     current device; this can make the runtime load the library's device code).  Make that first call during set-up,
+ *     with the right device current and before any stream capture begins; later calls on that GPU only enqueue.
+ * The result depends on (d_facet_momentum, nt) only: a fixed tree of 4096-facet parts.  Its summation order differs from
+ * tpmc_run's, so the two agree to rounding (a few ulp of sum |P_f|), not bit for bit. */
+#define TPMC_STATIC_MAX_FACETS 8388608LL
+int tpmc_facet_sum_static(const double* d_facet_momentum, int64_t nt, void* cuda_stream, double* d_force);
 
 const char* tpmc_strerror(int code);
 const char* tpmc_last_cuda_error(void);

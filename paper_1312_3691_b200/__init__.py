@@ -17,7 +17,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libtpmc.so")
 
-TPMC_OK, TPMC_EINVAL, TPMC_ENOMEM, TPMC_ECUDA = 0, -1, -2, -3
+TPMC_OK, TPMC_EINVAL, TPMC_ENOMEM, TPMC_ECUDA, TPMC_ECAPACITY = 0, -1, -2, -3, -4
+TPMC_STATIC_MAX_FACETS = 8388608
 TPMC_MEM_HOST, TPMC_MEM_DEVICE = 0, 1
 TPMC_MAX_SPECIES = 8
 TPMC_MAX_BOUNCES = 0x0FFFFFFF
@@ -27,7 +28,7 @@ TPMC_CV_SPHERE, TPMC_CV_BOX, TPMC_CV_BOX_UNWEIGHTED = 0, 1, 2
 
 EXPORTS = ["tpmc_mesh_create", "tpmc_mesh_destroy", "tpmc_mesh_info", "tpmc_mesh_copy_bvh", "tpmc_run",
            "tpmc_mesh_copy_horizon", "tpmc_run_host", "tpmc_seed", "tpmc_trace", "tpmc_strerror", "tpmc_last_cuda_error", "tpmc_version",
-           "tpmc_measure_peaks", "tpmc_mesh_set_surface", "tpmc_run_sweep", "tpmc_mesh_copy_wide"]
+           "tpmc_measure_peaks", "tpmc_mesh_set_surface", "tpmc_run_sweep", "tpmc_mesh_copy_wide", "tpmc_facet_sum_static"]
 
 
 class TpmcError(RuntimeError):
@@ -110,6 +111,8 @@ def lib():
         L.tpmc_seed.argtypes = [vp, C.POINTER(tpmc_params), vp, vp, vp, vp]
         L.tpmc_trace.restype = C.c_int
         L.tpmc_trace.argtypes = [vp, vp, vp, vp, C.c_int64, vp, vp, vp, vp]
+        L.tpmc_facet_sum_static.restype = C.c_int
+        L.tpmc_facet_sum_static.argtypes = [vp, C.c_int64, vp, vp]
         L.tpmc_measure_peaks.restype = C.c_int
         L.tpmc_measure_peaks.argtypes = [C.POINTER(tpmc_peaks), vp]
         for n in ("tpmc_strerror", "tpmc_last_cuda_error", "tpmc_version"):
@@ -123,7 +126,7 @@ def _check(rc: int, what: str):
     if rc != TPMC_OK:
         L = lib()
         msg = L.tpmc_strerror(rc).decode()
-        if rc == TPMC_ECUDA:
+        if rc in (TPMC_ECUDA, TPMC_ECAPACITY):
             msg += ": " + L.tpmc_last_cuda_error().decode()
         raise TpmcError(f"{what} failed ({rc}): {msg}")
 
@@ -393,6 +396,25 @@ def tpmc_seed(mesh: Mesh, cfg, **kw):
 
 def tpmc_trace(mesh: Mesh, o, d, f_prev=None, **kw):
     return mesh.trace(o, d, f_prev, **kw)
+
+
+def tpmc_facet_sum_static(facet_momentum, out=None, stream=None):
+    """Sum a device [nt,3] float64 facet-momentum tensor into a device [3] force with tpmc_facet_sum_static, the entry
+    point that allocates no device memory (its scratch is a fixed array inside libtpmc.so; see include/tpmc.h for who
+    needs that and what it costs: at most TPMC_STATIC_MAX_FACETS facets, one call at a time per GPU).  Pass `out` (device
+    [3] float64) to keep this wrapper from allocating the result too; without it a torch tensor is made for convenience."""
+    torch = _torch()
+    fm = facet_momentum
+    if not (fm.is_cuda and fm.dtype == torch.float64 and fm.is_contiguous() and fm.dim() == 2 and fm.shape[1] == 3):
+        raise TpmcError("facet_momentum must be a contiguous CUDA float64 tensor [nt, 3]")
+    if out is None:
+        out = torch.empty(3, dtype=torch.float64, device=fm.device)
+    elif not (out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == 3):
+        raise TpmcError("out must be a contiguous CUDA float64 tensor of 3 elements")
+    with torch.cuda.device(fm.device):
+        _check(lib().tpmc_facet_sum_static(fm.data_ptr() or None, int(fm.shape[0]), _stream_ptr(stream), out.data_ptr()),
+               "tpmc_facet_sum_static")
+    return out
 
 
 def tpmc_measure_peaks(stream=None) -> dict:

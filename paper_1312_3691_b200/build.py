@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtpmc.so")
-SOURCES = ["lbvh.cu", "run.cu", "peaks.cu"]
+SOURCES = ["lbvh.cu", "run.cu", "peaks.cu", "facet_sum_static.cu"]
 HEADERS = ["common.cuh", "radix.cuh", "sampling.cuh", "sort.cuh", "trace.cuh", os.path.join("..", "..", "include", "tpmc.h")]
 
 

@@ -1141,6 +1141,7 @@ extern "C" const char* tpmc_strerror(int code) {
     case TPMC_EINVAL: return "invalid argument";
     case TPMC_ENOMEM: return "out of memory";
     case TPMC_ECUDA: return "CUDA error";
+    case TPMC_ECAPACITY: return "input exceeds the fixed capacity of this entry point";
     default: return "unknown error";
   }
 }
