@@ -379,21 +379,23 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
     }
     if (has && w.cur == TPMC_SENTINEL && w.stash == 0) { has = false; fin = w.nc > 0; n_escaped += fin ? 0u : 1u; }
     // ---- finished rays with candidates -> hit list.  A warp reserves hit-list slots kHitBlock at a time (one atomic per
-    // block instead of one per finish event of ~5 rays, and no round trip to the counter on the common path); slots it
-    // does not use are marked empty (kNoRay) and skipped by the reflect step.
+    // block instead of one per finish event of ~5 rays, and no round trip to the counter on the common path).  Finishing
+    // lanes that do not fit the rest of the warp's block fill that rest first and go on in a fresh block, so every slot
+    // of every block but a warp's last is used: slots handed out <= hits + warps * kHitBlock <= 2 * wave_cap + kHitSlack,
+    // the size of hit_ray / hit_cand (ensure_scratch; the grid is clamped so that warps * kHitBlock <= kHitSlack).
+    // The unused tail of a warp's last block is marked empty (kNoRay) and skipped by the reflect step.
     const unsigned fm = __ballot_sync(FULL, fin);
     if (fm) {
-      const unsigned nf = __popc(fm);
-      if (hpool_next + nf > hpool_end) {
-        const unsigned rest = hpool_end - hpool_next;   // < nf <= 32
-        if ((unsigned)lane < rest) __stcs(hit_ray + hpool_next + lane, kNoRay);
+      const unsigned nf = __popc(fm), rest = hpool_end - hpool_next;   // nf <= 32 < kHitBlock
+      unsigned nbase = hpool_next;
+      if (nf > rest) {
         unsigned base = 0;
         if (lane == 0) base = atomicAdd(n_hits, (unsigned)kHitBlock);
-        hpool_next = __shfl_sync(FULL, base, 0);
-        hpool_end = hpool_next + kHitBlock;
+        nbase = __shfl_sync(FULL, base, 0) - rest;   // slot of rank k >= rest: (new block) + k - rest
       }
       if (fin) {
-        const unsigned h = hpool_next + __popc(fm & lanemask_lt());
+        const unsigned rk = __popc(fm & lanemask_lt());
+        const unsigned h = (rk < rest ? hpool_next : nbase) + rk;
         __stcs(hit_ray + h, r);
         int4 cd = make_int4(-1, -1, -1, -1);
         cd.x = w.cs[0];
@@ -403,7 +405,8 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_TRACE_MIN_BLOCKS) k_trace_wf
         __stcs(hit_cand + h, (w.nc > TPMC_MAX_CAND) ? make_int4(-1, -1, -1, TPMC_CAND_OVERFLOW) : cd);
         fin = false;
       }
-      hpool_next += nf;
+      if (nf > rest) { hpool_next = nbase + nf; hpool_end = nbase + rest + kHitBlock; }
+      else hpool_next += nf;
     }
   }
   for (unsigned int h = hpool_next + lane; h < hpool_end; h += 32u) __stcs(hit_ray + h, kNoRay);   // the unused rest of the last block

@@ -332,6 +332,37 @@ def test_trace_tie_and_sidedness_rules(T):
     assert f.cpu().numpy().tolist() == [0, -1, -1] and tau.cpu().numpy()[0] == 1.0
 
 
+def test_trace_every_ray_hits_with_the_queue_filled_to_capacity(T, O):
+    """The hit list holds one entry per ray that ends with a candidate facet and is sized from the queue capacity plus a
+    fixed slack (run.cu: ensure_scratch, kHitSlack).  Worst case for it: a queue filled to the last slot (tpmc_trace on a
+    fresh handle sizes the queue to exactly n rays) in which EVERY ray hits, at a size where any slot a warp reserved
+    and then left unused would add up to more than the slack (2^25 rays against 2^19 slots of slack)."""
+    import torch
+    m = ti.geodesic_sphere(32)
+    gm = T.Mesh(m.vertices, m.indices, m.flags)
+    om = O.OracleMesh(m.vertices, m.indices, m.flags)
+    n = 1 << 25
+    g = torch.Generator(device="cuda").manual_seed(11)
+    u = torch.randn((n, 3), generator=g, device="cuda", dtype=torch.float32)
+    o = 3.0 * u / u.norm(dim=1, keepdim=True)
+    t = torch.randn((n, 3), generator=g, device="cuda", dtype=torch.float32)
+    t = 0.9 * t / t.norm(dim=1, keepdim=True) * torch.rand((n, 1), generator=g, device="cuda") ** (1.0 / 3.0)
+    d = t - o                                                            # aimed at a point well inside the body
+    facet, tau = gm.trace(o, d)
+    assert int((facet < 0).sum()) == 0 and bool(torch.isfinite(tau).all())
+    hit = o.double() + tau[:, None] * d.double()
+    rad = hit.norm(dim=1)
+    assert float(rad.min()) > 0.995 and float(rad.max()) <= 1.0 + 1e-6     # on the faceted unit sphere, first crossing
+    assert bool(((hit * o.double()).sum(1) > 0).all())                      # ... on the side the ray came from
+    idx = np.random.default_rng(3).integers(0, n, 300)
+    oc, dc = o[idx].cpu().numpy(), d[idx].cpu().numpy()
+    fc, tc = facet[idx].cpu().numpy(), tau[idx].cpu().numpy()
+    for k in range(idx.size):
+        fo, to = om.closest_hit(oc[k], dc[k], -1, use_bvh=True)
+        assert fc[k] == fo and tc[k] == to
+    gm.close()
+
+
 # ------------------------------------------------------------------ whole path on the five configs
 def test_run_parity_c1_plate_all_particles(T, O):
     cfg = ti.config("C1")[0]
