@@ -228,14 +228,26 @@ class Mesh:
                 "nt": int(out.nt), "n_nodes": int(out.n_nodes), "build_ms": out.build_ms, "horizon_ms": out.horizon_ms}
 
     def set_surface(self, T_W=None, sigma=None, stream=None):
-        """Per-facet wall temperature / accommodation (tpmc_mesh_set_surface); None restores the run's scalar."""
-        tw = None if T_W is None else np.ascontiguousarray(T_W, dtype=np.float64)
-        sg = None if sigma is None else np.ascontiguousarray(sigma, dtype=np.float64)
+        """Per-facet wall temperature / accommodation (tpmc_mesh_set_surface); None restores the run's scalar.
+        Host arrays, or CUDA float64 tensors (then both must be CUDA tensors or None)."""
+        on_dev = [a is not None and hasattr(a, "is_cuda") and a.is_cuda for a in (T_W, sigma)]
+        if any(on_dev):
+            torch = _torch()
+            if not all(d or a is None for d, a in zip(on_dev, (T_W, sigma))):
+                raise TpmcError("surface arrays must live in one memory space")
+            tw = None if T_W is None else T_W.to(torch.float64).contiguous()
+            sg = None if sigma is None else sigma.to(torch.float64).contiguous()
+            ptr = lambda a: None if a is None else a.data_ptr()
+            space = TPMC_MEM_DEVICE
+        else:
+            tw = None if T_W is None else np.ascontiguousarray(T_W, dtype=np.float64)
+            sg = None if sigma is None else np.ascontiguousarray(sigma, dtype=np.float64)
+            ptr = lambda a: None if a is None else a.ctypes.data
+            space = TPMC_MEM_HOST
         for a in (tw, sg):
-            if a is not None and a.shape != (self.nt,):
+            if a is not None and tuple(a.shape) != (self.nt,):
                 raise TpmcError("surface arrays must have one entry per facet")
-        _check(lib().tpmc_mesh_set_surface(self._h, None if tw is None else tw.ctypes.data, None if sg is None else sg.ctypes.data,
-                                           TPMC_MEM_HOST, _stream_ptr(stream)), "tpmc_mesh_set_surface")
+        _check(lib().tpmc_mesh_set_surface(self._h, ptr(tw), ptr(sg), space, _stream_ptr(stream)), "tpmc_mesh_set_surface")
 
     def copy_bvh(self):
         n_nodes = self.info()["n_nodes"]

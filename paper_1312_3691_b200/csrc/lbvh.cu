@@ -1067,18 +1067,49 @@ extern "C" void tpmc_mesh_destroy(tpmc_mesh* m) {
 }
 
 // A23: per-facet wall temperature and accommodation, by facet id; either may be NULL (the run's scalar is used).
+namespace {
+// counts the entries a run could not use: T_W must be finite and > 0 (c_W = sqrt(2 k T_W / m)), sigma in [0, 1]
+__global__ void k_check_surface(const double* __restrict__ T_W, const double* __restrict__ sigma, int64_t nt,
+                                unsigned int* __restrict__ bad) {
+  const int64_t f = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  bool b = false;
+  if (f < nt) {
+    if (T_W) { const double t = T_W[f]; b = !(t > 0.0 && isfinite(t)); }
+    if (sigma) { const double g = sigma[f]; b = b || !(g >= 0.0 && g <= 1.0); }
+  }
+  if (__syncthreads_or(b) && threadIdx.x == 0) atomicAdd(bad, 1u);
+}
+}  // namespace
+
 extern "C" int tpmc_mesh_set_surface(tpmc_mesh* m, const double* T_W, const double* sigma, int mem_space, void* cuda_stream) {
   if (!m || (mem_space != TPMC_MEM_HOST && mem_space != TPMC_MEM_DEVICE)) return TPMC_EINVAL;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const size_t bytes = sizeof(double) * (size_t)m->nt;
   const cudaMemcpyKind kind = mem_space == TPMC_MEM_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
-  if (mem_space == TPMC_MEM_HOST) {   // validate what can be read here: T_W > 0, 0 <= sigma <= 1
+  // validate before anything is replaced: T_W > 0 and finite, 0 <= sigma <= 1 (a NaN passes neither)
+  if (mem_space == TPMC_MEM_HOST) {
     for (int64_t f = 0; f < m->nt; ++f) {
       if (T_W && !(T_W[f] > 0.0 && isfinite(T_W[f]))) return TPMC_EINVAL;
       if (sigma && !(sigma[f] >= 0.0 && sigma[f] <= 1.0)) return TPMC_EINVAL;
     }
+  } else if (T_W || sigma) {   // device arrays: the same test by a kernel, one word read back
+    unsigned int* d_bad = nullptr;
+    unsigned int h_bad = 0;
+    TPMC_CUDA_TRY(cudaMalloc((void**)&d_bad, sizeof(unsigned int)));
+    cudaError_t e = cudaMemsetAsync(d_bad, 0, sizeof(unsigned int), st);
+    if (e == cudaSuccess) {
+      k_check_surface<<<(unsigned)((m->nt + 255) / 256), 256, 0, st>>>(T_W, sigma, m->nt, d_bad);
+      e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&h_bad, d_bad, sizeof(unsigned int), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(d_bad);
+    TPMC_CUDA_TRY(e);
+    if (h_bad) return TPMC_EINVAL;
   }
-  TPMC_CUDA_TRY(cudaStreamSynchronize(st));   // no run may still read the arrays being replaced
+  // No run may still read the arrays being replaced or freed.  The header asks for all calls on a handle to share one
+  // stream, but nothing enforces it and this is a set-up call: wait for the whole device, not just for `st`.
+  TPMC_CUDA_TRY(cudaDeviceSynchronize());
   const double* src[2] = {T_W, sigma};
   double** dst[2] = {&m->surf_TW, &m->surf_sigma};
   for (int k = 0; k < 2; ++k) {

@@ -856,6 +856,26 @@ def test_per_facet_surface_and_energy_accommodation_parity(T, O):
     assert bool((z.hash == ref.hash).all())
     with pytest.raises(T.TpmcError):
         gm.set_surface(np.full(m.nt, -1.0), None)
+    # (6) arrays handed over in DEVICE memory: the same run as from host arrays, and the same checks -- a wall
+    # temperature <= 0 or NaN, or an accommodation outside [0, 1], anywhere in the array, is refused and changes nothing
+    import torch
+    TWd, sgd = torch.as_tensor(TW, device="cuda"), torch.as_tensor(sg, device="cuda")
+    gm.set_surface(TWd, sgd)
+    d2 = gm.run(base, first=0, count=150_000, debug=True)
+    assert bool((d2.hash == g2.hash).all())
+    assert np.linalg.norm(d2.force.cpu().numpy() - g2.force.cpu().numpy()) <= 1e-12 * np.linalg.norm(g2.force.cpu().numpy())
+    for k, val in ((0, 0.0), (m.nt // 2, float("nan")), (m.nt - 1, -5.0), (3, float("inf"))):
+        bad = TWd.clone(); bad[k] = val
+        with pytest.raises(T.TpmcError):
+            gm.set_surface(bad, sgd)
+    for k, val in ((1, 1.0 + 1e-9), (m.nt - 1, float("nan")), (7, -0.1)):
+        bad = sgd.clone(); bad[k] = val
+        with pytest.raises(T.TpmcError):
+            gm.set_surface(TWd, bad)
+        with pytest.raises(T.TpmcError):
+            gm.set_surface(None, bad)
+    d3 = gm.run(base, first=0, count=150_000, debug=True)                # the refused calls left the surface as it was
+    assert bool((d3.hash == g2.hash).all()) and bool(torch.isfinite(d3.force).all())
     with pytest.raises(T.TpmcError):
         gm.run(base.with_(energy_accommodation=1.5))
     gm.close()
