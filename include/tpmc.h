@@ -40,8 +40,12 @@ extern "C" {
 #define TPMC_FACET_TWO_SIDED 1u /* facet_flags bit0 */
 #define TPMC_MAX_BOUNCES 0x0FFFFFFFu /* largest max_bounces (the bounce count shares a word with the species) */
 
-/* tpmc_params.flags.  Each switches off, forces or adds a step that must not change any result -- the parity tests
- * run with and without them; the library's defaults are all zero. */
+/* tpmc_params.flags.  Each switches off, forces or adds a step that must not change the physics: the parity tests run
+ * with and without them and require the same hit sequence for every particle and sums equal to the order of the fp64
+ * additions (1e-12 relative).  "Same" is not "bit for bit" in one respect: the fp64 sampler stops its root searches on a
+ * step tolerance, and under NO_PRECULL it starts them from its own guess instead of the pre-cull's, so a seeded
+ * coordinate may differ in the last ulp of its fp64 value.  After the fp32 rounding of O9 that moves a ray with
+ * probability ~1e-9 per coordinate -- a few particles in 1e9, far inside the 99.99 % bar.  The defaults are all zero. */
 #define TPMC_FLAG_NO_PRECULL 0x01u  /* every particle through the fp64 sampler (no fp32 pre-cull pass) */
 #define TPMC_FLAG_NO_HORIZON 0x02u  /* every re-emitted ray is traced (no escape-horizon test) */
 #define TPMC_FLAG_ALIGN_OFF 0x04u   /* traversal on the body-frame hierarchy, whatever the attitude */
@@ -156,7 +160,8 @@ int tpmc_mesh_info(const tpmc_mesh* mesh, tpmc_mesh_info_t* out /* host */);
  * satellite surface temperature"): T_W [nt] wall temperature (K, > 0) and sigma [nt] accommodation in [0,1],
  * indexed by facet id as in `indices`, both where mem_space says; either may be NULL, which restores the run's scalar
  * (tpmc_params.T_W / .accommodation).  The arrays are copied; they apply to every later run on this handle.
- * Synchronises the stream (before replacing arrays a run may still read, and after the copy). */
+ * Host and device arrays alike are checked first (a value outside those ranges, or a NaN: TPMC_EINVAL, nothing changed).
+ * Waits for the whole device before replacing arrays a run may still read, and synchronises the stream after the copy. */
 int tpmc_mesh_set_surface(tpmc_mesh* mesh, const double* T_W, const double* sigma, int mem_space, void* cuda_stream);
 
 /* Copy the built hierarchy to the host for inspection: nodes [n_nodes][16] floats

@@ -94,11 +94,13 @@ struct tpmc_mesh {
   Pipe pipe[kPipes];
   double* facet_scratch;           // [nt][3] when the caller passes no per-facet buffer
   double* partials;                // reduction partials
-  unsigned long long* stats;       // [8] device counters
+  unsigned long long* stats;       // [ST_COUNT] device counters (enum below), one per tpmc_stats event
   double* totals;                  // [3] torque accumulators
   double* ft_dev;                  // [6] force | torque of tpmc_run_host
   cudaEvent_t ev0, ev1, ev_fork;
   unsigned long long last_launches;
+  bool in_run;                     // tpmc_run has enqueued work and not yet returned TPMC_OK (see its error path)
+  bool poisoned;                   // a failed run could not be drained: every later run on this handle returns TPMC_ECUDA
 };
 
 constexpr int kMaxTimedWaves = 1024;  // iterations covered by the per-kernel event times
