@@ -1130,11 +1130,45 @@ bool want_alignment(const tpmc_params* p) {
   return vabs > 0.0 && vmax < 0.9 * vabs;
 }
 
+int run_enqueue(tpmc_mesh* m, const tpmc_params* params, void* cuda_stream, double* d_force, double* d_torque,
+                double* d_facet_momentum, tpmc_stats* h_stats, const tpmc_debug* debug);
+
 }  // namespace
 
+// The run itself is run_enqueue below.  A failure after its first enqueue (a CUDA error, a failed refit) would leave
+// kernels queued on the handle's seed and side streams that nothing joins, with counters half-way: the next call on the
+// handle -- the next attitude of a sweep -- would race with them.  So a failed run is drained here before its code is
+// returned, and if even that fails (a sticky CUDA error) the handle is marked unusable instead of being trusted again.
 extern "C" int tpmc_run(tpmc_mesh* m, const tpmc_params* params, void* cuda_stream, double* d_force,
                         double* d_torque, double* d_facet_momentum, tpmc_stats* h_stats, const tpmc_debug* debug) {
   if (!m || !params || !d_force || !d_torque) return TPMC_EINVAL;
+  if (m->poisoned) {
+    snprintf(g_tpmc_cuda_error, sizeof(g_tpmc_cuda_error),
+             "tpmc_run: an earlier run on this mesh handle failed and could not be drained; destroy the handle");
+    return TPMC_ECUDA;
+  }
+  const int rcode = run_enqueue(m, params, cuda_stream, d_force, d_torque, d_facet_momentum, h_stats, debug);
+  if (rcode != TPMC_OK && m->in_run) {
+    char first_error[sizeof(g_tpmc_cuda_error)];
+    memcpy(first_error, g_tpmc_cuda_error, sizeof(first_error));   // the caller wants the error that failed the run
+    bool drained = true;
+    for (int pi = 0; pi < kPipes; ++pi) {
+      Pipe& pp = m->pipe[pi];
+      cudaStream_t ss[3] = {pp.seed, pp.side, pi > 0 ? pp.main : (cudaStream_t)cuda_stream};
+      for (cudaStream_t s : ss)
+        if (cudaStreamSynchronize(s) != cudaSuccess) drained = false;
+    }
+    cudaGetLastError();
+    if (!drained) m->poisoned = true;
+    memcpy(g_tpmc_cuda_error, first_error, sizeof(first_error));
+  }
+  m->in_run = false;
+  return rcode;
+}
+
+namespace {
+int run_enqueue(tpmc_mesh* m, const tpmc_params* params, void* cuda_stream, double* d_force, double* d_torque,
+                double* d_facet_momentum, tpmc_stats* h_stats, const tpmc_debug* debug) {
   RunConst rc;
   int rcode = make_run_const(m, params, &rc);
   if (rcode != TPMC_OK) return rcode;
@@ -1162,6 +1196,7 @@ extern "C" int tpmc_run(tpmc_mesh* m, const tpmc_params* params, void* cuda_stre
   SeedConstF sf;
   make_seed_const_f(m, rc, &sf);
   const QuantGrid qg = quant_grid(m);   // seed-time cull (body frame)
+  m->in_run = true;   // from here on a failure leaves work enqueued: tpmc_run drains it
   TPMC_CUDA_TRY(cudaEventRecord(m->ev0, st));
   // the traversal's hierarchy: body frame, or refitted in the stream frame of this run (x' = R^T x: z' along the stream)
   const QuantGrid* qg_t = m->grid_dev;
@@ -1329,6 +1364,7 @@ extern "C" int tpmc_run(tpmc_mesh* m, const tpmc_params* params, void* cuda_stre
   }
   return TPMC_OK;
 }
+}  // namespace
 
 // K attitudes of a sweep in one call: run k is `params` with V = h_V[k].  The handle's scratch, streams and events are
 // shared by all of them; nothing is read back between attitudes unless statistics are asked for.
