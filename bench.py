@@ -303,16 +303,24 @@ def main():
         p0, keep0 = tpmc.make_params(cfg0)
         L.tpmc_run_host(mesh._h, C.byref(p0), stream.cuda_stream or None, hF.ctypes.data, hT.ctypes.data, hP.ctypes.data, None)
         barrier()
+        e2e_s = 0.0
         t0 = time.perf_counter()
         for k in range(args.steps):
+            if flush is not None:            # same rule as the device-timed loop: L2 flushed between steps, outside the clock
+                flush.fill_(k & 0xFF)
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
             cfg = cfgs[attitude_index(args.warmup + k, rank, world, len(cfgs))]
             p, keep = tpmc.make_params(cfg)
             rc = L.tpmc_run_host(mesh._h, C.byref(p), stream.cuda_stream or None, hF.ctypes.data, hT.ctypes.data,
-                                 hP.ctypes.data, None)
+                                 hP.ctypes.data, None)           # returns after its own stream synchronisation
             if rc != 0:
                 raise SystemExit(f"tpmc_run_host failed: {rc}")
+            if flush is not None:
+                e2e_s += time.perf_counter() - t0
         barrier()
-        e2e_s = time.perf_counter() - t0
+        if flush is None:
+            e2e_s = time.perf_counter() - t0
         e2e = {"hits": hits, "s": e2e_s}
 
     peaks = None
@@ -362,10 +370,16 @@ def main():
             # hit L2), then instruction issue; DRAM is a few per cent.  Binding roofline: the gather path, against the
             # measured rate of independent 32-byte gathers over an array of the structure's size at this kernel's
             # residency.  The fp32-issue and HBM views are reported beside it.
-            gpk = peaks["gather32_bytes_per_s"] / 1e9
+            gpk = peaks["gather64_bytes_per_s"] / 1e9
+            t_ov = avg_ms_overlapped * 1e-3
             roof.update({"bound": "l2-gather", "achieved": alg_bw, "peak": gpk, "unit": "GB/s", "frac": alg_bw / gpk,
-                         "peak_source": "measured in this run (tpmc_measure_peaks): independent 32-byte ld.global.nc gathers over "
-                                        "83 MB, 8 x 128 threads per SM",
+                         # `value` is timed in the overlapped schedule (the next wave's seed kernels share the SMs), `frac` on
+                         # the kernel alone; the same ratio with the overlapped launch duration:
+                         "frac_as_scheduled": (rays_per_launch * per_seg_bytes / t_ov / 1e9 / gpk) if t_ov > 0 else None,
+                         "peak_source": "measured in this run (tpmc_measure_peaks.gather64_bytes_per_s): 64-byte records over 83 MB "
+                                        "read as two 32-byte ld.global.nc of one line, two records in flight per lane, 7 x 128 "
+                                        "threads per SM = k_trace_wf's access shape and residency; the one-load-in-flight figure "
+                                        "of earlier rounds is peaks.gather32_bytes_per_s",
                          "fetched_view": {"achieved": fetched_bw, "peak": gpk, "unit": "GB/s", "frac": fetched_bw / gpk,
                                           "what": "wide nodes x 64 B + facets x 48 B the kernel really fetched"},
                          "alu_view": {"achieved": alg_ops, "peak": peaks["fp32_lane_ops_per_s"] / 1e12, "unit": "T lane-op/s",
@@ -402,8 +416,11 @@ def main():
             per = max(1000, int(args.cpu_baseline_particles // threads))
             oracle_sample(cfgs, 1000, threads)
             h, dt, n = oracle_sample(cfgs, per, threads)
+            h1, dt1, n1 = oracle_sample(cfgs, max(1000, int(args.cpu_baseline_particles // 40)), 1)   # one thread
             line["cpu_baseline"] = {"value": h / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
-                                    "sample": f"{n} particles ({threads} slices) of the same N={N:.0e} stream, sweep point 0, {dt:.1f} s"}
+                                    "sample": f"{n} particles ({threads} slices) of the same N={N:.0e} stream, sweep point 0, {dt:.1f} s",
+                                    "per_core": {"value": h1 / dt1, "unit": UNIT, "cores": 1,
+                                                 "sample": f"{n1} particles, one thread, {dt1:.1f} s"}}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -230,7 +230,9 @@ int tpmc_trace(tpmc_mesh* mesh, const float* d_o, const float* d_d, const int32_
  * not nominal).  Hand-written micro-kernels, each timed once after a warm-up launch (about 0.1 s in all):
  *   fp32 FFMA lane-instruction rate at full occupancy; fp64 FMA rate; 32-byte read-only gathers (one 256-bit load per
  *   lane, every lane its own record) over an 83 MB array with the traversal kernel's residency (8 blocks of 128
- *   threads per SM), with independent addresses and as a pointer chase; fp64 red.global.add at 1, 2048 and 1e6
+ *   threads per SM), with independent addresses and as a pointer chase -- both with ONE load in flight per lane, i.e.
+ *   resident lanes x 32 B / latency; the same array read as 64-byte records the way the traversal kernel reads a wide
+ *   node, several loads in flight per lane (the throughput of the gather path); fp64 red.global.add at 1, 2048 and 1e6
  *   accumulators laid out like the per-facet momentum.  out: host.  Synchronises the stream. */
 typedef struct {
   int32_t sms;
@@ -243,6 +245,8 @@ typedef struct {
   double gather_array_bytes;
   double red_f64_per_s[3];          /* fp64 atomic adds per second ... */
   double red_f64_addresses[3];      /* ... over this many accumulators */
+  double gather64_bytes_per_s;      /* 64-byte records as two 32-byte loads of one line, two records in flight per lane,
+                                       7 blocks of 128 threads per SM: the traversal kernel's access shape and residency */
 } tpmc_peaks;
 int tpmc_measure_peaks(tpmc_peaks* out, void* cuda_stream);
 

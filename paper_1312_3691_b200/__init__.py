@@ -68,7 +68,8 @@ class tpmc_peaks(C.Structure):
     _fields_ = [("sms", C.c_int32), ("sm_clock_mhz_nominal", C.c_double), ("sm_clock_mhz_fp32", C.c_double),
                 ("fp32_lane_ops_per_s", C.c_double), ("fp64_fma_per_s", C.c_double), ("gather32_bytes_per_s", C.c_double),
                 ("gather32_dependent_bytes_per_s", C.c_double), ("gather_array_bytes", C.c_double),
-                ("red_f64_per_s", C.c_double * 3), ("red_f64_addresses", C.c_double * 3)]
+                ("red_f64_per_s", C.c_double * 3), ("red_f64_addresses", C.c_double * 3),
+                ("gather64_bytes_per_s", C.c_double)]
 
 
 class tpmc_debug(C.Structure):

@@ -62,6 +62,35 @@ __global__ void __launch_bounds__(128, 8) k_peak_gather(const uint4* __restrict_
   out[tid] = acc;
 }
 
+// The traversal kernel's own access shape: a 64-byte record (one wide node) fetched as the two 32-byte halves of one
+// line, every lane its own record, at that kernel's residency (128 threads per block, 7 blocks per SM) -- and with two
+// records (four loads) in flight per lane before the first result is used, so that the figure is the throughput of the
+// L1TEX / L2 gather path and not resident lanes x 32 B / latency, which is what one load in flight per lane measures
+// (k_peak_gather above: its independent and dependent variants come out equal for that reason).
+__global__ void __launch_bounds__(128, 7) k_peak_gather64(const uint4* __restrict__ buf, unsigned int n_rec64, int iters,
+                                                          unsigned int* __restrict__ out) {
+  const unsigned int tid = blockIdx.x * blockDim.x + threadIdx.x;
+  unsigned int acc = 0u;
+  for (int k = 0; k < iters; ++k) {
+    const unsigned int i0 = mix32(tid + 0x9E3779B9u * (unsigned int)(2 * k + 1)) % n_rec64;
+    const unsigned int i1 = mix32(tid + 0x9E3779B9u * (unsigned int)(2 * k + 2)) % n_rec64;
+    uint4 a[4], b[4];
+    const uint4* p0 = buf + 4 * (size_t)i0;
+    const uint4* p1 = buf + 4 * (size_t)i1;
+#define TPMC_LD256(A, B, P)                                                                                          \
+  asm volatile("ld.global.nc.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"                                                \
+               : "=r"(A.x), "=r"(A.y), "=r"(A.z), "=r"(A.w), "=r"(B.x), "=r"(B.y), "=r"(B.z), "=r"(B.w)              \
+               : "l"(P))
+    TPMC_LD256(a[0], b[0], p0);
+    TPMC_LD256(a[1], b[1], p0 + 2);
+    TPMC_LD256(a[2], b[2], p1);
+    TPMC_LD256(a[3], b[3], p1 + 2);
+#undef TPMC_LD256
+    acc ^= (a[0].y ^ b[0].w) ^ (a[1].y ^ b[1].w) ^ (a[2].y ^ b[2].w) ^ (a[3].y ^ b[3].w);
+  }
+  out[tid] = acc;
+}
+
 // fp64 atomic adds without return value (red.global.add.f64), spread over n_addr accumulators 24 bytes apart
 __global__ void __launch_bounds__(256) k_peak_red(double* __restrict__ acc, unsigned int n_addr, int iters) {
   const unsigned int tid = blockIdx.x * blockDim.x + threadIdx.x;
@@ -138,6 +167,11 @@ extern "C" int tpmc_measure_peaks(tpmc_peaks* out, void* cuda_stream) {
       PEAK_TIMED(ms, (k_peak_gather<<<blocks, 128, 0, st>>>((const uint4*)d_buf, n_rec, iters, dep, (unsigned int*)d_out)));
       const double loads = (double)blocks * 128.0 * iters;
       (dep ? out->gather32_dependent_bytes_per_s : out->gather32_bytes_per_s) = loads * 32.0 / (ms * 1e-3);
+    }
+    {   // 64-byte records, the traversal kernel's shape and residency
+      const int iters = 512, blocks = sms * 7;
+      PEAK_TIMED(ms, (k_peak_gather64<<<blocks, 128, 0, st>>>((const uint4*)d_buf, n_rec / 2, iters, (unsigned int*)d_out)));
+      out->gather64_bytes_per_s = (double)blocks * 128.0 * iters * 128.0 / (ms * 1e-3);   // 2 records x 64 B per iteration
     }
     out->gather_array_bytes = (double)gather_bytes;
     const unsigned int n_addr[3] = {1u, 2048u, red_max};
