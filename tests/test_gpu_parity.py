@@ -818,6 +818,46 @@ def test_c2_c3_c4_every_shortcut_off_at_timing_size(T, name, idx):
     _full_size_arms(T, ti.config(name)[idx], _arms(T))
 
 
+def test_c5_precull_and_horizon_off_on_every_attitude_of_the_sweep(T):
+    """The two shortcuts whose exactness rests on a margin rather than on a proof carried by the code (the fp32 pre-cull's
+    grown volumes and the per-facet escape horizons) switched off together on ALL 1e9 particles of
+    ALL 64 attitudes of the C5 sweep -- the three attitudes of the test above leave 61 directions of the stream, and with
+    them most of the facets' horizon sectors, unvisited.  Per attitude: same hits, same hash / bounce count / first facet
+    for every particle, same force to the order of the fp64 additions."""
+    import torch
+    cfgs = ti.config("C5")
+    m = cfgs[0].mesh()
+    gm = T.Mesh(m.vertices, m.indices, m.flags)
+    off = T.TPMC_FLAG_NO_PRECULL | T.TPMC_FLAG_NO_HORIZON
+    for k, cfg in enumerate(cfgs):
+        a = gm.run(cfg, debug=True, facets=False)
+        b = gm.run(cfg, debug=True, facets=False, flags=off)
+        check_conservation(a.stats, cfg.N)
+        check_conservation(b.stats, cfg.N)
+        assert b.stats["ret_precull_a"] + b.stats["ret_precull_b"] + b.stats["ret_horizon"] == 0
+        assert a.stats["ret_precull_a"] + a.stats["ret_precull_b"] > 0 and a.stats["ret_horizon"] > 0
+        assert a.stats["hits"] == b.stats["hits"] > 0, k
+        assert torch.equal(a.hash, b.hash), k
+        assert torch.equal(a.bounces, b.bounces) and torch.equal(a.first_facet, b.first_facet), k
+        Fa, Fb = a.force.cpu().numpy(), b.force.cpu().numpy()
+        assert np.linalg.norm(Fa - Fb) <= 1e-11 * np.linalg.norm(Fb), k
+        del a, b
+    gm.close()
+
+
+@pytest.mark.parametrize("S", [0.1, 0.3, 1.0])
+def test_precull_and_horizon_off_at_low_speed_ratio_all_particles(T, S):
+    """The same two switches where the thermal spread is largest: speed ratio S of the heavier species 0.1, 0.3, 1 (the
+    lighter one at half of that), 1e8 particles on the concave satellite.  At these S the particles arrive from all
+    round the control sphere and the pre-cull's certified-miss test works with wide velocity cones; every config of the
+    sweep tests runs at S >= 2."""
+    base = ti.config("C4")[5]
+    c_mp = np.sqrt(2.0 * ti.K_B * base.T_inf / (16.0 * ti.AMU))
+    vhat = np.array(base.V) / np.linalg.norm(base.V)
+    cfg = base.with_(N=100_000_000, V=tuple(S * c_mp * vhat), m=(16.0 * ti.AMU, 4.0 * ti.AMU), x=(0.7, 0.3))
+    _full_size_arms(T, cfg, [("no pre-cull", T.TPMC_FLAG_NO_PRECULL), ("no horizon", T.TPMC_FLAG_NO_HORIZON)])
+
+
 # ------------------------------------------------------------------ NEXT-3: surface models beyond one global T_W, sigma
 def test_per_facet_surface_and_energy_accommodation_parity(T, O):
     """Readings A22 / A23 against the oracle (whose versions are pinned by P17): wall temperature and accommodation
