@@ -9,6 +9,8 @@ One "step" = one tpmc_run of N particles at one point of the config's sweep (the
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl tpmc|reference] [--config C5] [--particles N]
 N > 1: launched by torchrun, one rank per GPU; rank r runs sweep points r, r+N, ... (weak scaling, no data-path
 collective: sweep points are independent problems); value = all ranks' bounces / max time.
+`--split slices` is the other split of SURVEY 8(e): every rank runs its particle range of the SAME sweep point and the
+outputs are all-reduced (NCCL, SUM) inside the timed region (strong scaling).
 Prints ONE JSON line on rank 0 (contract in DESIGN.md "Measurement").
 """
 from __future__ import annotations
@@ -128,6 +130,27 @@ def slice_of(rank: int, world: int, N: int):
     return first, (N - first if rank == world - 1 else per)
 
 
+def split_plan(split: str, step: int, rank: int, world: int, n_attitudes: int, N: int):
+    """What a rank runs at a step: (sweep point, first particle, particle count).
+    "attitudes": ranks take disjoint sweep points, each the whole stream (independent problems, no exchange).
+    "slices": every rank runs its contiguous range of the SAME point's stream (particles are independent, PAPER.md:69);
+    the outputs are then summed across ranks (allreduce_outputs) -- the split of SURVEY 8(e)."""
+    if split == "slices":
+        first, count = slice_of(rank, world, N)
+        return step % n_attitudes, first, count
+    return attitude_index(step, rank, world, n_attitudes), 0, N
+
+
+def allreduce_outputs(tensors, world: int):
+    """The one exchange step of the "slices" split: in-place SUM over ranks of a slice's force, torque and per-facet
+    momentum (3 + 3 + 3 nt doubles; NCCL on the device under torchrun, gloo on CPU tensors in the tests)."""
+    if world > 1:
+        import torch.distributed as dist
+        for t in tensors:
+            dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return tensors
+
+
 def oracle_sample(cfgs, count_per_thread, threads):
     """The oracle, as it stands, on a bounded slice of the same workload, one slice per host thread."""
     import oracle
@@ -187,6 +210,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-peaks", action="store_true")
+    ap.add_argument("--split", default="attitudes", choices=["attitudes", "slices"],
+                    help="N > 1: ranks take disjoint sweep points (default, weak scaling, no exchange), or disjoint particle "
+                         "ranges of the same point with an all-reduce of the outputs inside the timed region (strong scaling)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -232,13 +258,18 @@ def main():
     # between steps by writing a 512 MB buffer (outside the per-step event pairs).
     flush = None if args.config == "C5" else torch.empty(512 << 20, dtype=torch.uint8, device=dev)
 
+    slices = args.split == "slices"
+    my_count = split_plan(args.split, 0, rank, world, len(cfgs), N)[2]
+
     def step(k, stats=None, flags=0):
-        cfg = cfgs[attitude_index(k, rank, world, len(cfgs))]
-        p, keep = tpmc.make_params(cfg, flags=flags)
+        att, first, count = split_plan(args.split, k, rank, world, len(cfgs), N)
+        p, keep = tpmc.make_params(cfgs[att], first=first, count=count, flags=flags)
         rc = L.tpmc_run(mesh._h, C.byref(p), stream.cuda_stream or None, force.data_ptr(), torque.data_ptr(),
                         facets.data_ptr(), None if stats is None else C.byref(stats), None)
         if rc != 0:
             raise SystemExit(f"tpmc_run failed: {rc} {L.tpmc_last_cuda_error().decode()}")
+        if slices:      # the exchange step, inside the timed region: every rank ends the step with the whole run's outputs
+            allreduce_outputs([force, torque, facets], world)
 
     # ---- warm-up (untimed)
     for k in range(args.warmup):
@@ -298,9 +329,10 @@ def main():
     e2e = None
     if not args.no_e2e:
         hF, hT = np.empty(3), np.empty(3)
-        hP = torch.empty((mesh.nt, 3), dtype=torch.float64).pin_memory().numpy()
-        cfg0 = cfgs[attitude_index(args.warmup, rank, world, len(cfgs))]
-        p0, keep0 = tpmc.make_params(cfg0)
+        hP_t = torch.empty((mesh.nt, 3), dtype=torch.float64).pin_memory()
+        hP = hP_t.numpy()
+        att0, first0, count0 = split_plan(args.split, args.warmup, rank, world, len(cfgs), N)
+        p0, keep0 = tpmc.make_params(cfgs[att0], first=first0, count=count0)
         L.tpmc_run_host(mesh._h, C.byref(p0), stream.cuda_stream or None, hF.ctypes.data, hT.ctypes.data, hP.ctypes.data, None)
         barrier()
         e2e_s = 0.0
@@ -310,12 +342,19 @@ def main():
                 flush.fill_(k & 0xFF)
                 torch.cuda.synchronize()
                 t0 = time.perf_counter()
-            cfg = cfgs[attitude_index(args.warmup + k, rank, world, len(cfgs))]
-            p, keep = tpmc.make_params(cfg)
-            rc = L.tpmc_run_host(mesh._h, C.byref(p), stream.cuda_stream or None, hF.ctypes.data, hT.ctypes.data,
-                                 hP.ctypes.data, None)           # returns after its own stream synchronisation
-            if rc != 0:
-                raise SystemExit(f"tpmc_run_host failed: {rc}")
+            if slices and world > 1:
+                # host buffers at the end of the step need the exchange first: device run, all-reduce, then the D2H copies
+                step(args.warmup + k)
+                hP_t.copy_(facets, non_blocking=True)
+                hFT = torch.cat([force, torque]).cpu()
+                torch.cuda.synchronize()
+            else:
+                att, first, count = split_plan(args.split, args.warmup + k, rank, world, len(cfgs), N)
+                p, keep = tpmc.make_params(cfgs[att], first=first, count=count)
+                rc = L.tpmc_run_host(mesh._h, C.byref(p), stream.cuda_stream or None, hF.ctypes.data, hT.ctypes.data,
+                                     hP.ctypes.data, None)           # returns after its own stream synchronisation
+                if rc != 0:
+                    raise SystemExit(f"tpmc_run_host failed: {rc}")
             if flush is not None:
                 e2e_s += time.perf_counter() - t0
         barrier()
@@ -329,7 +368,7 @@ def main():
 
     # ---- max over ranks, totals over ranks
     (ms_total_max, e2e_s_max), (hits_all, segs_all, parts_all) = reduce_over_ranks(
-        [ms_total, e2e["s"] if e2e else 0.0], [hits, segs, N * args.steps], world, dev)
+        [ms_total, e2e["s"] if e2e else 0.0], [hits, segs, my_count * args.steps], world, dev)
 
     if rank == 0:
         value = hits_all / (ms_total_max * 1e-3)
@@ -390,10 +429,15 @@ def main():
         roof["hbm_view"] = {"achieved": alg_bw, "peak": hbm, "unit": "GB/s", "frac": alg_bw / hbm, "peak_source": hbm_src}
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_total_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_total_max / args.steps, "higher_is_better": True,
+            "scaling": "strong" if slices and world > 1 else "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": WORKLOADS[args.config], "particles_per_step": N, "facets": mesh.nt, "bvh_nodes": info["n_nodes"],
-                       "sweep": f"{len(cfgs)} points, point (step*world+rank) mod {len(cfgs)}", "cv_radius_factor": cfgs[0].cv_radius_factor,
+                       "sweep": (f"{len(cfgs)} points, point step mod {len(cfgs)} on every rank; rank r runs particles "
+                                 f"[r N/{world}, (r+1) N/{world}) and the outputs (force, torque, {mesh.nt} x 3 per-facet momentum, "
+                                 f"{24 * mesh.nt + 48} B) are all-reduced (NCCL, SUM) inside the timed region" if slices else
+                                 f"{len(cfgs)} points, point (step*world+rank) mod {len(cfgs)}"),
+                       "split": args.split, "cv_radius_factor": cfgs[0].cv_radius_factor,
                        "l2": ("inputs larger than L2: hierarchy + facets 149 MB, per-facet momentum 25 MB, ~2 GB of lists and ray "
                               "queues rewritten every wave" if flush is None else
                               "L2 flushed between steps (512 MB written); each step timed by its own event pair"),
@@ -410,7 +454,8 @@ def main():
         if e2e:
             line["e2e"] = {"value": hits_all / e2e_s_max, "unit": UNIT,
                            "h2d_bytes_per_step": int(C.sizeof(tpmc.tpmc_params) + 16 * len(cfgs[0].m)),
-                           "d2h_bytes_per_step": int(mesh.nt * 24 + 48), "api": "tpmc_run_host"}
+                           "d2h_bytes_per_step": int(mesh.nt * 24 + 48),
+                           "api": "tpmc_run + all-reduce + D2H copies" if slices and world > 1 else "tpmc_run_host"}
         if world == 1 and not args.no_cpu_baseline:
             threads = os.cpu_count() or 1
             per = max(1000, int(args.cpu_baseline_particles // threads))

@@ -61,8 +61,15 @@ def _slice_worker(rank, world, port, out):
     m = cfg.mesh()
     om = oracle.OracleMesh(m.vertices, m.indices, m.flags)
     first, count = bench.slice_of(rank, world, cfg.N)
+    # bench.py --split slices: the plan of a step (same sweep point on every rank, this rank's particle range) ...
+    assert bench.split_plan("slices", 70, rank, world, 64, cfg.N) == (6, first, count)
+    assert bench.split_plan("attitudes", 70, rank, world, 64, cfg.N) == (bench.attitude_index(70, rank, world, 64), 0, cfg.N)
     r = om.run(cfg, first=first, count=count, debug=False)
     F, Tq, P, hits = bench.sum_slices([r.force, r.torque, r.facet_momentum, np.array([float(r.hits)])], world)
+    # ... and its exchange step: the in-place all-reduce of the three output buffers, as the bench loop calls it
+    bufs = [torch.tensor(r.force), torch.tensor(r.torque), torch.tensor(r.facet_momentum)]
+    same = bench.allreduce_outputs(bufs, world)
+    assert same[0] is bufs[0] and torch.equal(bufs[0], F) and torch.equal(bufs[1], Tq) and torch.equal(bufs[2], P)
     res = None
     if rank == 0:
         full = om.run(cfg, debug=False)
@@ -94,6 +101,8 @@ def test_two_ranks_sum_particle_slices_of_one_run():
 def test_slices_cover_the_stream():
     sys.path.insert(0, ROOT)
     import bench
+    t = [torch.ones(3)]
+    assert bench.allreduce_outputs(t, 1)[0] is t[0] and bench.split_plan("slices", 3, 0, 1, 64, 10) == (3, 0, 10)
     for N, world in ((10, 3), (1_000_000_007, 8), (5, 8)):
         s = [bench.slice_of(r, world, N) for r in range(world)]
         assert s[0][0] == 0 and sum(c for _, c in s) == N

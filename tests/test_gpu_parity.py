@@ -422,6 +422,36 @@ def test_slices_are_additive_and_runs_repeat(T, O):
         check_conservation(r.stats, n)
 
 
+def test_two_slices_on_two_handles_and_streams_sum_to_the_full_run(T):
+    """SURVEY 8(e), the particle-range split as bench.py --split slices runs it on N GPUs, here with both "ranks" on one
+    device: two mesh handles, two streams, the two halves of one stream of particles in flight at the same time (handles
+    are independent, include/tpmc.h), outputs summed.  Equal to the undivided run: hits exactly, sums to the order of the
+    fp64 additions."""
+    import torch
+    import bench
+    cfg = ti.config("C4")[7].with_(N=6_000_001)
+    m = cfg.mesh()
+    handles = [T.Mesh(m.vertices, m.indices, m.flags) for _ in range(2)]
+    full = handles[0].run(cfg)
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    torch.cuda.synchronize()
+    parts = []
+    for rank in range(2):
+        att, first, count = bench.split_plan("slices", 7, rank, 2, 16, cfg.N)
+        assert att == 7 and (first, count) == ((0, 3_000_000) if rank == 0 else (3_000_000, 3_000_001))
+        with torch.cuda.stream(streams[rank]):
+            parts.append(handles[rank].run(cfg, first=first, count=count, stats=False, stream=streams[rank]))
+    torch.cuda.synchronize()
+    for name in ("force", "torque", "facet_momentum"):
+        tot = getattr(parts[0], name) + getattr(parts[1], name)
+        ref = getattr(full, name)
+        assert float((tot - ref).abs().max()) <= 1e-12 * float(ref.abs().max()) + 1e-30, name
+    again = [handles[r].run(cfg, first=r * 3_000_000, count=3_000_000 + r) for r in range(2)]
+    assert again[0].stats["hits"] + again[1].stats["hits"] == full.stats["hits"]
+    for h in handles:
+        h.close()
+
+
 def test_edge_cases_empty_truncated_host_buffers(T, O):
     cfg = ti.config("C4")[0].with_(N=100_000)
     gm, om = meshes(T, O, cfg)
