@@ -25,10 +25,12 @@ TPMC_MAX_BOUNCES = 0x0FFFFFFF
 TPMC_FLAG_NO_PRECULL, TPMC_FLAG_NO_HORIZON, TPMC_FLAG_ALIGN_OFF, TPMC_FLAG_ALIGN_ON = 0x01, 0x02, 0x04, 0x08
 TPMC_FLAG_EXACT_TRACE, TPMC_FLAG_SORT_RAYS, TPMC_FLAG_NO_AGGREGATION, TPMC_FLAG_SERIAL_SEED = 0x10, 0x20, 0x40, 0x80
 TPMC_CV_SPHERE, TPMC_CV_BOX, TPMC_CV_BOX_UNWEIGHTED = 0, 1, 2
+TPMC_MESH_NO_HORIZON = 0x1
 
 EXPORTS = ["tpmc_mesh_create", "tpmc_mesh_destroy", "tpmc_mesh_info", "tpmc_mesh_copy_bvh", "tpmc_run",
            "tpmc_mesh_copy_horizon", "tpmc_run_host", "tpmc_seed", "tpmc_trace", "tpmc_strerror", "tpmc_last_cuda_error", "tpmc_version",
-           "tpmc_measure_peaks", "tpmc_mesh_set_surface", "tpmc_run_sweep", "tpmc_mesh_copy_wide", "tpmc_facet_sum_static"]
+           "tpmc_measure_peaks", "tpmc_mesh_set_surface", "tpmc_run_sweep", "tpmc_mesh_copy_wide", "tpmc_facet_sum_static",
+           "tpmc_mesh_create_ex", "tpmc_mesh_build_horizon"]
 
 
 class TpmcError(RuntimeError):
@@ -90,6 +92,10 @@ def lib():
         vp = C.c_void_p
         L.tpmc_mesh_create.restype = C.c_int
         L.tpmc_mesh_create.argtypes = [vp, C.c_int64, vp, C.c_int64, vp, C.c_int, vp, C.POINTER(vp)]
+        L.tpmc_mesh_create_ex.restype = C.c_int
+        L.tpmc_mesh_create_ex.argtypes = [vp, C.c_int64, vp, C.c_int64, vp, C.c_int, C.c_uint32, vp, C.POINTER(vp)]
+        L.tpmc_mesh_build_horizon.restype = C.c_int
+        L.tpmc_mesh_build_horizon.argtypes = [vp, vp]
         L.tpmc_mesh_destroy.restype = None
         L.tpmc_mesh_destroy.argtypes = [vp]
         L.tpmc_mesh_info.restype = C.c_int
@@ -186,7 +192,8 @@ class RunResult:
 class Mesh:
     """Owns a tpmc_mesh handle (triangulation + on-device LBVH)."""
 
-    def __init__(self, vertices, indices, flags=None, stream=None):
+    def __init__(self, vertices, indices, flags=None, stream=None, mesh_flags=0):
+        """mesh_flags: TPMC_MESH_* (0 = tpmc_mesh_create's behaviour; else tpmc_mesh_create_ex)."""
         L = lib()
         torch = _torch()
         self._h = C.c_void_p()
@@ -195,8 +202,7 @@ class Mesh:
             i = np.ascontiguousarray(indices, dtype=np.int32)
             f = None if flags is None else np.ascontiguousarray(flags, dtype=np.uint8)
             nv, nt = v.shape[0], i.shape[0]
-            rc = L.tpmc_mesh_create(v.ctypes.data, nv, i.ctypes.data, nt, None if f is None else f.ctypes.data,
-                                    TPMC_MEM_HOST, _stream_ptr(stream), C.byref(self._h))
+            args = (v.ctypes.data, nv, i.ctypes.data, nt, None if f is None else f.ctypes.data, TPMC_MEM_HOST)
         else:
             v = vertices.to(dtype=torch.float32).contiguous()
             i = indices.to(dtype=torch.int32).contiguous()
@@ -204,9 +210,11 @@ class Mesh:
             if not (v.is_cuda and i.is_cuda and (f is None or f.is_cuda)):
                 raise TpmcError("device meshes need CUDA tensors")
             nv, nt = v.shape[0], i.shape[0]
-            rc = L.tpmc_mesh_create(v.data_ptr(), nv, i.data_ptr(), nt, None if f is None else f.data_ptr(),
-                                    TPMC_MEM_DEVICE, _stream_ptr(stream), C.byref(self._h))
-        _check(rc, "tpmc_mesh_create")
+            args = (v.data_ptr(), nv, i.data_ptr(), nt, None if f is None else f.data_ptr(), TPMC_MEM_DEVICE)
+        if mesh_flags:
+            _check(L.tpmc_mesh_create_ex(*args, int(mesh_flags), _stream_ptr(stream), C.byref(self._h)), "tpmc_mesh_create_ex")
+        else:
+            _check(L.tpmc_mesh_create(*args, _stream_ptr(stream), C.byref(self._h)), "tpmc_mesh_create")
         self.nt = int(nt)
         self.nv = int(nv)
 
@@ -249,6 +257,10 @@ class Mesh:
             if a is not None and tuple(a.shape) != (self.nt,):
                 raise TpmcError("surface arrays must have one entry per facet")
         _check(lib().tpmc_mesh_set_surface(self._h, ptr(tw), ptr(sg), space, _stream_ptr(stream)), "tpmc_mesh_set_surface")
+
+    def build_horizon(self, stream=None):
+        """Add the escape horizons to a mesh created with TPMC_MESH_NO_HORIZON (tpmc_mesh_build_horizon)."""
+        _check(lib().tpmc_mesh_build_horizon(self._h, _stream_ptr(stream)), "tpmc_mesh_build_horizon")
 
     def copy_bvh(self):
         n_nodes = self.info()["n_nodes"]
@@ -365,6 +377,14 @@ class Mesh:
 # C-ABI names, as plain functions -------------------------------------------------------------------
 def tpmc_mesh_create(vertices, indices, flags=None, stream=None) -> Mesh:
     return Mesh(vertices, indices, flags, stream)
+
+
+def tpmc_mesh_create_ex(vertices, indices, flags=None, mesh_flags=0, stream=None) -> Mesh:
+    return Mesh(vertices, indices, flags, stream, mesh_flags)
+
+
+def tpmc_mesh_build_horizon(mesh: Mesh, **kw) -> None:
+    mesh.build_horizon(**kw)
 
 
 def tpmc_mesh_destroy(mesh: Mesh) -> None:

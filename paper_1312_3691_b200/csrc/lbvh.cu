@@ -821,8 +821,55 @@ int build_cull_volume(tpmc_mesh* m, cudaStream_t st) {
 
 }  // namespace
 
+// The escape-horizon pass on its own (tpmc_mesh_create runs it unless told not to; tpmc_mesh_build_horizon runs it later).
+static int build_horizon(tpmc_mesh* m, cudaStream_t st) {
+  if (m->horizon) return TPMC_OK;
+  uint4* hz = nullptr;
+  cudaEvent_t h0 = nullptr, h1 = nullptr;
+  TPMC_CUDA_TRY(cudaMalloc((void**)&hz, sizeof(uint4) * m->nt));
+  cudaError_t e = cudaEventCreate(&h0);
+  if (e == cudaSuccess) e = cudaEventCreate(&h1);
+  if (e == cudaSuccess) e = cudaEventRecord(h0, st);
+  if (e == cudaSuccess) {
+    k_horizon<<<(unsigned)((m->nt + 127) / 128), 128, 0, st>>>(m->nodes, m->tris, m->nt, hz);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaEventRecord(h1, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  float ms = 0.0f;
+  if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, h0, h1);
+  if (h0) cudaEventDestroy(h0);
+  if (h1) cudaEventDestroy(h1);
+  if (e != cudaSuccess) cudaFree(hz);
+  TPMC_CUDA_TRY(e);
+  m->horizon = hz;   // runs enqueued from now on use it
+  m->horizon_ms = ms;
+  return TPMC_OK;
+}
+
+extern "C" int tpmc_mesh_build_horizon(tpmc_mesh* m, void* cuda_stream) {
+  if (!m) return TPMC_EINVAL;
+  return build_horizon(m, (cudaStream_t)cuda_stream);
+}
+
+static int mesh_create_impl(const float* vertices, int64_t nv, const int32_t* indices, int64_t nt, const uint8_t* facet_flags,
+                            int mem_space, uint32_t mesh_flags, void* cuda_stream, tpmc_mesh** out);
+
 extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t* indices, int64_t nt,
                                 const uint8_t* facet_flags, int mem_space, void* cuda_stream, tpmc_mesh** out) {
+  return mesh_create_impl(vertices, nv, indices, nt, facet_flags, mem_space, 0u, cuda_stream, out);
+}
+
+extern "C" int tpmc_mesh_create_ex(const float* vertices, int64_t nv, const int32_t* indices, int64_t nt,
+                                   const uint8_t* facet_flags, int mem_space, uint32_t mesh_flags, void* cuda_stream,
+                                   tpmc_mesh** out) {
+  if (out) *out = nullptr;
+  if (mesh_flags & ~(uint32_t)TPMC_MESH_NO_HORIZON) return TPMC_EINVAL;
+  return mesh_create_impl(vertices, nv, indices, nt, facet_flags, mem_space, mesh_flags, cuda_stream, out);
+}
+
+static int mesh_create_impl(const float* vertices, int64_t nv, const int32_t* indices, int64_t nt, const uint8_t* facet_flags,
+                            int mem_space, uint32_t mesh_flags, void* cuda_stream, tpmc_mesh** out) {
   if (!out) return TPMC_EINVAL;
   *out = nullptr;
   if (!vertices || !indices || nv < 3 || nt < 1 || nt > 0x3FFFFFFF || nv > 0x7FFFFFFF) return TPMC_EINVAL;
@@ -991,20 +1038,17 @@ extern "C" int tpmc_mesh_create(const float* vertices, int64_t nv, const int32_t
   }
   MESH_TRY(cudaGetLastError());
   MESH_TRY(cudaEventRecord(e1, st));
-  // escape horizons (timed apart from the hierarchy build)
-  MESH_TRY(cudaMalloc((void**)&m->horizon, sizeof(uint4) * nt));
-  cudaEvent_t e2;
-  MESH_TRY(cudaEventCreate(&e2));
-  k_horizon<<<(unsigned)((nt + 127) / 128), 128, 0, st>>>(m->nodes, m->tris, nt, m->horizon);
-  cudaEventRecord(e2, st);
   {
     const cudaError_t es = cudaStreamSynchronize(st);
-    float ms = 0.0f, ms2 = 0.0f;
-    if (es == cudaSuccess) { cudaEventElapsedTime(&ms, e0, e1); cudaEventElapsedTime(&ms2, e1, e2); }
-    cudaEventDestroy(e2);
-    MESH_TRY(es);
+    float ms = 0.0f;
+    if (es == cudaSuccess) cudaEventElapsedTime(&ms, e0, e1);
+    MESH_TRY(es);   // (e0, e1 belong to the handle from here on: m->ev0, m->ev1)
     m->build_ms = ms;
-    m->horizon_ms = ms2;
+  }
+  // escape horizons (timed apart from the hierarchy build; skipped on request: runs then trace every re-emitted ray)
+  if (!(mesh_flags & TPMC_MESH_NO_HORIZON)) {
+    const int rch = build_horizon(m, st);
+    if (rch != TPMC_OK) { tpmc_mesh_destroy(m); return rch; }
   }
 #undef MESH_TRY
   *out = m;
@@ -1161,7 +1205,7 @@ extern "C" int tpmc_mesh_copy_wide(const tpmc_mesh* m, int64_t* n_wide, uint32_t
 }
 
 extern "C" int tpmc_mesh_copy_horizon(const tpmc_mesh* m, uint8_t* h_horizon) {
-  if (!m || !h_horizon) return TPMC_EINVAL;
+  if (!m || !h_horizon || !m->horizon) return TPMC_EINVAL;   // (no horizons: created with TPMC_MESH_NO_HORIZON)
   TPMC_CUDA_TRY(cudaMemcpy(h_horizon, m->horizon, sizeof(uint4) * m->nt, cudaMemcpyDeviceToHost));
   return TPMC_OK;
 }

@@ -1186,7 +1186,7 @@ int run_enqueue(tpmc_mesh* m, const tpmc_params* params, void* cuda_stream, doub
   const int K = g.pipes;
   const bool timed = (h_stats != nullptr);   // per-kernel events only when the caller will read them
   const bool precull = !(params->flags & TPMC_FLAG_NO_PRECULL) && params->control_volume == TPMC_CV_SPHERE;
-  const bool use_horizon = !(params->flags & TPMC_FLAG_NO_HORIZON);
+  const bool use_horizon = !(params->flags & TPMC_FLAG_NO_HORIZON) && m->horizon != nullptr;   // (mesh built without: same results)
   const bool exact = (params->flags & TPMC_FLAG_EXACT_TRACE) != 0;
   const bool sorted = !exact && (params->flags & TPMC_FLAG_SORT_RAYS);
   const int aggregate = (m->nt <= kAggregateMaxFacets && !(params->flags & TPMC_FLAG_NO_AGGREGATION)) ? 1 : 0;

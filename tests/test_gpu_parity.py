@@ -262,6 +262,35 @@ def test_mesh_create_from_device_tensors_and_errors(T):
     a.run(good, flags=T.TPMC_FLAG_SERIAL_SEED | T.TPMC_FLAG_NO_AGGREGATION)  # every defined bit is accepted
 
 
+def test_mesh_without_escape_horizons_and_late_build(T):
+    """tpmc_mesh_create_ex(TPMC_MESH_NO_HORIZON): no horizon pass at creation, runs trace every re-emitted ray and give
+    the same hit sequences; tpmc_mesh_build_horizon adds the same horizons tpmc_mesh_create would have built."""
+    import torch
+    cfg = ti.config("C4")[3].with_(N=2_000_000)
+    m = cfg.mesh()
+    ref_mesh = T.Mesh(m.vertices, m.indices, m.flags)
+    lean = T.tpmc_mesh_create_ex(m.vertices, m.indices, m.flags, mesh_flags=T.TPMC_MESH_NO_HORIZON)
+    assert lean.info()["horizon_ms"] == 0.0 and ref_mesh.info()["horizon_ms"] > 0.0
+    with pytest.raises(T.TpmcError):
+        lean.copy_horizon()
+    ref = ref_mesh.run(cfg, debug=True)
+    a = lean.run(cfg, debug=True)
+    check_conservation(a.stats, cfg.N)
+    assert a.stats["ret_horizon"] == 0 and ref.stats["ret_horizon"] > 0
+    assert a.stats["hits"] == ref.stats["hits"] and torch.equal(a.hash, ref.hash) and torch.equal(a.bounces, ref.bounces)
+    assert np.linalg.norm((a.force - ref.force).cpu().numpy()) <= 1e-12 * np.linalg.norm(ref.force.cpu().numpy())
+    lean.build_horizon()
+    lean.build_horizon()                                                     # a second call is a no-op
+    assert lean.info()["horizon_ms"] > 0.0
+    assert np.array_equal(lean.copy_horizon(), ref_mesh.copy_horizon())
+    b = lean.run(cfg, debug=True)
+    assert b.stats["ret_horizon"] == ref.stats["ret_horizon"] and torch.equal(b.hash, ref.hash)
+    with pytest.raises(T.TpmcError):
+        T.tpmc_mesh_create_ex(m.vertices, m.indices, m.flags, mesh_flags=0x80)   # unknown option bit
+    lean.close()
+    ref_mesh.close()
+
+
 # ------------------------------------------------------------------ a3: closest hit, bit-exact
 def crafted_rays(m, om, rng, n_random=400):
     V = m.vertices.astype(np.float64)
