@@ -579,6 +579,9 @@ __device__ __forceinline__ void accumulate_warp(double* __restrict__ P, bool is_
 // Rays the traversal gave up on (too many candidates, stack too deep) and rays whose reflected successor
 // finds region A of the next queue full go, untouched, to the overflow list: k_finish follows them to escape
 // with the full fp64 traversal, densely, instead of one lane doing so here while its warp waits.
+#ifndef TPMC_REFLECT_PREFETCH
+#define TPMC_REFLECT_PREFETCH 0   // 1, 2: software-prefetch variants, measured slower or equal
+#endif
 __global__ void __launch_bounds__(kTraceBlock, TPMC_REFLECT_MIN_BLOCKS) k_reflect(const RunConst rc, unsigned int cap,
                                                          const float4* __restrict__ tris, const RayQueue qin,
                                                          const unsigned int* __restrict__ hit_ray,
@@ -597,15 +600,44 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_REFLECT_MIN_BLOCKS) k_reflec
   unsigned int c[kFlushCounters] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
   const unsigned int stride = gridDim.x * blockDim.x;
   const unsigned int nround = ((n + stride - 1) / stride) * stride;   // keep warps converged for the ballots
+#if TPMC_REFLECT_PREFETCH
+  // The chain hit list -> ray record -> facet -> horizon -> accumulators is a sequence of dependent scattered loads, and
+  // the kernel is bound by their latency (ncu: 7 long-scoreboard stalls per issue, no unit above 45 %).  The list entry of
+  // the thread's NEXT hit is therefore read one iteration ahead, and the lines it points to (ray record, first candidate
+  // facet) are prefetched while the current hit is worked on.
+  unsigned int h0 = blockIdx.x * blockDim.x + threadIdx.x;
+  unsigned int r_nx = h0 < n ? __ldcs(hit_ray + h0) : kNoRay;
+#if TPMC_REFLECT_PREFETCH == 1
+  int4 c_nx = h0 < n ? __ldcs(hit_cand + h0) : make_int4(-1, -1, -1, -1);
+#endif
+#endif
   for (unsigned int h = blockIdx.x * blockDim.x + threadIdx.x; h < nround; h += stride) {
     bool spill = false, is_hit = false;
     unsigned int r = 0;
     Particle p;
     Hit hit;
     hit.facet = -1;
+#if TPMC_REFLECT_PREFETCH
+    r = h < n ? r_nx : 0u;
+#if TPMC_REFLECT_PREFETCH == 1
+    const int4 cand_cur = c_nx;
+#endif
+    {
+      const unsigned int hn = h + stride;
+      r_nx = hn < n ? __ldcs(hit_ray + hn) : kNoRay;
+#if TPMC_REFLECT_PREFETCH == 1
+      c_nx = hn < n ? __ldcs(hit_cand + hn) : make_int4(-1, -1, -1, -1);
+#endif
+    }
+#else
     if (h < n) r = __ldcs(hit_ray + h);
+#endif
     if (h < n && r != kNoRay) {
+#if TPMC_REFLECT_PREFETCH == 1
+      const int4 cand = cand_cur;
+#else
       const int4 cand = __ldcs(hit_cand + h);
+#endif
       if (cand.w == TPMC_CAND_OVERFLOW) {
         spill = true;
         ++c[FC_RETRACE];
@@ -623,6 +655,24 @@ __global__ void __launch_bounds__(kTraceBlock, TPMC_REFLECT_MIN_BLOCKS) k_reflec
         c[FC_NOHIT] += is_hit ? 0u : 1u;
       }
     }
+#if TPMC_REFLECT_PREFETCH == 2
+    if (r_nx != kNoRay) {
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(qin.o + r_nx));
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(qin.v + r_nx));
+    }
+#endif
+#if TPMC_REFLECT_PREFETCH == 1
+    if (r_nx != kNoRay) {   // (by now the next list entry has arrived)
+      asm volatile("prefetch.global.L1 [%0];" ::"l"(qin.o + r_nx));
+      asm volatile("prefetch.global.L1 [%0];" ::"l"(qin.v + r_nx));
+      asm volatile("prefetch.global.L1 [%0];" ::"l"(qin.f + r_nx));
+      if (c_nx.x >= 0) {
+        const float4* tp = tris + 3 * (size_t)c_nx.x;
+        asm volatile("prefetch.global.L1 [%0];" ::"l"(tp));
+        asm volatile("prefetch.global.L1 [%0];" ::"l"(tp + 2));
+      }
+    }
+#endif
     // surface interaction, then a queue slot for every particle that goes on (warp-aggregated).  A particle
     // that finds region A of the next queue full writes its new state back into its own slot of this queue
     // and goes to the overflow list, like one the traversal gave up on.
